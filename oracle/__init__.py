@@ -1,0 +1,147 @@
+"""TEST INFRASTRUCTURE — ctypes front end of the CPU oracle (oracle/tangram_oracle.cpp).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import
+this.  It never imports the CUDA package and the CUDA package never imports it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_DIR, "tangram_oracle.cpp")
+_SO = os.path.join(_DIR, "libtangram_oracle.so")
+MAXK = 16
+INF = 1 << 30
+INT64_MAX = (1 << 63) - 1
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        tmp = _SO + f".tmp{os.getpid()}"
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", tmp, _SRC])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+class _Res(C.Structure):
+    _fields_ = [("iter_time_us", C.c_int64), ("sum_us", C.c_int64), ("bottleneck_us", C.c_int64),
+                ("n_stages", C.c_int32), ("island_mask", C.c_uint32), ("n_dp_run", C.c_int32),
+                ("n_candidates", C.c_int32), ("stage_begin", C.c_int32 * MAXK),
+                ("stage_island", C.c_int32 * MAXK), ("stage_plan", C.c_int32 * MAXK)]
+
+
+@dataclass
+class Result:
+    iter_time_us: int
+    sum_us: int
+    bottleneck_us: int
+    n_stages: int
+    island_mask: int
+    stages: list          # [(begin, island, plan)]
+    n_dp_run: int = 0
+    n_candidates: int = 0
+    first_island: int = -1
+
+    @property
+    def feasible(self) -> bool:
+        return self.iter_time_us != INT64_MAX
+
+    def plan_key(self):
+        return (self.iter_time_us, self.sum_us, self.bottleneck_us, self.island_mask, tuple(self.stages))
+
+
+_lib = None
+_I32P = C.POINTER(C.c_int32)
+_I64P = C.POINTER(C.c_int64)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_laneless_iter.restype = C.c_int64
+    return _lib
+
+
+def _p32(a):
+    return a.ctypes.data_as(_I32P)
+
+
+def _args(inst):
+    t = np.ascontiguousarray(inst.time_us, dtype=np.int32)
+    mm = np.ascontiguousarray(inst.mem_mb, dtype=np.int32)
+    cap = np.ascontiguousarray(inst.island_cap_mb, dtype=np.int32)
+    bw = np.ascontiguousarray(inst.bw_gbps, dtype=np.int32)
+    keep = (t, mm, cap, bw)
+    return keep, (C.c_int(inst.L), C.c_int(inst.K), C.c_int(inst.P), C.c_int(inst.m), _p32(t), _p32(mm),
+                  _p32(cap), _p32(bw), C.c_int(inst.act_mb))
+
+
+def _conv(r: _Res) -> Result:
+    n = r.n_stages
+    return Result(r.iter_time_us, r.sum_us, r.bottleneck_us, n, r.island_mask,
+                  [(r.stage_begin[i], r.stage_island[i], r.stage_plan[i]) for i in range(n)],
+                  r.n_dp_run, r.n_candidates, r.stage_island[0])
+
+
+def solve(inst, full_sweep: bool = False, n_threads: int = 1) -> Result:
+    keep, a = _args(inst)
+    r = _Res()
+    lib().orc_solve(*a, C.c_int(int(full_sweep)), C.c_int(n_threads), C.byref(r))
+    return _conv(r)
+
+
+def bruteforce(inst):
+    keep, a = _args(inst)
+    r = _Res()
+    n = C.c_int64(0)
+    lib().orc_bruteforce(*a, C.byref(r), C.byref(n))
+    return _conv(r), n.value
+
+
+def dp_at(inst, T: int, want_plan: bool = True) -> Result:
+    """DP at one threshold (T < 0: infinity).  sum_us = f_T; infeasible -> feasible == False."""
+    keep, a = _args(inst)
+    r = _Res()
+    lib().orc_dp_at(*a, C.c_int64(T), C.c_int(int(want_plan)), C.byref(r))
+    return _conv(r)
+
+
+def laneless_iter(inst, xc: int) -> int:
+    keep, a = _args(inst)
+    return lib().orc_laneless_iter(*a[:7], C.c_int64(xc))
+
+
+def reduce(inst):
+    """-> c [NS,K] int64 (2^30 none), argp [NS,K] int32, x [K,K] int64, candidates int64[]"""
+    keep, a = _args(inst)
+    NS = inst.L * (inst.L + 1) // 2
+    c = np.empty((NS, inst.K), dtype=np.int64)
+    argp = np.empty((NS, inst.K), dtype=np.int32)
+    x = np.empty((inst.K, inst.K), dtype=np.int64)
+    cand = np.empty(NS * inst.K, dtype=np.int64)
+    n = lib().orc_reduce(a[0], a[1], a[2], a[4], a[5], a[6], a[7], a[8], c.ctypes.data_as(_I64P),
+                         _p32(argp), x.ctypes.data_as(_I64P), cand.ctypes.data_as(_I64P))
+    return c, argp, x, cand[:n].copy()
+
+
+def prune(inst, mode: int = 0, threshold: int = 0):
+    """Returns (pruned copy of inst, counts[4]).  inst itself is not modified."""
+    out = inst.copy()
+    t = np.ascontiguousarray(out.time_us, dtype=np.int32)
+    mm = np.ascontiguousarray(out.mem_mb, dtype=np.int32)
+    cap = np.ascontiguousarray(out.island_cap_mb, dtype=np.int32)
+    counts = np.zeros(4, dtype=np.int64)
+    lib().orc_prune(C.c_int(out.L), C.c_int(out.K), C.c_int(out.P), _p32(t), _p32(mm), _p32(cap),
+                    C.c_int(mode), C.c_int64(threshold), counts.ctypes.data_as(_I64P))
+    out.time_us = t
+    return out, counts
+
+
+def hw_threads() -> int:
+    return lib().orc_hw_threads()
