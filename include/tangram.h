@@ -1,0 +1,153 @@
+/* libtangram — C ABI of the B200-native TANGRAM pipeline-composition search.
+ *
+ * What is computed: the composition step of TANGRAM §5.2 restated as an exact
+ * integer bitmask dynamic program (BASELINE.json:north_star).  For one planning
+ * instance with L layers (atoms), K GPU islands, P intra-slice plans and m microbatches:
+ *
+ *   slice  [a,b), 0 <= a < b <= L, index s(a,b) = a*(2L-a+1)/2 + (b-a-1), NS = L(L+1)/2
+ *   c[a][b][k] = min_p { time_us[s][k][p] : time != TG_INVALID, mem_mb[s][k][p] <= cap_mb[k] }
+ *                (PAPER.md:240 plans carry time and memory; :236 memory infeasibility)
+ *   x[j][k]    = ceil(act_mb*1000 / bw_gbps[j][k]) microseconds, j = upstream stage's island
+ *                (PAPER.md:240 only pipeline activations cross islands; :160 asymmetric links)
+ *   plan       = stages (a_i,b_i,k_i) tiling [0,L) with pairwise distinct islands
+ *   sum        = sum_i c[a_i][b_i][k_i] + sum_i x[k_i][k_{i+1}]
+ *   T          = max_i c[a_i][b_i][k_i]          (PAPER.md:250 (1): slowest stage is the bottleneck)
+ *   iter       = sum + (m-1)*T                   (1F1B; formula from north_star)
+ *   result     = argmin of (iter, T, mask, k_0, b_0, k_1, b_1, ...)   -- exactly one plan is correct
+ *
+ * All pointers in the signatures are plain C pointers; each argument says HOST, DEVICE or EITHER.
+ * "EITHER" pointers are classified with cudaPointerGetAttributes.  No call throws; every call
+ * returns a tg_status and leaves its outputs untouched on error.  tg_last_error() gives a
+ * thread-local message.  There is no CPU fallback: without a CUDA device every compute call
+ * returns TG_ERR_CUDA.
+ */
+#ifndef TANGRAM_H_
+#define TANGRAM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tg_instance tg_instance; /* opaque; owns DEVICE copies of every table passed in */
+
+typedef enum {
+    TG_OK = 0,
+    TG_ERR_NULL = 1,   /* a required pointer is NULL                       */
+    TG_ERR_SHAPE = 2,  /* L, K, P, m or n outside the limits below         */
+    TG_ERR_RANGE = 3,  /* a table value outside its documented range       */
+    TG_ERR_OOM = 4,    /* device or host allocation failed                 */
+    TG_ERR_CUDA = 5    /* any other CUDA failure, or no device             */
+} tg_status;
+
+enum {
+    TG_MAX_K = 16,
+    TG_MAX_L = 255,
+    TG_MAX_P = 255,
+    TG_MAX_M = 1 << 20,
+    TG_TIME_MAX = 1 << 25,
+    TG_INVALID = 0x7fffffff, /* "no such intra-slice plan" marker in time_us */
+    TG_INF = 1 << 30         /* saturating "no plan" value of the DP        */
+};
+
+/* tg_instance_create — SURVEY.md §8(b); north_star "tg_instance_create(cost/memory tables per
+ * slice x island x intra-plan, island GPU counts and capacities, bandwidth matrix, m)".
+ *   time_us      EITHER [NS][K][P] int32, p fastest; each entry in [0,TG_TIME_MAX] or TG_INVALID
+ *   mem_mb       EITHER [NS][K][P] int32, per-GPU MB needed by that plan, >= 0
+ *   island_gpus  EITHER [K] >= 1 (validated and kept; not used by the recurrence)
+ *   island_cap_mb EITHER [K] per-GPU capacity in MB, >= 0
+ *   bw_gbps      EITHER [K][K] sender-major, > 0 off the diagonal, diagonal ignored
+ *   act_mb       activation MB crossing every stage boundary, >= 0
+ * All inputs are copied to device memory owned by the instance; the caller keeps its buffers.
+ * Range validation of the tables runs on the device.  Errors: NULL -> TG_ERR_NULL; limits
+ * 1<=L<=TG_MAX_L, 1<=K<=TG_MAX_K, 1<=P<=TG_MAX_P, 1<=m<=TG_MAX_M -> TG_ERR_SHAPE; bad values ->
+ * TG_ERR_RANGE.  Synchronises the device's legacy default stream once. */
+tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const int32_t* time_us,
+                             const int32_t* mem_mb, const int32_t* island_gpus,
+                             const int32_t* island_cap_mb, const int32_t* bw_gbps, int32_t act_mb,
+                             tg_instance** out);
+
+/* NULL is a no-op.  The instance must not be in use by an unsynchronised tg_solve_batch. */
+tg_status tg_instance_destroy(tg_instance* inst);
+
+typedef struct { /* one per instance, POD, 8-byte aligned, 224 bytes */
+    int64_t iter_time_us;      /* sum + (m-1)*T* ; INT64_MAX if no feasible plan               */
+    int64_t sum_us;            /* sum of stage times + transfers of the returned plan          */
+    int32_t bottleneck_us;     /* T*                                                           */
+    int32_t n_stages;          /* 0 if infeasible                                              */
+    uint32_t island_mask;      /* S*                                                           */
+    uint32_t n_thresholds_run; /* diagnostics: DPs executed for this instance                  */
+    int32_t stage_begin[TG_MAX_K]; /* stage i covers [stage_begin[i], stage_begin[i+1]), last ends at L */
+    int32_t stage_island[TG_MAX_K];
+    int32_t stage_plan[TG_MAX_K];  /* lowest p attaining c for that (slice, island)            */
+} tg_result;
+
+enum { /* flags of tg_solve_batch_ex */
+    TG_SOLVE_DEFAULT = 0,   /* windowed sweep: lowest feasible T by search, exact stop rule */
+    TG_SOLVE_FULL_SWEEP = 1 /* run the DP at every candidate T (rate benchmark; same result)           */
+};
+
+typedef struct { /* optional diagnostics of one tg_solve_batch_ex call, written on the device  */
+    uint64_t n_dp;           /* DPs executed (all instances)                                   */
+    uint64_t plans_dense;    /* sum over DPs of NS*K*2^(K-1): SURVEY.md §8(d) "plans evaluated" */
+    uint64_t states_live;    /* sum over DPs of L*Ke*2^(Ke-1), Ke = islands alive at that T     */
+    uint64_t n_rounds;       /* scheduler rounds                                               */
+    uint64_t n_barriers;     /* grid-wide barriers executed                                    */
+    uint64_t n_items_global_c; /* DPs whose cost tables did not fit in shared memory           */
+    uint64_t reserved[2];
+} tg_solve_stats;
+
+/* tg_solve_batch — north_star "tg_solve_batch(instances, stream) -> best iteration time and plan".
+ * Steps: cost-table loader, transfer table, candidate thresholds, DP at T=inf,
+ * per-T popcount-wavefront DP, threshold-sweep reduction, plan back-tracker.
+ *   instances   HOST array of n instance handles (all created on the current device)
+ *   out         EITHER: n results.  DEVICE: written asynchronously on `cuda_stream`, valid after the
+ *               stream is synchronised.  HOST: the call copies the results back and synchronises.
+ *   cuda_stream a cudaStream_t (NULL = legacy default stream)
+ * Never mutates the instances.  An infeasible instance is not an error (iter_time_us = INT64_MAX,
+ * n_stages = 0).  n == 0 is a no-op.  Scratch memory is taken from the stream-ordered pool. */
+tg_status tg_solve_batch(tg_instance* const* instances, int32_t n, tg_result* out, void* cuda_stream);
+
+/* Same, with flags and optional statistics (stats: EITHER or NULL; HOST forces a synchronise). */
+tg_status tg_solve_batch_ex(tg_instance* const* instances, int32_t n, tg_result* out, uint32_t flags,
+                            tg_solve_stats* stats, void* cuda_stream);
+
+typedef enum {
+    TG_PRUNE_EXACT = 0,     /* R1 infeasible + R2 dominated; threshold ignored                  */
+    TG_PRUNE_IMBALANCE = 1, /* + R3, threshold = theta in permille, 1000..16384                 */
+    TG_PRUNE_BOTTLENECK = 2 /* + R4, threshold = stage-time cap in microseconds                 */
+} tg_prune_mode;
+
+/* tg_prune — north_star "tg_prune(threshold) for the dominated-plan pruning"
+ * (pruning policies), :43/:360 (incompatible partial plans); rules R1-R4 of SURVEY.md §8(c).
+ * Marks entries of the instance's time table dead (TG_INVALID), in place, idempotent, monotone.
+ *   counts_out  HOST int64[4]: entries newly killed by R1..R4.  The call synchronises `cuda_stream`. */
+tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4],
+                   void* cuda_stream);
+
+/* ---- step-level entry points (used by the parity tests to check single steps) ---------------- */
+
+/* Steps 1-3 alone: reduced tables and candidate thresholds.  All outputs HOST, any may be NULL.
+ *   c_out    [NS][K] int32, TG_INF where no feasible plan      argp_out [NS][K] int32, -1 if none
+ *   x_out    [K][K] int32 (0 on the diagonal, TG_INF if > TG_TIME_MAX)
+ *   cand_out capacity NS*K int32, ascending distinct finite c; *n_cand_out receives the count.
+ * Synchronises `cuda_stream`. */
+tg_status tg_reduce(tg_instance* inst, int32_t* c_out, int32_t* argp_out, int32_t* x_out,
+                    int32_t* cand_out, int32_t* n_cand_out, void* cuda_stream);
+
+/* Step 5 + 7 at ONE threshold: DP at T (T < 0 means infinity), top reduction and back-track.
+ * out (EITHER): iter_time_us = f_T + (m-1)*T with T = 2^30 for infinity, bottleneck_us = that T,
+ * INT64_MAX if no plan is admissible at T. */
+tg_status tg_dp_at(tg_instance* inst, int64_t T, tg_result* out, void* cuda_stream);
+
+/* Copies the instance's current time table (after pruning) to HOST time_out [NS][K][P]. */
+tg_status tg_instance_read_time(tg_instance* inst, int32_t* time_out);
+
+const char* tg_last_error(void); /* thread-local, valid until the next tg_* call on the thread */
+int32_t tg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TANGRAM_H_ */

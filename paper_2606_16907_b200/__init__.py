@@ -1,0 +1,232 @@
+"""Thin Python binding of libtangram (include/tangram.h): argument marshalling only.
+
+Every step of the path — cost-table loader, candidate thresholds, per-T wavefront DP, sweep
+reduction, back-tracker, pruning — runs in the CUDA kernels of `csrc/`.  There is no CPU fallback:
+if the shared library is missing or no CUDA device is present the calls raise.
+
+Names follow the C ABI: tg_instance_create, tg_instance_destroy, tg_solve_batch, tg_solve_batch_ex,
+tg_prune, tg_reduce, tg_dp_at, tg_instance_read_time, tg_last_error, tg_version.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_DIR, "libtangram.so")
+
+TG_MAX_K = 16
+TG_INVALID = 0x7FFFFFFF
+TG_INF = 1 << 30
+INT64_MAX = (1 << 63) - 1
+TG_SOLVE_DEFAULT, TG_SOLVE_FULL_SWEEP = 0, 1
+TG_PRUNE_EXACT, TG_PRUNE_IMBALANCE, TG_PRUNE_BOTTLENECK = 0, 1, 2
+STATUS = {0: "TG_OK", 1: "TG_ERR_NULL", 2: "TG_ERR_SHAPE", 3: "TG_ERR_RANGE", 4: "TG_ERR_OOM", 5: "TG_ERR_CUDA"}
+
+
+class TgResult(C.Structure):
+    _fields_ = [("iter_time_us", C.c_int64), ("sum_us", C.c_int64), ("bottleneck_us", C.c_int32),
+                ("n_stages", C.c_int32), ("island_mask", C.c_uint32), ("n_thresholds_run", C.c_uint32),
+                ("stage_begin", C.c_int32 * TG_MAX_K), ("stage_island", C.c_int32 * TG_MAX_K),
+                ("stage_plan", C.c_int32 * TG_MAX_K)]
+
+    @property
+    def feasible(self) -> bool:
+        return self.iter_time_us != INT64_MAX
+
+    @property
+    def stages(self):
+        return [(self.stage_begin[i], self.stage_island[i], self.stage_plan[i]) for i in range(self.n_stages)]
+
+
+class TgSolveStats(C.Structure):
+    _fields_ = [("n_dp", C.c_uint64), ("plans_dense", C.c_uint64), ("states_live", C.c_uint64),
+                ("n_rounds", C.c_uint64), ("n_barriers", C.c_uint64), ("n_items_global_c", C.c_uint64),
+                ("reserved", C.c_uint64 * 2)]
+
+
+RESULT_BYTES = C.sizeof(TgResult)
+RESULT_DTYPE = np.dtype([("iter_time_us", "<i8"), ("sum_us", "<i8"), ("bottleneck_us", "<i4"), ("n_stages", "<i4"),
+                         ("island_mask", "<u4"), ("n_thresholds_run", "<u4"), ("stage_begin", "<i4", (TG_MAX_K,)),
+                         ("stage_island", "<i4", (TG_MAX_K,)), ("stage_plan", "<i4", (TG_MAX_K,))])
+assert RESULT_DTYPE.itemsize == RESULT_BYTES == 224
+
+
+class TangramError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{STATUS.get(status, status)}: {msg}")
+        self.status = status
+
+
+_lib = None
+EXPORTS = ["tg_instance_create", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
+           "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_error", "tg_version"]
+
+
+def lib():
+    """Loads libtangram.so; raises if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_16907_b200.build`")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, u32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32
+        L.tg_instance_create.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, i32, C.POINTER(vp)]
+        L.tg_instance_destroy.argtypes = [vp]
+        L.tg_solve_batch.argtypes = [C.POINTER(vp), i32, vp, vp]
+        L.tg_solve_batch_ex.argtypes = [C.POINTER(vp), i32, vp, u32, vp, vp]
+        L.tg_prune.argtypes = [vp, C.c_int, i64, C.POINTER(i64), vp]
+        L.tg_reduce.argtypes = [vp, vp, vp, vp, vp, C.POINTER(i32), vp]
+        L.tg_dp_at.argtypes = [vp, i64, vp, vp]
+        L.tg_instance_read_time.argtypes = [vp, vp]
+        L.tg_last_error.restype = C.c_char_p
+        L.tg_version.restype = i32
+        for name in EXPORTS:
+            if name not in ("tg_last_error", "tg_version"):
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def tg_last_error() -> str:
+    return lib().tg_last_error().decode()
+
+
+def tg_version() -> int:
+    return lib().tg_version()
+
+
+def _check(st: int):
+    if st != 0:
+        raise TangramError(st, tg_last_error())
+
+
+def _ptr(a):
+    """Address of a numpy array (host) or torch tensor (host or device); None -> NULL."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    if isinstance(a, int):
+        return a
+    assert a.is_contiguous()
+    return a.data_ptr()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+class Instance:
+    """Owner of one tg_instance handle."""
+
+    def __init__(self, handle: int, L: int, K: int, P: int, m: int):
+        self.handle, self.L, self.K, self.P, self.m = handle, L, K, P, m
+        self.NS = L * (L + 1) // 2
+
+    def destroy(self):
+        if self.handle:
+            lib().tg_instance_destroy(self.handle)
+            self.handle = 0
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def tg_instance_create(L, K, P, m, time_us, mem_mb, island_gpus, island_cap_mb, bw_gbps, act_mb) -> Instance:
+    """Tables: int32 numpy arrays (host) or int32 torch tensors (host or device), C-contiguous."""
+    def prep(a):
+        if isinstance(a, np.ndarray):
+            return np.ascontiguousarray(a, dtype=np.int32)
+        return a
+    arrs = [prep(a) for a in (time_us, mem_mb, island_gpus, island_cap_mb, bw_gbps)]
+    h = C.c_void_p(0)
+    _check(lib().tg_instance_create(L, K, P, m, *[_ptr(a) for a in arrs], act_mb, C.byref(h)))
+    return Instance(h.value, L, K, P, m)
+
+
+def tg_instance_destroy(inst: Instance):
+    inst.destroy()
+
+
+def _handles(instances):
+    arr = (C.c_void_p * len(instances))(*[i.handle for i in instances])
+    return arr
+
+
+def tg_solve_batch(instances, out=None, stream=None, flags: int = TG_SOLVE_DEFAULT, stats=None):
+    """Solves the batch.  `out`: a uint8 CUDA tensor of len(instances)*224 bytes (asynchronous on
+    `stream`), or None for a host result array (synchronous).  Returns `out`, or a numpy structured
+    array of RESULT_DTYPE when out is None.  `stats`: optional TgSolveStats (host) filled on return."""
+    n = len(instances)
+    h = _handles(instances)
+    sp = _stream_ptr(stream)
+    host = None
+    if out is None:
+        host = np.zeros(n, dtype=RESULT_DTYPE)
+        optr = host.ctypes.data
+    else:
+        optr = _ptr(out)
+    sptr = C.addressof(stats) if stats is not None else None
+    _check(lib().tg_solve_batch_ex(h, n, optr, flags, sptr, sp))
+    return host if out is None else out
+
+
+def tg_solve_batch_ex(instances, out, flags, stats, stream=None):
+    return tg_solve_batch(instances, out, stream, flags, stats)
+
+
+def tg_dp_at(inst: Instance, T: int, stream=None) -> TgResult:
+    r = TgResult()
+    _check(lib().tg_dp_at(inst.handle, T, C.addressof(r), _stream_ptr(stream)))
+    return r
+
+
+def tg_reduce(inst: Instance, stream=None):
+    """-> c [NS,K] int32 (2^30 none), argp [NS,K] int32 (-1 none), x [K,K] int32, candidates int32[]"""
+    c = np.empty((inst.NS, inst.K), dtype=np.int32)
+    argp = np.empty((inst.NS, inst.K), dtype=np.int32)
+    x = np.empty((inst.K, inst.K), dtype=np.int32)
+    cand = np.empty(inst.NS * inst.K, dtype=np.int32)
+    n = C.c_int32(0)
+    _check(lib().tg_reduce(inst.handle, c.ctypes.data, argp.ctypes.data, x.ctypes.data, cand.ctypes.data,
+                           C.byref(n), _stream_ptr(stream)))
+    return c, argp, x, cand[:n.value].copy()
+
+
+def tg_prune(inst: Instance, mode: int = TG_PRUNE_EXACT, threshold: int = 0, stream=None) -> np.ndarray:
+    counts = (C.c_int64 * 4)()
+    _check(lib().tg_prune(inst.handle, mode, threshold, counts, _stream_ptr(stream)))
+    return np.array(list(counts), dtype=np.int64)
+
+
+def tg_instance_read_time(inst: Instance) -> np.ndarray:
+    t = np.empty((inst.NS, inst.K, inst.P), dtype=np.int32)
+    _check(lib().tg_instance_read_time(inst.handle, t.ctypes.data))
+    return t
+
+
+def results_from_tensor(out, n: int) -> np.ndarray:
+    """Device result tensor -> numpy structured array (synchronises)."""
+    return np.frombuffer(out.cpu().numpy().tobytes(), dtype=RESULT_DTYPE, count=n)
+
+
+def instance_from_inputs(inst, device_tables: bool = False) -> Instance:
+    """Convenience: build from a tg_inputs.Instance-like object (fields L,K,P,m,time_us,...)."""
+    if device_tables:
+        import torch
+        t = torch.from_numpy(np.ascontiguousarray(inst.time_us, dtype=np.int32)).cuda()
+        mm = torch.from_numpy(np.ascontiguousarray(inst.mem_mb, dtype=np.int32)).cuda()
+        return tg_instance_create(inst.L, inst.K, inst.P, inst.m, t, mm, inst.island_gpus, inst.island_cap_mb,
+                                  inst.bw_gbps, inst.act_mb)
+    return tg_instance_create(inst.L, inst.K, inst.P, inst.m, inst.time_us, inst.mem_mb, inst.island_gpus,
+                              inst.island_cap_mb, inst.bw_gbps, inst.act_mb)

@@ -1,0 +1,425 @@
+// libtangram host side: C-ABI entry points (include/tangram.h), instance ownership, workspace
+// carving and kernel launches.  No CPU fallback: every compute path ends in a CUDA launch.
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "tg_common.cuh"
+#include "tg_prep.cuh"
+#include "tg_solve.cuh"
+
+struct tg_instance {
+    int32_t L, K, P, m, act_mb, NS;
+    int device;
+    int32_t *time_us, *mem_mb, *gpus, *cap_mb, *bw;  // device
+};
+
+namespace {
+
+thread_local std::string g_err;
+
+tg_status fail(tg_status st, const std::string& msg) {
+    g_err = msg;
+    return st;
+}
+
+#define TG_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? TG_ERR_OOM : TG_ERR_CUDA,                \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                       \
+    } while (0)
+
+struct DeviceState {
+    bool ready = false;
+    int numSMs = 0;
+    int smemOptin = 0;
+    uint16_t* maskOf = nullptr;
+    uint16_t* rankOf = nullptr;
+};
+std::mutex g_mu;
+DeviceState g_dev[64];
+
+tg_status deviceInit(int dev, DeviceState** out) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (dev < 0 || dev >= 64) return fail(TG_ERR_CUDA, "device ordinal out of range");
+    DeviceState& D = g_dev[dev];
+    if (!D.ready) {
+        cudaDeviceProp prop;
+        TG_CUDA(cudaGetDeviceProperties(&prop, dev));
+        D.numSMs = prop.multiProcessorCount;
+        D.smemOptin = int(prop.sharedMemPerBlockOptin);
+        int coop = 0;
+        TG_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+        if (!coop) return fail(TG_ERR_CUDA, "device lacks cooperative launch");
+        // masks ordered by (popcount, value) == colexicographic rank inside each popcount class
+        std::vector<uint16_t> maskOf(65536), rankOf(65536);
+        uint16_t binom[17][17];
+        memset(binom, 0, sizeof(binom));
+        for (int n = 0; n <= 16; ++n) {
+            binom[n][0] = 1;
+            for (int r = 1; r <= n; ++r) binom[n][r] = uint16_t(binom[n - 1][r - 1] + (r <= n - 1 ? binom[n - 1][r] : 0));
+        }
+        uint32_t popOff[18];
+        popOff[0] = 0;
+        for (int r = 0; r <= 16; ++r) popOff[r + 1] = popOff[r] + binom[16][r];
+        uint32_t fill[17];
+        memset(fill, 0, sizeof(fill));
+        for (uint32_t mk = 0; mk < 65536; ++mk) {
+            const int r = __builtin_popcount(mk);
+            maskOf[popOff[r] + fill[r]] = uint16_t(mk);
+            rankOf[mk] = uint16_t(fill[r]);
+            ++fill[r];
+        }
+        TG_CUDA(cudaMalloc(&D.maskOf, 65536 * sizeof(uint16_t)));
+        TG_CUDA(cudaMalloc(&D.rankOf, 65536 * sizeof(uint16_t)));
+        TG_CUDA(cudaMemcpy(D.maskOf, maskOf.data(), 65536 * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        TG_CUDA(cudaMemcpy(D.rankOf, rankOf.data(), 65536 * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        TG_CUDA(cudaMemcpyToSymbol(tgBinom, binom, sizeof(binom)));
+        TG_CUDA(cudaMemcpyToSymbol(tgPopOff, popOff, sizeof(popOff)));
+        TG_CUDA(cudaFuncSetAttribute(tgPrepareKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TG_SORT_SMEM_MAX * 4));
+        cudaFuncAttributes fa;
+        TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
+        const int dyn = D.smemOptin - int(fa.sharedSizeBytes) - 1024;
+        if (dyn < 96 * 1024) return fail(TG_ERR_CUDA, "not enough shared memory per block for the solver");
+        TG_CUDA(cudaFuncSetAttribute(tgSolveKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+        // keep stream-ordered scratch cached between calls
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            uint64_t thr = UINT64_MAX;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+        D.ready = true;
+    }
+    *out = &D;
+    return TG_OK;
+}
+
+inline size_t alignUp(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Carver {
+    size_t off = 0;
+    size_t take(size_t bytes, size_t align = 256) {
+        off = alignUp(off, align);
+        const size_t o = off;
+        off += bytes;
+        return o;
+    }
+};
+
+bool isDevicePtr(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+struct Workspace {
+    char* base = nullptr;
+    size_t bytes = 0;
+    TgInstDev* inst = nullptr;
+    TgSolveCtx ctx;
+    tg_result* outDev = nullptr;
+    int dynSmem = 0;
+    int numSMs = 0;
+};
+
+// Lays out the per-call workspace, uploads the instance records and runs loader + prepare.
+tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStream_t st, Workspace& W) {
+    if (!instances) return fail(TG_ERR_NULL, "instances is NULL");
+    if (n < 1 || n > 65535) return fail(TG_ERR_SHAPE, "n must be in [1, 65535]");
+    for (int i = 0; i < n; ++i)
+        if (!instances[i]) return fail(TG_ERR_NULL, "instances[" + std::to_string(i) + "] is NULL");
+    int dev = 0;
+    TG_CUDA(cudaGetDevice(&dev));
+    for (int i = 0; i < n; ++i)
+        if (instances[i]->device != dev) return fail(TG_ERR_CUDA, "instance was created on another device");
+    DeviceState* D;
+    tg_status s = deviceInit(dev, &D);
+    if (s != TG_OK) return s;
+
+    Carver cv;
+    const size_t oInst = cv.take(sizeof(TgInstDev) * n);
+    std::vector<TgInstDev> h(n);
+    std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSuf(n);
+    int maxCells = 0, maxLp = 4;
+    uint64_t hardMin = 0, sumFull = 0;
+    size_t denseCs = 0;
+    for (int i = 0; i < n; ++i) {
+        const tg_instance& t = *instances[i];
+        TgInstDev& I = h[i];
+        memset(&I, 0, sizeof(I));
+        I.time_us = t.time_us; I.mem_mb = t.mem_mb; I.cap_mb = t.cap_mb; I.bw_gbps = t.bw;
+        I.L = t.L; I.K = t.K; I.P = t.P; I.m = t.m; I.act_mb = t.act_mb; I.NS = t.NS;
+        I.Lp = (t.L + 3) & ~3;
+        I.triG = int(tgGOff(t.L, t.L + 1));
+        const int cells = t.NS * t.K;
+        int cap = 2;
+        while (cap < cells) cap <<= 1;
+        I.sortCap = cap;
+        for (int k = 0; k < TG_MAX_K; ++k) I.cminAll[k] = TG_INFU;
+        I.phase = TG_PH_NEW;
+        uint64_t mx = 1;
+        {   // widest wavefront and full table in rows
+            uint64_t binom[17][17];
+            memset(binom, 0, sizeof(binom));
+            for (int a = 0; a <= 16; ++a) { binom[a][0] = 1; for (int r = 1; r <= a; ++r) binom[a][r] = binom[a - 1][r - 1] + binom[a - 1][r]; }
+            for (int r = 0; r < t.K; ++r) mx = std::max<uint64_t>(mx, binom[t.K][r] * uint64_t(t.K - r));
+        }
+        const uint64_t full = uint64_t(t.K) * (1ull << (t.K - 1)) * uint64_t(I.Lp);
+        I.fullWords = full;
+        hardMin = std::max<uint64_t>(hardMin, std::max<uint64_t>(full, 2 * mx * uint64_t(I.Lp)));
+        sumFull += full;
+        denseCs = std::max<size_t>(denseCs, size_t(t.K) * tgSOff(t.L, t.L));
+        maxCells = std::max(maxCells, cells);
+        maxLp = std::max(maxLp, int(I.Lp));
+        oCd[i] = cv.take(size_t(t.K) * I.triG * 4);
+        oArgp[i] = cv.take(size_t(cells));
+        oCand[i] = cv.take(size_t(cells) * 4);
+        oSort[i] = cv.take(size_t(cap) * 4);
+        oSuf[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
+    }
+    const size_t oItems = cv.take(sizeof(TgItem) * 2 * TG_MAX_ITEMS);
+    const size_t oKeys = cv.take(sizeof(unsigned long long) * 2 * TG_MAX_ITEMS);
+    const size_t oPre = cv.take(sizeof(uint32_t) * 2 * (TG_MAX_K + 1) * (TG_MAX_ITEMS + 1));
+    const size_t oCtrl = cv.take(sizeof(TgCtrl));
+    const size_t oOut = cv.take(sizeof(tg_result) * n);
+    const uint64_t softWords = 24ull << 20;  // 96 MB: two wavefronts of a round stay inside the 126 MB L2
+    uint64_t scratchWords = 0;
+    if (needSolve) {
+        scratchWords = std::max<uint64_t>(hardMin + 2048, std::min<uint64_t>(std::max<uint64_t>(sumFull, softWords), 256ull << 20));
+        scratchWords += uint64_t(std::min(n * 32, TG_MAX_ITEMS)) * 1024;  // per-item 4 KB rounding
+        scratchWords = alignUp(scratchWords, 1024);
+    }
+    const size_t oScratch = cv.take(size_t(scratchWords) * 4, 4096);
+    W.bytes = cv.off + 4096;
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&W.base), W.bytes, st));
+    for (int i = 0; i < n; ++i) {
+        h[i].cd = reinterpret_cast<uint32_t*>(W.base + oCd[i]);
+        h[i].argp = reinterpret_cast<uint8_t*>(W.base + oArgp[i]);
+        h[i].cand = reinterpret_cast<uint32_t*>(W.base + oCand[i]);
+        h[i].sortbuf = reinterpret_cast<uint32_t*>(W.base + oSort[i]);
+        h[i].sufMin = reinterpret_cast<uint32_t*>(W.base + oSuf[i]);
+    }
+    W.inst = reinterpret_cast<TgInstDev*>(W.base + oInst);
+    W.outDev = reinterpret_cast<tg_result*>(W.base + oOut);
+    W.numSMs = D->numSMs;
+    TG_CUDA(cudaMemcpyAsync(W.inst, h.data(), sizeof(TgInstDev) * n, cudaMemcpyHostToDevice, st));
+    TG_CUDA(cudaMemsetAsync(W.base + oCtrl, 0, sizeof(TgCtrl), st));
+
+    // shared-memory split of the solver: H tile rows vs staged cost tables
+    cudaFuncAttributes fa;
+    TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
+    W.dynSmem = (D->smemOptin - int(fa.sharedSizeBytes) - 1024) & ~15;
+    const int totalWords = W.dynSmem / 4;
+    int rows = 256;
+    while (rows > 64 && totalWords - (rows + 1) * (maxLp + 8) < int(std::min<size_t>(denseCs, size_t(totalWords)))) rows -= 32;
+    TgSolveCtx& c = W.ctx;
+    memset(&c, 0, sizeof(c));
+    c.hsWords = (rows + 1) * (maxLp + 8);
+    c.csWords = (totalWords - c.hsWords) & ~3;
+    if (c.csWords < 0) return fail(TG_ERR_SHAPE, "shared memory too small for this instance shape");
+    c.inst = W.inst; c.nInst = n;
+    c.items = reinterpret_cast<TgItem*>(W.base + oItems);
+    c.keys = reinterpret_cast<unsigned long long*>(W.base + oKeys);
+    c.tilePrefix = reinterpret_cast<uint32_t*>(W.base + oPre);
+    c.scratch = reinterpret_cast<uint32_t*>(W.base + oScratch);
+    c.scratchWords = scratchWords; c.softWords = softWords;
+    c.ctrl = reinterpret_cast<TgCtrl*>(W.base + oCtrl);
+    c.maskOf = D->maskOf; c.rankOf = D->rankOf;
+
+    const dim3 g((maxCells + 255) / 256, n);
+    tgLoadKernel<<<g, 256, 0, st>>>(W.inst);
+    tgPrepareKernel<<<n, TG_PREP_NT, TG_SORT_SMEM_MAX * 4, st>>>(W.inst);
+    TG_CUDA(cudaGetLastError());
+    return TG_OK;
+}
+
+tg_status launchSolve(Workspace& W, cudaStream_t st) {
+    TgSolveCtx ctx = W.ctx;
+    void* args[] = {&ctx};
+    TG_CUDA(cudaLaunchCooperativeKernel((const void*)tgSolveKernel, dim3(W.numSMs), dim3(TG_NT), args, size_t(W.dynSmem), st));
+    return TG_OK;
+}
+
+tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cudaStream_t st) {
+    const bool outDev = isDevicePtr(out);
+    bool sync = !outDev;
+    TG_CUDA(cudaMemcpyAsync(out, W.outDev, sizeof(tg_result) * n, cudaMemcpyDefault, st));
+    if (stats) {
+        if (!isDevicePtr(stats)) sync = true;
+        // the error flag rides in reserved[0]
+        TG_CUDA(cudaMemcpyAsync(&W.ctx.ctrl->stats.reserved[0], &W.ctx.ctrl->errFlag, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        TG_CUDA(cudaMemcpyAsync(stats, &W.ctx.ctrl->stats, sizeof(tg_solve_stats), cudaMemcpyDefault, st));
+    }
+    int32_t err = 0;
+    if (sync) TG_CUDA(cudaMemcpyAsync(&err, &W.ctx.ctrl->errFlag, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    TG_CUDA(cudaFreeAsync(W.base, st));
+    W.base = nullptr;
+    if (sync) {
+        TG_CUDA(cudaStreamSynchronize(st));
+        if (err) return fail(TG_ERR_CUDA, "solver reported internal error " + std::to_string(err));
+    }
+    return TG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tg_last_error(void) { return g_err.c_str(); }
+int32_t tg_version(void) { return 100; }
+
+tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const int32_t* time_us,
+                             const int32_t* mem_mb, const int32_t* island_gpus, const int32_t* island_cap_mb,
+                             const int32_t* bw_gbps, int32_t act_mb, tg_instance** out) {
+    if (!time_us || !mem_mb || !island_gpus || !island_cap_mb || !bw_gbps || !out) return fail(TG_ERR_NULL, "NULL argument");
+    if (L < 1 || L > TG_MAX_L || K < 1 || K > TG_MAX_K || P < 1 || P > TG_MAX_P || m < 1 || m > TG_MAX_M)
+        return fail(TG_ERR_SHAPE, "L, K, P or m outside limits");
+    if (act_mb < 0 || act_mb > (1 << 20)) return fail(TG_ERR_RANGE, "act_mb outside [0, 2^20]");
+    int dev = 0;
+    TG_CUDA(cudaGetDevice(&dev));
+    DeviceState* D;
+    tg_status s = deviceInit(dev, &D);
+    if (s != TG_OK) return s;
+    const int NS = L * (L + 1) / 2;
+    const size_t nE = size_t(NS) * K * P;
+    char* base = nullptr;
+    Carver cv;
+    const size_t oT = cv.take(nE * 4), oM = cv.take(nE * 4), oG = cv.take(K * 4), oC = cv.take(K * 4), oB = cv.take(K * K * 4), oE = cv.take(4);
+    TG_CUDA(cudaMalloc(reinterpret_cast<void**>(&base), cv.off));
+    tg_instance* t = new (std::nothrow) tg_instance();
+    if (!t) { cudaFree(base); return fail(TG_ERR_OOM, "host allocation failed"); }
+    t->L = L; t->K = K; t->P = P; t->m = m; t->act_mb = act_mb; t->NS = NS; t->device = dev;
+    t->time_us = reinterpret_cast<int32_t*>(base + oT); t->mem_mb = reinterpret_cast<int32_t*>(base + oM);
+    t->gpus = reinterpret_cast<int32_t*>(base + oG); t->cap_mb = reinterpret_cast<int32_t*>(base + oC);
+    t->bw = reinterpret_cast<int32_t*>(base + oB);
+    int* dErr = reinterpret_cast<int*>(base + oE);
+    cudaError_t e = cudaMemcpy(t->time_us, time_us, nE * 4, cudaMemcpyDefault);
+    if (e == cudaSuccess) e = cudaMemcpy(t->mem_mb, mem_mb, nE * 4, cudaMemcpyDefault);
+    if (e == cudaSuccess) e = cudaMemcpy(t->gpus, island_gpus, K * 4, cudaMemcpyDefault);
+    if (e == cudaSuccess) e = cudaMemcpy(t->cap_mb, island_cap_mb, K * 4, cudaMemcpyDefault);
+    if (e == cudaSuccess) e = cudaMemcpy(t->bw, bw_gbps, K * K * 4, cudaMemcpyDefault);
+    if (e == cudaSuccess) e = cudaMemset(dErr, 0, 4);
+    int herr = 0;
+    if (e == cudaSuccess) {
+        const int blocks = int(std::min<size_t>((nE + 255) / 256, 4096));
+        tgValidateKernel<<<std::max(blocks, 1), 256>>>(t->time_us, t->mem_mb, t->gpus, t->cap_mb, t->bw, K, nE, dErr);
+        e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);
+    }
+    if (e != cudaSuccess || herr) {
+        cudaFree(base);
+        delete t;
+        if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("instance upload: ") + cudaGetErrorString(e));
+        return fail(TG_ERR_RANGE, "table value out of range (bits: 1 time, 2 mem, 4 bw, 8 gpus, 16 cap): " + std::to_string(herr));
+    }
+    *out = t;
+    return TG_OK;
+}
+
+tg_status tg_instance_destroy(tg_instance* inst) {
+    if (!inst) return TG_OK;
+    cudaFree(inst->time_us);  // base of the single allocation
+    delete inst;
+    return TG_OK;
+}
+
+tg_status tg_solve_batch_ex(tg_instance* const* instances, int32_t n, tg_result* out, uint32_t flags,
+                            tg_solve_stats* stats, void* cuda_stream) {
+    if (n == 0) return TG_OK;
+    if (!out) return fail(TG_ERR_NULL, "out is NULL");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Workspace W;
+    tg_status s = prepare(instances, n, true, st, W);
+    if (s != TG_OK) { if (W.base) cudaFreeAsync(W.base, st); return s; }
+    W.ctx.out = W.outDev; W.ctx.flags = flags; W.ctx.mode = 0;
+    s = launchSolve(W, st);
+    if (s != TG_OK) { cudaFreeAsync(W.base, st); return s; }
+    return finish(W, n, out, stats, st);
+}
+
+tg_status tg_solve_batch(tg_instance* const* instances, int32_t n, tg_result* out, void* cuda_stream) {
+    return tg_solve_batch_ex(instances, n, out, TG_SOLVE_DEFAULT, nullptr, cuda_stream);
+}
+
+tg_status tg_dp_at(tg_instance* inst, int64_t T, tg_result* out, void* cuda_stream) {
+    if (!inst || !out) return fail(TG_ERR_NULL, "NULL argument");
+    if (T > TG_TIME_MAX) T = -1;  // every finite cost is admissible
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Workspace W;
+    tg_instance* arr[1] = {inst};
+    tg_status s = prepare(arr, 1, true, st, W);
+    if (s != TG_OK) { if (W.base) cudaFreeAsync(W.base, st); return s; }
+    W.ctx.out = W.outDev; W.ctx.flags = 0; W.ctx.mode = 1;
+    W.ctx.dpT = T < 0 ? TG_TINF : uint32_t(T);
+    s = launchSolve(W, st);
+    if (s != TG_OK) { cudaFreeAsync(W.base, st); return s; }
+    return finish(W, 1, out, nullptr, st);
+}
+
+tg_status tg_reduce(tg_instance* inst, int32_t* c_out, int32_t* argp_out, int32_t* x_out, int32_t* cand_out,
+                    int32_t* n_cand_out, void* cuda_stream) {
+    if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    Workspace W;
+    tg_instance* arr[1] = {inst};
+    tg_status s = prepare(arr, 1, false, st, W);
+    if (s != TG_OK) { if (W.base) cudaFreeAsync(W.base, st); return s; }
+    const int cells = inst->NS * inst->K, K = inst->K;
+    int32_t *dc = nullptr, *da = nullptr, *dx = nullptr;
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&dc), size_t(cells) * 4 * 2 + K * K * 4, st));
+    da = dc + cells; dx = da + cells;
+    tgExportKernel<<<std::max(1, std::min((cells + 255) / 256, 1024)), 256, 0, st>>>(W.inst, dc, da, dx);
+    TgInstDev hI;
+    TG_CUDA(cudaMemcpyAsync(&hI, W.inst, sizeof(TgInstDev), cudaMemcpyDeviceToHost, st));
+    TG_CUDA(cudaStreamSynchronize(st));
+    if (c_out) TG_CUDA(cudaMemcpyAsync(c_out, dc, size_t(cells) * 4, cudaMemcpyDeviceToHost, st));
+    if (argp_out) TG_CUDA(cudaMemcpyAsync(argp_out, da, size_t(cells) * 4, cudaMemcpyDeviceToHost, st));
+    if (x_out) TG_CUDA(cudaMemcpyAsync(x_out, dx, size_t(K) * K * 4, cudaMemcpyDeviceToHost, st));
+    if (cand_out && hI.ncand > 0) TG_CUDA(cudaMemcpyAsync(cand_out, hI.cand, size_t(hI.ncand) * 4, cudaMemcpyDeviceToHost, st));
+    if (n_cand_out) *n_cand_out = hI.ncand;
+    TG_CUDA(cudaStreamSynchronize(st));
+    TG_CUDA(cudaFreeAsync(dc, st));
+    TG_CUDA(cudaFreeAsync(W.base, st));
+    return TG_OK;
+}
+
+tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4], void* cuda_stream) {
+    if (!inst || !counts_out) return fail(TG_ERR_NULL, "NULL argument");
+    if (mode != TG_PRUNE_EXACT && mode != TG_PRUNE_IMBALANCE && mode != TG_PRUNE_BOTTLENECK)
+        return fail(TG_ERR_RANGE, "unknown prune mode");
+    if (mode == TG_PRUNE_IMBALANCE && (threshold < 1000 || threshold > 16384))
+        return fail(TG_ERR_RANGE, "theta must be in [1000, 16384] permille");
+    if (mode == TG_PRUNE_BOTTLENECK && threshold < 0) return fail(TG_ERR_RANGE, "bottleneck cap must be >= 0");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int cells = inst->NS * inst->K;
+    char* ws = nullptr;
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&ws), 4 * 8 + (TG_MAX_K + 1) * 8, st));
+    unsigned long long* dCounts = reinterpret_cast<unsigned long long*>(ws);
+    long long* dCap = reinterpret_cast<long long*>(ws + 32);
+    TG_CUDA(cudaMemsetAsync(ws, 0, 32, st));
+    tgPruneCellKernel<<<(cells + 255) / 256, 256, 0, st>>>(inst->time_us, inst->mem_mb, inst->cap_mb, cells, inst->K,
+                                                          inst->P, int(mode), threshold, dCounts);
+    if (mode == TG_PRUNE_IMBALANCE) {
+        tgPruneTauKernel<<<1, 256, 0, st>>>(inst->time_us, inst->L, inst->K, inst->P, dCap);
+        tgPruneImbalanceKernel<<<(cells + 255) / 256, 256, 0, st>>>(inst->time_us, dCap, inst->L, inst->K, inst->P, cells,
+                                                                   threshold, dCounts);
+    }
+    TG_CUDA(cudaGetLastError());
+    unsigned long long hc[4];
+    TG_CUDA(cudaMemcpyAsync(hc, dCounts, 32, cudaMemcpyDeviceToHost, st));
+    TG_CUDA(cudaStreamSynchronize(st));
+    TG_CUDA(cudaFreeAsync(ws, st));
+    for (int i = 0; i < 4; ++i) counts_out[i] = int64_t(hc[i]);
+    return TG_OK;
+}
+
+tg_status tg_instance_read_time(tg_instance* inst, int32_t* time_out) {
+    if (!inst || !time_out) return fail(TG_ERR_NULL, "NULL argument");
+    TG_CUDA(cudaMemcpy(time_out, inst->time_us, size_t(inst->NS) * inst->K * inst->P * 4, cudaMemcpyDeviceToHost));
+    return TG_OK;
+}
+
+}  // extern "C"

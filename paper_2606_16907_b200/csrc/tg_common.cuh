@@ -1,0 +1,106 @@
+// Shared device/host definitions of libtangram (CUDA side only; the CPU oracle shares nothing
+// with this directory).  Notation follows SURVEY.md §8: slice [a,b), island k, mask S, R = S\{k}.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tangram.h"
+
+#define TG_INFU 0x40000000u   // saturating "no plan" (2^30); all DP values are uint32 <= 2^31
+#define TG_TINF 0x3fffffffu   // threshold standing for T = infinity: c <= TG_TINF  <=>  c finite
+#define TG_NT 512             // threads per CTA of the persistent solver
+#define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
+#define TG_MAX_NR 32          // masks R per tile
+#define TG_KEY_NONE 0xffffffffffffffffull
+
+// Row geometry of the diagonal-major cost tables.  Diagonal d = b - a (1..L).
+//   global  cd_k: row d holds a = 0..L-d        (b = a+d <= L),  padded to a multiple of 4
+//   staged  Cs_k: row d holds a = 0..L-1-d      (b <= L-1),       padded to a multiple of 4
+// tgF(m) = sum_{i=0..m} 4*floor(i/4); sum_{i=0..n} ceil4(i) = tgF(n+3).
+__host__ __device__ __forceinline__ uint32_t tgF(int m) {
+    if (m < 0) return 0;
+    const int q = m >> 2, rem = m & 3;
+    return uint32_t(8 * q * (q - 1) + 4 * q * (rem + 1));
+}
+// offset (words) of global row d (d = 1..L+1): sum_{d'<d} ceil4(L-d'+1)
+__host__ __device__ __forceinline__ uint32_t tgGOff(int L, int d) { return tgF(L + 3) - tgF(L - d + 4); }
+// offset (words) of staged row d (d = 1..L): sum_{d'<d} ceil4(L-d')
+__host__ __device__ __forceinline__ uint32_t tgSOff(int L, int d) { return tgF(L + 2) - tgF(L - d + 3); }
+
+__host__ __device__ __forceinline__ int tgSliceIdx(int L, int a, int b) {
+    return a * (2 * L - a + 1) / 2 + (b - a - 1);
+}
+
+// Per-instance record in the per-call workspace.  The host fills the pointers and dimensions; the
+// loader / prepare kernels fill the derived tables; the solver owns the state block.
+struct TgInstDev {
+    const int32_t* time_us;  // [NS][K][P] (instance-owned)
+    const int32_t* mem_mb;   // [NS][K][P]
+    const int32_t* cap_mb;   // [K]
+    const int32_t* bw_gbps;  // [K][K]
+    uint32_t* cd;            // [K][triG] diagonal-major reduced costs, TG_INFU = none
+    uint8_t* argp;           // [NS][K] lowest p attaining c, 0xff = none
+    uint32_t* cand;          // [nCandCap] ascending distinct finite c (first ncand valid)
+    uint32_t* sortbuf;       // [sortCap] scratch of the candidate sort (power of two)
+    uint32_t* sufMin;        // [K][L+2]: sufMin[k][d] = min over d' >= d, b <= L-1 of c  (d = 1..L)
+    int32_t L, K, P, m, act_mb, NS, Lp, triG;
+    int32_t sortCap, ncand;
+    uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
+    uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major
+    // ---- solver state (one scheduler thread per instance) ----
+    int32_t phase, lo, hi, next;
+    int32_t itemBeg, itemCnt, probeCnt, nrun;
+    uint32_t fInf;
+    int32_t incIdx;
+    int64_t incIter;
+    uint64_t fullWords;  // scratch words of a full-table DP of this instance (K islands alive)
+};
+
+enum { TG_PH_NEW = 0, TG_PH_INIT = 1, TG_PH_SEARCH = 2, TG_PH_SWEEP = 3, TG_PH_FINAL = 4, TG_PH_DONE = 5 };
+
+// One (instance, T) DP of a scheduler round.
+struct TgItem {
+    int32_t inst;
+    uint32_t T;          // threshold actually applied (TG_TINF for infinity)
+    int32_t tidx;        // index into cand, -1 = explicit T (infinity / tg_dp_at)
+    uint16_t alive;      // islands with some admissible slice at T (original labels)
+    uint8_t Ke;          // popcount(alive)
+    uint8_t flags;       // bit0: keep every level (back-track follows)
+    uint8_t isl[TG_MAX_K];  // compact label -> original island
+    uint64_t off;        // scratch offset in words
+    uint64_t bufWords;   // words of one ping-pong half (0 when every level is kept)
+};
+
+struct TgCtrl {
+    int32_t nItems[2];    // per round parity
+    int32_t nLevels[2];
+    int32_t done;
+    int32_t round;
+    uint32_t barrier;     // monotone arrival counter of the grid barrier
+    int32_t errFlag;
+    tg_solve_stats stats;
+};
+
+struct TgSolveCtx {
+    TgInstDev* inst;
+    int32_t nInst;
+    TgItem* items;              // [2][TG_MAX_ITEMS]
+    unsigned long long* keys;   // [2][TG_MAX_ITEMS] best (value, S, k) per item
+    uint32_t* tilePrefix;       // [2][TG_MAX_K + 1][TG_MAX_ITEMS + 1]
+    uint32_t* scratch;          // DP tables
+    uint64_t scratchWords;      // hard budget
+    uint64_t softWords;         // per-round target (keeps two wavefronts in L2)
+    TgCtrl* ctrl;
+    tg_result* out;
+    const uint16_t* maskOf;     // [65536] masks ordered by (popcount, value)
+    const uint16_t* rankOf;     // [65536] rank of a mask inside its popcount class
+    uint32_t flags;             // TG_SOLVE_*
+    int32_t mode;               // 0 = solve, 1 = single DP at dpT (tg_dp_at)
+    uint32_t dpT;
+    int32_t hsWords;            // words of shared memory for the H tile
+    int32_t csWords;            // words of shared memory available for staged cost tables
+};
+
+// binomials up to 16 choose r and popcount-class offsets into maskOf
+__constant__ uint16_t tgBinom[17][17];
+__constant__ uint32_t tgPopOff[18];

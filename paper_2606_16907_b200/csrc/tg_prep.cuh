@@ -1,0 +1,330 @@
+// Streaming kernels around the DP: input validation, cost-table loader,
+// transfer table (step 2), candidate thresholds (step 3) and the pruning pass (step 0, tg_prune).
+#pragma once
+#include "tg_common.cuh"
+
+// ---------------------------------------------------------------------------------------------
+// small helpers
+// ---------------------------------------------------------------------------------------------
+
+// slice index s -> (a, b):  s(a,b) = a(2L-a+1)/2 + (b-a-1)
+__device__ __forceinline__ void tgSliceAB(int L, int s, int& a, int& b) {
+    const float t = float(2 * L + 1);
+    int aa = int((t - sqrtf(fmaxf(t * t - 8.0f * float(s), 0.0f))) * 0.5f);
+    aa = max(0, min(aa, L - 1));
+    while (aa > 0 && aa * (2 * L - aa + 1) / 2 > s) --aa;
+    while (aa + 1 < L && (aa + 1) * (2 * L - aa) / 2 <= s) ++aa;
+    a = aa;
+    b = aa + 1 + (s - aa * (2 * L - aa + 1) / 2);
+}
+
+// exclusive block scan of one value per thread (blockDim.x <= 1024, multiple of 32);
+// returns the exclusive prefix and writes the block total to `total`.
+__device__ __forceinline__ uint32_t tgBlockExScan(uint32_t v, uint32_t* warpSums /*[33]*/, uint32_t& total) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    __syncthreads();  // protect warpSums reuse
+    if (lane == 31) warpSums[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t s = lane < nw ? warpSums[lane] : 0u, si = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, si, o);
+            if (lane >= o) si += t;
+        }
+        if (lane < nw) warpSums[lane] = si - s;
+        if (lane == 31) warpSums[32] = si;
+    }
+    __syncthreads();
+    total = warpSums[32];
+    return warpSums[w] + inc - v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// validation (tg_instance_create): err[0] |= bit per violated rule
+// ---------------------------------------------------------------------------------------------
+__global__ void tgValidateKernel(const int32_t* __restrict__ time_us, const int32_t* __restrict__ mem_mb,
+                                 const int32_t* __restrict__ gpus, const int32_t* __restrict__ cap,
+                                 const int32_t* __restrict__ bw, int K, size_t nEntries, int* err) {
+    int bad = 0;
+    for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < nEntries; i += size_t(gridDim.x) * blockDim.x) {
+        const int32_t t = time_us[i], mm = mem_mb[i];
+        if (t != TG_INVALID && (t < 0 || t > TG_TIME_MAX)) bad |= 1;
+        if (mm < 0) bad |= 2;
+    }
+    if (blockIdx.x == 0 && threadIdx.x < K * K) {
+        const int j = threadIdx.x / K, k = threadIdx.x % K;
+        if (j != k && bw[threadIdx.x] <= 0) bad |= 4;
+        if (j == 0) {
+            if (gpus[k] < 1) bad |= 8;
+            if (cap[k] < 0) bad |= 16;
+        }
+    }
+    if (bad) atomicOr(err, bad);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 1: cost-table loader.  One thread per (slice, island) cell, reduction over the P plans.
+//   c = min_p { time : time != INVALID, mem <= cap_k }, ties -> lowest p
+// Output goes straight into the diagonal-major layout the DP stages from, plus a flat copy for
+// the candidate sort.  HBM-bound stream: 8*P bytes read per cell.
+// ---------------------------------------------------------------------------------------------
+template <bool VEC4>
+__device__ __forceinline__ void tgReduceCell(const int32_t* __restrict__ tp, const int32_t* __restrict__ mp,
+                                             int P, int32_t capk, uint32_t& best, int& bp) {
+    best = TG_INFU;
+    bp = 0xff;
+    if (VEC4) {
+        const int4* t4 = reinterpret_cast<const int4*>(tp);
+        const int4* m4 = reinterpret_cast<const int4*>(mp);
+        for (int q = 0; q < (P >> 2); ++q) {
+            const int4 t = __ldg(t4 + q), mm = __ldg(m4 + q);
+            const int32_t tv[4] = {t.x, t.y, t.z, t.w}, mv[4] = {mm.x, mm.y, mm.z, mm.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                if (tv[e] != TG_INVALID && mv[e] <= capk && uint32_t(tv[e]) < best) { best = uint32_t(tv[e]); bp = 4 * q + e; }
+        }
+    } else {
+        for (int p = 0; p < P; ++p) {
+            const int32_t t = __ldg(tp + p), mm = __ldg(mp + p);
+            if (t != TG_INVALID && mm <= capk && uint32_t(t) < best) { best = uint32_t(t); bp = p; }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ insts) {
+    TgInstDev& I = insts[blockIdx.y];
+    const int L = I.L, K = I.K, P = I.P;
+    const int nCells = I.NS * K;
+    __shared__ uint32_t sMin[TG_MAX_K];
+    if (int(blockIdx.x) * 256 >= nCells) return;
+    if (threadIdx.x < TG_MAX_K) sMin[threadIdx.x] = TG_INFU;
+    __syncthreads();
+    const int cell = blockIdx.x * 256 + threadIdx.x;
+    if (cell < nCells) {
+        const int s = cell / K, k = cell - s * K;
+        const int32_t capk = __ldg(I.cap_mb + k);
+        uint32_t best; int bp;
+        const size_t e = size_t(cell) * P;
+        if ((P & 3) == 0) tgReduceCell<true>(I.time_us + e, I.mem_mb + e, P, capk, best, bp);
+        else tgReduceCell<false>(I.time_us + e, I.mem_mb + e, P, capk, best, bp);
+        int a, b;
+        tgSliceAB(L, s, a, b);
+        const int d = b - a;
+        uint32_t* row = I.cd + size_t(k) * I.triG + tgGOff(L, d);
+        row[a] = best;
+        if (b == L) {  // last element of the row: write the INF padding up to a multiple of 4
+            const int rl = (L - d + 1 + 3) & ~3;
+            for (int p = a + 1; p < rl; ++p) row[p] = TG_INFU;
+        }
+        I.argp[cell] = uint8_t(bp);
+        I.sortbuf[cell] = best;
+        if (best < TG_INFU) atomicMin(&sMin[k], best);
+    }
+    __syncthreads();
+    if (threadIdx.x < K && sMin[threadIdx.x] < TG_INFU) atomicMin(&I.cminAll[threadIdx.x], sMin[threadIdx.x]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Steps 2-3 and per-instance DP metadata.  One CTA per instance.
+//   x[j][k] = ceil(act_mb*1000 / bw[j][k])
+//   sufMin[k][d] = min over d' >= d, a <= L-1-d' of c[a][a+d'][k]  (widest admissible diagonal at T)
+//   cand = ascending distinct finite c                            (PAPER.md:250 (1))
+// Sort: bitonic network on a power-of-two buffer, in shared memory when it fits, else in place in
+// global memory (L2 resident).
+// ---------------------------------------------------------------------------------------------
+#define TG_PREP_NT 1024
+#define TG_SORT_SMEM_MAX 32768
+
+__global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restrict__ insts) {
+    extern __shared__ uint32_t sbuf[];
+    __shared__ uint32_t warpSums[33];
+    TgInstDev& I = insts[blockIdx.x];
+    const int L = I.L, K = I.K, tid = threadIdx.x;
+    // transfer table
+    if (tid < K * K) {
+        const int j = tid / K, k = tid % K;
+        uint32_t v = 0;
+        if (j != k) {
+            const int64_t num = int64_t(I.act_mb) * 1000, den = I.bw_gbps[tid];
+            const int64_t q = (num + den - 1) / den;
+            v = q > TG_TIME_MAX ? TG_INFU : uint32_t(q);
+        }
+        I.x[j * TG_MAX_K + k] = v;
+    }
+    // row minima (b <= L-1 only) then suffix minima over the diagonal index
+    uint32_t* sm = I.sufMin;
+    const int stride = L + 2;
+    for (int w = tid; w < K * (L + 2); w += TG_PREP_NT) {
+        const int k = w / stride, d = w - k * stride;
+        uint32_t mn = TG_INFU;
+        if (d >= 1 && d <= L - 1) {
+            const uint32_t* row = I.cd + size_t(k) * I.triG + tgGOff(L, d);
+            for (int a = 0; a <= L - 1 - d; ++a) mn = min(mn, row[a]);
+        }
+        sm[w] = mn;
+    }
+    __syncthreads();
+    if (tid < K) {
+        uint32_t run = TG_INFU;
+        for (int d = L + 1; d >= 0; --d) { run = min(run, sm[tid * stride + d]); sm[tid * stride + d] = run; }
+    }
+    // candidate sort
+    const int n = I.NS * K, N = I.sortCap;
+    uint32_t* buf = (N <= TG_SORT_SMEM_MAX) ? sbuf : I.sortbuf;
+    if (N <= TG_SORT_SMEM_MAX) {
+        for (int i = tid; i < N; i += TG_PREP_NT) sbuf[i] = i < n ? I.sortbuf[i] : 0xffffffffu;
+    } else {
+        for (int i = n + tid; i < N; i += TG_PREP_NT) I.sortbuf[i] = 0xffffffffu;
+    }
+    __syncthreads();
+    for (int kk = 2; kk <= N; kk <<= 1)
+        for (int j = kk >> 1; j > 0; j >>= 1) {
+            for (int i = tid; i < (N >> 1); i += TG_PREP_NT) {
+                const int l = ((i & ~(j - 1)) << 1) | (i & (j - 1)), r = l + j;
+                const uint32_t va = buf[l], vb = buf[r];
+                const bool asc = (l & kk) == 0;
+                if ((va > vb) == asc) { buf[l] = vb; buf[r] = va; }
+            }
+            __syncthreads();
+        }
+    // unique, finite only
+    uint32_t base = 0;
+    for (int i0 = 0; i0 < n; i0 += TG_PREP_NT) {
+        const int i = i0 + tid;
+        uint32_t v = 0xffffffffu, f = 0;
+        if (i < n) { v = buf[i]; f = (v < TG_INFU && (i == 0 || buf[i - 1] != v)) ? 1u : 0u; }
+        uint32_t tot;
+        const uint32_t pos = tgBlockExScan(f, warpSums, tot);
+        if (f) I.cand[base + pos] = v;
+        base += tot;
+    }
+    if (tid == 0) I.ncand = int(base);
+}
+
+// ---------------------------------------------------------------------------------------------
+// tg_reduce read-back: diagonal-major cd -> slice-major c[NS][K]
+// ---------------------------------------------------------------------------------------------
+__global__ void tgExportKernel(const TgInstDev* __restrict__ insts, int32_t* __restrict__ c_out,
+                               int32_t* __restrict__ argp_out, int32_t* __restrict__ x_out) {
+    const TgInstDev& I = insts[0];
+    const int L = I.L, K = I.K, nCells = I.NS * K;
+    for (int cell = blockIdx.x * blockDim.x + threadIdx.x; cell < nCells; cell += gridDim.x * blockDim.x) {
+        const int s = cell / K, k = cell - s * K;
+        int a, b;
+        tgSliceAB(L, s, a, b);
+        c_out[cell] = int32_t(I.cd[size_t(k) * I.triG + tgGOff(L, b - a) + a]);
+        const uint8_t p = I.argp[cell];
+        argp_out[cell] = p == 0xff ? -1 : int32_t(p);
+    }
+    if (blockIdx.x == 0 && threadIdx.x < K * K)
+        x_out[threadIdx.x] = int32_t(I.x[(threadIdx.x / K) * TG_MAX_K + threadIdx.x % K]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Step 0: pruning pass (SURVEY.md §8(c) rules R1-R4)
+// ---------------------------------------------------------------------------------------------
+// R1 infeasible, R2 dominated inside one (slice, island) cell, optional R4 bottleneck cap.
+__global__ void __launch_bounds__(256) tgPruneCellKernel(int32_t* __restrict__ time_us, const int32_t* __restrict__ mem_mb,
+                                                         const int32_t* __restrict__ cap, int nCells, int K, int P,
+                                                         int mode, int64_t threshold, unsigned long long* counts) {
+    const int cell = blockIdx.x * 256 + threadIdx.x;
+    unsigned c1 = 0, c2 = 0, c4 = 0;
+    if (cell < nCells) {
+        int32_t* t = time_us + size_t(cell) * P;
+        const int32_t* mm = mem_mb + size_t(cell) * P;
+        const int32_t capk = cap[cell % K];
+        for (int p = 0; p < P; ++p)
+            if (t[p] != TG_INVALID && mm[p] > capk) { t[p] = TG_INVALID; ++c1; }
+        uint32_t dead[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int p = 0; p < P; ++p) {
+            const int32_t tp = t[p];
+            if (tp == TG_INVALID) continue;
+            const int32_t mp = mm[p];
+            bool dd = false;
+            for (int q = 0; q < P && !dd; ++q) {
+                const int32_t tq = t[q];
+                if (q == p || tq == TG_INVALID) continue;
+                const int32_t mq = mm[q];
+                dd = (tq < tp && mq <= mp) || (tq <= tp && mq < mp) || (tq == tp && mq == mp && q < p);
+            }
+            if (dd) dead[p >> 5] |= 1u << (p & 31);
+        }
+        for (int p = 0; p < P; ++p)
+            if (dead[p >> 5] >> (p & 31) & 1u) { t[p] = TG_INVALID; ++c2; }
+        if (mode == TG_PRUNE_BOTTLENECK)
+            for (int p = 0; p < P; ++p)
+                if (t[p] != TG_INVALID && int64_t(t[p]) > threshold) { t[p] = TG_INVALID; ++c4; }
+    }
+    // warp-aggregate the counters
+    for (int o = 16; o > 0; o >>= 1) {
+        c1 += __shfl_down_sync(0xffffffffu, c1, o);
+        c2 += __shfl_down_sync(0xffffffffu, c2, o);
+        c4 += __shfl_down_sync(0xffffffffu, c4, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (c1) atomicAdd(counts + 0, (unsigned long long)c1);
+        if (c2) atomicAdd(counts + 1, (unsigned long long)c2);
+        if (c4) atomicAdd(counts + 3, (unsigned long long)c4);
+    }
+}
+
+// R3 pre-pass: island capacity from profiled atom throughput.  capOut[k] = floor(2^32 / tau_k)
+// (0 = exempt), capOut[K] = sum.  One CTA.
+__global__ void tgPruneTauKernel(const int32_t* __restrict__ time_us, int L, int K, int P, long long* capOut) {
+    __shared__ unsigned long long tau[TG_MAX_K];
+    __shared__ int bad[TG_MAX_K];
+    if (threadIdx.x < TG_MAX_K) { tau[threadIdx.x] = 0; bad[threadIdx.x] = 0; }
+    __syncthreads();
+    for (int w = threadIdx.x; w < K * L; w += blockDim.x) {
+        const int k = w / L, l = w - k * L;
+        const int32_t* t = time_us + (size_t(tgSliceIdx(L, l, l + 1)) * K + k) * P;
+        long long best = TG_INF;
+        for (int p = 0; p < P; ++p) if (t[p] != TG_INVALID) best = min(best, (long long)t[p]);
+        if (best >= TG_INF) atomicOr(&bad[k], 1);
+        else atomicAdd(&tau[k], (unsigned long long)best);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long tot = 0;
+        for (int k = 0; k < K; ++k) {
+            long long C = 0;
+            if (!bad[k]) { long long tk = (long long)tau[k]; if (tk < 1) tk = 1; C = (1ll << 32) / tk; }
+            capOut[k] = C;
+            tot += C;
+        }
+        capOut[K] = tot;
+    }
+}
+
+// R3 imbalance: kill every plan of a (slice, island) pair whose atom share mismatches the island's
+// capacity share by more than theta (permille).
+__global__ void __launch_bounds__(256) tgPruneImbalanceKernel(int32_t* __restrict__ time_us, const long long* __restrict__ capIn,
+                                                              int L, int K, int P, int nCells, int64_t theta,
+                                                              unsigned long long* counts) {
+    const int cell = blockIdx.x * 256 + threadIdx.x;
+    unsigned c3 = 0;
+    if (cell < nCells) {
+        const int s = cell / K, k = cell - s * K;
+        const long long Ck = capIn[k], Ct = capIn[K];
+        if (Ck != 0) {
+            int a, b;
+            tgSliceAB(L, s, a, b);
+            const long long len = b - a;
+            const bool over = len * Ct * 1000 > theta * Ck * L;
+            const bool under = len * Ct * theta < 1000ll * Ck * L;
+            if (over || under) {
+                int32_t* t = time_us + size_t(cell) * P;
+                for (int p = 0; p < P; ++p) if (t[p] != TG_INVALID) { t[p] = TG_INVALID; ++c3; }
+            }
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) c3 += __shfl_down_sync(0xffffffffu, c3, o);
+    if ((threadIdx.x & 31) == 0 && c3) atomicAdd(counts + 2, (unsigned long long)c3);
+}

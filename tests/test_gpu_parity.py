@@ -1,0 +1,116 @@
+"""GPU parity: every step of the CUDA path against the CPU oracle, bit-exact, through the C ABI
+(paper_2606_16907_b200 is argument marshalling only).  Integer work: no tolerance anywhere."""
+import numpy as np
+import pytest
+
+import oracle
+import tg_inputs as gen
+from conftest import rescore
+
+pytestmark = pytest.mark.gpu
+
+STYLES = ["mixed", "ties", "tightmem", "asym", "sparse"]
+
+
+@pytest.fixture(scope="module")
+def tg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2606_16907_b200 as tg
+    tg.lib()
+    return tg
+
+
+def same(o, g, what=""):
+    """o: oracle.Result, g: numpy record or TgResult"""
+    feas = int(g["iter_time_us"]) != (1 << 63) - 1
+    assert o.feasible == feas, what
+    if not feas:
+        assert int(g["n_stages"]) == 0
+        return
+    n = int(g["n_stages"])
+    stages = [(int(g["stage_begin"][i]), int(g["stage_island"][i]), int(g["stage_plan"][i])) for i in range(n)]
+    assert (o.iter_time_us, o.sum_us, o.bottleneck_us, o.island_mask) == \
+           (int(g["iter_time_us"]), int(g["sum_us"]), int(g["bottleneck_us"]), int(g["island_mask"])), what
+    assert o.stages == stages, what
+
+
+def rec(r):
+    return {k: getattr(r, k) for k, _ in r._fields_}
+
+
+def solve_all(tg, insts, flags=0):
+    hs = [tg.instance_from_inputs(i) for i in insts]
+    res = tg.tg_solve_batch(hs, flags=flags)
+    for h in hs:
+        h.destroy()
+    return res
+
+
+def test_reduce_steps_1_to_3(tg):
+    for inst in [gen.config1(), gen.config1(0, 10), gen.config2(), gen.random_small(5, style="sparse"),
+                 gen.random_small(7, style="tightmem"), gen.config3(0, L=20, K=5)]:
+        h = tg.instance_from_inputs(inst)
+        c, argp, x, cand = tg.tg_reduce(h)
+        oc, oargp, ox, ocand = oracle.reduce(inst)
+        assert np.array_equal(c.astype(np.int64), oc)
+        assert np.array_equal(argp, oargp)
+        assert np.array_equal(x.astype(np.int64), ox)
+        assert np.array_equal(cand.astype(np.int64), ocand)
+        h.destroy()
+
+
+@pytest.mark.parametrize("style", STYLES)
+def test_random_small_batches(tg, style):
+    insts = [gen.random_small(s, Lmax=9, Kmax=6, Pmax=3, style=style) for s in range(400)]
+    res = solve_all(tg, insts)
+    for inst, g in zip(insts, res):
+        same(oracle.solve(inst), g, inst.name)
+
+
+def test_full_sweep_equals_windowed(tg):
+    insts = [gen.random_small(s + 900, Lmax=8, Kmax=5, Pmax=3, style=STYLES[s % 5]) for s in range(100)]
+    a = solve_all(tg, insts)
+    b = solve_all(tg, insts, flags=1)
+    for inst, ga, gb in zip(insts, a, b):
+        o = oracle.solve(inst)
+        same(o, ga, inst.name)
+        same(o, gb, inst.name + " full")
+
+
+def test_config1_and_twins(tg):
+    insts = [gen.config1(0, d) for d in (1, 10, 20)]
+    for inst, g in zip(insts, solve_all(tg, insts)):
+        same(oracle.solve(inst), g, inst.name)
+
+
+def test_config2(tg):
+    inst = gen.config2()
+    g = solve_all(tg, [inst])[0]
+    o = oracle.solve(inst)
+    same(o, g, inst.name)
+    st = [(int(g["stage_begin"][i]), int(g["stage_island"][i]), int(g["stage_plan"][i])) for i in range(int(g["n_stages"]))]
+    s, T, it, mask = rescore(inst, st)
+    assert (s, T, it, mask) == (int(g["sum_us"]), int(g["bottleneck_us"]), int(g["iter_time_us"]), int(g["island_mask"]))
+
+
+def test_dp_at_single_threshold(tg):
+    """Step 5 + 7 at one T against oracle.dp_at, including T = infinity and infeasible T."""
+    for inst in [gen.config1(), gen.config2(), gen.random_small(11, style="asym"), gen.config3(0, L=24, K=7)]:
+        h = tg.instance_from_inputs(inst)
+        _, _, _, cand = oracle.reduce(inst)
+        picks = [-1, int(cand[0]), int(cand[len(cand) // 3]), int(cand[len(cand) // 2]), int(cand[-1]), int(cand[-1]) + 5]
+        for T in picks:
+            o = oracle.dp_at(inst, T)
+            g = rec(tg.tg_dp_at(h, T))
+            same(o, g, f"{inst.name} T={T}")
+        h.destroy()
+
+
+def test_mid_size_scaled_configs(tg):
+    """Scaled-down twins of configs 3-5 that the oracle still solves in seconds: several tiles per
+    level, ragged last tile, L not a multiple of 4."""
+    insts = [gen.config3(0, L=30, K=8), gen.config4(0, L=22, K=9), gen.config5_one(3, L=26, K=7),
+             gen.config3(1, L=37, K=6), gen.config5_one(4, L=17, K=8)]
+    for inst, g in zip(insts, solve_all(tg, insts)):
+        same(oracle.solve(inst, n_threads=8), g, inst.name)
