@@ -541,7 +541,8 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
                     I.incIdx = n - 1;
                     I.incIter = int64_t(I.fInf) + int64_t(I.m - 1) * int64_t(I.cand[n - 1]);
                     if (full) { I.phase = TG_PH_SWEEP; I.next = 0; }
-                    else { I.phase = TG_PH_SEARCH; I.lo = 0; I.hi = n - 1; }
+                    else if (n > 1) { I.phase = TG_PH_SEARCH; I.lo = 0; I.hi = n - 1; }
+                    else { I.phase = TG_PH_SWEEP; I.next = n; }  // single candidate: already seeded
                 }
             } else if (I.phase == TG_PH_SEARCH) {
                 int lo = I.lo, hi = I.hi, prevIdx = -1;
