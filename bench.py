@@ -1,0 +1,264 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the TANGRAM composition search on B200 (contract: see DESIGN.md §Measurement).
+
+A step = one tg_solve_batch over the workload's synthetic instances (whole hot path: loader,
+candidate thresholds, DP at T=inf, windowed per-T wavefront DPs, sweep reduction, back-track).
+metric  = slice/island plans evaluated per second, "plans evaluated" of one DP(T) being the dense
+          relaxation count NS*K*2^(K-1), summed over the DPs the solver ran.
+value   = device-timed (CUDA events on the launching stream), instances resident in HBM.
+e2e     = same metric through the C ABI with HOST tables: tg_instance_create (H2D) + tg_solve_batch
+          with a host result buffer (D2H) inside the timed region.
+roofline= the persistent solver kernel: algorithmic bytes (every live DP state written once and read
+          once, 8 B per state) / its own event-timed duration, against the measured HBM copy peak.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "slice_island_plans_evaluated_per_sec"
+UNIT = "plans/s"
+
+
+def make_workload(name: str, rank: int, n_inst: int):
+    """Seeded synthetic instances (DESIGN.md input recipe).  Rank r takes its own seeds (weak scaling)."""
+    import tg_inputs as gen
+    if name == "cfg4":
+        return [gen.config4(rank)], "cfg4 MoE-like L=64 K=16 P=8 m=64 (BASELINE.json configs[3]), 1 instance/GPU"
+    if name == "cfg3":
+        return [gen.config3(rank)], "cfg3 70B-like L=80 K=12 P=8 m=32 (configs[2]), 1 instance/GPU"
+    if name == "cfg2":
+        return [gen.config2(rank)], "cfg2 7B-like L=32 K=6 P=4 m=16 (configs[1]), 1 instance/GPU"
+    if name == "cfg5":
+        return gen.config5(n_inst, first_seed=rank * n_inst), \
+            f"cfg5 throughput batch: {n_inst} instances L=48 K=10 P=4 m in {{4..64}} (configs[4]) per GPU"
+    raise SystemExit(f"unknown workload {name}")
+
+
+def dense_plans(inst) -> int:
+    return inst.L * (inst.L + 1) // 2 * inst.K * (1 << (inst.K - 1))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (profiling recipe)."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.rows, self.stop, self.index = [], threading.Event(), index
+        self.th = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                    "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                if o:
+                    self.rows.append([c.strip() for c in o.splitlines()[0].split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.1)
+
+    def __enter__(self):
+        self.th.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.th.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": int(self.rows[0][1]) if self.rows[0][1].isdigit() else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def oracle_sample(insts, workload: str, threads: int):
+    """Bounded sample of the workload on the CPU oracle, as it stands: `threads` concurrent single
+    DP(T) calls (oracle.dp_at releases the GIL inside the C++ library).  Returns (plans, seconds, text)."""
+    import oracle
+    inst = insts[0]
+    _, _, _, cand = oracle.reduce(inst)
+    # thresholds spread over the upper half of the candidate list (feasible region)
+    picks = [int(cand[len(cand) // 2 + (i * (len(cand) // 2 - 1)) // max(1, threads - 1)]) for i in range(threads)]
+    t0 = time.perf_counter()
+    ths = [threading.Thread(target=oracle.dp_at, args=(inst, T, False)) for T in picks]
+    for t in ths:
+        t.start()
+    for t in ths:
+        t.join()
+    dt = time.perf_counter() - t0
+    return dense_plans(inst) * len(picks), dt, f"{len(picks)} single-threshold DPs (oracle.dp_at) of {inst.name}, one per thread"
+
+
+def run_reference(args):
+    """Reference arm = the CPU oracle (this tier has no reference implementation)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    insts, desc = make_workload(args.workload, 0, min(args.n_inst, 4))
+    cores = max(1, min(oracle.hw_threads(), args.cpu_threads))
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(insts, args.workload, cores)
+    plans = secs = 0.0
+    sample = ""
+    for _ in range(args.steps):
+        p, dt, sample = oracle_sample(insts, args.workload, cores)
+        plans += p
+        secs += dt
+    v = plans / secs
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": desc, "l2": "n/a (CPU)"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_16907_b200 as tg
+    tg.lib()  # fail loudly if the CUDA library is missing
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    insts, desc = make_workload(args.workload, rank, args.n_inst)
+    n = len(insts)
+    stream = torch.cuda.current_stream()
+    flags = tg.TG_SOLVE_FULL_SWEEP if args.full_sweep else tg.TG_SOLVE_DEFAULT
+    handles = [tg.instance_from_inputs(i) for i in insts]            # resident in HBM
+    out = torch.empty(n * tg.RESULT_BYTES, dtype=torch.uint8, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    st = tg.TgSolveStats()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        tg.tg_solve_batch(handles, out=out, flags=flags, stats=st)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern_ms, plans, states, n_dp = [], 0, 0, 0
+    with ClockSampler(local) as clk:
+        for s in range(args.steps):
+            flush.fill_(s & 0xff)                                     # evict L2 between timed steps
+            ev[s][0].record(stream)
+            tg.tg_solve_batch(handles, out=out, flags=flags, stats=st)   # stats on host => synchronises
+            ev[s][1].record(stream)
+            torch.cuda.synchronize()
+            kern_ms.append(tg.tg_last_solver_kernel_ms())
+            plans += st.plans_dense
+            states += st.states_live
+            n_dp += st.n_dp
+            assert st.reserved[0] == 0, "solver error flag"
+        barrier()
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    # ---- end to end: host tables -> create (H2D) -> solve -> host results (D2H) ----
+    h2d = sum(i.time_us.nbytes + i.mem_mb.nbytes + i.bw_gbps.nbytes + 8 * i.K for i in insts)
+    d2h = n * tg.RESULT_BYTES
+    e2e_steps = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        hs = [tg.instance_from_inputs(i) for i in insts]
+        res = tg.tg_solve_batch(hs, out=None, flags=flags)            # host result buffer: D2H + sync inside
+        for h in hs:
+            h.destroy()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device="cuda")
+    u = torch.tensor([float(plans), float(plans) / args.steps * e2e_steps, float(n_dp)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    total_ms, e2e_s = t.tolist()
+    plans_all, plans_e2e, ndp_all = u.tolist()
+    if rank == 0:
+        peak, peak_src = peaks()
+        km = sum(kern_ms) / len(kern_ms)
+        alg_bytes = states / args.steps * 8.0                          # live state: 4 B written + 4 B read
+        achieved = alg_bytes / (km * 1e-3) / 1e9
+        inst0 = insts[0]
+        line = {"metric": METRIC, "value": plans_all / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+                "config": {"workload": desc, "sweep": "full" if args.full_sweep else "windowed (exact stop rule)",
+                           "l2": "256 MB buffer written between timed steps", "instances_per_gpu": n,
+                           "dps_per_step": ndp_all / args.steps / world,
+                           "planning_ms_per_instance": total_ms / args.steps / n},
+                "clocks": clk.summary(),
+                "e2e": {"value": plans_e2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "ms_per_step": e2e_s / e2e_steps * 1e3},
+                "gpu_launches": 3 * args.steps,
+                "roofline": {"bound": "hbm", "kernel": "tgSolveKernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                             "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                             "kernel_ms": km, "algorithmic_bytes_per_launch": alg_bytes,
+                             "us_per_dp": km * 1e3 / (n_dp / args.steps)}}
+        if not args.no_cpu_baseline:
+            import oracle
+            cores = max(1, min(oracle.hw_threads(), args.cpu_threads))
+            p, dt, sample = oracle_sample(insts, args.workload, cores)
+            line["cpu_baseline"] = {"value": p / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                    "seconds": dt}
+        print(json.dumps(line), flush=True)
+    for h in handles:
+        h.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--n-inst", type=int, default=1024, help="instances per GPU of the cfg5 batch")
+    ap.add_argument("--full-sweep", action="store_true", help="run the DP at every candidate T")
+    ap.add_argument("--cpu-threads", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

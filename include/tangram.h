@@ -144,6 +144,10 @@ tg_status tg_dp_at(tg_instance* inst, int64_t T, tg_result* out, void* cuda_stre
 /* Copies the instance's current time table (after pruning) to HOST time_out [NS][K][P]. */
 tg_status tg_instance_read_time(tg_instance* inst, int32_t* time_out);
 
+/* Device time in milliseconds of the persistent solver kernel most recently launched by this host
+ * thread (CUDA events recorded on its stream around the launch; waits for it to finish).  HOST out. */
+tg_status tg_last_solver_kernel_ms(float* ms_out);
+
 const char* tg_last_error(void); /* thread-local, valid until the next tg_* call on the thread */
 int32_t tg_version(void);
 

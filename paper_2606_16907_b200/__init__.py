@@ -62,7 +62,7 @@ class TangramError(RuntimeError):
 
 _lib = None
 EXPORTS = ["tg_instance_create", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
-           "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_error", "tg_version"]
+           "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_error", "tg_version"]
 
 
 def lib():
@@ -81,6 +81,7 @@ def lib():
         L.tg_reduce.argtypes = [vp, vp, vp, vp, vp, C.POINTER(i32), vp]
         L.tg_dp_at.argtypes = [vp, i64, vp, vp]
         L.tg_instance_read_time.argtypes = [vp, vp]
+        L.tg_last_solver_kernel_ms.argtypes = [C.POINTER(C.c_float)]
         L.tg_last_error.restype = C.c_char_p
         L.tg_version.restype = i32
         for name in EXPORTS:
@@ -213,6 +214,12 @@ def tg_instance_read_time(inst: Instance) -> np.ndarray:
     t = np.empty((inst.NS, inst.K, inst.P), dtype=np.int32)
     _check(lib().tg_instance_read_time(inst.handle, t.ctypes.data))
     return t
+
+
+def tg_last_solver_kernel_ms() -> float:
+    ms = C.c_float(0)
+    _check(lib().tg_last_solver_kernel_ms(C.byref(ms)))
+    return ms.value
 
 
 def results_from_tensor(out, n: int) -> np.ndarray:

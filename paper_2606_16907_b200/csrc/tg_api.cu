@@ -237,10 +237,15 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     return TG_OK;
 }
 
+thread_local cudaEvent_t g_evA = nullptr, g_evB = nullptr;  // bracket the last solver kernel of this thread
+
 tg_status launchSolve(Workspace& W, cudaStream_t st) {
     TgSolveCtx ctx = W.ctx;
     void* args[] = {&ctx};
+    if (!g_evA) { TG_CUDA(cudaEventCreate(&g_evA)); TG_CUDA(cudaEventCreate(&g_evB)); }
+    TG_CUDA(cudaEventRecord(g_evA, st));
     TG_CUDA(cudaLaunchCooperativeKernel((const void*)tgSolveKernel, dim3(W.numSMs), dim3(TG_NT), args, size_t(W.dynSmem), st));
+    TG_CUDA(cudaEventRecord(g_evB, st));
     return TG_OK;
 }
 
@@ -413,6 +418,14 @@ tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int
     TG_CUDA(cudaStreamSynchronize(st));
     TG_CUDA(cudaFreeAsync(ws, st));
     for (int i = 0; i < 4; ++i) counts_out[i] = int64_t(hc[i]);
+    return TG_OK;
+}
+
+tg_status tg_last_solver_kernel_ms(float* ms_out) {
+    if (!ms_out) return fail(TG_ERR_NULL, "ms_out is NULL");
+    if (!g_evA) return fail(TG_ERR_CUDA, "no solver kernel was launched on this thread");
+    TG_CUDA(cudaEventSynchronize(g_evB));
+    TG_CUDA(cudaEventElapsedTime(ms_out, g_evA, g_evB));
     return TG_OK;
 }
 
