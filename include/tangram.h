@@ -121,7 +121,9 @@ typedef enum {
 
 /* tg_prune — north_star "tg_prune(threshold) for the dominated-plan pruning"
  * (pruning policies), :43/:360 (incompatible partial plans); rules R1-R4 of SURVEY.md §8(c).
- * Marks entries of the instance's time table dead (TG_INVALID), in place, idempotent, monotone.
+ * Marks entries of the instance's time table dead (TG_INVALID), in place and monotone (never revives
+ * an entry).  EXACT and BOTTLENECK are idempotent; IMBALANCE re-estimates the islands' atom profile
+ * from the live table on every call, so a second call may kill more.
  *   counts_out  HOST int64[4]: entries newly killed by R1..R4.  The call synchronises `cuda_stream`. */
 tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4],
                    void* cuda_stream);

@@ -1,0 +1,59 @@
+#!/usr/bin/env python
+"""Writes tests/golden/expected_<cfg>.json: the CPU oracle's result (value AND plan) on the full-size
+configs of BASELINE.json, which take the oracle minutes and so cannot be recomputed inside the test run.
+Calls ONLY oracle/ and the seeded input generator; never the CUDA path.
+
+    python tests/golden/make_expected.py cfg3 cfg4 cfg5      (cfg5 = a fixed sample of the 1024 seeds)
+
+Also stores oracle.dp_at results at fixed quantile thresholds (single-DP parity for tg_dp_at)."""
+import json
+import os
+import sys
+import time
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
+
+import oracle            # noqa: E402
+import tg_inputs as gen  # noqa: E402
+
+CFG5_SEEDS = list(range(0, 1024, 32)) + [1, 2, 3, 4, 1023]      # 37 of the 1024 instances, every m value
+DP_QUANTILES = [0.35, 0.5, 0.8]                                 # thresholds for the single-DP records
+
+
+def rec(r):
+    return {"iter_time_us": r.iter_time_us, "sum_us": r.sum_us, "bottleneck_us": r.bottleneck_us,
+            "island_mask": r.island_mask, "stages": [list(s) for s in r.stages], "n_dp_run": r.n_dp_run,
+            "n_candidates": r.n_candidates, "feasible": r.feasible}
+
+
+def one(inst, threads, with_dp):
+    t0 = time.time()
+    out = {"name": inst.name, "L": inst.L, "K": inst.K, "P": inst.P, "m": inst.m, "solve": rec(oracle.solve(inst, n_threads=threads))}
+    if with_dp:
+        _, _, _, cand = oracle.reduce(inst)
+        out["dp_at"] = []
+        for T in [-1] + [int(cand[int(q * (len(cand) - 1))]) for q in DP_QUANTILES]:
+            out["dp_at"].append({"T": T, "res": rec(oracle.dp_at(inst, T, want_plan=True))})
+    out["oracle_seconds"] = round(time.time() - t0, 1)
+    return out
+
+
+def main():
+    threads = max(1, min(8, oracle.hw_threads()))
+    for name in sys.argv[1:]:
+        if name == "cfg3":
+            data = [one(gen.config3(), threads, True)]
+        elif name == "cfg4":
+            data = [one(gen.config4(), threads, True)]
+        elif name == "cfg5":
+            data = [dict(one(gen.config5_one(s), threads, False), seed=s) for s in CFG5_SEEDS]
+        else:
+            raise SystemExit(f"unknown config {name}")
+        with open(os.path.join(HERE, f"expected_{name}.json"), "w") as f:
+            json.dump({"written_by": "tests/golden/make_expected.py (CPU oracle only)", "records": data}, f, indent=1)
+        print(name, "done", [d["oracle_seconds"] for d in data], flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,95 @@
+"""GPU parity of tg_prune (rules R1-R4) against oracle.prune: the pruned time
+table and the per-rule counts, bit-exact; and solve(prune(x)) on the device against the oracle."""
+import numpy as np
+import pytest
+
+import oracle
+import tg_inputs as gen
+from test_gpu_parity import same, solve_all, STYLES
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def tg():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2606_16907_b200 as tg
+    tg.lib()
+    return tg
+
+
+def cases():
+    out = [gen.random_small(s + 8000, Lmax=9, Kmax=6, Pmax=7, style=STYLES[s % 5]) for s in range(60)]
+    out += [gen.config1(), gen.config1(0, 10), gen.config2(), gen.config3(0, L=21, K=5), gen.config4(0, L=18, K=6)]
+    return out
+
+
+@pytest.mark.parametrize("mode,thr", [(0, 0), (1, 16384), (1, 3000), (1, 1500), (1, 1000), (2, 0), (2, 700), (2, 5000), (2, 1 << 25)])
+def test_prune_table_and_counts(tg, mode, thr):
+    for inst in cases():
+        h = tg.instance_from_inputs(inst)
+        counts = tg.tg_prune(h, mode, thr)
+        t = tg.tg_instance_read_time(h)
+        pr, ocounts = oracle.prune(inst, mode, thr)
+        assert counts.tolist() == ocounts.tolist(), (inst.name, mode, thr)
+        assert np.array_equal(t, pr.time_us.reshape(t.shape)), (inst.name, mode, thr)
+        again = tg.tg_prune(h, mode, thr)                       # monotone; idempotent except R3, which
+        pr2, ocounts2 = oracle.prune(pr, mode, thr)             # re-profiles the live table (DESIGN.md R-r3)
+        assert again.tolist() == ocounts2.tolist()
+        if mode != 1:
+            assert again.tolist() == [0, 0, 0, 0]
+        t2 = tg.tg_instance_read_time(h)
+        assert np.array_equal(t2, pr2.time_us.reshape(t.shape)) and ((t == 0x7FFFFFFF) <= (t2 == 0x7FFFFFFF)).all()
+        pr = pr2
+        g = tg.tg_solve_batch([h])[0]                           # the pruned instance solves like the oracle's
+        same(oracle.solve(pr), g, inst.name)
+        h.destroy()
+
+
+def test_prune_errors(tg):
+    h = tg.instance_from_inputs(gen.config1())
+    for mode, thr in [(3, 0), (1, 999), (1, 16385), (2, -1)]:
+        with pytest.raises(tg.TangramError) as e:
+            tg.tg_prune(h, mode, thr)
+        assert e.value.status == 3
+    h.destroy()
+
+
+def test_create_rejects_bad_tables(tg):
+    inst = gen.config1()
+    bad = inst.copy(); bad.time_us[3, 1, 0] = -5
+    with pytest.raises(tg.TangramError) as e:
+        tg.instance_from_inputs(bad)
+    assert e.value.status == 3
+    bad = inst.copy(); bad.time_us[3, 1, 0] = (1 << 25) + 1
+    with pytest.raises(tg.TangramError):
+        tg.instance_from_inputs(bad)
+    bad = inst.copy(); bad.mem_mb[0, 0, 0] = -1
+    with pytest.raises(tg.TangramError):
+        tg.instance_from_inputs(bad)
+    bad = inst.copy(); bad.bw_gbps[0, 1] = 0
+    with pytest.raises(tg.TangramError):
+        tg.instance_from_inputs(bad)
+    bad = inst.copy(); bad.island_gpus[2] = 0
+    with pytest.raises(tg.TangramError):
+        tg.instance_from_inputs(bad)
+    ok = inst.copy(); ok.time_us[:] = 0x7FFFFFFF                # nothing feasible is not an error
+    g = solve_all(tg, [ok])[0]
+    assert int(g["iter_time_us"]) == (1 << 63) - 1 and int(g["n_stages"]) == 0
+
+
+def test_device_resident_tables_and_async_out(tg):
+    """EITHER pointers: device tables in, device results out on a side stream."""
+    import torch
+    insts = [gen.config2(s) for s in range(3)]
+    hs = [tg.instance_from_inputs(i, device_tables=True) for i in insts]
+    st = torch.cuda.Stream()
+    out = torch.empty(len(hs) * tg.RESULT_BYTES, dtype=torch.uint8, device="cuda")
+    with torch.cuda.stream(st):
+        tg.tg_solve_batch(hs, out=out, stream=st)
+    st.synchronize()
+    for inst, g in zip(insts, tg.results_from_tensor(out, len(hs))):
+        same(oracle.solve(inst), g, inst.name)
+    for h in hs:
+        h.destroy()
