@@ -173,6 +173,7 @@ def run_ours(args):
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     kern_ms, plans, states, n_dp = [], 0, 0, 0
+    cyc = [0] * 8
     with ClockSampler(local) as clk:
         for s in range(args.steps):
             flush.fill_(s & 0xff)                                     # evict L2 between timed steps
@@ -185,6 +186,7 @@ def run_ours(args):
             states += st.states_live
             n_dp += st.n_dp
             assert st.reserved[0] == 0, "solver error flag"
+            cyc = [c + int(v) for c, v in zip(cyc, st.cyc)]
         barrier()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     # ---- end to end: host tables -> create (H2D) -> solve -> host results (D2H) ----
@@ -227,7 +229,10 @@ def run_ours(args):
                 "roofline": {"bound": "hbm", "kernel": "tgSolveKernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                              "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                              "kernel_ms": km, "algorithmic_bytes_per_launch": alg_bytes,
-                             "us_per_dp": km * 1e3 / (n_dp / args.steps)}}
+                             "us_per_dp": km * 1e3 / (n_dp / args.steps),
+                             "cta_cycle_shares": dict(zip(["stage", "tile_meta", "transfer_min", "minplus", "team_wait",
+                                                           "grid_wait", "scheduler", "backtrack"],
+                                                          [round(c / max(1, sum(cyc)), 4) for c in cyc]))}}
         if not args.no_cpu_baseline:
             import oracle
             cores = max(1, min(oracle.hw_threads(), args.cpu_threads))

@@ -25,7 +25,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc] + NVCC_FLAGS + ["-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("TG_EXTRA_NVCC_FLAGS", "").split() + ["-o", tmp] + [os.path.join(CSRC, f) for f in SOURCES]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             sys.stderr.write(r.stdout + r.stderr)

@@ -1,6 +1,7 @@
 // libtangram host side: C-ABI entry points (include/tangram.h), instance ownership, workspace
 // carving and kernel launches.  No CPU fallback: every compute path ends in a CUDA launch.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -37,10 +38,15 @@ struct DeviceState {
     bool ready = false;
     int numSMs = 0;
     int smemOptin = 0;
+    int smemPerSM = 0;
+    int ctasPerSM = 0;    // co-resident CTAs of the solver per SM
+    int dynSmem = 0;      // dynamic shared memory of one solver CTA
     uint16_t* maskOf = nullptr;
     uint16_t* rankOf = nullptr;
 };
 std::mutex g_mu;
+// DPs per instance and scheduler round (speculation width of the threshold search / sweep)
+int g_wishMax = [] { const char* e = getenv("TG_WISH_MAX"); int v = e ? atoi(e) : 64; return v < 1 ? 1 : (v > 64 ? 64 : v); }();
 DeviceState g_dev[64];
 
 tg_status deviceInit(int dev, DeviceState** out) {
@@ -52,6 +58,7 @@ tg_status deviceInit(int dev, DeviceState** out) {
         TG_CUDA(cudaGetDeviceProperties(&prop, dev));
         D.numSMs = prop.multiProcessorCount;
         D.smemOptin = int(prop.sharedMemPerBlockOptin);
+        D.smemPerSM = int(prop.sharedMemPerMultiprocessor);
         int coop = 0;
         TG_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
         if (!coop) return fail(TG_ERR_CUDA, "device lacks cooperative launch");
@@ -83,9 +90,17 @@ tg_status deviceInit(int dev, DeviceState** out) {
         TG_CUDA(cudaFuncSetAttribute(tgPrepareKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TG_SORT_SMEM_MAX * 4));
         cudaFuncAttributes fa;
         TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
-        const int dyn = D.smemOptin - int(fa.sharedSizeBytes) - 1024;
-        if (dyn < 96 * 1024) return fail(TG_ERR_CUDA, "not enough shared memory per block for the solver");
+        // two co-resident CTAs per SM: each gets half of the SM's shared memory minus its static part
+        // and the 1 KB the driver reserves per CTA
+        int dyn = std::min(D.smemOptin, D.smemPerSM / 2) - int(fa.sharedSizeBytes) - 1024;
+        dyn &= ~1023;
+        if (dyn < 64 * 1024) return fail(TG_ERR_CUDA, "not enough shared memory per block for the solver");
         TG_CUDA(cudaFuncSetAttribute(tgSolveKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+        int occ = 0;
+        TG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tgSolveKernel, TG_NT, size_t(dyn)));
+        if (occ < 1) return fail(TG_ERR_CUDA, "solver kernel does not fit on an SM");
+        D.ctasPerSM = std::min(occ, 2);
+        D.dynSmem = dyn;
         // keep stream-ordered scratch cached between calls
         cudaMemPool_t pool;
         if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
@@ -123,7 +138,7 @@ struct Workspace {
     TgSolveCtx ctx;
     tg_result* outDev = nullptr;
     int dynSmem = 0;
-    int numSMs = 0;
+    int numCtas = 0;
 };
 
 // Lays out the per-call workspace, uploads the instance records and runs loader + prepare.
@@ -145,7 +160,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     std::vector<TgInstDev> h(n);
     std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSuf(n);
     int maxCells = 0, maxLp = 4;
-    uint64_t hardMin = 0, sumFull = 0;
+    uint64_t maxFull = 0;
     size_t denseCs = 0;
     for (int i = 0; i < n; ++i) {
         const tg_instance& t = *instances[i];
@@ -170,8 +185,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         }
         const uint64_t full = uint64_t(t.K) * (1ull << (t.K - 1)) * uint64_t(I.Lp);
         I.fullWords = full;
-        hardMin = std::max<uint64_t>(hardMin, std::max<uint64_t>(full, 2 * mx * uint64_t(I.Lp)));
-        sumFull += full;
+        maxFull = std::max<uint64_t>(maxFull, std::max<uint64_t>(full, 2 * mx * uint64_t(I.Lp)));
         denseCs = std::max<size_t>(denseCs, size_t(t.K) * tgSOff(t.L, t.L));
         maxCells = std::max(maxCells, cells);
         maxLp = std::max(maxLp, int(I.Lp));
@@ -183,17 +197,22 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     }
     const size_t oItems = cv.take(sizeof(TgItem) * 2 * TG_MAX_ITEMS);
     const size_t oKeys = cv.take(sizeof(unsigned long long) * 2 * TG_MAX_ITEMS);
-    const size_t oPre = cv.take(sizeof(uint32_t) * 2 * (TG_MAX_K + 1) * (TG_MAX_ITEMS + 1));
     const size_t oCtrl = cv.take(sizeof(TgCtrl));
     const size_t oOut = cv.take(sizeof(tg_result) * n);
-    const uint64_t softWords = 24ull << 20;  // 96 MB: two wavefronts of a round stay inside the 126 MB L2
-    uint64_t scratchWords = 0;
+    // DP scratch: nSlots slots, each able to hold every level of the largest instance.  A slot
+    // belongs to one team (team mode) or one CTA (solo mode) for the duration of a DP.
+    const int numCtas = D->numSMs * D->ctasPerSM;
+    const uint64_t slotWords = alignUp(size_t(maxFull) + 1024, 1024);
+    int nSlots = 0;
     if (needSolve) {
-        scratchWords = std::max<uint64_t>(hardMin + 2048, std::min<uint64_t>(std::max<uint64_t>(sumFull, softWords), 256ull << 20));
-        scratchWords += uint64_t(std::min(n * 32, TG_MAX_ITEMS)) * 1024;  // per-item 4 KB rounding
-        scratchWords = alignUp(scratchWords, 1024);
+        size_t freeB = 0, totalB = 0;
+        TG_CUDA(cudaMemGetInfo(&freeB, &totalB));
+        const uint64_t budget = std::min<uint64_t>(uint64_t(freeB) * 6 / 10, 12ull << 30);   // bytes
+        nSlots = int(std::min<uint64_t>(uint64_t(numCtas), budget / (slotWords * 4)));
+        if (nSlots < 1) nSlots = 1;   // let the allocation decide
     }
-    const size_t oScratch = cv.take(size_t(scratchWords) * 4, 4096);
+    const size_t oBar = cv.take(sizeof(uint32_t) * size_t(std::max(nSlots, 1)));
+    const size_t oScratch = cv.take(size_t(slotWords) * 4 * size_t(nSlots), 4096);
     W.bytes = cv.off + 4096;
     TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&W.base), W.bytes, st));
     for (int i = 0; i < n; ++i) {
@@ -205,28 +224,30 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     }
     W.inst = reinterpret_cast<TgInstDev*>(W.base + oInst);
     W.outDev = reinterpret_cast<tg_result*>(W.base + oOut);
-    W.numSMs = D->numSMs;
+    W.numCtas = numCtas;
     TG_CUDA(cudaMemcpyAsync(W.inst, h.data(), sizeof(TgInstDev) * n, cudaMemcpyHostToDevice, st));
     TG_CUDA(cudaMemsetAsync(W.base + oCtrl, 0, sizeof(TgCtrl), st));
 
     // shared-memory split of the solver: H tile rows vs staged cost tables
-    cudaFuncAttributes fa;
-    TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
-    W.dynSmem = (D->smemOptin - int(fa.sharedSizeBytes) - 1024) & ~15;
+    W.dynSmem = D->dynSmem;
     const int totalWords = W.dynSmem / 4;
-    int rows = 256;
-    while (rows > 64 && totalWords - (rows + 1) * (maxLp + 8) < int(std::min<size_t>(denseCs, size_t(totalWords)))) rows -= 32;
+    // H rows and source rows per tile: together at most ~2/3 of the dynamic shared memory
+    int rows = 128;
+    while (rows > 16 && (rows + 1) * (maxLp + 8) + rows * maxLp > totalWords * 2 / 3) rows -= 16;
     TgSolveCtx& c = W.ctx;
     memset(&c, 0, sizeof(c));
+    c.npRows = rows; c.srcRows = rows;
     c.hsWords = (rows + 1) * (maxLp + 8);
-    c.csWords = (totalWords - c.hsWords) & ~3;
+    c.srcWords = rows * maxLp;
+    c.csWords = (totalWords - c.hsWords - c.srcWords) & ~3;
     if (c.csWords < 0) return fail(TG_ERR_SHAPE, "shared memory too small for this instance shape");
     c.inst = W.inst; c.nInst = n;
     c.items = reinterpret_cast<TgItem*>(W.base + oItems);
     c.keys = reinterpret_cast<unsigned long long*>(W.base + oKeys);
-    c.tilePrefix = reinterpret_cast<uint32_t*>(W.base + oPre);
     c.scratch = reinterpret_cast<uint32_t*>(W.base + oScratch);
-    c.scratchWords = scratchWords; c.softWords = softWords;
+    c.slotWords = slotWords; c.nSlots = nSlots;
+    c.slotBar = reinterpret_cast<uint32_t*>(W.base + oBar);
+    c.wishMax = g_wishMax;
     c.ctrl = reinterpret_cast<TgCtrl*>(W.base + oCtrl);
     c.maskOf = D->maskOf; c.rankOf = D->rankOf;
 
@@ -244,7 +265,7 @@ tg_status launchSolve(Workspace& W, cudaStream_t st) {
     void* args[] = {&ctx};
     if (!g_evA) { TG_CUDA(cudaEventCreate(&g_evA)); TG_CUDA(cudaEventCreate(&g_evB)); }
     TG_CUDA(cudaEventRecord(g_evA, st));
-    TG_CUDA(cudaLaunchCooperativeKernel((const void*)tgSolveKernel, dim3(W.numSMs), dim3(TG_NT), args, size_t(W.dynSmem), st));
+    TG_CUDA(cudaLaunchCooperativeKernel((const void*)tgSolveKernel, dim3(W.numCtas), dim3(TG_NT), args, size_t(W.dynSmem), st));
     TG_CUDA(cudaEventRecord(g_evB, st));
     return TG_OK;
 }

@@ -8,7 +8,7 @@
 
 #define TG_INFU 0x40000000u   // saturating "no plan" (2^30); all DP values are uint32 <= 2^31
 #define TG_TINF 0x3fffffffu   // threshold standing for T = infinity: c <= TG_TINF  <=>  c finite
-#define TG_NT 512             // threads per CTA of the persistent solver
+#define TG_NT 256             // threads per CTA of the persistent solver (2 CTAs per SM)
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
 #define TG_MAX_NR 32          // masks R per tile
 #define TG_KEY_NONE 0xffffffffffffffffull
@@ -67,13 +67,12 @@ struct TgItem {
     uint8_t Ke;          // popcount(alive)
     uint8_t flags;       // bit0: keep every level (back-track follows)
     uint8_t isl[TG_MAX_K];  // compact label -> original island
-    uint64_t off;        // scratch offset in words
     uint64_t bufWords;   // words of one ping-pong half (0 when every level is kept)
 };
 
 struct TgCtrl {
     int32_t nItems[2];    // per round parity
-    int32_t nLevels[2];
+    uint32_t queue[2];    // solo mode: next item to hand out
     int32_t done;
     int32_t round;
     uint32_t barrier;     // monotone arrival counter of the grid barrier
@@ -86,10 +85,11 @@ struct TgSolveCtx {
     int32_t nInst;
     TgItem* items;              // [2][TG_MAX_ITEMS]
     unsigned long long* keys;   // [2][TG_MAX_ITEMS] best (value, S, k) per item
-    uint32_t* tilePrefix;       // [2][TG_MAX_K + 1][TG_MAX_ITEMS + 1]
-    uint32_t* scratch;          // DP tables
-    uint64_t scratchWords;      // hard budget
-    uint64_t softWords;         // per-round target (keeps two wavefronts in L2)
+    uint32_t* scratch;          // DP tables: nSlots slots of slotWords words
+    uint64_t slotWords;         // one slot holds every level of the largest instance of the batch
+    int32_t nSlots;             // <= gridDim.x; a slot belongs to one team (team mode) or one CTA (solo mode)
+    int32_t wishMax;            // DPs per instance and round, upper bound
+    uint32_t* slotBar;          // [nSlots] arrival counters of the team barriers, zeroed every round
     TgCtrl* ctrl;
     tg_result* out;
     const uint16_t* maskOf;     // [65536] masks ordered by (popcount, value)
@@ -97,7 +97,10 @@ struct TgSolveCtx {
     uint32_t flags;             // TG_SOLVE_*
     int32_t mode;               // 0 = solve, 1 = single DP at dpT (tg_dp_at)
     uint32_t dpT;
-    int32_t hsWords;            // words of shared memory for the H tile
+    int32_t hsWords;            // words of shared memory for the H tile: (npRows + 1) * (Lp + 8)
+    int32_t npRows;             // H rows = (mask, island) pairs per tile
+    int32_t srcRows;            // source rows of level r-1 staged per tile
+    int32_t srcWords;           // words of shared memory for the source rows
     int32_t csWords;            // words of shared memory available for staged cost tables
 };
 

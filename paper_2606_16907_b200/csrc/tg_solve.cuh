@@ -1,16 +1,22 @@
 // Persistent cooperative solver: scheduler state machine, per-T popcount-wavefront DP
 // (SURVEY.md §8(a) steps 4-5), threshold-sweep reduction (step 6) and plan back-tracker (step 7).
 //
-// One launch per tg_solve_batch.  Grid = one CTA per SM (cooperative launch, all CTAs resident).
+// One launch per tg_solve_batch.  Grid = 2 CTAs of 256 threads per SM (cooperative launch, all
+// co-resident), so that one CTA's memory phase overlaps the other's arithmetic phase.
 // A scheduler round is: CTA 0 folds the previous round's results into the per-instance state
-// machines and plans the next list of (instance, T) DPs ("items"); then all CTAs walk the
-// wavefront levels r = |R| = 0, 1, ... of ALL items of the round in lockstep, separated by a
-// grid-wide barrier, because level r reads only level r-1 (PAPER.md:250 (2): a stage is added in
-// front of a memoised suffix).  State g[a][S][k] is stored as G_r[rank(R)][slot(k)][a], R = S\{k}.
+// machines and plans the next list of (instance, T) DPs ("items"); grid barrier; the items are
+// executed; grid barrier.  Execution of a round's items:
+//   solo mode (items >= slots): every CTA pulls whole DPs from an atomic queue and walks all
+//        wavefront levels of its DP alone; levels are separated by __syncthreads only.
+//   team mode (items <  slots): the CTAs are dealt to the items in contiguous teams; a team
+//        walks the levels of its DP in lockstep, separated by a team barrier (one arrival
+//        counter per slot), never by a grid barrier.
+// Level r = |R| reads only level r-1 (PAPER.md:250 (2): a stage is added in front of a memoised
+// suffix).  State g[a][S][k] is stored as G_r[rank(R)][slot(k)][a], R = S\{k}.
 //
-// One tile = up to 32 masks R of one level of one item, processed by one CTA:
+// One tile = up to 32 masks R of one level, processed by one CTA:
 //   phase 1  H[R][k][b] = min_{j in R} x[k][j] + G_{r-1}[R\{j}][j][b]      (transfer pre-minimum;
-//            every source row is read from L2 once per tile, results stay in shared memory)
+//            every source row is read once, results stay in shared memory)
 //   phase 2  G_r[R][k][a] = min_{b>a, c<=T} c_k[a][b] + H[R][k][b]         (min-plus product against
 //            the thresholded, diagonal-major cost tables staged in shared memory; 4x4 register
 //            tiles, one add-min (VIADDMNMX) per relaxation, only admissible diagonals visited)
@@ -18,12 +24,21 @@
 #include "tg_common.cuh"
 #include "tg_prep.cuh"
 
-#define TG_MAXG 160           // groups of 4 pairs per tile: <= 512/4 + 16
-#define TG_NP_CAP 512         // rows of the H tile, upper bound
+#define TG_MAXG 64            // groups of 4 pairs per tile: <= 128/4 + 16
+
+#define TG_XM_WORDS 1536      // transfer sub-matrices of one tile: cnt * r * roundup4(nk) words
+
+struct TgTileMeta {
+    uint16_t tileMask[TG_MAX_NR];
+    uint8_t kList[TG_MAX_NR][TG_MAX_K];   // islands not in R, ascending
+    uint8_t jList[TG_MAX_NR][TG_MAX_K];   // islands in R, ascending
+    uint16_t grpPair[TG_MAXG][4];         // H rows of a group of 4 pairs with the same island
+    uint8_t grpK[TG_MAXG];
+    int nGroups, cnt, first;
+};
 
 struct TgShared {
     // staged item
-    int stagedItem;           // round * TG_MAX_ITEMS + item index, -1 = nothing staged
     int useGlobalC;
     int sL, sLp, sKe, sInst;
     uint32_t sT;
@@ -33,20 +48,28 @@ struct TgShared {
     uint32_t xS[TG_MAX_K][TG_MAX_K];
     uint8_t isl[TG_MAX_K];
     uint16_t rowOffS[258];
-    // tile
-    uint16_t tileMask[TG_MAX_NR];
-    uint8_t kList[TG_MAX_NR][TG_MAX_K];
-    uint8_t jList[TG_MAX_NR][TG_MAX_K];
-    uint32_t srcRow[TG_MAX_NR][TG_MAX_K];
-    uint16_t grpPair[TG_MAXG][4];
-    uint8_t grpK[TG_MAXG];
-    int nGroups;
-    unsigned long long tileKey;
-    // scheduler
+    uint16_t binom[17][17];
+    // tiles (double-buffered metadata: tile i+1 is prepared while tile i computes)
+    TgTileMeta meta[2];
+    alignas(16) uint32_t xm[TG_XM_WORDS];
+    alignas(8) unsigned long long mbar;
+    // scheduler / queue
     uint32_t warpSums[33];
     int iTmp[8];
     unsigned long long llTmp[2];
+    int curItem;
+    long long tmark;                // phase timer of thread 0
+    unsigned long long cyc[8];      // per-CTA cycle counters, flushed to the statistics at exit
 };
+
+// Phase timer: thread 0 charges the cycles since its previous mark to counter `which`.
+__device__ __forceinline__ void tgMark(TgShared& sm, int which) {
+    if (threadIdx.x == 0) {
+        const long long now = clock64();
+        sm.cyc[which] += (unsigned long long)(now - sm.tmark);
+        sm.tmark = now;
+    }
+}
 
 __device__ __forceinline__ uint32_t tgAddMin(uint32_t a, uint32_t b, uint32_t c) { return __viaddmin_u32(a, b, c); }
 
@@ -63,8 +86,20 @@ __device__ __forceinline__ void tgGridBarrier(TgCtrl* ctrl, uint32_t& epoch) {
         while (true) {
             const uint32_t v = *reinterpret_cast<volatile uint32_t*>(&ctrl->barrier);
             if (int32_t(v - target) >= 0) break;
-            __nanosleep(32);
+            __nanosleep(64);
         }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// Barrier of one team on its slot counter (zeroed by the scheduler every round).
+__device__ __forceinline__ void tgTeamBarrier(uint32_t* bar, uint32_t target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(bar, 1u);
+        while (*reinterpret_cast<volatile uint32_t*>(bar) < target) __nanosleep(32);
         __threadfence();
     }
     __syncthreads();
@@ -73,23 +108,12 @@ __device__ __forceinline__ void tgGridBarrier(TgCtrl* ctrl, uint32_t& epoch) {
 // rows (R,k) of wavefront level r with Ke islands alive
 __device__ __forceinline__ uint32_t tgLevelRows(int Ke, int r) { return uint32_t(tgBinom[Ke][r]) * uint32_t(Ke - r); }
 
-__device__ __forceinline__ uint64_t tgLevelOff(const TgItem& it, int Lp, int r) {
-    if (it.bufWords) return it.off + uint64_t(r & 1) * it.bufWords;
+// word offset of level r inside a slot: ping-pong halves, or every level kept (bufWords == 0)
+__device__ __forceinline__ uint64_t tgLevelOff(uint64_t bufWords, int Ke, int Lp, int r) {
+    if (bufWords) return uint64_t(r & 1) * bufWords;
     uint64_t rows = 0;
-    for (int q = 0; q < r; ++q) rows += tgLevelRows(it.Ke, q);
-    return it.off + rows * uint64_t(Lp);
-}
-
-// H-tile rows available for an instance of padded length Lp (one row is reserved as the all-INF dummy)
-__device__ __forceinline__ int tgNP(const TgSolveCtx& ctx, int Lp) {
-    return min(ctx.hsWords / (Lp + 8) - 1, TG_NP_CAP);
-}
-__device__ __forceinline__ int tgNR(int np, int nk) { return max(1, min(TG_MAX_NR, np / nk)); }
-__device__ __forceinline__ uint32_t tgTiles(const TgSolveCtx& ctx, int Ke, int Lp, int r) {
-    if (r >= Ke) return 0;
-    if (r == 0) return 1;
-    const int nr = tgNR(tgNP(ctx, Lp), Ke - r);
-    return (uint32_t(tgBinom[Ke][r]) + nr - 1) / nr;
+    for (int q = 0; q < r; ++q) rows += tgLevelRows(Ke, q);
+    return rows * uint64_t(Lp);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -98,13 +122,13 @@ __device__ __forceinline__ uint32_t tgTiles(const TgSolveCtx& ctx, int Ke, int L
 // Only diagonals d <= dmaxK[k] (widest admissible slice of island k at T) are staged; dmaxTile
 // gives the widest admissible diagonal of each 4-row tile, which bounds the phase-2 loop.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, const TgItem* itp, int itemId) {
+__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, const TgItem* itp) {
     __syncthreads();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
     const TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
     const int L = I.L, Lp = I.Lp, Ke = __ldcg(&itp->Ke);
     const uint32_t T = __ldcg(&itp->T);
-    if (tid == 0) { sm.stagedItem = itemId; sm.sL = L; sm.sLp = Lp; sm.sKe = Ke; sm.sT = T; sm.sInst = itp->inst; }
+    if (tid == 0) { sm.sL = L; sm.sLp = Lp; sm.sKe = Ke; sm.sT = T; sm.sInst = __ldcg(&itp->inst); }
     if (tid < TG_MAX_K) sm.isl[tid] = __ldcg(&itp->isl[tid]);
     for (int d = tid; d <= L + 1; d += TG_NT) sm.rowOffS[d] = d >= 1 && d <= L ? uint16_t(tgSOff(L, d)) : uint16_t(0);
     if (tid < Ke * Ke) {
@@ -130,7 +154,7 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     }
     // the all-INF dummy row of the H tile
     {
-        const int HS = Lp + 8, np = tgNP(ctx, Lp);
+        const int HS = Lp + 8, np = ctx.npRows;
         for (int w = tid; w < HS; w += TG_NT) Hs[np * HS + w] = TG_INFU;
     }
     __syncthreads();
@@ -165,12 +189,12 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
 
 // ---------------------------------------------------------------------------------------------
 // Level 0: R = {} : G_0[k][a] = c[a][L][k] if <= T  (single stage [a,L) on island k)
+// Every member of a team writes the same values (saves one team barrier); member 0 posts the key.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, const TgItem* itp, int itemIdx, unsigned long long* keys) {
+__device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsigned long long* key, bool post) {
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int L = sm.sL, Lp = sm.sLp, Ke = sm.sKe;
     const uint32_t T = sm.sT;
-    uint32_t* G = ctx.scratch + __ldcg(&itp->off);  // level 0 sits at the item's base in both layouts
     for (int w = threadIdx.x; w < Ke * Lp; w += TG_NT) {
         const int kc = w / Lp, a = w - kc * Lp;
         uint32_t v = TG_INFU;
@@ -179,46 +203,79 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, const TgItem* itp,
             if (v > T) v = TG_INFU;
         }
         G[w] = v;
-        if (a == 0 && v < TG_INFU)
-            atomicMin(keys + itemIdx, (unsigned long long)v << 32 | (unsigned long long)(1u << kc) << 8 | (unsigned long long)kc);
+        if (post && a == 0 && v < TG_INFU)
+            atomicMin(key, (unsigned long long)v << 32 | (unsigned long long)(1u << kc) << 8 | (unsigned long long)kc);
     }
+    asm volatile("fence.proxy.async.global;" ::: "memory");   // level 0 is read by bulk async copies
 }
 
 // ---------------------------------------------------------------------------------------------
-// One tile of level r >= 1: masks R = maskOf[popOff[r] + first .. first+cnt) of the staged item.
+// Tiles of level r >= 1.  A tile = `cnt` consecutive masks R (colexicographic rank first..) of the
+// staged item; its pairs (R, k), k not in R, are rows of the H tile.  Per tile:
+//   meta    unrank the masks, list members (j) and non-members (k), group pairs by island
+//   issue   one bulk async copy (TMA, cp.async.bulk) per source row G_{r-1}[R\{j}][j][.] into
+//           shared memory, completion on an mbarrier; issued one tile ahead of its use
+//   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[R][j][b]
+//   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]
 // ---------------------------------------------------------------------------------------------
-__device__ void tgTile(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* Hs, const TgItem* itp,
-                       int itemIdx, unsigned long long* keys, int r, int tile) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
-    const TgInstDev& I = ctx.inst[sm.sInst];
-    const int L = sm.sL, Lp = sm.sLp, Ke = sm.sKe, HS = Lp + 8, nb4 = Lp >> 2;
-    const uint32_t T = sm.sT;
-    const int nk = Ke - r;
-    const int np = tgNP(ctx, Lp), NR = tgNR(np, nk);
-    const int nMasks = tgBinom[Ke][r];
-    const int first = tile * NR, cnt = min(NR, nMasks - first);
-    TgItem itv;
-    itv.off = __ldcg(&itp->off); itv.bufWords = __ldcg(&itp->bufWords); itv.Ke = uint8_t(Ke);
-    const uint32_t* Gprev = ctx.scratch + tgLevelOff(itv, Lp, r - 1);
-    uint32_t* Gcur = ctx.scratch + tgLevelOff(itv, Lp, r);
+__device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
-    // ---- phase 0: tile metadata -------------------------------------------------------------
-    if (tid < cnt) {
-        const uint32_t R = ctx.maskOf[tgPopOff[r] + first + tid];
-        sm.tileMask[tid] = uint16_t(R);
-        int ji = 0, ki = 0;
-        for (int e = 0; e < Ke; ++e) {
-            if (R >> e & 1u) {
-                const uint32_t Rp = R ^ (1u << e);
-                sm.srcRow[tid][ji] = uint32_t(ctx.rankOf[Rp]) * uint32_t(nk + 1) + uint32_t(e - __popc(R & ((1u << e) - 1u)));
-                sm.jList[tid][ji++] = uint8_t(e);
-            } else {
-                sm.kList[tid][ki++] = uint8_t(e);
-            }
-        }
+__device__ __forceinline__ void tgMbarInit(unsigned long long* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tgSmemAddr(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void tgMbarExpect(unsigned long long* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tgSmemAddr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tgMbarWait(unsigned long long* bar, uint32_t parity) {
+    const uint32_t a = tgSmemAddr(bar);
+    uint32_t ok = 0;
+    while (!ok) {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
     }
-    if (warp == 0) {
-        const uint32_t R = lane < cnt ? uint32_t(ctx.maskOf[tgPopOff[r] + first + lane]) : 0xffffffffu;
+}
+__device__ __forceinline__ void tgBulkLoad(uint32_t* dstSmem, const uint32_t* srcGlobal, uint32_t bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(tgSmemAddr(dstSmem)), "l"(srcGlobal), "r"(bytes), "r"(tgSmemAddr(bar)) : "memory");
+}
+
+// masks per tile at level r: bounded by the H rows (cnt*nk), the source rows (cnt*r) and the xm table
+__device__ __forceinline__ int tgNR(const TgSolveCtx& ctx, int Ke, int r) {
+    const int nk = Ke - r, nkp = (nk + 3) & ~3;
+    int nr = min(TG_MAX_NR, ctx.npRows / nk);
+    nr = min(nr, ctx.srcRows / r);
+    nr = min(nr, TG_XM_WORDS / (r * nkp));
+    return max(nr, 1);
+}
+__device__ __forceinline__ uint32_t tgTiles(const TgSolveCtx& ctx, int Ke, int r) {
+    return (uint32_t(tgBinom[Ke][r]) + tgNR(ctx, Ke, r) - 1) / tgNR(ctx, Ke, r);
+}
+
+__device__ void tgTileMeta(TgShared& sm, TgTileMeta& M, int Ke, int r, int first, int cnt) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5, nk = Ke - r;
+    if (tid < cnt) {   // unrank: colexicographic rank -> mask (masks of one popcount ordered by value)
+        uint32_t rank = uint32_t(first + tid), R = 0;
+        int e = Ke - 1;
+        for (int i = r; i >= 1; --i) {
+            while (uint32_t(sm.binom[e][i]) > rank) --e;
+            rank -= sm.binom[e][i];
+            R |= 1u << e;
+            --e;
+        }
+        M.tileMask[tid] = uint16_t(R);
+    }
+    if (tid == 0) { M.cnt = cnt; M.first = first; }
+    __syncthreads();
+    for (int w = tid; w < cnt * Ke; w += TG_NT) {
+        const int rl = w / Ke, e = w - rl * Ke;
+        const uint32_t R = M.tileMask[rl];
+        const int below = __popc(R & ((1u << e) - 1u));
+        if (R >> e & 1u) M.jList[rl][below] = uint8_t(e);
+        else M.kList[rl][e - below] = uint8_t(e);
+    }
+    if (warp == nWarps - 1) {   // groups of 4 (mask, k) pairs sharing the island k
+        const uint32_t R = lane < cnt ? uint32_t(M.tileMask[lane]) : 0xffffffffu;
         int gbase = 0;
         for (int k = 0; k < Ke; ++k) {
             const bool ex = !(R >> k & 1u);
@@ -226,42 +283,83 @@ __device__ void tgTile(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, 
             const int n = __popc(bal), ng = (n + 3) >> 2;
             if (ex) {
                 const int rk = __popc(bal & ((1u << lane) - 1u));
-                sm.grpPair[gbase + (rk >> 2)][rk & 3] = uint16_t(lane * nk + (k - __popc(R & ((1u << k) - 1u))));
+                M.grpPair[gbase + (rk >> 2)][rk & 3] = uint16_t(lane * nk + (k - __popc(R & ((1u << k) - 1u))));
             }
-            if (lane < ng) sm.grpK[gbase + lane] = uint8_t(k);
-            if (lane < ((4 - (n & 3)) & 3)) sm.grpPair[gbase + ng - 1][3 - lane] = 0xffffu;  // pad the last group
+            if (lane < ng) M.grpK[gbase + lane] = uint8_t(k);
+            if (lane < ((4 - (n & 3)) & 3)) M.grpPair[gbase + ng - 1][3 - lane] = 0xffffu;  // pad the last group
             gbase += ng;
         }
-        if (lane == 0) { sm.nGroups = gbase; sm.tileKey = TG_KEY_NONE; }
+        if (lane == 0) M.nGroups = gbase;
     }
-    __syncthreads();
+}
 
-    // ---- phase 1: transfer pre-minimum into the H tile ----------------------------------------
-    // Hs[pair][i] = H[b = i+1]; thread = (mask, 4 consecutive b); all k not in R at once.
+// Issue the source-row copies of a tile and fill its transfer sub-matrices xm[(rl, ji)][s].
+__device__ void tgTileIssue(TgShared& sm, const TgTileMeta& M, uint32_t* src, const uint32_t* Gprev, int Ke, int r) {
+    const int tid = threadIdx.x, nk = Ke - r, nkp = (nk + 3) & ~3, Lp = sm.sLp, cnt = M.cnt;
+#ifndef TG_GENERIC_COPY
+    if (tid == 0) tgMbarExpect(&sm.mbar, uint32_t(cnt * r * Lp * 4));
+#endif
+    bool fenced = false;
+    for (int w = tid; w < cnt * r; w += TG_NT) {
+        const int rl = w / r, ji = w - rl * r;
+        uint32_t R = M.tileMask[rl];
+        // rank of R \ {e_ji}: elements before keep their position, elements after move down by one
+        uint32_t rank = 0;
+        int ej = 0;
+        for (int i = 0; i < r; ++i) {
+            const int e = __ffs(R) - 1;
+            R &= R - 1;
+            if (i < ji) rank += sm.binom[e][i + 1];
+            else if (i > ji) rank += sm.binom[e][i];
+            else ej = e;
+        }
+        const uint32_t row = rank * uint32_t(nk + 1) + uint32_t(ej - ji);
+        if (!fenced) { asm volatile("fence.proxy.async.global;" ::: "memory"); fenced = true; }
+#ifndef TG_GENERIC_COPY
+        tgBulkLoad(src + size_t(w) * Lp, Gprev + size_t(row) * Lp, uint32_t(Lp * 4), &sm.mbar);
+#else
+        for (int q = 0; q < Lp; q += 4)
+            *reinterpret_cast<uint4*>(src + size_t(w) * Lp + q) = tgLdcg4(Gprev + size_t(row) * Lp + q);
+#endif
+        uint32_t* xr = sm.xm + w * nkp;
+        for (int s = 0; s < nkp; ++s) xr[s] = s < nk ? sm.xS[M.kList[rl][s]][ej] : TG_INFU;   // x[k][j]: k sends to j
+    }
+}
+
+// phase 1: thread = (mask, 4 consecutive b), all k not in R at once.  Hs[pair][i] = H[b = i+1].
+__device__ __forceinline__ void tgTilePhase1(TgShared& sm, const TgTileMeta& M, uint32_t* Hs, const uint32_t* src, int Ke, int r) {
+    const int tid = threadIdx.x, nk = Ke - r, nkp = (nk + 3) & ~3, Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, cnt = M.cnt;
     for (int w = tid; w < cnt * nb4; w += TG_NT) {
         const int rl = w / nb4, b4 = w - rl * nb4;
-        uint32_t acc[TG_MAX_K - 1][4];
+        uint32_t acc[TG_MAX_K][4];
 #pragma unroll
-        for (int s = 0; s < TG_MAX_K - 1; ++s) { acc[s][0] = acc[s][1] = acc[s][2] = acc[s][3] = TG_INFU; }
+        for (int s = 0; s < TG_MAX_K; ++s) { acc[s][0] = acc[s][1] = acc[s][2] = acc[s][3] = TG_INFU; }
+        const bool hasNx = b4 + 1 < nb4;
+        const uint32_t* sp = src + size_t(rl * r) * Lp + 4 * b4;
+        const uint32_t* xp = sm.xm + (rl * r) * nkp;
         for (int ji = 0; ji < r; ++ji) {
-            const uint32_t* src = Gprev + size_t(sm.srcRow[rl][ji]) * Lp + 4 * b4;
-            const uint4 g4 = tgLdcg4(src);
-            const uint32_t nx = (b4 + 1 < nb4) ? __ldcg(src + 4) : TG_INFU;
-            const uint32_t* xr = &sm.xS[0][sm.jList[rl][ji]];
+            const uint4 g4 = *reinterpret_cast<const uint4*>(sp);
+            const uint32_t nx = hasNx ? sp[4] : TG_INFU;
 #pragma unroll
-            for (int s = 0; s < TG_MAX_K - 1; ++s) {
-                if (s < nk) {
-                    const uint32_t xv = xr[int(sm.kList[rl][s]) * TG_MAX_K];   // x[k][j]: k sends to j
-                    acc[s][0] = tgAddMin(xv, g4.y, acc[s][0]);
-                    acc[s][1] = tgAddMin(xv, g4.z, acc[s][1]);
-                    acc[s][2] = tgAddMin(xv, g4.w, acc[s][2]);
-                    acc[s][3] = tgAddMin(xv, nx, acc[s][3]);
+            for (int s4 = 0; s4 < TG_MAX_K / 4; ++s4) {
+                if (4 * s4 < nk) {
+                    const uint4 xv = *reinterpret_cast<const uint4*>(xp + 4 * s4);
+                    const uint32_t xa[4] = {xv.x, xv.y, xv.z, xv.w};
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        acc[4 * s4 + u][0] = tgAddMin(xa[u], g4.y, acc[4 * s4 + u][0]);
+                        acc[4 * s4 + u][1] = tgAddMin(xa[u], g4.z, acc[4 * s4 + u][1]);
+                        acc[4 * s4 + u][2] = tgAddMin(xa[u], g4.w, acc[4 * s4 + u][2]);
+                        acc[4 * s4 + u][3] = tgAddMin(xa[u], nx, acc[4 * s4 + u][3]);
+                    }
                 }
             }
+            sp += Lp;
+            xp += nkp;
         }
         uint32_t* hrow = Hs + size_t(rl * nk) * HS + 4 * b4;
 #pragma unroll
-        for (int s = 0; s < TG_MAX_K - 1; ++s) {
+        for (int s = 0; s < TG_MAX_K; ++s) {
             if (s < nk) {
                 *reinterpret_cast<uint4*>(hrow + size_t(s) * HS) = make_uint4(acc[s][0], acc[s][1], acc[s][2], acc[s][3]);
                 if (b4 == nb4 - 1) {
@@ -271,21 +369,27 @@ __device__ void tgTile(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, 
             }
         }
     }
-    __syncthreads();
+}
 
-    // ---- phase 2: min-plus product with the thresholded cost tables ------------------------------
-    const int nGroups = sm.nGroups;
+// phase 2: min-plus product with the thresholded cost tables; lane = 4 pairs of one island x 4 starts a
+__device__ __forceinline__ void tgTilePhase2(const TgSolveCtx& ctx, TgShared& sm, const TgTileMeta& M, const uint32_t* Cs,
+                                             const uint32_t* Hs, uint32_t* Gcur, unsigned long long* key, int Ke, int r) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
+    const TgInstDev& I = ctx.inst[sm.sInst];
+    const int L = sm.sL, Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, nk = Ke - r;
+    const uint32_t T = sm.sT;
+    const int nGroups = M.nGroups, first = M.first;
     const int nGQ = (nGroups + 3) >> 2, nAH = (nb4 + 7) >> 3;
-    const int dummy = np;  // all-INF row
+    const int dummy = ctx.npRows;  // all-INF row
     unsigned long long bestKey = TG_KEY_NONE;
     for (int wi = warp; wi < nGQ * nAH; wi += nWarps) {
         const int gq = wi / nAH, ah = wi - gq * nAH;
         const int g = gq * 4 + (lane >> 3), t = ah * 8 + (lane & 7);
         if (g >= nGroups || t >= nb4) continue;
-        const int k = sm.grpK[g];
+        const int k = M.grpK[g];
         int pr[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) { const int p = sm.grpPair[g][i]; pr[i] = p == 0xffff ? -1 : p; }
+        for (int i = 0; i < 4; ++i) { const int p = M.grpPair[g][i]; pr[i] = p == 0xffff ? -1 : p; }
         const int a0 = 4 * t;
         uint32_t acc[4][4];
 #pragma unroll
@@ -348,58 +452,74 @@ __device__ void tgTile(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, 
             *reinterpret_cast<uint4*>(Gcur + (size_t(first) * nk + pr[i]) * Lp + a0) =
                 make_uint4(acc[0][i], acc[1][i], acc[2][i], acc[3][i]);
             if (t == 0 && acc[0][i] < TG_INFU) {
-                const uint32_t S = uint32_t(sm.tileMask[pr[i] / nk]) | (1u << k);
-                const unsigned long long key = (unsigned long long)acc[0][i] << 32 | (unsigned long long)S << 8 | (unsigned long long)k;
-                bestKey = key < bestKey ? key : bestKey;
+                const uint32_t S = uint32_t(M.tileMask[pr[i] / nk]) | (1u << k);
+                const unsigned long long kk = (unsigned long long)acc[0][i] << 32 | (unsigned long long)S << 8 | (unsigned long long)k;
+                bestKey = kk < bestKey ? kk : bestKey;
             }
         }
     }
-    if (bestKey != TG_KEY_NONE) atomicMin(&sm.tileKey, bestKey);
+    // the rows just written are read by bulk async copies (async proxy) of the next level
+#ifdef TG_HEAVY_FENCE
+    __threadfence();
+    asm volatile("fence.proxy.async;" ::: "memory");
+#else
+    asm volatile("fence.proxy.async.global;" ::: "memory");
+#endif
+    if (__any_sync(0xffffffffu, bestKey != TG_KEY_NONE)) {
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long ot = __shfl_xor_sync(0xffffffffu, bestKey, o);
+            bestKey = ot < bestKey ? ot : bestKey;
+        }
+        if (lane == 0) atomicMin(key, bestKey);
+    }
+}
+
+// All tiles of level r that belong to this CTA (member, member + teamSize, ...), software-pipelined:
+// the source rows of tile i+1 are in flight while tile i runs its min-plus product.
+__device__ void tgRunLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* Hs, uint32_t* src,
+                           const uint32_t* Gprev, uint32_t* Gcur, unsigned long long* key, int Ke, int r, int member,
+                           int teamSize, uint32_t& parity) {
+    const int NR = tgNR(ctx, Ke, r), nMasks = tgBinom[Ke][r];
+    const int nT = (nMasks + NR - 1) / NR;
+    if (member >= nT) return;
+    tgTileMeta(sm, sm.meta[0], Ke, r, member * NR, min(NR, nMasks - member * NR));
     __syncthreads();
-    if (tid == 0 && sm.tileKey != TG_KEY_NONE) atomicMin(keys + itemIdx, sm.tileKey);
-}
-
-// ---------------------------------------------------------------------------------------------
-// Level dispatch: CTA c owns the contiguous tile range [N*c/G, N*(c+1)/G) of level r.
-// ---------------------------------------------------------------------------------------------
-__device__ void tgProcessLevel(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, int par, int r,
-                               int nItems, int round) {
-    const uint32_t* pre = ctx.tilePrefix + (size_t(par) * (TG_MAX_K + 1) + r) * (TG_MAX_ITEMS + 1);
-    const TgItem* items = ctx.items + size_t(par) * TG_MAX_ITEMS;
-    unsigned long long* keys = ctx.keys + size_t(par) * TG_MAX_ITEMS;
-    const uint32_t total = __ldcg(pre + nItems);
-    const uint32_t t0 = uint32_t(uint64_t(total) * blockIdx.x / gridDim.x);
-    const uint32_t t1 = uint32_t(uint64_t(total) * (blockIdx.x + 1) / gridDim.x);
-    if (t0 >= t1) return;
-    int lo = 0, hi = nItems - 1;  // last item with pre[item] <= t0
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if (__ldcg(pre + mid) <= t0) lo = mid; else hi = mid - 1;
-    }
-    int it = lo;
-    for (uint32_t t = t0; t < t1; ++t) {
-        while (t >= __ldcg(pre + it + 1)) ++it;
-        const int tileInItem = int(t - __ldcg(pre + it));
-        const int id = round * TG_MAX_ITEMS + it;
-        if (sm.stagedItem != id) tgStageItem(ctx, sm, Cs, Hs, items + it, id);
-        if (r == 0) tgLevel0(ctx, sm, items + it, it, keys);
-        else tgTile(ctx, sm, Cs, Hs, items + it, it, keys, r, tileInItem);
+    tgTileIssue(sm, sm.meta[0], src, Gprev, Ke, r);
+    tgMark(sm, 1);
+    int i = 0;
+    for (int tile = member; tile < nT; tile += teamSize, ++i) {
+        TgTileMeta& cur = sm.meta[i & 1];
+        TgTileMeta& nxt = sm.meta[(i + 1) & 1];
+        const int tn = tile + teamSize;
+        const bool hasNext = tn < nT;
+        if (hasNext) tgTileMeta(sm, nxt, Ke, r, tn * NR, min(NR, nMasks - tn * NR));
+        else __syncthreads();   // xm of this tile was written by other threads (tgTileIssue)
+        tgMark(sm, 1);
+#ifndef TG_GENERIC_COPY
+        tgMbarWait(&sm.mbar, parity);
+        parity ^= 1u;
+#endif
+        tgTilePhase1(sm, cur, Hs, src, Ke, r);
         __syncthreads();
+        tgMark(sm, 2);
+        if (hasNext) tgTileIssue(sm, nxt, src, Gprev, Ke, r);
+        tgTilePhase2(ctx, sm, cur, Cs, Hs, Gcur, key, Ke, r);
+        __syncthreads();
+        tgMark(sm, 3);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// Step 7: plan back-tracker.  One warp per kept-table item: re-derive the per-state argmin
-// (lowest b, then lowest j — SURVEY A13) along the optimal path from the stored G levels.
+// Step 7: plan back-tracker.  One warp, right after a DP that kept every level: re-derive the
+// per-state argmin (lowest b, then lowest j — SURVEY A13) along the optimal path from the stored
+// G levels of the slot.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned long long key) {
+__device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned long long key, const uint32_t* slot) {
     const int lane = threadIdx.x & 31;
     TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
     const int L = I.L, Lp = I.Lp, K = I.K, Ke = __ldcg(&itp->Ke);
     const uint32_t T = __ldcg(&itp->T);
     tg_result* out = ctx.out + __ldcg(&itp->inst);
-    TgItem itv;
-    itv.off = __ldcg(&itp->off); itv.bufWords = 0; itv.Ke = uint8_t(Ke);
     uint8_t isl[TG_MAX_K];
 #pragma unroll
     for (int e = 0; e < TG_MAX_K; ++e) isl[e] = __ldcg(&itp->isl[e]);
@@ -428,7 +548,7 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned l
             b = L;
         } else {
             const int r = __popc(R);
-            const uint32_t* Gl = ctx.scratch + tgLevelOff(itv, Lp, r - 1);
+            const uint32_t* Gl = slot + tgLevelOff(0, Ke, Lp, r - 1);
             const uint32_t* cdk = I.cd + size_t(ko) * I.triG;
             unsigned long long best = TG_KEY_NONE;
             for (int bb = a + 1 + lane; bb <= L - 1; bb += 32) {
@@ -481,6 +601,35 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned l
 }
 
 // ---------------------------------------------------------------------------------------------
+// One DP(T): all wavefront levels of one item by a team of `teamSize` CTAs (this CTA = `member`).
+// ---------------------------------------------------------------------------------------------
+__device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, uint32_t* src, const TgItem* itp,
+                          unsigned long long* key, int member, int teamSize, int slotIdx, uint32_t& parity) {
+    tgStageItem(ctx, sm, Cs, Hs, itp);
+    tgMark(sm, 0);
+    const int Ke = sm.sKe, Lp = sm.sLp;
+    const uint64_t bufWords = __ldcg(&itp->bufWords);
+    uint32_t* slot = ctx.scratch + uint64_t(slotIdx) * ctx.slotWords;
+    uint32_t* bar = ctx.slotBar + slotIdx;
+    uint32_t arrivals = 0;
+    if (Ke > 0) {
+        tgLevel0(ctx, sm, slot, key, member == 0);
+        __syncthreads();
+        for (int r = 1; r < Ke; ++r) {
+            const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Lp, r - 1);
+            uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Lp, r);
+            tgRunLevel(ctx, sm, Cs, Hs, src, Gprev, Gcur, key, Ke, r, member, teamSize, parity);
+            if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); tgMark(sm, 4); }
+            else __syncthreads();
+        }
+    }
+    tgMark(sm, 0);
+    if ((__ldcg(&itp->flags) & 1) && member == 0 && threadIdx.x < 32) tgBacktrack(ctx, itp, __ldcg(key), slot);
+    __syncthreads();
+    tgMark(sm, 7);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Scheduler (CTA 0): fold results of the previous round, plan the next one.
 //   NEW -> INIT   : DP at T = infinity gives f_inf, the lower bound of the stop rule
 //   SEARCH        : multi-section search for the lowest feasible candidate (feasibility is monotone)
@@ -501,8 +650,17 @@ __device__ __forceinline__ void tgFoldResult(TgInstDev& I, unsigned long long ke
     if (it < I.incIter || (it == I.incIter && tidx < I.incIdx)) { I.incIter = it; I.incIdx = tidx; }
 }
 
-__device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, int round) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// DPs per round an instance with K islands should run: enough that a team (grid / DPs) has about ten
+// tiles per member at the widest level, i.e. few members idle at the thin levels.
+__device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
+    int widest = 1;
+    for (int r = 1; r < K; ++r) widest = max(widest, int(tgTiles(ctx, K, r)));
+    const int team = max(1, widest / 10);
+    return min(max(int(gridDim.x) / team, 16), 64);
+}
+
+__device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
+    const int tid = threadIdx.x;
     const int par = round & 1, prv = par ^ 1;
     TgCtrl* ctrl = ctx.ctrl;
     TgItem* items = ctx.items + size_t(par) * TG_MAX_ITEMS;
@@ -511,12 +669,8 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
     const unsigned long long* keysPrev = ctx.keys + size_t(prv) * TG_MAX_ITEMS;
     const bool full = (ctx.flags & TG_SOLVE_FULL_SWEEP) != 0;
     const int nInst = ctx.nInst;
-    // planner scratch in dynamic shared memory
-    uint32_t* kw = dyn;                                        // [TG_MAX_ITEMS]
-    uint8_t* itKe = reinterpret_cast<uint8_t*>(dyn + TG_MAX_ITEMS);  // [TG_MAX_ITEMS]
-    uint16_t* itLp = reinterpret_cast<uint16_t*>(dyn + TG_MAX_ITEMS + TG_MAX_ITEMS / 4);  // [TG_MAX_ITEMS]
 
-    if (tid == 0) { sm.iTmp[0] = 0; sm.iTmp[1] = 0; sm.iTmp[2] = 0; sm.iTmp[3] = 0; sm.llTmp[0] = 0; sm.llTmp[1] = 0; sm.stagedItem = -1; }
+    if (tid == 0) { sm.iTmp[0] = 0; sm.iTmp[1] = 0; sm.llTmp[0] = 0; sm.llTmp[1] = 0; }
     __syncthreads();
 
     // ---- A: fold the previous round ---------------------------------------------------------
@@ -578,46 +732,31 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
     __syncthreads();
     nActive = sm.iTmp[0];
     if (nActive == 0) {
-        if (tid == 0) { ctrl->done = 1; ctrl->nItems[par] = 0; ctrl->nLevels[par] = 0; }
+        if (tid == 0) { ctrl->done = 1; ctrl->nItems[par] = 0; }
         return;
     }
 
-    // ---- C: wishes ---------------------------------------------------------------------------
-    const int capPerInst = max(1, min(32, TG_MAX_ITEMS / nActive));
+    // ---- B: how many DPs each instance may run this round -------------------------------------------
+    const int capAll = max(1, min(ctx.wishMax, TG_MAX_ITEMS / nActive));
     uint32_t carry = 0;
     for (int base = 0; base < nInst; base += TG_NT) {
         const int i = base + tid;
         int cnt = 0, kind = 0, first = 0, probes = 0, span = 0;
         if (i < nInst) {
             TgInstDev& I = ctx.inst[i];
-            if (I.phase == TG_PH_NEW || I.phase == TG_PH_INIT) {
-                I.phase = ctx.mode == 1 ? TG_PH_FINAL : TG_PH_INIT;
-            }
+            if (I.phase == TG_PH_NEW || I.phase == TG_PH_INIT) I.phase = ctx.mode == 1 ? TG_PH_FINAL : TG_PH_INIT;
             if (I.phase == TG_PH_SWEEP && !(I.next < I.ncand && tgMustEval(I, I.next, full))) I.phase = TG_PH_FINAL;
-            if (I.phase == TG_PH_INIT || I.phase == TG_PH_FINAL) { cnt = 1; kind = I.phase; }
-            else if (I.phase == TG_PH_SEARCH || I.phase == TG_PH_SWEEP) {
-                // size the wish by the scratch an item needs at its first threshold
-                const int tix = I.phase == TG_PH_SEARCH ? I.lo : I.next;
-                const uint32_t T = I.cand[tix];
-                int Ke = 0;
-                for (int k = 0; k < I.K; ++k) Ke += I.cminAll[k] <= T ? 1 : 0;
-                uint32_t mx = 1;
-                for (int q = 0; q < Ke; ++q) mx = max(mx, tgLevelRows(Ke, q));
-                const uint64_t est = 2ull * mx * uint64_t(I.Lp) * uint64_t(nActive);
-                uint64_t wsh = ctx.softWords / est;
-                if (wsh < 1) wsh = 1;
-                if (wsh > uint64_t(capPerInst)) wsh = uint64_t(capPerInst);
-                const int wish = int(wsh);
-                kind = I.phase;
-                if (I.phase == TG_PH_SEARCH) {
-                    span = I.hi - I.lo;
-                    probes = min(wish, span);
-                    cnt = probes; first = I.lo;
-                } else {
-                    first = I.next;
-                    int idx = first;
-                    while (cnt < wish && idx < I.ncand && tgMustEval(I, idx, full)) { ++cnt; ++idx; }
-                }
+            kind = I.phase;
+            const int capPerInst = min(capAll, tgWish(ctx, I.K));
+            if (I.phase == TG_PH_INIT || I.phase == TG_PH_FINAL) cnt = 1;
+            else if (I.phase == TG_PH_SEARCH) {
+                span = I.hi - I.lo;
+                probes = min(capPerInst, span);
+                cnt = probes; first = I.lo;
+            } else if (I.phase == TG_PH_SWEEP) {
+                first = I.next;
+                int idx = first;
+                while (cnt < capPerInst && idx < I.ncand && tgMustEval(I, idx, full)) { ++cnt; ++idx; }
             }
         }
         uint32_t tot;
@@ -646,7 +785,8 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
     __syncthreads();
     const int nIt = sm.iTmp[1];
 
-    // ---- D: per-item geometry ----------------------------------------------------------------
+    // ---- C: per-item geometry, statistics ------------------------------------------------------------
+    unsigned long long dense = 0, live = 0;
     for (int idx = tid; idx < nIt; idx += TG_NT) {
         TgItem& it = items[idx];
         const TgInstDev& I = ctx.inst[it.inst];
@@ -655,88 +795,28 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
             if (I.cminAll[k] <= it.T) { alive |= 1u << k; it.isl[Ke++] = uint8_t(k); }
         for (int e = Ke; e < TG_MAX_K; ++e) it.isl[e] = 0;
         it.alive = uint16_t(alive); it.Ke = uint8_t(Ke);
-        uint64_t words = 0;
-        if (Ke > 0) {
-            if (it.flags & 1) { it.bufWords = 0; words = uint64_t(Ke) * (1ull << (Ke - 1)) * uint64_t(I.Lp); }
-            else {
-                uint32_t mx = 1;
-                for (int q = 0; q < Ke; ++q) mx = max(mx, tgLevelRows(Ke, q));
-                it.bufWords = uint64_t(mx) * uint64_t(I.Lp);
-                words = 2 * it.bufWords;
-            }
-        } else it.bufWords = 0;
-        kw[idx] = uint32_t((words + 1023) >> 10);
-        itKe[idx] = uint8_t(Ke);
-        itLp[idx] = uint16_t(I.Lp);
-    }
-    __syncthreads();
-
-    // ---- E: scratch offsets, hard budget -------------------------------------------------------
-    uint32_t carryKw = 0;
-    const uint32_t budgetKw = uint32_t(ctx.scratchWords >> 10);
-    for (int base = 0; base < nIt; base += TG_NT) {
-        const int idx = base + tid;
-        const uint32_t v = idx < nIt ? kw[idx] : 0u;
-        uint32_t tot;
-        const uint32_t pos = tgBlockExScan(v, sm.warpSums, tot) + carryKw;
-        carryKw += tot;
-        if (idx < nIt) {
-            items[idx].off = uint64_t(pos) << 10;
-            if (pos + v <= budgetKw) atomicAdd(&sm.iTmp[2], 1);
+        it.bufWords = 0;
+        if (Ke > 0 && !(it.flags & 1)) {
+            uint32_t mx = 1;
+            for (int q = 0; q < Ke; ++q) mx = max(mx, tgLevelRows(Ke, q));
+            it.bufWords = uint64_t(mx) * uint64_t(I.Lp);
         }
-    }
-    __syncthreads();
-    const int nFit = sm.iTmp[2];
-
-    // ---- F: trim the instances' item ranges; statistics ------------------------------------------
-    for (int i = tid; i < nInst; i += TG_NT) {
-        TgInstDev& I = ctx.inst[i];
-        if (I.itemCnt > 0) {
-            if (I.itemBeg >= nFit) I.itemCnt = 0;
-            else I.itemCnt = min(I.itemCnt, nFit - I.itemBeg);
-        }
-    }
-    unsigned long long dense = 0, live = 0;
-    int maxKe = 0;
-    for (int idx = tid; idx < nFit; idx += TG_NT) {
         keys[idx] = TG_KEY_NONE;
-        const TgInstDev& I = ctx.inst[items[idx].inst];
-        const int Ke = itKe[idx];
         dense += (unsigned long long)I.NS * I.K << (I.K - 1);
         if (Ke) live += (unsigned long long)I.L * Ke << (Ke - 1);
-        maxKe = max(maxKe, Ke);
     }
     if (dense) atomicAdd(&sm.llTmp[0], dense);
     if (live) atomicAdd(&sm.llTmp[1], live);
-    if (maxKe) atomicMax(&sm.iTmp[3], maxKe);
-
-    // ---- H: per-level tile prefix sums, one warp per level -----------------------------------------
-    if (warp < TG_MAX_K) {
-        uint32_t* pre = ctx.tilePrefix + (size_t(par) * (TG_MAX_K + 1) + warp) * (TG_MAX_ITEMS + 1);
-        uint32_t run = 0;
-        for (int base = 0; base < nFit; base += 32) {
-            const int idx = base + lane;
-            const uint32_t v = idx < nFit ? tgTiles(ctx, itKe[idx], itLp[idx], warp) : 0u;
-            uint32_t inc = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += t;
-            }
-            if (idx < nFit) pre[idx] = run + inc - v;
-            run += __shfl_sync(0xffffffffu, inc, 31);
-        }
-        if (lane == 0) pre[nFit] = run;
-    }
+    for (int s = tid; s < ctx.nSlots; s += TG_NT) ctx.slotBar[s] = 0;
     __syncthreads();
     if (tid == 0) {
-        ctrl->nItems[par] = nFit;
-        ctrl->nLevels[par] = sm.iTmp[3];
-        ctrl->stats.n_dp += uint64_t(nFit);
+        ctrl->nItems[par] = nIt;
+        ctrl->queue[par] = 0;
+        ctrl->stats.n_dp += uint64_t(nIt);
         ctrl->stats.plans_dense += sm.llTmp[0];
         ctrl->stats.states_live += sm.llTmp[1];
         ctrl->stats.n_rounds += 1;
-        if (nFit == 0) { ctrl->errFlag = 1; ctrl->done = 1; }
+        if (nIt == 0) { ctrl->errFlag = 1; ctrl->done = 1; }
     }
 }
 
@@ -745,35 +825,56 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
 // ---------------------------------------------------------------------------------------------
 extern __shared__ uint4 tgDynSmem[];
 
-__global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) {
+__global__ void __launch_bounds__(TG_NT, 2) tgSolveKernel(const TgSolveCtx ctx) {
     __shared__ TgShared sm;
     uint32_t* dyn = reinterpret_cast<uint32_t*>(tgDynSmem);
     uint32_t* Cs = dyn;
     uint32_t* Hs = dyn + ctx.csWords;
-    uint32_t epoch = 0;
+    uint32_t* src = Hs + ctx.hsWords;
+    uint32_t epoch = 0, parity = 0;
     TgCtrl* ctrl = ctx.ctrl;
-    if (threadIdx.x == 0) sm.stagedItem = -1;
+    const int nCta = int(gridDim.x), b = int(blockIdx.x);
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 8; ++i) sm.cyc[i] = 0;
+        sm.tmark = clock64();
+        tgMbarInit(&sm.mbar, 1);
+    }
+    for (int w = threadIdx.x; w < 17 * 17; w += TG_NT) sm.binom[w / 17][w % 17] = tgBinom[w / 17][w % 17];
     __syncthreads();
     for (int round = 0;; ++round) {
-        const int par = round & 1, prv = par ^ 1;
-        // back-track the kept-table items of the previous round (their scratch is still intact)
-        if (round > 0) {
-            const int nPrev = __ldcg(&ctrl->nItems[prv]);
-            const TgItem* itemsPrev = ctx.items + size_t(prv) * TG_MAX_ITEMS;
-            const unsigned long long* keysPrev = ctx.keys + size_t(prv) * TG_MAX_ITEMS;
-            const int gw = blockIdx.x * (TG_NT >> 5) + (threadIdx.x >> 5), nw = gridDim.x * (TG_NT >> 5);
-            // CTA 0 is busy scheduling: give it the back-track work last
-            for (int idx = nw - 1 - gw; idx < nPrev; idx += nw)
-                if (__ldcg(&itemsPrev[idx].flags) & 1) tgBacktrack(ctx, itemsPrev + idx, __ldcg(keysPrev + idx));
-        }
-        if (blockIdx.x == 0) tgSchedule(ctx, sm, dyn, round);
+        const int par = round & 1;
+        if (b == 0) { tgSchedule(ctx, sm, round); tgMark(sm, 6); }
         tgGridBarrier(ctrl, epoch);
+        tgMark(sm, 5);
         if (__ldcg(&ctrl->done)) break;
-        const int nItems = __ldcg(&ctrl->nItems[par]), nLevels = __ldcg(&ctrl->nLevels[par]);
-        for (int r = 0; r < nLevels; ++r) {
-            tgProcessLevel(ctx, sm, Cs, Hs, par, r, nItems, round);
-            tgGridBarrier(ctrl, epoch);
+        const int nItems = __ldcg(&ctrl->nItems[par]);
+        const TgItem* items = ctx.items + size_t(par) * TG_MAX_ITEMS;
+        unsigned long long* keys = ctx.keys + size_t(par) * TG_MAX_ITEMS;
+        if (nItems >= ctx.nSlots) {
+            // solo mode: slot = CTA; whole DPs from the queue
+            if (b < ctx.nSlots) {
+                while (true) {
+                    __syncthreads();
+                    if (threadIdx.x == 0) sm.curItem = int(atomicAdd(&ctrl->queue[par], 1u));
+                    __syncthreads();
+                    const int it = sm.curItem;
+                    if (it >= nItems) break;
+                    tgRunItem(ctx, sm, Cs, Hs, src, items + it, keys + it, 0, 1, b, parity);
+                }
+            }
+        } else {
+            // team mode: team t = CTAs [t*nCta/nItems, (t+1)*nCta/nItems), slot = t
+            int t = int((int64_t(b) * nItems) / nCta);
+            while (t + 1 < nItems && int((int64_t(t + 1) * nCta) / nItems) <= b) ++t;
+            while (t > 0 && int((int64_t(t) * nCta) / nItems) > b) --t;
+            const int start = int((int64_t(t) * nCta) / nItems), end = int((int64_t(t + 1) * nCta) / nItems);
+            tgRunItem(ctx, sm, Cs, Hs, src, items + t, keys + t, b - start, end - start, t, parity);
         }
+        tgMark(sm, 0);
+        tgGridBarrier(ctrl, epoch);
+        tgMark(sm, 5);
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) ctrl->stats.n_barriers = epoch;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < 8; ++i) atomicAdd((unsigned long long*)&ctrl->stats.cyc[i], sm.cyc[i]);
+    if (b == 0 && threadIdx.x == 0) ctrl->stats.n_barriers = epoch;
 }
