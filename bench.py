@@ -174,6 +174,7 @@ def run_ours(args):
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     kern_ms, plans, states, n_dp = [], 0, 0, 0
     cyc = [0] * 8
+    relax = 0
     with ClockSampler(local) as clk:
         for s in range(args.steps):
             flush.fill_(s & 0xff)                                     # evict L2 between timed steps
@@ -187,6 +188,7 @@ def run_ours(args):
             n_dp += st.n_dp
             assert st.reserved[0] == 0, "solver error flag"
             cyc = [c + int(v) for c, v in zip(cyc, st.cyc)]
+            relax += int(st.reserved[1])
         barrier()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     # ---- end to end: host tables -> create (H2D) -> solve -> host results (D2H) ----
@@ -230,6 +232,10 @@ def run_ours(args):
                              "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                              "kernel_ms": km, "algorithmic_bytes_per_launch": alg_bytes,
                              "us_per_dp": km * 1e3 / (n_dp / args.steps),
+                             "alu": {"relaxations_per_launch": relax / args.steps,
+                                     "achieved_Trelax_s": relax / args.steps / (km * 1e-3) / 1e12,
+                                     "peak_Trelax_s": 148 * 64 * 1.965e9 / 1e12,
+                                     "frac": relax / args.steps / (km * 1e-3) / (148 * 64 * 1.965e9)},
                              "cta_cycle_shares": dict(zip(["stage", "tile_meta", "transfer_min", "minplus", "team_wait",
                                                            "grid_wait", "scheduler", "backtrack"],
                                                           [round(c / max(1, sum(cyc)), 4) for c in cyc]))}}

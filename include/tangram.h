@@ -95,7 +95,8 @@ typedef struct { /* optional diagnostics of one tg_solve_batch_ex call, written 
     uint64_t n_rounds;       /* scheduler rounds                                               */
     uint64_t n_barriers;     /* grid-wide barriers executed                                    */
     uint64_t n_items_global_c; /* DPs whose cost tables did not fit in shared memory           */
-    uint64_t reserved[2];    /* reserved[0] = internal error flag (0 = none)                  */
+    uint64_t reserved[2];    /* [0] internal error flag (0 = none); [1] admissible relaxations executed:
+                                stage (c <= T) + transfer, summed over DPs                      */
     uint64_t cyc[8];         /* SM cycles summed over CTAs (thread 0 of each): 0 cost-table staging,
                                 1 tile metadata, 2 transfer pre-minimum, 3 min-plus product, 4 team-barrier
                                 wait, 5 grid-barrier wait, 6 scheduler, 7 back-track                     */

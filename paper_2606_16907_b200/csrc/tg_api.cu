@@ -280,6 +280,17 @@ tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cud
         TG_CUDA(cudaMemcpyAsync(&W.ctx.ctrl->stats.reserved[0], &W.ctx.ctrl->errFlag, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
         TG_CUDA(cudaMemcpyAsync(stats, &W.ctx.ctrl->stats, sizeof(tg_solve_stats), cudaMemcpyDefault, st));
     }
+    static const bool dbg = getenv("TG_DEBUG") != nullptr;
+    if (dbg) {
+        static TgCtrl hc;
+        TG_CUDA(cudaMemcpyAsync(&hc, W.ctx.ctrl, sizeof(TgCtrl), cudaMemcpyDeviceToHost, st));
+        TG_CUDA(cudaStreamSynchronize(st));
+        const int nr = int(std::min<uint64_t>(hc.stats.n_rounds, 256));
+        fprintf(stderr, "[tg] rounds=%d dps=%llu\n", nr, (unsigned long long)hc.stats.n_dp);
+        for (int r = 0; r < nr; ++r)
+            fprintf(stderr, "[tg]  round %3d items %5d  %8.1f us\n", r, hc.roundItems[r],
+                    r + 1 < nr ? double(hc.roundNs[r + 1] - hc.roundNs[r]) * 1e-3 : 0.0);
+    }
     int32_t err = 0;
     if (sync) TG_CUDA(cudaMemcpyAsync(&err, &W.ctx.ctrl->errFlag, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     TG_CUDA(cudaFreeAsync(W.base, st));

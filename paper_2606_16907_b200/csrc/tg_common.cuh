@@ -78,6 +78,9 @@ struct TgCtrl {
     uint32_t barrier;     // monotone arrival counter of the grid barrier
     int32_t errFlag;
     tg_solve_stats stats;
+    // debugging aid (TG_DEBUG=1): start time and item count of the first rounds
+    unsigned long long roundNs[256];
+    int32_t roundItems[256];
 };
 
 struct TgSolveCtx {

@@ -44,10 +44,9 @@ struct TgShared {
     uint32_t sT;
     uint32_t baseK[TG_MAX_K];
     int dmaxK[TG_MAX_K];
-    int dmaxTile[TG_MAX_K][64];
+    uint8_t dmaxTile[TG_MAX_K][64];
     uint32_t xS[TG_MAX_K][TG_MAX_K];
     uint8_t isl[TG_MAX_K];
-    uint16_t rowOffS[258];
     uint16_t binom[17][17];
     // tiles (double-buffered metadata: tile i+1 is prepared while tile i computes)
     TgTileMeta meta[2];
@@ -118,19 +117,20 @@ __device__ __forceinline__ uint64_t tgLevelOff(uint64_t bufWords, int Ke, int Lp
 
 // ---------------------------------------------------------------------------------------------
 // Staging of one item's thresholded cost tables into shared memory.
-//   Cs_k[d][a] = c[a][a+d][k] if <= T and a+d <= L-1, else INF   (k in compact labels)
-// Only diagonals d <= dmaxK[k] (widest admissible slice of island k at T) are staged; dmaxTile
-// gives the widest admissible diagonal of each 4-row tile, which bounds the phase-2 loop.
+//   Cs_k[(d-1)*Lp + a] = c[a][a+d][k] if <= T and a+d <= L-1, else INF   (k in compact labels)
+// Rows d = 1..D_k, D_k = dmaxK[k] (widest admissible slice of island k at T) rounded up to a
+// multiple of 4 so that the min-plus loop needs no row predicate; uniform row stride Lp.
+// dmaxTile[k][t] = widest admissible diagonal of starts a = 4t..4t+3: bounds the phase-2 loop.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, const TgItem* itp) {
+__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, const TgItem* itp, bool count) {
     __syncthreads();
+    unsigned nAdm = 0;   // admissible (a, b, k) cost entries with b <= L-1 seen by this thread
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
     const TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
-    const int L = I.L, Lp = I.Lp, Ke = __ldcg(&itp->Ke);
+    const int L = I.L, Lp = I.Lp, Ke = __ldcg(&itp->Ke), nb4 = Lp >> 2;
     const uint32_t T = __ldcg(&itp->T);
     if (tid == 0) { sm.sL = L; sm.sLp = Lp; sm.sKe = Ke; sm.sT = T; sm.sInst = __ldcg(&itp->inst); }
     if (tid < TG_MAX_K) sm.isl[tid] = __ldcg(&itp->isl[tid]);
-    for (int d = tid; d <= L + 1; d += TG_NT) sm.rowOffS[d] = d >= 1 && d <= L ? uint16_t(tgSOff(L, d)) : uint16_t(0);
     if (tid < Ke * Ke) {
         const int kc = tid / Ke, jc = tid - kc * Ke;
         sm.xS[kc][jc] = I.x[int(__ldcg(&itp->isl[kc])) * TG_MAX_K + int(__ldcg(&itp->isl[jc]))];
@@ -144,11 +144,10 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         }
         sm.dmaxK[tid] = lo;
     }
-    for (int w = tid; w < TG_MAX_K * 64; w += TG_NT) (&sm.dmaxTile[0][0])[w] = 0;
     __syncthreads();
     if (tid == 0) {
         uint32_t acc = 0;
-        for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += sm.rowOffS[sm.dmaxK[kc] + 1]; }
+        for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += uint32_t((sm.dmaxK[kc] + 3) & ~3) * uint32_t(Lp); }
         sm.useGlobalC = acc > uint32_t(ctx.csWords) ? 1 : 0;
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
     }
@@ -160,29 +159,53 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     __syncthreads();
     if (!sm.useGlobalC) {
         for (int kc = 0; kc < Ke; ++kc) {
-            const int dk = sm.dmaxK[kc];
+            const int dk = sm.dmaxK[kc], Dk = (dk + 3) & ~3;
             const uint32_t* cdk = I.cd + size_t(sm.isl[kc]) * I.triG;
             uint32_t* dst = Cs + sm.baseK[kc];
-            for (int d0 = 1 + warp * 2; d0 <= dk; d0 += nWarps * 2) {
-#pragma unroll
-                for (int u = 0; u < 2; ++u) {
-                    const int d = d0 + u;
-                    if (d > dk) break;
-                    const int rl4 = (L - d + 3) >> 2;
-                    const uint32_t* src = cdk + tgGOff(L, d);
-                    for (int a4 = lane; a4 < rl4; a4 += 32) {
-                        uint4 v = __ldg(reinterpret_cast<const uint4*>(src) + a4);
-                        const int a = a4 * 4, amax = L - 1 - d;
-                        v.x = (a + 0 <= amax && v.x <= T) ? v.x : TG_INFU;
-                        v.y = (a + 1 <= amax && v.y <= T) ? v.y : TG_INFU;
-                        v.z = (a + 2 <= amax && v.z <= T) ? v.z : TG_INFU;
-                        v.w = (a + 3 <= amax && v.w <= T) ? v.w : TG_INFU;
-                        reinterpret_cast<uint4*>(dst + sm.rowOffS[d])[a4] = v;
-                        if (min(min(v.x, v.y), min(v.z, v.w)) < TG_INFU) atomicMax(&sm.dmaxTile[kc][a4], d);
-                    }
+            for (int w = tid; w < Dk * nb4; w += TG_NT) {
+                const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
+                uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+                if (d <= dk && a4 < ((L - d + 3) >> 2)) {
+                    v = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + a4);
+                    const int a = a4 * 4, amax = L - 1 - d;
+                    v.x = (a + 0 <= amax && v.x <= T) ? v.x : TG_INFU;
+                    v.y = (a + 1 <= amax && v.y <= T) ? v.y : TG_INFU;
+                    v.z = (a + 2 <= amax && v.z <= T) ? v.z : TG_INFU;
+                    v.w = (a + 3 <= amax && v.w <= T) ? v.w : TG_INFU;
+                    nAdm += (v.x < TG_INFU) + (v.y < TG_INFU) + (v.z < TG_INFU) + (v.w < TG_INFU);
                 }
+                reinterpret_cast<uint4*>(dst)[w] = v;
             }
         }
+        __syncthreads();
+        for (int w = tid; w < Ke * nb4; w += TG_NT) {   // widest admissible diagonal per 4 starts
+            const int kc = w / nb4, a4 = w - kc * nb4;
+            const uint4* col = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc]) + a4;
+            int d = sm.dmaxK[kc];
+            for (; d >= 1; --d) {
+                const uint4 v = col[(d - 1) * nb4];
+                if (min(min(v.x, v.y), min(v.z, v.w)) < TG_INFU) break;
+            }
+            sm.dmaxTile[kc][a4] = uint8_t(d);
+        }
+    } else {
+        for (int w = tid; w < Ke * nb4; w += TG_NT) {
+            const int kc = w / nb4, a4 = w - kc * nb4;
+            sm.dmaxTile[kc][a4] = uint8_t(max(0, min(sm.dmaxK[kc], L - 1 - 4 * a4)));
+        }
+        if (count)
+            for (int kc = 0; kc < Ke; ++kc) {
+                const uint32_t* cdk = I.cd + size_t(sm.isl[kc]) * I.triG;
+                for (int d = 1; d <= sm.dmaxK[kc]; ++d)
+                    for (int a = tid; a <= L - 1 - d; a += TG_NT) nAdm += cdk[tgGOff(L, d) + a] <= T ? 1u : 0u;
+            }
+    }
+    if (count) {   // statistics: admissible relaxations of this DP (stage + transfer)
+        for (int o = 16; o > 0; o >>= 1) nAdm += __shfl_down_sync(0xffffffffu, nAdm, o);
+        if (lane == 0 && nAdm && Ke > 0)
+            atomicAdd((unsigned long long*)&ctx.ctrl->stats.reserved[1], (unsigned long long)nAdm << (Ke - 1));
+        if (tid == 0 && Ke >= 2)
+            atomicAdd((unsigned long long*)&ctx.ctrl->stats.reserved[1], (unsigned long long)L * Ke * (Ke - 1) << (Ke - 2));
     }
     __syncthreads();
 }
@@ -371,100 +394,112 @@ __device__ __forceinline__ void tgTilePhase1(TgShared& sm, const TgTileMeta& M, 
     }
 }
 
-// phase 2: min-plus product with the thresholded cost tables; lane = 4 pairs of one island x 4 starts a
+__device__ __forceinline__ uint4 tgLds4(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+
+// One block of 4 diagonals d = d0+1..d0+4 for 4 pairs x 4 starts.  lo = H window [a0+d0, a0+d0+4),
+// hi = the next 4 values (loaded here); c rows at cAddr + e*cStride.  16 add-mins per diagonal.
+#define TG_P2_STEP(LO, HI)                                                                          \
+    {                                                                                               \
+        _Pragma("unroll") for (int i = 0; i < 4; ++i) {                                             \
+            const uint4 h = tgLds4(hAddr[i]);                                                       \
+            HI[i][0] = h.x; HI[i][1] = h.y; HI[i][2] = h.z; HI[i][3] = h.w;                         \
+            hAddr[i] += 16;                                                                         \
+        }                                                                                           \
+        _Pragma("unroll") for (int e = 0; e < 4; ++e) {                                             \
+            const uint4 c4 = tgLds4(cAddr + e * cStride);                                           \
+            const uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};                                        \
+            _Pragma("unroll") for (int ai = 0; ai < 4; ++ai)                                        \
+                _Pragma("unroll") for (int i = 0; i < 4; ++i)                                       \
+                    acc[ai][i] = tgAddMin(cv[ai], (ai + e < 4 ? LO[i][ai + e] : HI[i][ai + e - 4]), acc[ai][i]); \
+        }                                                                                           \
+        cAddr += 4 * cStride;                                                                       \
+    }
+
+// phase 2: min-plus product with the thresholded cost tables.  A quarter-warp owns a group of 4 pairs
+// of one island; its 8 lanes walk the 4-start tiles a0 = 4t of the row.
 __device__ __forceinline__ void tgTilePhase2(const TgSolveCtx& ctx, TgShared& sm, const TgTileMeta& M, const uint32_t* Cs,
                                              const uint32_t* Hs, uint32_t* Gcur, unsigned long long* key, int Ke, int r) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int L = sm.sL, Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, nk = Ke - r;
     const uint32_t T = sm.sT;
-    const int nGroups = M.nGroups, first = M.first;
-    const int nGQ = (nGroups + 3) >> 2, nAH = (nb4 + 7) >> 3;
-    const int dummy = ctx.npRows;  // all-INF row
+    const int nGroups = M.nGroups;
+    const int nGQ = (nGroups + 3) >> 2;
+    const uint32_t hsBase = tgSmemAddr(Hs), csBase = tgSmemAddr(Cs), cStride = uint32_t(Lp) * 4u;
+    uint32_t* const gBase = Gcur + size_t(M.first) * nk * Lp;
     unsigned long long bestKey = TG_KEY_NONE;
-    for (int wi = warp; wi < nGQ * nAH; wi += nWarps) {
-        const int gq = wi / nAH, ah = wi - gq * nAH;
-        const int g = gq * 4 + (lane >> 3), t = ah * 8 + (lane & 7);
-        if (g >= nGroups || t >= nb4) continue;
+    for (int gq = warp; gq < nGQ; gq += nWarps) {
+        const int g = gq * 4 + (lane >> 3);
+        if (g >= nGroups) continue;
         const int k = M.grpK[g];
         int pr[4];
 #pragma unroll
         for (int i = 0; i < 4; ++i) { const int p = M.grpPair[g][i]; pr[i] = p == 0xffff ? -1 : p; }
-        const int a0 = 4 * t;
-        uint32_t acc[4][4];
+        for (int t = lane & 7; t < nb4; t += 8) {
+            const int a0 = 4 * t;
+            uint32_t acc[4][4];
 #pragma unroll
-        for (int ai = 0; ai < 4; ++ai)
+            for (int ai = 0; ai < 4; ++ai)
 #pragma unroll
-            for (int i = 0; i < 4; ++i) acc[ai][i] = TG_INFU;
-        const uint32_t* hp[4];
+                for (int i = 0; i < 4; ++i) acc[ai][i] = TG_INFU;
+            if (!sm.useGlobalC) {
+                const int nq = (int(sm.dmaxTile[k][t]) + 3) >> 2;
+                if (nq > 0) {
+                    uint32_t hAddr[4];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) hp[i] = Hs + size_t(pr[i] < 0 ? dummy : pr[i]) * HS + a0;
-
-        if (!sm.useGlobalC) {
-            const int dm = sm.dmaxTile[k][t];
-            const uint32_t* cb = Cs + sm.baseK[k] + a0;
-            uint32_t W[4][8];
-            if (dm > 0) {
+                    for (int i = 0; i < 4; ++i) hAddr[i] = hsBase + uint32_t((pr[i] < 0 ? ctx.npRows : pr[i]) * HS + a0) * 4u;
+                    uint32_t cAddr = csBase + (sm.baseK[k] + uint32_t(a0)) * 4u;
+                    uint32_t Wa[4][4], Wb[4][4];
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const uint4 h = *reinterpret_cast<const uint4*>(hp[i]);
-                    W[i][4] = h.x; W[i][5] = h.y; W[i][6] = h.z; W[i][7] = h.w;
+                    for (int i = 0; i < 4; ++i) {
+                        const uint4 h = tgLds4(hAddr[i]);
+                        Wa[i][0] = h.x; Wa[i][1] = h.y; Wa[i][2] = h.z; Wa[i][3] = h.w;
+                        hAddr[i] += 16;
+                    }
+#pragma unroll 1
+                    for (int q = 0; q < nq; q += 2) {
+                        TG_P2_STEP(Wa, Wb)
+                        if (q + 1 >= nq) break;
+                        TG_P2_STEP(Wb, Wa)
+                    }
+                }
+            } else {
+                // cost tables too large for shared memory: read the reduced table from global (L2)
+                const uint32_t* cdk = I.cd + size_t(sm.isl[k]) * I.triG;
+                const int dm = sm.dmaxTile[k][t];
+                const uint32_t* hp[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) hp[i] = Hs + size_t(pr[i] < 0 ? ctx.npRows : pr[i]) * HS + a0;
+                for (int d = 1; d <= dm; ++d) {
+                    uint4 c4 = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d) + a0));
+                    const int amax = L - 1 - d;
+                    uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+                    for (int ai = 0; ai < 4; ++ai) {
+                        if (a0 + ai > amax || cv[ai] > T) cv[ai] = TG_INFU;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) acc[ai][i] = tgAddMin(cv[ai], hp[i][ai + d - 1], acc[ai][i]);
+                    }
                 }
             }
-            for (int q = 0; 4 * q < dm; ++q) {
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    W[i][0] = W[i][4]; W[i][1] = W[i][5]; W[i][2] = W[i][6]; W[i][3] = W[i][7];
-                    const uint4 h = *reinterpret_cast<const uint4*>(hp[i] + 4 * q + 4);
-                    W[i][4] = h.x; W[i][5] = h.y; W[i][6] = h.z; W[i][7] = h.w;
+            for (int i = 0; i < 4; ++i) {
+                if (pr[i] < 0) continue;
+                *reinterpret_cast<uint4*>(gBase + size_t(pr[i]) * Lp + a0) = make_uint4(acc[0][i], acc[1][i], acc[2][i], acc[3][i]);
+                if (t == 0 && acc[0][i] < TG_INFU) {
+                    const uint32_t S = uint32_t(M.tileMask[pr[i] / nk]) | (1u << k);
+                    const unsigned long long kk = (unsigned long long)acc[0][i] << 32 | (unsigned long long)S << 8 | (unsigned long long)k;
+                    bestKey = kk < bestKey ? kk : bestKey;
                 }
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int d = 4 * q + 1 + e;
-                    uint4 c4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
-                    if (d <= dm) c4 = *reinterpret_cast<const uint4*>(cb + sm.rowOffS[d]);
-                    const uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};
-#pragma unroll
-                    for (int ai = 0; ai < 4; ++ai)
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) acc[ai][i] = tgAddMin(cv[ai], W[i][ai + e], acc[ai][i]);
-                }
-            }
-        } else {
-            // cost tables too large for shared memory: read the reduced table from global (L2)
-            const uint32_t* cdk = I.cd + size_t(sm.isl[k]) * I.triG;
-            const int dm = min(sm.dmaxK[k], L - 1 - a0);
-            for (int d = 1; d <= dm; ++d) {
-                uint4 c4 = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d) + a0));
-                const int amax = L - 1 - d;
-                uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};
-#pragma unroll
-                for (int ai = 0; ai < 4; ++ai) {
-                    if (a0 + ai > amax || cv[ai] > T) cv[ai] = TG_INFU;
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) acc[ai][i] = tgAddMin(cv[ai], hp[i][ai + d - 1], acc[ai][i]);
-                }
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            if (pr[i] < 0) continue;
-            *reinterpret_cast<uint4*>(Gcur + (size_t(first) * nk + pr[i]) * Lp + a0) =
-                make_uint4(acc[0][i], acc[1][i], acc[2][i], acc[3][i]);
-            if (t == 0 && acc[0][i] < TG_INFU) {
-                const uint32_t S = uint32_t(M.tileMask[pr[i] / nk]) | (1u << k);
-                const unsigned long long kk = (unsigned long long)acc[0][i] << 32 | (unsigned long long)S << 8 | (unsigned long long)k;
-                bestKey = kk < bestKey ? kk : bestKey;
             }
         }
     }
     // the rows just written are read by bulk async copies (async proxy) of the next level
-#ifdef TG_HEAVY_FENCE
-    __threadfence();
-    asm volatile("fence.proxy.async;" ::: "memory");
-#else
     asm volatile("fence.proxy.async.global;" ::: "memory");
-#endif
     if (__any_sync(0xffffffffu, bestKey != TG_KEY_NONE)) {
         for (int o = 16; o > 0; o >>= 1) {
             const unsigned long long ot = __shfl_xor_sync(0xffffffffu, bestKey, o);
@@ -605,7 +640,7 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned l
 // ---------------------------------------------------------------------------------------------
 __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, uint32_t* src, const TgItem* itp,
                           unsigned long long* key, int member, int teamSize, int slotIdx, uint32_t& parity) {
-    tgStageItem(ctx, sm, Cs, Hs, itp);
+    tgStageItem(ctx, sm, Cs, Hs, itp, member == 0);
     tgMark(sm, 0);
     const int Ke = sm.sKe, Lp = sm.sLp;
     const uint64_t bufWords = __ldcg(&itp->bufWords);
@@ -810,6 +845,12 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     for (int s = tid; s < ctx.nSlots; s += TG_NT) ctx.slotBar[s] = 0;
     __syncthreads();
     if (tid == 0) {
+        if (round < 256) {
+            unsigned long long ns;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
+            ctrl->roundNs[round] = ns;
+            ctrl->roundItems[round] = nIt;
+        }
         ctrl->nItems[par] = nIt;
         ctrl->queue[par] = 0;
         ctrl->stats.n_dp += uint64_t(nIt);
