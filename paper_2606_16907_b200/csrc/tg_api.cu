@@ -90,16 +90,14 @@ tg_status deviceInit(int dev, DeviceState** out) {
         TG_CUDA(cudaFuncSetAttribute(tgPrepareKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TG_SORT_SMEM_MAX * 4));
         cudaFuncAttributes fa;
         TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
-        // two co-resident CTAs per SM: each gets half of the SM's shared memory minus its static part
-        // and the 1 KB the driver reserves per CTA
-        int dyn = std::min(D.smemOptin, D.smemPerSM / 2) - int(fa.sharedSizeBytes) - 1024;
+        int dyn = D.smemOptin - int(fa.sharedSizeBytes) - 1024;   // one CTA per SM
         dyn &= ~1023;
         if (dyn < 64 * 1024) return fail(TG_ERR_CUDA, "not enough shared memory per block for the solver");
         TG_CUDA(cudaFuncSetAttribute(tgSolveKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
         int occ = 0;
         TG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tgSolveKernel, TG_NT, size_t(dyn)));
         if (occ < 1) return fail(TG_ERR_CUDA, "solver kernel does not fit on an SM");
-        D.ctasPerSM = std::min(occ, 2);
+        D.ctasPerSM = 1;
         D.dynSmem = dyn;
         // keep stream-ordered scratch cached between calls
         cudaMemPool_t pool;
@@ -159,7 +157,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const size_t oInst = cv.take(sizeof(TgInstDev) * n);
     std::vector<TgInstDev> h(n);
     std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSuf(n);
-    int maxCells = 0, maxLp = 4;
+    int maxCells = 0, maxLp = 4, maxK = 1;
     uint64_t maxFull = 0;
     size_t denseCs = 0;
     for (int i = 0; i < n; ++i) {
@@ -189,6 +187,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         denseCs = std::max<size_t>(denseCs, size_t(t.K) * tgSOff(t.L, t.L));
         maxCells = std::max(maxCells, cells);
         maxLp = std::max(maxLp, int(I.Lp));
+        maxK = std::max(maxK, int(t.K));
         oCd[i] = cv.take(size_t(t.K) * I.triG * 4);
         oArgp[i] = cv.take(size_t(cells));
         oCand[i] = cv.take(size_t(cells) * 4);
@@ -228,19 +227,16 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     TG_CUDA(cudaMemcpyAsync(W.inst, h.data(), sizeof(TgInstDev) * n, cudaMemcpyHostToDevice, st));
     TG_CUDA(cudaMemsetAsync(W.base + oCtrl, 0, sizeof(TgCtrl), st));
 
-    // shared-memory split of the solver: H tile rows vs staged cost tables
+    // shared-memory split of the solver: warp-private row buffers (H rows + two source buffers =
+    // 2*Kmax rows of Lp+8 words per warp) vs staged cost tables (at least a quarter of the total)
     W.dynSmem = D->dynSmem;
     const int totalWords = W.dynSmem / 4;
-    // H rows and source rows per tile: together at most ~2/3 of the dynamic shared memory
-    int rows = 128;
-    while (rows > 16 && (rows + 1) * (maxLp + 8) + rows * maxLp > totalWords * 2 / 3) rows -= 16;
     TgSolveCtx& c = W.ctx;
     memset(&c, 0, sizeof(c));
-    c.npRows = rows; c.srcRows = rows;
-    c.hsWords = (rows + 1) * (maxLp + 8);
-    c.srcWords = rows * maxLp;
-    c.csWords = (totalWords - c.hsWords - c.srcWords) & ~3;
-    if (c.csWords < 0) return fail(TG_ERR_SHAPE, "shared memory too small for this instance shape");
+    c.wbufWords = 2 * maxK * (maxLp + 8);
+    c.nActiveWarps = std::min(TG_NT / 32, (totalWords * 3 / 4) / c.wbufWords);
+    if (c.nActiveWarps < 1) return fail(TG_ERR_SHAPE, "shared memory too small for this instance shape");
+    c.csWords = (totalWords - c.nActiveWarps * c.wbufWords) & ~3;
     c.inst = W.inst; c.nInst = n;
     c.items = reinterpret_cast<TgItem*>(W.base + oItems);
     c.keys = reinterpret_cast<unsigned long long*>(W.base + oKeys);

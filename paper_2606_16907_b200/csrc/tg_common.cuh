@@ -8,7 +8,7 @@
 
 #define TG_INFU 0x40000000u   // saturating "no plan" (2^30); all DP values are uint32 <= 2^31
 #define TG_TINF 0x3fffffffu   // threshold standing for T = infinity: c <= TG_TINF  <=>  c finite
-#define TG_NT 256             // threads per CTA of the persistent solver (2 CTAs per SM)
+#define TG_NT 512             // threads per CTA of the persistent solver (1 CTA per SM)
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
 #define TG_MAX_NR 32          // masks R per tile
 #define TG_KEY_NONE 0xffffffffffffffffull
@@ -100,11 +100,9 @@ struct TgSolveCtx {
     uint32_t flags;             // TG_SOLVE_*
     int32_t mode;               // 0 = solve, 1 = single DP at dpT (tg_dp_at)
     uint32_t dpT;
-    int32_t hsWords;            // words of shared memory for the H tile: (npRows + 1) * (Lp + 8)
-    int32_t npRows;             // H rows = (mask, island) pairs per tile
-    int32_t srcRows;            // source rows of level r-1 staged per tile
-    int32_t srcWords;           // words of shared memory for the source rows
     int32_t csWords;            // words of shared memory available for staged cost tables
+    int32_t wbufWords;          // words of warp-private shared memory: 2*Kmax rows of (Lp + 8)
+    int32_t nActiveWarps;       // warps per CTA that stream masks (all of them unless L is huge)
 };
 
 // binomials up to 16 choose r and popcount-class offsets into maskOf

@@ -1,8 +1,7 @@
 // Persistent cooperative solver: scheduler state machine, per-T popcount-wavefront DP
 // (SURVEY.md §8(a) steps 4-5), threshold-sweep reduction (step 6) and plan back-tracker (step 7).
 //
-// One launch per tg_solve_batch.  Grid = 2 CTAs of 256 threads per SM (cooperative launch, all
-// co-resident), so that one CTA's memory phase overlaps the other's arithmetic phase.
+// One launch per tg_solve_batch.  Grid = one CTA of 16 warps per SM (cooperative launch, all co-resident).
 // A scheduler round is: CTA 0 folds the previous round's results into the per-instance state
 // machines and plans the next list of (instance, T) DPs ("items"); grid barrier; the items are
 // executed; grid barrier.  Execution of a round's items:
@@ -13,29 +12,12 @@
 //        counter per slot), never by a grid barrier.
 // Level r = |R| reads only level r-1 (PAPER.md:250 (2): a stage is added in front of a memoised
 // suffix).  State g[a][S][k] is stored as G_r[rank(R)][slot(k)][a], R = S\{k}.
-//
-// One tile = up to 32 masks R of one level, processed by one CTA:
-//   phase 1  H[R][k][b] = min_{j in R} x[k][j] + G_{r-1}[R\{j}][j][b]      (transfer pre-minimum;
-//            every source row is read once, results stay in shared memory)
-//   phase 2  G_r[R][k][a] = min_{b>a, c<=T} c_k[a][b] + H[R][k][b]         (min-plus product against
-//            the thresholded, diagonal-major cost tables staged in shared memory; 4x4 register
-//            tiles, one add-min (VIADDMNMX) per relaxation, only admissible diagonals visited)
+// Inside a level every warp streams over its own range of masks R (see tgWarpLevel).
 #pragma once
 #include "tg_common.cuh"
 #include "tg_prep.cuh"
 
-#define TG_MAXG 64            // groups of 4 pairs per tile: <= 128/4 + 16
-
-#define TG_XM_WORDS 1536      // transfer sub-matrices of one tile: cnt * r * roundup4(nk) words
-
-struct TgTileMeta {
-    uint16_t tileMask[TG_MAX_NR];
-    uint8_t kList[TG_MAX_NR][TG_MAX_K];   // islands not in R, ascending
-    uint8_t jList[TG_MAX_NR][TG_MAX_K];   // islands in R, ascending
-    uint16_t grpPair[TG_MAXG][4];         // H rows of a group of 4 pairs with the same island
-    uint8_t grpK[TG_MAXG];
-    int nGroups, cnt, first;
-};
+#define TG_NW (TG_NT / 32)     // warps per CTA
 
 struct TgShared {
     // staged item
@@ -45,13 +27,12 @@ struct TgShared {
     uint32_t baseK[TG_MAX_K];
     int dmaxK[TG_MAX_K];
     uint8_t dmaxTile[TG_MAX_K][64];
-    uint32_t xS[TG_MAX_K][TG_MAX_K];
+    alignas(16) uint32_t xS[TG_MAX_K][TG_MAX_K];
     uint8_t isl[TG_MAX_K];
     uint16_t binom[17][17];
-    // tiles (double-buffered metadata: tile i+1 is prepared while tile i computes)
-    TgTileMeta meta[2];
-    alignas(16) uint32_t xm[TG_XM_WORDS];
-    alignas(8) unsigned long long mbar;
+    // per-warp streaming state
+    alignas(8) unsigned long long mbar[TG_NW][2];   // completion of the two source buffers
+    uint8_t kl[TG_NW][TG_MAX_K];                    // islands not in the current mask, ascending
     // scheduler / queue
     uint32_t warpSums[33];
     int iTmp[8];
@@ -122,7 +103,7 @@ __device__ __forceinline__ uint64_t tgLevelOff(uint64_t bufWords, int Ke, int Lp
 // multiple of 4 so that the min-plus loop needs no row predicate; uniform row stride Lp.
 // dmaxTile[k][t] = widest admissible diagonal of starts a = 4t..4t+3: bounds the phase-2 loop.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, const TgItem* itp, bool count) {
+__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t*, const TgItem* itp, bool count) {
     __syncthreads();
     unsigned nAdm = 0;   // admissible (a, b, k) cost entries with b <= L-1 seen by this thread
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
@@ -150,11 +131,6 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += uint32_t((sm.dmaxK[kc] + 3) & ~3) * uint32_t(Lp); }
         sm.useGlobalC = acc > uint32_t(ctx.csWords) ? 1 : 0;
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
-    }
-    // the all-INF dummy row of the H tile
-    {
-        const int HS = Lp + 8, np = ctx.npRows;
-        for (int w = tid; w < HS; w += TG_NT) Hs[np * HS + w] = TG_INFU;
     }
     __syncthreads();
     if (!sm.useGlobalC) {
@@ -233,19 +209,21 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
 }
 
 // ---------------------------------------------------------------------------------------------
-// Tiles of level r >= 1.  A tile = `cnt` consecutive masks R (colexicographic rank first..) of the
-// staged item; its pairs (R, k), k not in R, are rows of the H tile.  Per tile:
-//   meta    unrank the masks, list members (j) and non-members (k), group pairs by island
-//   issue   one bulk async copy (TMA, cp.async.bulk) per source row G_{r-1}[R\{j}][j][.] into
-//           shared memory, completion on an mbarrier; issued one tile ahead of its use
-//   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[R][j][b]
-//   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]
+// Levels r >= 1: one WARP per mask R, streaming over a contiguous range of masks (colexicographic
+// order, successor by Gosper's hack).  Nothing but the item's staged tables is shared between the
+// warps of a CTA, so a level needs no CTA barrier at all.  Per mask R (|R| = r, nk = Ke - r):
+//   issue   lane i < r: one bulk async copy (TMA, cp.async.bulk) of the source row
+//           G_{r-1}[R\{j_i}][j_i][.] into the warp's shared-memory buffer, completion on the warp's
+//           mbarrier; issued one mask ahead of its use (double buffer)
+//   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[j][b]       lane = (4 consecutive b) x (k group)
+//   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]    lane = (4 consecutive a) x (k group)
+// Warp-private shared memory: rows of HS = Lp + 8 words: [0, nk) the H rows (H[b] at index b-1,
+// INF-padded), then two source buffers of r rows each.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
 __device__ __forceinline__ void tgMbarInit(unsigned long long* bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tgSmemAddr(bar)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
 __device__ __forceinline__ void tgMbarExpect(unsigned long long* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tgSmemAddr(bar)), "r"(bytes) : "memory");
@@ -258,207 +236,195 @@ __device__ __forceinline__ void tgMbarWait(unsigned long long* bar, uint32_t par
                      : "=r"(ok) : "r"(a), "r"(parity) : "memory");
     }
 }
-__device__ __forceinline__ void tgBulkLoad(uint32_t* dstSmem, const uint32_t* srcGlobal, uint32_t bytes, unsigned long long* bar) {
+__device__ __forceinline__ void tgBulkLoad(uint32_t dstSmemAddr, const uint32_t* srcGlobal, uint32_t bytes, unsigned long long* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(tgSmemAddr(dstSmem)), "l"(srcGlobal), "r"(bytes), "r"(tgSmemAddr(bar)) : "memory");
+                 ::"r"(dstSmemAddr), "l"(srcGlobal), "r"(bytes), "r"(tgSmemAddr(bar)) : "memory");
 }
-
-// masks per tile at level r: bounded by the H rows (cnt*nk), the source rows (cnt*r) and the xm table
-__device__ __forceinline__ int tgNR(const TgSolveCtx& ctx, int Ke, int r) {
-    const int nk = Ke - r, nkp = (nk + 3) & ~3;
-    int nr = min(TG_MAX_NR, ctx.npRows / nk);
-    nr = min(nr, ctx.srcRows / r);
-    nr = min(nr, TG_XM_WORDS / (r * nkp));
-    return max(nr, 1);
-}
-__device__ __forceinline__ uint32_t tgTiles(const TgSolveCtx& ctx, int Ke, int r) {
-    return (uint32_t(tgBinom[Ke][r]) + tgNR(ctx, Ke, r) - 1) / tgNR(ctx, Ke, r);
-}
-
-__device__ void tgTileMeta(TgShared& sm, TgTileMeta& M, int Ke, int r, int first, int cnt) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5, nk = Ke - r;
-    if (tid < cnt) {   // unrank: colexicographic rank -> mask (masks of one popcount ordered by value)
-        uint32_t rank = uint32_t(first + tid), R = 0;
-        int e = Ke - 1;
-        for (int i = r; i >= 1; --i) {
-            while (uint32_t(sm.binom[e][i]) > rank) --e;
-            rank -= sm.binom[e][i];
-            R |= 1u << e;
-            --e;
-        }
-        M.tileMask[tid] = uint16_t(R);
-    }
-    if (tid == 0) { M.cnt = cnt; M.first = first; }
-    __syncthreads();
-    for (int w = tid; w < cnt * Ke; w += TG_NT) {
-        const int rl = w / Ke, e = w - rl * Ke;
-        const uint32_t R = M.tileMask[rl];
-        const int below = __popc(R & ((1u << e) - 1u));
-        if (R >> e & 1u) M.jList[rl][below] = uint8_t(e);
-        else M.kList[rl][e - below] = uint8_t(e);
-    }
-    if (warp == nWarps - 1) {   // groups of 4 (mask, k) pairs sharing the island k
-        const uint32_t R = lane < cnt ? uint32_t(M.tileMask[lane]) : 0xffffffffu;
-        int gbase = 0;
-        for (int k = 0; k < Ke; ++k) {
-            const bool ex = !(R >> k & 1u);
-            const uint32_t bal = __ballot_sync(0xffffffffu, ex);
-            const int n = __popc(bal), ng = (n + 3) >> 2;
-            if (ex) {
-                const int rk = __popc(bal & ((1u << lane) - 1u));
-                M.grpPair[gbase + (rk >> 2)][rk & 3] = uint16_t(lane * nk + (k - __popc(R & ((1u << k) - 1u))));
-            }
-            if (lane < ng) M.grpK[gbase + lane] = uint8_t(k);
-            if (lane < ((4 - (n & 3)) & 3)) M.grpPair[gbase + ng - 1][3 - lane] = 0xffffu;  // pad the last group
-            gbase += ng;
-        }
-        if (lane == 0) M.nGroups = gbase;
-    }
-}
-
-// Issue the source-row copies of a tile and fill its transfer sub-matrices xm[(rl, ji)][s].
-__device__ void tgTileIssue(TgShared& sm, const TgTileMeta& M, uint32_t* src, const uint32_t* Gprev, int Ke, int r) {
-    const int tid = threadIdx.x, nk = Ke - r, nkp = (nk + 3) & ~3, Lp = sm.sLp, cnt = M.cnt;
-#ifndef TG_GENERIC_COPY
-    if (tid == 0) tgMbarExpect(&sm.mbar, uint32_t(cnt * r * Lp * 4));
-#endif
-    bool fenced = false;
-    for (int w = tid; w < cnt * r; w += TG_NT) {
-        const int rl = w / r, ji = w - rl * r;
-        uint32_t R = M.tileMask[rl];
-        // rank of R \ {e_ji}: elements before keep their position, elements after move down by one
-        uint32_t rank = 0;
-        int ej = 0;
-        for (int i = 0; i < r; ++i) {
-            const int e = __ffs(R) - 1;
-            R &= R - 1;
-            if (i < ji) rank += sm.binom[e][i + 1];
-            else if (i > ji) rank += sm.binom[e][i];
-            else ej = e;
-        }
-        const uint32_t row = rank * uint32_t(nk + 1) + uint32_t(ej - ji);
-        if (!fenced) { asm volatile("fence.proxy.async.global;" ::: "memory"); fenced = true; }
-#ifndef TG_GENERIC_COPY
-        tgBulkLoad(src + size_t(w) * Lp, Gprev + size_t(row) * Lp, uint32_t(Lp * 4), &sm.mbar);
-#else
-        for (int q = 0; q < Lp; q += 4)
-            *reinterpret_cast<uint4*>(src + size_t(w) * Lp + q) = tgLdcg4(Gprev + size_t(row) * Lp + q);
-#endif
-        uint32_t* xr = sm.xm + w * nkp;
-        for (int s = 0; s < nkp; ++s) xr[s] = s < nk ? sm.xS[M.kList[rl][s]][ej] : TG_INFU;   // x[k][j]: k sends to j
-    }
-}
-
-// phase 1: thread = (mask, 4 consecutive b), all k not in R at once.  Hs[pair][i] = H[b = i+1].
-__device__ __forceinline__ void tgTilePhase1(TgShared& sm, const TgTileMeta& M, uint32_t* Hs, const uint32_t* src, int Ke, int r) {
-    const int tid = threadIdx.x, nk = Ke - r, nkp = (nk + 3) & ~3, Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, cnt = M.cnt;
-    for (int w = tid; w < cnt * nb4; w += TG_NT) {
-        const int rl = w / nb4, b4 = w - rl * nb4;
-        uint32_t acc[TG_MAX_K][4];
-#pragma unroll
-        for (int s = 0; s < TG_MAX_K; ++s) { acc[s][0] = acc[s][1] = acc[s][2] = acc[s][3] = TG_INFU; }
-        const bool hasNx = b4 + 1 < nb4;
-        const uint32_t* sp = src + size_t(rl * r) * Lp + 4 * b4;
-        const uint32_t* xp = sm.xm + (rl * r) * nkp;
-        for (int ji = 0; ji < r; ++ji) {
-            const uint4 g4 = *reinterpret_cast<const uint4*>(sp);
-            const uint32_t nx = hasNx ? sp[4] : TG_INFU;
-#pragma unroll
-            for (int s4 = 0; s4 < TG_MAX_K / 4; ++s4) {
-                if (4 * s4 < nk) {
-                    const uint4 xv = *reinterpret_cast<const uint4*>(xp + 4 * s4);
-                    const uint32_t xa[4] = {xv.x, xv.y, xv.z, xv.w};
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        acc[4 * s4 + u][0] = tgAddMin(xa[u], g4.y, acc[4 * s4 + u][0]);
-                        acc[4 * s4 + u][1] = tgAddMin(xa[u], g4.z, acc[4 * s4 + u][1]);
-                        acc[4 * s4 + u][2] = tgAddMin(xa[u], g4.w, acc[4 * s4 + u][2]);
-                        acc[4 * s4 + u][3] = tgAddMin(xa[u], nx, acc[4 * s4 + u][3]);
-                    }
-                }
-            }
-            sp += Lp;
-            xp += nkp;
-        }
-        uint32_t* hrow = Hs + size_t(rl * nk) * HS + 4 * b4;
-#pragma unroll
-        for (int s = 0; s < TG_MAX_K; ++s) {
-            if (s < nk) {
-                *reinterpret_cast<uint4*>(hrow + size_t(s) * HS) = make_uint4(acc[s][0], acc[s][1], acc[s][2], acc[s][3]);
-                if (b4 == nb4 - 1) {
-                    *reinterpret_cast<uint4*>(hrow + size_t(s) * HS + 4) = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
-                    *reinterpret_cast<uint4*>(hrow + size_t(s) * HS + 8) = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
-                }
-            }
-        }
-    }
-}
-
 __device__ __forceinline__ uint4 tgLds4(uint32_t addr) {
     uint4 v;
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ uint32_t tgLds1(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void tgSts4(uint32_t addr, uint4 v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 
-// One block of 4 diagonals d = d0+1..d0+4 for 4 pairs x 4 starts.  lo = H window [a0+d0, a0+d0+4),
-// hi = the next 4 values (loaded here); c rows at cAddr + e*cStride.  16 add-mins per diagonal.
-#define TG_P2_STEP(LO, HI)                                                                          \
-    {                                                                                               \
-        _Pragma("unroll") for (int i = 0; i < 4; ++i) {                                             \
-            const uint4 h = tgLds4(hAddr[i]);                                                       \
-            HI[i][0] = h.x; HI[i][1] = h.y; HI[i][2] = h.z; HI[i][3] = h.w;                         \
-            hAddr[i] += 16;                                                                         \
-        }                                                                                           \
-        _Pragma("unroll") for (int e = 0; e < 4; ++e) {                                             \
-            const uint4 c4 = tgLds4(cAddr + e * cStride);                                           \
-            const uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};                                        \
-            _Pragma("unroll") for (int ai = 0; ai < 4; ++ai)                                        \
-                _Pragma("unroll") for (int i = 0; i < 4; ++i)                                       \
-                    acc[ai][i] = tgAddMin(cv[ai], (ai + e < 4 ? LO[i][ai + e] : HI[i][ai + e - 4]), acc[ai][i]); \
-        }                                                                                           \
-        cAddr += 4 * cStride;                                                                       \
+// colexicographic unrank: rank -> mask with r bits among Ke (masks of one popcount ordered by value)
+__device__ __forceinline__ uint32_t tgUnrank(const TgShared& sm, uint32_t rank, int r, int Ke) {
+    uint32_t R = 0;
+    int e = Ke - 1;
+    for (int i = r; i >= 1; --i) {
+        while (uint32_t(sm.binom[e][i]) > rank) --e;
+        rank -= sm.binom[e][i];
+        R |= 1u << e;
+        --e;
+    }
+    return R;
+}
+// next mask with the same popcount (Gosper)
+__device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
+    const uint32_t c = R & (0u - R), t = R + c;
+    return (((R ^ t) >> 2) >> (__ffs(c) - 1)) | t;
+}
+
+// Issue the r source-row copies of mask R into the warp's buffer `buf` (lane i copies source i).
+__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int r, int nk, int Lp, uint32_t bufAddr,
+                                            uint32_t rowBytes, const uint32_t* Gprev, unsigned long long* bar, int lane) {
+    if (lane == 0) tgMbarExpect(bar, uint32_t(r) * uint32_t(Lp) * 4u);
+    __syncwarp();
+    if (lane < r) {
+        // rank of R \ {e_lane}: elements before keep their position, elements after move down by one
+        uint32_t Rb = R, rank = 0;
+        int ej = 0;
+        for (int i = 0; i < r; ++i) {
+            const int e = __ffs(Rb) - 1;
+            Rb &= Rb - 1;
+            if (i < lane) rank += sm.binom[e][i + 1];
+            else if (i > lane) rank += sm.binom[e][i];
+            else ej = e;
+        }
+        const uint32_t row = rank * uint32_t(nk + 1) + uint32_t(ej - lane);
+        tgBulkLoad(bufAddr + uint32_t(lane) * rowBytes, Gprev + size_t(row) * Lp, uint32_t(Lp) * 4u, bar);
+    }
+}
+
+#define TG_SPL 8   // k slots per lane handled together (accumulators: TG_SPL x 4)
+
+// One block of 4 diagonals d = 4q+1..4q+4 for one row and 4 starts: LO = H window [a0+4q, a0+4q+4),
+// HI = the next 4 values (loaded here).
+#define TG_P2_STEP(LO, HI)                                                                     \
+    {                                                                                          \
+        const uint4 h = tgLds4(hA);                                                            \
+        hA += 16;                                                                              \
+        HI[0] = h.x; HI[1] = h.y; HI[2] = h.z; HI[3] = h.w;                                    \
+        _Pragma("unroll") for (int e = 0; e < 4; ++e) {                                        \
+            uint4 c4;                                                                          \
+            if (GLOBALC) {                                                                     \
+                const int d = dq + 1 + e;                                                      \
+                c4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);                           \
+                if (d <= dm && c < ((L - d + 3) >> 2)) {                                       \
+                    c4 = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + c);        \
+                    const int amax = L - 1 - d;                                                \
+                    c4.x = (a0 + 0 <= amax && c4.x <= T) ? c4.x : TG_INFU;                     \
+                    c4.y = (a0 + 1 <= amax && c4.y <= T) ? c4.y : TG_INFU;                     \
+                    c4.z = (a0 + 2 <= amax && c4.z <= T) ? c4.z : TG_INFU;                     \
+                    c4.w = (a0 + 3 <= amax && c4.w <= T) ? c4.w : TG_INFU;                     \
+                }                                                                              \
+            } else {                                                                           \
+                c4 = tgLds4(cA + e * cStride);                                                 \
+            }                                                                                  \
+            const uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};                                   \
+            _Pragma("unroll") for (int ai = 0; ai < 4; ++ai)                                   \
+                out[ai] = tgAddMin(cv[ai], (ai + e < 4 ? LO[ai + e] : HI[ai + e - 4]), out[ai]); \
+        }                                                                                      \
+        cA += 4 * cStride;                                                                     \
+        dq += 4;                                                                               \
     }
 
-// phase 2: min-plus product with the thresholded cost tables.  A quarter-warp owns a group of 4 pairs
-// of one island; its 8 lanes walk the 4-start tiles a0 = 4t of the row.
-__device__ __forceinline__ void tgTilePhase2(const TgSolveCtx& ctx, TgShared& sm, const TgTileMeta& M, const uint32_t* Cs,
-                                             const uint32_t* Hs, uint32_t* Gcur, unsigned long long* key, int Ke, int r) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
+template <bool GLOBALC>
+__device__ __forceinline__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf,
+                                            const uint32_t* Gprev, uint32_t* Gcur, unsigned long long* key, int Ke, int r,
+                                            int gw, int GW, uint32_t& par) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int L = sm.sL, Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, nk = Ke - r;
     const uint32_t T = sm.sT;
-    const int nGroups = M.nGroups;
-    const int nGQ = (nGroups + 3) >> 2;
-    const uint32_t hsBase = tgSmemAddr(Hs), csBase = tgSmemAddr(Cs), cStride = uint32_t(Lp) * 4u;
-    uint32_t* const gBase = Gcur + size_t(M.first) * nk * Lp;
+    const int nMasks = sm.binom[Ke][r];
+    const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
+    if (lo >= hi) return;
+    const int chShift = nb4 <= 8 ? 3 : (nb4 <= 16 ? 4 : 5), CH = 1 << chShift, NG = 32 >> chShift;
+    const int c0 = lane & (CH - 1), g = lane >> chShift;
+    const uint32_t rowBytes = uint32_t(HS) * 4u, cStride = uint32_t(Lp) * 4u;
+    const uint32_t hAddr0 = tgSmemAddr(wbuf), csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
+    const uint32_t bufAddr[2] = {hAddr0 + uint32_t(nk) * rowBytes, hAddr0 + uint32_t(nk + r) * rowBytes};
+    unsigned long long* bars = &sm.mbar[warp][0];
+    uint8_t* kl = &sm.kl[warp][0];
+    const uint32_t keMask = (1u << Ke) - 1u;
     unsigned long long bestKey = TG_KEY_NONE;
-    for (int gq = warp; gq < nGQ; gq += nWarps) {
-        const int g = gq * 4 + (lane >> 3);
-        if (g >= nGroups) continue;
-        const int k = M.grpK[g];
-        int pr[4];
+
+    uint32_t R = tgUnrank(sm, uint32_t(lo), r, Ke);
+    asm volatile("fence.proxy.async.global;" ::: "memory");
+    tgIssueMask(sm, R, r, nk, Lp, bufAddr[0], rowBytes, Gprev, bars + 0, lane);
+    int b = 0;
+    for (int idx = lo; idx < hi; ++idx, b ^= 1) {
+        const uint32_t Rn = tgNextMask(R);
+        if (idx + 1 < hi) tgIssueMask(sm, Rn, r, nk, Lp, bufAddr[b ^ 1], rowBytes, Gprev, bars + (b ^ 1), lane);
+        const uint32_t comp = ~R & keMask;
+        if (lane < Ke && (comp >> lane & 1u)) kl[__popc(comp & ((1u << lane) - 1u))] = uint8_t(lane);
+        __syncwarp();
+        tgMbarWait(bars + b, (par >> b) & 1u);
+        par ^= 1u << b;
+
+        // ---- phase 1: transfer pre-minimum, H rows into the warp's shared memory ---------------
+        for (int sb = 0; sb * NG * TG_SPL < nk; ++sb) {
+            int slot[TG_SPL];
+            uint32_t xrow[TG_SPL];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) { const int p = M.grpPair[g][i]; pr[i] = p == 0xffff ? -1 : p; }
-        for (int t = lane & 7; t < nb4; t += 8) {
-            const int a0 = 4 * t;
-            uint32_t acc[4][4];
+            for (int i = 0; i < TG_SPL; ++i) {
+                slot[i] = g + NG * (sb * TG_SPL + i);
+                xrow[i] = xsBase + uint32_t(slot[i] < nk ? kl[slot[i]] : 0) * (TG_MAX_K * 4u);
+            }
+            for (int c = c0; c < nb4; c += CH) {
+                uint32_t acc[TG_SPL][4];
 #pragma unroll
-            for (int ai = 0; ai < 4; ++ai)
+                for (int i = 0; i < TG_SPL; ++i) { acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = TG_INFU; }
+                const bool hasNx = c + 1 < nb4;
+                uint32_t sA = bufAddr[b] + uint32_t(c) * 16u;
+                uint32_t Rb = R;
+                for (int ji = 0; ji < r; ++ji) {
+                    const uint32_t j4 = uint32_t(__ffs(Rb) - 1) * 4u;
+                    Rb &= Rb - 1;
+                    const uint4 g4 = tgLds4(sA);
+                    const uint32_t nx = hasNx ? tgLds1(sA + 16) : TG_INFU;
+                    sA += rowBytes;
 #pragma unroll
-                for (int i = 0; i < 4; ++i) acc[ai][i] = TG_INFU;
-            if (!sm.useGlobalC) {
-                const int nq = (int(sm.dmaxTile[k][t]) + 3) >> 2;
+                    for (int i = 0; i < TG_SPL; ++i) {
+                        if (slot[i] < nk) {
+                            const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
+                            acc[i][0] = tgAddMin(xv, g4.y, acc[i][0]);
+                            acc[i][1] = tgAddMin(xv, g4.z, acc[i][1]);
+                            acc[i][2] = tgAddMin(xv, g4.w, acc[i][2]);
+                            acc[i][3] = tgAddMin(xv, nx, acc[i][3]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int i = 0; i < TG_SPL; ++i) {
+                    if (slot[i] < nk) {
+                        const uint32_t hA = hAddr0 + uint32_t(slot[i]) * rowBytes + uint32_t(c) * 16u;
+                        tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));
+                        if (!hasNx) {
+                            tgSts4(hA + 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+                            tgSts4(hA + 32, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+                        }
+                    }
+                }
+            }
+        }
+        __syncwarp();
+
+        // ---- phase 2: min-plus product with the thresholded cost rows ----------------------------
+        uint32_t* const gRow = Gcur + size_t(idx) * nk * Lp;
+        for (int s = g; s < nk; s += NG) {
+            const int k = kl[s];
+            const uint32_t* cdk = GLOBALC ? I.cd + size_t(sm.isl[k]) * I.triG : nullptr;
+            for (int c = c0; c < nb4; c += CH) {
+                const int a0 = 4 * c, dm = sm.dmaxTile[k][c], nq = (dm + 3) >> 2;
+                uint32_t out[4] = {TG_INFU, TG_INFU, TG_INFU, TG_INFU};
                 if (nq > 0) {
-                    uint32_t hAddr[4];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) hAddr[i] = hsBase + uint32_t((pr[i] < 0 ? ctx.npRows : pr[i]) * HS + a0) * 4u;
-                    uint32_t cAddr = csBase + (sm.baseK[k] + uint32_t(a0)) * 4u;
-                    uint32_t Wa[4][4], Wb[4][4];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const uint4 h = tgLds4(hAddr[i]);
-                        Wa[i][0] = h.x; Wa[i][1] = h.y; Wa[i][2] = h.z; Wa[i][3] = h.w;
-                        hAddr[i] += 16;
+                    uint32_t hA = hAddr0 + uint32_t(s) * rowBytes + uint32_t(c) * 16u;
+                    uint32_t cA = csBase + (sm.baseK[k] + uint32_t(a0)) * 4u;
+                    int dq = 0;
+                    uint32_t Wa[4], Wb[4];
+                    {
+                        const uint4 h = tgLds4(hA);
+                        hA += 16;
+                        Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
                     }
 #pragma unroll 1
                     for (int q = 0; q < nq; q += 2) {
@@ -467,36 +433,15 @@ __device__ __forceinline__ void tgTilePhase2(const TgSolveCtx& ctx, TgShared& sm
                         TG_P2_STEP(Wb, Wa)
                     }
                 }
-            } else {
-                // cost tables too large for shared memory: read the reduced table from global (L2)
-                const uint32_t* cdk = I.cd + size_t(sm.isl[k]) * I.triG;
-                const int dm = sm.dmaxTile[k][t];
-                const uint32_t* hp[4];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) hp[i] = Hs + size_t(pr[i] < 0 ? ctx.npRows : pr[i]) * HS + a0;
-                for (int d = 1; d <= dm; ++d) {
-                    uint4 c4 = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d) + a0));
-                    const int amax = L - 1 - d;
-                    uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};
-#pragma unroll
-                    for (int ai = 0; ai < 4; ++ai) {
-                        if (a0 + ai > amax || cv[ai] > T) cv[ai] = TG_INFU;
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) acc[ai][i] = tgAddMin(cv[ai], hp[i][ai + d - 1], acc[ai][i]);
-                    }
-                }
-            }
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                if (pr[i] < 0) continue;
-                *reinterpret_cast<uint4*>(gBase + size_t(pr[i]) * Lp + a0) = make_uint4(acc[0][i], acc[1][i], acc[2][i], acc[3][i]);
-                if (t == 0 && acc[0][i] < TG_INFU) {
-                    const uint32_t S = uint32_t(M.tileMask[pr[i] / nk]) | (1u << k);
-                    const unsigned long long kk = (unsigned long long)acc[0][i] << 32 | (unsigned long long)S << 8 | (unsigned long long)k;
+                *reinterpret_cast<uint4*>(gRow + size_t(s) * Lp + a0) = make_uint4(out[0], out[1], out[2], out[3]);
+                if (c == 0 && out[0] < TG_INFU) {
+                    const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)(R | (1u << k)) << 8 | (unsigned long long)k;
                     bestKey = kk < bestKey ? kk : bestKey;
                 }
             }
         }
+        __syncwarp();
+        R = Rn;
     }
     // the rows just written are read by bulk async copies (async proxy) of the next level
     asm volatile("fence.proxy.async.global;" ::: "memory");
@@ -506,41 +451,6 @@ __device__ __forceinline__ void tgTilePhase2(const TgSolveCtx& ctx, TgShared& sm
             bestKey = ot < bestKey ? ot : bestKey;
         }
         if (lane == 0) atomicMin(key, bestKey);
-    }
-}
-
-// All tiles of level r that belong to this CTA (member, member + teamSize, ...), software-pipelined:
-// the source rows of tile i+1 are in flight while tile i runs its min-plus product.
-__device__ void tgRunLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* Hs, uint32_t* src,
-                           const uint32_t* Gprev, uint32_t* Gcur, unsigned long long* key, int Ke, int r, int member,
-                           int teamSize, uint32_t& parity) {
-    const int NR = tgNR(ctx, Ke, r), nMasks = tgBinom[Ke][r];
-    const int nT = (nMasks + NR - 1) / NR;
-    if (member >= nT) return;
-    tgTileMeta(sm, sm.meta[0], Ke, r, member * NR, min(NR, nMasks - member * NR));
-    __syncthreads();
-    tgTileIssue(sm, sm.meta[0], src, Gprev, Ke, r);
-    tgMark(sm, 1);
-    int i = 0;
-    for (int tile = member; tile < nT; tile += teamSize, ++i) {
-        TgTileMeta& cur = sm.meta[i & 1];
-        TgTileMeta& nxt = sm.meta[(i + 1) & 1];
-        const int tn = tile + teamSize;
-        const bool hasNext = tn < nT;
-        if (hasNext) tgTileMeta(sm, nxt, Ke, r, tn * NR, min(NR, nMasks - tn * NR));
-        else __syncthreads();   // xm of this tile was written by other threads (tgTileIssue)
-        tgMark(sm, 1);
-#ifndef TG_GENERIC_COPY
-        tgMbarWait(&sm.mbar, parity);
-        parity ^= 1u;
-#endif
-        tgTilePhase1(sm, cur, Hs, src, Ke, r);
-        __syncthreads();
-        tgMark(sm, 2);
-        if (hasNext) tgTileIssue(sm, nxt, src, Gprev, Ke, r);
-        tgTilePhase2(ctx, sm, cur, Cs, Hs, Gcur, key, Ke, r);
-        __syncthreads();
-        tgMark(sm, 3);
     }
 }
 
@@ -638,14 +548,15 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned l
 // ---------------------------------------------------------------------------------------------
 // One DP(T): all wavefront levels of one item by a team of `teamSize` CTAs (this CTA = `member`).
 // ---------------------------------------------------------------------------------------------
-__device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* Hs, uint32_t* src, const TgItem* itp,
-                          unsigned long long* key, int member, int teamSize, int slotIdx, uint32_t& parity) {
-    tgStageItem(ctx, sm, Cs, Hs, itp, member == 0);
+__device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* wbufAll, const TgItem* itp,
+                          unsigned long long* key, int member, int teamSize, int slotIdx, uint32_t& par) {
+    tgStageItem(ctx, sm, Cs, wbufAll, itp, member == 0);
     tgMark(sm, 0);
-    const int Ke = sm.sKe, Lp = sm.sLp;
+    const int Ke = sm.sKe, Lp = sm.sLp, nW = ctx.nActiveWarps, warp = threadIdx.x >> 5;
     const uint64_t bufWords = __ldcg(&itp->bufWords);
     uint32_t* slot = ctx.scratch + uint64_t(slotIdx) * ctx.slotWords;
     uint32_t* bar = ctx.slotBar + slotIdx;
+    uint32_t* wbuf = wbufAll + size_t(warp) * ctx.wbufWords;
     uint32_t arrivals = 0;
     if (Ke > 0) {
         tgLevel0(ctx, sm, slot, key, member == 0);
@@ -653,9 +564,13 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         for (int r = 1; r < Ke; ++r) {
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Lp, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Lp, r);
-            tgRunLevel(ctx, sm, Cs, Hs, src, Gprev, Gcur, key, Ke, r, member, teamSize, parity);
-            if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); tgMark(sm, 4); }
+            if (warp >= nW) {}
+            else if (sm.useGlobalC) tgWarpLevel<true>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, par);
+            else tgWarpLevel<false>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, par);
+            tgMark(sm, 3);
+            if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();
+            tgMark(sm, 4);
         }
     }
     tgMark(sm, 0);
@@ -685,12 +600,11 @@ __device__ __forceinline__ void tgFoldResult(TgInstDev& I, unsigned long long ke
     if (it < I.incIter || (it == I.incIter && tidx < I.incIdx)) { I.incIter = it; I.incIdx = tidx; }
 }
 
-// DPs per round an instance with K islands should run: enough that a team (grid / DPs) has about ten
-// tiles per member at the widest level, i.e. few members idle at the thin levels.
+// DPs per round an instance with K islands should run: enough that every warp of a team (grid / DPs)
+// has about eight masks at the widest level, i.e. few warps idle at the thin levels.
 __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
-    int widest = 1;
-    for (int r = 1; r < K; ++r) widest = max(widest, int(tgTiles(ctx, K, r)));
-    const int team = max(1, widest / 10);
+    const int widest = tgBinom[K][K >> 1];
+    const int team = max(1, widest / (8 * ctx.nActiveWarps));
     return min(max(int(gridDim.x) / team, 16), 64);
 }
 
@@ -866,19 +780,19 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
 // ---------------------------------------------------------------------------------------------
 extern __shared__ uint4 tgDynSmem[];
 
-__global__ void __launch_bounds__(TG_NT, 2) tgSolveKernel(const TgSolveCtx ctx) {
+__global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) {
     __shared__ TgShared sm;
     uint32_t* dyn = reinterpret_cast<uint32_t*>(tgDynSmem);
     uint32_t* Cs = dyn;
-    uint32_t* Hs = dyn + ctx.csWords;
-    uint32_t* src = Hs + ctx.hsWords;
-    uint32_t epoch = 0, parity = 0;
+    uint32_t* wbufAll = dyn + ctx.csWords;
+    uint32_t epoch = 0, mbPar = 0;
     TgCtrl* ctrl = ctx.ctrl;
     const int nCta = int(gridDim.x), b = int(blockIdx.x);
     if (threadIdx.x == 0) {
         for (int i = 0; i < 8; ++i) sm.cyc[i] = 0;
         sm.tmark = clock64();
-        tgMbarInit(&sm.mbar, 1);
+        for (int w = 0; w < TG_NW; ++w) { tgMbarInit(&sm.mbar[w][0], 1); tgMbarInit(&sm.mbar[w][1], 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int w = threadIdx.x; w < 17 * 17; w += TG_NT) sm.binom[w / 17][w % 17] = tgBinom[w / 17][w % 17];
     __syncthreads();
@@ -900,7 +814,7 @@ __global__ void __launch_bounds__(TG_NT, 2) tgSolveKernel(const TgSolveCtx ctx) 
                     __syncthreads();
                     const int it = sm.curItem;
                     if (it >= nItems) break;
-                    tgRunItem(ctx, sm, Cs, Hs, src, items + it, keys + it, 0, 1, b, parity);
+                    tgRunItem(ctx, sm, Cs, wbufAll, items + it, keys + it, 0, 1, b, mbPar);
                 }
             }
         } else {
@@ -909,7 +823,7 @@ __global__ void __launch_bounds__(TG_NT, 2) tgSolveKernel(const TgSolveCtx ctx) 
             while (t + 1 < nItems && int((int64_t(t + 1) * nCta) / nItems) <= b) ++t;
             while (t > 0 && int((int64_t(t) * nCta) / nItems) > b) --t;
             const int start = int((int64_t(t) * nCta) / nItems), end = int((int64_t(t + 1) * nCta) / nItems);
-            tgRunItem(ctx, sm, Cs, Hs, src, items + t, keys + t, b - start, end - start, t, parity);
+            tgRunItem(ctx, sm, Cs, wbufAll, items + t, keys + t, b - start, end - start, t, mbPar);
         }
         tgMark(sm, 0);
         tgGridBarrier(ctrl, epoch);
