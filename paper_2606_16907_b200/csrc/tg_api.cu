@@ -46,7 +46,7 @@ struct DeviceState {
 };
 std::mutex g_mu;
 // DPs per instance and scheduler round (speculation width of the threshold search / sweep)
-int g_wishMax = [] { const char* e = getenv("TG_WISH_MAX"); int v = e ? atoi(e) : 64; return v < 1 ? 1 : (v > 64 ? 64 : v); }();
+int g_wishMax = [] { const char* e = getenv("TG_WISH_MAX"); int v = e ? atoi(e) : 64; return v < 1 ? 1 : (v > TG_MAX_WISH ? TG_MAX_WISH : v); }();
 DeviceState g_dev[64];
 
 tg_status deviceInit(int dev, DeviceState** out) {
@@ -156,7 +156,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     Carver cv;
     const size_t oInst = cv.take(sizeof(TgInstDev) * n);
     std::vector<TgInstDev> h(n);
-    std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSuf(n);
+    std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
     int maxCells = 0, maxLp = 4, maxK = 1;
     uint64_t maxFull = 0;
     size_t denseCs = 0;
@@ -174,6 +174,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         I.sortCap = cap;
         for (int k = 0; k < TG_MAX_K; ++k) I.cminAll[k] = TG_INFU;
         I.phase = TG_PH_NEW;
+        I.incIdx = -1; I.hiFeas = -1; I.loInf = -1;
         uint64_t mx = 1;
         {   // widest wavefront and full table in rows
             uint64_t binom[17][17];
@@ -193,6 +194,9 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         oCand[i] = cv.take(size_t(cells) * 4);
         oSort[i] = cv.take(size_t(cap) * 4);
         oSuf[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
+        oSufA[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
+        oEI[i] = cv.take(size_t(TG_MAX_EVAL) * 4);
+        oEF[i] = cv.take(size_t(TG_MAX_EVAL) * 4);
     }
     const size_t oItems = cv.take(sizeof(TgItem) * 2 * TG_MAX_ITEMS);
     const size_t oKeys = cv.take(sizeof(unsigned long long) * 2 * TG_MAX_ITEMS);
@@ -220,6 +224,9 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         h[i].cand = reinterpret_cast<uint32_t*>(W.base + oCand[i]);
         h[i].sortbuf = reinterpret_cast<uint32_t*>(W.base + oSort[i]);
         h[i].sufMin = reinterpret_cast<uint32_t*>(W.base + oSuf[i]);
+        h[i].sufMinAll = reinterpret_cast<uint32_t*>(W.base + oSufA[i]);
+        h[i].eIdx = reinterpret_cast<int32_t*>(W.base + oEI[i]);
+        h[i].eF = reinterpret_cast<uint32_t*>(W.base + oEF[i]);
     }
     W.inst = reinterpret_cast<TgInstDev*>(W.base + oInst);
     W.outDev = reinterpret_cast<tg_result*>(W.base + oOut);

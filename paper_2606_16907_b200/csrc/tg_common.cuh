@@ -10,7 +10,9 @@
 #define TG_TINF 0x3fffffffu   // threshold standing for T = infinity: c <= TG_TINF  <=>  c finite
 #define TG_NT 512             // threads per CTA of the persistent solver (1 CTA per SM)
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
-#define TG_MAX_NR 32          // masks R per tile
+#define TG_MAX_EVAL 1024      // evaluated thresholds remembered per instance
+#define TG_MAX_WISH 64        // DPs per instance and round, upper bound
+#define TG_EDONE 0x40000000   // flag in eIdx: every candidate between the previous evaluated point and this one is resolved
 #define TG_KEY_NONE 0xffffffffffffffffull
 
 // Row geometry of the diagonal-major cost tables.  Diagonal d = b - a (1..L).
@@ -43,20 +45,25 @@ struct TgInstDev {
     uint32_t* cand;          // [nCandCap] ascending distinct finite c (first ncand valid)
     uint32_t* sortbuf;       // [sortCap] scratch of the candidate sort (power of two)
     uint32_t* sufMin;        // [K][L+2]: sufMin[k][d] = min over d' >= d, b <= L-1 of c  (d = 1..L)
+    uint32_t* sufMinAll;     // [K][L+2]: same over all slices (b <= L): longest admissible slice at T
+    int32_t* eIdx;           // [TG_MAX_EVAL] evaluated feasible candidates, ascending (bit 30: interval below resolved)
+    uint32_t* eF;            // [TG_MAX_EVAL] their f_T
     int32_t L, K, P, m, act_mb, NS, Lp, triG;
     int32_t sortCap, ncand;
     uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
     uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major
     // ---- solver state (one scheduler thread per instance) ----
-    int32_t phase, lo, hi, next;
-    int32_t itemBeg, itemCnt, probeCnt, nrun;
-    uint32_t fInf;
-    int32_t incIdx;
+    int32_t phase, loInf, hiFeas, next;   // FEAS bracket: largest infeasible / smallest feasible candidate
+    int32_t itemBeg, itemCnt, gstep, nrun;
+    int32_t lbIdx;                        // first candidate passing the necessary condition sum_k maxlen_k(T) >= L
+    int32_t incIdx;                       // incumbent = lexicographic min of (iter, candidate index); -1 = none
     int64_t incIter;
+    int32_t nEval, nProbe;
+    int32_t probe[TG_MAX_WISH];           // candidates to evaluate this round, ascending
     uint64_t fullWords;  // scratch words of a full-table DP of this instance (K islands alive)
 };
 
-enum { TG_PH_NEW = 0, TG_PH_INIT = 1, TG_PH_SEARCH = 2, TG_PH_SWEEP = 3, TG_PH_FINAL = 4, TG_PH_DONE = 5 };
+enum { TG_PH_NEW = 0, TG_PH_FEAS = 1, TG_PH_BNB = 2, TG_PH_SWEEP = 3, TG_PH_FINAL = 4, TG_PH_DONE = 5 };
 
 // One (instance, T) DP of a scheduler round.
 struct TgItem {

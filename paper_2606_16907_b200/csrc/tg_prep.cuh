@@ -160,20 +160,25 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     }
     // row minima (b <= L-1 only) then suffix minima over the diagonal index
     uint32_t* sm = I.sufMin;
+    uint32_t* sma = I.sufMinAll;
     const int stride = L + 2;
     for (int w = tid; w < K * (L + 2); w += TG_PREP_NT) {
         const int k = w / stride, d = w - k * stride;
-        uint32_t mn = TG_INFU;
-        if (d >= 1 && d <= L - 1) {
+        uint32_t mn = TG_INFU, mnAll = TG_INFU;
+        if (d >= 1 && d <= L) {
             const uint32_t* row = I.cd + size_t(k) * I.triG + tgGOff(L, d);
             for (int a = 0; a <= L - 1 - d; ++a) mn = min(mn, row[a]);
+            mnAll = min(mn, row[L - d]);
         }
         sm[w] = mn;
+        sma[w] = mnAll;
     }
     __syncthreads();
-    if (tid < K) {
+    if (tid < 2 * K) {
+        uint32_t* s2 = tid < K ? sm : sma;
+        const int k = tid < K ? tid : tid - K;
         uint32_t run = TG_INFU;
-        for (int d = L + 1; d >= 0; --d) { run = min(run, sm[tid * stride + d]); sm[tid * stride + d] = run; }
+        for (int d = L + 1; d >= 0; --d) { run = min(run, s2[k * stride + d]); s2[k * stride + d] = run; }
     }
     // candidate sort
     const int n = I.NS * K, N = I.sortCap;
@@ -206,6 +211,31 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
         base += tot;
     }
     if (tid == 0) I.ncand = int(base);
+    __syncthreads();
+    // Necessary condition for feasibility at T: the longest admissible slices of the islands must add
+    // up to at least L layers.  lbIdx = first candidate that passes (ncand if none): the threshold
+    // search starts there.
+    if (tid < 32) {
+        const int nc = int(base);
+        int lo = 0, hi = nc;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const uint32_t T = I.cand[mid];
+            int len = 0;
+            if (tid < K) {
+                const uint32_t* sf = sma + tid * stride;
+                int l2 = 0, h2 = L;
+                while (l2 < h2) {
+                    const int m2 = (l2 + h2 + 1) >> 1;
+                    if (sf[m2] <= T) l2 = m2; else h2 = m2 - 1;
+                }
+                len = l2;
+            }
+            for (int o = 16; o > 0; o >>= 1) len += __shfl_xor_sync(0xffffffffu, len, o);
+            if (len >= L) hi = mid; else lo = mid + 1;
+        }
+        if (tid == 0) I.lbIdx = lo;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -579,33 +579,164 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     tgMark(sm, 7);
 }
 
-// ---------------------------------------------------------------------------------------------
-// Scheduler (CTA 0): fold results of the previous round, plan the next one.
-//   NEW -> INIT   : DP at T = infinity gives f_inf, the lower bound of the stop rule
-//   SEARCH        : multi-section search for the lowest feasible candidate (feasibility is monotone)
-//   SWEEP         : ascending candidates while  (f_inf + (m-1)T, idx) < (incumbent iter, its idx)
-//   FINAL         : DP at T* keeping every level, followed by the back-track
-// The incumbent is the lexicographic minimum of (iter, candidate index) over every DP evaluated,
-// which equals the oracle's ascending sweep with strict improvement (lowest T wins ties).
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool tgMustEval(const TgInstDev& I, int idx, bool full) {
-    if (full) return true;
-    const int64_t lb = int64_t(I.fInf) + int64_t(I.m - 1) * int64_t(I.cand[idx]);
-    return lb < I.incIter || (lb == I.incIter && idx < I.incIdx);
-}
-
-__device__ __forceinline__ void tgFoldResult(TgInstDev& I, unsigned long long key, int tidx) {
-    if (key == TG_KEY_NONE) return;
-    const int64_t it = int64_t(key >> 32) + int64_t(I.m - 1) * int64_t(I.cand[tidx]);
-    if (it < I.incIter || (it == I.incIter && tidx < I.incIdx)) { I.incIter = it; I.incIdx = tidx; }
-}
-
 // DPs per round an instance with K islands should run: enough that every warp of a team (grid / DPs)
 // has about eight masks at the widest level, i.e. few warps idle at the thin levels.
 __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
     const int widest = tgBinom[K][K >> 1];
     const int team = max(1, widest / (8 * ctx.nActiveWarps));
     return min(max(int(gridDim.x) / team, 16), 64);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Scheduler (CTA 0): fold results of the previous round, plan the next one.  Exact search over the
+// candidate thresholds cand[0..n) (reading R-search); f_T = best sum at T is
+// non-increasing in T and feasibility is monotone in T:
+//   FEAS   find the lowest feasible candidate: galloping from the necessary-condition index
+//          lbIdx, then multi-section inside the bracket (loInf, hiFeas]
+//   BNB    branch and bound over the remaining candidates: for c between two evaluated points
+//          i < c < j,  iter_c >= f_j + (m-1) T_c  (f_c >= f_j); above the last evaluated point
+//          iter_c >= (m-1) T_c.  A candidate is dropped when its bound cannot beat the incumbent
+//          = lexicographic min of (iter, candidate index) over every DP evaluated, which is what
+//          the full ascending sweep with strict improvement returns (lowest T wins ties).
+//          Unresolved stretches are probed at evenly spaced points that include their right end.
+//   SWEEP  (TG_SOLVE_FULL_SWEEP) every candidate in ascending order
+//   FINAL  DP at T* keeping every level, followed by the back-track
+// ---------------------------------------------------------------------------------------------
+// could candidate c, whose sum is at least lbF, still beat the incumbent?
+__device__ __forceinline__ bool tgBeats(const TgInstDev& I, int64_t lbF, int c) {
+    if (I.incIdx < 0) return true;
+    const int64_t lb = lbF + int64_t(I.m - 1) * int64_t(I.cand[c]);
+    return lb < I.incIter || (lb == I.incIter && c < I.incIdx);
+}
+
+// last c in [lo, hi] with tgBeats(lbF, c), given tgBeats(lbF, lo) (the predicate holds on a prefix)
+__device__ __forceinline__ int tgLastBeating(const TgInstDev& I, int64_t lbF, int lo, int hi) {
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (tgBeats(I, lbF, mid)) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+}
+
+__device__ void tgWriteInfeasible(const TgSolveCtx& ctx, TgInstDev& I, int i) {
+    tg_result z;
+    memset(&z, 0, sizeof(z));
+    z.iter_time_us = INT64_MAX;
+    z.n_thresholds_run = uint32_t(I.nrun);
+    ctx.out[i] = z;
+    I.phase = TG_PH_DONE;
+}
+
+// Fold the results of instance i's items of the previous round (ascending candidate index).
+__device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem* itemsPrev, const unsigned long long* keysPrev,
+                               bool full) {
+    const int beg = I.itemBeg, cnt = I.itemCnt;
+    I.itemCnt = 0;
+    if (I.phase == TG_PH_FINAL) { I.phase = TG_PH_DONE; return; }   // result written by the back-tracker
+    int nf = 0;
+    for (int q = 0; q < cnt; ++q) {
+        const int tidx = __ldcg(&itemsPrev[beg + q].tidx);
+        const unsigned long long key = __ldcg(keysPrev + beg + q);
+        if (key == TG_KEY_NONE) { I.loInf = max(I.loInf, tidx); continue; }
+        ++nf;
+        I.hiFeas = I.hiFeas < 0 ? tidx : min(I.hiFeas, tidx);
+        const int64_t it = int64_t(key >> 32) + int64_t(I.m - 1) * int64_t(I.cand[tidx]);
+        if (I.incIdx < 0 || it < I.incIter || (it == I.incIter && tidx < I.incIdx)) { I.incIter = it; I.incIdx = tidx; }
+    }
+    I.nrun += cnt;
+    if (I.phase == TG_PH_SWEEP) { I.next = __ldcg(&itemsPrev[beg + cnt - 1].tidx) + 1; return; }
+    if (full || nf == 0) return;
+    // merge the feasible results into the evaluated list (both ascending), from the back
+    if (I.nEval + nf > TG_MAX_EVAL) { atomicExch(&ctx.ctrl->errFlag, 3); return; }
+    int e = I.nEval - 1, w = I.nEval + nf - 1, q = cnt - 1;
+    while (q >= 0) {
+        const unsigned long long key = __ldcg(keysPrev + beg + q);
+        if (key == TG_KEY_NONE) { --q; continue; }
+        const int tidx = __ldcg(&itemsPrev[beg + q].tidx);
+        if (e >= 0 && (I.eIdx[e] & ~TG_EDONE) > tidx) { I.eIdx[w] = I.eIdx[e]; I.eF[w] = I.eF[e]; --e; --w; }
+        else { I.eIdx[w] = tidx; I.eF[w] = uint32_t(key >> 32); --w; --q; }
+    }
+    I.nEval += nf;
+}
+
+// Plan the probes of instance i for this round into I.probe[0..nProbe).  Returns the item kind.
+__device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W, bool full) {
+    const int n = I.ncand;
+    I.nProbe = 0;
+    if (I.phase == TG_PH_NEW) {
+        if (ctx.mode == 1) I.phase = TG_PH_FINAL;
+        else if (n == 0 || I.lbIdx >= n) { tgWriteInfeasible(ctx, I, i); return TG_PH_DONE; }
+        else if (full) { I.phase = TG_PH_SWEEP; I.next = 0; }
+        else { I.phase = TG_PH_FEAS; I.loInf = I.lbIdx - 1; I.hiFeas = -1; I.gstep = 1; }
+    }
+    if (I.phase == TG_PH_FEAS) {
+        if (I.hiFeas < 0) {
+            if (I.loInf >= n - 1) { tgWriteInfeasible(ctx, I, i); return TG_PH_DONE; }
+            // galloping: loInf + gstep, + 2 gstep, ... ; at most 8 probes a round, the step keeps doubling
+            int step = I.gstep;
+            const int nmax = min(W, 8);
+            while (I.nProbe < nmax) {
+                const int c = min(int64_t(n - 1), int64_t(I.loInf) + step);
+                I.probe[I.nProbe++] = c;
+                if (c == n - 1) break;
+                step = step < (1 << 28) ? step * 2 : step;
+            }
+            I.gstep = step;
+            return TG_PH_FEAS;
+        }
+        const int span = I.hiFeas - I.loInf - 1;   // undecided candidates strictly inside the bracket
+        if (span > 0) {
+            if (span <= W) for (int q = 0; q < span; ++q) I.probe[I.nProbe++] = I.loInf + 1 + q;
+            else for (int q = 0; q < W; ++q) I.probe[I.nProbe++] = I.loInf + int((int64_t(q + 1) * (span + 1)) / (W + 1));
+            return TG_PH_FEAS;
+        }
+        I.phase = TG_PH_BNB;   // hiFeas is the lowest feasible candidate
+    }
+    if (I.phase == TG_PH_BNB) {
+        // unresolved stretches (left end exclusive, right end inclusive), at most 16 a round
+        int sLo[16], sHi[16], ns = 0;
+        long long total = 0;
+        for (int t = 1; t < I.nEval && ns < 15; ++t) {
+            const int ej = I.eIdx[t];
+            if (ej & TG_EDONE) continue;
+            const int a = I.eIdx[t - 1] & ~TG_EDONE;
+            if (ej - a <= 1 || !tgBeats(I, int64_t(I.eF[t]), a + 1)) { I.eIdx[t] = ej | TG_EDONE; continue; }
+            sLo[ns] = a; sHi[ns] = tgLastBeating(I, int64_t(I.eF[t]), a + 1, ej - 1);
+            total += sHi[ns] - sLo[ns];
+            ++ns;
+        }
+        {   // above the last evaluated point only the trivial bound f >= 0 is known
+            const int a = I.eIdx[I.nEval - 1] & ~TG_EDONE;
+            if (a < n - 1 && tgBeats(I, 0, a + 1)) {
+                sLo[ns] = a; sHi[ns] = tgLastBeating(I, 0, a + 1, n - 1);
+                total += sHi[ns] - sLo[ns];
+                ++ns;
+            }
+        }
+        if (ns == 0) I.phase = TG_PH_FINAL;
+        else {
+            int budget = W;
+            for (int s = 0; s < ns && budget > 0; ++s) {
+                const int size = sHi[s] - sLo[s];
+                int share = int(max(1ll, (long long)W * size / total));
+                share = min(min(share, size), budget);
+                for (int q = 1; q <= share; ++q) I.probe[I.nProbe++] = sLo[s] + int(((long long)q * size + share - 1) / share);
+                budget -= share;
+            }
+            return TG_PH_BNB;
+        }
+    }
+    if (I.phase == TG_PH_SWEEP) {
+        if (I.next >= n) {
+            if (I.incIdx < 0) { tgWriteInfeasible(ctx, I, i); return TG_PH_DONE; }
+            I.phase = TG_PH_FINAL;
+        } else {
+            for (int q = 0; q < W && I.next + q < n; ++q) I.probe[I.nProbe++] = I.next + q;
+            return TG_PH_SWEEP;
+        }
+    }
+    if (I.phase == TG_PH_FINAL) { I.probe[0] = ctx.mode == 1 ? -1 : I.incIdx; I.nProbe = 1; return TG_PH_FINAL; }
+    return TG_PH_DONE;
 }
 
 __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
@@ -626,55 +757,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     int nActive = 0;
     for (int i = tid; i < nInst; i += TG_NT) {
         TgInstDev& I = ctx.inst[i];
-        if (I.itemCnt > 0) {
-            const int beg = I.itemBeg, cnt = I.itemCnt;
-            if (I.phase == TG_PH_INIT) {
-                const unsigned long long key = __ldcg(keysPrev + beg);
-                I.nrun += 1;
-                if (key == TG_KEY_NONE) {
-                    tg_result z;
-                    memset(&z, 0, sizeof(z));
-                    z.iter_time_us = INT64_MAX;
-                    z.n_thresholds_run = uint32_t(I.nrun);
-                    ctx.out[i] = z;
-                    I.phase = TG_PH_DONE;
-                } else {
-                    I.fInf = uint32_t(key >> 32);
-                    const int n = I.ncand;
-                    I.incIdx = n - 1;
-                    I.incIter = int64_t(I.fInf) + int64_t(I.m - 1) * int64_t(I.cand[n - 1]);
-                    if (full) { I.phase = TG_PH_SWEEP; I.next = 0; }
-                    else if (n > 1) { I.phase = TG_PH_SEARCH; I.lo = 0; I.hi = n - 1; }
-                    else { I.phase = TG_PH_SWEEP; I.next = n; }  // single candidate: already seeded
-                }
-            } else if (I.phase == TG_PH_SEARCH) {
-                int lo = I.lo, hi = I.hi, prevIdx = -1;
-                bool found = false;
-                for (int q = 0; q < cnt; ++q) {
-                    const int tidx = __ldcg(&itemsPrev[beg + q].tidx);
-                    const unsigned long long key = __ldcg(keysPrev + beg + q);
-                    tgFoldResult(I, key, tidx);
-                    if (!found) {
-                        if (key != TG_KEY_NONE) { found = true; hi = tidx; if (prevIdx >= 0) lo = prevIdx + 1; }
-                        else prevIdx = tidx;
-                    }
-                }
-                if (!found) lo = prevIdx + 1;
-                I.lo = lo; I.hi = hi; I.nrun += cnt;
-                if (lo >= hi) { I.phase = TG_PH_SWEEP; I.next = hi + 1; }
-            } else if (I.phase == TG_PH_SWEEP) {
-                int last = I.next;
-                for (int q = 0; q < cnt; ++q) {
-                    const int tidx = __ldcg(&itemsPrev[beg + q].tidx);
-                    tgFoldResult(I, __ldcg(keysPrev + beg + q), tidx);
-                    last = tidx + 1;
-                }
-                I.next = last; I.nrun += cnt;
-            } else if (I.phase == TG_PH_FINAL) {
-                I.phase = TG_PH_DONE;  // result written by the back-tracker
-            }
-            I.itemCnt = 0;
-        }
+        if (I.itemCnt > 0) tgFoldInstance(ctx, I, itemsPrev, keysPrev, full);
         if (I.phase != TG_PH_DONE) ++nActive;
     }
     if (nActive) atomicAdd(&sm.iTmp[0], nActive);
@@ -685,49 +768,31 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
         return;
     }
 
-    // ---- B: how many DPs each instance may run this round -------------------------------------------
+    // ---- B: plan every instance's probes, lay the items out ------------------------------------------
     const int capAll = max(1, min(ctx.wishMax, TG_MAX_ITEMS / nActive));
     uint32_t carry = 0;
     for (int base = 0; base < nInst; base += TG_NT) {
         const int i = base + tid;
-        int cnt = 0, kind = 0, first = 0, probes = 0, span = 0;
-        if (i < nInst) {
+        int cnt = 0, kind = TG_PH_DONE;
+        if (i < nInst && ctx.inst[i].phase != TG_PH_DONE) {
             TgInstDev& I = ctx.inst[i];
-            if (I.phase == TG_PH_NEW || I.phase == TG_PH_INIT) I.phase = ctx.mode == 1 ? TG_PH_FINAL : TG_PH_INIT;
-            if (I.phase == TG_PH_SWEEP && !(I.next < I.ncand && tgMustEval(I, I.next, full))) I.phase = TG_PH_FINAL;
-            kind = I.phase;
-            const int capPerInst = min(capAll, tgWish(ctx, I.K));
-            if (I.phase == TG_PH_INIT || I.phase == TG_PH_FINAL) cnt = 1;
-            else if (I.phase == TG_PH_SEARCH) {
-                span = I.hi - I.lo;
-                probes = min(capPerInst, span);
-                cnt = probes; first = I.lo;
-            } else if (I.phase == TG_PH_SWEEP) {
-                first = I.next;
-                int idx = first;
-                while (cnt < capPerInst && idx < I.ncand && tgMustEval(I, idx, full)) { ++cnt; ++idx; }
-            }
+            kind = tgPlanInstance(ctx, I, i, min(capAll, tgWish(ctx, I.K)), full);
+            cnt = I.nProbe;
         }
         uint32_t tot;
         const uint32_t pos = tgBlockExScan(uint32_t(cnt), sm.warpSums, tot) + carry;
         carry += tot;
-        if (i < nInst && cnt > 0) {
+        if (cnt > 0) {
             TgInstDev& I = ctx.inst[i];
-            if (pos + cnt > TG_MAX_ITEMS) cnt = 0;
+            if (pos + cnt > TG_MAX_ITEMS) cnt = 0;   // cannot happen: cnt <= capAll <= TG_MAX_ITEMS / nActive
             I.itemBeg = int(pos); I.itemCnt = cnt;
             if (cnt > 0) atomicMax(&sm.iTmp[1], int(pos) + cnt);
             for (int q = 0; q < cnt; ++q) {
                 TgItem& it = items[pos + q];
                 it.inst = i;
-                if (kind == TG_PH_INIT) { it.tidx = -1; it.T = TG_TINF; it.flags = 0; }
-                else if (kind == TG_PH_FINAL) {
-                    if (ctx.mode == 1) { it.tidx = -1; it.T = ctx.dpT; }
-                    else { it.tidx = I.incIdx; it.T = I.cand[I.incIdx]; }
-                    it.flags = 1;
-                } else if (kind == TG_PH_SEARCH) {
-                    it.tidx = first + int((int64_t(q + 1) * span) / (probes + 1));
-                    it.T = I.cand[it.tidx]; it.flags = 0;
-                } else { it.tidx = first + q; it.T = I.cand[it.tidx]; it.flags = 0; }
+                it.tidx = I.probe[q];
+                it.T = it.tidx >= 0 ? I.cand[it.tidx] : ctx.dpT;
+                it.flags = kind == TG_PH_FINAL ? 1 : 0;
             }
         }
     }
@@ -771,7 +836,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
         ctrl->stats.plans_dense += sm.llTmp[0];
         ctrl->stats.states_live += sm.llTmp[1];
         ctrl->stats.n_rounds += 1;
-        if (nIt == 0) { ctrl->errFlag = 1; ctrl->done = 1; }
+        if (nIt == 0) ctrl->done = 1;   // every remaining instance was found infeasible while planning
     }
 }
 
