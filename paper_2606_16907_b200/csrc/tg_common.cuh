@@ -58,6 +58,7 @@ struct TgInstDev {
     int32_t lbIdx;                        // first candidate passing the necessary condition sum_k maxlen_k(T) >= L
     int32_t incIdx;                       // incumbent = lexicographic min of (iter, candidate index); -1 = none
     int64_t incIter;
+    uint32_t incMask;                     // island mask (original labels) of the incumbent's best state
     int32_t nEval, nProbe;
     int32_t probe[TG_MAX_WISH];           // candidates to evaluate this round, ascending
     uint64_t fullWords;  // scratch words of a full-table DP of this instance (K islands alive)

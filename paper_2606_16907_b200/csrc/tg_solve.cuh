@@ -272,24 +272,28 @@ __device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
     return (((R ^ t) >> 2) >> (__ffs(c) - 1)) | t;
 }
 
-// Issue the r source-row copies of mask R into the warp's buffer `buf` (lane i copies source i).
+// Issue the r source-row copies of mask R into the warp's buffer (the lane whose index is a member
+// j of R copies that source).  Source row of j = state (R\{j}, first island j) of level r-1, whose
+// mask rank is  sum_{i<p} C(e_i, i+1) + sum_{i>p} C(e_i, i)  (p = position of j in R: the elements
+// below keep their position, those above move down by one) -- two warp scans over the member lanes.
 __device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int r, int nk, int Lp, uint32_t bufAddr,
                                             uint32_t rowBytes, const uint32_t* Gprev, unsigned long long* bar, int lane) {
     if (lane == 0) tgMbarExpect(bar, uint32_t(r) * uint32_t(Lp) * 4u);
-    __syncwarp();
-    if (lane < r) {
-        // rank of R \ {e_lane}: elements before keep their position, elements after move down by one
-        uint32_t Rb = R, rank = 0;
-        int ej = 0;
-        for (int i = 0; i < r; ++i) {
-            const int e = __ffs(Rb) - 1;
-            Rb &= Rb - 1;
-            if (i < lane) rank += sm.binom[e][i + 1];
-            else if (i > lane) rank += sm.binom[e][i];
-            else ej = e;
-        }
-        const uint32_t row = rank * uint32_t(nk + 1) + uint32_t(ej - lane);
-        tgBulkLoad(bufAddr + uint32_t(lane) * rowBytes, Gprev + size_t(row) * Lp, uint32_t(Lp) * 4u, bar);
+    const bool member = (R >> lane) & 1u;
+    const int p = __popc(R & ((1u << lane) - 1u));
+    uint32_t up = member ? uint32_t(sm.binom[lane & 15][p + 1]) : 0u;   // C(e, p+1): kept position
+    uint32_t dn = member ? uint32_t(sm.binom[lane & 15][p]) : 0u;       // C(e, p): moved down
+    uint32_t upIncl = up, dnIncl = dn;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        const uint32_t a = __shfl_up_sync(0xffffffffu, upIncl, o), c = __shfl_up_sync(0xffffffffu, dnIncl, o);
+        if ((lane & 15) >= o) { upIncl += a; dnIncl += c; }
+    }
+    const uint32_t dnTotal = __shfl_sync(0xffffffffu, dnIncl, 15);
+    if (member && lane < 16) {
+        const uint32_t rank = (upIncl - up) + (dnTotal - dnIncl);
+        const uint32_t row = rank * uint32_t(nk + 1) + uint32_t(lane - p);
+        tgBulkLoad(bufAddr + uint32_t(p) * rowBytes, Gprev + size_t(row) * Lp, uint32_t(Lp) * 4u, bar);
     }
 }
 
@@ -641,7 +645,13 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem
         ++nf;
         I.hiFeas = I.hiFeas < 0 ? tidx : min(I.hiFeas, tidx);
         const int64_t it = int64_t(key >> 32) + int64_t(I.m - 1) * int64_t(I.cand[tidx]);
-        if (I.incIdx < 0 || it < I.incIter || (it == I.incIter && tidx < I.incIdx)) { I.incIter = it; I.incIdx = tidx; }
+        if (I.incIdx < 0 || it < I.incIter || (it == I.incIter && tidx < I.incIdx)) {
+            I.incIter = it; I.incIdx = tidx;
+            const uint32_t Sc = uint32_t(key >> 8) & 0xffffu;   // compact labels of that item
+            uint32_t So = 0;
+            for (int e = 0; e < TG_MAX_K; ++e) if (Sc >> e & 1u) So |= 1u << __ldcg(&itemsPrev[beg + q].isl[e]);
+            I.incMask = So;
+        }
     }
     I.nrun += cnt;
     if (I.phase == TG_PH_SWEEP) { I.next = __ldcg(&itemsPrev[beg + cnt - 1].tidx) + 1; return; }
@@ -805,8 +815,11 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
         TgItem& it = items[idx];
         const TgInstDev& I = ctx.inst[it.inst];
         uint32_t alive = 0; int Ke = 0;
+        // the final DP only needs the islands of the optimal mask S*: S* is the lowest mask attaining
+        // the optimum at T*, so no subset of it ties, and the back-track never leaves its subsets
+        const uint32_t allow = ((it.flags & 1) && ctx.mode == 0) ? I.incMask : 0xffffu;
         for (int k = 0; k < I.K; ++k)
-            if (I.cminAll[k] <= it.T) { alive |= 1u << k; it.isl[Ke++] = uint8_t(k); }
+            if (I.cminAll[k] <= it.T && (allow >> k & 1u)) { alive |= 1u << k; it.isl[Ke++] = uint8_t(k); }
         for (int e = Ke; e < TG_MAX_K; ++e) it.isl[e] = 0;
         it.alive = uint16_t(alive); it.Ke = uint8_t(Ke);
         it.bufWords = 0;
