@@ -28,6 +28,7 @@ struct TgShared {
     int dmaxK[TG_MAX_K];
     uint8_t dmaxTile[TG_MAX_K][64];
     alignas(16) uint32_t xS[TG_MAX_K][TG_MAX_K];
+    alignas(16) uint32_t xInf[TG_MAX_K];            // all-INF transfer row for a lane's unused k slot
     uint8_t isl[TG_MAX_K];
     uint16_t binom[17][17];
     // per-warp streaming state
@@ -297,9 +298,60 @@ __device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int 
     }
 }
 
-#define TG_SPL 8   // k slots per lane handled together (accumulators: TG_SPL x 4)
+#define TG_SPL 8   // k slots per lane handled together in phase 1 (accumulators: TG_SPL x 4)
 
-// One block of 4 diagonals d = 4q+1..4q+4 for one row and 4 starts: LO = H window [a0+4q, a0+4q+4),
+// phase 1 for the NSL k slots  slot0, slot0+NG, ...  of this lane's island group and its b chunks:
+//   H[R][k][b] = min_{j in R} x[k][j] + src[j][b],  written to the warp's H rows.
+// All slots but the last are valid for every lane; an invalid last slot reads an all-INF x row.
+template <int NSL>
+__device__ __forceinline__ void tgPhase1(const TgShared& sm, uint32_t R, int r, int nk, int nb4, int c0, int CH, int NG,
+                                         int slot0, uint32_t srcAddr, uint32_t rowBytes, uint32_t hAddr0, const uint8_t* kl,
+                                         uint32_t xsBase, uint32_t xInfAddr) {
+    uint32_t xrow[NSL];
+#pragma unroll
+    for (int i = 0; i < NSL; ++i) {
+        const int s = slot0 + NG * i;
+        xrow[i] = (i + 1 < NSL || s < nk) ? xsBase + uint32_t(kl[s]) * (TG_MAX_K * 4u) : xInfAddr;
+    }
+    const bool lastValid = slot0 + NG * (NSL - 1) < nk;
+    for (int c = c0; c < nb4; c += CH) {
+        uint32_t acc[NSL][4];
+#pragma unroll
+        for (int i = 0; i < NSL; ++i) { acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = TG_INFU; }
+        const bool hasNx = c + 1 < nb4;
+        uint32_t sA = srcAddr + uint32_t(c) * 16u;
+        uint32_t Rb = R;
+#pragma unroll 2
+        for (int ji = 0; ji < r; ++ji) {
+            const uint32_t j4 = uint32_t(__ffs(Rb) - 1) * 4u;
+            Rb &= Rb - 1;
+            const uint4 g4 = tgLds4(sA);
+            const uint32_t nx = hasNx ? tgLds1(sA + 16) : TG_INFU;
+            sA += rowBytes;
+#pragma unroll
+            for (int i = 0; i < NSL; ++i) {
+                const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
+                acc[i][0] = tgAddMin(xv, g4.y, acc[i][0]);
+                acc[i][1] = tgAddMin(xv, g4.z, acc[i][1]);
+                acc[i][2] = tgAddMin(xv, g4.w, acc[i][2]);
+                acc[i][3] = tgAddMin(xv, nx, acc[i][3]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NSL; ++i) {
+            if (i + 1 < NSL || lastValid) {
+                const uint32_t hA = hAddr0 + uint32_t(slot0 + NG * i) * rowBytes + uint32_t(c) * 16u;
+                tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));
+                if (!hasNx) {
+                    tgSts4(hA + 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+                    tgSts4(hA + 32, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+                }
+            }
+        }
+    }
+}
+
+// One block of 4 diagonals d = dq+1..dq+4 for one row and 4 starts: LO = H window [a0+dq, a0+dq+4),
 // HI = the next 4 values (loaded here).
 #define TG_P2_STEP(LO, HI)                                                                     \
     {                                                                                          \
@@ -330,14 +382,53 @@ __device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int 
         dq += 4;                                                                               \
     }
 
+// phase 2 for this lane's rows (slots g, g+NG, ...) and a chunks of mask R:
+//   G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]
 template <bool GLOBALC>
-__device__ __forceinline__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf,
-                                            const uint32_t* Gprev, uint32_t* Gcur, unsigned long long* key, int Ke, int r,
-                                            int gw, int GW, uint32_t& par) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+__device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& sm, uint32_t R, int nk, int nb4, int c0, int CH,
+                                         int NG, int g, uint32_t hAddr0, uint32_t rowBytes, uint32_t csBase, uint32_t cStride,
+                                         const uint8_t* kl, uint32_t* gRow, unsigned long long& bestKey) {
     const TgInstDev& I = ctx.inst[sm.sInst];
-    const int L = sm.sL, Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, nk = Ke - r;
+    const int L = sm.sL, Lp = sm.sLp;
     const uint32_t T = sm.sT;
+    for (int s = g; s < nk; s += NG) {
+        const int k = kl[s];
+        const uint32_t* cdk = GLOBALC ? I.cd + size_t(sm.isl[k]) * I.triG : nullptr;
+        const uint32_t cBase = csBase + sm.baseK[k] * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes;
+        uint32_t* const gOut = gRow + size_t(s) * Lp;
+        for (int c = c0; c < nb4; c += CH) {
+            const int a0 = 4 * c, dm = sm.dmaxTile[k][c], nq = (dm + 3) >> 2;
+            uint32_t out[4] = {TG_INFU, TG_INFU, TG_INFU, TG_INFU};
+            if (nq > 0) {
+                uint32_t hA = hRow + uint32_t(c) * 16u;
+                uint32_t cA = cBase + uint32_t(c) * 16u;
+                int dq = 0;
+                uint32_t Wa[4], Wb[4];
+                {
+                    const uint4 h = tgLds4(hA);
+                    hA += 16;
+                    Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
+                }
+#pragma unroll 1
+                for (int q = 0; q < nq; q += 2) {
+                    TG_P2_STEP(Wa, Wb)
+                    if (q + 1 >= nq) break;
+                    TG_P2_STEP(Wb, Wa)
+                }
+            }
+            *reinterpret_cast<uint4*>(gOut + a0) = make_uint4(out[0], out[1], out[2], out[3]);
+            if (c == 0 && out[0] < TG_INFU) {
+                const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)(R | (1u << k)) << 8 | (unsigned long long)k;
+                bestKey = kk < bestKey ? kk : bestKey;
+            }
+        }
+    }
+}
+
+__device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
+                            uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW, uint32_t& par) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, nk = Ke - r;
     const int nMasks = sm.binom[Ke][r];
     const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
     if (lo >= hi) return;
@@ -345,10 +436,12 @@ __device__ __forceinline__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm,
     const int c0 = lane & (CH - 1), g = lane >> chShift;
     const uint32_t rowBytes = uint32_t(HS) * 4u, cStride = uint32_t(Lp) * 4u;
     const uint32_t hAddr0 = tgSmemAddr(wbuf), csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
+    const uint32_t xInfAddr = tgSmemAddr(&sm.xInf[0]);
     const uint32_t bufAddr[2] = {hAddr0 + uint32_t(nk) * rowBytes, hAddr0 + uint32_t(nk + r) * rowBytes};
     unsigned long long* bars = &sm.mbar[warp][0];
     uint8_t* kl = &sm.kl[warp][0];
     const uint32_t keMask = (1u << Ke) - 1u;
+    const bool globalC = sm.useGlobalC != 0;
     unsigned long long bestKey = TG_KEY_NONE;
 
     uint32_t R = tgUnrank(sm, uint32_t(lo), r, Ke);
@@ -365,85 +458,21 @@ __device__ __forceinline__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm,
         par ^= 1u << b;
 
         // ---- phase 1: transfer pre-minimum, H rows into the warp's shared memory ---------------
-        for (int sb = 0; sb * NG * TG_SPL < nk; ++sb) {
-            int slot[TG_SPL];
-            uint32_t xrow[TG_SPL];
-#pragma unroll
-            for (int i = 0; i < TG_SPL; ++i) {
-                slot[i] = g + NG * (sb * TG_SPL + i);
-                xrow[i] = xsBase + uint32_t(slot[i] < nk ? kl[slot[i]] : 0) * (TG_MAX_K * 4u);
+        for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
+            const int nsl = min(TG_SPL, (nk - s0 + NG - 1) / NG);   // slots of the widest island group
+#define TG_P1_CASE(N) case N: tgPhase1<N>(sm, R, r, nk, nb4, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
+            switch (nsl) {
+                TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
+                TG_P1_CASE(5) TG_P1_CASE(6) TG_P1_CASE(7) TG_P1_CASE(8)
             }
-            for (int c = c0; c < nb4; c += CH) {
-                uint32_t acc[TG_SPL][4];
-#pragma unroll
-                for (int i = 0; i < TG_SPL; ++i) { acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = TG_INFU; }
-                const bool hasNx = c + 1 < nb4;
-                uint32_t sA = bufAddr[b] + uint32_t(c) * 16u;
-                uint32_t Rb = R;
-                for (int ji = 0; ji < r; ++ji) {
-                    const uint32_t j4 = uint32_t(__ffs(Rb) - 1) * 4u;
-                    Rb &= Rb - 1;
-                    const uint4 g4 = tgLds4(sA);
-                    const uint32_t nx = hasNx ? tgLds1(sA + 16) : TG_INFU;
-                    sA += rowBytes;
-#pragma unroll
-                    for (int i = 0; i < TG_SPL; ++i) {
-                        if (slot[i] < nk) {
-                            const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
-                            acc[i][0] = tgAddMin(xv, g4.y, acc[i][0]);
-                            acc[i][1] = tgAddMin(xv, g4.z, acc[i][1]);
-                            acc[i][2] = tgAddMin(xv, g4.w, acc[i][2]);
-                            acc[i][3] = tgAddMin(xv, nx, acc[i][3]);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int i = 0; i < TG_SPL; ++i) {
-                    if (slot[i] < nk) {
-                        const uint32_t hA = hAddr0 + uint32_t(slot[i]) * rowBytes + uint32_t(c) * 16u;
-                        tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));
-                        if (!hasNx) {
-                            tgSts4(hA + 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
-                            tgSts4(hA + 32, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
-                        }
-                    }
-                }
-            }
+#undef TG_P1_CASE
         }
         __syncwarp();
 
         // ---- phase 2: min-plus product with the thresholded cost rows ----------------------------
         uint32_t* const gRow = Gcur + size_t(idx) * nk * Lp;
-        for (int s = g; s < nk; s += NG) {
-            const int k = kl[s];
-            const uint32_t* cdk = GLOBALC ? I.cd + size_t(sm.isl[k]) * I.triG : nullptr;
-            for (int c = c0; c < nb4; c += CH) {
-                const int a0 = 4 * c, dm = sm.dmaxTile[k][c], nq = (dm + 3) >> 2;
-                uint32_t out[4] = {TG_INFU, TG_INFU, TG_INFU, TG_INFU};
-                if (nq > 0) {
-                    uint32_t hA = hAddr0 + uint32_t(s) * rowBytes + uint32_t(c) * 16u;
-                    uint32_t cA = csBase + (sm.baseK[k] + uint32_t(a0)) * 4u;
-                    int dq = 0;
-                    uint32_t Wa[4], Wb[4];
-                    {
-                        const uint4 h = tgLds4(hA);
-                        hA += 16;
-                        Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
-                    }
-#pragma unroll 1
-                    for (int q = 0; q < nq; q += 2) {
-                        TG_P2_STEP(Wa, Wb)
-                        if (q + 1 >= nq) break;
-                        TG_P2_STEP(Wb, Wa)
-                    }
-                }
-                *reinterpret_cast<uint4*>(gRow + size_t(s) * Lp + a0) = make_uint4(out[0], out[1], out[2], out[3]);
-                if (c == 0 && out[0] < TG_INFU) {
-                    const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)(R | (1u << k)) << 8 | (unsigned long long)k;
-                    bestKey = kk < bestKey ? kk : bestKey;
-                }
-            }
-        }
+        if (globalC) tgPhase2<true>(ctx, sm, R, nk, nb4, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+        else tgPhase2<false>(ctx, sm, R, nk, nb4, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
         __syncwarp();
         R = Rn;
     }
@@ -568,9 +597,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         for (int r = 1; r < Ke; ++r) {
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Lp, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Lp, r);
-            if (warp >= nW) {}
-            else if (sm.useGlobalC) tgWarpLevel<true>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, par);
-            else tgWarpLevel<false>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, par);
+            if (warp < nW) tgWarpLevel(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, par);
             tgMark(sm, 3);
             if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();
@@ -873,6 +900,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int w = threadIdx.x; w < 17 * 17; w += TG_NT) sm.binom[w / 17][w % 17] = tgBinom[w / 17][w % 17];
+    if (threadIdx.x < TG_MAX_K) sm.xInf[threadIdx.x] = TG_INFU;
     __syncthreads();
     for (int round = 0;; ++round) {
         const int par = round & 1;
