@@ -156,7 +156,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     Carver cv;
     const size_t oInst = cv.take(sizeof(TgInstDev) * n);
     std::vector<TgInstDev> h(n);
-    std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
+    std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSort2(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
     int maxCells = 0, maxLp = 4, maxK = 1;
     uint64_t maxFull = 0;
     size_t denseCs = 0;
@@ -192,7 +192,8 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         oCd[i] = cv.take(size_t(t.K) * I.triG * 4);
         oArgp[i] = cv.take(size_t(cells));
         oCand[i] = cv.take(size_t(cells) * 4);
-        oSort[i] = cv.take(size_t(cap) * 4);
+        oSort[i] = cv.take(size_t(cells) * 4);
+        oSort2[i] = cv.take(size_t(cells) * 4);
         oSuf[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
         oSufA[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
         oEI[i] = cv.take(size_t(TG_MAX_EVAL) * 4);
@@ -223,6 +224,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         h[i].argp = reinterpret_cast<uint8_t*>(W.base + oArgp[i]);
         h[i].cand = reinterpret_cast<uint32_t*>(W.base + oCand[i]);
         h[i].sortbuf = reinterpret_cast<uint32_t*>(W.base + oSort[i]);
+        h[i].sortbuf2 = reinterpret_cast<uint32_t*>(W.base + oSort2[i]);
         h[i].sufMin = reinterpret_cast<uint32_t*>(W.base + oSuf[i]);
         h[i].sufMinAll = reinterpret_cast<uint32_t*>(W.base + oSufA[i]);
         h[i].eIdx = reinterpret_cast<int32_t*>(W.base + oEI[i]);

@@ -43,7 +43,8 @@ struct TgInstDev {
     uint32_t* cd;            // [K][triG] diagonal-major reduced costs, TG_INFU = none
     uint8_t* argp;           // [NS][K] lowest p attaining c, 0xff = none
     uint32_t* cand;          // [nCandCap] ascending distinct finite c (first ncand valid)
-    uint32_t* sortbuf;       // [sortCap] scratch of the candidate sort (power of two)
+    uint32_t* sortbuf;       // [NS*K] reduced costs, flat: input of the candidate sort
+    uint32_t* sortbuf2;      // [NS*K] scratch of the candidate sort
     uint32_t* sufMin;        // [K][L+2]: sufMin[k][d] = min over d' >= d, b <= L-1 of c  (d = 1..L)
     uint32_t* sufMinAll;     // [K][L+2]: same over all slices (b <= L): longest admissible slice at T
     int32_t* eIdx;           // [TG_MAX_EVAL] evaluated feasible candidates, ascending (bit 30: interval below resolved)

@@ -139,8 +139,57 @@ __global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ inst
 // Sort: bitonic network on a power-of-two buffer, in shared memory when it fits, else in place in
 // global memory (L2 resident).
 // ---------------------------------------------------------------------------------------------
+// Stable LSD radix sort of A[0..n) (32-bit keys), 4 passes of 8 bits; B is scratch of the same size.
+// One CTA of TG_PREP_NT threads; hist = 32 warps x 256 digits in shared memory.  Returns A.
+__device__ uint32_t* tgRadixSort(uint32_t* A, uint32_t* B, int n, uint32_t* hist, uint32_t* warpSums) {
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, nW = blockDim.x >> 5;
+    const int chunk = (((n + nW - 1) / nW) + 31) & ~31;
+    const int beg = min(n, w * chunk), end = min(n, beg + chunk);
+    uint32_t* myHist = hist + w * 256;
+    uint32_t *src = A, *dst = B;
+    for (int pass = 0; pass < 4; ++pass) {
+        const int shift = 8 * pass;
+        for (int e = tid; e < nW * 256; e += blockDim.x) hist[e] = 0;
+        __syncthreads();
+        for (int b0 = beg; b0 < end; b0 += 32) {
+            const int i = b0 + lane;
+            const uint32_t d = i < end ? (__ldcg(src + i) >> shift) & 255u : 256u + uint32_t(lane);
+            const uint32_t peers = __match_any_sync(0xffffffffu, d);
+            if (d < 256u && lane == __ffs(peers) - 1) myHist[d] += __popc(peers);
+            __syncwarp();
+        }
+        __syncthreads();
+        {   // exclusive scan in (digit major, warp minor) order; each thread owns 8 consecutive entries
+            const int per = (nW * 256) / blockDim.x;   // 8 for 32 warps
+            uint32_t loc[8], sum = 0;
+            for (int q = 0; q < per; ++q) { const int e = tid * per + q; loc[q] = hist[(e % nW) * 256 + e / nW]; sum += loc[q]; }
+            uint32_t tot;
+            uint32_t run = tgBlockExScan(sum, warpSums, tot);
+            for (int q = 0; q < per; ++q) { const int e = tid * per + q; hist[(e % nW) * 256 + e / nW] = run; run += loc[q]; }
+        }
+        __syncthreads();
+        for (int b0 = beg; b0 < end; b0 += 32) {
+            const int i = b0 + lane;
+            const uint32_t v = i < end ? __ldcg(src + i) : 0u;
+            const uint32_t d = i < end ? (v >> shift) & 255u : 256u + uint32_t(lane);
+            const uint32_t peers = __match_any_sync(0xffffffffu, d);
+            uint32_t pos = 0;
+            if (d < 256u) pos = myHist[d] + __popc(peers & ((1u << lane) - 1u));
+            __syncwarp();
+            if (d < 256u) {
+                dst[pos] = v;
+                if (lane == __ffs(peers) - 1) myHist[d] += __popc(peers);
+            }
+            __syncwarp();
+        }
+        __syncthreads();
+        uint32_t* t = src; src = dst; dst = t;
+    }
+    return src;   // 4 passes: back in A
+}
+
 #define TG_PREP_NT 1024
-#define TG_SORT_SMEM_MAX 32768
+#define TG_SORT_SMEM_MAX 8192     // words of dynamic shared memory of the prepare kernel (radix histograms)
 
 __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restrict__ insts) {
     extern __shared__ uint32_t sbuf[];
@@ -180,31 +229,16 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
         uint32_t run = TG_INFU;
         for (int d = L + 1; d >= 0; --d) { run = min(run, s2[k * stride + d]); s2[k * stride + d] = run; }
     }
-    // candidate sort
-    const int n = I.NS * K, N = I.sortCap;
-    uint32_t* buf = (N <= TG_SORT_SMEM_MAX) ? sbuf : I.sortbuf;
-    if (N <= TG_SORT_SMEM_MAX) {
-        for (int i = tid; i < N; i += TG_PREP_NT) sbuf[i] = i < n ? I.sortbuf[i] : 0xffffffffu;
-    } else {
-        for (int i = n + tid; i < N; i += TG_PREP_NT) I.sortbuf[i] = 0xffffffffu;
-    }
-    __syncthreads();
-    for (int kk = 2; kk <= N; kk <<= 1)
-        for (int j = kk >> 1; j > 0; j >>= 1) {
-            for (int i = tid; i < (N >> 1); i += TG_PREP_NT) {
-                const int l = ((i & ~(j - 1)) << 1) | (i & (j - 1)), r = l + j;
-                const uint32_t va = buf[l], vb = buf[r];
-                const bool asc = (l & kk) == 0;
-                if ((va > vb) == asc) { buf[l] = vb; buf[r] = va; }
-            }
-            __syncthreads();
-        }
+    // candidate sort: stable LSD radix sort, 8-bit digits, ping-pong between the two global buffers
+    // (L2 resident); per-warp digit histograms in shared memory, warp w owns a contiguous chunk
+    const int n = I.NS * K;
+    uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, sbuf, warpSums);
     // unique, finite only
     uint32_t base = 0;
     for (int i0 = 0; i0 < n; i0 += TG_PREP_NT) {
         const int i = i0 + tid;
         uint32_t v = 0xffffffffu, f = 0;
-        if (i < n) { v = buf[i]; f = (v < TG_INFU && (i == 0 || buf[i - 1] != v)) ? 1u : 0u; }
+        if (i < n) { v = __ldcg(buf + i); f = (v < TG_INFU && (i == 0 || __ldcg(buf + i - 1) != v)) ? 1u : 0u; }
         uint32_t tot;
         const uint32_t pos = tgBlockExScan(f, warpSums, tot);
         if (f) I.cand[base + pos] = v;
