@@ -331,28 +331,29 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
     char* base = nullptr;
     Carver cv;
     const size_t oT = cv.take(nE * 4), oM = cv.take(nE * 4), oG = cv.take(K * 4), oC = cv.take(K * 4), oB = cv.take(K * K * 4), oE = cv.take(4);
-    TG_CUDA(cudaMalloc(reinterpret_cast<void**>(&base), cv.off));
+    // stream-ordered allocation on the legacy default stream (pool-cached: no device synchronisation)
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&base), cv.off, 0));
     tg_instance* t = new (std::nothrow) tg_instance();
-    if (!t) { cudaFree(base); return fail(TG_ERR_OOM, "host allocation failed"); }
+    if (!t) { cudaFreeAsync(base, 0); return fail(TG_ERR_OOM, "host allocation failed"); }
     t->L = L; t->K = K; t->P = P; t->m = m; t->act_mb = act_mb; t->NS = NS; t->device = dev;
     t->time_us = reinterpret_cast<int32_t*>(base + oT); t->mem_mb = reinterpret_cast<int32_t*>(base + oM);
     t->gpus = reinterpret_cast<int32_t*>(base + oG); t->cap_mb = reinterpret_cast<int32_t*>(base + oC);
     t->bw = reinterpret_cast<int32_t*>(base + oB);
     int* dErr = reinterpret_cast<int*>(base + oE);
-    cudaError_t e = cudaMemcpy(t->time_us, time_us, nE * 4, cudaMemcpyDefault);
-    if (e == cudaSuccess) e = cudaMemcpy(t->mem_mb, mem_mb, nE * 4, cudaMemcpyDefault);
-    if (e == cudaSuccess) e = cudaMemcpy(t->gpus, island_gpus, K * 4, cudaMemcpyDefault);
-    if (e == cudaSuccess) e = cudaMemcpy(t->cap_mb, island_cap_mb, K * 4, cudaMemcpyDefault);
-    if (e == cudaSuccess) e = cudaMemcpy(t->bw, bw_gbps, K * K * 4, cudaMemcpyDefault);
-    if (e == cudaSuccess) e = cudaMemset(dErr, 0, 4);
+    cudaError_t e = cudaMemcpyAsync(t->time_us, time_us, nE * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(t->mem_mb, mem_mb, nE * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(t->gpus, island_gpus, K * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(t->cap_mb, island_cap_mb, K * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(t->bw, bw_gbps, K * K * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dErr, 0, 4, 0);
     int herr = 0;
     if (e == cudaSuccess) {
         const int blocks = int(std::min<size_t>((nE + 255) / 256, 4096));
         tgValidateKernel<<<std::max(blocks, 1), 256>>>(t->time_us, t->mem_mb, t->gpus, t->cap_mb, t->bw, K, nE, dErr);
-        e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);
+        e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);   // the one synchronisation of the call
     }
     if (e != cudaSuccess || herr) {
-        cudaFree(base);
+        cudaFreeAsync(base, 0);
         delete t;
         if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("instance upload: ") + cudaGetErrorString(e));
         return fail(TG_ERR_RANGE, "table value out of range (bits: 1 time, 2 mem, 4 bw, 8 gpus, 16 cap): " + std::to_string(herr));
@@ -363,7 +364,7 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
 
 tg_status tg_instance_destroy(tg_instance* inst) {
     if (!inst) return TG_OK;
-    cudaFree(inst->time_us);  // base of the single allocation
+    cudaFreeAsync(inst->time_us, 0);  // base of the single allocation
     delete inst;
     return TG_OK;
 }
