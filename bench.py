@@ -32,6 +32,11 @@ METRIC = "slice_island_plans_evaluated_per_sec"
 UNIT = "plans/s"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE tgSolveKernel launch from the committed ncu capture
+# (profiles/r1_ncu_cfg4_solver.md); only valid for the default cfg4 windowed run
+NCU_TRAFFIC_BYTES = {("cfg4", False): 9.112e9}
+
+
 def make_workload(name: str, rank: int, n_inst: int):
     """Seeded synthetic instances (DESIGN.md input recipe).  Rank r takes its own seeds (weak scaling)."""
     import tg_inputs as gen
@@ -42,7 +47,8 @@ def make_workload(name: str, rank: int, n_inst: int):
     if name == "cfg2":
         return [gen.config2(rank)], "cfg2 7B-like L=32 K=6 P=4 m=16 (configs[1]), 1 instance/GPU"
     if name == "cfg5":
-        return gen.config5(n_inst, first_seed=rank * n_inst), \
+        from paper_2606_16907_b200.shard import weak_seeds
+        return [gen.config5_one(sd) for sd in weak_seeds(n_inst, rank)], \
             f"cfg5 throughput batch: {n_inst} instances L=48 K=10 P=4 m in {{4..64}} (configs[4]) per GPU"
     raise SystemExit(f"unknown workload {name}")
 
@@ -207,13 +213,9 @@ def run_ours(args):
             h.destroy()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device="cuda")
-    u = torch.tensor([float(plans), float(plans) / args.steps * e2e_steps, float(n_dp)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-    total_ms, e2e_s = t.tolist()
-    plans_all, plans_e2e, ndp_all = u.tolist()
+    from paper_2606_16907_b200.shard import aggregate
+    (plans_all, plans_e2e, ndp_all), (total_ms, e2e_s) = aggregate(
+        [float(plans), float(plans) / args.steps * e2e_steps, float(n_dp)], [total_ms, e2e_s], device="cuda")
     if rank == 0:
         peak, peak_src = peaks()
         km = sum(kern_ms) / len(kern_ms)
@@ -230,9 +232,11 @@ def run_ours(args):
                 "clocks": clk.summary(),
                 "e2e": {"value": plans_e2e / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "ms_per_step": e2e_s / e2e_steps * 1e3},
-                "gpu_launches": 3 * args.steps,
+                "gpu_launches": 3 * args.steps,   # tgLoadKernel + tgPrepareKernel + tgSolveKernel per tg_solve_batch
                 "roofline": {"bound": "hbm", "kernel": "tgSolveKernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                             "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                             "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.full_sweep)),
+                             "traffic_source": "profiles/r1_ncu_cfg4_solver.md" if (args.workload, args.full_sweep) in NCU_TRAFFIC_BYTES else None,
+                             "peak_source": peak_src,
                              "kernel_ms": km, "algorithmic_bytes_per_launch": alg_bytes,
                              "us_per_dp": km * 1e3 / (n_dp / args.steps),
                              "alu": {"relaxations_per_launch": relax / args.steps,

@@ -114,3 +114,42 @@ def test_mid_size_scaled_configs(tg):
              gen.config3(1, L=37, K=6), gen.config5_one(4, L=17, K=8)]
     for inst, g in zip(insts, solve_all(tg, insts)):
         same(oracle.solve(inst, n_threads=8), g, inst.name)
+
+
+def test_extreme_shapes(tg):
+    """Limits of the ABI: L = 1, L = 255 (TG_MAX_L), K = 16 (TG_MAX_K) with a tiny L, P = 255, m = 1 and
+    m = 2^20, nothing feasible, only the whole-model slice feasible."""
+    import numpy as np
+    insts = []
+    a = gen.random_small(1, Lmax=1, Kmax=1, Pmax=1); insts.append(a)
+    b = gen.random_small(2, Lmax=6, Kmax=3, Pmax=2); b.m = 1 << 20; insts.append(b)
+    c = gen.random_small(3, Lmax=6, Kmax=3, Pmax=2); c.m = 1; insts.append(c)
+    d = gen.random_small(4, Lmax=6, Kmax=3, Pmax=2); d.time_us[:] = 0x7FFFFFFF; insts.append(d)
+    e = gen.config3(0, L=6, K=3)   # only the whole model on island 1 is feasible
+    keep = e.time_us[gen.slice_index(6, 0, 6), 1, :].copy()
+    e.time_us[:] = 0x7FFFFFFF; e.time_us[gen.slice_index(6, 0, 6), 1, :] = keep; insts.append(e)
+    insts.append(gen.config4(0, L=3, K=16))                       # 65536 masks, L not a multiple of 4
+    for L, K, P in [(255, 2, 1), (5, 3, 255)]:                     # TG_MAX_L, TG_MAX_P
+        NS = L * (L + 1) // 2
+        idx = np.arange(NS * K * P).reshape(NS, K, P)
+        aa, bb = gen.slice_bounds(L)
+        t = ((bb - aa)[:, None, None] * gen.urand(9, 1, idx, 100, 900)).astype(np.int32)
+        mm = gen.urand(9, 2, idx, 1, 50).astype(np.int32)
+        insts.append(gen.Instance(f"L{L}K{K}P{P}", L, K, P, 4, t, mm, np.ones(K, np.int32), np.full(K, 25, np.int32),
+                                  np.full((K, K), 50, np.int32), 32))
+    for inst, g in zip(insts, solve_all(tg, insts)):
+        same(oracle.solve(inst, n_threads=8), g, inst.name)
+    for inst, g in zip(insts, solve_all(tg, insts, flags=1)):
+        same(oracle.solve(inst, n_threads=8), g, inst.name + " full sweep")
+
+
+@pytest.mark.parametrize("style", ["ties", "mixed", "tightmem"])
+def test_threshold_search_stress(tg, style):
+    """Branch-and-bound threshold search against the oracle's sweep on mid-size instances with every m,
+    heavy ties and binding memory; teams and solo mode (one batch of 60, then each alone)."""
+    insts = [gen.random_small(s + 20_000, Lmax=20, Kmax=8, Pmax=3, style=style) for s in range(60)]
+    want = [oracle.solve(i, n_threads=8) for i in insts]
+    for inst, o, g in zip(insts, want, solve_all(tg, insts)):
+        same(o, g, inst.name)
+    for inst, o in list(zip(insts, want))[:12]:
+        same(o, solve_all(tg, [inst])[0], inst.name + " alone")
