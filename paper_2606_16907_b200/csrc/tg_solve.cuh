@@ -24,6 +24,9 @@ struct TgShared {
     int useGlobalC;
     int sL, sLp, sKe, sInst;
     uint32_t sT;
+    // row windows (see "Row windows" below): rows hold Wd starts, row of state (S, k) begins at start lo4(cap(S))
+    int sWd, sSlack, sWindowed;
+    uint8_t maxlenK[TG_MAX_K];      // longest admissible slice of island k at T, any position
     uint32_t baseK[TG_MAX_K];
     int dmaxK[TG_MAX_K];
     uint8_t dmaxTile[TG_MAX_K][64];
@@ -97,6 +100,17 @@ __device__ __forceinline__ uint64_t tgLevelOff(uint64_t bufWords, int Ke, int Lp
     return rows * uint64_t(Lp);
 }
 
+// Row windows.  With maxlen_k = longest admissible slice of island k at T and cap(S) = sum of maxlen
+// over S, a state (a, S, k) is finite only if L - a <= cap(S), and it can be part of a full plan
+// only if the prefix [0, a) fits the other islands: a <= Ctot - cap(S), Ctot = cap(all).  So every
+// row needs just the starts  a in [L - cap(S), Ctot - cap(S)]  — Ctot - L + 1 of them, usually a small
+// fraction of L near T*.  Rows are stored with Wd = ceil4(Ctot - L + 4) entries beginning at the
+// 4-aligned start lo4(S) = floor4(max(0, L - cap(S))); entries left of the window are INF by the
+// first bound, entries right of it are never read by a state inside its own window.
+__device__ __forceinline__ int tgLo4(const TgShared& sm, int cap) {
+    return sm.sWindowed ? (max(0, sm.sL - cap) & ~3) : 0;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Staging of one item's thresholded cost tables into shared memory.
 //   Cs_k[(d-1)*Lp + a] = c[a][a+d][k] if <= T and a+d <= L-1, else INF   (k in compact labels)
@@ -126,8 +140,23 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         }
         sm.dmaxK[tid] = lo;
     }
+    if (tid >= 32 && tid < 32 + Ke) {  // longest admissible slice at any position (b <= L)
+        const uint32_t* sf = I.sufMinAll + size_t(__ldcg(&itp->isl[tid - 32])) * (L + 2);
+        int lo = 0, hi = L;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (sf[mid] <= T) lo = mid; else hi = mid - 1;
+        }
+        sm.maxlenK[tid - 32] = uint8_t(lo);
+    }
     __syncthreads();
     if (tid == 0) {
+        int ctot = 0;
+        for (int kc = 0; kc < Ke; ++kc) ctot += sm.maxlenK[kc];
+        const int wd = (ctot - L + 4 + 3) & ~3;
+        sm.sSlack = ctot - L;
+        sm.sWindowed = (ctot >= L && wd < Lp) ? 1 : 0;
+        sm.sWd = sm.sWindowed ? wd : Lp;
         uint32_t acc = 0;
         for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += uint32_t((sm.dmaxK[kc] + 3) & ~3) * uint32_t(Lp); }
         sm.useGlobalC = acc > uint32_t(ctx.csWords) ? 1 : 0;
@@ -193,10 +222,10 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
 // ---------------------------------------------------------------------------------------------
 __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsigned long long* key, bool post) {
     const TgInstDev& I = ctx.inst[sm.sInst];
-    const int L = sm.sL, Lp = sm.sLp, Ke = sm.sKe;
+    const int L = sm.sL, Wd = sm.sWd, Ke = sm.sKe;
     const uint32_t T = sm.sT;
-    for (int w = threadIdx.x; w < Ke * Lp; w += TG_NT) {
-        const int kc = w / Lp, a = w - kc * Lp;
+    for (int w = threadIdx.x; w < Ke * Wd; w += TG_NT) {
+        const int kc = w / Wd, a = tgLo4(sm, sm.maxlenK[kc]) + (w - kc * Wd);
         uint32_t v = TG_INFU;
         if (a < L) {
             v = I.cd[size_t(sm.isl[kc]) * I.triG + tgGOff(L, L - a) + a];
@@ -218,7 +247,7 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
 //           mbarrier; issued one mask ahead of its use (double buffer)
 //   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[j][b]       lane = (4 consecutive b) x (k group)
 //   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]    lane = (4 consecutive a) x (k group)
-// Warp-private shared memory: rows of HS = Lp + 8 words: [0, nk) the H rows (H[b] at index b-1,
+// Warp-private shared memory: rows of HS = Lp + 8 words: [0, nk) the H rows (H[b] at index b - lo4R,
 // INF-padded), then two source buffers of r rows each.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
@@ -277,9 +306,9 @@ __device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
 // j of R copies that source).  Source row of j = state (R\{j}, first island j) of level r-1, whose
 // mask rank is  sum_{i<p} C(e_i, i+1) + sum_{i>p} C(e_i, i)  (p = position of j in R: the elements
 // below keep their position, those above move down by one) -- two warp scans over the member lanes.
-__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int r, int nk, int Lp, uint32_t bufAddr,
+__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int r, int nk, int Wd, uint32_t bufAddr,
                                             uint32_t rowBytes, const uint32_t* Gprev, unsigned long long* bar, int lane) {
-    if (lane == 0) tgMbarExpect(bar, uint32_t(r) * uint32_t(Lp) * 4u);
+    if (lane == 0) tgMbarExpect(bar, uint32_t(r) * uint32_t(Wd) * 4u);
     const bool member = (R >> lane) & 1u;
     const int p = __popc(R & ((1u << lane) - 1u));
     uint32_t up = member ? uint32_t(sm.binom[lane & 15][p + 1]) : 0u;   // C(e, p+1): kept position
@@ -294,7 +323,7 @@ __device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int 
     if (member && lane < 16) {
         const uint32_t rank = (upIncl - up) + (dnTotal - dnIncl);
         const uint32_t row = rank * uint32_t(nk + 1) + uint32_t(lane - p);
-        tgBulkLoad(bufAddr + uint32_t(p) * rowBytes, Gprev + size_t(row) * Lp, uint32_t(Lp) * 4u, bar);
+        tgBulkLoad(bufAddr + uint32_t(p) * rowBytes, Gprev + size_t(row) * Wd, uint32_t(Wd) * 4u, bar);
     }
 }
 
@@ -326,22 +355,23 @@ __device__ __forceinline__ void tgPhase1(const TgShared& sm, uint32_t R, int r, 
             const uint32_t j4 = uint32_t(__ffs(Rb) - 1) * 4u;
             Rb &= Rb - 1;
             const uint4 g4 = tgLds4(sA);
-            const uint32_t nx = hasNx ? tgLds1(sA + 16) : TG_INFU;
             sA += rowBytes;
 #pragma unroll
             for (int i = 0; i < NSL; ++i) {
                 const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
-                acc[i][0] = tgAddMin(xv, g4.y, acc[i][0]);
-                acc[i][1] = tgAddMin(xv, g4.z, acc[i][1]);
-                acc[i][2] = tgAddMin(xv, g4.w, acc[i][2]);
-                acc[i][3] = tgAddMin(xv, nx, acc[i][3]);
+                acc[i][0] = tgAddMin(xv, g4.x, acc[i][0]);
+                acc[i][1] = tgAddMin(xv, g4.y, acc[i][1]);
+                acc[i][2] = tgAddMin(xv, g4.z, acc[i][2]);
+                acc[i][3] = tgAddMin(xv, g4.w, acc[i][3]);
             }
         }
 #pragma unroll
         for (int i = 0; i < NSL; ++i) {
             if (i + 1 < NSL || lastValid) {
-                const uint32_t hA = hAddr0 + uint32_t(slot0 + NG * i) * rowBytes + uint32_t(c) * 16u;
+                // H row = [4 x INF | Wd values, H[b] at index b - lo4R | 8 x INF]
+                const uint32_t hA = hAddr0 + uint32_t(slot0 + NG * i) * rowBytes + 16u + uint32_t(c) * 16u;
                 tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));
+                if (c == 0) tgSts4(hA - 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
                 if (!hasNx) {
                     tgSts4(hA + 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
                     tgSts4(hA + 32, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
@@ -351,8 +381,8 @@ __device__ __forceinline__ void tgPhase1(const TgShared& sm, uint32_t R, int r, 
     }
 }
 
-// One block of 4 diagonals d = dq+1..dq+4 for one row and 4 starts: LO = H window [a0+dq, a0+dq+4),
-// HI = the next 4 values (loaded here).
+// One block of 4 diagonals d = dq+1..dq+4 for one row and 4 starts a0..a0+3: LO = H[a0+dq .. a0+dq+3],
+// HI = the next 4 values (loaded here); start a0+ai at diagonal d reads H[a0+ai+d].
 #define TG_P2_STEP(LO, HI)                                                                     \
     {                                                                                          \
         const uint4 h = tgLds4(hA);                                                            \
@@ -376,7 +406,7 @@ __device__ __forceinline__ void tgPhase1(const TgShared& sm, uint32_t R, int r, 
             }                                                                                  \
             const uint32_t cv[4] = {c4.x, c4.y, c4.z, c4.w};                                   \
             _Pragma("unroll") for (int ai = 0; ai < 4; ++ai)                                   \
-                out[ai] = tgAddMin(cv[ai], (ai + e < 4 ? LO[ai + e] : HI[ai + e - 4]), out[ai]); \
+                out[ai] = tgAddMin(cv[ai], (ai + e + 1 < 4 ? LO[ai + e + 1] : HI[ai + e - 3]), out[ai]); \
         }                                                                                      \
         cA += 4 * cStride;                                                                     \
         dq += 4;                                                                               \
@@ -384,40 +414,50 @@ __device__ __forceinline__ void tgPhase1(const TgShared& sm, uint32_t R, int r, 
 
 // phase 2 for this lane's rows (slots g, g+NG, ...) and a chunks of mask R:
 //   G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]
+// Row of (R u {k}, k) starts at start lo4S = lo4(capR + maxlen_k); the H row starts at b = lo4R, so
+// H[a + d] sits at stored index (a - lo4S) + d - delta, delta = lo4R - lo4S (a multiple of 4).
 template <bool GLOBALC>
-__device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& sm, uint32_t R, int nk, int nb4, int c0, int CH,
-                                         int NG, int g, uint32_t hAddr0, uint32_t rowBytes, uint32_t csBase, uint32_t cStride,
-                                         const uint8_t* kl, uint32_t* gRow, unsigned long long& bestKey) {
+__device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& sm, uint32_t R, int capR, int nk, int nbw, int c0,
+                                         int CH, int NG, int g, uint32_t hAddr0, uint32_t rowBytes, uint32_t csBase,
+                                         uint32_t cStride, const uint8_t* kl, uint32_t* gRow, unsigned long long& bestKey) {
     const TgInstDev& I = ctx.inst[sm.sInst];
-    const int L = sm.sL, Lp = sm.sLp;
+    const int L = sm.sL, Lp = sm.sLp, Wd = sm.sWd;
     const uint32_t T = sm.sT;
+    const int lo4R = tgLo4(sm, capR);
     for (int s = g; s < nk; s += NG) {
         const int k = kl[s];
+        const int lo4S = tgLo4(sm, capR + sm.maxlenK[k]), dq4 = (lo4R - lo4S) >> 2;
         const uint32_t* cdk = GLOBALC ? I.cd + size_t(sm.isl[k]) * I.triG : nullptr;
-        const uint32_t cBase = csBase + sm.baseK[k] * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes;
-        uint32_t* const gOut = gRow + size_t(s) * Lp;
-        for (int c = c0; c < nb4; c += CH) {
-            const int a0 = 4 * c, dm = sm.dmaxTile[k][c], nq = (dm + 3) >> 2;
+        const uint32_t cBase = csBase + (sm.baseK[k] + uint32_t(lo4S)) * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes + 16u;
+        uint32_t* const gOut = gRow + size_t(s) * Wd;
+        for (int cw = c0; cw < nbw; cw += CH) {
+            const int a0 = lo4S + 4 * cw, c = a0 >> 2;   // c = absolute tile of 4 starts
             uint32_t out[4] = {TG_INFU, TG_INFU, TG_INFU, TG_INFU};
-            if (nq > 0) {
-                uint32_t hA = hRow + uint32_t(c) * 16u;
-                uint32_t cA = cBase + uint32_t(c) * 16u;
-                int dq = 0;
-                uint32_t Wa[4], Wb[4];
-                {
-                    const uint4 h = tgLds4(hA);
-                    hA += 16;
-                    Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
-                }
+            if (a0 < Lp) {
+                // blocks of 4 diagonals: from the first that reaches the H row to the last admissible one
+                // (never past the end of the H row: such entries lie right of this row's window)
+                const int dm = sm.dmaxTile[k][c], q0 = max(0, dq4 - 1 - cw);
+                const int nq = min((dm + 3) >> 2, nbw - cw + dq4 + 1);
+                if (q0 < nq) {
+                    uint32_t hA = hRow + uint32_t(4 * (cw + q0 - dq4)) * 4u;
+                    uint32_t cA = cBase + uint32_t(cw) * 16u + uint32_t(4 * q0) * cStride;
+                    int dq = 4 * q0;
+                    uint32_t Wa[4], Wb[4];
+                    {
+                        const uint4 h = tgLds4(hA);
+                        hA += 16;
+                        Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
+                    }
 #pragma unroll 1
-                for (int q = 0; q < nq; q += 2) {
-                    TG_P2_STEP(Wa, Wb)
-                    if (q + 1 >= nq) break;
-                    TG_P2_STEP(Wb, Wa)
+                    for (int q = q0; q < nq; q += 2) {
+                        TG_P2_STEP(Wa, Wb)
+                        if (q + 1 >= nq) break;
+                        TG_P2_STEP(Wb, Wa)
+                    }
                 }
             }
-            *reinterpret_cast<uint4*>(gOut + a0) = make_uint4(out[0], out[1], out[2], out[3]);
-            if (c == 0 && out[0] < TG_INFU) {
+            *reinterpret_cast<uint4*>(gOut + 4 * cw) = make_uint4(out[0], out[1], out[2], out[3]);
+            if (a0 == 0 && out[0] < TG_INFU) {
                 const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)(R | (1u << k)) << 8 | (unsigned long long)k;
                 bestKey = kk < bestKey ? kk : bestKey;
             }
@@ -428,11 +468,13 @@ __device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& 
 __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
                             uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW, uint32_t& par) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int Lp = sm.sLp, HS = Lp + 8, nb4 = Lp >> 2, nk = Ke - r;
+    const int Lp = sm.sLp, Wd = sm.sWd, HS = Wd + 12, nbw = Wd >> 2, nk = Ke - r;
     const int nMasks = sm.binom[Ke][r];
     const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
     if (lo >= hi) return;
-    const int chShift = nb4 <= 8 ? 3 : (nb4 <= 16 ? 4 : 5), CH = 1 << chShift, NG = 32 >> chShift;
+    // lane = (chunk of 4 starts) x (island group): CH chunk lanes, NG = 32 / CH groups
+    const int chShift = nbw <= 2 ? 1 : (nbw <= 4 ? 2 : (nbw <= 8 ? 3 : (nbw <= 16 ? 4 : 5)));
+    const int CH = 1 << chShift, NG = 32 >> chShift;
     const int c0 = lane & (CH - 1), g = lane >> chShift;
     const uint32_t rowBytes = uint32_t(HS) * 4u, cStride = uint32_t(Lp) * 4u;
     const uint32_t hAddr0 = tgSmemAddr(wbuf), csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
@@ -442,17 +484,22 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     uint8_t* kl = &sm.kl[warp][0];
     const uint32_t keMask = (1u << Ke) - 1u;
     const bool globalC = sm.useGlobalC != 0;
+    const int myLen = lane < Ke ? int(sm.maxlenK[lane]) : 0;
     unsigned long long bestKey = TG_KEY_NONE;
 
     uint32_t R = tgUnrank(sm, uint32_t(lo), r, Ke);
     asm volatile("fence.proxy.async.global;" ::: "memory");
-    tgIssueMask(sm, R, r, nk, Lp, bufAddr[0], rowBytes, Gprev, bars + 0, lane);
+    tgIssueMask(sm, R, r, nk, Wd, bufAddr[0], rowBytes, Gprev, bars + 0, lane);
     int b = 0;
     for (int idx = lo; idx < hi; ++idx, b ^= 1) {
         const uint32_t Rn = tgNextMask(R);
-        if (idx + 1 < hi) tgIssueMask(sm, Rn, r, nk, Lp, bufAddr[b ^ 1], rowBytes, Gprev, bars + (b ^ 1), lane);
+        if (idx + 1 < hi) tgIssueMask(sm, Rn, r, nk, Wd, bufAddr[b ^ 1], rowBytes, Gprev, bars + (b ^ 1), lane);
         const uint32_t comp = ~R & keMask;
         if (lane < Ke && (comp >> lane & 1u)) kl[__popc(comp & ((1u << lane) - 1u))] = uint8_t(lane);
+        int capR = (R >> lane & 1u) ? myLen : 0;   // cap(R) = sum of maxlen over the members
+#pragma unroll
+        for (int o = 8; o > 0; o >>= 1) capR += __shfl_xor_sync(0xffffffffu, capR, o);
+        capR = __shfl_sync(0xffffffffu, capR, 0);
         __syncwarp();
         tgMbarWait(bars + b, (par >> b) & 1u);
         par ^= 1u << b;
@@ -460,7 +507,7 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
         // ---- phase 1: transfer pre-minimum, H rows into the warp's shared memory ---------------
         for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
             const int nsl = min(TG_SPL, (nk - s0 + NG - 1) / NG);   // slots of the widest island group
-#define TG_P1_CASE(N) case N: tgPhase1<N>(sm, R, r, nk, nb4, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
+#define TG_P1_CASE(N) case N: tgPhase1<N>(sm, R, r, nk, nbw, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
             switch (nsl) {
                 TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
                 TG_P1_CASE(5) TG_P1_CASE(6) TG_P1_CASE(7) TG_P1_CASE(8)
@@ -470,9 +517,9 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
         __syncwarp();
 
         // ---- phase 2: min-plus product with the thresholded cost rows ----------------------------
-        uint32_t* const gRow = Gcur + size_t(idx) * nk * Lp;
-        if (globalC) tgPhase2<true>(ctx, sm, R, nk, nb4, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
-        else tgPhase2<false>(ctx, sm, R, nk, nb4, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+        uint32_t* const gRow = Gcur + size_t(idx) * nk * Wd;
+        if (globalC) tgPhase2<true>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+        else tgPhase2<false>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
         __syncwarp();
         R = Rn;
     }
@@ -492,10 +539,10 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
 // per-state argmin (lowest b, then lowest j — SURVEY A13) along the optimal path from the stored
 // G levels of the slot.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned long long key, const uint32_t* slot) {
+__device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgItem* itp, unsigned long long key, const uint32_t* slot) {
     const int lane = threadIdx.x & 31;
     TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
-    const int L = I.L, Lp = I.Lp, K = I.K, Ke = __ldcg(&itp->Ke);
+    const int L = I.L, K = I.K, Ke = __ldcg(&itp->Ke);
     const uint32_t T = __ldcg(&itp->T);
     tg_result* out = ctx.out + __ldcg(&itp->inst);
     uint8_t isl[TG_MAX_K];
@@ -526,18 +573,22 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgItem* itp, unsigned l
             b = L;
         } else {
             const int r = __popc(R);
-            const uint32_t* Gl = slot + tgLevelOff(0, Ke, Lp, r - 1);
+            const int Wd = sm.sWd;
+            const uint32_t* Gl = slot + tgLevelOff(0, Ke, Wd, r - 1);
             const uint32_t* cdk = I.cd + size_t(ko) * I.triG;
+            int capR = 0;   // every source row (R\{j}, j) starts at start lo4(cap(R))
+            for (int j = 0; j < Ke; ++j) if (R >> j & 1u) capR += sm.maxlenK[j];
+            const int lo4R = tgLo4(sm, capR);
             unsigned long long best = TG_KEY_NONE;
             for (int bb = a + 1 + lane; bb <= L - 1; bb += 32) {
                 const uint32_t c = cdk[tgGOff(L, bb - a) + a];
-                if (c > T) continue;
+                if (c > T || bb < lo4R || bb >= lo4R + Wd) continue;
                 uint32_t h = TG_INFU; int hj = 0;
                 for (int j = 0; j < Ke; ++j) {
                     if (!(R >> j & 1u)) continue;
                     const uint32_t Rp = R ^ (1u << j);
                     const size_t row = size_t(ctx.rankOf[Rp]) * (Ke - r + 1) + (j - __popc(R & ((1u << j) - 1u)));
-                    const uint32_t v = I.x[ko * TG_MAX_K + isl[j]] + __ldcg(Gl + row * Lp + bb);
+                    const uint32_t v = I.x[ko * TG_MAX_K + isl[j]] + __ldcg(Gl + row * Wd + (bb - lo4R));
                     if (v < h) { h = v; hj = j; }
                 }
                 const uint32_t v = c + h;
@@ -585,7 +636,8 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
                           unsigned long long* key, int member, int teamSize, int slotIdx, uint32_t& par) {
     tgStageItem(ctx, sm, Cs, wbufAll, itp, member == 0);
     tgMark(sm, 0);
-    const int Ke = sm.sKe, Lp = sm.sLp, nW = ctx.nActiveWarps, warp = threadIdx.x >> 5;
+    const int Ke = sm.sSlack >= 0 ? sm.sKe : 0;   // the islands' longest slices cannot cover L layers: infeasible at T
+    const int Wd = sm.sWd, nW = ctx.nActiveWarps, warp = threadIdx.x >> 5;
     const uint64_t bufWords = __ldcg(&itp->bufWords);
     uint32_t* slot = ctx.scratch + uint64_t(slotIdx) * ctx.slotWords;
     uint32_t* bar = ctx.slotBar + slotIdx;
@@ -595,8 +647,8 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         tgLevel0(ctx, sm, slot, key, member == 0);
         __syncthreads();
         for (int r = 1; r < Ke; ++r) {
-            const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Lp, r - 1);
-            uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Lp, r);
+            const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Wd, r - 1);
+            uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Wd, r);
             if (warp < nW) tgWarpLevel(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, par);
             tgMark(sm, 3);
             if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
@@ -605,7 +657,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         }
     }
     tgMark(sm, 0);
-    if ((__ldcg(&itp->flags) & 1) && member == 0 && threadIdx.x < 32) tgBacktrack(ctx, itp, __ldcg(key), slot);
+    if ((__ldcg(&itp->flags) & 1) && member == 0 && threadIdx.x < 32) tgBacktrack(ctx, sm, itp, __ldcg(key), slot);
     __syncthreads();
     tgMark(sm, 7);
 }
