@@ -35,7 +35,7 @@ struct TgShared {
     uint8_t isl[TG_MAX_K];
     uint16_t binom[17][17];
     // per-warp streaming state
-    alignas(8) unsigned long long mbar[TG_NW][2];   // completion of the two source buffers
+    uint32_t rowOf[TG_NW][TG_MAX_K];                // source row of each member of the mask being issued
     uint8_t kl[TG_NW][TG_MAX_K];                    // islands not in the current mask, ascending
     // scheduler / queue
     uint32_t warpSums[33];
@@ -235,7 +235,6 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
         if (post && a == 0 && v < TG_INFU)
             atomicMin(key, (unsigned long long)v << 32 | (unsigned long long)(1u << kc) << 8 | (unsigned long long)kc);
     }
-    asm volatile("fence.proxy.async.global;" ::: "memory");   // level 0 is read by bulk async copies
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -302,13 +301,15 @@ __device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
     return (((R ^ t) >> 2) >> (__ffs(c) - 1)) | t;
 }
 
-// Issue the r source-row copies of mask R into the warp's buffer (the lane whose index is a member
-// j of R copies that source).  Source row of j = state (R\{j}, first island j) of level r-1, whose
-// mask rank is  sum_{i<p} C(e_i, i+1) + sum_{i>p} C(e_i, i)  (p = position of j in R: the elements
-// below keep their position, those above move down by one) -- two warp scans over the member lanes.
-__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int r, int nk, int Wd, uint32_t bufAddr,
-                                            uint32_t rowBytes, const uint32_t* Gprev, unsigned long long* bar, int lane) {
-    if (lane == 0) tgMbarExpect(bar, uint32_t(r) * uint32_t(Wd) * 4u);
+// Issue the copies of the r source rows of mask R into the warp's buffer: 16-byte asynchronous copies
+// (cp.async, LDGSTS), one lane per (source, chunk of 4 starts), committed as one group.  Source row of
+// member j = state (R\{j}, first island j) of level r-1, whose mask rank is
+//   sum_{i<p} C(e_i, i+1) + sum_{i>p} C(e_i, i)   (p = position of j in R: the elements below keep their
+// position, those above move down by one) -- two warp scans over the member lanes.
+// (Bulk TMA copies, one per row, were measured slower here: with row windows a row is often 32-64 bytes
+// and the per-SM TMA issue rate, not bandwidth, became the bound -- DESIGN.md 7.4.)
+__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int r, int nk, int Wd, int nbw, int chShift,
+                                            uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
     const bool member = (R >> lane) & 1u;
     const int p = __popc(R & ((1u << lane) - 1u));
     uint32_t up = member ? uint32_t(sm.binom[lane & 15][p + 1]) : 0u;   // C(e, p+1): kept position
@@ -320,10 +321,15 @@ __device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int 
         if ((lane & 15) >= o) { upIncl += a; dnIncl += c; }
     }
     const uint32_t dnTotal = __shfl_sync(0xffffffffu, dnIncl, 15);
-    if (member && lane < 16) {
-        const uint32_t rank = (upIncl - up) + (dnTotal - dnIncl);
-        const uint32_t row = rank * uint32_t(nk + 1) + uint32_t(lane - p);
-        tgBulkLoad(bufAddr + uint32_t(p) * rowBytes, Gprev + size_t(row) * Wd, uint32_t(Wd) * 4u, bar);
+    if (member && lane < 16) rowOf[p] = ((upIncl - up) + (dnTotal - dnIncl)) * uint32_t(nk + 1) + uint32_t(lane - p);
+    __syncwarp();
+    const int cpShift = nbw > 32 ? 6 : chShift, CH = 1 << cpShift;   // chunks per row, rounded up to a power of two
+    for (int w = lane; w < (r << cpShift); w += 32) {
+        const int ji = w >> cpShift, ch = w & (CH - 1);
+        if (ch < nbw) {
+            const uint32_t* src = Gprev + size_t(rowOf[ji]) * Wd + 4 * ch;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(bufAddr + uint32_t(ji) * rowBytes + uint32_t(ch) * 16u), "l"(src) : "memory");
+        }
     }
 }
 
@@ -423,10 +429,11 @@ __device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& 
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int L = sm.sL, Lp = sm.sLp, Wd = sm.sWd;
     const uint32_t T = sm.sT;
-    const int lo4R = tgLo4(sm, capR);
+    const int Lw = sm.sWindowed ? L : 0;              // lo4(cap) = floor4(max(0, Lw - cap)): 0 when rows are not windowed
+    const int lo4R = max(0, Lw - capR) & ~3;
     for (int s = g; s < nk; s += NG) {
         const int k = kl[s];
-        const int lo4S = tgLo4(sm, capR + sm.maxlenK[k]), dq4 = (lo4R - lo4S) >> 2;
+        const int lo4S = max(0, Lw - capR - int(sm.maxlenK[k])) & ~3, dq4 = (lo4R - lo4S) >> 2;
         const uint32_t* cdk = GLOBALC ? I.cd + size_t(sm.isl[k]) * I.triG : nullptr;
         const uint32_t cBase = csBase + (sm.baseK[k] + uint32_t(lo4S)) * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes + 16u;
         uint32_t* const gOut = gRow + size_t(s) * Wd;
@@ -480,7 +487,7 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     const uint32_t hAddr0 = tgSmemAddr(wbuf), csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
     const uint32_t xInfAddr = tgSmemAddr(&sm.xInf[0]);
     const uint32_t bufAddr[2] = {hAddr0 + uint32_t(nk) * rowBytes, hAddr0 + uint32_t(nk + r) * rowBytes};
-    unsigned long long* bars = &sm.mbar[warp][0];
+    uint32_t* rowOf = &sm.rowOf[warp][0];
     uint8_t* kl = &sm.kl[warp][0];
     const uint32_t keMask = (1u << Ke) - 1u;
     const bool globalC = sm.useGlobalC != 0;
@@ -488,25 +495,25 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     unsigned long long bestKey = TG_KEY_NONE;
 
     uint32_t R = tgUnrank(sm, uint32_t(lo), r, Ke);
-    asm volatile("fence.proxy.async.global;" ::: "memory");
-    tgIssueMask(sm, R, r, nk, Wd, bufAddr[0], rowBytes, Gprev, bars + 0, lane);
+    tgIssueMask(sm, R, r, nk, Wd, nbw, chShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
+    asm volatile("cp.async.commit_group;" ::: "memory");
     int b = 0;
     for (int idx = lo; idx < hi; ++idx, b ^= 1) {
         const uint32_t Rn = tgNextMask(R);
-        if (idx + 1 < hi) tgIssueMask(sm, Rn, r, nk, Wd, bufAddr[b ^ 1], rowBytes, Gprev, bars + (b ^ 1), lane);
+        if (idx + 1 < hi) tgIssueMask(sm, Rn, r, nk, Wd, nbw, chShift, bufAddr[b ^ 1], rowBytes, Gprev, rowOf, lane);
+        asm volatile("cp.async.commit_group;" ::: "memory");   // possibly empty: keeps the group count uniform
         const uint32_t comp = ~R & keMask;
         if (lane < Ke && (comp >> lane & 1u)) kl[__popc(comp & ((1u << lane) - 1u))] = uint8_t(lane);
         int capR = (R >> lane & 1u) ? myLen : 0;   // cap(R) = sum of maxlen over the members
 #pragma unroll
         for (int o = 8; o > 0; o >>= 1) capR += __shfl_xor_sync(0xffffffffu, capR, o);
         capR = __shfl_sync(0xffffffffu, capR, 0);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");   // this mask's rows have landed (the next mask's may be in flight)
         __syncwarp();
-        tgMbarWait(bars + b, (par >> b) & 1u);
-        par ^= 1u << b;
 
         // ---- phase 1: transfer pre-minimum, H rows into the warp's shared memory ---------------
         for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
-            const int nsl = min(TG_SPL, (nk - s0 + NG - 1) / NG);   // slots of the widest island group
+            const int nsl = min(TG_SPL, (nk - s0 + NG - 1) >> (5 - chShift));   // slots of the widest island group
 #define TG_P1_CASE(N) case N: tgPhase1<N>(sm, R, r, nk, nbw, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
             switch (nsl) {
                 TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
@@ -523,8 +530,7 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
         __syncwarp();
         R = Rn;
     }
-    // the rows just written are read by bulk async copies (async proxy) of the next level
-    asm volatile("fence.proxy.async.global;" ::: "memory");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     if (__any_sync(0xffffffffu, bestKey != TG_KEY_NONE)) {
         for (int o = 16; o > 0; o >>= 1) {
             const unsigned long long ot = __shfl_xor_sync(0xffffffffu, bestKey, o);
@@ -948,8 +954,6 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
     if (threadIdx.x == 0) {
         for (int i = 0; i < 8; ++i) sm.cyc[i] = 0;
         sm.tmark = clock64();
-        for (int w = 0; w < TG_NW; ++w) { tgMbarInit(&sm.mbar[w][0], 1); tgMbarInit(&sm.mbar[w][1], 1); }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int w = threadIdx.x; w < 17 * 17; w += TG_NT) sm.binom[w / 17][w % 17] = tgBinom[w / 17][w % 17];
     if (threadIdx.x < TG_MAX_K) sm.xInf[threadIdx.x] = TG_INFU;
