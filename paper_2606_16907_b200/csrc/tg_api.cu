@@ -41,7 +41,6 @@ struct DeviceState {
     int smemPerSM = 0;
     int ctasPerSM = 0;    // co-resident CTAs of the solver per SM
     int dynSmem = 0;      // dynamic shared memory of one solver CTA
-    uint16_t* maskOf = nullptr;
     uint16_t* rankOf = nullptr;
 };
 std::mutex g_mu;
@@ -62,31 +61,24 @@ tg_status deviceInit(int dev, DeviceState** out) {
         int coop = 0;
         TG_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
         if (!coop) return fail(TG_ERR_CUDA, "device lacks cooperative launch");
-        // masks ordered by (popcount, value) == colexicographic rank inside each popcount class
-        std::vector<uint16_t> maskOf(65536), rankOf(65536);
+        // rankOf[mask] = colexicographic rank inside its popcount class (masks of one popcount ordered by value)
+        std::vector<uint16_t> rankOf(65536);
         uint16_t binom[17][17];
         memset(binom, 0, sizeof(binom));
         for (int n = 0; n <= 16; ++n) {
             binom[n][0] = 1;
             for (int r = 1; r <= n; ++r) binom[n][r] = uint16_t(binom[n - 1][r - 1] + (r <= n - 1 ? binom[n - 1][r] : 0));
         }
-        uint32_t popOff[18];
-        popOff[0] = 0;
-        for (int r = 0; r <= 16; ++r) popOff[r + 1] = popOff[r] + binom[16][r];
         uint32_t fill[17];
         memset(fill, 0, sizeof(fill));
         for (uint32_t mk = 0; mk < 65536; ++mk) {
             const int r = __builtin_popcount(mk);
-            maskOf[popOff[r] + fill[r]] = uint16_t(mk);
             rankOf[mk] = uint16_t(fill[r]);
             ++fill[r];
         }
-        TG_CUDA(cudaMalloc(&D.maskOf, 65536 * sizeof(uint16_t)));
         TG_CUDA(cudaMalloc(&D.rankOf, 65536 * sizeof(uint16_t)));
-        TG_CUDA(cudaMemcpy(D.maskOf, maskOf.data(), 65536 * sizeof(uint16_t), cudaMemcpyHostToDevice));
         TG_CUDA(cudaMemcpy(D.rankOf, rankOf.data(), 65536 * sizeof(uint16_t), cudaMemcpyHostToDevice));
         TG_CUDA(cudaMemcpyToSymbol(tgBinom, binom, sizeof(binom)));
-        TG_CUDA(cudaMemcpyToSymbol(tgPopOff, popOff, sizeof(popOff)));
         TG_CUDA(cudaFuncSetAttribute(tgPrepareKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TG_SORT_SMEM_MAX * 4));
         cudaFuncAttributes fa;
         TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
@@ -254,7 +246,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.slotBar = reinterpret_cast<uint32_t*>(W.base + oBar);
     c.wishMax = g_wishMax;
     c.ctrl = reinterpret_cast<TgCtrl*>(W.base + oCtrl);
-    c.maskOf = D->maskOf; c.rankOf = D->rankOf;
+    c.rankOf = D->rankOf;
 
     const dim3 g((maxCells + 255) / 256, n);
     tgLoadKernel<<<g, 256, 0, st>>>(W.inst);

@@ -104,7 +104,6 @@ struct TgSolveCtx {
     uint32_t* slotBar;          // [nSlots] arrival counters of the team barriers, zeroed every round
     TgCtrl* ctrl;
     tg_result* out;
-    const uint16_t* maskOf;     // [65536] masks ordered by (popcount, value)
     const uint16_t* rankOf;     // [65536] rank of a mask inside its popcount class
     uint32_t flags;             // TG_SOLVE_*
     int32_t mode;               // 0 = solve, 1 = single DP at dpT (tg_dp_at)
@@ -114,6 +113,5 @@ struct TgSolveCtx {
     int32_t nActiveWarps;       // warps per CTA that stream masks (all of them unless L is huge)
 };
 
-// binomials up to 16 choose r and popcount-class offsets into maskOf
+// binomials up to 16 choose r
 __constant__ uint16_t tgBinom[17][17];
-__constant__ uint32_t tgPopOff[18];

@@ -57,8 +57,6 @@ __device__ __forceinline__ void tgMark(TgShared& sm, int which) {
 
 __device__ __forceinline__ uint32_t tgAddMin(uint32_t a, uint32_t b, uint32_t c) { return __viaddmin_u32(a, b, c); }
 
-__device__ __forceinline__ uint4 tgLdcg4(const uint32_t* p) { return __ldcg(reinterpret_cast<const uint4*>(p)); }
-
 // Grid-wide barrier on a monotone counter (all CTAs are co-resident: cooperative launch).
 __device__ __forceinline__ void tgGridBarrier(TgCtrl* ctrl, uint32_t& epoch) {
     __syncthreads();
@@ -121,7 +119,7 @@ __device__ __forceinline__ int tgLo4(const TgShared& sm, int cap) {
 __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t*, const TgItem* itp, bool count) {
     __syncthreads();
     unsigned nAdm = 0;   // admissible (a, b, k) cost entries with b <= L-1 seen by this thread
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nWarps = TG_NT >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
     const TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
     const int L = I.L, Lp = I.Lp, Ke = __ldcg(&itp->Ke), nb4 = Lp >> 2;
     const uint32_t T = __ldcg(&itp->T);
@@ -241,34 +239,15 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
 // Levels r >= 1: one WARP per mask R, streaming over a contiguous range of masks (colexicographic
 // order, successor by Gosper's hack).  Nothing but the item's staged tables is shared between the
 // warps of a CTA, so a level needs no CTA barrier at all.  Per mask R (|R| = r, nk = Ke - r):
-//   issue   lane i < r: one bulk async copy (TMA, cp.async.bulk) of the source row
-//           G_{r-1}[R\{j_i}][j_i][.] into the warp's shared-memory buffer, completion on the warp's
-//           mbarrier; issued one mask ahead of its use (double buffer)
+//   issue   16-byte cp.async copies of the r source rows G_{r-1}[R\{j}][j][.] into the warp's
+//           shared-memory buffer, one mask ahead of their use (double buffer, commit / wait_group)
 //   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[j][b]       lane = (4 consecutive b) x (k group)
 //   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]    lane = (4 consecutive a) x (k group)
-// Warp-private shared memory: rows of HS = Lp + 8 words: [0, nk) the H rows (H[b] at index b - lo4R,
-// INF-padded), then two source buffers of r rows each.
+// Warp-private shared memory: rows of Wd + 12 words: [0, nk) the H rows (4 INF | H[b] at index
+// b - lo4(R) | 8 INF), then two source buffers of r rows each.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
-__device__ __forceinline__ void tgMbarInit(unsigned long long* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tgSmemAddr(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void tgMbarExpect(unsigned long long* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tgSmemAddr(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void tgMbarWait(unsigned long long* bar, uint32_t parity) {
-    const uint32_t a = tgSmemAddr(bar);
-    uint32_t ok = 0;
-    while (!ok) {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
-    }
-}
-__device__ __forceinline__ void tgBulkLoad(uint32_t dstSmemAddr, const uint32_t* srcGlobal, uint32_t bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dstSmemAddr), "l"(srcGlobal), "r"(bytes), "r"(tgSmemAddr(bar)) : "memory");
-}
 __device__ __forceinline__ uint4 tgLds4(uint32_t addr) {
     uint4 v;
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
@@ -473,7 +452,7 @@ __device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& 
 }
 
 __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
-                            uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW, uint32_t& par) {
+                            uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int Lp = sm.sLp, Wd = sm.sWd, HS = Wd + 12, nbw = Wd >> 2, nk = Ke - r;
     const int nMasks = sm.binom[Ke][r];
@@ -639,7 +618,7 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
 // One DP(T): all wavefront levels of one item by a team of `teamSize` CTAs (this CTA = `member`).
 // ---------------------------------------------------------------------------------------------
 __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* wbufAll, const TgItem* itp,
-                          unsigned long long* key, int member, int teamSize, int slotIdx, uint32_t& par) {
+                          unsigned long long* key, int member, int teamSize, int slotIdx) {
     tgStageItem(ctx, sm, Cs, wbufAll, itp, member == 0);
     tgMark(sm, 0);
     const int Ke = sm.sSlack >= 0 ? sm.sKe : 0;   // the islands' longest slices cannot cover L layers: infeasible at T
@@ -655,7 +634,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         for (int r = 1; r < Ke; ++r) {
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Wd, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Wd, r);
-            if (warp < nW) tgWarpLevel(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, par);
+            if (warp < nW) tgWarpLevel(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
             tgMark(sm, 3);
             if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();
@@ -673,7 +652,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
 __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
     const int widest = tgBinom[K][K >> 1];
     const int team = max(1, widest / (8 * ctx.nActiveWarps));
-    return min(max(int(gridDim.x) / team, 16), 64);
+    return min(max(int(gridDim.x) / team, 8), 64);   // measured at cfg4: 8 probes a round beat 16 (less speculation)
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -948,7 +927,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
     uint32_t* dyn = reinterpret_cast<uint32_t*>(tgDynSmem);
     uint32_t* Cs = dyn;
     uint32_t* wbufAll = dyn + ctx.csWords;
-    uint32_t epoch = 0, mbPar = 0;
+    uint32_t epoch = 0;
     TgCtrl* ctrl = ctx.ctrl;
     const int nCta = int(gridDim.x), b = int(blockIdx.x);
     if (threadIdx.x == 0) {
@@ -976,7 +955,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
                     __syncthreads();
                     const int it = sm.curItem;
                     if (it >= nItems) break;
-                    tgRunItem(ctx, sm, Cs, wbufAll, items + it, keys + it, 0, 1, b, mbPar);
+                    tgRunItem(ctx, sm, Cs, wbufAll, items + it, keys + it, 0, 1, b);
                 }
             }
         } else {
@@ -985,7 +964,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
             while (t + 1 < nItems && int((int64_t(t + 1) * nCta) / nItems) <= b) ++t;
             while (t > 0 && int((int64_t(t) * nCta) / nItems) > b) --t;
             const int start = int((int64_t(t) * nCta) / nItems), end = int((int64_t(t + 1) * nCta) / nItems);
-            tgRunItem(ctx, sm, Cs, wbufAll, items + t, keys + t, b - start, end - start, t, mbPar);
+            tgRunItem(ctx, sm, Cs, wbufAll, items + t, keys + t, b - start, end - start, t);
         }
         tgMark(sm, 0);
         tgGridBarrier(ctrl, epoch);
