@@ -12,6 +12,7 @@
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
 #define TG_MAX_EVAL 1024      // evaluated thresholds remembered per instance
 #define TG_MAX_WISH 64        // DPs per instance and round, upper bound
+#define TG_PROBE_FINAL 0x40000000   // flag in probe[]: final DP (keep every level, back-track)
 #define TG_EDONE 0x40000000   // flag in eIdx: every candidate between the previous evaluated point and this one is resolved
 #define TG_KEY_NONE 0xffffffffffffffffull
 
@@ -61,6 +62,7 @@ struct TgInstDev {
     int64_t incIter;
     uint32_t incMask;                     // island mask (original labels) of the incumbent's best state
     int32_t nEval, nProbe;
+    int32_t specIdx;                      // candidate of a speculative final DP already run (-1 = none)
     int32_t probe[TG_MAX_WISH];           // candidates to evaluate this round, ascending
     uint64_t fullWords;  // scratch words of a full-table DP of this instance (K islands alive)
 };

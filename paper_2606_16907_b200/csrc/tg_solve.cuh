@@ -702,7 +702,9 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem
     I.itemCnt = 0;
     if (I.phase == TG_PH_FINAL) { I.phase = TG_PH_DONE; return; }   // result written by the back-tracker
     int nf = 0;
-    for (int q = 0; q < cnt; ++q) {
+    int nRes = cnt;   // a speculative final DP, if any, is the last item: not a search result
+    if (nRes > 0 && (__ldcg(&itemsPrev[beg + nRes - 1].flags) & 1)) --nRes;
+    for (int q = 0; q < nRes; ++q) {
         const int tidx = __ldcg(&itemsPrev[beg + q].tidx);
         const unsigned long long key = __ldcg(keysPrev + beg + q);
         if (key == TG_KEY_NONE) { I.loInf = max(I.loInf, tidx); continue; }
@@ -719,10 +721,11 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem
     }
     I.nrun += cnt;
     if (I.phase == TG_PH_SWEEP) { I.next = __ldcg(&itemsPrev[beg + cnt - 1].tidx) + 1; return; }
+    if (nRes == 0) return;
     if (full || nf == 0) return;
     // merge the feasible results into the evaluated list (both ascending), from the back
     if (I.nEval + nf > TG_MAX_EVAL) { atomicExch(&ctx.ctrl->errFlag, 3); return; }
-    int e = I.nEval - 1, w = I.nEval + nf - 1, q = cnt - 1;
+    int e = I.nEval - 1, w = I.nEval + nf - 1, q = nRes - 1;
     while (q >= 0) {
         const unsigned long long key = __ldcg(keysPrev + beg + q);
         if (key == TG_KEY_NONE) { --q; continue; }
@@ -770,7 +773,9 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
         // unresolved stretches (left end exclusive, right end inclusive), at most 16 a round
         int sLo[16], sHi[16], ns = 0;
         long long total = 0;
-        for (int t = 1; t < I.nEval && ns < 15; ++t) {
+        bool truncated = false;
+        for (int t = 1; t < I.nEval; ++t) {
+            if (ns >= 15) { truncated = true; break; }
             const int ej = I.eIdx[t];
             if (ej & TG_EDONE) continue;
             const int a = I.eIdx[t - 1] & ~TG_EDONE;
@@ -797,6 +802,10 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
                 for (int q = 1; q <= share; ++q) I.probe[I.nProbe++] = sLo[s] + int(((long long)q * size + share - 1) / share);
                 budget -= share;
             }
+            // every unresolved candidate is probed this round: run the final DP at the incumbent alongside
+            // (speculation: it stands unless one of these probes takes the incumbent over)
+            I.specIdx = -1;
+            if (!truncated && total < W && I.nProbe == int(total)) { I.probe[I.nProbe++] = I.incIdx | TG_PROBE_FINAL; I.specIdx = I.incIdx; }
             return TG_PH_BNB;
         }
     }
@@ -809,7 +818,11 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
             return TG_PH_SWEEP;
         }
     }
-    if (I.phase == TG_PH_FINAL) { I.probe[0] = ctx.mode == 1 ? -1 : I.incIdx; I.nProbe = 1; return TG_PH_FINAL; }
+    if (I.phase == TG_PH_FINAL) {
+        if (ctx.mode == 0 && I.specIdx >= 0 && I.specIdx == I.incIdx) { I.phase = TG_PH_DONE; return TG_PH_DONE; }   // already back-tracked
+        I.probe[0] = ctx.mode == 1 ? -1 : I.incIdx; I.nProbe = 1;
+        return TG_PH_FINAL;
+    }
     return TG_PH_DONE;
 }
 
@@ -864,9 +877,10 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
             for (int q = 0; q < cnt; ++q) {
                 TgItem& it = items[pos + q];
                 it.inst = i;
-                it.tidx = I.probe[q];
+                const int pq = I.probe[q];
+                it.tidx = pq >= 0 ? (pq & ~TG_PROBE_FINAL) : -1;
                 it.T = it.tidx >= 0 ? I.cand[it.tidx] : ctx.dpT;
-                it.flags = kind == TG_PH_FINAL ? 1 : 0;
+                it.flags = (kind == TG_PH_FINAL || (pq >= 0 && (pq & TG_PROBE_FINAL))) ? 1 : 0;
             }
         }
     }
