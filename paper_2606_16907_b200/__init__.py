@@ -70,6 +70,10 @@ def lib():
     global _lib
     if _lib is None:
         if not os.path.exists(LIB_PATH):
+            # not a fallback: the same CUDA library, compiled on first use (nvcc, sm_100a); raises if that fails
+            from . import build as _build
+            _build.build()
+        if not os.path.exists(LIB_PATH):
             raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_16907_b200.build`")
         L = C.CDLL(LIB_PATH)
         vp, i32, i64, u32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32
