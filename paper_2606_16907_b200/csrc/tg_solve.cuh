@@ -724,7 +724,22 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem
     if (nRes == 0) return;
     if (full || nf == 0) return;
     // merge the feasible results into the evaluated list (both ascending), from the back
-    if (I.nEval + nf > TG_MAX_EVAL) { atomicExch(&ctx.ctrl->errFlag, 3); return; }
+    if (I.nEval + nf > TG_MAX_EVAL / 2) {
+        // compaction: an evaluated point whose stretches on both sides are resolved is no longer needed
+        // (the resolved flag of its right neighbour then covers both stretches; flags are never re-checked)
+        int w = 1;
+        for (int t = 1; t < I.nEval; ++t) {
+            const bool last = t + 1 == I.nEval;
+            const bool drop = !last && (I.eIdx[t] & TG_EDONE) && (I.eIdx[t + 1] & TG_EDONE);
+            if (!drop) { I.eIdx[w] = I.eIdx[t]; I.eF[w] = I.eF[t]; ++w; }
+        }
+        I.nEval = min(I.nEval, w);
+    }
+    if (I.nEval + nf > TG_MAX_EVAL) {   // cannot happen in practice; stop the search rather than loop
+        atomicExch(&ctx.ctrl->errFlag, 3);
+        I.phase = TG_PH_FINAL;
+        return;
+    }
     int e = I.nEval - 1, w = I.nEval + nf - 1, q = nRes - 1;
     while (q >= 0) {
         const unsigned long long key = __ldcg(keysPrev + beg + q);

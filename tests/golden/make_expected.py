@@ -3,7 +3,7 @@
 configs of BASELINE.json, which take the oracle minutes and so cannot be recomputed inside the test run.
 Calls ONLY oracle/ and the seeded input generator; never the CUDA path.
 
-    python tests/golden/make_expected.py cfg3 cfg4 cfg5      (cfg5 = a fixed sample of the 1024 seeds)
+    python tests/golden/make_expected.py cfg3 cfg4 cfg5 cfg3x cfg4x   (cfg5 = a fixed sample of the 1024 seeds)
 
 Also stores oracle.dp_at results at fixed quantile thresholds (single-DP parity for tg_dp_at)."""
 import json
@@ -46,6 +46,10 @@ def main():
             data = [one(gen.config3(), threads, True)]
         elif name == "cfg4":
             data = [one(gen.config4(), threads, True)]
+        elif name == "cfg3x":      # more seeds of the 70B-like config
+            data = [dict(one(gen.config3(s), threads, False), seed=s) for s in (1, 2, 3, 4)]
+        elif name == "cfg4x":      # a second MoE-like instance
+            data = [dict(one(gen.config4(1), threads, False), seed=1)]
         elif name == "cfg5":
             data = [dict(one(gen.config5_one(s), threads, False), seed=s) for s in CFG5_SEEDS]
         else:

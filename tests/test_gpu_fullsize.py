@@ -97,3 +97,19 @@ def test_cfg5_batch_1024(tg):
     for inst, g in zip(insts, res):
         assert int(g["iter_time_us"]) != I64MAX
         check_rescore(inst, g)
+
+
+def test_more_full_size_seeds(tg):
+    """Other seeds of the 70B-like and MoE-like configs (different island mixes, hence different threshold
+    windows and row windows) in one batch; stored oracle results (tests/golden/make_expected.py cfg3x cfg4x)."""
+    exp3 = {r["seed"]: r for r in expected("cfg3x")}
+    exp4 = {r["seed"]: r for r in expected("cfg4x")}
+    insts = [gen.config3(s) for s in exp3] + [gen.config4(s) for s in exp4]
+    exps = list(exp3.values()) + list(exp4.values())
+    hs = [tg.instance_from_inputs(i) for i in insts]
+    res = tg.tg_solve_batch(hs)
+    for h in hs:
+        h.destroy()
+    for inst, e, g in zip(insts, exps, res):
+        check(e["solve"], g, inst.name)
+        check_rescore(inst, g)
