@@ -291,16 +291,17 @@ __device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int 
                                             uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
     const bool member = (R >> lane) & 1u;
     const int p = __popc(R & ((1u << lane) - 1u));
-    uint32_t up = member ? uint32_t(sm.binom[lane & 15][p + 1]) : 0u;   // C(e, p+1): kept position
-    uint32_t dn = member ? uint32_t(sm.binom[lane & 15][p]) : 0u;       // C(e, p): moved down
-    uint32_t upIncl = up, dnIncl = dn;
+    // both sums stay below C(16,8) = 12870, so they share one register: low half "kept position", high half "moved down"
+    const uint32_t mine = member ? (uint32_t(sm.binom[lane & 15][p + 1]) | uint32_t(sm.binom[lane & 15][p]) << 16) : 0u;
+    uint32_t incl = mine;
 #pragma unroll
     for (int o = 1; o < 16; o <<= 1) {
-        const uint32_t a = __shfl_up_sync(0xffffffffu, upIncl, o), c = __shfl_up_sync(0xffffffffu, dnIncl, o);
-        if ((lane & 15) >= o) { upIncl += a; dnIncl += c; }
+        const uint32_t a = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((lane & 15) >= o) incl += a;
     }
-    const uint32_t dnTotal = __shfl_sync(0xffffffffu, dnIncl, 15);
-    if (member && lane < 16) rowOf[p] = ((upIncl - up) + (dnTotal - dnIncl)) * uint32_t(nk + 1) + uint32_t(lane - p);
+    const uint32_t total = __shfl_sync(0xffffffffu, incl, 15);
+    if (member && lane < 16)
+        rowOf[p] = (((incl - mine) & 0xffffu) + ((total - incl) >> 16)) * uint32_t(nk + 1) + uint32_t(lane - p);
     __syncwarp();
     const int cpShift = nbw > 32 ? 6 : chShift, CH = 1 << cpShift;   // chunks per row, rounded up to a power of two
     for (int w = lane; w < (r << cpShift); w += 32) {
@@ -483,10 +484,7 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
         asm volatile("cp.async.commit_group;" ::: "memory");   // possibly empty: keeps the group count uniform
         const uint32_t comp = ~R & keMask;
         if (lane < Ke && (comp >> lane & 1u)) kl[__popc(comp & ((1u << lane) - 1u))] = uint8_t(lane);
-        int capR = (R >> lane & 1u) ? myLen : 0;   // cap(R) = sum of maxlen over the members
-#pragma unroll
-        for (int o = 8; o > 0; o >>= 1) capR += __shfl_xor_sync(0xffffffffu, capR, o);
-        capR = __shfl_sync(0xffffffffu, capR, 0);
+        const int capR = int(__reduce_add_sync(0xffffffffu, (R >> lane & 1u) ? unsigned(myLen) : 0u));   // cap(R)
         asm volatile("cp.async.wait_group 1;" ::: "memory");   // this mask's rows have landed (the next mask's may be in flight)
         __syncwarp();
 
