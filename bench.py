@@ -192,9 +192,9 @@ def run_ours(args):
             plans += st.plans_dense
             states += st.states_live
             n_dp += st.n_dp
-            assert st.reserved[0] == 0, "solver error flag"
+            assert st.error_flag == 0, "solver error flag"
             cyc = [c + int(v) for c, v in zip(cyc, st.cyc)]
-            relax += int(st.reserved[1])
+            relax += int(st.relax_admissible)
         barrier()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     # ---- end to end: host tables -> create (H2D) -> solve -> host results (D2H) ----
@@ -225,7 +225,7 @@ def run_ours(args):
         line = {"metric": METRIC, "value": plans_all / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-                "config": {"workload": desc, "sweep": "full" if args.full_sweep else "windowed (exact stop rule)",
+                "config": {"workload": desc, "sweep": "full" if args.full_sweep else "exact branch-and-bound over thresholds",
                            "l2": "256 MB buffer written between timed steps", "instances_per_gpu": n,
                            "dps_per_step": ndp_all / args.steps / world,
                            "planning_ms_per_instance": total_ms / args.steps / n},
@@ -243,7 +243,7 @@ def run_ours(args):
                                      "achieved_Trelax_s": relax / args.steps / (km * 1e-3) / 1e12,
                                      "peak_Trelax_s": 148 * 64 * 1.965e9 / 1e12,
                                      "frac": relax / args.steps / (km * 1e-3) / (148 * 64 * 1.965e9)},
-                             "cta_cycle_shares": dict(zip(["stage", "tile_meta", "transfer_min", "minplus", "team_wait",
+                             "cta_cycle_shares": dict(zip(["stage", "unused1", "unused2", "dp_levels", "level_barrier_wait",
                                                            "grid_wait", "scheduler", "backtrack"],
                                                           [round(c / max(1, sum(cyc)), 4) for c in cyc]))}}
         if not args.no_cpu_baseline:

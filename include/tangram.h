@@ -84,7 +84,7 @@ typedef struct { /* one per instance, POD, 8-byte aligned, 224 bytes */
 } tg_result;
 
 enum { /* flags of tg_solve_batch_ex */
-    TG_SOLVE_DEFAULT = 0,   /* windowed sweep: lowest feasible T by search, exact stop rule */
+    TG_SOLVE_DEFAULT = 0,   /* exact branch-and-bound search over the candidate thresholds (DESIGN.md R-search) */
     TG_SOLVE_FULL_SWEEP = 1 /* run the DP at every candidate T (rate benchmark; same result)           */
 };
 
@@ -95,16 +95,17 @@ typedef struct { /* optional diagnostics of one tg_solve_batch_ex call, written 
     uint64_t n_rounds;       /* scheduler rounds                                               */
     uint64_t n_barriers;     /* grid-wide barriers executed                                    */
     uint64_t n_items_global_c; /* DPs whose cost tables did not fit in shared memory           */
-    uint64_t reserved[2];    /* [0] internal error flag (0 = none); [1] admissible relaxations executed:
-                                stage (c <= T) + transfer, summed over DPs                      */
-    uint64_t cyc[8];         /* SM cycles summed over CTAs (thread 0 of each): 0 cost-table staging,
-                                1 tile metadata, 2 transfer pre-minimum, 3 min-plus product, 4 team-barrier
-                                wait, 5 grid-barrier wait, 6 scheduler, 7 back-track                     */
+    uint64_t error_flag;     /* internal consistency flag of the solver, 0 = none                */
+    uint64_t relax_admissible; /* admissible relaxations executed: stage (c <= T) + transfer, summed over DPs */
+    uint64_t cyc[8];         /* SM cycles summed over CTAs (thread 0 of each): 0 cost-table staging, 3 DP levels
+                                (streaming over masks), 4 wait at the level barrier (team or CTA), 5 wait at the
+                                grid barrier between rounds, 6 scheduler, 7 back-track; 1, 2 unused         */
 } tg_solve_stats;
 
 /* tg_solve_batch — north_star "tg_solve_batch(instances, stream) -> best iteration time and plan".
- * Steps: cost-table loader, transfer table, candidate thresholds, DP at T=inf,
- * per-T popcount-wavefront DP, threshold-sweep reduction, plan back-tracker.
+ * Steps: cost-table loader, transfer table, candidate thresholds, exact threshold
+ * search with monotone bounds (in place of the T=inf lower-bound run), per-T popcount-wavefront DP,
+ * threshold-sweep reduction, plan back-tracker.
  *   instances   HOST array of n instance handles (all created on the current device)
  *   out         EITHER: n results.  DEVICE: written asynchronously on `cuda_stream`, valid after the
  *               stream is synchronised.  HOST: the call copies the results back and synchronises.

@@ -44,7 +44,7 @@ class TgResult(C.Structure):
 class TgSolveStats(C.Structure):
     _fields_ = [("n_dp", C.c_uint64), ("plans_dense", C.c_uint64), ("states_live", C.c_uint64),
                 ("n_rounds", C.c_uint64), ("n_barriers", C.c_uint64), ("n_items_global_c", C.c_uint64),
-                ("reserved", C.c_uint64 * 2), ("cyc", C.c_uint64 * 8)]
+                ("error_flag", C.c_uint64), ("relax_admissible", C.c_uint64), ("cyc", C.c_uint64 * 8)]
 
 
 RESULT_BYTES = C.sizeof(TgResult)

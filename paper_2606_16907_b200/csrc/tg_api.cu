@@ -273,8 +273,7 @@ tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cud
     TG_CUDA(cudaMemcpyAsync(out, W.outDev, sizeof(tg_result) * n, cudaMemcpyDefault, st));
     if (stats) {
         if (!isDevicePtr(stats)) sync = true;
-        // the error flag rides in reserved[0]
-        TG_CUDA(cudaMemcpyAsync(&W.ctx.ctrl->stats.reserved[0], &W.ctx.ctrl->errFlag, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+        TG_CUDA(cudaMemcpyAsync(&W.ctx.ctrl->stats.error_flag, &W.ctx.ctrl->errFlag, sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
         TG_CUDA(cudaMemcpyAsync(stats, &W.ctx.ctrl->stats, sizeof(tg_solve_stats), cudaMemcpyDefault, st));
     }
     static const bool dbg = getenv("TG_DEBUG") != nullptr;

@@ -207,9 +207,9 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     if (count) {   // statistics: admissible relaxations of this DP (stage + transfer)
         for (int o = 16; o > 0; o >>= 1) nAdm += __shfl_down_sync(0xffffffffu, nAdm, o);
         if (lane == 0 && nAdm && Ke > 0)
-            atomicAdd((unsigned long long*)&ctx.ctrl->stats.reserved[1], (unsigned long long)nAdm << (Ke - 1));
+            atomicAdd((unsigned long long*)&ctx.ctrl->stats.relax_admissible, (unsigned long long)nAdm << (Ke - 1));
         if (tid == 0 && Ke >= 2)
-            atomicAdd((unsigned long long*)&ctx.ctrl->stats.reserved[1], (unsigned long long)L * Ke * (Ke - 1) << (Ke - 2));
+            atomicAdd((unsigned long long*)&ctx.ctrl->stats.relax_admissible, (unsigned long long)L * Ke * (Ke - 1) << (Ke - 2));
     }
     __syncthreads();
 }
