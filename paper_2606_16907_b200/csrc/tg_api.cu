@@ -234,7 +234,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const int totalWords = W.dynSmem / 4;
     TgSolveCtx& c = W.ctx;
     memset(&c, 0, sizeof(c));
-    c.wbufWords = 2 * maxK * (maxLp + 12);
+    c.wbufWords = 2 * maxK * (maxLp + 16);
     c.nActiveWarps = std::min(TG_NT / 32, (totalWords * 3 / 4) / c.wbufWords);
     if (c.nActiveWarps < 1) return fail(TG_ERR_SHAPE, "shared memory too small for this instance shape");
     c.csWords = (totalWords - c.nActiveWarps * c.wbufWords) & ~3;

@@ -111,7 +111,7 @@ struct TgSolveCtx {
     int32_t mode;               // 0 = solve, 1 = single DP at dpT (tg_dp_at)
     uint32_t dpT;
     int32_t csWords;            // words of shared memory available for staged cost tables
-    int32_t wbufWords;          // words of warp-private shared memory: 2*Kmax rows of (Lp + 12)
+    int32_t wbufWords;          // words of warp-private shared memory: 2*Kmax rows of up to Lp + 16
     int32_t nActiveWarps;       // warps per CTA that stream masks (all of them unless L is huge)
 };
 

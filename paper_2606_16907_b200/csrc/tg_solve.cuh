@@ -156,7 +156,9 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         sm.sWindowed = (ctot >= L && wd < Lp) ? 1 : 0;
         sm.sWd = sm.sWindowed ? wd : Lp;
         uint32_t acc = 0;
-        for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += uint32_t((sm.dmaxK[kc] + 3) & ~3) * uint32_t(Lp); }
+        // + 4 words per island: tables of different islands start in different 16-byte bank groups, so the
+        // island groups of a warp do not collide when they read the same diagonal
+        for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += uint32_t((sm.dmaxK[kc] + 3) & ~3) * uint32_t(Lp) + 4u; }
         sm.useGlobalC = acc > uint32_t(ctx.csWords) ? 1 : 0;
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
     }
@@ -243,7 +245,7 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
 //           shared-memory buffer, one mask ahead of their use (double buffer, commit / wait_group)
 //   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[j][b]       lane = (4 consecutive b) x (k group)
 //   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]    lane = (4 consecutive a) x (k group)
-// Warp-private shared memory: rows of Wd + 12 words: [0, nk) the H rows (4 INF | H[b] at index
+// Warp-private shared memory: rows of Wd + 12 (+4 against bank conflicts) words: [0, nk) the H rows (4 INF | H[b] at index
 // b - lo4(R) | 8 INF), then two source buffers of r rows each.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
@@ -455,7 +457,10 @@ __device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& 
 __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
                             uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int Lp = sm.sLp, Wd = sm.sWd, HS = Wd + 12, nbw = Wd >> 2, nk = Ke - r;
+    const int Lp = sm.sLp, Wd = sm.sWd, nbw = Wd >> 2, nk = Ke - r;
+    // row stride = 4 (mod 8) words: consecutive rows start in different 16-byte bank groups (rows are read by
+    // several island groups at the same chunk offset)
+    const int HS = Wd + 12 + (((Wd + 12) & 7) == 0 ? 4 : 0);
     const int nMasks = sm.binom[Ke][r];
     const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
     if (lo >= hi) return;
