@@ -283,6 +283,16 @@ tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cud
         TG_CUDA(cudaStreamSynchronize(st));
         const int nr = int(std::min<uint64_t>(hc.stats.n_rounds, 256));
         fprintf(stderr, "[tg] rounds=%d dps=%llu\n", nr, (unsigned long long)hc.stats.n_dp);
+        {
+            static TgInstDev hi;
+            TG_CUDA(cudaMemcpy(&hi, W.inst, sizeof(TgInstDev), cudaMemcpyDeviceToHost));
+            std::vector<int32_t> e(hi.nEval > 0 ? hi.nEval : 1);
+            TG_CUDA(cudaMemcpy(e.data(), hi.eIdx, sizeof(int32_t) * e.size(), cudaMemcpyDeviceToHost));
+            fprintf(stderr, "[tg] inst0: ncand=%d lbIdx=%d lowestFeasible=%d incIdx=%d nEval=%d evaluated:", hi.ncand, hi.lbIdx,
+                    hi.nEval > 0 ? (e[0] & ~TG_EDONE) : -1, hi.incIdx, hi.nEval);
+            for (int q = 0; q < hi.nEval && q < 48; ++q) fprintf(stderr, " %d", e[q] & ~TG_EDONE);
+            fprintf(stderr, "\n");
+        }
         for (int r = 0; r < nr; ++r)
             fprintf(stderr, "[tg]  round %3d items %5d  %8.1f us\n", r, hc.roundItems[r],
                     r + 1 < nr ? double(hc.roundNs[r + 1] - hc.roundNs[r]) * 1e-3 : 0.0);

@@ -802,24 +802,24 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
             total += sHi[ns] - sLo[ns];
             ++ns;
         }
-        {   // above the last evaluated point only the trivial bound f >= 0 is known
+        int topEnd = -1;
+        {   // above the last evaluated point only the trivial bound f >= 0 is known: probe just the right end of
+            // that stretch; once it is evaluated the stretch gets a real bound and shrinks
             const int a = I.eIdx[I.nEval - 1] & ~TG_EDONE;
-            if (a < n - 1 && tgBeats(I, 0, a + 1)) {
-                sLo[ns] = a; sHi[ns] = tgLastBeating(I, 0, a + 1, n - 1);
-                total += sHi[ns] - sLo[ns];
-                ++ns;
-            }
+            if (a < n - 1 && tgBeats(I, 0, a + 1)) topEnd = tgLastBeating(I, 0, a + 1, n - 1);
         }
-        if (ns == 0) I.phase = TG_PH_FINAL;
+        if (ns == 0 && topEnd < 0) I.phase = TG_PH_FINAL;
         else {
-            int budget = W;
+            int budget = topEnd >= 0 ? W - 1 : W;
+            const int budget0 = budget;
             for (int s = 0; s < ns && budget > 0; ++s) {
                 const int size = sHi[s] - sLo[s];
-                int share = int(max(1ll, (long long)W * size / total));
+                int share = int(max(1ll, (long long)budget0 * size / max(total, 1ll)));
                 share = min(min(share, size), budget);
                 for (int q = 1; q <= share; ++q) I.probe[I.nProbe++] = sLo[s] + int(((long long)q * size + share - 1) / share);
                 budget -= share;
             }
+            if (topEnd >= 0) { I.probe[I.nProbe++] = topEnd; total += W; }   // (total += W: not every candidate is probed)
             // every unresolved candidate is probed this round: run the final DP at the incumbent alongside
             // (speculation: it stands unless one of these probes takes the incumbent over)
             I.specIdx = -1;
