@@ -44,6 +44,7 @@ struct DeviceState {
     uint16_t* rankOf = nullptr;
 };
 std::mutex g_mu;
+int g_gallopMax = [] { const char* e = getenv("TG_GALLOP_MAX"); int v = e ? atoi(e) : 8; return v < 1 ? 1 : (v > 16 ? 16 : v); }();
 // DPs per instance and scheduler round (speculation width of the threshold search / sweep)
 int g_wishMax = [] { const char* e = getenv("TG_WISH_MAX"); int v = e ? atoi(e) : 64; return v < 1 ? 1 : (v > TG_MAX_WISH ? TG_MAX_WISH : v); }();
 DeviceState g_dev[64];
@@ -245,6 +246,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.slotWords = slotWords; c.nSlots = nSlots;
     c.slotBar = reinterpret_cast<uint32_t*>(W.base + oBar);
     c.wishMax = g_wishMax;
+    c.gallopMax = g_gallopMax;
     c.ctrl = reinterpret_cast<TgCtrl*>(W.base + oCtrl);
     c.rankOf = D->rankOf;
 

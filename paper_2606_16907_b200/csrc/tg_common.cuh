@@ -103,6 +103,7 @@ struct TgSolveCtx {
     uint64_t slotWords;         // one slot holds every level of the largest instance of the batch
     int32_t nSlots;             // <= gridDim.x; a slot belongs to one team (team mode) or one CTA (solo mode)
     int32_t wishMax;            // DPs per instance and round, upper bound
+    int32_t gallopMax;          // probes of one galloping round
     uint32_t* slotBar;          // [nSlots] arrival counters of the team barriers, zeroed every round
     TgCtrl* ctrl;
     tg_result* out;

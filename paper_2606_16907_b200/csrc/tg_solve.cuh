@@ -769,7 +769,7 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
             if (I.loInf >= n - 1) { tgWriteInfeasible(ctx, I, i); return TG_PH_DONE; }
             // galloping: loInf + gstep, + 2 gstep, ... ; at most 8 probes a round, the step keeps doubling
             int step = I.gstep;
-            const int nmax = min(W, 8);
+            const int nmax = min(W, ctx.gallopMax);
             while (I.nProbe < nmax) {
                 const int c = min(int64_t(n - 1), int64_t(I.loInf) + step);
                 I.probe[I.nProbe++] = c;
