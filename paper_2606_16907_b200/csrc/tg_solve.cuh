@@ -651,11 +651,12 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
 }
 
 // DPs per round an instance with K islands should run: enough that every warp of a team (grid / DPs)
-// has about eight masks at the widest level, i.e. few warps idle at the thin levels.
+// has about eight masks at the widest level, but few enough that little of a round is speculation:
+// measured best at 8 (cfg4, K = 16) to 10-12 (cfg3, K = 12) probes a round.
 __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
     const int widest = tgBinom[K][K >> 1];
     const int team = max(1, widest / (8 * ctx.nActiveWarps));
-    return min(max(int(gridDim.x) / team, 8), 64);   // measured at cfg4: 8 probes a round beat 16 (less speculation)
+    return min(max(int(gridDim.x) / team, 8), 12);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -881,7 +882,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
         int cnt = 0, kind = TG_PH_DONE;
         if (i < nInst && ctx.inst[i].phase != TG_PH_DONE) {
             TgInstDev& I = ctx.inst[i];
-            kind = tgPlanInstance(ctx, I, i, min(capAll, tgWish(ctx, I.K)), full);
+            kind = tgPlanInstance(ctx, I, i, full ? capAll : min(capAll, tgWish(ctx, I.K)), full);   // a full sweep has no speculation
             cnt = I.nProbe;
         }
         uint32_t tot;
