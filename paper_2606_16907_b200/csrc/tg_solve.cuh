@@ -890,7 +890,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
         carry += tot;
         if (cnt > 0) {
             TgInstDev& I = ctx.inst[i];
-            if (pos + cnt > TG_MAX_ITEMS) cnt = 0;   // cannot happen: cnt <= capAll <= TG_MAX_ITEMS / nActive
+            if (pos + cnt > TG_MAX_ITEMS) { cnt = 0; I.specIdx = -1; }   // more active instances than items: wait a round
             I.itemBeg = int(pos); I.itemCnt = cnt;
             if (cnt > 0) atomicMax(&sm.iTmp[1], int(pos) + cnt);
             for (int q = 0; q < cnt; ++q) {

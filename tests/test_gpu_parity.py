@@ -153,3 +153,11 @@ def test_threshold_search_stress(tg, style):
         same(o, g, inst.name)
     for inst, o in list(zip(insts, want))[:12]:
         same(o, solve_all(tg, [inst])[0], inst.name + " alone")
+
+
+def test_more_instances_than_items_per_round(tg):
+    """9000 instances in one call: more active instances than the scheduler's 8192 items per round."""
+    insts = [gen.random_small(s + 40_000, Lmax=5, Kmax=3, Pmax=2, style=STYLES[s % 5]) for s in range(9000)]
+    res = solve_all(tg, insts)
+    for inst, g in zip(insts, res):
+        same(oracle.solve(inst), g, inst.name)
