@@ -74,11 +74,9 @@ struct TgItem {
     int32_t inst;
     uint32_t T;          // threshold actually applied (TG_TINF for infinity)
     int32_t tidx;        // index into cand, -1 = explicit T (infinity / tg_dp_at)
-    uint16_t alive;      // islands with some admissible slice at T (original labels)
-    uint8_t Ke;          // popcount(alive)
+    uint8_t Ke;          // islands with some admissible slice at T (written by the CTA that runs the item)
     uint8_t flags;       // bit0: keep every level (back-track follows)
     uint8_t isl[TG_MAX_K];  // compact label -> original island
-    uint64_t bufWords;   // words of one ping-pong half (0 when every level is kept)
 };
 
 struct TgCtrl {

@@ -121,16 +121,37 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     unsigned nAdm = 0;   // admissible (a, b, k) cost entries with b <= L-1 seen by this thread
     const int tid = threadIdx.x, lane = tid & 31;
     const TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
-    const int L = I.L, Lp = I.Lp, Ke = __ldcg(&itp->Ke), nb4 = Lp >> 2;
+    const int L = I.L, Lp = I.Lp, nb4 = Lp >> 2;
     const uint32_t T = __ldcg(&itp->T);
-    if (tid == 0) { sm.sL = L; sm.sLp = Lp; sm.sKe = Ke; sm.sT = T; sm.sInst = __ldcg(&itp->inst); }
-    if (tid < TG_MAX_K) sm.isl[tid] = __ldcg(&itp->isl[tid]);
+    // geometry of the item: the islands with some admissible slice at T, in compact labels.  The final
+    // DP only needs the islands of the optimal mask S*: S* is the lowest mask attaining the optimum at
+    // T*, so no subset of it ties, and the back-track never leaves its subsets.
+    if (tid < 32) {
+        const uint32_t allow = ((__ldcg(&itp->flags) & 1) && ctx.mode == 0) ? I.incMask : 0xffffu;
+        const bool ok = lane < I.K && I.cminAll[lane] <= T && (allow >> lane & 1u);
+        const uint32_t bal = __ballot_sync(0xffffffffu, ok);
+        if (lane < TG_MAX_K) sm.isl[lane] = 0;
+        __syncwarp();
+        if (ok) sm.isl[__popc(bal & ((1u << lane) - 1u))] = uint8_t(lane);
+        if (lane == 0) { sm.sL = L; sm.sLp = Lp; sm.sKe = __popc(bal); sm.sT = T; sm.sInst = __ldcg(&itp->inst); }
+    }
+    __syncthreads();
+    const int Ke = sm.sKe;
+    if (count) {   // member 0 publishes the geometry (the scheduler maps the best state's mask back through isl) and counts
+        TgItem* itw = const_cast<TgItem*>(itp);
+        if (tid < TG_MAX_K) itw->isl[tid] = sm.isl[tid];
+        if (tid == 0) {
+            itw->Ke = uint8_t(Ke);
+            atomicAdd((unsigned long long*)&ctx.ctrl->stats.plans_dense, (unsigned long long)I.NS * I.K << (I.K - 1));
+            if (Ke) atomicAdd((unsigned long long*)&ctx.ctrl->stats.states_live, (unsigned long long)L * Ke << (Ke - 1));
+        }
+    }
     if (tid < Ke * Ke) {
         const int kc = tid / Ke, jc = tid - kc * Ke;
-        sm.xS[kc][jc] = I.x[int(__ldcg(&itp->isl[kc])) * TG_MAX_K + int(__ldcg(&itp->isl[jc]))];
+        sm.xS[kc][jc] = I.x[int(sm.isl[kc]) * TG_MAX_K + int(sm.isl[jc])];
     }
     if (tid < Ke) {  // widest diagonal with an admissible entry: sufMin is non-decreasing in d
-        const uint32_t* sf = I.sufMin + size_t(__ldcg(&itp->isl[tid])) * (L + 2);
+        const uint32_t* sf = I.sufMin + size_t(sm.isl[tid]) * (L + 2);
         int lo = 0, hi = L - 1;  // answer in [0, L-1]; 0 = none
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
@@ -139,7 +160,7 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         sm.dmaxK[tid] = lo;
     }
     if (tid >= 32 && tid < 32 + Ke) {  // longest admissible slice at any position (b <= L)
-        const uint32_t* sf = I.sufMinAll + size_t(__ldcg(&itp->isl[tid - 32])) * (L + 2);
+        const uint32_t* sf = I.sufMinAll + size_t(sm.isl[tid - 32]) * (L + 2);
         int lo = 0, hi = L;
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
@@ -530,12 +551,12 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
 __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgItem* itp, unsigned long long key, const uint32_t* slot) {
     const int lane = threadIdx.x & 31;
     TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
-    const int L = I.L, K = I.K, Ke = __ldcg(&itp->Ke);
+    const int L = I.L, K = I.K, Ke = sm.sKe;
     const uint32_t T = __ldcg(&itp->T);
     tg_result* out = ctx.out + __ldcg(&itp->inst);
     uint8_t isl[TG_MAX_K];
 #pragma unroll
-    for (int e = 0; e < TG_MAX_K; ++e) isl[e] = __ldcg(&itp->isl[e]);
+    for (int e = 0; e < TG_MAX_K; ++e) isl[e] = sm.isl[e];
     const int64_t Trep = (T == TG_TINF) ? int64_t(TG_INF) : int64_t(T);
     if (key == TG_KEY_NONE) {
         if (lane == 0) {
@@ -626,7 +647,12 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     tgMark(sm, 0);
     const int Ke = sm.sSlack >= 0 ? sm.sKe : 0;   // the islands' longest slices cannot cover L layers: infeasible at T
     const int Wd = sm.sWd, nW = ctx.nActiveWarps, warp = threadIdx.x >> 5;
-    const uint64_t bufWords = __ldcg(&itp->bufWords);
+    uint64_t bufWords = 0;   // words of one ping-pong half; 0 = keep every level (a back-track follows)
+    if (Ke > 0 && !(__ldcg(&itp->flags) & 1)) {
+        uint32_t mx = 1;
+        for (int q = 0; q < Ke; ++q) mx = max(mx, tgLevelRows(Ke, q));
+        bufWords = uint64_t(mx) * uint64_t(sm.sLp);
+    }
     uint32_t* slot = ctx.scratch + uint64_t(slotIdx) * ctx.slotWords;
     uint32_t* bar = ctx.slotBar + slotIdx;
     uint32_t* wbuf = wbufAll + size_t(warp) * ctx.wbufWords;
@@ -677,7 +703,7 @@ __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
 // could candidate c, whose sum is at least lbF, still beat the incumbent?
 __device__ __forceinline__ bool tgBeats(const TgInstDev& I, int64_t lbF, int c) {
     if (I.incIdx < 0) return true;
-    const int64_t lb = lbF + int64_t(I.m - 1) * int64_t(I.cand[c]);
+    const int64_t lb = lbF + int64_t(I.m - 1) * int64_t(__ldg(I.cand + c));   // cand is read-only during the solve
     return lb < I.incIter || (lb == I.incIter && c < I.incIdx);
 }
 
@@ -906,31 +932,8 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     __syncthreads();
     const int nIt = sm.iTmp[1];
 
-    // ---- C: per-item geometry, statistics ------------------------------------------------------------
-    unsigned long long dense = 0, live = 0;
-    for (int idx = tid; idx < nIt; idx += TG_NT) {
-        TgItem& it = items[idx];
-        const TgInstDev& I = ctx.inst[it.inst];
-        uint32_t alive = 0; int Ke = 0;
-        // the final DP only needs the islands of the optimal mask S*: S* is the lowest mask attaining
-        // the optimum at T*, so no subset of it ties, and the back-track never leaves its subsets
-        const uint32_t allow = ((it.flags & 1) && ctx.mode == 0) ? I.incMask : 0xffffu;
-        for (int k = 0; k < I.K; ++k)
-            if (I.cminAll[k] <= it.T && (allow >> k & 1u)) { alive |= 1u << k; it.isl[Ke++] = uint8_t(k); }
-        for (int e = Ke; e < TG_MAX_K; ++e) it.isl[e] = 0;
-        it.alive = uint16_t(alive); it.Ke = uint8_t(Ke);
-        it.bufWords = 0;
-        if (Ke > 0 && !(it.flags & 1)) {
-            uint32_t mx = 1;
-            for (int q = 0; q < Ke; ++q) mx = max(mx, tgLevelRows(Ke, q));
-            it.bufWords = uint64_t(mx) * uint64_t(I.Lp);
-        }
-        keys[idx] = TG_KEY_NONE;
-        dense += (unsigned long long)I.NS * I.K << (I.K - 1);
-        if (Ke) live += (unsigned long long)I.L * Ke << (Ke - 1);
-    }
-    if (dense) atomicAdd(&sm.llTmp[0], dense);
-    if (live) atomicAdd(&sm.llTmp[1], live);
+    // (the geometry of an item -- islands alive at its T -- is worked out by the CTAs that run it)
+    for (int idx = tid; idx < nIt; idx += TG_NT) keys[idx] = TG_KEY_NONE;
     for (int s = tid; s < ctx.nSlots; s += TG_NT) ctx.slotBar[s] = 0;
     __syncthreads();
     if (tid == 0) {
@@ -943,8 +946,6 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
         ctrl->nItems[par] = nIt;
         ctrl->queue[par] = 0;
         ctrl->stats.n_dp += uint64_t(nIt);
-        ctrl->stats.plans_dense += sm.llTmp[0];
-        ctrl->stats.states_live += sm.llTmp[1];
         ctrl->stats.n_rounds += 1;
         if (nIt == 0) ctrl->done = 1;   // every remaining instance was found infeasible while planning
     }
