@@ -14,6 +14,7 @@ import numpy as np
 
 _DIR = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_DIR, "tangram_oracle.cpp")
+_SRC_DEPTH = os.path.join(_DIR, "tangram_oracle_depth.cpp")   # NEXT-1 variant, separate translation unit
 _SO = os.path.join(_DIR, "libtangram_oracle.so")
 MAXK = 16
 INF = 1 << 30
@@ -21,9 +22,9 @@ INT64_MAX = (1 << 63) - 1
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_DEPTH)):
         tmp = _SO + f".tmp{os.getpid()}"
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", tmp, _SRC])
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", tmp, _SRC, _SRC_DEPTH])
         os.replace(tmp, _SO)
     return _SO
 
@@ -141,6 +142,27 @@ def prune(inst, mode: int = 0, threshold: int = 0):
                     C.c_int(mode), C.c_int64(threshold), counts.ctypes.data_as(_I64P))
     out.time_us = t
     return out, counts
+
+
+def _args_depth(inst):
+    keep, a = _args(inst)
+    am = np.ascontiguousarray(inst.actmem_mb, dtype=np.int32)
+    return (keep, am), a[:6] + (_p32(am),) + a[6:]
+
+
+def solve_depth(inst) -> Result:
+    """NEXT-1: depth-aware activation memory (inst.actmem_mb [NS,K,P])."""
+    keep, a = _args_depth(inst)
+    r = _Res()
+    lib().orc_depth_solve(*a, C.byref(r))
+    return _conv(r)
+
+
+def bruteforce_depth(inst) -> Result:
+    keep, a = _args_depth(inst)
+    r = _Res()
+    lib().orc_depth_bruteforce(*a, C.byref(r))
+    return _conv(r)
 
 
 def hw_threads() -> int:

@@ -1,0 +1,268 @@
+// TEST INFRASTRUCTURE — NOT PART OF THE PRODUCT PATH.
+//
+// CPU oracle for SURVEY.md §8(f) NEXT-1: depth-aware activation memory under 1F1B
+// (PAPER.md:246 "earlier stages hold more in-flight activations", :248-250, :258(i) "request a plan
+// until it is no longer feasible", :324).  Separate translation unit: the core oracle
+// (tangram_oracle.cpp) and its pins stay untouched.  Shares no code with the CUDA library.
+//
+// Model (reading N1): a stage followed by r later stages holds q = r + 1 microbatches in
+// flight, so intra-slice plan p of (slice, island k) is feasible at depth q iff
+//     mem_mb[e] + q * actmem_mb[e] <= cap_mb[k]                                   (int64)
+// and the stage's time is  c_q[a][b][k] = min over feasible p of time (ties -> lowest p).
+// Everything else is the core definition: plan = stages tiling [0,L) on distinct islands,
+// sum = sum c_q + sum x, T = max c_q, iter = sum + (m-1) T, result = argmin of
+// (iter, T, mask, k_0, b_0, k_1, b_1, ...).  Stage i of an n-stage plan has q = n - i.
+//
+// Pins (tests/test_oracle_depth.py): orc_depth_solve == orc_depth_bruteforce (literal enumeration)
+// on thousands of tiny instances; actmem = 0 reproduces the core oracle bit for bit; raising actmem
+// never improves the optimum; a plan re-scored from the raw tables with the depth rule reproduces
+// (sum, T, iter).
+
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <thread>
+#include <vector>
+
+namespace {
+
+constexpr int64_t INF = int64_t(1) << 30;
+constexpr int32_t INVALID = 0x7fffffff;
+constexpr int64_t TIME_MAX = int64_t(1) << 25;
+constexpr int MAXK = 16;
+
+struct Inst {
+    int L, K, P, m;
+    const int32_t *time_us, *mem_mb, *actmem_mb, *cap_mb, *bw_gbps;
+    int act_mb;
+    int NS() const { return L * (L + 1) / 2; }
+};
+
+inline int sidx(int L, int a, int b) { return a * (2 * L - a + 1) / 2 + (b - a - 1); }
+
+struct Reduced {
+    std::vector<int64_t> c;     // [K+1][NS][K]: c[q] for depth q = 1..K (index 0 unused)
+    std::vector<int32_t> argp;  // same shape, -1 = none
+    std::vector<int64_t> x;     // [K][K]
+    int NS, K;
+    int64_t C(int q, int s, int k) const { return c[(size_t(q) * NS + s) * K + k]; }
+    int32_t A(int q, int s, int k) const { return argp[(size_t(q) * NS + s) * K + k]; }
+};
+
+Reduced reduce_tables(const Inst& I) {
+    Reduced R;
+    const int NS = I.NS(), K = I.K, P = I.P;
+    R.NS = NS; R.K = K;
+    R.c.assign(size_t(K + 1) * NS * K, INF);
+    R.argp.assign(size_t(K + 1) * NS * K, -1);
+    for (int q = 1; q <= K; ++q)
+        for (int s = 0; s < NS; ++s)
+            for (int k = 0; k < K; ++k)
+                for (int p = 0; p < P; ++p) {
+                    const size_t e = (size_t(s) * K + k) * P + p;
+                    if (I.time_us[e] == INVALID) continue;
+                    if (int64_t(I.mem_mb[e]) + int64_t(q) * int64_t(I.actmem_mb[e]) > int64_t(I.cap_mb[k])) continue;
+                    const size_t o = (size_t(q) * NS + s) * K + k;
+                    if (int64_t(I.time_us[e]) < R.c[o]) { R.c[o] = I.time_us[e]; R.argp[o] = p; }   // strict: lowest p
+                }
+    R.x.assign(size_t(K) * K, 0);
+    for (int j = 0; j < K; ++j)
+        for (int k = 0; k < K; ++k) {
+            if (j == k) continue;
+            const int64_t num = int64_t(I.act_mb) * 1000, den = I.bw_gbps[j * K + k];
+            int64_t v = (num + den - 1) / den;
+            if (v > TIME_MAX) v = INF;
+            R.x[size_t(j) * K + k] = v;
+        }
+    return R;
+}
+
+std::vector<int64_t> candidates(const Reduced& R) {
+    std::vector<int64_t> v;
+    for (int64_t c : R.c) if (c < INF) v.push_back(c);
+    std::sort(v.begin(), v.end());
+    v.erase(std::unique(v.begin(), v.end()), v.end());
+    return v;
+}
+
+inline int64_t sat(int64_t v) { return v >= INF ? INF : v; }
+
+struct DP {
+    int L, K;
+    std::vector<int32_t> g, h;
+    std::vector<uint8_t> gb, hj;
+    size_t at(int a, uint32_t S, int k) const { return (size_t(S) * K + k) * (L + 1) + a; }
+};
+struct Top { int64_t best; uint32_t S; int k; };
+
+// The core recurrence with one change: the first stage of a suffix that uses the islands S has
+// depth q = popcount(S) and takes its cost from c_q.
+Top run_dp(const Inst& I, const Reduced& R, int64_t T, DP& D, bool keep) {
+    const int L = I.L, K = I.K;
+    const uint32_t NM = 1u << K;
+    D.L = L; D.K = K;
+    D.g.assign(size_t(NM) * K * (L + 1), int32_t(INF));
+    D.h.assign(size_t(NM) * K * (L + 1), int32_t(INF));
+    if (keep) { D.gb.assign(D.g.size(), 0); D.hj.assign(D.g.size(), 0); }
+    for (int d = 1; d <= K; ++d) {
+        if (d >= 2)
+            for (uint32_t Rm = 1; Rm < NM; ++Rm) {
+                if (__builtin_popcount(Rm) != d - 1) continue;
+                for (int k = 0; k < K; ++k) {
+                    if (Rm >> k & 1) continue;
+                    for (int b = 1; b < L; ++b) {
+                        int64_t best = INF; int bj = 0;
+                        for (int j = 0; j < K; ++j) {
+                            if (!(Rm >> j & 1)) continue;
+                            const int64_t v = sat(R.x[size_t(k) * K + j] + D.g[D.at(b, Rm, j)]);
+                            if (v < best) { best = v; bj = j; }
+                        }
+                        D.h[D.at(b, Rm, k)] = int32_t(best);
+                        if (keep) D.hj[D.at(b, Rm, k)] = uint8_t(bj);
+                    }
+                }
+            }
+        for (uint32_t S = 1; S < NM; ++S) {
+            if (__builtin_popcount(S) != d) continue;
+            for (int k = 0; k < K; ++k) {
+                if (!(S >> k & 1)) continue;
+                const uint32_t Rm = S ^ (1u << k);
+                for (int a = L - 1; a >= 0; --a) {
+                    int64_t best = INF; int bb = 0;
+                    for (int b = a + 1; b <= L; ++b) {
+                        const int64_t cv = R.C(d, sidx(L, a, b), k);      // depth q = d = popcount(S)
+                        if (cv >= INF || cv > T) continue;
+                        int64_t cand;
+                        if (b == L) cand = (Rm == 0) ? cv : INF;
+                        else cand = (Rm == 0) ? INF : sat(cv + D.h[D.at(b, Rm, k)]);
+                        if (cand < best) { best = cand; bb = b; }
+                    }
+                    D.g[D.at(a, S, k)] = int32_t(best);
+                    if (keep) D.gb[D.at(a, S, k)] = uint8_t(bb);
+                }
+            }
+        }
+    }
+    Top t{INF, 0, 0};
+    for (uint32_t S = 1; S < NM; ++S)
+        for (int k = 0; k < K; ++k)
+            if ((S >> k & 1) && D.g[D.at(0, S, k)] < t.best) t = Top{D.g[D.at(0, S, k)], S, k};
+    return t;
+}
+
+}  // namespace
+
+extern "C" {
+
+struct orc_result {   // same layout as the core oracle's
+    int64_t iter_time_us, sum_us, bottleneck_us;
+    int32_t n_stages;
+    uint32_t island_mask;
+    int32_t n_dp_run, n_candidates;
+    int32_t stage_begin[MAXK], stage_island[MAXK], stage_plan[MAXK];
+};
+
+static void set_infeasible(orc_result* o) { std::memset(o, 0, sizeof(*o)); o->iter_time_us = INT64_MAX; }
+
+// Full ascending sweep with the exact stop rule f_inf + (m-1)T >= incumbent, then a
+// choice-keeping run at T* and the back-track.
+int orc_depth_solve(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                    const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
+    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb};
+    Reduced R = reduce_tables(I);
+    std::vector<int64_t> cand = candidates(R);
+    set_infeasible(out);
+    out->n_candidates = int(cand.size());
+    DP D0;
+    const Top tinf = run_dp(I, R, INF, D0, false);
+    if (tinf.best >= INF) return 0;
+    bool have = false; int64_t best_iter = 0, best_T = 0; int n_dp = 0;
+    for (int64_t T : cand) {
+        if (have && tinf.best + int64_t(m - 1) * T >= best_iter) break;
+        DP D; ++n_dp;
+        const Top t = run_dp(I, R, T, D, false);
+        if (t.best >= INF) continue;
+        const int64_t it = t.best + int64_t(m - 1) * T;
+        if (!have || it < best_iter) { have = true; best_iter = it; best_T = T; }
+    }
+    DP D;
+    const Top t = run_dp(I, R, best_T, D, true);
+    out->iter_time_us = best_iter; out->sum_us = t.best; out->bottleneck_us = best_T;
+    out->island_mask = t.S; out->n_dp_run = n_dp;
+    int a = 0, k = t.k, n = 0; uint32_t S = t.S;
+    while (true) {
+        const int b = D.gb[D.at(a, S, k)];
+        out->stage_begin[n] = a; out->stage_island[n] = k;
+        out->stage_plan[n] = R.A(__builtin_popcount(S), sidx(L, a, b), k);
+        ++n;
+        if (b == L) break;
+        const uint32_t Rm = S ^ (1u << k);
+        const int j = D.hj[D.at(b, Rm, k)];
+        a = b; S = Rm; k = j;
+    }
+    out->n_stages = n;
+    return 0;
+}
+
+// Literal enumeration: every cut set and every ordered choice of distinct islands; the depth of
+// stage i is known once the plan is complete (q = n - i).
+namespace {
+struct BF {
+    const Inst* I; const Reduced* R;
+    std::vector<int64_t> bestkey; bool have = false;
+    std::vector<int> ks, bs;
+    int64_t n_plans = 0;
+    void leaf() {
+        const int L = I->L, n = int(ks.size());
+        int64_t sum = 0, T = 0; uint32_t mask = 0;
+        int a = 0;
+        for (int i = 0; i < n; ++i) {
+            const int64_t cv = R->C(n - i, sidx(L, a, bs[i]), ks[i]);
+            if (cv >= INF) return;
+            sum += cv; T = std::max(T, cv); mask |= 1u << ks[i];
+            if (i + 1 < n) { const int64_t xs = R->x[size_t(ks[i]) * I->K + ks[i + 1]]; if (xs >= INF) return; sum += xs; }
+            a = bs[i];
+        }
+        ++n_plans;
+        std::vector<int64_t> key{sum + int64_t(I->m - 1) * T, T, int64_t(mask)};
+        for (int i = 0; i < n; ++i) { key.push_back(ks[i]); key.push_back(bs[i]); }
+        if (!have || key < bestkey) { have = true; bestkey = key; }
+    }
+    void rec(int a, uint32_t used) {
+        if (a == I->L) { leaf(); return; }
+        for (int k = 0; k < I->K; ++k) {
+            if (used >> k & 1) continue;
+            for (int b = a + 1; b <= I->L; ++b) {
+                ks.push_back(k); bs.push_back(b);
+                rec(b, used | (1u << k));
+                ks.pop_back(); bs.pop_back();
+            }
+        }
+    }
+};
+}  // namespace
+
+int orc_depth_bruteforce(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                         const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
+    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb};
+    Reduced R = reduce_tables(I);
+    BF bf; bf.I = &I; bf.R = &R;
+    bf.rec(0, 0);
+    set_infeasible(out);
+    if (!bf.have) return 0;
+    out->iter_time_us = bf.bestkey[0]; out->bottleneck_us = bf.bestkey[1];
+    out->island_mask = uint32_t(bf.bestkey[2]);
+    out->sum_us = bf.bestkey[0] - int64_t(m - 1) * bf.bestkey[1];
+    const int n = int(bf.bestkey.size() - 3) / 2;
+    out->n_stages = n;
+    int a = 0;
+    for (int i = 0; i < n; ++i) {
+        const int k = int(bf.bestkey[3 + 2 * i]), b = int(bf.bestkey[4 + 2 * i]);
+        out->stage_begin[i] = a; out->stage_island[i] = k;
+        out->stage_plan[i] = R.A(n - i, sidx(L, a, b), k);
+        a = b;
+    }
+    return 0;
+}
+
+}  // extern "C"

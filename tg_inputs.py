@@ -78,11 +78,13 @@ class Instance:
     bw_gbps: np.ndarray       # [K, K] int32 sender-major
     act_mb: int
     meta: dict = field(default_factory=dict)
+    actmem_mb: np.ndarray = None   # [NS, K, P] int32 or None: MB per in-flight microbatch (NEXT-1, depth-aware memory)
 
     def copy(self) -> "Instance":
         return Instance(self.name, self.L, self.K, self.P, self.m, self.time_us.copy(),
                         self.mem_mb.copy(), self.island_gpus.copy(), self.island_cap_mb.copy(),
-                        self.bw_gbps.copy(), self.act_mb, dict(self.meta))
+                        self.bw_gbps.copy(), self.act_mb, dict(self.meta),
+                        None if self.actmem_mb is None else self.actmem_mb.copy())
 
 
 def _cdiv(a, b):
@@ -259,6 +261,17 @@ def random_small(seed: int, Lmax: int = 8, Kmax: int = 5, Pmax: int = 3, style: 
     return Instance(f"rand_{style}_s{seed}", L, K, P, m, t.astype(np.int32), mm.astype(np.int32),
                     urand(seed, S_NGPU, np.arange(K), 1, 8).astype(np.int32), cap.astype(np.int32),
                     bw.astype(np.int32), act)
+
+
+def with_actmem(inst: Instance, seed: int, lo: int = 0, hi: int = 60) -> Instance:
+    """Adds a per-plan activation footprint (MB per in-flight microbatch) proportional to the slice length."""
+    o = inst.copy()
+    NS, K, P = inst.time_us.shape
+    a, b = slice_bounds(inst.L)
+    idx = np.arange(NS * K * P).reshape(NS, K, P)
+    o.actmem_mb = ((b - a)[:, None, None] * urand(seed, S_MISC + 30, idx, lo, hi)).astype(np.int32)
+    o.name = inst.name + "_act"
+    return o
 
 
 def by_name(name: str, seed: int = 0):
