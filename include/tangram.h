@@ -68,6 +68,17 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
                              const int32_t* island_cap_mb, const int32_t* bw_gbps, int32_t act_mb,
                              tg_instance** out);
 
+/* tg_instance_set_actmem — SURVEY.md §8(f) NEXT-1, depth-aware activation memory under 1F1B (PAPER.md:246
+ * "earlier stages hold more in-flight activations", :258(i)).  actmem_mb: EITHER [NS][K][P] int32 in
+ * [0, 2^20], MB that plan p of (slice, island) needs PER in-flight microbatch, copied; NULL removes the table.
+ * With the table set, a stage followed by r later stages holds q = r + 1 microbatches, so its plan p is
+ * feasible iff mem_mb + q * actmem_mb <= cap_mb[k]; the stage cost becomes c_q = min over the plans feasible
+ * at depth q, and the candidate thresholds are the distinct finite c_q of all depths.  Everything else
+ * (sum, T, iter, tie-breaks) is unchanged; stage_plan[i] is the lowest p attaining c_q of that stage.
+ * tg_reduce keeps reporting depth 1; tg_prune returns TG_ERR_RANGE for such instances.  Synchronises the
+ * legacy default stream. */
+tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb);
+
 /* NULL is a no-op.  The instance must not be in use by an unsynchronised tg_solve_batch. */
 tg_status tg_instance_destroy(tg_instance* inst);
 

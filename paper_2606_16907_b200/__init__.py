@@ -61,7 +61,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
+EXPORTS = ["tg_instance_create", "tg_instance_set_actmem", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
            "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -79,6 +79,7 @@ def lib():
         vp, i32, i64, u32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32
         L.tg_instance_create.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, i32, C.POINTER(vp)]
         L.tg_instance_destroy.argtypes = [vp]
+        L.tg_instance_set_actmem.argtypes = [vp, vp]
         L.tg_solve_batch.argtypes = [C.POINTER(vp), i32, vp, vp]
         L.tg_solve_batch_ex.argtypes = [C.POINTER(vp), i32, vp, u32, vp, vp]
         L.tg_prune.argtypes = [vp, C.c_int, i64, C.POINTER(i64), vp]
@@ -157,6 +158,12 @@ def tg_instance_create(L, K, P, m, time_us, mem_mb, island_gpus, island_cap_mb, 
     h = C.c_void_p(0)
     _check(lib().tg_instance_create(L, K, P, m, *[_ptr(a) for a in arrs], act_mb, C.byref(h)))
     return Instance(h.value, L, K, P, m)
+
+
+def tg_instance_set_actmem(inst: Instance, actmem_mb):
+    """NEXT-1: per-plan MB per in-flight microbatch ([NS,K,P] int32 numpy array or torch tensor); None removes it."""
+    a = np.ascontiguousarray(actmem_mb, dtype=np.int32) if isinstance(actmem_mb, np.ndarray) else actmem_mb
+    _check(lib().tg_instance_set_actmem(inst.handle, _ptr(a)))
 
 
 def tg_instance_destroy(inst: Instance):
@@ -239,5 +246,8 @@ def instance_from_inputs(inst, device_tables: bool = False) -> Instance:
         mm = torch.from_numpy(np.ascontiguousarray(inst.mem_mb, dtype=np.int32)).cuda()
         return tg_instance_create(inst.L, inst.K, inst.P, inst.m, t, mm, inst.island_gpus, inst.island_cap_mb,
                                   inst.bw_gbps, inst.act_mb)
-    return tg_instance_create(inst.L, inst.K, inst.P, inst.m, inst.time_us, inst.mem_mb, inst.island_gpus,
-                              inst.island_cap_mb, inst.bw_gbps, inst.act_mb)
+    h = tg_instance_create(inst.L, inst.K, inst.P, inst.m, inst.time_us, inst.mem_mb, inst.island_gpus,
+                           inst.island_cap_mb, inst.bw_gbps, inst.act_mb)
+    if getattr(inst, "actmem_mb", None) is not None:
+        tg_instance_set_actmem(h, inst.actmem_mb)
+    return h

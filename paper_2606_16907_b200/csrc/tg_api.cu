@@ -15,6 +15,7 @@ struct tg_instance {
     int32_t L, K, P, m, act_mb, NS;
     int device;
     int32_t *time_us, *mem_mb, *gpus, *cap_mb, *bw;  // device
+    int32_t* actmem;                                 // device, or nullptr (tg_instance_set_actmem)
 };
 
 namespace {
@@ -158,6 +159,8 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         TgInstDev& I = h[i];
         memset(&I, 0, sizeof(I));
         I.time_us = t.time_us; I.mem_mb = t.mem_mb; I.cap_mb = t.cap_mb; I.bw_gbps = t.bw;
+        I.actmem_mb = t.actmem;
+        I.nDepth = t.actmem ? t.K : 1;
         I.L = t.L; I.K = t.K; I.P = t.P; I.m = t.m; I.act_mb = t.act_mb; I.NS = t.NS;
         I.Lp = (t.L + 3) & ~3;
         I.triG = int(tgGOff(t.L, t.L + 1));
@@ -182,11 +185,12 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         maxCells = std::max(maxCells, cells);
         maxLp = std::max(maxLp, int(I.Lp));
         maxK = std::max(maxK, int(t.K));
-        oCd[i] = cv.take(size_t(t.K) * I.triG * 4);
-        oArgp[i] = cv.take(size_t(cells));
-        oCand[i] = cv.take(size_t(cells) * 4);
-        oSort[i] = cv.take(size_t(cells) * 4);
-        oSort2[i] = cv.take(size_t(cells) * 4);
+        const size_t nd = size_t(I.nDepth);
+        oCd[i] = cv.take(nd * size_t(t.K) * I.triG * 4);
+        oArgp[i] = cv.take(nd * size_t(cells));
+        oCand[i] = cv.take(nd * size_t(cells) * 4);
+        oSort[i] = cv.take(nd * size_t(cells) * 4);
+        oSort2[i] = cv.take(nd * size_t(cells) * 4);
         oSuf[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
         oSufA[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
         oEI[i] = cv.take(size_t(TG_MAX_EVAL) * 4);
@@ -339,6 +343,7 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
     tg_instance* t = new (std::nothrow) tg_instance();
     if (!t) { cudaFreeAsync(base, 0); return fail(TG_ERR_OOM, "host allocation failed"); }
     t->L = L; t->K = K; t->P = P; t->m = m; t->act_mb = act_mb; t->NS = NS; t->device = dev;
+    t->actmem = nullptr;
     t->time_us = reinterpret_cast<int32_t*>(base + oT); t->mem_mb = reinterpret_cast<int32_t*>(base + oM);
     t->gpus = reinterpret_cast<int32_t*>(base + oG); t->cap_mb = reinterpret_cast<int32_t*>(base + oC);
     t->bw = reinterpret_cast<int32_t*>(base + oB);
@@ -367,8 +372,34 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
 
 tg_status tg_instance_destroy(tg_instance* inst) {
     if (!inst) return TG_OK;
+    if (inst->actmem) cudaFreeAsync(inst->actmem, 0);
     cudaFreeAsync(inst->time_us, 0);  // base of the single allocation
     delete inst;
+    return TG_OK;
+}
+
+tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb) {
+    if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
+    if (inst->actmem) { cudaFreeAsync(inst->actmem, 0); inst->actmem = nullptr; }
+    if (!actmem_mb) return TG_OK;
+    const size_t nE = size_t(inst->NS) * inst->K * inst->P;
+    int32_t* d = nullptr;
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), nE * 4 + 4, 0));
+    int* dErr = reinterpret_cast<int*>(d + nE);
+    cudaError_t e = cudaMemcpyAsync(d, actmem_mb, nE * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dErr, 0, 4, 0);
+    int herr = 0;
+    if (e == cudaSuccess) {
+        const int blocks = int(std::min<size_t>((nE + 255) / 256, 4096));
+        tgValidateNonNegKernel<<<std::max(blocks, 1), 256>>>(d, nE, dErr);
+        e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);
+    }
+    if (e != cudaSuccess || herr) {
+        cudaFreeAsync(d, 0);
+        if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("actmem upload: ") + cudaGetErrorString(e));
+        return fail(TG_ERR_RANGE, "actmem_mb must be in [0, 2^20]");
+    }
+    inst->actmem = d;
     return TG_OK;
 }
 
@@ -439,6 +470,7 @@ tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int
     if (mode == TG_PRUNE_IMBALANCE && (threshold < 1000 || threshold > 16384))
         return fail(TG_ERR_RANGE, "theta must be in [1000, 16384] permille");
     if (mode == TG_PRUNE_BOTTLENECK && threshold < 0) return fail(TG_ERR_RANGE, "bottleneck cap must be >= 0");
+    if (inst->actmem) return fail(TG_ERR_RANGE, "tg_prune is not defined for instances with an actmem table (dominance would need the third axis)");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const int cells = inst->NS * inst->K;
     char* ws = nullptr;

@@ -39,10 +39,12 @@ __host__ __device__ __forceinline__ int tgSliceIdx(int L, int a, int b) {
 struct TgInstDev {
     const int32_t* time_us;  // [NS][K][P] (instance-owned)
     const int32_t* mem_mb;   // [NS][K][P]
+    const int32_t* actmem_mb;  // [NS][K][P] MB per in-flight microbatch, or nullptr (NEXT-1: depth-aware memory)
     const int32_t* cap_mb;   // [K]
     const int32_t* bw_gbps;  // [K][K]
-    uint32_t* cd;            // [K][triG] diagonal-major reduced costs, TG_INFU = none
-    uint8_t* argp;           // [NS][K] lowest p attaining c, 0xff = none
+    uint32_t* cd;            // [nDepth][K][triG] diagonal-major reduced costs, TG_INFU = none; table q-1 holds the costs
+                             // of a stage with q microbatches in flight (q = its own stage + the later ones)
+    uint8_t* argp;           // [nDepth][NS][K] lowest p attaining c, 0xff = none
     uint32_t* cand;          // [nCandCap] ascending distinct finite c (first ncand valid)
     uint32_t* sortbuf;       // [NS*K] reduced costs, flat: input of the candidate sort
     uint32_t* sortbuf2;      // [NS*K] scratch of the candidate sort
@@ -51,6 +53,7 @@ struct TgInstDev {
     int32_t* eIdx;           // [TG_MAX_EVAL] evaluated feasible candidates, ascending (bit 30: interval below resolved)
     uint32_t* eF;            // [TG_MAX_EVAL] their f_T
     int32_t L, K, P, m, act_mb, NS, Lp, triG;
+    int32_t nDepth;          // 1, or K when actmem_mb is set
     int32_t sortCap, ncand;
     uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
     uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major

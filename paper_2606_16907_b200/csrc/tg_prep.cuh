@@ -69,6 +69,13 @@ __global__ void tgValidateKernel(const int32_t* __restrict__ time_us, const int3
     if (bad) atomicOr(err, bad);
 }
 
+__global__ void tgValidateNonNegKernel(const int32_t* __restrict__ v, size_t n, int* err) {
+    int bad = 0;
+    for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += size_t(gridDim.x) * blockDim.x)
+        if (v[i] < 0 || v[i] > (1 << 20)) bad = 1;
+    if (bad) atomicOr(err, 1);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Step 1: cost-table loader.  One thread per (slice, island) cell, reduction over the P plans.
 //   c = min_p { time : time != INVALID, mem <= cap_k }, ties -> lowest p
@@ -110,21 +117,38 @@ __global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ inst
     if (cell < nCells) {
         const int s = cell / K, k = cell - s * K;
         const int32_t capk = __ldg(I.cap_mb + k);
-        uint32_t best; int bp;
         const size_t e = size_t(cell) * P;
-        if ((P & 3) == 0) tgReduceCell<true>(I.time_us + e, I.mem_mb + e, P, capk, best, bp);
-        else tgReduceCell<false>(I.time_us + e, I.mem_mb + e, P, capk, best, bp);
         int a, b;
         tgSliceAB(L, s, a, b);
         const int d = b - a;
-        uint32_t* row = I.cd + size_t(k) * I.triG + tgGOff(L, d);
-        row[a] = best;
-        if (b == L) {  // last element of the row: write the INF padding up to a multiple of 4
-            const int rl = (L - d + 1 + 3) & ~3;
-            for (int p = a + 1; p < rl; ++p) row[p] = TG_INFU;
+        const int rl = (L - d + 1 + 3) & ~3;
+        uint32_t best = TG_INFU, prev = TG_INFU;   // best ends up as the depth-1 cost (the least constrained)
+        for (int q = I.nDepth; q >= 1; --q) {
+            // depth q: the stage holds q microbatches in flight: feasible iff
+            // mem + q * actmem <= cap.  Without an actmem table there is the one static test.
+            uint32_t bq; int bp;
+            if (I.actmem_mb == nullptr) {
+                if ((P & 3) == 0) tgReduceCell<true>(I.time_us + e, I.mem_mb + e, P, capk, bq, bp);
+                else tgReduceCell<false>(I.time_us + e, I.mem_mb + e, P, capk, bq, bp);
+            } else {
+                bq = TG_INFU; bp = 0xff;
+                for (int p = 0; p < P; ++p) {
+                    const int32_t t = __ldg(I.time_us + e + p);
+                    const long long need = (long long)__ldg(I.mem_mb + e + p) + (long long)q * __ldg(I.actmem_mb + e + p);
+                    if (t != TG_INVALID && need <= (long long)capk && uint32_t(t) < bq) { bq = uint32_t(t); bp = p; }
+                }
+            }
+            uint32_t* row = I.cd + (size_t(q - 1) * K + k) * I.triG + tgGOff(L, d);
+            row[a] = bq;
+            if (b == L)   // last element of the row: write the INF padding up to a multiple of 4
+                for (int p = a + 1; p < rl; ++p) row[p] = TG_INFU;
+            I.argp[size_t(q - 1) * nCells + cell] = uint8_t(bp);
+            // candidate thresholds: every distinct finite cost of any depth (deeper costs repeat the shallower one
+            // until a plan stops fitting, so equal neighbours are dropped here already)
+            I.sortbuf[size_t(q - 1) * nCells + cell] = (q == I.nDepth || bq != prev) ? bq : TG_INFU;
+            prev = bq;
+            best = bq;
         }
-        I.argp[cell] = uint8_t(bp);
-        I.sortbuf[cell] = best;
         if (best < TG_INFU) atomicMin(&sMin[k], best);
     }
     __syncthreads();
@@ -231,7 +255,7 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     }
     // candidate sort: stable LSD radix sort, 8-bit digits, ping-pong between the two global buffers
     // (L2 resident); per-warp digit histograms in shared memory, warp w owns a contiguous chunk
-    const int n = I.NS * K;
+    const int n = I.NS * K * I.nDepth;
     uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, sbuf, warpSums);
     // unique, finite only
     uint32_t base = 0;

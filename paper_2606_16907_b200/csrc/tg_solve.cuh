@@ -26,6 +26,7 @@ struct TgShared {
     uint32_t sT;
     // row windows (see "Row windows" below): rows hold Wd starts, row of state (S, k) begins at start lo4(cap(S))
     int sWd, sSlack, sWindowed;
+    uint32_t cdOff;                 // word offset of the reduced table of the depth currently staged
     uint8_t maxlenK[TG_MAX_K];      // longest admissible slice of island k at T, any position
     uint32_t baseK[TG_MAX_K];
     int dmaxK[TG_MAX_K];
@@ -109,6 +110,65 @@ __device__ __forceinline__ int tgLo4(const TgShared& sm, int cap) {
     return sm.sWindowed ? (max(0, sm.sL - cap) & ~3) : 0;
 }
 
+// Fills the staged cost rows (and dmaxTile) from the reduced table of depth q (q = 1 unless the instance has
+// an actmem table: then level r of the DP, whose stages have r later stages, uses q = r + 1 -- SURVEY NEXT-1).
+// The layout (baseK, D_k) comes from depth 1, whose costs are the lowest, so it covers every depth.
+// Returns this thread's count of admissible entries; ends with a CTA barrier.
+__device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, int q, bool count) {
+    const int tid = threadIdx.x;
+    const TgInstDev& I = ctx.inst[sm.sInst];
+    const int L = sm.sL, Lp = sm.sLp, Ke = sm.sKe, nb4 = Lp >> 2;
+    const uint32_t T = sm.sT;
+    unsigned nAdm = 0;
+    if (tid == 0) sm.cdOff = uint32_t(q - 1) * uint32_t(I.K) * uint32_t(I.triG);
+    __syncthreads();
+    if (!sm.useGlobalC) {
+        for (int kc = 0; kc < Ke; ++kc) {
+            const int dk = sm.dmaxK[kc], Dk = (dk + 3) & ~3;
+            const uint32_t* cdk = I.cd + sm.cdOff + size_t(sm.isl[kc]) * I.triG;
+            uint32_t* dst = Cs + sm.baseK[kc];
+            for (int w = tid; w < Dk * nb4; w += TG_NT) {
+                const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
+                uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+                if (d <= dk && a4 < ((L - d + 3) >> 2)) {
+                    v = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + a4);
+                    const int a = a4 * 4, amax = L - 1 - d;
+                    v.x = (a + 0 <= amax && v.x <= T) ? v.x : TG_INFU;
+                    v.y = (a + 1 <= amax && v.y <= T) ? v.y : TG_INFU;
+                    v.z = (a + 2 <= amax && v.z <= T) ? v.z : TG_INFU;
+                    v.w = (a + 3 <= amax && v.w <= T) ? v.w : TG_INFU;
+                    nAdm += (v.x < TG_INFU) + (v.y < TG_INFU) + (v.z < TG_INFU) + (v.w < TG_INFU);
+                }
+                reinterpret_cast<uint4*>(dst)[w] = v;
+            }
+        }
+        __syncthreads();
+        for (int w = tid; w < Ke * nb4; w += TG_NT) {   // widest admissible diagonal per 4 starts
+            const int kc = w / nb4, a4 = w - kc * nb4;
+            const uint4* col = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc]) + a4;
+            int d = sm.dmaxK[kc];
+            for (; d >= 1; --d) {
+                const uint4 v = col[(d - 1) * nb4];
+                if (min(min(v.x, v.y), min(v.z, v.w)) < TG_INFU) break;
+            }
+            sm.dmaxTile[kc][a4] = uint8_t(d);
+        }
+    } else {
+        for (int w = tid; w < Ke * nb4; w += TG_NT) {
+            const int kc = w / nb4, a4 = w - kc * nb4;
+            sm.dmaxTile[kc][a4] = uint8_t(max(0, min(sm.dmaxK[kc], L - 1 - 4 * a4)));
+        }
+        if (count)
+            for (int kc = 0; kc < Ke; ++kc) {
+                const uint32_t* cdk = I.cd + sm.cdOff + size_t(sm.isl[kc]) * I.triG;
+                for (int d = 1; d <= sm.dmaxK[kc]; ++d)
+                    for (int a = tid; a <= L - 1 - d; a += TG_NT) nAdm += cdk[tgGOff(L, d) + a] <= T ? 1u : 0u;
+            }
+    }
+    __syncthreads();
+    return nAdm;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Staging of one item's thresholded cost tables into shared memory.
 //   Cs_k[(d-1)*Lp + a] = c[a][a+d][k] if <= T and a+d <= L-1, else INF   (k in compact labels)
@@ -121,7 +181,7 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     unsigned nAdm = 0;   // admissible (a, b, k) cost entries with b <= L-1 seen by this thread
     const int tid = threadIdx.x, lane = tid & 31;
     const TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
-    const int L = I.L, Lp = I.Lp, nb4 = Lp >> 2;
+    const int L = I.L, Lp = I.Lp;
     const uint32_t T = __ldcg(&itp->T);
     // geometry of the item: the islands with some admissible slice at T, in compact labels.  The final
     // DP only needs the islands of the optimal mask S*: S* is the lowest mask attaining the optimum at
@@ -184,49 +244,7 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
     }
     __syncthreads();
-    if (!sm.useGlobalC) {
-        for (int kc = 0; kc < Ke; ++kc) {
-            const int dk = sm.dmaxK[kc], Dk = (dk + 3) & ~3;
-            const uint32_t* cdk = I.cd + size_t(sm.isl[kc]) * I.triG;
-            uint32_t* dst = Cs + sm.baseK[kc];
-            for (int w = tid; w < Dk * nb4; w += TG_NT) {
-                const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
-                uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
-                if (d <= dk && a4 < ((L - d + 3) >> 2)) {
-                    v = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + a4);
-                    const int a = a4 * 4, amax = L - 1 - d;
-                    v.x = (a + 0 <= amax && v.x <= T) ? v.x : TG_INFU;
-                    v.y = (a + 1 <= amax && v.y <= T) ? v.y : TG_INFU;
-                    v.z = (a + 2 <= amax && v.z <= T) ? v.z : TG_INFU;
-                    v.w = (a + 3 <= amax && v.w <= T) ? v.w : TG_INFU;
-                    nAdm += (v.x < TG_INFU) + (v.y < TG_INFU) + (v.z < TG_INFU) + (v.w < TG_INFU);
-                }
-                reinterpret_cast<uint4*>(dst)[w] = v;
-            }
-        }
-        __syncthreads();
-        for (int w = tid; w < Ke * nb4; w += TG_NT) {   // widest admissible diagonal per 4 starts
-            const int kc = w / nb4, a4 = w - kc * nb4;
-            const uint4* col = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc]) + a4;
-            int d = sm.dmaxK[kc];
-            for (; d >= 1; --d) {
-                const uint4 v = col[(d - 1) * nb4];
-                if (min(min(v.x, v.y), min(v.z, v.w)) < TG_INFU) break;
-            }
-            sm.dmaxTile[kc][a4] = uint8_t(d);
-        }
-    } else {
-        for (int w = tid; w < Ke * nb4; w += TG_NT) {
-            const int kc = w / nb4, a4 = w - kc * nb4;
-            sm.dmaxTile[kc][a4] = uint8_t(max(0, min(sm.dmaxK[kc], L - 1 - 4 * a4)));
-        }
-        if (count)
-            for (int kc = 0; kc < Ke; ++kc) {
-                const uint32_t* cdk = I.cd + size_t(sm.isl[kc]) * I.triG;
-                for (int d = 1; d <= sm.dmaxK[kc]; ++d)
-                    for (int a = tid; a <= L - 1 - d; a += TG_NT) nAdm += cdk[tgGOff(L, d) + a] <= T ? 1u : 0u;
-            }
-    }
+    nAdm = tgStageCosts(ctx, sm, Cs, 1, count);
     if (count) {   // statistics: admissible relaxations of this DP (stage + transfer)
         for (int o = 16; o > 0; o >>= 1) nAdm += __shfl_down_sync(0xffffffffu, nAdm, o);
         if (lane == 0 && nAdm && Ke > 0)
@@ -437,7 +455,7 @@ __device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& 
     for (int s = g; s < nk; s += NG) {
         const int k = kl[s];
         const int lo4S = max(0, Lw - capR - int(sm.maxlenK[k])) & ~3, dq4 = (lo4R - lo4S) >> 2;
-        const uint32_t* cdk = GLOBALC ? I.cd + size_t(sm.isl[k]) * I.triG : nullptr;
+        const uint32_t* cdk = GLOBALC ? I.cd + sm.cdOff + size_t(sm.isl[k]) * I.triG : nullptr;
         const uint32_t cBase = csBase + (sm.baseK[k] + uint32_t(lo4S)) * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes + 16u;
         uint32_t* const gOut = gRow + size_t(s) * Wd;
         for (int cw = c0; cw < nbw; cw += CH) {
@@ -584,7 +602,9 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
             const int r = __popc(R);
             const int Wd = sm.sWd;
             const uint32_t* Gl = slot + tgLevelOff(0, Ke, Wd, r - 1);
-            const uint32_t* cdk = I.cd + size_t(ko) * I.triG;
+            // this stage is followed by r later ones: its cost and plan come from the table of depth r + 1
+            const size_t dq = I.nDepth > 1 ? size_t(r) : 0;
+            const uint32_t* cdk = I.cd + (dq * K + ko) * I.triG;
             int capR = 0;   // every source row (R\{j}, j) starts at start lo4(cap(R))
             for (int j = 0; j < Ke; ++j) if (R >> j & 1u) capR += sm.maxlenK[j];
             const int lo4R = tgLo4(sm, capR);
@@ -612,7 +632,7 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
             if (best == TG_KEY_NONE) { bad = true; break; }
             b = int(best >> 8) & 0xffffff;
             const int j = int(best & 0xffu);
-            sb[n] = a; si[n] = ko; sp[n] = I.argp[size_t(tgSliceIdx(L, a, b)) * K + ko];
+            sb[n] = a; si[n] = ko; sp[n] = I.argp[dq * size_t(I.NS) * K + size_t(tgSliceIdx(L, a, b)) * K + ko];
             ++n;
             a = b; k = j; R ^= 1u << j;
             continue;
@@ -645,6 +665,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
                           unsigned long long* key, int member, int teamSize, int slotIdx) {
     tgStageItem(ctx, sm, Cs, wbufAll, itp, member == 0);
     tgMark(sm, 0);
+    const TgInstDev& I = ctx.inst[sm.sInst];
     const int Ke = sm.sSlack >= 0 ? sm.sKe : 0;   // the islands' longest slices cannot cover L layers: infeasible at T
     const int Wd = sm.sWd, nW = ctx.nActiveWarps, warp = threadIdx.x >> 5;
     uint64_t bufWords = 0;   // words of one ping-pong half; 0 = keep every level (a back-track follows)
@@ -663,6 +684,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         for (int r = 1; r < Ke; ++r) {
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Wd, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Wd, r);
+            if (I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
             if (warp < nW) tgWarpLevel(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
             tgMark(sm, 3);
             if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
