@@ -46,6 +46,12 @@ def make_workload(name: str, rank: int, n_inst: int):
         return [gen.config3(rank)], "cfg3 70B-like L=80 K=12 P=8 m=32 (configs[2]), 1 instance/GPU"
     if name == "cfg2":
         return [gen.config2(rank)], "cfg2 7B-like L=32 K=6 P=4 m=16 (configs[1]), 1 instance/GPU"
+    if name == "cfg4d":   # cfg4 with a per-plan activation footprint
+        return [gen.with_actmem(gen.config4(rank), 11 + rank, 300, 3000)], \
+            "cfg4 MoE-like L=64 K=16 P=8 m=64 + depth-aware activation memory (NEXT-1), 1 instance/GPU"
+    if name == "cfg3d":
+        return [gen.with_actmem(gen.config3(rank), 7 + rank, 500, 6000)], \
+            "cfg3 70B-like L=80 K=12 P=8 m=32 + depth-aware activation memory (NEXT-1), 1 instance/GPU"
     if name == "cfg5":
         from paper_2606_16907_b200.shard import weak_seeds
         return [gen.config5_one(sd) for sd in weak_seeds(n_inst, rank)], \
@@ -198,16 +204,22 @@ def run_ours(args):
         barrier()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     # ---- end to end: host tables -> create (H2D) -> solve -> host results (D2H) ----
-    h2d = sum(i.time_us.nbytes + i.mem_mb.nbytes + i.bw_gbps.nbytes + 8 * i.K for i in insts)
+    h2d = sum(i.time_us.nbytes + i.mem_mb.nbytes + i.bw_gbps.nbytes + 8 * i.K +
+              (i.actmem_mb.nbytes if i.actmem_mb is not None else 0) for i in insts)
     d2h = n * tg.RESULT_BYTES
     e2e_steps = max(1, min(args.steps, 3))
     # inputs of the end-to-end leg wait in PINNED host memory
     pinned = [[torch.from_numpy(np.ascontiguousarray(a, dtype=np.int32)).pin_memory()
                for a in (i.time_us, i.mem_mb, i.island_gpus, i.island_cap_mb, i.bw_gbps)] for i in insts]
+    pinned_act = [torch.from_numpy(np.ascontiguousarray(i.actmem_mb, dtype=np.int32)).pin_memory()
+                  if i.actmem_mb is not None else None for i in insts]
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         hs = [tg.tg_instance_create(i.L, i.K, i.P, i.m, *pp, i.act_mb) for i, pp in zip(insts, pinned)]
+        for h, pa in zip(hs, pinned_act):
+            if pa is not None:
+                tg.tg_instance_set_actmem(h, pa)
         res = tg.tg_solve_batch(hs, out=None, flags=flags)            # host result buffer: D2H + sync inside
         for h in hs:
             h.destroy()
@@ -265,7 +277,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5", "cfg3d", "cfg4d"])
     ap.add_argument("--n-inst", type=int, default=1024, help="instances per GPU of the cfg5 batch")
     ap.add_argument("--full-sweep", action="store_true", help="run the DP at every candidate T")
     ap.add_argument("--cpu-threads", type=int, default=8)

@@ -302,6 +302,13 @@ tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cud
         for (int r = 0; r < nr; ++r)
             fprintf(stderr, "[tg]  round %3d items %5d  %8.1f us\n", r, hc.roundItems[r],
                     r + 1 < nr ? double(hc.roundNs[r + 1] - hc.roundNs[r]) * 1e-3 : 0.0);
+        for (int r = 0; r < nr && r < 8; ++r) {
+            if (hc.roundItems[r] > 16 || hc.roundItems[r] >= W.ctx.nSlots) continue;
+            fprintf(stderr, "[tg]  round %3d items (candidate: us)", r);
+            for (int t = 0; t < hc.roundItems[r]; ++t)
+                fprintf(stderr, " %d: %.0f", hc.itemTidx[r][t], double(hc.itemNs[r][t] - hc.roundNs[r]) * 1e-3);
+            fprintf(stderr, "\n");
+        }
     }
     int32_t err = 0;
     if (sync) TG_CUDA(cudaMemcpyAsync(&err, &W.ctx.ctrl->errFlag, sizeof(int32_t), cudaMemcpyDeviceToHost, st));

@@ -93,6 +93,8 @@ struct TgCtrl {
     // debugging aid (TG_DEBUG=1): start time and item count of the first rounds
     unsigned long long roundNs[256];
     int32_t roundItems[256];
+    unsigned long long itemNs[8][16];   // team mode: finish time of the first items of the first rounds
+    int32_t itemTidx[8][16];
 };
 
 struct TgSolveCtx {

@@ -1021,6 +1021,12 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
             while (t > 0 && int((int64_t(t) * nCta) / nItems) > b) --t;
             const int start = int((int64_t(t) * nCta) / nItems), end = int((int64_t(t + 1) * nCta) / nItems);
             tgRunItem(ctx, sm, Cs, wbufAll, items + t, keys + t, b - start, end - start, t);
+            if (b == start && threadIdx.x == 0 && round < 8 && t < 16) {
+                unsigned long long ns;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
+                ctrl->itemNs[round][t] = ns;
+                ctrl->itemTidx[round][t] = items[t].tidx;
+            }
         }
         tgMark(sm, 0);
         tgGridBarrier(ctrl, epoch);

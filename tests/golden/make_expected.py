@@ -50,6 +50,12 @@ def main():
             data = [dict(one(gen.config3(s), threads, False), seed=s) for s in (1, 2, 3, 4)]
         elif name == "cfg4x":      # a second MoE-like instance
             data = [dict(one(gen.config4(1), threads, False), seed=1)]
+        elif name == "cfg3d":      # NEXT-1: the 70B-like config with a per-plan activation footprint (depth oracle)
+            inst = gen.with_actmem(gen.config3(), 7, 500, 6000)
+            t0 = time.time()
+            data = [{"name": inst.name, "L": inst.L, "K": inst.K, "P": inst.P, "m": inst.m,
+                     "solve": rec(oracle.solve_depth(inst)), "core": rec(oracle.solve(inst, n_threads=threads)),
+                     "oracle_seconds": round(time.time() - t0, 1)}]
         elif name == "cfg5":
             data = [dict(one(gen.config5_one(s), threads, False), seed=s) for s in CFG5_SEEDS]
         else:

@@ -74,3 +74,21 @@ def test_errors_with_actmem(tg):
         tg.tg_instance_set_actmem(h, bad)
     assert e.value.status == 3
     h.destroy()
+
+
+def test_full_size_cfg3_with_actmem(tg):
+    """Full-size 70B-like config with a footprint; stored result of the depth oracle
+    (tests/golden/make_expected.py cfg3d)."""
+    import json, os
+    p = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "expected_cfg3d.json")
+    e = json.load(open(p))["records"][0]
+    inst = gen.with_actmem(gen.config3(), 7, 500, 6000)
+    g = solve_all(tg, [inst])[0]
+    n = int(g["n_stages"])
+    got = [int(g["iter_time_us"]), int(g["sum_us"]), int(g["bottleneck_us"]), int(g["island_mask"]),
+           [[int(g["stage_begin"][i]), int(g["stage_island"][i]), int(g["stage_plan"][i])] for i in range(n)]]
+    s = e["solve"]
+    assert got == [s["iter_time_us"], s["sum_us"], s["bottleneck_us"], s["island_mask"], s["stages"]]
+    assert s["iter_time_us"] >= e["core"]["iter_time_us"]
+    st = [tuple(x) for x in got[4]]
+    assert rescore_depth(inst, st) == (got[1], got[2], got[0], got[3])
