@@ -36,8 +36,8 @@ struct TgShared {
     uint8_t isl[TG_MAX_K];
     uint16_t binom[17][17];
     // per-warp streaming state
-    uint32_t rowOf[TG_NW][TG_MAX_K];                // source row of each member of the mask being issued
-    uint8_t kl[TG_NW][TG_MAX_K];                    // islands not in the current mask, ascending
+    uint32_t rowOf[TG_NW][2 * TG_MAX_K];            // source row of each member of the mask being issued (per half warp)
+    uint8_t kl[TG_NW][2 * TG_MAX_K];                // islands not in the current mask, ascending (per half warp)
     // scheduler / queue
     uint32_t warpSums[33];
     int iTmp[8];
@@ -328,28 +328,34 @@ __device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
 // position, those above move down by one) -- two warp scans over the member lanes.
 // (Bulk TMA copies, one per row, were measured slower here: with row windows a row is often 32-64 bytes
 // and the per-SM TMA issue rate, not bandwidth, became the bound -- DESIGN.md 7.4.)
-__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, int r, int nk, int Wd, int nbw, int chShift,
+// SW = lanes per mask (32, or 16 when a warp runs two masks side by side); sl = lane within the sub-warp;
+// `valid` = this sub-warp has a mask to issue (the shuffles are executed by every lane regardless).
+template <int SW>
+__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, bool valid, int r, int nk, int Wd, int nbw, int cpShift,
                                             uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
-    const bool member = (R >> lane) & 1u;
-    const int p = __popc(R & ((1u << lane) - 1u));
+    const int sl = lane & (SW - 1);
+    const bool member = valid && ((R >> sl) & 1u);   // R < 2^16: lanes 16..31 of a full warp are never members
+    const int p = __popc(R & ((1u << sl) - 1u));
     // both sums stay below C(16,8) = 12870, so they share one register: low half "kept position", high half "moved down"
-    const uint32_t mine = member ? (uint32_t(sm.binom[lane & 15][p + 1]) | uint32_t(sm.binom[lane & 15][p]) << 16) : 0u;
+    const uint32_t mine = member ? (uint32_t(sm.binom[sl & 15][p + 1]) | uint32_t(sm.binom[sl & 15][p]) << 16) : 0u;
     uint32_t incl = mine;
 #pragma unroll
     for (int o = 1; o < 16; o <<= 1) {
         const uint32_t a = __shfl_up_sync(0xffffffffu, incl, o);
         if ((lane & 15) >= o) incl += a;
     }
-    const uint32_t total = __shfl_sync(0xffffffffu, incl, 15);
-    if (member && lane < 16)
-        rowOf[p] = (((incl - mine) & 0xffffu) + ((total - incl) >> 16)) * uint32_t(nk + 1) + uint32_t(lane - p);
+    const uint32_t total = __shfl_sync(0xffffffffu, incl, (lane & 16) | 15);
+    if (member)
+        rowOf[p] = (((incl - mine) & 0xffffu) + ((total - incl) >> 16)) * uint32_t(nk + 1) + uint32_t(sl - p);
     __syncwarp();
-    const int cpShift = nbw > 32 ? 6 : chShift, CH = 1 << cpShift;   // chunks per row, rounded up to a power of two
-    for (int w = lane; w < (r << cpShift); w += 32) {
-        const int ji = w >> cpShift, ch = w & (CH - 1);
-        if (ch < nbw) {
-            const uint32_t* src = Gprev + size_t(rowOf[ji]) * Wd + 4 * ch;
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(bufAddr + uint32_t(ji) * rowBytes + uint32_t(ch) * 16u), "l"(src) : "memory");
+    if (valid) {
+        const int CP = 1 << cpShift;   // chunks per row, rounded up to a power of two
+        for (int w = sl; w < (r << cpShift); w += SW) {
+            const int ji = w >> cpShift, ch = w & (CP - 1);
+            if (ch < nbw) {
+                const uint32_t* src = Gprev + size_t(rowOf[ji]) * Wd + 4 * ch;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(bufAddr + uint32_t(ji) * rowBytes + uint32_t(ch) * 16u), "l"(src) : "memory");
+            }
         }
     }
 }
@@ -493,61 +499,88 @@ __device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& 
     }
 }
 
+// words between consecutive rows of a warp's buffer: 4 (mod 8), so consecutive rows start in different 16-byte
+// bank groups (rows are read by several island groups at the same chunk offset)
+__device__ __forceinline__ int tgRowStride(int Wd) { return Wd + 12 + (((Wd + 12) & 7) == 0 ? 4 : 0); }
+
+// One wavefront level for this warp's share of the masks.  SW = 32: one mask at a time on the whole warp.
+// SW = 16: two masks side by side, one per half warp (narrow row windows leave most of a full warp idle and
+// the per-mask bookkeeping -- successor, ranks, copies, windows -- then costs more than the relaxations;
+// two masks share every one of those instructions).  Each sub-warp owns a contiguous run of masks and its
+// own H rows and source buffers inside the warp's buffer.
+template <int SW>
 __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
                             uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW) {
+    constexpr int M = 32 / SW, SWSH = SW == 32 ? 5 : 4;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane >> SWSH, sl = lane & (SW - 1);
     const int Lp = sm.sLp, Wd = sm.sWd, nbw = Wd >> 2, nk = Ke - r;
-    // row stride = 4 (mod 8) words: consecutive rows start in different 16-byte bank groups (rows are read by
-    // several island groups at the same chunk offset)
-    const int HS = Wd + 12 + (((Wd + 12) & 7) == 0 ? 4 : 0);
+    const int HS = tgRowStride(Wd);
     const int nMasks = sm.binom[Ke][r];
     const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
     if (lo >= hi) return;
-    // lane = (chunk of 4 starts) x (island group): CH chunk lanes, NG = 32 / CH groups
-    const int chShift = nbw <= 2 ? 1 : (nbw <= 4 ? 2 : (nbw <= 8 ? 3 : (nbw <= 16 ? 4 : 5)));
-    const int CH = 1 << chShift, NG = 32 >> chShift;
-    const int c0 = lane & (CH - 1), g = lane >> chShift;
+    const int per = (hi - lo + M - 1) / M;                       // masks per sub-warp
+    const int myLo = lo + sub * per, myHi = min(hi, myLo + per);
+    // sub-lane = (chunk of 4 starts) x (island group): CH chunk lanes, NG = SW / CH groups
+    const int cpShift = nbw <= 2 ? 1 : (nbw <= 4 ? 2 : (nbw <= 8 ? 3 : (nbw <= 16 ? 4 : (nbw <= 32 ? 5 : 6))));
+    const int chShift = min(cpShift, SWSH);
+    const int CH = 1 << chShift, NG = SW >> chShift;
+    const int c0 = sl & (CH - 1), g = sl >> chShift;
     const uint32_t rowBytes = uint32_t(HS) * 4u, cStride = uint32_t(Lp) * 4u;
-    const uint32_t hAddr0 = tgSmemAddr(wbuf), csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
+    const uint32_t hAddr0 = tgSmemAddr(wbuf) + uint32_t(sub) * uint32_t(nk + 2 * r) * rowBytes;
+    const uint32_t csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
     const uint32_t xInfAddr = tgSmemAddr(&sm.xInf[0]);
     const uint32_t bufAddr[2] = {hAddr0 + uint32_t(nk) * rowBytes, hAddr0 + uint32_t(nk + r) * rowBytes};
-    uint32_t* rowOf = &sm.rowOf[warp][0];
-    uint8_t* kl = &sm.kl[warp][0];
+    uint32_t* rowOf = &sm.rowOf[warp][sub * TG_MAX_K];
+    uint8_t* kl = &sm.kl[warp][sub * TG_MAX_K];
     const uint32_t keMask = (1u << Ke) - 1u;
     const bool globalC = sm.useGlobalC != 0;
-    const int myLen = lane < Ke ? int(sm.maxlenK[lane]) : 0;
+    const int myLen = sl < Ke ? int(sm.maxlenK[sl & 15]) : 0;
     unsigned long long bestKey = TG_KEY_NONE;
 
-    uint32_t R = tgUnrank(sm, uint32_t(lo), r, Ke);
-    tgIssueMask(sm, R, r, nk, Wd, nbw, chShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
+    uint32_t R = myLo < myHi ? tgUnrank(sm, uint32_t(myLo), r, Ke) : 0u;
+    tgIssueMask<SW>(sm, R, myLo < myHi, r, nk, Wd, nbw, cpShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
     asm volatile("cp.async.commit_group;" ::: "memory");
     int b = 0;
-    for (int idx = lo; idx < hi; ++idx, b ^= 1) {
-        const uint32_t Rn = tgNextMask(R);
-        if (idx + 1 < hi) tgIssueMask(sm, Rn, r, nk, Wd, nbw, chShift, bufAddr[b ^ 1], rowBytes, Gprev, rowOf, lane);
+    for (int it = 0; it < per; ++it, b ^= 1) {
+        const int idx = myLo + it;
+        const bool valid = idx < myHi, more = idx + 1 < myHi;
+        const uint32_t Rn = more ? tgNextMask(R) : 0u;
+        tgIssueMask<SW>(sm, Rn, more, r, nk, Wd, nbw, cpShift, bufAddr[b ^ 1], rowBytes, Gprev, rowOf, lane);
         asm volatile("cp.async.commit_group;" ::: "memory");   // possibly empty: keeps the group count uniform
         const uint32_t comp = ~R & keMask;
-        if (lane < Ke && (comp >> lane & 1u)) kl[__popc(comp & ((1u << lane) - 1u))] = uint8_t(lane);
-        const int capR = int(__reduce_add_sync(0xffffffffu, (R >> lane & 1u) ? unsigned(myLen) : 0u));   // cap(R)
+        if (valid && sl < Ke && (comp >> sl & 1u)) kl[__popc(comp & ((1u << sl) - 1u))] = uint8_t(sl);
+        int capR;                                               // cap(R) = sum of the members' longest slices
+        if (SW == 32) {
+            capR = int(__reduce_add_sync(0xffffffffu, (R >> sl & 1u) ? unsigned(myLen) : 0u));
+        } else {
+            capR = (R >> sl & 1u) ? myLen : 0;
+#pragma unroll
+            for (int o = SW / 2; o > 0; o >>= 1) capR += __shfl_xor_sync(0xffffffffu, capR, o);
+        }
         asm volatile("cp.async.wait_group 1;" ::: "memory");   // this mask's rows have landed (the next mask's may be in flight)
         __syncwarp();
 
-        // ---- phase 1: transfer pre-minimum, H rows into the warp's shared memory ---------------
-        for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
-            const int nsl = min(TG_SPL, (nk - s0 + NG - 1) >> (5 - chShift));   // slots of the widest island group
+        // ---- phase 1: transfer pre-minimum, H rows into the sub-warp's shared memory -----------
+        if (valid) {
+            for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
+                const int nsl = min(TG_SPL, (nk - s0 + NG - 1) >> (SWSH - chShift));   // slots of the widest island group
 #define TG_P1_CASE(N) case N: tgPhase1<N>(sm, R, r, nk, nbw, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
-            switch (nsl) {
-                TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
-                TG_P1_CASE(5) TG_P1_CASE(6) TG_P1_CASE(7) TG_P1_CASE(8)
-            }
+                switch (nsl) {
+                    TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
+                    TG_P1_CASE(5) TG_P1_CASE(6) TG_P1_CASE(7) TG_P1_CASE(8)
+                }
 #undef TG_P1_CASE
+            }
         }
         __syncwarp();
 
         // ---- phase 2: min-plus product with the thresholded cost rows ----------------------------
-        uint32_t* const gRow = Gcur + size_t(idx) * nk * Wd;
-        if (globalC) tgPhase2<true>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
-        else tgPhase2<false>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+        if (valid) {
+            uint32_t* const gRow = Gcur + size_t(idx) * nk * Wd;
+            if (globalC) tgPhase2<true>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+            else tgPhase2<false>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+        }
         __syncwarp();
         R = Rn;
     }
@@ -685,7 +718,12 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Wd, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Wd, r);
             if (I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
-            if (warp < nW) tgWarpLevel(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
+            if (warp < nW) {
+                // two masks per warp when the windows are narrow and both masks' rows fit the warp's buffer
+                const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= ctx.wbufWords;
+                if (pair) tgWarpLevel<16>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
+                else tgWarpLevel<32>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
+            }
             tgMark(sm, 3);
             if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();
