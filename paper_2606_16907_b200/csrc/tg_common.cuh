@@ -80,6 +80,7 @@ struct TgItem {
     uint8_t Ke;          // islands with some admissible slice at T (written by the CTA that runs the item)
     uint8_t flags;       // bit0: keep every level (back-track follows)
     uint8_t isl[TG_MAX_K];  // compact label -> original island
+    uint8_t ctaBeg, ctaCnt;  // team of CTAs that runs the item (weighted team mode; written by the scheduler)
 };
 
 struct TgCtrl {
@@ -89,6 +90,8 @@ struct TgCtrl {
     int32_t round;
     uint32_t barrier;     // monotone arrival counter of the grid barrier
     int32_t errFlag;
+    int32_t weighted[2];  // per round parity: team sizes follow the items' estimated cost (teamOf / ctaBeg / ctaCnt)
+    uint8_t teamOf[2][256];   // weighted team mode: item of each CTA
     tg_solve_stats stats;
     // debugging aid (TG_DEBUG=1): start time and item count of the first rounds
     unsigned long long roundNs[256];

@@ -40,6 +40,7 @@ struct TgShared {
     uint8_t kl[TG_NW][2 * TG_MAX_K];                // islands not in the current mask, ascending (per half warp)
     // scheduler / queue
     uint32_t warpSums[33];
+    float wgt[32];                  // estimated cost of the round's items (weighted team mode)
     int iTmp[8];
     unsigned long long llTmp[2];
     int curItem;
@@ -996,7 +997,77 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     for (int idx = tid; idx < nIt; idx += TG_NT) keys[idx] = TG_KEY_NONE;
     for (int s = tid; s < ctx.nSlots; s += TG_NT) ctx.slotBar[s] = 0;
     __syncthreads();
+    // ---- C: team sizes.  A few items share the grid as teams of CTAs; a DP's cost varies a lot with its
+    // threshold (row-window width, islands alive) and with the instance shape, so the CTAs are dealt out in
+    // proportion to an estimate of it:  masks x rows x (per-row bookkeeping + lanes a row's chunks occupy).
+    const bool weighted = nIt > 1 && nIt <= 32 && nIt < ctx.nSlots && gridDim.x <= 255;
+    if (weighted) {
+        const int lane = tid & 31, warp = tid >> 5;
+        for (int t = warp; t < nIt; t += TG_NW) {
+            const TgItem& it = items[t];
+            const TgInstDev& I = ctx.inst[it.inst];
+            const int L = I.L, K = I.K;
+            const uint32_t T = it.T;
+            const uint32_t allow = ((it.flags & 1) && ctx.mode == 0) ? I.incMask : 0xffffu;   // as in tgStageItem
+            int ctot = 0, ke = 0;
+            for (int k = 0; k < K; ++k) {
+                if (!(allow >> k & 1u)) continue;
+                const uint32_t* sf = I.sufMinAll + size_t(k) * (L + 2);
+                unsigned cnt = 0;
+                for (int d = 1 + lane; d <= L; d += 32) cnt += (sf[d] <= T) ? 1u : 0u;   // sufMinAll is non-decreasing in d
+                cnt = __reduce_add_sync(0xffffffffu, cnt);                                // = longest admissible slice of k
+                ctot += int(cnt);
+                ke += cnt > 0 ? 1 : 0;
+            }
+            if (lane == 0) {
+                float w = 1.0f;
+                if (ctot >= L && ke > 0) {
+                    const int wd = min(I.Lp, (ctot - L + 4 + 3) & ~3), nbw = wd >> 2;
+                    int chp = 2;
+                    while (chp < nbw && chp < 16) chp <<= 1;
+                    w = float(ke) * exp2f(float(ke - 1)) * (5.5f + float(max(chp, nbw)));
+                }
+                sm.wgt[t] = w;
+            }
+        }
+        __syncthreads();
+        if (tid < 32) {
+            const int nCta = int(gridDim.x);
+            const float w = tid < nIt ? sm.wgt[tid] : 0.0f;
+            float tot = w;
+            for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+            int n = tid < nIt ? max(1, int(w / tot * float(nCta))) : 0;
+            int used = int(__reduce_add_sync(0xffffffffu, unsigned(n)));
+            // hand out what the rounding left (or take back what the one-CTA minimum overdrew), one CTA at a time,
+            // where it changes the slowest team's estimated time the most (least)
+            for (int guard = 0; used != nCta && guard < 512; ++guard) {
+                const bool give = used < nCta;
+                float v = tid < nIt ? (give ? w / float(n) : (n > 1 ? -w / float(n - 1) : -3.0e38f)) : -3.4e38f;
+                int who = tid;
+                for (int o = 16; o > 0; o >>= 1) {
+                    const float ov = __shfl_xor_sync(0xffffffffu, v, o);
+                    const int ow = __shfl_xor_sync(0xffffffffu, who, o);
+                    if (ov > v || (ov == v && ow < who)) { v = ov; who = ow; }
+                }
+                if (tid == who) n += give ? 1 : -1;
+                used += give ? 1 : -1;
+            }
+            int beg = n;
+            for (int o = 1; o < 32; o <<= 1) {
+                const int a = __shfl_up_sync(0xffffffffu, beg, o);
+                if (tid >= o) beg += a;
+            }
+            beg -= n;
+            if (tid < nIt) {
+                items[tid].ctaBeg = uint8_t(beg);
+                items[tid].ctaCnt = uint8_t(n);
+                for (int c = beg; c < beg + n; ++c) ctrl->teamOf[par][c] = uint8_t(tid);
+            }
+        }
+        __syncthreads();
+    }
     if (tid == 0) {
+        ctrl->weighted[par] = weighted ? 1 : 0;
         if (round < 256) {
             unsigned long long ns;
             asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
@@ -1054,10 +1125,18 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
             }
         } else {
             // team mode: team t = CTAs [t*nCta/nItems, (t+1)*nCta/nItems), slot = t
-            int t = int((int64_t(b) * nItems) / nCta);
-            while (t + 1 < nItems && int((int64_t(t + 1) * nCta) / nItems) <= b) ++t;
-            while (t > 0 && int((int64_t(t) * nCta) / nItems) > b) --t;
-            const int start = int((int64_t(t) * nCta) / nItems), end = int((int64_t(t + 1) * nCta) / nItems);
+            int t, start, end;
+            if (__ldcg(&ctrl->weighted[par])) {   // team sizes follow the estimated cost of the items
+                t = int(__ldcg(&ctrl->teamOf[par][b]));
+                start = int(__ldcg(&items[t].ctaBeg));
+                end = start + int(__ldcg(&items[t].ctaCnt));
+            } else {
+                t = int((int64_t(b) * nItems) / nCta);
+                while (t + 1 < nItems && int((int64_t(t + 1) * nCta) / nItems) <= b) ++t;
+                while (t > 0 && int((int64_t(t) * nCta) / nItems) > b) --t;
+                start = int((int64_t(t) * nCta) / nItems);
+                end = int((int64_t(t + 1) * nCta) / nItems);
+            }
             tgRunItem(ctx, sm, Cs, wbufAll, items + t, keys + t, b - start, end - start, t);
             if (b == start && threadIdx.x == 0 && round < 8 && t < 16) {
                 unsigned long long ns;
