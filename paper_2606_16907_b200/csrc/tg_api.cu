@@ -302,6 +302,9 @@ tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cud
         for (int r = 0; r < nr; ++r)
             fprintf(stderr, "[tg]  round %3d items %5d  %8.1f us\n", r, hc.roundItems[r],
                     r + 1 < nr ? double(hc.roundNs[r + 1] - hc.roundNs[r]) * 1e-3 : 0.0);
+        for (int r = 0; r < nr && r < 8; ++r)
+            fprintf(stderr, "[tg]  round %3d scheduler cycles: fold %lld plan %lld teams %lld\n", r, hc.schedCyc[r][1] - hc.schedCyc[r][0],
+                    hc.schedCyc[r][2] - hc.schedCyc[r][1], hc.schedCyc[r][3] - hc.schedCyc[r][2]);
         for (int r = 0; r < nr && r < 8; ++r) {
             if (hc.roundItems[r] > 16 || hc.roundItems[r] >= W.ctx.nSlots) continue;
             fprintf(stderr, "[tg]  round %3d items (candidate: us)", r);

@@ -98,6 +98,7 @@ struct TgCtrl {
     int32_t roundItems[256];
     unsigned long long itemNs[8][16];   // team mode: finish time of the first items of the first rounds
     int32_t itemTidx[8][16];
+    long long schedCyc[8][4];           // scheduler of the first rounds: clock at entry, after fold, after plan, at exit
 };
 
 struct TgSolveCtx {

@@ -643,20 +643,19 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
             for (int j = 0; j < Ke; ++j) if (R >> j & 1u) capR += sm.maxlenK[j];
             const int lo4R = tgLo4(sm, capR);
             unsigned long long best = TG_KEY_NONE;
-            for (int bb = a + 1 + lane; bb <= L - 1; bb += 32) {
+            // lanes over (member j, boundary b) pairs, b inside the source rows' window: every load is independent
+            const int bLo = max(a + 1, lo4R), nb = min(L - 1, lo4R + Wd - 1) - bLo + 1;
+            for (int p = lane; p < nb * r; p += 32) {
+                const int ji = p / nb, bb = bLo + (p - ji * nb);
                 const uint32_t c = cdk[tgGOff(L, bb - a) + a];
-                if (c > T || bb < lo4R || bb >= lo4R + Wd) continue;
-                uint32_t h = TG_INFU; int hj = 0;
-                for (int j = 0; j < Ke; ++j) {
-                    if (!(R >> j & 1u)) continue;
-                    const uint32_t Rp = R ^ (1u << j);
-                    const size_t row = size_t(ctx.rankOf[Rp]) * (Ke - r + 1) + (j - __popc(R & ((1u << j) - 1u)));
-                    const uint32_t v = I.x[ko * TG_MAX_K + isl[j]] + __ldcg(Gl + row * Wd + (bb - lo4R));
-                    if (v < h) { h = v; hj = j; }
-                }
-                const uint32_t v = c + h;
+                if (c > T) continue;
+                const int j = int(__fns(R, 0, ji + 1));
+                const uint32_t Rp = R ^ (1u << j);
+                const size_t row = size_t(ctx.rankOf[Rp]) * (Ke - r + 1) + (j - __popc(R & ((1u << j) - 1u)));
+                const uint32_t v = c + I.x[ko * TG_MAX_K + isl[j]] + __ldcg(Gl + row * Wd + (bb - lo4R));
                 if (v >= TG_INFU) continue;
-                const unsigned long long kk = (unsigned long long)v << 32 | (unsigned long long)bb << 8 | (unsigned long long)hj;
+                // lowest value, then lowest b, then lowest j
+                const unsigned long long kk = (unsigned long long)v << 32 | (unsigned long long)bb << 8 | (unsigned long long)j;
                 best = kk < best ? kk : best;
             }
             for (int o = 16; o > 0; o >>= 1) {
@@ -786,22 +785,38 @@ __device__ void tgWriteInfeasible(const TgSolveCtx& ctx, TgInstDev& I, int i) {
     I.phase = TG_PH_DONE;
 }
 
+// The previous round's items as the scheduler reads them: the first nStage are staged in shared memory by
+// the whole CTA (one L2 round trip for all of them instead of one per access of a single thread).
+struct TgPrev {
+    const TgItem* items;
+    const unsigned long long* keys;
+    const unsigned long long* keyS;
+    const int32_t* tidxS;
+    const uint32_t* candS;   // cand[tidx] of the item's instance
+    const uint8_t* flagS;
+    int nStage;
+    __device__ __forceinline__ unsigned long long key(int i) const { return i < nStage ? keyS[i] : __ldcg(keys + i); }
+    __device__ __forceinline__ int tidx(int i) const { return i < nStage ? tidxS[i] : __ldcg(&items[i].tidx); }
+    __device__ __forceinline__ int flags(int i) const { return i < nStage ? int(flagS[i]) : int(__ldcg(&items[i].flags)); }
+    __device__ __forceinline__ uint32_t cand(const TgInstDev& I, int i, int tx) const { return i < nStage ? candS[i] : I.cand[tx]; }
+};
+
 // Fold the results of instance i's items of the previous round (ascending candidate index).
-__device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem* itemsPrev, const unsigned long long* keysPrev,
-                               bool full) {
+__device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev& P, bool full) {
+    const TgItem* itemsPrev = P.items;
     const int beg = I.itemBeg, cnt = I.itemCnt;
     I.itemCnt = 0;
     if (I.phase == TG_PH_FINAL) { I.phase = TG_PH_DONE; return; }   // result written by the back-tracker
     int nf = 0;
     int nRes = cnt;   // a speculative final DP, if any, is the last item: not a search result
-    if (nRes > 0 && (__ldcg(&itemsPrev[beg + nRes - 1].flags) & 1)) --nRes;
+    if (nRes > 0 && (P.flags(beg + nRes - 1) & 1)) --nRes;
     for (int q = 0; q < nRes; ++q) {
-        const int tidx = __ldcg(&itemsPrev[beg + q].tidx);
-        const unsigned long long key = __ldcg(keysPrev + beg + q);
+        const int tidx = P.tidx(beg + q);
+        const unsigned long long key = P.key(beg + q);
         if (key == TG_KEY_NONE) { I.loInf = max(I.loInf, tidx); continue; }
         ++nf;
         I.hiFeas = I.hiFeas < 0 ? tidx : min(I.hiFeas, tidx);
-        const int64_t it = int64_t(key >> 32) + int64_t(I.m - 1) * int64_t(I.cand[tidx]);
+        const int64_t it = int64_t(key >> 32) + int64_t(I.m - 1) * int64_t(P.cand(I, beg + q, tidx));
         if (I.incIdx < 0 || it < I.incIter || (it == I.incIter && tidx < I.incIdx)) {
             I.incIter = it; I.incIdx = tidx;
             const uint32_t Sc = uint32_t(key >> 8) & 0xffffu;   // compact labels of that item
@@ -811,7 +826,7 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem
         }
     }
     I.nrun += cnt;
-    if (I.phase == TG_PH_SWEEP) { I.next = __ldcg(&itemsPrev[beg + cnt - 1].tidx) + 1; return; }
+    if (I.phase == TG_PH_SWEEP) { I.next = P.tidx(beg + cnt - 1) + 1; return; }
     if (nRes == 0) return;
     if (full || nf == 0) return;
     // merge the feasible results into the evaluated list (both ascending), from the back
@@ -833,9 +848,9 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgItem
     }
     int e = I.nEval - 1, w = I.nEval + nf - 1, q = nRes - 1;
     while (q >= 0) {
-        const unsigned long long key = __ldcg(keysPrev + beg + q);
+        const unsigned long long key = P.key(beg + q);
         if (key == TG_KEY_NONE) { --q; continue; }
-        const int tidx = __ldcg(&itemsPrev[beg + q].tidx);
+        const int tidx = P.tidx(beg + q);
         if (e >= 0 && (I.eIdx[e] & ~TG_EDONE) > tidx) { I.eIdx[w] = I.eIdx[e]; I.eF[w] = I.eF[e]; --e; --w; }
         else { I.eIdx[w] = tidx; I.eF[w] = uint32_t(key >> 32); --w; --q; }
     }
@@ -932,7 +947,7 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
     return TG_PH_DONE;
 }
 
-__device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
+__device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, int round) {
     const int tid = threadIdx.x;
     const int par = round & 1, prv = par ^ 1;
     TgCtrl* ctrl = ctx.ctrl;
@@ -944,18 +959,39 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     const int nInst = ctx.nInst;
 
     if (tid == 0) { sm.iTmp[0] = 0; sm.iTmp[1] = 0; sm.llTmp[0] = 0; sm.llTmp[1] = 0; }
+    if (tid == 0 && round < 8) ctrl->schedCyc[round][0] = clock64();
     __syncthreads();
 
     // ---- A: fold the previous round ---------------------------------------------------------
+    TgPrev P;
+    {   // stage keys, candidate indices, their thresholds and flags of the previous items in the (idle) dynamic shared memory
+        const int nPrev = round > 0 ? ctrl->nItems[prv] : 0;
+        const int room = int((size_t(ctx.csWords) + size_t(ctx.nActiveWarps) * ctx.wbufWords) * 4 / 20);   // 17 bytes an item, padded
+        const int nStage = min(nPrev, room) & ~1;   // even: keeps the arrays behind the keys 8-byte aligned
+        unsigned long long* keyS = reinterpret_cast<unsigned long long*>(dyn);
+        int32_t* tidxS = reinterpret_cast<int32_t*>(keyS + nStage);
+        uint32_t* candS = reinterpret_cast<uint32_t*>(tidxS + nStage);
+        uint8_t* flagS = reinterpret_cast<uint8_t*>(candS + nStage);
+        for (int q = tid; q < nStage; q += TG_NT) {
+            const int tx = __ldcg(&itemsPrev[q].tidx);
+            keyS[q] = __ldcg(keysPrev + q);
+            tidxS[q] = tx;
+            flagS[q] = __ldcg(&itemsPrev[q].flags);
+            candS[q] = tx >= 0 ? ctx.inst[__ldcg(&itemsPrev[q].inst)].cand[tx] : 0u;
+        }
+        P.items = itemsPrev; P.keys = keysPrev; P.keyS = keyS; P.tidxS = tidxS; P.candS = candS; P.flagS = flagS; P.nStage = nStage;
+        __syncthreads();
+    }
     int nActive = 0;
     for (int i = tid; i < nInst; i += TG_NT) {
         TgInstDev& I = ctx.inst[i];
-        if (I.itemCnt > 0) tgFoldInstance(ctx, I, itemsPrev, keysPrev, full);
+        if (I.itemCnt > 0) tgFoldInstance(ctx, I, P, full);
         if (I.phase != TG_PH_DONE) ++nActive;
     }
     if (nActive) atomicAdd(&sm.iTmp[0], nActive);
     __syncthreads();
     nActive = sm.iTmp[0];
+    if (tid == 0 && round < 8) ctrl->schedCyc[round][1] = clock64();
     if (nActive == 0) {
         if (tid == 0) { ctrl->done = 1; ctrl->nItems[par] = 0; }
         return;
@@ -992,6 +1028,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     }
     __syncthreads();
     const int nIt = sm.iTmp[1];
+    if (tid == 0 && round < 8) ctrl->schedCyc[round][2] = clock64();
 
     // (the geometry of an item -- islands alive at its T -- is worked out by the CTAs that run it)
     for (int idx = tid; idx < nIt; idx += TG_NT) keys[idx] = TG_KEY_NONE;
@@ -1009,16 +1046,18 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
             const int L = I.L, K = I.K;
             const uint32_t T = it.T;
             const uint32_t allow = ((it.flags & 1) && ctx.mode == 0) ? I.incMask : 0xffffu;   // as in tgStageItem
-            int ctot = 0, ke = 0;
-            for (int k = 0; k < K; ++k) {
-                if (!(allow >> k & 1u)) continue;
+            // lane = (island k, half of the lengths d): counts the admissible lengths of its half -- sufMinAll is
+            // non-decreasing in d, so the count over both halves is the longest admissible slice of k
+            const int k = lane & 15, half = lane >> 4;
+            unsigned cnt = 0;
+            if (k < K && (allow >> k & 1u)) {
                 const uint32_t* sf = I.sufMinAll + size_t(k) * (L + 2);
-                unsigned cnt = 0;
-                for (int d = 1 + lane; d <= L; d += 32) cnt += (sf[d] <= T) ? 1u : 0u;   // sufMinAll is non-decreasing in d
-                cnt = __reduce_add_sync(0xffffffffu, cnt);                                // = longest admissible slice of k
-                ctot += int(cnt);
-                ke += cnt > 0 ? 1 : 0;
+#pragma unroll 8
+                for (int d = 1 + half; d <= L; d += 2) cnt += (sf[d] <= T) ? 1u : 0u;
             }
+            cnt += __shfl_xor_sync(0xffffffffu, cnt, 16);
+            const int ke = __popc(__ballot_sync(0xffffffffu, cnt > 0) & 0xffffu);
+            const int ctot = int(__reduce_add_sync(0xffffffffu, half == 0 ? cnt : 0u));
             if (lane == 0) {
                 float w = 1.0f;
                 if (ctot >= L && ke > 0) {
@@ -1068,6 +1107,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     }
     if (tid == 0) {
         ctrl->weighted[par] = weighted ? 1 : 0;
+        if (round < 8) ctrl->schedCyc[round][3] = clock64();
         if (round < 256) {
             unsigned long long ns;
             asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
@@ -1104,7 +1144,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
     __syncthreads();
     for (int round = 0;; ++round) {
         const int par = round & 1;
-        if (b == 0) { tgSchedule(ctx, sm, round); tgMark(sm, 6); }
+        if (b == 0) { tgSchedule(ctx, sm, dyn, round); tgMark(sm, 6); }
         tgGridBarrier(ctrl, epoch);
         tgMark(sm, 5);
         if (__ldcg(&ctrl->done)) break;
