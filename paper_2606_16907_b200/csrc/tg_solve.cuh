@@ -761,17 +761,24 @@ __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
 //   FINAL  DP at T* keeping every level, followed by the back-track
 // ---------------------------------------------------------------------------------------------
 // could candidate c, whose sum is at least lbF, still beat the incumbent?
-__device__ __forceinline__ bool tgBeats(const TgInstDev& I, int64_t lbF, int c) {
-    if (I.incIdx < 0) return true;
-    const int64_t lb = lbF + int64_t(I.m - 1) * int64_t(__ldg(I.cand + c));   // cand is read-only during the solve
-    return lb < I.incIter || (lb == I.incIter && c < I.incIdx);
+// (the incumbent and the candidate list, read once into registers: the scheduler is a single thread per
+// instance and every field of TgInstDev it touches is a memory access)
+struct TgInc {
+    int64_t incIter, m1;
+    int incIdx;
+    const uint32_t* cand;
+};
+__device__ __forceinline__ bool tgBeats(const TgInc& B, int64_t lbF, int c) {
+    if (B.incIdx < 0) return true;
+    const int64_t lb = lbF + B.m1 * int64_t(__ldg(B.cand + c));   // cand is read-only during the solve
+    return lb < B.incIter || (lb == B.incIter && c < B.incIdx);
 }
 
 // last c in [lo, hi] with tgBeats(lbF, c), given tgBeats(lbF, lo) (the predicate holds on a prefix)
-__device__ __forceinline__ int tgLastBeating(const TgInstDev& I, int64_t lbF, int lo, int hi) {
+__device__ __forceinline__ int tgLastBeating(const TgInc& B, int64_t lbF, int lo, int hi) {
     while (lo < hi) {
         const int mid = (lo + hi + 1) >> 1;
-        if (tgBeats(I, lbF, mid)) lo = mid; else hi = mid - 1;
+        if (tgBeats(B, lbF, mid)) lo = mid; else hi = mid - 1;
     }
     return lo;
 }
@@ -810,20 +817,26 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev
     int nf = 0;
     int nRes = cnt;   // a speculative final DP, if any, is the last item: not a search result
     if (nRes > 0 && (P.flags(beg + nRes - 1) & 1)) --nRes;
+    int loInf = I.loInf, hiFeas = I.hiFeas, incIdx = I.incIdx, incQ = -1;
+    int64_t incIter = I.incIter;
+    const int64_t m1 = int64_t(I.m - 1);
+    unsigned long long incKey = 0;
     for (int q = 0; q < nRes; ++q) {
         const int tidx = P.tidx(beg + q);
         const unsigned long long key = P.key(beg + q);
-        if (key == TG_KEY_NONE) { I.loInf = max(I.loInf, tidx); continue; }
+        if (key == TG_KEY_NONE) { loInf = max(loInf, tidx); continue; }
         ++nf;
-        I.hiFeas = I.hiFeas < 0 ? tidx : min(I.hiFeas, tidx);
-        const int64_t it = int64_t(key >> 32) + int64_t(I.m - 1) * int64_t(P.cand(I, beg + q, tidx));
-        if (I.incIdx < 0 || it < I.incIter || (it == I.incIter && tidx < I.incIdx)) {
-            I.incIter = it; I.incIdx = tidx;
-            const uint32_t Sc = uint32_t(key >> 8) & 0xffffu;   // compact labels of that item
-            uint32_t So = 0;
-            for (int e = 0; e < TG_MAX_K; ++e) if (Sc >> e & 1u) So |= 1u << __ldcg(&itemsPrev[beg + q].isl[e]);
-            I.incMask = So;
-        }
+        hiFeas = hiFeas < 0 ? tidx : min(hiFeas, tidx);
+        const int64_t it = int64_t(key >> 32) + m1 * int64_t(P.cand(I, beg + q, tidx));
+        if (incIdx < 0 || it < incIter || (it == incIter && tidx < incIdx)) { incIter = it; incIdx = tidx; incQ = q; incKey = key; }
+    }
+    I.loInf = loInf; I.hiFeas = hiFeas;
+    if (incQ >= 0) {
+        I.incIter = incIter; I.incIdx = incIdx;
+        const uint32_t Sc = uint32_t(incKey >> 8) & 0xffffu;   // compact labels of that item
+        uint32_t So = 0;
+        for (int e = 0; e < TG_MAX_K; ++e) if (Sc >> e & 1u) So |= 1u << __ldcg(&itemsPrev[beg + incQ].isl[e]);
+        I.incMask = So;
     }
     I.nrun += cnt;
     if (I.phase == TG_PH_SWEEP) { I.next = P.tidx(beg + cnt - 1) + 1; return; }
@@ -846,15 +859,19 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev
         I.phase = TG_PH_FINAL;
         return;
     }
-    int e = I.nEval - 1, w = I.nEval + nf - 1, q = nRes - 1;
+    const int nEval = I.nEval;
+    int32_t* const eIdx = I.eIdx;
+    uint32_t* const eF = I.eF;
+    int e = nEval - 1, w = nEval + nf - 1, q = nRes - 1;
     while (q >= 0) {
         const unsigned long long key = P.key(beg + q);
         if (key == TG_KEY_NONE) { --q; continue; }
         const int tidx = P.tidx(beg + q);
-        if (e >= 0 && (I.eIdx[e] & ~TG_EDONE) > tidx) { I.eIdx[w] = I.eIdx[e]; I.eF[w] = I.eF[e]; --e; --w; }
-        else { I.eIdx[w] = tidx; I.eF[w] = uint32_t(key >> 32); --w; --q; }
+        const int ev = e >= 0 ? eIdx[e] : 0;
+        if (e >= 0 && (ev & ~TG_EDONE) > tidx) { eIdx[w] = ev; eF[w] = eF[e]; --e; --w; }
+        else { eIdx[w] = tidx; eF[w] = uint32_t(key >> 32); --w; --q; }
     }
-    I.nEval += nf;
+    I.nEval = nEval + nf;
 }
 
 // Plan the probes of instance i for this round into I.probe[0..nProbe).  Returns the item kind.
@@ -895,38 +912,48 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
         int sLo[16], sHi[16], ns = 0;
         long long total = 0;
         bool truncated = false;
-        for (int t = 1; t < I.nEval; ++t) {
+        const TgInc B = {I.incIter, int64_t(I.m - 1), I.incIdx, I.cand};
+        const int nEval = I.nEval;
+        int32_t* const eIdx = I.eIdx;
+        const uint32_t* const eF = I.eF;
+        int a = eIdx[0] & ~TG_EDONE;   // left neighbour of the point under test
+        for (int t = 1; t < nEval; ++t) {
             if (ns >= 15) { truncated = true; break; }
-            const int ej = I.eIdx[t];
+            const int ej = eIdx[t], aPrev = a;
+            a = ej & ~TG_EDONE;
             if (ej & TG_EDONE) continue;
-            const int a = I.eIdx[t - 1] & ~TG_EDONE;
-            if (ej - a <= 1 || !tgBeats(I, int64_t(I.eF[t]), a + 1)) { I.eIdx[t] = ej | TG_EDONE; continue; }
-            sLo[ns] = a; sHi[ns] = tgLastBeating(I, int64_t(I.eF[t]), a + 1, ej - 1);
+            const int64_t f = int64_t(eF[t]);
+            if (ej - aPrev <= 1 || !tgBeats(B, f, aPrev + 1)) { eIdx[t] = ej | TG_EDONE; continue; }
+            sLo[ns] = aPrev; sHi[ns] = tgLastBeating(B, f, aPrev + 1, ej - 1);
             total += sHi[ns] - sLo[ns];
             ++ns;
         }
         int topEnd = -1;
         {   // above the last evaluated point only the trivial bound f >= 0 is known: probe just the right end of
             // that stretch; once it is evaluated the stretch gets a real bound and shrinks
-            const int a = I.eIdx[I.nEval - 1] & ~TG_EDONE;
-            if (a < n - 1 && tgBeats(I, 0, a + 1)) topEnd = tgLastBeating(I, 0, a + 1, n - 1);
+            const int last = eIdx[nEval - 1] & ~TG_EDONE;
+            if (last < n - 1 && tgBeats(B, 0, last + 1)) topEnd = tgLastBeating(B, 0, last + 1, n - 1);
         }
         if (ns == 0 && topEnd < 0) I.phase = TG_PH_FINAL;
         else {
             int budget = topEnd >= 0 ? W - 1 : W;
             const int budget0 = budget;
+            int32_t* const probe = I.probe;
+            int np = 0;
             for (int s = 0; s < ns && budget > 0; ++s) {
                 const int size = sHi[s] - sLo[s];
                 int share = int(max(1ll, (long long)budget0 * size / max(total, 1ll)));
                 share = min(min(share, size), budget);
-                for (int q = 1; q <= share; ++q) I.probe[I.nProbe++] = sLo[s] + int(((long long)q * size + share - 1) / share);
+                for (int q = 1; q <= share; ++q) probe[np++] = sLo[s] + int(((long long)q * size + share - 1) / share);
                 budget -= share;
             }
-            if (topEnd >= 0) { I.probe[I.nProbe++] = topEnd; total += W; }   // (total += W: not every candidate is probed)
+            if (topEnd >= 0) { probe[np++] = topEnd; total += W; }   // (total += W: not every candidate is probed)
             // every unresolved candidate is probed this round: run the final DP at the incumbent alongside
             // (speculation: it stands unless one of these probes takes the incumbent over)
-            I.specIdx = -1;
-            if (!truncated && total < W && I.nProbe == int(total)) { I.probe[I.nProbe++] = I.incIdx | TG_PROBE_FINAL; I.specIdx = I.incIdx; }
+            int spec = -1;
+            if (!truncated && total < W && np == int(total)) { probe[np++] = B.incIdx | TG_PROBE_FINAL; spec = B.incIdx; }
+            I.specIdx = spec;
+            I.nProbe = np;
             return TG_PH_BNB;
         }
     }
