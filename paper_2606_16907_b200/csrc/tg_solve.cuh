@@ -1091,7 +1091,8 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
                     const int wd = min(I.Lp, (ctot - L + 4 + 3) & ~3), nbw = wd >> 2;
                     int chp = 2;
                     while (chp < nbw && chp < 16) chp <<= 1;
-                    w = float(ke) * exp2f(float(ke - 1)) * (5.5f + float(max(chp, nbw)));
+                    w = float(ke) * exp2f(float(ke - 1)) * (3.5f + float(max(chp, nbw)));
+                    if (it.flags & 1) w *= 1.5f;   // every level kept, a back-track at the end
                 }
                 sm.wgt[t] = w;
             }
