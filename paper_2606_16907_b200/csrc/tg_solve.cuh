@@ -64,15 +64,14 @@ __device__ __forceinline__ void tgGridBarrier(TgCtrl* ctrl, uint32_t& epoch) {
     __syncthreads();
     if (threadIdx.x == 0) {
         ++epoch;
-        __threadfence();
-        atomicAdd(&ctrl->barrier, 1u);
         const uint32_t target = epoch * gridDim.x;
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&ctrl->barrier) : "memory");
         while (true) {
-            const uint32_t v = *reinterpret_cast<volatile uint32_t*>(&ctrl->barrier);
+            uint32_t v;
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(&ctrl->barrier) : "memory");
             if (int32_t(v - target) >= 0) break;
-            __nanosleep(64);
+            __nanosleep(32);
         }
-        __threadfence();
     }
     __syncthreads();
 }
@@ -81,10 +80,13 @@ __device__ __forceinline__ void tgGridBarrier(TgCtrl* ctrl, uint32_t& epoch) {
 __device__ __forceinline__ void tgTeamBarrier(uint32_t* bar, uint32_t target) {
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(bar, 1u);
-        while (*reinterpret_cast<volatile uint32_t*>(bar) < target) __nanosleep(32);
-        __threadfence();
+        // release-arrive / acquire-poll: the CTA's writes (ordered before this thread by the barrier above) become
+        // visible to whoever observes the count, and what the other members wrote is visible after the poll
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+        uint32_t v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while (v < target);
     }
     __syncthreads();
 }
