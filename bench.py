@@ -64,41 +64,83 @@ def dense_plans(inst) -> int:
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled during the timed region (profiling recipe)."""
+    """SM clocks and throttle reasons sampled during the timed region (profiling recipe's clocks line).
+    Sampled in-process through NVML (the library nvidia-smi itself queries): spawning nvidia-smi ten times a
+    second from a thread of the timed process stalled the launching thread for tens of ms now and then.
+    Falls back to the nvidia-smi command line when the NVML binding is not importable."""
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+    BITS = [("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4)]
 
     def __init__(self, index: int):
         self.rows, self.stop, self.index = [], threading.Event(), index
+        self.active = threading.Event()      # set while the timed region runs: only those samples are kept
+        self.nvml = self.handle = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            try:
+                self.handle = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + str(torch.cuda.get_device_properties(index).uuid)).encode())
+            except Exception:
+                self.handle = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.reasons_fn = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or \
+                pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+            self.max_sm = int(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.nvml = pynvml
+        except Exception:
+            self.nvml = None
         self.th = threading.Thread(target=self._run, daemon=True)
+        self.th.start()                      # started before the warm-up: the first queries initialise driver state and are slow
+
+    def _sample_nvml(self):
+        n = self.nvml
+        sm = int(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+        mask = int(self.reasons_fn(self.handle))
+        self.rows.append([str(sm), str(self.max_sm)] + ["Active" if mask & bit else "Not Active" for _, bit in self.BITS])
+
+    def _sample_smi(self):
+        o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                            "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+        if o:
+            self.rows.append([c.strip() for c in o.splitlines()[0].split(",")])
 
     def _run(self):
         while not self.stop.is_set():
             try:
-                o = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                    "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
-                if o:
-                    self.rows.append([c.strip() for c in o.splitlines()[0].split(",")])
+                if self.nvml is not None:
+                    self._sample_nvml()
+                else:
+                    self._sample_smi()
             except Exception:
                 pass
-            self.stop.wait(0.1)
+            if not self.active.is_set():
+                self.rows.clear()            # priming samples outside the timed region are dropped
+            self.stop.wait(0.05 if self.nvml is not None else 0.25)
 
     def __enter__(self):
-        self.th.start()
+        self.rows.clear()
+        self.active.set()
         return self
 
     def __exit__(self, *a):
+        try:
+            if self.nvml is not None and not self.rows:
+                self._sample_nvml()          # a timed region shorter than the sampling period: sample before it closes
+        except Exception:
+            pass
+        self.active.clear()
         self.stop.set()
         self.th.join(timeout=6)
 
     def summary(self):
         if not self.rows:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["clock query unavailable"]}
         sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        names = [n for n, _ in self.BITS]
         reasons = [n for i, n in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in self.rows)]
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": int(self.rows[0][1]) if self.rows[0][1].isdigit() else None,
-                "reasons": reasons, "samples": len(self.rows)}
+                "reasons": reasons, "samples": len(self.rows), "source": "nvml" if self.nvml is not None else "nvidia-smi"}
 
 
 def peaks():
@@ -180,6 +222,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    clk = ClockSampler(local)
     for _ in range(args.warmup):
         tg.tg_solve_batch(handles, out=out, flags=flags, stats=st)
     barrier()
@@ -187,7 +230,7 @@ def run_ours(args):
     kern_ms, plans, states, n_dp = [], 0, 0, 0
     cyc = [0] * 8
     relax = 0
-    with ClockSampler(local) as clk:
+    with clk:
         for s in range(args.steps):
             flush.fill_(s & 0xff)                                     # evict L2 between timed steps
             ev[s][0].record(stream)
@@ -202,7 +245,8 @@ def run_ours(args):
             cyc = [c + int(v) for c, v in zip(cyc, st.cyc)]
             relax += int(st.relax_admissible)
         barrier()
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
     # ---- end to end: host tables -> create (H2D) -> solve -> host results (D2H) ----
     h2d = sum(i.time_us.nbytes + i.mem_mb.nbytes + i.bw_gbps.nbytes + 8 * i.K +
               (i.actmem_mb.nbytes if i.actmem_mb is not None else 0) for i in insts)
@@ -249,7 +293,9 @@ def run_ours(args):
                              "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.full_sweep)),
                              "traffic_source": "profiles/r1_ncu_cfg4_solver.md" if (args.workload, args.full_sweep) in NCU_TRAFFIC_BYTES else None,
                              "peak_source": peak_src,
-                             "kernel_ms": km, "algorithmic_bytes_per_launch": alg_bytes,
+                             "kernel_ms": km, "step_ms": [round(x, 3) for x in step_ms],
+                             "kernel_ms_steps": [round(x, 3) for x in kern_ms],
+                             "algorithmic_bytes_per_launch": alg_bytes,
                              "us_per_dp": km * 1e3 / (n_dp / args.steps),
                              "alu": {"relaxations_per_launch": relax / args.steps,
                                      "achieved_Trelax_s": relax / args.steps / (km * 1e-3) / 1e12,
