@@ -169,6 +169,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         while (cap < cells) cap <<= 1;
         I.sortCap = cap;
         for (int k = 0; k < TG_MAX_K; ++k) I.cminAll[k] = TG_INFU;
+        I.maxKey = 0;
         I.phase = TG_PH_NEW;
         I.incIdx = -1; I.hiFeas = -1; I.loInf = -1; I.specIdx = -1;
         uint64_t mx = 1;

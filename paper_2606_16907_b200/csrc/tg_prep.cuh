@@ -110,9 +110,12 @@ __global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ inst
     const int L = I.L, K = I.K, P = I.P;
     const int nCells = I.NS * K;
     __shared__ uint32_t sMin[TG_MAX_K];
+    __shared__ uint32_t sMax;
     if (int(blockIdx.x) * 256 >= nCells) return;
     if (threadIdx.x < TG_MAX_K) sMin[threadIdx.x] = TG_INFU;
+    if (threadIdx.x == 0) sMax = 0;
     __syncthreads();
+    uint32_t myMax = 0;
     const int cell = blockIdx.x * 256 + threadIdx.x;
     if (cell < nCells) {
         const int s = cell / K, k = cell - s * K;
@@ -148,11 +151,15 @@ __global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ inst
             I.sortbuf[size_t(q - 1) * nCells + cell] = (q == I.nDepth || bq != prev) ? bq : TG_INFU;
             prev = bq;
             best = bq;
+            if (bq < TG_INFU) myMax = max(myMax, bq);
         }
         if (best < TG_INFU) atomicMin(&sMin[k], best);
     }
+    myMax = __reduce_max_sync(0xffffffffu, myMax);
+    if ((threadIdx.x & 31) == 0 && myMax) atomicMax(&sMax, myMax);
     __syncthreads();
     if (threadIdx.x < K && sMin[threadIdx.x] < TG_INFU) atomicMin(&I.cminAll[threadIdx.x], sMin[threadIdx.x]);
+    if (threadIdx.x == 0 && sMax) atomicMax(&I.maxKey, sMax);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -163,57 +170,81 @@ __global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ inst
 // Sort: bitonic network on a power-of-two buffer, in shared memory when it fits, else in place in
 // global memory (L2 resident).
 // ---------------------------------------------------------------------------------------------
-// Stable LSD radix sort of A[0..n) (32-bit keys), 4 passes of 8 bits; B is scratch of the same size.
-// One CTA of TG_PREP_NT threads; hist = 32 warps x 256 digits in shared memory.  Returns A.
-__device__ uint32_t* tgRadixSort(uint32_t* A, uint32_t* B, int n, uint32_t* hist, uint32_t* warpSums) {
+// Stable LSD radix sort of A[0..n) (32-bit keys); B is scratch of the same size.  One CTA of TG_PREP_NT
+// threads; hist = 32 warps x 2^DB digits in shared memory.  Keys are either finite (<= maxKey) or TG_INFU:
+// they are sorted by  key' = min(key, maxKey + 1), which has nbits = bits(maxKey + 1) significant bits, in
+// ceil(nbits / DB) passes of DB = 8 or 9 bits (the paper-shaped tables need 17-19 bits: 2 passes of 9 instead
+// of 4 of 8).  Returns the buffer that holds the result.
+__device__ uint32_t* tgRadixSort(uint32_t* A, uint32_t* B, int n, uint32_t maxKey, uint32_t* hist, uint32_t* warpSums) {
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, nW = blockDim.x >> 5;
     const int chunk = (((n + nW - 1) / nW) + 31) & ~31;
     const int beg = min(n, w * chunk), end = min(n, beg + chunk);
-    uint32_t* myHist = hist + w * 256;
+    const uint32_t cap = maxKey + 1u;
+    const int nbits = 32 - __clz(cap);
+    const int DB = (nbits + 8) / 9 < (nbits + 7) / 8 ? 9 : 8;     // 9-bit digits only when they save a pass
+    const int nPass = (nbits + DB - 1) / DB, NB = 1 << DB;
+    const uint32_t dmask = uint32_t(NB - 1);
+    uint32_t* myHist = hist + w * NB;
     uint32_t *src = A, *dst = B;
-    for (int pass = 0; pass < 4; ++pass) {
-        const int shift = 8 * pass;
-        for (int e = tid; e < nW * 256; e += blockDim.x) hist[e] = 0;
+    for (int pass = 0; pass < nPass; ++pass) {
+        const int shift = DB * pass;
+        for (int e = tid; e < nW * NB; e += blockDim.x) hist[e] = 0;
         __syncthreads();
-        for (int b0 = beg; b0 < end; b0 += 32) {
-            const int i = b0 + lane;
-            const uint32_t d = i < end ? (__ldcg(src + i) >> shift) & 255u : 256u + uint32_t(lane);
-            const uint32_t peers = __match_any_sync(0xffffffffu, d);
-            if (d < 256u && lane == __ffs(peers) - 1) myHist[d] += __popc(peers);
-            __syncwarp();
+        for (int b0 = beg; b0 < end; b0 += 128) {   // four groups of 32 keys, loaded together (one L2 latency, not four)
+            uint32_t v4[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) { const int i = b0 + 32 * e + lane; v4[e] = i < end ? __ldcg(src + i) : 0u; }
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int i = b0 + 32 * e + lane;
+                const uint32_t d = i < end ? (min(v4[e], cap) >> shift) & dmask : uint32_t(NB + lane);
+                const uint32_t peers = __match_any_sync(0xffffffffu, d);
+                if (d < uint32_t(NB) && lane == __ffs(peers) - 1) myHist[d] += __popc(peers);
+                __syncwarp();
+            }
         }
         __syncthreads();
-        {   // exclusive scan in (digit major, warp minor) order; each thread owns 8 consecutive entries
-            const int per = (nW * 256) / blockDim.x;   // 8 for 32 warps
-            uint32_t loc[8], sum = 0;
-            for (int q = 0; q < per; ++q) { const int e = tid * per + q; loc[q] = hist[(e % nW) * 256 + e / nW]; sum += loc[q]; }
+        {   // exclusive scan in (digit major, warp minor) order; each thread owns `per` consecutive entries
+            const int per = (nW * NB) / blockDim.x;   // 8 or 16 for 32 warps
+            uint32_t loc[16], sum = 0;
+#pragma unroll
+            for (int q = 0; q < 16; ++q)
+                if (q < per) { const int e = tid * per + q; loc[q] = hist[(e % nW) * NB + e / nW]; sum += loc[q]; }
             uint32_t tot;
             uint32_t run = tgBlockExScan(sum, warpSums, tot);
-            for (int q = 0; q < per; ++q) { const int e = tid * per + q; hist[(e % nW) * 256 + e / nW] = run; run += loc[q]; }
+#pragma unroll
+            for (int q = 0; q < 16; ++q)
+                if (q < per) { const int e = tid * per + q; hist[(e % nW) * NB + e / nW] = run; run += loc[q]; }
         }
         __syncthreads();
-        for (int b0 = beg; b0 < end; b0 += 32) {
-            const int i = b0 + lane;
-            const uint32_t v = i < end ? __ldcg(src + i) : 0u;
-            const uint32_t d = i < end ? (v >> shift) & 255u : 256u + uint32_t(lane);
-            const uint32_t peers = __match_any_sync(0xffffffffu, d);
-            uint32_t pos = 0;
-            if (d < 256u) pos = myHist[d] + __popc(peers & ((1u << lane) - 1u));
-            __syncwarp();
-            if (d < 256u) {
-                dst[pos] = v;
-                if (lane == __ffs(peers) - 1) myHist[d] += __popc(peers);
+        for (int b0 = beg; b0 < end; b0 += 128) {   // groups in index order (stability), loads up front
+            uint32_t v4[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) { const int i = b0 + 32 * e + lane; v4[e] = i < end ? __ldcg(src + i) : 0u; }
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int i = b0 + 32 * e + lane;
+                const uint32_t v = v4[e];
+                const uint32_t d = i < end ? (min(v, cap) >> shift) & dmask : uint32_t(NB + lane);
+                const uint32_t peers = __match_any_sync(0xffffffffu, d);
+                uint32_t pos = 0;
+                if (d < uint32_t(NB)) pos = myHist[d] + __popc(peers & ((1u << lane) - 1u));
+                __syncwarp();
+                if (d < uint32_t(NB)) {
+                    dst[pos] = v;
+                    if (lane == __ffs(peers) - 1) myHist[d] += __popc(peers);
+                }
+                __syncwarp();
             }
-            __syncwarp();
         }
         __syncthreads();
         uint32_t* t = src; src = dst; dst = t;
     }
-    return src;   // 4 passes: back in A
+    return src;
 }
 
 #define TG_PREP_NT 1024
-#define TG_SORT_SMEM_MAX 8192     // words of dynamic shared memory of the prepare kernel (radix histograms)
+#define TG_SORT_SMEM_MAX 16384    // words of dynamic shared memory of the prepare kernel (radix histograms: 32 warps x 512 digits)
 
 __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restrict__ insts) {
     extern __shared__ uint32_t sbuf[];
@@ -243,32 +274,42 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
             for (int a = 0; a <= L - 1 - d; ++a) mn = min(mn, row[a]);
             mnAll = min(mn, row[L - d]);
         }
-        sm[w] = mn;
-        sma[w] = mnAll;
+        sbuf[w] = mn;                 // (shared memory: the suffix scan below is a chain of dependent accesses)
+        sbuf[K * stride + w] = mnAll;
     }
     __syncthreads();
     if (tid < 2 * K) {
-        uint32_t* s2 = tid < K ? sm : sma;
-        const int k = tid < K ? tid : tid - K;
+        uint32_t* s2 = sbuf + tid * stride;   // rows 0..K-1: b <= L-1 only, rows K..2K-1: every slice
         uint32_t run = TG_INFU;
-        for (int d = L + 1; d >= 0; --d) { run = min(run, s2[k * stride + d]); s2[k * stride + d] = run; }
+        for (int d = L + 1; d >= 0; --d) { run = min(run, s2[d]); s2[d] = run; }
     }
-    // candidate sort: stable LSD radix sort, 8-bit digits, ping-pong between the two global buffers
+    __syncthreads();
+    for (int w = tid; w < K * stride; w += TG_PREP_NT) { sm[w] = sbuf[w]; sma[w] = sbuf[K * stride + w]; }
+    __syncthreads();
+    // candidate sort: stable LSD radix sort, 8- or 9-bit digits, ping-pong between the two global buffers
     // (L2 resident); per-warp digit histograms in shared memory, warp w owns a contiguous chunk
     const int n = I.NS * K * I.nDepth;
-    uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, sbuf, warpSums);
+    uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, I.maxKey, sbuf, warpSums);
     // unique, finite only
     uint32_t base = 0;
-    for (int i0 = 0; i0 < n; i0 += TG_PREP_NT) {
-        const int i = i0 + tid;
-        uint32_t v = 0xffffffffu, f = 0;
-        if (i < n) { v = __ldcg(buf + i); f = (v < TG_INFU && (i == 0 || __ldcg(buf + i - 1) != v)) ? 1u : 0u; }
+    for (int i0 = 0; i0 < n; i0 += 4 * TG_PREP_NT) {   // four consecutive keys a thread: one block scan per 4096 keys
+        const int i = i0 + 4 * tid;
+        uint32_t v[5], f[4], cnt = 0;
+        v[0] = (i > 0 && i < n) ? __ldcg(buf + i - 1) : 0xffffffffu;   // left neighbour of the thread's first key
+#pragma unroll
+        for (int e = 0; e < 4; ++e) v[e + 1] = i + e < n ? __ldcg(buf + i + e) : 0xffffffffu;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { f[e] = (v[e + 1] < TG_INFU && (i + e == 0 || v[e] != v[e + 1])) ? 1u : 0u; cnt += f[e]; }
         uint32_t tot;
-        const uint32_t pos = tgBlockExScan(f, warpSums, tot);
-        if (f) I.cand[base + pos] = v;
+        uint32_t pos = base + tgBlockExScan(cnt, warpSums, tot);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) if (f[e]) I.cand[pos++] = v[e + 1];
         base += tot;
     }
     if (tid == 0) I.ncand = int(base);
+    // (the suffix minima go to shared memory for the search below: it is a chain of dependent reads)
+    uint32_t* smaS = sbuf;
+    for (int w = tid; w < K * stride; w += TG_PREP_NT) smaS[w] = sma[w];
     __syncthreads();
     // Necessary condition for feasibility at T: the longest admissible slices of the islands must add
     // up to at least L layers.  lbIdx = first candidate that passes (ncand if none): the threshold
@@ -281,7 +322,7 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
             const uint32_t T = I.cand[mid];
             int len = 0;
             if (tid < K) {
-                const uint32_t* sf = sma + tid * stride;
+                const uint32_t* sf = smaS + tid * stride;
                 int l2 = 0, h2 = L;
                 while (l2 < h2) {
                     const int m2 = (l2 + h2 + 1) >> 1;
