@@ -165,5 +165,28 @@ def bruteforce_depth(inst) -> Result:
     return _conv(r)
 
 
+def _args_variant(inst):
+    keep, a = _args(inst)
+    am = None if inst.actmem_mb is None else np.ascontiguousarray(inst.actmem_mb, dtype=np.int32)
+    amp = C.cast(None, _I32P) if am is None else _p32(am)
+    return (keep, am), a[:6] + (amp,) + a[6:] + (C.c_int(1 if getattr(inst, "transfer_bound", False) else 0),)
+
+
+def solve_variant(inst) -> Result:
+    """Variants of SURVEY §8(f): NEXT-1 depth-aware memory (inst.actmem_mb) and NEXT-3(b) transfers bounded by
+    T (inst.transfer_bound), alone or together; with neither this is the core definition."""
+    keep, a = _args_variant(inst)
+    r = _Res()
+    lib().orc_variant_solve(*a, C.byref(r))
+    return _conv(r)
+
+
+def bruteforce_variant(inst) -> Result:
+    keep, a = _args_variant(inst)
+    r = _Res()
+    lib().orc_variant_bruteforce(*a, C.byref(r))
+    return _conv(r)
+
+
 def hw_threads() -> int:
     return lib().orc_hw_threads()

@@ -13,6 +13,16 @@
 // sum = sum c_q + sum x, T = max c_q, iter = sum + (m-1) T, result = argmin of
 // (iter, T, mask, k_0, b_0, k_1, b_1, ...).  Stage i of an n-stage plan has q = n - i.
 //
+// Second variant in the same unit, SURVEY.md §8(f) NEXT-3(b) / reading A2: the transfer counts toward the
+// bottleneck ("communication can be the bottleneck"; each boundary transfer is its own pipeline
+// slot).  With the flag `xbound` (reading N3b) a plan's bottleneck is
+//     T = max( max_i c_i , max_i x[k_i][k_{i+1}] )
+// i.e. at threshold T a transfer is admissible iff x <= T, and the candidate thresholds are the distinct
+// finite values of c and of the off-diagonal x.  Everything else is unchanged; xbound = 0 and actmem = null
+// (treated as zeros) is the core definition.  Pinned like the depth variant: orc_variant_solve ==
+// orc_variant_bruteforce on tiny instances, flag off == core oracle, the optimum never improves when the
+// flag is switched on, re-scoring from the raw tables.
+//
 // Pins (tests/test_oracle_depth.py): orc_depth_solve == orc_depth_bruteforce (literal enumeration)
 // on thousands of tiny instances; actmem = 0 reproduces the core oracle bit for bit; raising actmem
 // never improves the optimum; a plan re-scored from the raw tables with the depth rule reproduces
@@ -33,8 +43,9 @@ constexpr int MAXK = 16;
 
 struct Inst {
     int L, K, P, m;
-    const int32_t *time_us, *mem_mb, *actmem_mb, *cap_mb, *bw_gbps;
+    const int32_t *time_us, *mem_mb, *actmem_mb, *cap_mb, *bw_gbps;   // actmem_mb may be null (= zeros)
     int act_mb;
+    int xbound = 0;   // NEXT-3(b): transfers are bounded by T as well
     int NS() const { return L * (L + 1) / 2; }
 };
 
@@ -61,7 +72,8 @@ Reduced reduce_tables(const Inst& I) {
                 for (int p = 0; p < P; ++p) {
                     const size_t e = (size_t(s) * K + k) * P + p;
                     if (I.time_us[e] == INVALID) continue;
-                    if (int64_t(I.mem_mb[e]) + int64_t(q) * int64_t(I.actmem_mb[e]) > int64_t(I.cap_mb[k])) continue;
+                    const int64_t am = I.actmem_mb ? int64_t(I.actmem_mb[e]) : 0;
+                    if (int64_t(I.mem_mb[e]) + int64_t(q) * am > int64_t(I.cap_mb[k])) continue;
                     const size_t o = (size_t(q) * NS + s) * K + k;
                     if (int64_t(I.time_us[e]) < R.c[o]) { R.c[o] = I.time_us[e]; R.argp[o] = p; }   // strict: lowest p
                 }
@@ -77,9 +89,13 @@ Reduced reduce_tables(const Inst& I) {
     return R;
 }
 
-std::vector<int64_t> candidates(const Reduced& R) {
+std::vector<int64_t> candidates(const Reduced& R, bool xbound) {
     std::vector<int64_t> v;
     for (int64_t c : R.c) if (c < INF) v.push_back(c);
+    if (xbound)
+        for (int j = 0; j < R.K; ++j)
+            for (int k = 0; k < R.K; ++k)
+                if (j != k && R.x[size_t(j) * R.K + k] < INF) v.push_back(R.x[size_t(j) * R.K + k]);
     std::sort(v.begin(), v.end());
     v.erase(std::unique(v.begin(), v.end()), v.end());
     return v;
@@ -114,6 +130,7 @@ Top run_dp(const Inst& I, const Reduced& R, int64_t T, DP& D, bool keep) {
                         int64_t best = INF; int bj = 0;
                         for (int j = 0; j < K; ++j) {
                             if (!(Rm >> j & 1)) continue;
+                            if (I.xbound && R.x[size_t(k) * K + j] > T) continue;   // NEXT-3(b): the transfer is a pipeline slot
                             const int64_t v = sat(R.x[size_t(k) * K + j] + D.g[D.at(b, Rm, j)]);
                             if (v < best) { best = v; bj = j; }
                         }
@@ -166,11 +183,11 @@ static void set_infeasible(orc_result* o) { std::memset(o, 0, sizeof(*o)); o->it
 
 // Full ascending sweep with the exact stop rule f_inf + (m-1)T >= incumbent, then a
 // choice-keeping run at T* and the back-track.
-int orc_depth_solve(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
-                    const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
-    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb};
+int orc_variant_solve(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                      const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, int xbound, orc_result* out) {
+    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, xbound};
     Reduced R = reduce_tables(I);
-    std::vector<int64_t> cand = candidates(R);
+    std::vector<int64_t> cand = candidates(R, xbound != 0);
     set_infeasible(out);
     out->n_candidates = int(cand.size());
     DP D0;
@@ -204,6 +221,11 @@ int orc_depth_solve(int L, int K, int P, int m, const int32_t* time_us, const in
     return 0;
 }
 
+int orc_depth_solve(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                    const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
+    return orc_variant_solve(L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, 0, out);
+}
+
 // Literal enumeration: every cut set and every ordered choice of distinct islands; the depth of
 // stage i is known once the plan is complete (q = n - i).
 namespace {
@@ -220,7 +242,12 @@ struct BF {
             const int64_t cv = R->C(n - i, sidx(L, a, bs[i]), ks[i]);
             if (cv >= INF) return;
             sum += cv; T = std::max(T, cv); mask |= 1u << ks[i];
-            if (i + 1 < n) { const int64_t xs = R->x[size_t(ks[i]) * I->K + ks[i + 1]]; if (xs >= INF) return; sum += xs; }
+            if (i + 1 < n) {
+                const int64_t xs = R->x[size_t(ks[i]) * I->K + ks[i + 1]];
+                if (xs >= INF) return;
+                sum += xs;
+                if (I->xbound) T = std::max(T, xs);
+            }
             a = bs[i];
         }
         ++n_plans;
@@ -242,9 +269,9 @@ struct BF {
 };
 }  // namespace
 
-int orc_depth_bruteforce(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
-                         const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
-    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb};
+int orc_variant_bruteforce(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                           const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, int xbound, orc_result* out) {
+    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, xbound};
     Reduced R = reduce_tables(I);
     BF bf; bf.I = &I; bf.R = &R;
     bf.rec(0, 0);
@@ -263,6 +290,11 @@ int orc_depth_bruteforce(int L, int K, int P, int m, const int32_t* time_us, con
         a = b;
     }
     return 0;
+}
+
+int orc_depth_bruteforce(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                         const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
+    return orc_variant_bruteforce(L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, 0, out);
 }
 
 }  // extern "C"

@@ -79,12 +79,13 @@ class Instance:
     act_mb: int
     meta: dict = field(default_factory=dict)
     actmem_mb: np.ndarray = None   # [NS, K, P] int32 or None: MB per in-flight microbatch (NEXT-1, depth-aware memory)
+    transfer_bound: bool = False   # NEXT-3(b): transfers count toward the bottleneck (x <= T as well)
 
     def copy(self) -> "Instance":
         return Instance(self.name, self.L, self.K, self.P, self.m, self.time_us.copy(),
                         self.mem_mb.copy(), self.island_gpus.copy(), self.island_cap_mb.copy(),
                         self.bw_gbps.copy(), self.act_mb, dict(self.meta),
-                        None if self.actmem_mb is None else self.actmem_mb.copy())
+                        None if self.actmem_mb is None else self.actmem_mb.copy(), self.transfer_bound)
 
 
 def _cdiv(a, b):
@@ -271,6 +272,14 @@ def with_actmem(inst: Instance, seed: int, lo: int = 0, hi: int = 60) -> Instanc
     idx = np.arange(NS * K * P).reshape(NS, K, P)
     o.actmem_mb = ((b - a)[:, None, None] * urand(seed, S_MISC + 30, idx, lo, hi)).astype(np.int32)
     o.name = inst.name + "_act"
+    return o
+
+
+def with_transfer_bound(inst: Instance) -> Instance:
+    """Same tables, transfers bounded by the threshold as well (NEXT-3(b))."""
+    o = inst.copy()
+    o.transfer_bound = True
+    o.name = inst.name + "_xb"
     return o
 
 
