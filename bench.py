@@ -52,6 +52,12 @@ def make_workload(name: str, rank: int, n_inst: int):
     if name == "cfg3d":
         return [gen.with_actmem(gen.config3(rank), 7 + rank, 500, 6000)], \
             "cfg3 70B-like L=80 K=12 P=8 m=32 + depth-aware activation memory (NEXT-1), 1 instance/GPU"
+    if name == "cfg4xb":  # cfg4 with the boundary transfers bounded by the threshold
+        return [gen.with_transfer_bound(gen.config4(rank))], \
+            "cfg4 MoE-like L=64 K=16 P=8 m=64 + transfers as pipeline slots (NEXT-3(b)), 1 instance/GPU"
+    if name == "cfg3xb":
+        return [gen.with_transfer_bound(gen.config3(rank))], \
+            "cfg3 70B-like L=80 K=12 P=8 m=32 + transfers as pipeline slots (NEXT-3(b)), 1 instance/GPU"
     if name == "cfg5":
         from paper_2606_16907_b200.shard import weak_seeds
         return [gen.config5_one(sd) for sd in weak_seeds(n_inst, rank)], \
@@ -261,9 +267,11 @@ def run_ours(args):
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         hs = [tg.tg_instance_create(i.L, i.K, i.P, i.m, *pp, i.act_mb) for i, pp in zip(insts, pinned)]
-        for h, pa in zip(hs, pinned_act):
+        for h, pa, i in zip(hs, pinned_act, insts):
             if pa is not None:
                 tg.tg_instance_set_actmem(h, pa)
+            if i.transfer_bound:
+                tg.tg_instance_set_transfer_bound(h, True)
         res = tg.tg_solve_batch(hs, out=None, flags=flags)            # host result buffer: D2H + sync inside
         for h in hs:
             h.destroy()
@@ -323,7 +331,7 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5", "cfg3d", "cfg4d"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5", "cfg3d", "cfg4d", "cfg3xb", "cfg4xb"])
     ap.add_argument("--n-inst", type=int, default=1024, help="instances per GPU of the cfg5 batch")
     ap.add_argument("--full-sweep", action="store_true", help="run the DP at every candidate T")
     ap.add_argument("--cpu-threads", type=int, default=8)

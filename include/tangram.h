@@ -79,6 +79,14 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
  * legacy default stream. */
 tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb);
 
+/* tg_instance_set_transfer_bound — SURVEY.md §8(c) A2 variant / §8(f) NEXT-3(b): the activation transfer between
+ * two stages is its own pipeline slot ("communication can be the bottleneck").  With on != 0 a
+ * transfer is admissible at threshold T iff x[j][k] <= T, so a plan's bottleneck is
+ * T = max(max stage time, max boundary transfer), the candidate thresholds are the distinct finite stage costs
+ * and off-diagonal transfer times, and iter = sum + (m-1) * T as before (the sum still includes the transfers).
+ * on == 0 restores the core definition.  Combines with tg_instance_set_actmem.  No device work. */
+tg_status tg_instance_set_transfer_bound(tg_instance* inst, int32_t on);
+
 /* NULL is a no-op.  The instance must not be in use by an unsynchronised tg_solve_batch. */
 tg_status tg_instance_destroy(tg_instance* inst);
 

@@ -61,7 +61,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_set_actmem", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
+EXPORTS = ["tg_instance_create", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
            "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -166,6 +166,11 @@ def tg_instance_set_actmem(inst: Instance, actmem_mb):
     _check(lib().tg_instance_set_actmem(inst.handle, _ptr(a)))
 
 
+def tg_instance_set_transfer_bound(inst: Instance, on: bool):
+    """NEXT-3(b): transfers count toward the bottleneck (x <= T as well)."""
+    _check(lib().tg_instance_set_transfer_bound(inst.handle, C.c_int32(1 if on else 0)))
+
+
 def tg_instance_destroy(inst: Instance):
     inst.destroy()
 
@@ -250,4 +255,6 @@ def instance_from_inputs(inst, device_tables: bool = False) -> Instance:
                            inst.island_cap_mb, inst.bw_gbps, inst.act_mb)
     if getattr(inst, "actmem_mb", None) is not None:
         tg_instance_set_actmem(h, inst.actmem_mb)
+    if getattr(inst, "transfer_bound", False):
+        tg_instance_set_transfer_bound(h, True)
     return h

@@ -16,6 +16,7 @@ struct tg_instance {
     int device;
     int32_t *time_us, *mem_mb, *gpus, *cap_mb, *bw;  // device
     int32_t* actmem;                                 // device, or nullptr (tg_instance_set_actmem)
+    int32_t xbound;                                  // tg_instance_set_transfer_bound
 };
 
 namespace {
@@ -161,6 +162,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         I.time_us = t.time_us; I.mem_mb = t.mem_mb; I.cap_mb = t.cap_mb; I.bw_gbps = t.bw;
         I.actmem_mb = t.actmem;
         I.nDepth = t.actmem ? t.K : 1;
+        I.xbound = t.xbound;
         I.L = t.L; I.K = t.K; I.P = t.P; I.m = t.m; I.act_mb = t.act_mb; I.NS = t.NS;
         I.Lp = (t.L + 3) & ~3;
         I.triG = int(tgGOff(t.L, t.L + 1));
@@ -189,9 +191,10 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         const size_t nd = size_t(I.nDepth);
         oCd[i] = cv.take(nd * size_t(t.K) * I.triG * 4);
         oArgp[i] = cv.take(nd * size_t(cells));
-        oCand[i] = cv.take(nd * size_t(cells) * 4);
-        oSort[i] = cv.take(nd * size_t(cells) * 4);
-        oSort2[i] = cv.take(nd * size_t(cells) * 4);
+        const size_t nKeys = nd * size_t(cells) + size_t(t.K) * t.K;   // every reduced cost + (transfer bound) every transfer time
+        oCand[i] = cv.take(nKeys * 4);
+        oSort[i] = cv.take(nKeys * 4);
+        oSort2[i] = cv.take(nKeys * 4);
         oSuf[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
         oSufA[i] = cv.take(size_t(t.K) * (t.L + 2) * 4);
         oEI[i] = cv.take(size_t(TG_MAX_EVAL) * 4);
@@ -355,6 +358,7 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
     if (!t) { cudaFreeAsync(base, 0); return fail(TG_ERR_OOM, "host allocation failed"); }
     t->L = L; t->K = K; t->P = P; t->m = m; t->act_mb = act_mb; t->NS = NS; t->device = dev;
     t->actmem = nullptr;
+    t->xbound = 0;
     t->time_us = reinterpret_cast<int32_t*>(base + oT); t->mem_mb = reinterpret_cast<int32_t*>(base + oM);
     t->gpus = reinterpret_cast<int32_t*>(base + oG); t->cap_mb = reinterpret_cast<int32_t*>(base + oC);
     t->bw = reinterpret_cast<int32_t*>(base + oB);
@@ -411,6 +415,12 @@ tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb) {
         return fail(TG_ERR_RANGE, "actmem_mb must be in [0, 2^20]");
     }
     inst->actmem = d;
+    return TG_OK;
+}
+
+tg_status tg_instance_set_transfer_bound(tg_instance* inst, int32_t on) {
+    if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
+    inst->xbound = on ? 1 : 0;
     return TG_OK;
 }
 

@@ -57,6 +57,7 @@ struct TgInstDev {
     int32_t sortCap, ncand;
     uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
     uint32_t maxKey;                  // largest finite reduced cost of any depth (bounds the radix sort's passes)
+    int32_t xbound;                   // NEXT-3(b): transfers are admissible only if x <= T (tg_instance_set_transfer_bound)
     uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major
     // ---- solver state (one scheduler thread per instance) ----
     int32_t phase, loInf, hiFeas, next;   // FEAS bracket: largest infeasible / smallest feasible candidate

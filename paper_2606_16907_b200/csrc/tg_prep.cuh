@@ -249,8 +249,11 @@ __device__ uint32_t* tgRadixSort(uint32_t* A, uint32_t* B, int n, uint32_t maxKe
 __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restrict__ insts) {
     extern __shared__ uint32_t sbuf[];
     __shared__ uint32_t warpSums[33];
+    __shared__ uint32_t sMaxX;
     TgInstDev& I = insts[blockIdx.x];
     const int L = I.L, K = I.K, tid = threadIdx.x;
+    if (tid == 0) sMaxX = 0;
+    __syncthreads();
     // transfer table
     if (tid < K * K) {
         const int j = tid / K, k = tid % K;
@@ -261,6 +264,12 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
             v = q > TG_TIME_MAX ? TG_INFU : uint32_t(q);
         }
         I.x[j * TG_MAX_K + k] = v;
+        // transfer bound (NEXT-3(b)): the finite transfer times are candidate thresholds too
+        if (I.xbound) {
+            const bool fin = j != k && v < TG_INFU;
+            I.sortbuf[size_t(I.NS) * K * I.nDepth + tid] = fin ? v : TG_INFU;
+            if (fin) atomicMax(&sMaxX, v);
+        }
     }
     // row minima (b <= L-1 only) then suffix minima over the diagonal index
     uint32_t* sm = I.sufMin;
@@ -288,8 +297,8 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     __syncthreads();
     // candidate sort: stable LSD radix sort, 8- or 9-bit digits, ping-pong between the two global buffers
     // (L2 resident); per-warp digit histograms in shared memory, warp w owns a contiguous chunk
-    const int n = I.NS * K * I.nDepth;
-    uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, I.maxKey, sbuf, warpSums);
+    const int n = I.NS * K * I.nDepth + (I.xbound ? K * K : 0);
+    uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, max(I.maxKey, sMaxX), sbuf, warpSums);
     // unique, finite only
     uint32_t base = 0;
     for (int i0 = 0; i0 < n; i0 += 4 * TG_PREP_NT) {   // four consecutive keys a thread: one block scan per 4096 keys

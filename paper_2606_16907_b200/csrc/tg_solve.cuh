@@ -211,7 +211,8 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     }
     if (tid < Ke * Ke) {
         const int kc = tid / Ke, jc = tid - kc * Ke;
-        sm.xS[kc][jc] = I.x[int(sm.isl[kc]) * TG_MAX_K + int(sm.isl[jc])];
+        const uint32_t xv = I.x[int(sm.isl[kc]) * TG_MAX_K + int(sm.isl[jc])];
+        sm.xS[kc][jc] = (I.xbound && xv > T) ? TG_INFU : xv;   // transfer bound (NEXT-3(b)): a slower link is not admissible at T
     }
     if (tid < Ke) {  // widest diagonal with an admissible entry: sufMin is non-decreasing in d
         const uint32_t* sf = I.sufMin + size_t(sm.isl[tid]) * (L + 2);
@@ -654,7 +655,9 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
                 const int j = int(__fns(R, 0, ji + 1));
                 const uint32_t Rp = R ^ (1u << j);
                 const size_t row = size_t(ctx.rankOf[Rp]) * (Ke - r + 1) + (j - __popc(R & ((1u << j) - 1u)));
-                const uint32_t v = c + I.x[ko * TG_MAX_K + isl[j]] + __ldcg(Gl + row * Wd + (bb - lo4R));
+                const uint32_t xv = I.x[ko * TG_MAX_K + isl[j]];
+                if (I.xbound && xv > T) continue;
+                const uint32_t v = c + xv + __ldcg(Gl + row * Wd + (bb - lo4R));
                 if (v >= TG_INFU) continue;
                 // lowest value, then lowest b, then lowest j
                 const unsigned long long kk = (unsigned long long)v << 32 | (unsigned long long)bb << 8 | (unsigned long long)j;

@@ -56,6 +56,12 @@ def main():
             data = [{"name": inst.name, "L": inst.L, "K": inst.K, "P": inst.P, "m": inst.m,
                      "solve": rec(oracle.solve_depth(inst)), "core": rec(oracle.solve(inst, n_threads=threads)),
                      "oracle_seconds": round(time.time() - t0, 1)}]
+        elif name == "cfg3xb":     # NEXT-3(b): the 70B-like config with transfers bounded by the threshold (variant oracle)
+            inst = gen.with_transfer_bound(gen.config3())
+            t0 = time.time()
+            data = [{"name": inst.name, "L": inst.L, "K": inst.K, "P": inst.P, "m": inst.m,
+                     "solve": rec(oracle.solve_variant(inst)), "core": rec(oracle.solve(inst, n_threads=threads)),
+                     "oracle_seconds": round(time.time() - t0, 1)}]
         elif name == "cfg5":
             data = [dict(one(gen.config5_one(s), threads, False), seed=s) for s in CFG5_SEEDS]
         else:
