@@ -266,7 +266,7 @@ def run_ours(args):
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        hs = [tg.tg_instance_create(i.L, i.K, i.P, i.m, *pp, i.act_mb) for i, pp in zip(insts, pinned)]
+        hs = tg.tg_instance_create_batch([(i.L, i.K, i.P, i.m, *pp, i.act_mb) for i, pp in zip(insts, pinned)])
         for h, pa, i in zip(hs, pinned_act, insts):
             if pa is not None:
                 tg.tg_instance_set_actmem(h, pa)

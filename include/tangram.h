@@ -68,6 +68,17 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
                              const int32_t* island_cap_mb, const int32_t* bw_gbps, int32_t act_mb,
                              tg_instance** out);
 
+/* tg_instance_create_batch — n instances in one call: element i of every array argument describes instance i
+ * exactly as the arguments of tg_instance_create do (L, K, P, m, act_mb: HOST arrays of n int32; time_us ...
+ * bw_gbps: HOST arrays of n pointers, each EITHER host or device).  All uploads and validations are enqueued
+ * first and the call synchronises ONCE (tg_instance_create synchronises once per instance: 1024 instances cost
+ * 1024 round trips).  All or nothing: on any error nothing is created, out[0..n) is NULL and the message names
+ * the first offending instance.  n == 0 is a no-op. */
+tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K, const int32_t* P, const int32_t* m,
+                                   const int32_t* const* time_us, const int32_t* const* mem_mb,
+                                   const int32_t* const* island_gpus, const int32_t* const* island_cap_mb,
+                                   const int32_t* const* bw_gbps, const int32_t* act_mb, tg_instance** out);
+
 /* tg_instance_set_actmem — SURVEY.md §8(f) NEXT-1, depth-aware activation memory under 1F1B (PAPER.md:246
  * "earlier stages hold more in-flight activations", :258(i)).  actmem_mb: EITHER [NS][K][P] int32 in
  * [0, 2^20], MB that plan p of (slice, island) needs PER in-flight microbatch, copied; NULL removes the table.

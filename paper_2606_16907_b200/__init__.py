@@ -61,7 +61,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
+EXPORTS = ["tg_instance_create", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
            "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -158,6 +158,25 @@ def tg_instance_create(L, K, P, m, time_us, mem_mb, island_gpus, island_cap_mb, 
     h = C.c_void_p(0)
     _check(lib().tg_instance_create(L, K, P, m, *[_ptr(a) for a in arrs], act_mb, C.byref(h)))
     return Instance(h.value, L, K, P, m)
+
+
+def tg_instance_create_batch(specs) -> list:
+    """specs: sequence of (L, K, P, m, time_us, mem_mb, island_gpus, island_cap_mb, bw_gbps, act_mb), tables as in
+    tg_instance_create.  One synchronisation for the whole batch; all or nothing."""
+    n = len(specs)
+    if n == 0:
+        return []
+    def prep(a):
+        return np.ascontiguousarray(a, dtype=np.int32) if isinstance(a, np.ndarray) else a
+    keep = [[prep(a) for a in s[4:9]] for s in specs]           # keeps converted copies alive during the call
+    I32 = C.c_int32 * n
+    PP = C.c_void_p * n
+    scal = [I32(*[int(s[j]) for s in specs]) for j in (0, 1, 2, 3)]
+    acts = I32(*[int(s[9]) for s in specs])
+    ptrs = [PP(*[_ptr(k[j]) for k in keep]) for j in range(5)]
+    out = PP()
+    _check(lib().tg_instance_create_batch(C.c_int32(n), *scal, *ptrs, acts, out))
+    return [Instance(out[i], int(s[0]), int(s[1]), int(s[2]), int(s[3])) for i, s in enumerate(specs)]
 
 
 def tg_instance_set_actmem(inst: Instance, actmem_mb):

@@ -335,9 +335,15 @@ extern "C" {
 const char* tg_last_error(void) { return g_err.c_str(); }
 int32_t tg_version(void) { return 100; }
 
-tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const int32_t* time_us,
-                             const int32_t* mem_mb, const int32_t* island_gpus, const int32_t* island_cap_mb,
-                             const int32_t* bw_gbps, int32_t act_mb, tg_instance** out) {
+}  // extern "C"
+
+namespace {
+
+// Allocation, uploads and the validation kernel of one instance, all enqueued on the legacy default stream; the
+// error word (device) is read by the caller after it has synchronised.
+tg_status createAsync(int32_t L, int32_t K, int32_t P, int32_t m, const int32_t* time_us,
+                      const int32_t* mem_mb, const int32_t* island_gpus, const int32_t* island_cap_mb,
+                      const int32_t* bw_gbps, int32_t act_mb, tg_instance** out, int** dErrOut) {
     if (!time_us || !mem_mb || !island_gpus || !island_cap_mb || !bw_gbps || !out) return fail(TG_ERR_NULL, "NULL argument");
     if (L < 1 || L > TG_MAX_L || K < 1 || K > TG_MAX_K || P < 1 || P > TG_MAX_P || m < 1 || m > TG_MAX_M)
         return fail(TG_ERR_SHAPE, "L, K, P or m outside limits");
@@ -369,19 +375,80 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
     if (e == cudaSuccess) e = cudaMemcpyAsync(t->cap_mb, island_cap_mb, K * 4, cudaMemcpyDefault, 0);
     if (e == cudaSuccess) e = cudaMemcpyAsync(t->bw, bw_gbps, K * K * 4, cudaMemcpyDefault, 0);
     if (e == cudaSuccess) e = cudaMemsetAsync(dErr, 0, 4, 0);
-    int herr = 0;
     if (e == cudaSuccess) {
         const int blocks = int(std::min<size_t>((nE + 255) / 256, 4096));
         tgValidateKernel<<<std::max(blocks, 1), 256>>>(t->time_us, t->mem_mb, t->gpus, t->cap_mb, t->bw, K, nE, dErr);
-        e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);   // the one synchronisation of the call
+        e = cudaGetLastError();
     }
-    if (e != cudaSuccess || herr) {
+    if (e != cudaSuccess) {
         cudaFreeAsync(base, 0);
         delete t;
-        if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("instance upload: ") + cudaGetErrorString(e));
-        return fail(TG_ERR_RANGE, "table value out of range (bits: 1 time, 2 mem, 4 bw, 8 gpus, 16 cap): " + std::to_string(herr));
+        return fail(TG_ERR_CUDA, std::string("instance upload: ") + cudaGetErrorString(e));
     }
     *out = t;
+    *dErrOut = dErr;
+    return TG_OK;
+}
+
+tg_status rangeError(int herr, int index) {
+    return fail(TG_ERR_RANGE, (index >= 0 ? "instance " + std::to_string(index) + ": " : std::string()) +
+                                  "table value out of range (bits: 1 time, 2 mem, 4 bw, 8 gpus, 16 cap): " + std::to_string(herr));
+}
+
+}  // namespace
+
+extern "C" {
+
+tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const int32_t* time_us,
+                             const int32_t* mem_mb, const int32_t* island_gpus, const int32_t* island_cap_mb,
+                             const int32_t* bw_gbps, int32_t act_mb, tg_instance** out) {
+    if (!out) return fail(TG_ERR_NULL, "NULL argument");
+    tg_instance* t = nullptr;
+    int* dErr = nullptr;
+    tg_status s = createAsync(L, K, P, m, time_us, mem_mb, island_gpus, island_cap_mb, bw_gbps, act_mb, &t, &dErr);
+    if (s != TG_OK) return s;
+    int herr = 0;
+    const cudaError_t e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);   // the one synchronisation of the call
+    if (e != cudaSuccess || herr) {
+        tg_instance_destroy(t);
+        if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("instance upload: ") + cudaGetErrorString(e));
+        return rangeError(herr, -1);
+    }
+    *out = t;
+    return TG_OK;
+}
+
+tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K, const int32_t* P, const int32_t* m,
+                                   const int32_t* const* time_us, const int32_t* const* mem_mb,
+                                   const int32_t* const* island_gpus, const int32_t* const* island_cap_mb,
+                                   const int32_t* const* bw_gbps, const int32_t* act_mb, tg_instance** out) {
+    if (n < 0) return fail(TG_ERR_SHAPE, "n < 0");
+    if (n == 0) return TG_OK;
+    if (!L || !K || !P || !m || !time_us || !mem_mb || !island_gpus || !island_cap_mb || !bw_gbps || !act_mb || !out)
+        return fail(TG_ERR_NULL, "NULL argument");
+    std::vector<int*> dErr(size_t(n), nullptr);
+    tg_status s = TG_OK;
+    int made = 0;
+    for (; made < n; ++made) {
+        out[made] = nullptr;
+        s = createAsync(L[made], K[made], P[made], m[made], time_us[made], mem_mb[made], island_gpus[made],
+                        island_cap_mb[made], bw_gbps[made], act_mb[made], &out[made], &dErr[size_t(made)]);
+        if (s != TG_OK) { g_err = "instance " + std::to_string(made) + ": " + g_err; break; }
+    }
+    std::string err = g_err;
+    if (s == TG_OK) {   // every upload and validation is in flight: one synchronisation for the whole batch
+        std::vector<int> herr(size_t(n), 0);
+        cudaError_t e = cudaSuccess;
+        for (int i = 0; i < n && e == cudaSuccess; ++i) e = cudaMemcpyAsync(&herr[size_t(i)], dErr[size_t(i)], 4, cudaMemcpyDeviceToHost, 0);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+        if (e != cudaSuccess) { s = TG_ERR_CUDA; err = std::string("instance upload: ") + cudaGetErrorString(e); }
+        for (int i = 0; i < n && s == TG_OK; ++i)
+            if (herr[size_t(i)]) { s = rangeError(herr[size_t(i)], i); err = g_err; }
+    }
+    if (s != TG_OK) {   // all or nothing
+        for (int i = 0; i < made; ++i) { tg_instance_destroy(out[i]); out[i] = nullptr; }
+        return fail(s, err);
+    }
     return TG_OK;
 }
 

@@ -161,3 +161,29 @@ def test_more_instances_than_items_per_round(tg):
     res = solve_all(tg, insts)
     for inst, g in zip(insts, res):
         same(oracle.solve(inst), g, inst.name)
+
+
+def test_create_batch(tg):
+    """tg_instance_create_batch == one tg_instance_create per instance; a bad table anywhere creates nothing."""
+    insts = [gen.random_small(s + 95_000, Lmax=8, Kmax=5, Pmax=3, style=STYLES[s % 5]) for s in range(64)] + \
+            [gen.config2(), gen.config3(0, L=20, K=6)]
+    spec = lambda i: (i.L, i.K, i.P, i.m, i.time_us, i.mem_mb, i.island_gpus, i.island_cap_mb, i.bw_gbps, i.act_mb)
+    hs = tg.tg_instance_create_batch([spec(i) for i in insts])
+    assert len(hs) == len(insts) and all(h.handle for h in hs)
+    res = tg.tg_solve_batch(hs)
+    for inst, g in zip(insts, res):
+        same(oracle.solve(inst), g, inst.name)
+    for h in hs:
+        h.destroy()
+    assert tg.tg_instance_create_batch([]) == []
+    bad = insts[5].copy()
+    bad.time_us = bad.time_us.copy()
+    bad.time_us[0, 0, 0] = -7
+    with pytest.raises(tg.TangramError) as e:
+        tg.tg_instance_create_batch([spec(i) for i in insts[:5]] + [spec(bad)] + [spec(i) for i in insts[6:9]])
+    assert e.value.status == 3 and "instance 5" in str(e.value)
+    shape = list(spec(insts[0]))
+    shape[1] = 17                                  # K above TG_MAX_K
+    with pytest.raises(tg.TangramError) as e:
+        tg.tg_instance_create_batch([spec(insts[1]), tuple(shape)])
+    assert e.value.status == 2 and "instance 1" in str(e.value)
