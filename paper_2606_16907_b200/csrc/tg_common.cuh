@@ -57,6 +57,7 @@ struct TgInstDev {
     int32_t sortCap, ncand;
     uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
     uint32_t maxKey;                  // largest finite reduced cost of any depth (bounds the radix sort's passes)
+    int32_t planKind;                 // wide scheduling: item kind returned by this round's planning
     int32_t xbound;                   // NEXT-3(b): transfers are admissible only if x <= T (tg_instance_set_transfer_bound)
     uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major
     // ---- solver state (one scheduler thread per instance) ----
@@ -92,6 +93,7 @@ struct TgCtrl {
     int32_t round;
     uint32_t barrier;     // monotone arrival counter of the grid barrier
     int32_t errFlag;
+    int32_t nActive;      // instances not done after the previous round's planning (wide scheduling: bounds W)
     int32_t weighted[2];  // per round parity: team sizes follow the items' estimated cost (teamOf / ctaBeg / ctaCnt)
     uint8_t teamOf[2][256];   // weighted team mode: item of each CTA
     tg_solve_stats stats;

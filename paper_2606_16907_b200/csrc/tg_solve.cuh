@@ -979,24 +979,22 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
     return TG_PH_DONE;
 }
 
-__device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, int round) {
-    const int tid = threadIdx.x;
-    const int par = round & 1, prv = par ^ 1;
+// Fold the previous round into every instance's search state and plan its next probes (I.probe, I.nProbe,
+// I.planKind).  Narrow (few instances): CTA 0, one thread per instance, the previous items staged in shared
+// memory.  Wide (many instances): the fold and the planning are single-thread, branchy code -- packed 32 to a warp
+// on CTA 0 they serialise (cfg5: 0.35 ms a round with the whole grid waiting) -- so every warp of the grid takes
+// at most one instance at a time (lane 0), followed by one grid barrier before CTA 0 lays the items out.
+#define TG_WIDE_MIN_INST 64
+__device__ void tgFoldPlanAll(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, int round, bool wide) {
+    const int tid = threadIdx.x, prv = (round & 1) ^ 1;
     TgCtrl* ctrl = ctx.ctrl;
-    TgItem* items = ctx.items + size_t(par) * TG_MAX_ITEMS;
     const TgItem* itemsPrev = ctx.items + size_t(prv) * TG_MAX_ITEMS;
-    unsigned long long* keys = ctx.keys + size_t(par) * TG_MAX_ITEMS;
     const unsigned long long* keysPrev = ctx.keys + size_t(prv) * TG_MAX_ITEMS;
     const bool full = (ctx.flags & TG_SOLVE_FULL_SWEEP) != 0;
-    const int nInst = ctx.nInst;
-
-    if (tid == 0) { sm.iTmp[0] = 0; sm.iTmp[1] = 0; sm.llTmp[0] = 0; sm.llTmp[1] = 0; }
-    if (tid == 0 && round < 8) ctrl->schedCyc[round][0] = clock64();
-    __syncthreads();
-
-    // ---- A: fold the previous round ---------------------------------------------------------
+    if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->schedCyc[round][0] = clock64();
     TgPrev P;
-    {   // stage keys, candidate indices, their thresholds and flags of the previous items in the (idle) dynamic shared memory
+    P.items = itemsPrev; P.keys = keysPrev; P.keyS = nullptr; P.tidxS = nullptr; P.candS = nullptr; P.flagS = nullptr; P.nStage = 0;
+    if (!wide) {   // stage keys, candidate indices, their thresholds and flags of the previous items in the (idle) dynamic shared memory
         const int nPrev = round > 0 ? ctrl->nItems[prv] : 0;
         const int room = int((size_t(ctx.csWords) + size_t(ctx.nActiveWarps) * ctx.wbufWords) * 4 / 20);   // 17 bytes an item, padded
         const int nStage = min(nPrev, room) & ~1;   // even: keeps the arrays behind the keys 8-byte aligned
@@ -1011,33 +1009,55 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, i
             flagS[q] = __ldcg(&itemsPrev[q].flags);
             candS[q] = tx >= 0 ? ctx.inst[__ldcg(&itemsPrev[q].inst)].cand[tx] : 0u;
         }
-        P.items = itemsPrev; P.keys = keysPrev; P.keyS = keyS; P.tidxS = tidxS; P.candS = candS; P.flagS = flagS; P.nStage = nStage;
+        P.keyS = keyS; P.tidxS = tidxS; P.candS = candS; P.flagS = flagS; P.nStage = nStage;
         __syncthreads();
     }
+    // W is bounded by the item list shared among the instances still running (count of the previous round: an upper bound)
+    const int nActive = round > 0 ? max(1, __ldcg(&ctrl->nActive)) : ctx.nInst;
+    const int capAll = max(1, min(ctx.wishMax, TG_MAX_ITEMS / nActive));
+    const bool mine = wide ? (tid & 31) == 0 : true;
+    const int first = wide ? int(blockIdx.x) * TG_NW + (tid >> 5) : tid;
+    const int stride = wide ? int(gridDim.x) * TG_NW : TG_NT;
+    if (mine)
+        for (int i = first; i < ctx.nInst; i += stride) {
+            TgInstDev& I = ctx.inst[i];
+            if (I.itemCnt > 0) tgFoldInstance(ctx, I, P, full);
+            if (I.phase != TG_PH_DONE) I.planKind = tgPlanInstance(ctx, I, i, full ? capAll : min(capAll, tgWish(ctx, I.K)), full);   // a full sweep has no speculation
+        }
+    __syncthreads();
+    if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->schedCyc[round][1] = clock64();
+}
+
+// Scheduler, second half (CTA 0): lay the planned probes out as the round's item list, size the teams.
+__device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
+    const int tid = threadIdx.x;
+    const int par = round & 1;
+    TgCtrl* ctrl = ctx.ctrl;
+    TgItem* items = ctx.items + size_t(par) * TG_MAX_ITEMS;
+    unsigned long long* keys = ctx.keys + size_t(par) * TG_MAX_ITEMS;
+    const int nInst = ctx.nInst;
+
+    if (tid == 0) { sm.iTmp[0] = 0; sm.iTmp[1] = 0; sm.llTmp[0] = 0; sm.llTmp[1] = 0; }
+    __syncthreads();
     int nActive = 0;
-    for (int i = tid; i < nInst; i += TG_NT) {
-        TgInstDev& I = ctx.inst[i];
-        if (I.itemCnt > 0) tgFoldInstance(ctx, I, P, full);
-        if (I.phase != TG_PH_DONE) ++nActive;
-    }
+    for (int i = tid; i < nInst; i += TG_NT) nActive += ctx.inst[i].phase != TG_PH_DONE ? 1 : 0;
     if (nActive) atomicAdd(&sm.iTmp[0], nActive);
     __syncthreads();
     nActive = sm.iTmp[0];
-    if (tid == 0 && round < 8) ctrl->schedCyc[round][1] = clock64();
     if (nActive == 0) {
         if (tid == 0) { ctrl->done = 1; ctrl->nItems[par] = 0; }
         return;
     }
+    if (tid == 0) ctrl->nActive = nActive;
 
     // ---- B: plan every instance's probes, lay the items out ------------------------------------------
-    const int capAll = max(1, min(ctx.wishMax, TG_MAX_ITEMS / nActive));
     uint32_t carry = 0;
     for (int base = 0; base < nInst; base += TG_NT) {
         const int i = base + tid;
         int cnt = 0, kind = TG_PH_DONE;
         if (i < nInst && ctx.inst[i].phase != TG_PH_DONE) {
             TgInstDev& I = ctx.inst[i];
-            kind = tgPlanInstance(ctx, I, i, full ? capAll : min(capAll, tgWish(ctx, I.K)), full);   // a full sweep has no speculation
+            kind = I.planKind;
             cnt = I.nProbe;
         }
         uint32_t tot;
@@ -1175,9 +1195,12 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
     for (int w = threadIdx.x; w < 17 * 17; w += TG_NT) sm.binom[w / 17][w % 17] = tgBinom[w / 17][w % 17];
     if (threadIdx.x < TG_MAX_K) sm.xInf[threadIdx.x] = TG_INFU;
     __syncthreads();
+    const bool wide = ctx.nInst >= TG_WIDE_MIN_INST;
     for (int round = 0;; ++round) {
         const int par = round & 1;
-        if (b == 0) { tgSchedule(ctx, sm, dyn, round); tgMark(sm, 6); }
+        if (wide || b == 0) { tgFoldPlanAll(ctx, sm, dyn, round, wide); tgMark(sm, 6); }
+        if (wide) { tgGridBarrier(ctrl, epoch); tgMark(sm, 5); }
+        if (b == 0) { tgSchedule(ctx, sm, round); tgMark(sm, 6); }
         tgGridBarrier(ctrl, epoch);
         tgMark(sm, 5);
         if (__ldcg(&ctrl->done)) break;
