@@ -26,6 +26,8 @@ struct TgShared {
     uint32_t sT;
     // row windows (see "Row windows" below): rows hold Wd starts, row of state (S, k) begins at start lo4(cap(S))
     int sWd, sSlack, sWindowed;
+    // split of the dynamic shared memory for this item: [cost rows | nWarps x wbufWords]
+    int nWarps, wbufWords, wbufOff;
     uint32_t cdOff;                 // word offset of the reduced table of the depth currently staged
     uint8_t maxlenK[TG_MAX_K];      // longest admissible slice of island k at T, any position
     uint32_t baseK[TG_MAX_K];
@@ -172,6 +174,10 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
     return nAdm;
 }
 
+// words between consecutive rows of a warp's buffer: 4 (mod 8), so consecutive rows start in different 16-byte
+// bank groups (rows are read by several island groups at the same chunk offset)
+__device__ __forceinline__ int tgRowStride(int Wd) { return Wd + 12 + (((Wd + 12) & 7) == 0 ? 4 : 0); }
+
 // ---------------------------------------------------------------------------------------------
 // Staging of one item's thresholded cost tables into shared memory.
 //   Cs_k[(d-1)*Lp + a] = c[a][a+d][k] if <= T and a+d <= L-1, else INF   (k in compact labels)
@@ -244,7 +250,17 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         // + 4 words per island: tables of different islands start in different 16-byte bank groups, so the
         // island groups of a warp do not collide when they read the same diagonal
         for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += uint32_t((sm.dmaxK[kc] + 3) & ~3) * uint32_t(Lp) + 4u; }
-        sm.useGlobalC = acc > uint32_t(ctx.csWords) ? 1 : 0;
+        // dynamic shared memory of this item: every warp gets room for one mask's rows at the widest level
+        // (2 Ke - 1 rows), the cost rows come next if they still fit, and what is left doubles the warps'
+        // buffers so that two masks run side by side (tgWarpLevel<16>)
+        const int total = ctx.csWords + ctx.nActiveWarps * ctx.wbufWords;
+        const int perMask = max(1, 2 * Ke - 1) * tgRowStride(sm.sWd);
+        const int nWp = max(1, min(TG_NW, total / perMask));
+        sm.useGlobalC = acc > uint32_t(total - nWp * perMask) ? 1 : 0;
+        const int csUsed = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
+        sm.nWarps = nWp;
+        sm.wbufOff = csUsed;
+        sm.wbufWords = min(2 * perMask, (total - csUsed) / nWp) & ~3;
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
     }
     __syncthreads();
@@ -503,10 +519,6 @@ __device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& 
     }
 }
 
-// words between consecutive rows of a warp's buffer: 4 (mod 8), so consecutive rows start in different 16-byte
-// bank groups (rows are read by several island groups at the same chunk offset)
-__device__ __forceinline__ int tgRowStride(int Wd) { return Wd + 12 + (((Wd + 12) & 7) == 0 ? 4 : 0); }
-
 // One wavefront level for this warp's share of the masks.  SW = 32: one mask at a time on the whole warp.
 // SW = 16: two masks side by side, one per half warp (narrow row windows leave most of a full warp idle and
 // the per-mask bookkeeping -- successor, ranks, copies, windows -- then costs more than the relaxations;
@@ -705,7 +717,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     tgMark(sm, 0);
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int Ke = sm.sSlack >= 0 ? sm.sKe : 0;   // the islands' longest slices cannot cover L layers: infeasible at T
-    const int Wd = sm.sWd, nW = ctx.nActiveWarps, warp = threadIdx.x >> 5;
+    const int Wd = sm.sWd, nW = sm.nWarps, warp = threadIdx.x >> 5;
     uint64_t bufWords = 0;   // words of one ping-pong half; 0 = keep every level (a back-track follows)
     if (Ke > 0 && !(__ldcg(&itp->flags) & 1)) {
         uint32_t mx = 1;
@@ -714,7 +726,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     }
     uint32_t* slot = ctx.scratch + uint64_t(slotIdx) * ctx.slotWords;
     uint32_t* bar = ctx.slotBar + slotIdx;
-    uint32_t* wbuf = wbufAll + size_t(warp) * ctx.wbufWords;
+    uint32_t* wbuf = wbufAll + sm.wbufOff + size_t(warp) * sm.wbufWords;   // (wbufAll = start of the dynamic shared memory)
     uint32_t arrivals = 0;
     if (Ke > 0) {
         tgLevel0(ctx, sm, slot, key, member == 0);
@@ -725,7 +737,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
             if (I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
             if (warp < nW) {
                 // two masks per warp when the windows are narrow and both masks' rows fit the warp's buffer
-                const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= ctx.wbufWords;
+                const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= sm.wbufWords;
                 if (pair) tgWarpLevel<16>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
                 else tgWarpLevel<32>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
             }
@@ -1184,7 +1196,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
     __shared__ TgShared sm;
     uint32_t* dyn = reinterpret_cast<uint32_t*>(tgDynSmem);
     uint32_t* Cs = dyn;
-    uint32_t* wbufAll = dyn + ctx.csWords;
+    uint32_t* wbufAll = dyn;   // the split between cost rows and warp buffers is per item (tgStageItem)
     uint32_t epoch = 0;
     TgCtrl* ctrl = ctx.ctrl;
     const int nCta = int(gridDim.x), b = int(blockIdx.x);
