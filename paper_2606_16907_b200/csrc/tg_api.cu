@@ -173,7 +173,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         for (int k = 0; k < TG_MAX_K; ++k) I.cminAll[k] = TG_INFU;
         I.maxKey = 0;
         I.phase = TG_PH_NEW;
-        I.incIdx = -1; I.hiFeas = -1; I.loInf = -1; I.specIdx = -1;
+        I.incIdx = -1; I.hiFeas = -1; I.loInf = -1; I.specIdx = -1; I.specItem = -1;
         uint64_t mx = 1;
         {   // widest wavefront and full table in rows
             uint64_t binom[17][17];
@@ -204,6 +204,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const size_t oKeys = cv.take(sizeof(unsigned long long) * 2 * TG_MAX_ITEMS);
     const size_t oCtrl = cv.take(sizeof(TgCtrl));
     const size_t oOut = cv.take(sizeof(tg_result) * n);
+    const size_t oSpec = cv.take(sizeof(tg_result) * TG_MAX_ITEMS);
     // DP scratch: nSlots slots, each able to hold every level of the largest instance.  A slot
     // belongs to one team (team mode) or one CTA (solo mode) for the duration of a DP.
     const int numCtas = D->numSMs * D->ctasPerSM;
@@ -257,6 +258,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.gallopMax = g_gallopMax;
     c.ctrl = reinterpret_cast<TgCtrl*>(W.base + oCtrl);
     c.rankOf = D->rankOf;
+    c.specOut = reinterpret_cast<tg_result*>(W.base + oSpec);
 
     const dim3 g((maxCells + 255) / 256, n);
     tgLoadKernel<<<g, 256, 0, st>>>(W.inst);

@@ -12,7 +12,14 @@
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
 #define TG_MAX_EVAL 1024      // evaluated thresholds remembered per instance
 #define TG_MAX_WISH 64        // DPs per instance and round, upper bound
-#define TG_PROBE_FINAL 0x40000000   // flag in probe[]: final DP (keep every level, back-track)
+#define TG_PROBE_FINAL 0x40000000   // flag in probe[]: speculative final DP at the incumbent (S* only; keep every level, back-track)
+#define TG_PROBE_KEEP 0x20000000    // flag in probe[]: search probe that also keeps every level and back-tracks (last round of a search)
+// item flags: 1 = keep every level and back-track; 2 = the result goes to specOut[item], not out[instance];
+//             4 = all islands (a search probe), not only those of the incumbent's mask
+#define TG_IT_TRACK 1
+#define TG_IT_SPEC 2
+#define TG_IT_ALLISL 4
+#define TG_SPEC_ALL_MAX_INST 4   // up to this many instances every probe of a search's last round back-tracks
 #define TG_EDONE 0x40000000   // flag in eIdx: every candidate between the previous evaluated point and this one is resolved
 #define TG_KEY_NONE 0xffffffffffffffffull
 
@@ -69,6 +76,7 @@ struct TgInstDev {
     uint32_t incMask;                     // island mask (original labels) of the incumbent's best state
     int32_t nEval, nProbe;
     int32_t specIdx;                      // candidate of a speculative final DP already run (-1 = none)
+    int32_t specItem;                     // item of the previous round whose back-tracked result is the incumbent's (-1 = none)
     int32_t probe[TG_MAX_WISH];           // candidates to evaluate this round, ascending
     uint64_t fullWords;  // scratch words of a full-table DP of this instance (K islands alive)
 };
@@ -117,6 +125,7 @@ struct TgSolveCtx {
     int32_t gallopMax;          // probes of one galloping round
     uint32_t* slotBar;          // [nSlots] arrival counters of the team barriers, zeroed every round
     TgCtrl* ctrl;
+    tg_result* specOut;         // [TG_MAX_ITEMS] results of the current round's speculative back-tracks
     tg_result* out;
     const uint16_t* rankOf;     // [65536] rank of a mask inside its popcount class
     uint32_t flags;             // TG_SOLVE_*

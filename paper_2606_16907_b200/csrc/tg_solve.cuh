@@ -196,7 +196,8 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     // DP only needs the islands of the optimal mask S*: S* is the lowest mask attaining the optimum at
     // T*, so no subset of it ties, and the back-track never leaves its subsets.
     if (tid < 32) {
-        const uint32_t allow = ((__ldcg(&itp->flags) & 1) && ctx.mode == 0) ? I.incMask : 0xffffu;
+        const int fl = __ldcg(&itp->flags);
+        const uint32_t allow = ((fl & TG_IT_TRACK) && !(fl & TG_IT_ALLISL) && ctx.mode == 0) ? I.incMask : 0xffffu;
         const bool ok = lane < I.K && I.cminAll[lane] <= T && (allow >> lane & 1u);
         const uint32_t bal = __ballot_sync(0xffffffffu, ok);
         if (lane < TG_MAX_K) sm.isl[lane] = 0;
@@ -615,12 +616,12 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
 // per-state argmin (lowest b, then lowest j — SURVEY A13) along the optimal path from the stored
 // G levels of the slot.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgItem* itp, unsigned long long key, const uint32_t* slot) {
+__device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgItem* itp, unsigned long long key, const uint32_t* slot,
+                            tg_result* out) {
     const int lane = threadIdx.x & 31;
     TgInstDev& I = ctx.inst[__ldcg(&itp->inst)];
     const int L = I.L, K = I.K, Ke = sm.sKe;
     const uint32_t T = __ldcg(&itp->T);
-    tg_result* out = ctx.out + __ldcg(&itp->inst);
     uint8_t isl[TG_MAX_K];
 #pragma unroll
     for (int e = 0; e < TG_MAX_K; ++e) isl[e] = sm.isl[e];
@@ -701,8 +702,8 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
         z.island_mask = So;
         z.n_stages = n;
         z.n_thresholds_run = uint32_t(I.nrun + 1);
-        if (ctx.mode == 1) { z.bottleneck_us = int32_t(Trep); z.iter_time_us = int64_t(val) + int64_t(I.m - 1) * Trep; }
-        else { z.bottleneck_us = int32_t(T); z.iter_time_us = I.incIter; }
+        z.bottleneck_us = int32_t(Trep);
+        z.iter_time_us = int64_t(val) + int64_t(I.m - 1) * Trep;   // (= the incumbent's value when this is the final DP)
         for (int e = 0; e < n; ++e) { z.stage_begin[e] = sb[e]; z.stage_island[e] = si[e]; z.stage_plan[e] = sp[e]; }
         *out = z;
     }
@@ -712,7 +713,7 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
 // One DP(T): all wavefront levels of one item by a team of `teamSize` CTAs (this CTA = `member`).
 // ---------------------------------------------------------------------------------------------
 __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* wbufAll, const TgItem* itp,
-                          unsigned long long* key, int member, int teamSize, int slotIdx) {
+                          unsigned long long* key, int member, int teamSize, int slotIdx, int itemIdx) {
     tgStageItem(ctx, sm, Cs, wbufAll, itp, member == 0);
     tgMark(sm, 0);
     const TgInstDev& I = ctx.inst[sm.sInst];
@@ -748,7 +749,9 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         }
     }
     tgMark(sm, 0);
-    if ((__ldcg(&itp->flags) & 1) && member == 0 && threadIdx.x < 32) tgBacktrack(ctx, sm, itp, __ldcg(key), slot);
+    if ((__ldcg(&itp->flags) & TG_IT_TRACK) && member == 0 && threadIdx.x < 32)
+        tgBacktrack(ctx, sm, itp, __ldcg(key), slot,
+                    (__ldcg(&itp->flags) & TG_IT_SPEC) ? ctx.specOut + itemIdx : ctx.out + __ldcg(&itp->inst));
     __syncthreads();
     tgMark(sm, 7);
 }
@@ -833,7 +836,7 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev
     if (I.phase == TG_PH_FINAL) { I.phase = TG_PH_DONE; return; }   // result written by the back-tracker
     int nf = 0;
     int nRes = cnt;   // a speculative final DP, if any, is the last item: not a search result
-    if (nRes > 0 && (P.flags(beg + nRes - 1) & 1)) --nRes;
+    if (nRes > 0) { const int fl = P.flags(beg + nRes - 1); if ((fl & TG_IT_TRACK) && !(fl & TG_IT_ALLISL)) --nRes; }
     int loInf = I.loInf, hiFeas = I.hiFeas, incIdx = I.incIdx, incQ = -1;
     int64_t incIter = I.incIter;
     const int64_t m1 = int64_t(I.m - 1);
@@ -848,6 +851,10 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev
         if (incIdx < 0 || it < incIter || (it == incIter && tidx < incIdx)) { incIter = it; incIdx = tidx; incQ = q; incKey = key; }
     }
     I.loInf = loInf; I.hiFeas = hiFeas;
+    I.specItem = -1;
+    if (I.specIdx >= 0)   // speculation ran: is the incumbent's back-tracked result among the items of that round?
+        for (int q = 0; q < cnt; ++q)
+            if ((P.flags(beg + q) & TG_IT_SPEC) && P.tidx(beg + q) == incIdx) { I.specItem = beg + q; break; }
     if (incQ >= 0) {
         I.incIter = incIter; I.incIdx = incIdx;
         const uint32_t Sc = uint32_t(incKey >> 8) & 0xffffu;   // compact labels of that item
@@ -895,6 +902,8 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev
 __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W, bool full) {
     const int n = I.ncand;
     I.nProbe = 0;
+    const int specItem = I.specItem;   // refers to the round just folded
+    I.specItem = -1;
     if (I.phase == TG_PH_NEW) {
         if (ctx.mode == 1) I.phase = TG_PH_FINAL;
         else if (n == 0 || I.lbIdx >= n) { tgWriteInfeasible(ctx, I, i); return TG_PH_DONE; }
@@ -968,7 +977,14 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
             // every unresolved candidate is probed this round: run the final DP at the incumbent alongside
             // (speculation: it stands unless one of these probes takes the incumbent over)
             int spec = -1;
-            if (!truncated && total < W && np == int(total)) { probe[np++] = B.incIdx | TG_PROBE_FINAL; spec = B.incIdx; }
+            if (!truncated && total < W && np == int(total)) {
+                // last round of the search.  With few instances a round costs a DP's latency whatever it holds, so
+                // every probe keeps its levels and back-tracks too: whichever ends up as the optimum already has its plan
+                if (ctx.nInst <= TG_SPEC_ALL_MAX_INST)
+                    for (int q = 0; q < np; ++q) probe[q] |= TG_PROBE_KEEP;
+                probe[np++] = B.incIdx | TG_PROBE_FINAL;
+                spec = B.incIdx;
+            }
             I.specIdx = spec;
             I.nProbe = np;
             return TG_PH_BNB;
@@ -984,7 +1000,14 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
         }
     }
     if (I.phase == TG_PH_FINAL) {
-        if (ctx.mode == 0 && I.specIdx >= 0 && I.specIdx == I.incIdx) { I.phase = TG_PH_DONE; return TG_PH_DONE; }   // already back-tracked
+        if (ctx.mode == 0 && specItem >= 0) {   // already back-tracked (speculatively) in the round just folded
+            const unsigned long long* src = reinterpret_cast<const unsigned long long*>(ctx.specOut + specItem);
+            unsigned long long* dst = reinterpret_cast<unsigned long long*>(ctx.out + i);
+            for (int w = 0; w < int(sizeof(tg_result) / 8); ++w) dst[w] = __ldcg(src + w);
+            ctx.out[i].n_thresholds_run = uint32_t(I.nrun);
+            I.phase = TG_PH_DONE;
+            return TG_PH_DONE;
+        }
         I.probe[0] = ctx.mode == 1 ? -1 : I.incIdx; I.nProbe = 1;
         return TG_PH_FINAL;
     }
@@ -1084,9 +1107,11 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
                 TgItem& it = items[pos + q];
                 it.inst = i;
                 const int pq = I.probe[q];
-                it.tidx = pq >= 0 ? (pq & ~TG_PROBE_FINAL) : -1;
+                it.tidx = pq >= 0 ? (pq & ~(TG_PROBE_FINAL | TG_PROBE_KEEP)) : -1;
                 it.T = it.tidx >= 0 ? I.cand[it.tidx] : ctx.dpT;
-                it.flags = (kind == TG_PH_FINAL || (pq >= 0 && (pq & TG_PROBE_FINAL))) ? 1 : 0;
+                it.flags = kind == TG_PH_FINAL ? TG_IT_TRACK
+                           : (pq >= 0 && (pq & TG_PROBE_FINAL)) ? (TG_IT_TRACK | TG_IT_SPEC)
+                           : (pq >= 0 && (pq & TG_PROBE_KEEP)) ? (TG_IT_TRACK | TG_IT_SPEC | TG_IT_ALLISL) : 0;
             }
         }
     }
@@ -1109,7 +1134,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
             const TgInstDev& I = ctx.inst[it.inst];
             const int L = I.L, K = I.K;
             const uint32_t T = it.T;
-            const uint32_t allow = ((it.flags & 1) && ctx.mode == 0) ? I.incMask : 0xffffu;   // as in tgStageItem
+            const uint32_t allow = ((it.flags & TG_IT_TRACK) && !(it.flags & TG_IT_ALLISL) && ctx.mode == 0) ? I.incMask : 0xffffu;   // as in tgStageItem
             // lane = (island k, half of the lengths d): counts the admissible lengths of its half -- sufMinAll is
             // non-decreasing in d, so the count over both halves is the longest admissible slice of k
             const int k = lane & 15, half = lane >> 4;
@@ -1228,7 +1253,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
                     __syncthreads();
                     const int it = sm.curItem;
                     if (it >= nItems) break;
-                    tgRunItem(ctx, sm, Cs, wbufAll, items + it, keys + it, 0, 1, b);
+                    tgRunItem(ctx, sm, Cs, wbufAll, items + it, keys + it, 0, 1, b, it);
                 }
             }
         } else {
@@ -1245,7 +1270,7 @@ __global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) 
                 start = int((int64_t(t) * nCta) / nItems);
                 end = int((int64_t(t + 1) * nCta) / nItems);
             }
-            tgRunItem(ctx, sm, Cs, wbufAll, items + t, keys + t, b - start, end - start, t);
+            tgRunItem(ctx, sm, Cs, wbufAll, items + t, keys + t, b - start, end - start, t, t);
             if (b == start && threadIdx.x == 0 && round < 8 && t < 16) {
                 unsigned long long ns;
                 asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ns));
