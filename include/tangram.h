@@ -68,6 +68,20 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
                              const int32_t* island_cap_mb, const int32_t* bw_gbps, int32_t act_mb,
                              tg_instance** out);
 
+/* tg_instance_create_classes — SURVEY.md §8(f) NEXT-3(a), redundancy pruning by signature (slices
+ * with the same composition of atoms are queried once).  The tables are given per signature class:
+ *   class_of_slice  EITHER [NS] int32 in [0, n_classes): class of slice s(a,b)
+ *   class_time_us   EITHER [n_classes][K][P], class_mem_mb likewise (same value rules as tg_instance_create)
+ * and the instance is by definition the one whose time_us[s][k][p] = class_time_us[class_of_slice[s]][k][p] (same
+ * for mem_mb); 1 <= n_classes <= NS.  Only the class tables cross the host-device link (for identical layers
+ * n_classes = L: NS/L = (L+1)/2 times fewer bytes); they are expanded on the device.  Everything else as
+ * tg_instance_create; a class index out of range -> TG_ERR_RANGE. */
+tg_status tg_instance_create_classes(int32_t L, int32_t K, int32_t P, int32_t m, int32_t n_classes,
+                                     const int32_t* class_of_slice, const int32_t* class_time_us,
+                                     const int32_t* class_mem_mb, const int32_t* island_gpus,
+                                     const int32_t* island_cap_mb, const int32_t* bw_gbps, int32_t act_mb,
+                                     tg_instance** out);
+
 /* tg_instance_create_batch — n instances in one call: element i of every array argument describes instance i
  * exactly as the arguments of tg_instance_create do (L, K, P, m, act_mb: HOST arrays of n int32; time_us ...
  * bw_gbps: HOST arrays of n pointers, each EITHER host or device).  All uploads and validations are enqueued

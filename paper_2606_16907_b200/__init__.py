@@ -61,7 +61,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
+EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
            "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -78,6 +78,9 @@ def lib():
         L = C.CDLL(LIB_PATH)
         vp, i32, i64, u32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32
         L.tg_instance_create.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp, i32, C.POINTER(vp)]
+        L.tg_instance_create_classes.argtypes = [i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, i32, C.POINTER(vp)]
+        L.tg_instance_create_batch.argtypes = [i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.tg_instance_set_transfer_bound.argtypes = [vp, i32]
         L.tg_instance_destroy.argtypes = [vp]
         L.tg_instance_set_actmem.argtypes = [vp, vp]
         L.tg_solve_batch.argtypes = [C.POINTER(vp), i32, vp, vp]
@@ -157,6 +160,18 @@ def tg_instance_create(L, K, P, m, time_us, mem_mb, island_gpus, island_cap_mb, 
     arrs = [prep(a) for a in (time_us, mem_mb, island_gpus, island_cap_mb, bw_gbps)]
     h = C.c_void_p(0)
     _check(lib().tg_instance_create(L, K, P, m, *[_ptr(a) for a in arrs], act_mb, C.byref(h)))
+    return Instance(h.value, L, K, P, m)
+
+
+def tg_instance_create_classes(L, K, P, m, class_of_slice, class_time_us, class_mem_mb, island_gpus, island_cap_mb,
+                               bw_gbps, act_mb) -> Instance:
+    """NEXT-3(a): tables per signature class ([NC,K,P]) and the class of every slice ([NS])."""
+    def prep(a):
+        return np.ascontiguousarray(a, dtype=np.int32) if isinstance(a, np.ndarray) else a
+    arrs = [prep(a) for a in (class_of_slice, class_time_us, class_mem_mb, island_gpus, island_cap_mb, bw_gbps)]
+    nc = int(arrs[1].shape[0])
+    h = C.c_void_p(0)
+    _check(lib().tg_instance_create_classes(L, K, P, m, nc, *[_ptr(a) for a in arrs], act_mb, C.byref(h)))
     return Instance(h.value, L, K, P, m)
 
 

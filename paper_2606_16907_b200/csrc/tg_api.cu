@@ -420,6 +420,66 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
     return TG_OK;
 }
 
+tg_status tg_instance_create_classes(int32_t L, int32_t K, int32_t P, int32_t m, int32_t n_classes,
+                                     const int32_t* class_of_slice, const int32_t* class_time_us,
+                                     const int32_t* class_mem_mb, const int32_t* island_gpus,
+                                     const int32_t* island_cap_mb, const int32_t* bw_gbps, int32_t act_mb, tg_instance** out) {
+    if (!class_of_slice || !class_time_us || !class_mem_mb || !island_gpus || !island_cap_mb || !bw_gbps || !out)
+        return fail(TG_ERR_NULL, "NULL argument");
+    if (L < 1 || L > TG_MAX_L || K < 1 || K > TG_MAX_K || P < 1 || P > TG_MAX_P || m < 1 || m > TG_MAX_M)
+        return fail(TG_ERR_SHAPE, "L, K, P or m outside limits");
+    const int NS = L * (L + 1) / 2;
+    if (n_classes < 1 || n_classes > NS) return fail(TG_ERR_SHAPE, "n_classes outside [1, NS]");
+    if (act_mb < 0 || act_mb > (1 << 20)) return fail(TG_ERR_RANGE, "act_mb outside [0, 2^20]");
+    int dev = 0;
+    TG_CUDA(cudaGetDevice(&dev));
+    DeviceState* D;
+    tg_status s = deviceInit(dev, &D);
+    if (s != TG_OK) return s;
+    const size_t KP = size_t(K) * P, nE = size_t(NS) * KP, nC = size_t(n_classes) * KP;
+    char *base = nullptr, *tmp = nullptr;
+    Carver cv, ct;
+    const size_t oT = cv.take(nE * 4), oM = cv.take(nE * 4), oG = cv.take(K * 4), oC = cv.take(K * 4), oB = cv.take(K * K * 4), oE = cv.take(4);
+    const size_t oCls = ct.take(size_t(NS) * 4), oCt = ct.take(nC * 4), oCm = ct.take(nC * 4);
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&base), cv.off, 0));
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&tmp), ct.off, 0);
+    if (e != cudaSuccess) { cudaFreeAsync(base, 0); return fail(TG_ERR_OOM, std::string("class tables: ") + cudaGetErrorString(e)); }
+    tg_instance* t = new (std::nothrow) tg_instance();
+    if (!t) { cudaFreeAsync(base, 0); cudaFreeAsync(tmp, 0); return fail(TG_ERR_OOM, "host allocation failed"); }
+    t->L = L; t->K = K; t->P = P; t->m = m; t->act_mb = act_mb; t->NS = NS; t->device = dev;
+    t->actmem = nullptr;
+    t->xbound = 0;
+    t->time_us = reinterpret_cast<int32_t*>(base + oT); t->mem_mb = reinterpret_cast<int32_t*>(base + oM);
+    t->gpus = reinterpret_cast<int32_t*>(base + oG); t->cap_mb = reinterpret_cast<int32_t*>(base + oC);
+    t->bw = reinterpret_cast<int32_t*>(base + oB);
+    int* dErr = reinterpret_cast<int*>(base + oE);
+    int32_t* dCls = reinterpret_cast<int32_t*>(tmp + oCls);
+    int32_t* dCt = reinterpret_cast<int32_t*>(tmp + oCt);
+    int32_t* dCm = reinterpret_cast<int32_t*>(tmp + oCm);
+    e = cudaMemcpyAsync(dCls, class_of_slice, size_t(NS) * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dCt, class_time_us, nC * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dCm, class_mem_mb, nC * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(t->gpus, island_gpus, K * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(t->cap_mb, island_cap_mb, K * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(t->bw, bw_gbps, K * K * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dErr, 0, 4, 0);
+    int herr = 0;
+    if (e == cudaSuccess) {
+        const int blocks = std::max(1, int(std::min<size_t>((nE + 255) / 256, 4096)));
+        tgExpandClassesKernel<<<blocks, 256>>>(dCls, dCt, dCm, n_classes, int(KP), nE, t->time_us, t->mem_mb, dErr);
+        tgValidateKernel<<<blocks, 256>>>(t->time_us, t->mem_mb, t->gpus, t->cap_mb, t->bw, K, nE, dErr);
+        e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);   // the one synchronisation of the call
+    }
+    cudaFreeAsync(tmp, 0);
+    if (e != cudaSuccess || herr) {
+        tg_instance_destroy(t);
+        if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("instance upload: ") + cudaGetErrorString(e));
+        return fail(TG_ERR_RANGE, "value out of range (bits: 1 time, 2 mem, 4 bw, 8 gpus, 16 cap, 32 class index): " + std::to_string(herr));
+    }
+    *out = t;
+    return TG_OK;
+}
+
 tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K, const int32_t* P, const int32_t* m,
                                    const int32_t* const* time_us, const int32_t* const* mem_mb,
                                    const int32_t* const* island_gpus, const int32_t* const* island_cap_mb,

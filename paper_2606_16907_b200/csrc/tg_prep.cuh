@@ -69,6 +69,21 @@ __global__ void tgValidateKernel(const int32_t* __restrict__ time_us, const int3
     if (bad) atomicOr(err, bad);
 }
 
+// tg_instance_create_classes: time/mem[s][k][p] = class table[class_of[s]][k][p]; err bit 32 = class index out of range
+__global__ void tgExpandClassesKernel(const int32_t* __restrict__ classOf, const int32_t* __restrict__ ctime,
+                                      const int32_t* __restrict__ cmem, int nClasses, int KP, size_t nEntries,
+                                      int32_t* __restrict__ time_us, int32_t* __restrict__ mem_mb, int* err) {
+    int bad = 0;
+    for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < nEntries; i += size_t(gridDim.x) * blockDim.x) {
+        const size_t s = i / size_t(KP), r = i - s * size_t(KP);
+        const int c = classOf[s];
+        if (c < 0 || c >= nClasses) { bad = 32; time_us[i] = TG_INVALID; mem_mb[i] = 0; continue; }
+        time_us[i] = ctime[size_t(c) * KP + r];
+        mem_mb[i] = cmem[size_t(c) * KP + r];
+    }
+    if (bad) atomicOr(err, bad);
+}
+
 __global__ void tgValidateNonNegKernel(const int32_t* __restrict__ v, size_t n, int* err) {
     int bad = 0;
     for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += size_t(gridDim.x) * blockDim.x)

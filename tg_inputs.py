@@ -275,6 +275,21 @@ def with_actmem(inst: Instance, seed: int, lo: int = 0, hi: int = 60) -> Instanc
     return o
 
 
+def length_classes(inst: Instance):
+    """Signature classes of a model of identical layers (NEXT-3(a)): the class of a slice is its length, and the class
+    tables are the rows of the slices that start at layer 0.  Returns (class_of_slice [NS], class_time [L,K,P],
+    class_mem [L,K,P], the expanded Instance these define)."""
+    L = inst.L
+    a, b = slice_bounds(L)
+    class_of = (b - a - 1).astype(np.int32)
+    rows = np.array([slice_index(L, 0, d) for d in range(1, L + 1)])
+    ct, cm = inst.time_us[rows].copy(), inst.mem_mb[rows].copy()
+    o = inst.copy()
+    o.time_us, o.mem_mb = ct[class_of], cm[class_of]
+    o.name = inst.name + "_cls"
+    return class_of, ct, cm, o
+
+
 def with_transfer_bound(inst: Instance) -> Instance:
     """Same tables, transfers bounded by the threshold as well (NEXT-3(b))."""
     o = inst.copy()
