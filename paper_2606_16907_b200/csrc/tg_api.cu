@@ -300,6 +300,8 @@ tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cud
             TG_CUDA(cudaMemcpy(&hi, W.inst, sizeof(TgInstDev), cudaMemcpyDeviceToHost));
             std::vector<int32_t> e(hi.nEval > 0 ? hi.nEval : 1);
             TG_CUDA(cudaMemcpy(e.data(), hi.eIdx, sizeof(int32_t) * e.size(), cudaMemcpyDeviceToHost));
+            fprintf(stderr, "[tg] inst0 prepare cycles: minima %lld sort %lld unique %lld lbIdx %lld\n", hi.prepCyc[1] - hi.prepCyc[0],
+                    hi.prepCyc[2] - hi.prepCyc[1], hi.prepCyc[3] - hi.prepCyc[2], hi.prepCyc[4] - hi.prepCyc[3]);
             fprintf(stderr, "[tg] inst0: ncand=%d lbIdx=%d lowestFeasible=%d incIdx=%d nEval=%d evaluated:", hi.ncand, hi.lbIdx,
                     hi.nEval > 0 ? (e[0] & ~TG_EDONE) : -1, hi.incIdx, hi.nEval);
             for (int q = 0; q < hi.nEval && q < 48; ++q) fprintf(stderr, " %d", e[q] & ~TG_EDONE);

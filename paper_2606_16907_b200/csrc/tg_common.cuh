@@ -64,6 +64,7 @@ struct TgInstDev {
     int32_t sortCap, ncand;
     uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
     uint32_t maxKey;                  // largest finite reduced cost of any depth (bounds the radix sort's passes)
+    long long prepCyc[6];             // TG_DEBUG: clock stamps of the prepare kernel's stages
     int32_t planKind;                 // wide scheduling: item kind returned by this round's planning
     int32_t xbound;                   // NEXT-3(b): transfers are admissible only if x <= T (tg_instance_set_transfer_bound)
     uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major

@@ -259,7 +259,7 @@ __device__ uint32_t* tgRadixSort(uint32_t* A, uint32_t* B, int n, uint32_t maxKe
 }
 
 #define TG_PREP_NT 1024
-#define TG_SORT_SMEM_MAX 16384    // words of dynamic shared memory of the prepare kernel (radix histograms: 32 warps x 512 digits)
+#define TG_SORT_SMEM_MAX 32768    // words of dynamic shared memory of the prepare kernel (key bitmap of 2^20 bits; radix histograms need half)
 
 __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restrict__ insts) {
     extern __shared__ uint32_t sbuf[];
@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     __shared__ uint32_t sMaxX;
     TgInstDev& I = insts[blockIdx.x];
     const int L = I.L, K = I.K, tid = threadIdx.x;
-    if (tid == 0) sMaxX = 0;
+    if (tid == 0) { sMaxX = 0; I.prepCyc[0] = clock64(); }
     __syncthreads();
     // transfer table
     if (tid < K * K) {
@@ -310,27 +310,62 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     __syncthreads();
     for (int w = tid; w < K * stride; w += TG_PREP_NT) { sm[w] = sbuf[w]; sma[w] = sbuf[K * stride + w]; }
     __syncthreads();
-    // candidate sort: stable LSD radix sort, 8- or 9-bit digits, ping-pong between the two global buffers
-    // (L2 resident); per-warp digit histograms in shared memory, warp w owns a contiguous chunk
+    if (tid == 0) I.prepCyc[1] = clock64();
+    // Step 3, candidate thresholds = ascending distinct finite keys.  The keys are bounded by maxKey, which for
+    // microsecond stage times is far below the number of bits shared memory holds (2^20): mark every key in a
+    // bitmap with shared-memory atomics and read the set bits back in order -- O(n + maxKey/32) instead of a sort.
+    // Larger keys: stable LSD radix sort (8- or 9-bit digits, per-warp histograms, ping-pong between two global
+    // buffers) followed by a unique pass.
     const int n = I.NS * K * I.nDepth + (I.xbound ? K * K : 0);
-    uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, max(I.maxKey, sMaxX), sbuf, warpSums);
-    // unique, finite only
+    const uint32_t maxKey = max(I.maxKey, sMaxX);
+    const uint32_t nWords = (maxKey >> 5) + 1u;
     uint32_t base = 0;
-    for (int i0 = 0; i0 < n; i0 += 4 * TG_PREP_NT) {   // four consecutive keys a thread: one block scan per 4096 keys
-        const int i = i0 + 4 * tid;
-        uint32_t v[5], f[4], cnt = 0;
-        v[0] = (i > 0 && i < n) ? __ldcg(buf + i - 1) : 0xffffffffu;   // left neighbour of the thread's first key
+    if (nWords <= uint32_t(TG_SORT_SMEM_MAX)) {
+        for (uint32_t w = tid; w < nWords; w += TG_PREP_NT) sbuf[w] = 0u;
+        __syncthreads();
+        for (int i0 = 0; i0 < n; i0 += 4 * TG_PREP_NT) {   // four independent loads a thread
+            uint32_t v[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) v[e + 1] = i + e < n ? __ldcg(buf + i + e) : 0xffffffffu;
+            for (int e = 0; e < 4; ++e) { const int i = i0 + e * TG_PREP_NT + tid; v[e] = i < n ? __ldcg(I.sortbuf + i) : TG_INFU; }
 #pragma unroll
-        for (int e = 0; e < 4; ++e) { f[e] = (v[e + 1] < TG_INFU && (i + e == 0 || v[e] != v[e + 1])) ? 1u : 0u; cnt += f[e]; }
+            for (int e = 0; e < 4; ++e) if (v[e] <= maxKey) atomicOr(&sbuf[v[e] >> 5], 1u << (v[e] & 31u));
+        }
+        __syncthreads();
+        if (tid == 0) I.prepCyc[2] = clock64();
+        const uint32_t per = (nWords + TG_PREP_NT - 1) / TG_PREP_NT, w0 = uint32_t(tid) * per;
+        uint32_t cnt = 0;
+        for (uint32_t q = 0; q < per; ++q) cnt += (w0 + q < nWords) ? uint32_t(__popc(sbuf[w0 + q])) : 0u;
         uint32_t tot;
-        uint32_t pos = base + tgBlockExScan(cnt, warpSums, tot);
+        uint32_t pos = tgBlockExScan(cnt, warpSums, tot);
+        for (uint32_t q = 0; q < per && w0 + q < nWords; ++q) {
+            uint32_t bits = sbuf[w0 + q];
+            while (bits) {
+                I.cand[pos++] = ((w0 + q) << 5) + uint32_t(__ffs(bits) - 1);
+                bits &= bits - 1u;
+            }
+        }
+        base = tot;
+        __syncthreads();   // the bitmap is overwritten below
+    } else {
+        uint32_t* buf = tgRadixSort(I.sortbuf, I.sortbuf2, n, maxKey, sbuf, warpSums);
+        if (tid == 0) I.prepCyc[2] = clock64();
+        // unique, finite only
+        for (int i0 = 0; i0 < n; i0 += 4 * TG_PREP_NT) {   // four consecutive keys a thread: one block scan per 4096 keys
+            const int i = i0 + 4 * tid;
+            uint32_t v[5], f[4], cnt = 0;
+            v[0] = (i > 0 && i < n) ? __ldcg(buf + i - 1) : 0xffffffffu;   // left neighbour of the thread's first key
 #pragma unroll
-        for (int e = 0; e < 4; ++e) if (f[e]) I.cand[pos++] = v[e + 1];
-        base += tot;
+            for (int e = 0; e < 4; ++e) v[e + 1] = i + e < n ? __ldcg(buf + i + e) : 0xffffffffu;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) { f[e] = (v[e + 1] < TG_INFU && (i + e == 0 || v[e] != v[e + 1])) ? 1u : 0u; cnt += f[e]; }
+            uint32_t tot;
+            uint32_t pos = base + tgBlockExScan(cnt, warpSums, tot);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) if (f[e]) I.cand[pos++] = v[e + 1];
+            base += tot;
+        }
     }
-    if (tid == 0) I.ncand = int(base);
+    if (tid == 0) { I.ncand = int(base); I.prepCyc[3] = clock64(); }
     // (the suffix minima go to shared memory for the search below: it is a chain of dependent reads)
     uint32_t* smaS = sbuf;
     for (int w = tid; w < K * stride; w += TG_PREP_NT) smaS[w] = sma[w];
@@ -357,7 +392,7 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
             for (int o = 16; o > 0; o >>= 1) len += __shfl_xor_sync(0xffffffffu, len, o);
             if (len >= L) hi = mid; else lo = mid + 1;
         }
-        if (tid == 0) I.lbIdx = lo;
+        if (tid == 0) { I.lbIdx = lo; I.prepCyc[4] = clock64(); }
     }
 }
 

@@ -187,3 +187,27 @@ def test_create_batch(tg):
     with pytest.raises(tg.TangramError) as e:
         tg.tg_instance_create_batch([spec(insts[1]), tuple(shape)])
     assert e.value.status == 2 and "instance 1" in str(e.value)
+
+
+def test_large_stage_times(tg):
+    """Stage times up to TG_TIME_MAX = 2^25 us: candidate extraction leaves the shared-memory bitmap (keys < 2^20) for
+    the radix sort; times just below and above the switch, and the largest allowed value."""
+    insts = []
+    for seed, scale in [(0, 10), (1, 300), (2, 3000)]:
+        i = gen.config3(seed, L=14, K=5)
+        valid = i.time_us != 0x7FFFFFFF
+        i.time_us = np.where(valid, np.minimum(i.time_us.astype(np.int64) * scale, 1 << 25), 0x7FFFFFFF).astype(np.int32)
+        i.name += f"_x{scale}"
+        insts.append(i)
+    j = gen.random_small(11, Lmax=6, Kmax=3, Pmax=2)
+    j.time_us = np.where(j.time_us != 0x7FFFFFFF, (1 << 25) - (j.time_us % 7), 0x7FFFFFFF).astype(np.int32)
+    insts.append(j)
+    assert max(int(i.time_us[i.time_us != 0x7FFFFFFF].max()) for i in insts[:1]) < (1 << 20) <= \
+        min(int(i.time_us[i.time_us != 0x7FFFFFFF].max()) for i in insts[1:])
+    for inst, g in zip(insts, solve_all(tg, insts)):
+        same(oracle.solve(inst), g, inst.name)
+    for inst in insts:
+        h = tg.instance_from_inputs(inst)
+        cand = tg.tg_reduce(h)[3]
+        assert np.array_equal(cand.astype(np.int64), oracle.reduce(inst)[3]), inst.name
+        h.destroy()
