@@ -43,6 +43,8 @@ struct DeviceState {
     int smemPerSM = 0;
     int ctasPerSM = 0;    // co-resident CTAs of the solver per SM
     int dynSmem = 0;      // dynamic shared memory of one solver CTA
+    uint64_t budget = 0;  // bytes the DP scratch may take (from cudaMemGetInfo; refreshed every 64 solves or after a failed allocation)
+    int budgetAge = 0;
     uint16_t* rankOf = nullptr;
 };
 std::mutex g_mu;
@@ -211,16 +213,26 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const uint64_t slotWords = alignUp(size_t(maxFull) + 1024, 1024);
     int nSlots = 0;
     if (needSolve) {
-        size_t freeB = 0, totalB = 0;
-        TG_CUDA(cudaMemGetInfo(&freeB, &totalB));
-        const uint64_t budget = std::min<uint64_t>(uint64_t(freeB) * 6 / 10, 12ull << 30);   // bytes
-        nSlots = int(std::min<uint64_t>(uint64_t(numCtas), budget / (slotWords * 4)));
+        if (D->budget == 0 || ++D->budgetAge >= 64) {   // (the query costs tens of microseconds: not on every solve)
+            size_t freeB = 0, totalB = 0;
+            TG_CUDA(cudaMemGetInfo(&freeB, &totalB));
+            D->budget = std::min<uint64_t>(uint64_t(freeB) * 6 / 10, 12ull << 30);   // bytes
+            D->budgetAge = 0;
+        }
+        nSlots = int(std::min<uint64_t>(uint64_t(numCtas), D->budget / (slotWords * 4)));
         if (nSlots < 1) nSlots = 1;   // let the allocation decide
     }
     const size_t oBar = cv.take(sizeof(uint32_t) * size_t(std::max(nSlots, 1)));
     const size_t oScratch = cv.take(size_t(slotWords) * 4 * size_t(nSlots), 4096);
     W.bytes = cv.off + 4096;
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&W.base), W.bytes, st));
+    {
+        const cudaError_t ea = cudaMallocAsync(reinterpret_cast<void**>(&W.base), W.bytes, st);
+        if (ea != cudaSuccess) {
+            D->budget = 0;   // measure again on the next call
+            cudaGetLastError();
+            return fail(ea == cudaErrorMemoryAllocation ? TG_ERR_OOM : TG_ERR_CUDA, std::string("workspace allocation: ") + cudaGetErrorString(ea));
+        }
+    }
     for (int i = 0; i < n; ++i) {
         h[i].cd = reinterpret_cast<uint32_t*>(W.base + oCd[i]);
         h[i].argp = reinterpret_cast<uint8_t*>(W.base + oArgp[i]);
