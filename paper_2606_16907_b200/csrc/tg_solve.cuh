@@ -762,7 +762,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
 __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
     const int widest = tgBinom[K][K >> 1];
     const int team = max(1, widest / (8 * ctx.nActiveWarps));
-    return min(max(int(gridDim.x) / team, 8), 12);
+    return min(max(int(gridDim.x) / team, 8), ctx.wishCap);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -913,7 +913,9 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
     if (I.phase == TG_PH_FEAS) {
         if (I.hiFeas < 0) {
             if (I.loInf >= n - 1) { tgWriteInfeasible(ctx, I, i); return TG_PH_DONE; }
-            // galloping: loInf + gstep, + 2 gstep, ... ; at most 8 probes a round, the step keeps doubling
+            // galloping: loInf + gstep, + 2 gstep, ... ; at most gallopMax (10) probes a round, the step keeps doubling.
+            // (More probes reach thresholds far above the optimum, whose DPs have full-width rows: 16 probes made
+            // cfg3 four times slower; fewer need another round: 8 cost cfg3 20 %.)
             int step = I.gstep;
             const int nmax = min(W, ctx.gallopMax);
             while (I.nProbe < nmax) {
