@@ -50,6 +50,7 @@ struct DeviceState {
 std::mutex g_mu;
 int g_gallopMax = [] { const char* e = getenv("TG_GALLOP_MAX"); int v = e ? atoi(e) : 10; return v < 1 ? 1 : (v > 16 ? 16 : v); }();
 // DPs per instance and scheduler round (speculation width of the threshold search / sweep)
+int g_wishFloor = [] { const char* e = getenv("TG_WISH_FLOOR"); int v = e ? atoi(e) : 8; return v < 1 ? 1 : (v > 12 ? 12 : v); }();
 int g_wishCap = [] { const char* e = getenv("TG_WISH_CAP"); int v = e ? atoi(e) : 12; return v < 8 ? 8 : (v > TG_MAX_WISH ? TG_MAX_WISH : v); }();
 int g_wishMax = [] { const char* e = getenv("TG_WISH_MAX"); int v = e ? atoi(e) : 64; return v < 1 ? 1 : (v > TG_MAX_WISH ? TG_MAX_WISH : v); }();
 DeviceState g_dev[64];
@@ -270,6 +271,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.wishMax = g_wishMax;
     c.gallopMax = g_gallopMax;
     c.wishCap = g_wishCap;
+    c.wishFloor = g_wishFloor;
     c.ctrl = reinterpret_cast<TgCtrl*>(W.base + oCtrl);
     c.rankOf = D->rankOf;
     c.specOut = reinterpret_cast<tg_result*>(W.base + oSpec);

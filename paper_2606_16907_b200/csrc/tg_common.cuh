@@ -124,6 +124,7 @@ struct TgSolveCtx {
     int32_t nSlots;             // <= gridDim.x; a slot belongs to one team (team mode) or one CTA (solo mode)
     int32_t wishMax;            // DPs per instance and round, upper bound
     int32_t gallopMax;          // probes of one galloping round
+    int32_t wishFloor;          // lower end of the same
     int32_t wishCap;            // upper end of the per-round probe count chosen from the instance shape (tgWish)
     uint32_t* slotBar;          // [nSlots] arrival counters of the team barriers, zeroed every round
     TgCtrl* ctrl;

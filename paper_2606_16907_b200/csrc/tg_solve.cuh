@@ -762,7 +762,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
 __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
     const int widest = tgBinom[K][K >> 1];
     const int team = max(1, widest / (8 * ctx.nActiveWarps));
-    return min(max(int(gridDim.x) / team, 8), ctx.wishCap);
+    return min(max(int(gridDim.x) / team, ctx.wishFloor), ctx.wishCap);
 }
 
 // ---------------------------------------------------------------------------------------------
