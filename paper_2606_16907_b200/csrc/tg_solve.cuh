@@ -221,23 +221,23 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         const uint32_t xv = I.x[int(sm.isl[kc]) * TG_MAX_K + int(sm.isl[jc])];
         sm.xS[kc][jc] = (I.xbound && xv > T) ? TG_INFU : xv;   // transfer bound (NEXT-3(b)): a slower link is not admissible at T
     }
-    if (tid < Ke) {  // widest diagonal with an admissible entry: sufMin is non-decreasing in d
-        const uint32_t* sf = I.sufMin + size_t(sm.isl[tid]) * (L + 2);
-        int lo = 0, hi = L - 1;  // answer in [0, L-1]; 0 = none
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (sf[mid] <= T) lo = mid; else hi = mid - 1;
+    // widest diagonal with an admissible entry (b <= L-1) and longest admissible slice at any position (b <= L) of
+    // every island: sufMin / sufMinAll are non-decreasing in d, so each is the number of lengths whose entry is
+    // <= T.  One warp per island, lanes over the lengths: one round trip to L2 instead of a binary search's seven.
+    {
+        const int w = tid >> 5;
+        if (w < Ke) {
+            const uint32_t* sf = I.sufMin + size_t(sm.isl[w]) * (L + 2);
+            const uint32_t* sa = I.sufMinAll + size_t(sm.isl[w]) * (L + 2);
+            unsigned nd = 0, nl = 0;
+            for (int d = 1 + lane; d <= L; d += 32) {
+                nd += (d <= L - 1 && sf[d] <= T) ? 1u : 0u;
+                nl += (sa[d] <= T) ? 1u : 0u;
+            }
+            nd = __reduce_add_sync(0xffffffffu, nd);
+            nl = __reduce_add_sync(0xffffffffu, nl);
+            if (lane == 0) { sm.dmaxK[w] = int(nd); sm.maxlenK[w] = uint8_t(nl); }
         }
-        sm.dmaxK[tid] = lo;
-    }
-    if (tid >= 32 && tid < 32 + Ke) {  // longest admissible slice at any position (b <= L)
-        const uint32_t* sf = I.sufMinAll + size_t(sm.isl[tid - 32]) * (L + 2);
-        int lo = 0, hi = L;
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (sf[mid] <= T) lo = mid; else hi = mid - 1;
-        }
-        sm.maxlenK[tid - 32] = uint8_t(lo);
     }
     __syncthreads();
     if (tid == 0) {
