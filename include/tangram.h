@@ -86,7 +86,9 @@ tg_status tg_instance_create_classes(int32_t L, int32_t K, int32_t P, int32_t m,
  * exactly as the arguments of tg_instance_create do (L, K, P, m, act_mb: HOST arrays of n int32; time_us ...
  * bw_gbps: HOST arrays of n pointers, each EITHER host or device).  All uploads and validations are enqueued
  * first and the call synchronises ONCE (tg_instance_create synchronises once per instance: 1024 instances cost
- * 1024 round trips).  All or nothing: on any error nothing is created, out[0..n) is NULL and the message names
+ * 1024 round trips).  The instances of a batch share ONE device allocation (two table uploads per instance, one
+ * validation launch for the batch); each is destroyed individually with tg_instance_destroy and the allocation is
+ * released with the last of them.  All or nothing: on any error nothing is created, out[0..n) is NULL and the message names
  * the first offending instance.  n == 0 is a no-op. */
 tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K, const int32_t* P, const int32_t* m,
                                    const int32_t* const* time_us, const int32_t* const* mem_mb,

@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <atomic>
 #include <mutex>
 #include <string>
 #include <vector>
@@ -11,7 +12,14 @@
 #include "tg_prep.cuh"
 #include "tg_solve.cuh"
 
+// One device allocation shared by the instances of a tg_instance_create_batch call; freed with the last of them.
+struct TgBatchBlock {
+    char* base = nullptr;
+    std::atomic<int> refs{0};
+};
+
 struct tg_instance {
+    TgBatchBlock* block = nullptr;                   // nullptr: the instance owns its allocation (time_us is its base)
     int32_t L, K, P, m, act_mb, NS;
     int device;
     int32_t *time_us, *mem_mb, *gpus, *cap_mb, *bw;  // device
@@ -506,27 +514,110 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
     if (n == 0) return TG_OK;
     if (!L || !K || !P || !m || !time_us || !mem_mb || !island_gpus || !island_cap_mb || !bw_gbps || !act_mb || !out)
         return fail(TG_ERR_NULL, "NULL argument");
-    std::vector<int*> dErr(size_t(n), nullptr);
-    tg_status s = TG_OK;
-    int made = 0;
-    for (; made < n; ++made) {
-        out[made] = nullptr;
-        s = createAsync(L[made], K[made], P[made], m[made], time_us[made], mem_mb[made], island_gpus[made],
-                        island_cap_mb[made], bw_gbps[made], act_mb[made], &out[made], &dErr[size_t(made)]);
-        if (s != TG_OK) { g_err = "instance " + std::to_string(made) + ": " + g_err; break; }
+    for (int i = 0; i < n; ++i) out[i] = nullptr;
+    for (int i = 0; i < n; ++i) {
+        const std::string who = "instance " + std::to_string(i) + ": ";
+        if (!time_us[i] || !mem_mb[i] || !island_gpus[i] || !island_cap_mb[i] || !bw_gbps[i]) return fail(TG_ERR_NULL, who + "NULL argument");
+        if (L[i] < 1 || L[i] > TG_MAX_L || K[i] < 1 || K[i] > TG_MAX_K || P[i] < 1 || P[i] > TG_MAX_P || m[i] < 1 || m[i] > TG_MAX_M)
+            return fail(TG_ERR_SHAPE, who + "L, K, P or m outside limits");
+        if (act_mb[i] < 0 || act_mb[i] > (1 << 20)) return fail(TG_ERR_RANGE, who + "act_mb outside [0, 2^20]");
     }
-    std::string err = g_err;
-    if (s == TG_OK) {   // every upload and validation is in flight: one synchronisation for the whole batch
-        std::vector<int> herr(size_t(n), 0);
-        cudaError_t e = cudaSuccess;
-        for (int i = 0; i < n && e == cudaSuccess; ++i) e = cudaMemcpyAsync(&herr[size_t(i)], dErr[size_t(i)], 4, cudaMemcpyDeviceToHost, 0);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(0);
-        if (e != cudaSuccess) { s = TG_ERR_CUDA; err = std::string("instance upload: ") + cudaGetErrorString(e); }
+    int dev = 0;
+    TG_CUDA(cudaGetDevice(&dev));
+    DeviceState* D;
+    tg_status s = deviceInit(dev, &D);
+    if (s != TG_OK) return s;
+
+    // One allocation for the batch: [per instance: time, mem] [small arrays of all instances] [descriptors] [error words].
+    // A handful of driver calls per instance (two table uploads) instead of eight, one validation launch, one
+    // synchronisation.
+    Carver cv;
+    const size_t nn = size_t(n);
+    std::vector<size_t> oT(nn), oM(nn), oS(nn);
+    size_t smallInts = 0, maxE = 0;
+    for (int i = 0; i < n; ++i) {
+        const size_t nE = size_t(L[i]) * (L[i] + 1) / 2 * K[i] * P[i];
+        oT[size_t(i)] = cv.take(nE * 4);
+        oM[size_t(i)] = cv.take(nE * 4);
+        oS[size_t(i)] = smallInts;                       // gpus[K], cap[K], bw[K*K]
+        smallInts += size_t(K[i]) * (2 + K[i]);
+        maxE = std::max(maxE, nE);
+    }
+    const size_t oSmall = cv.take(smallInts * 4), oDesc = cv.take(sizeof(TgValidateDesc) * size_t(n)), oErr = cv.take(size_t(n) * 4);
+    TgBatchBlock* blk = new (std::nothrow) TgBatchBlock();
+    if (!blk) return fail(TG_ERR_OOM, "host allocation failed");
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&blk->base), cv.off, 0);
+    if (e != cudaSuccess) {
+        delete blk;
+        cudaGetLastError();
+        return fail(e == cudaErrorMemoryAllocation ? TG_ERR_OOM : TG_ERR_CUDA, std::string("batch allocation: ") + cudaGetErrorString(e));
+    }
+    char* base = blk->base;
+    int32_t* dSmall = reinterpret_cast<int32_t*>(base + oSmall);
+    std::vector<int32_t> hSmall(smallInts);
+    std::vector<TgValidateDesc> hDesc(nn);
+    struct Late { const int32_t* src; int32_t* dst; size_t ints; };
+    std::vector<Late> late;                              // small arrays that live in device memory: copied after the staged ones
+    int made = 0;
+    for (; made < n && e == cudaSuccess; ++made) {
+        const int i = made;
+        tg_instance* t = new (std::nothrow) tg_instance();
+        if (!t) { e = cudaErrorMemoryAllocation; break; }
+        const int Ki = K[i];
+        const size_t nE = size_t(L[i]) * (L[i] + 1) / 2 * Ki * P[i];
+        t->block = blk;
+        blk->refs.fetch_add(1);
+        t->L = L[i]; t->K = Ki; t->P = P[i]; t->m = m[i]; t->act_mb = act_mb[i]; t->NS = L[i] * (L[i] + 1) / 2; t->device = dev;
+        t->actmem = nullptr;
+        t->xbound = 0;
+        t->time_us = reinterpret_cast<int32_t*>(base + oT[size_t(i)]);
+        t->mem_mb = reinterpret_cast<int32_t*>(base + oM[size_t(i)]);
+        t->gpus = dSmall + oS[size_t(i)];
+        t->cap_mb = t->gpus + Ki;
+        t->bw = t->cap_mb + Ki;
+        out[i] = t;
+        e = cudaMemcpyAsync(t->time_us, time_us[i], nE * 4, cudaMemcpyDefault, 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(t->mem_mb, mem_mb[i], nE * 4, cudaMemcpyDefault, 0);
+        const int32_t* srcs[3] = {island_gpus[i], island_cap_mb[i], bw_gbps[i]};
+        int32_t* dsts[3] = {t->gpus, t->cap_mb, t->bw};
+        const size_t lens[3] = {size_t(Ki), size_t(Ki), size_t(Ki) * Ki};
+        for (int q = 0; q < 3; ++q) {
+            int32_t* hdst = hSmall.data() + (dsts[q] - dSmall);
+            if (isDevicePtr(srcs[q])) { late.push_back({srcs[q], dsts[q], lens[q]}); memset(hdst, 0, lens[q] * 4); }
+            else memcpy(hdst, srcs[q], lens[q] * 4);
+        }
+        hDesc[size_t(i)] = TgValidateDesc{t->time_us, t->mem_mb, t->gpus, t->cap_mb, t->bw, Ki, (unsigned long long)nE};
+    }
+    int* dErr = reinterpret_cast<int*>(base + oErr);
+    std::vector<int> herr(nn, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dSmall, hSmall.data(), smallInts * 4, cudaMemcpyHostToDevice, 0);
+    for (size_t q = 0; q < late.size() && e == cudaSuccess; ++q)
+        e = cudaMemcpyAsync(late[q].dst, late[q].src, late[q].ints * 4, cudaMemcpyDeviceToDevice, 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(base + oDesc, hDesc.data(), sizeof(TgValidateDesc) * size_t(n), cudaMemcpyHostToDevice, 0);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dErr, 0, size_t(n) * 4, 0);
+    if (e == cudaSuccess) {
+        const int bx = int(std::max<size_t>(1, std::min<size_t>((maxE + 255) / 256, 64)));
+        for (int y0 = 0; y0 < n && e == cudaSuccess; y0 += 65535) {      // gridDim.y limit
+            const int ny = std::min(n - y0, 65535);
+            tgValidateBatchKernel<<<dim3(bx, ny), 256>>>(reinterpret_cast<const TgValidateDesc*>(base + oDesc) + y0, dErr + y0);
+            e = cudaGetLastError();
+        }
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(herr.data(), dErr, size_t(n) * 4, cudaMemcpyDeviceToHost, 0);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(0);   // the one synchronisation of the call
+    std::string err;
+    if (e != cudaSuccess) {
+        s = e == cudaErrorMemoryAllocation ? TG_ERR_OOM : TG_ERR_CUDA;
+        err = std::string("batch upload: ") + cudaGetErrorString(e);
+        cudaGetLastError();
+    } else {
         for (int i = 0; i < n && s == TG_OK; ++i)
             if (herr[size_t(i)]) { s = rangeError(herr[size_t(i)], i); err = g_err; }
     }
     if (s != TG_OK) {   // all or nothing
-        for (int i = 0; i < made; ++i) { tg_instance_destroy(out[i]); out[i] = nullptr; }
+        bool any = false;
+        for (int i = 0; i < n; ++i) if (out[i]) { any = true; tg_instance_destroy(out[i]); out[i] = nullptr; }
+        if (!any) { cudaFreeAsync(blk->base, 0); delete blk; }
         return fail(s, err);
     }
     return TG_OK;
@@ -535,7 +626,12 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
 tg_status tg_instance_destroy(tg_instance* inst) {
     if (!inst) return TG_OK;
     if (inst->actmem) cudaFreeAsync(inst->actmem, 0);
-    cudaFreeAsync(inst->time_us, 0);  // base of the single allocation
+    if (inst->block) {   // created by tg_instance_create_batch: the allocation goes with the last instance of the batch
+        TgBatchBlock* blk = inst->block;
+        if (blk->refs.fetch_sub(1) == 1) { cudaFreeAsync(blk->base, 0); delete blk; }
+    } else {
+        cudaFreeAsync(inst->time_us, 0);  // base of the single allocation
+    }
     delete inst;
     return TG_OK;
 }

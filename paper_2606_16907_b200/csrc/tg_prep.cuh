@@ -69,6 +69,31 @@ __global__ void tgValidateKernel(const int32_t* __restrict__ time_us, const int3
     if (bad) atomicOr(err, bad);
 }
 
+// tg_instance_create_batch: the same checks for a whole batch, instance = blockIdx.y
+struct TgValidateDesc {
+    const int32_t *time_us, *mem_mb, *gpus, *cap, *bw;
+    int32_t K;
+    unsigned long long nEntries;
+};
+__global__ void tgValidateBatchKernel(const TgValidateDesc* __restrict__ desc, int* err) {
+    const TgValidateDesc d = desc[blockIdx.y];
+    int bad = 0;
+    for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < d.nEntries; i += size_t(gridDim.x) * blockDim.x) {
+        const int32_t t = d.time_us[i], mm = d.mem_mb[i];
+        if (t != TG_INVALID && (t < 0 || t > TG_TIME_MAX)) bad |= 1;
+        if (mm < 0) bad |= 2;
+    }
+    if (blockIdx.x == 0 && int(threadIdx.x) < d.K * d.K) {
+        const int j = threadIdx.x / d.K, k = threadIdx.x % d.K;
+        if (j != k && d.bw[threadIdx.x] <= 0) bad |= 4;
+        if (j == 0) {
+            if (d.gpus[k] < 1) bad |= 8;
+            if (d.cap[k] < 0) bad |= 16;
+        }
+    }
+    if (bad) atomicOr(err + blockIdx.y, bad);
+}
+
 // tg_instance_create_classes: time/mem[s][k][p] = class table[class_of[s]][k][p]; err bit 32 = class index out of range
 __global__ void tgExpandClassesKernel(const int32_t* __restrict__ classOf, const int32_t* __restrict__ ctime,
                                       const int32_t* __restrict__ cmem, int nClasses, int KP, size_t nEntries,
