@@ -28,6 +28,7 @@ struct TgShared {
     int sWd, sSlack, sWindowed;
     // split of the dynamic shared memory for this item: [cost rows | nWarps x wbufWords]
     int nWarps, wbufWords, wbufOff;
+    int csUsed4;                    // 16-byte words of the staged cost rows of all islands (incl. the pads between them)
     uint32_t cdOff;                 // word offset of the reduced table of the depth currently staged
     uint8_t maxlenK[TG_MAX_K];      // longest admissible slice of island k at T, any position
     uint32_t baseK[TG_MAX_K];
@@ -128,24 +129,29 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
     if (tid == 0) sm.cdOff = uint32_t(q - 1) * uint32_t(I.K) * uint32_t(I.triG);
     __syncthreads();
     if (!sm.useGlobalC) {
-        for (int kc = 0; kc < Ke; ++kc) {
+        // one flat loop over the 16-byte words of every island's rows (island k occupies D_k * nb4 + 1 of them from
+        // baseK[k] / 4): all loads of a thread are independent, one trip to L2 for the whole table instead of one
+        // per island
+        const int tot4 = sm.csUsed4;
+        for (int f = tid; f < tot4; f += TG_NT) {
+            int kc = 0;
+            while (kc + 1 < Ke && int(sm.baseK[kc + 1] >> 2) <= f) ++kc;
+            const int w = f - int(sm.baseK[kc] >> 2);
             const int dk = sm.dmaxK[kc], Dk = (dk + 3) & ~3;
+            if (w >= Dk * nb4) continue;   // the pad between two islands' tables
             const uint32_t* cdk = I.cd + sm.cdOff + size_t(sm.isl[kc]) * I.triG;
-            uint32_t* dst = Cs + sm.baseK[kc];
-            for (int w = tid; w < Dk * nb4; w += TG_NT) {
-                const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
-                uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
-                if (d <= dk && a4 < ((L - d + 3) >> 2)) {
-                    v = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + a4);
-                    const int a = a4 * 4, amax = L - 1 - d;
-                    v.x = (a + 0 <= amax && v.x <= T) ? v.x : TG_INFU;
-                    v.y = (a + 1 <= amax && v.y <= T) ? v.y : TG_INFU;
-                    v.z = (a + 2 <= amax && v.z <= T) ? v.z : TG_INFU;
-                    v.w = (a + 3 <= amax && v.w <= T) ? v.w : TG_INFU;
-                    nAdm += (v.x < TG_INFU) + (v.y < TG_INFU) + (v.z < TG_INFU) + (v.w < TG_INFU);
-                }
-                reinterpret_cast<uint4*>(dst)[w] = v;
+            const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
+            uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+            if (d <= dk && a4 < ((L - d + 3) >> 2)) {
+                v = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + a4);
+                const int a = a4 * 4, amax = L - 1 - d;
+                v.x = (a + 0 <= amax && v.x <= T) ? v.x : TG_INFU;
+                v.y = (a + 1 <= amax && v.y <= T) ? v.y : TG_INFU;
+                v.z = (a + 2 <= amax && v.z <= T) ? v.z : TG_INFU;
+                v.w = (a + 3 <= amax && v.w <= T) ? v.w : TG_INFU;
+                nAdm += (v.x < TG_INFU) + (v.y < TG_INFU) + (v.z < TG_INFU) + (v.w < TG_INFU);
             }
+            reinterpret_cast<uint4*>(Cs + sm.baseK[kc])[w] = v;
         }
         __syncthreads();
         for (int w = tid; w < Ke * nb4; w += TG_NT) {   // widest admissible diagonal per 4 starts
@@ -260,6 +266,7 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         sm.useGlobalC = acc > uint32_t(total - nWp * perMask) ? 1 : 0;
         const int csUsed = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
         sm.nWarps = nWp;
+        sm.csUsed4 = int(acc >> 2);
         sm.wbufOff = csUsed;
         sm.wbufWords = min(2 * perMask, (total - csUsed) / nWp) & ~3;
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
