@@ -337,6 +337,10 @@ tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cud
         for (int r = 0; r < nr && r < 8; ++r)
             fprintf(stderr, "[tg]  round %3d scheduler cycles: fold %lld plan %lld teams %lld\n", r, hc.schedCyc[r][1] - hc.schedCyc[r][0],
                     hc.schedCyc[r][2] - hc.schedCyc[r][1], hc.schedCyc[r][3] - hc.schedCyc[r][2]);
+        for (int r = 0; r < nr && r < 8; ++r)
+            fprintf(stderr, "[tg]  round %3d fold/plan detail: stage-prev %lld copy-in %lld fold %lld plan %lld copy-out %lld\n", r,
+                    hc.dbgCyc[r][0] - hc.schedCyc[r][0], hc.dbgCyc[r][1] - hc.dbgCyc[r][0], hc.dbgCyc[r][2] - hc.dbgCyc[r][1],
+                    hc.dbgCyc[r][3] - hc.dbgCyc[r][2], hc.schedCyc[r][1] - hc.dbgCyc[r][3]);
         for (int r = 0; r < nr && r < 8; ++r) {
             if (hc.roundItems[r] > 16 || hc.roundItems[r] >= W.ctx.nSlots) continue;
             fprintf(stderr, "[tg]  round %3d items (candidate: us)", r);

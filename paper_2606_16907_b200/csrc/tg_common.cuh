@@ -19,6 +19,8 @@
 #define TG_IT_TRACK 1
 #define TG_IT_SPEC 2
 #define TG_IT_ALLISL 4
+#define TG_CAND_WIN 2048          // candidates staged per instance for the scheduler's bound tests
+#define TG_SCHED_SMEM_INST 8      // up to this many instances the scheduler works on shared-memory copies of their search state
 #define TG_SPEC_ALL_MAX_INST 4   // up to this many instances every probe of a search's last round back-tracks
 #define TG_EDONE 0x40000000   // flag in eIdx: every candidate between the previous evaluated point and this one is resolved
 #define TG_KEY_NONE 0xffffffffffffffffull
@@ -65,6 +67,8 @@ struct TgInstDev {
     uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
     uint32_t maxKey;                  // largest finite reduced cost of any depth (bounds the radix sort's passes)
     long long prepCyc[6];             // TG_DEBUG: clock stamps of the prepare kernel's stages
+    const uint32_t* candWin;          // scheduler, few instances: cand[candWinLo .. candWinLo + candWinN) staged in shared memory
+    int32_t candWinLo, candWinN;
     int32_t planKind;                 // wide scheduling: item kind returned by this round's planning
     int32_t xbound;                   // NEXT-3(b): transfers are admissible only if x <= T (tg_instance_set_transfer_bound)
     uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major
@@ -111,6 +115,7 @@ struct TgCtrl {
     int32_t roundItems[256];
     unsigned long long itemNs[8][16];   // team mode: finish time of the first items of the first rounds
     int32_t itemTidx[8][16];
+    long long dbgCyc[8][8];
     long long schedCyc[8][4];           // scheduler of the first rounds: clock at entry, after fold, after plan, at exit
 };
 

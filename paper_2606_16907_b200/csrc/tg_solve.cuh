@@ -794,10 +794,14 @@ struct TgInc {
     int64_t incIter, m1;
     int incIdx;
     const uint32_t* cand;
+    const uint32_t* win;   // cand[winLo .. winLo + winN) in shared memory (or null)
+    int winLo, winN;
 };
 __device__ __forceinline__ bool tgBeats(const TgInc& B, int64_t lbF, int c) {
     if (B.incIdx < 0) return true;
-    const int64_t lb = lbF + B.m1 * int64_t(__ldg(B.cand + c));   // cand is read-only during the solve
+    const unsigned off = unsigned(c - B.winLo);
+    const uint32_t Tc = off < unsigned(B.winN) ? B.win[off] : __ldg(B.cand + c);   // cand is read-only during the solve
+    const int64_t lb = lbF + B.m1 * int64_t(Tc);
     return lb < B.incIter || (lb == B.incIter && c < B.incIdx);
 }
 
@@ -947,7 +951,7 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
         int sLo[16], sHi[16], ns = 0;
         long long total = 0;
         bool truncated = false;
-        const TgInc B = {I.incIter, int64_t(I.m - 1), I.incIdx, I.cand};
+        const TgInc B = {I.incIter, int64_t(I.m - 1), I.incIdx, I.cand, I.candWin, I.candWinLo, I.candWin ? I.candWinN : 0};
         const int nEval = I.nEval;
         int32_t* const eIdx = I.eIdx;
         const uint32_t* const eF = I.eF;
@@ -1056,19 +1060,78 @@ __device__ void tgFoldPlanAll(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn
         P.keyS = keyS; P.tidxS = tidxS; P.candS = candS; P.flagS = flagS; P.nStage = nStage;
         __syncthreads();
     }
+    if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->dbgCyc[round][0] = clock64();
     // W is bounded by the item list shared among the instances still running (count of the previous round: an upper bound)
     const int nActive = round > 0 ? max(1, __ldcg(&ctrl->nActive)) : ctx.nInst;
     const int capAll = max(1, min(ctx.wishMax, TG_MAX_ITEMS / nActive));
     const bool mine = wide ? (tid & 31) == 0 : true;
     const int first = wide ? int(blockIdx.x) * TG_NW + (tid >> 5) : tid;
     const int stride = wide ? int(gridDim.x) * TG_NW : TG_NT;
+    // A handful of instances (the latency-bound case): their search state -- the TgInstDev record and the evaluated
+    // list -- is copied to shared memory by the whole CTA, folded and planned there by one thread each, and copied
+    // back.  In global memory every field access of that single thread is a dependent L1/L2 access, and a store
+    // invalidates the line the next load wants (the merge of the evaluated list paid one L2 trip per entry).
+    constexpr int INST_W = int(sizeof(TgInstDev) / 4);
+    const size_t dynWords = size_t(ctx.csWords) + size_t(ctx.nActiveWarps) * ctx.wbufWords;
+    const bool local = !wide && ctx.nInst <= TG_SCHED_SMEM_INST &&
+                       ((5 * size_t(P.nStage) + 3) & ~size_t(3)) + size_t(ctx.nInst) * (INST_W + 2 * TG_MAX_EVAL + TG_CAND_WIN) <= dynWords;
+    uint32_t* sInst = dyn + ((5 * size_t(P.nStage) + 3) & ~size_t(3));   // behind the staged previous items (17 bytes each)
+    uint32_t* sEval = sInst + size_t(ctx.nInst) * INST_W;                 // [nInst][2][TG_MAX_EVAL]
+    if (local) {
+        for (int i = 0; i < ctx.nInst; ++i) {
+            const uint32_t* src = reinterpret_cast<const uint32_t*>(ctx.inst + i);
+            for (int w = tid; w < INST_W; w += TG_NT) sInst[size_t(i) * INST_W + w] = src[w];
+        }
+        __syncthreads();
+        for (int i = 0; i < ctx.nInst; ++i) {
+            const TgInstDev& S = *reinterpret_cast<const TgInstDev*>(sInst + size_t(i) * INST_W);
+            const int ne = min(max(S.nEval, 0), TG_MAX_EVAL);
+            for (int w = tid; w < ne; w += TG_NT) {
+                sEval[(size_t(i) * 2 + 0) * TG_MAX_EVAL + w] = uint32_t(S.eIdx[w]);
+                sEval[(size_t(i) * 2 + 1) * TG_MAX_EVAL + w] = S.eF[w];
+            }
+            // the candidates the bound tests will look at start at the lowest feasible one (first evaluated point)
+            const int lo = ne > 0 ? int(uint32_t(S.eIdx[0]) & ~uint32_t(TG_EDONE)) : max(S.lbIdx, 0);
+            const int nw = max(0, min(TG_CAND_WIN, S.ncand - lo));
+            uint32_t* sCand = sEval + size_t(ctx.nInst) * 2 * TG_MAX_EVAL + size_t(i) * TG_CAND_WIN;
+            for (int w = tid; w < nw; w += TG_NT) sCand[w] = S.cand[lo + w];
+            if (tid == 0) {
+                TgInstDev& Sw = *reinterpret_cast<TgInstDev*>(sInst + size_t(i) * INST_W);
+                Sw.candWin = sCand; Sw.candWinLo = lo; Sw.candWinN = nw;
+            }
+        }
+        __syncthreads();
+    }
+    if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->dbgCyc[round][1] = clock64();
     if (mine)
         for (int i = first; i < ctx.nInst; i += stride) {
-            TgInstDev& I = ctx.inst[i];
+            TgInstDev& I = local ? *reinterpret_cast<TgInstDev*>(sInst + size_t(i) * INST_W) : ctx.inst[i];
+            int32_t* gIdx = I.eIdx;
+            uint32_t* gF = I.eF;
+            if (local) {
+                I.eIdx = reinterpret_cast<int32_t*>(sEval + (size_t(i) * 2 + 0) * TG_MAX_EVAL);
+                I.eF = sEval + (size_t(i) * 2 + 1) * TG_MAX_EVAL;
+            }
             if (I.itemCnt > 0) tgFoldInstance(ctx, I, P, full);
+            if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->dbgCyc[round][2] = clock64();
             if (I.phase != TG_PH_DONE) I.planKind = tgPlanInstance(ctx, I, i, full ? capAll : min(capAll, tgWish(ctx, I.K)), full);   // a full sweep has no speculation
+            if (local) { I.eIdx = gIdx; I.eF = gF; I.candWin = nullptr; I.candWinN = 0; }
+            if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->dbgCyc[round][3] = clock64();
         }
     __syncthreads();
+    if (local) {
+        for (int i = 0; i < ctx.nInst; ++i) {
+            const TgInstDev& S = *reinterpret_cast<const TgInstDev*>(sInst + size_t(i) * INST_W);
+            const int ne = min(max(S.nEval, 0), TG_MAX_EVAL);
+            for (int w = tid; w < ne; w += TG_NT) {
+                S.eIdx[w] = int32_t(sEval[(size_t(i) * 2 + 0) * TG_MAX_EVAL + w]);
+                S.eF[w] = sEval[(size_t(i) * 2 + 1) * TG_MAX_EVAL + w];
+            }
+            uint32_t* dst = reinterpret_cast<uint32_t*>(ctx.inst + i);
+            for (int w = tid; w < INST_W; w += TG_NT) dst[w] = sInst[size_t(i) * INST_W + w];
+        }
+        __syncthreads();
+    }
     if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->schedCyc[round][1] = clock64();
 }
 
