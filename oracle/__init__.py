@@ -188,5 +188,19 @@ def bruteforce_variant(inst) -> Result:
     return _conv(r)
 
 
+def prune_depth(inst, mode: int = 0, threshold: int = 0):
+    """tg_prune on an instance with a footprint table (3-way dominance).  Returns (pruned copy, counts[4])."""
+    out = inst.copy()
+    t = np.ascontiguousarray(out.time_us, dtype=np.int32)
+    mm = np.ascontiguousarray(out.mem_mb, dtype=np.int32)
+    am = np.ascontiguousarray(out.actmem_mb, dtype=np.int32)
+    cap = np.ascontiguousarray(out.island_cap_mb, dtype=np.int32)
+    counts = np.zeros(4, dtype=np.int64)
+    lib().orc_prune_depth(C.c_int(out.L), C.c_int(out.K), C.c_int(out.P), _p32(t), _p32(mm), _p32(am), _p32(cap),
+                          C.c_int(mode), C.c_int64(threshold), counts.ctypes.data_as(_I64P))
+    out.time_us = t
+    return out, counts
+
+
 def hw_threads() -> int:
     return lib().orc_hw_threads()

@@ -27,6 +27,11 @@
 // on thousands of tiny instances; actmem = 0 reproduces the core oracle bit for bit; raising actmem
 // never improves the optimum; a plan re-scored from the raw tables with the depth rule reproduces
 // (sum, T, iter).
+//
+// orc_prune_depth (tg_prune with a footprint: 3-way dominance) is pinned in tests/test_oracle_prune_depth.py:
+// a set-based restatement of R1/R2 in Python, the literal enumeration (orc_depth_bruteforce) giving the same
+// optimum before and after pruning, zero footprint == the core orc_prune, survivors form an antichain, a
+// hand-worked cell, idempotence.
 
 #include <algorithm>
 #include <cstdint>
@@ -295,6 +300,66 @@ int orc_variant_bruteforce(int L, int K, int P, int m, const int32_t* time_us, c
 int orc_depth_bruteforce(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
                          const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
     return orc_variant_bruteforce(L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, 0, out);
+}
+
+// tg_prune oracle for instances WITH a footprint table (SURVEY.md §8(f) NEXT-1 "R2 dominance becomes 3-way";
+// DESIGN.md reading N1-prune).  Rules, on the entry e = (slice, island k, plan p):
+//   R1  never feasible: the shallowest depth is q = 1, so  mem + 1*actmem > cap  kills;
+//   R2  dominated inside its (slice, island) cell on (time, mem, actmem): q kills p iff  tq <= tp, mq <= mp,
+//       aq <= ap  with one of them strict, or all three equal and q < p.  Then mq + d*aq <= mp + d*ap at every
+//       depth d >= 1, so q is feasible wherever p is and no slower (PAPER.md:43, :360, :258(i));
+//   R3 (mode 1, theta per mille) and R4 (mode 2, cap in us) look at the times only and are the core rules.
+// R2 is decided on the cell as R1 left it (dominance is a strict partial order plus the index tie-break, so
+// every dominated entry has a surviving dominator).  time_us modified in place, counts[4] as in orc_prune.
+int orc_prune_depth(int L, int K, int P, int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                    const int32_t* cap_mb, int mode, int64_t threshold, int64_t* counts) {
+    const int NS = L * (L + 1) / 2;
+    counts[0] = counts[1] = counts[2] = counts[3] = 0;
+    auto E = [&](int s, int k, int p) { return (size_t(s) * K + k) * P + p; };
+    for (int s = 0; s < NS; ++s) for (int k = 0; k < K; ++k) for (int p = 0; p < P; ++p) {
+        const size_t e = E(s, k, p);
+        if (time_us[e] != INVALID && int64_t(mem_mb[e]) + int64_t(actmem_mb[e]) > int64_t(cap_mb[k])) { time_us[e] = INVALID; ++counts[0]; }
+    }
+    for (int s = 0; s < NS; ++s) for (int k = 0; k < K; ++k) {
+        std::vector<char> dead(P, 0);
+        for (int p = 0; p < P; ++p) {
+            const size_t ep = E(s, k, p);
+            if (time_us[ep] == INVALID) continue;
+            for (int q = 0; q < P; ++q) {
+                const size_t eq = E(s, k, q);
+                if (q == p || time_us[eq] == INVALID) continue;
+                const bool le = time_us[eq] <= time_us[ep] && mem_mb[eq] <= mem_mb[ep] && actmem_mb[eq] <= actmem_mb[ep];
+                const bool eqv = time_us[eq] == time_us[ep] && mem_mb[eq] == mem_mb[ep] && actmem_mb[eq] == actmem_mb[ep];
+                if (le && (!eqv || q < p)) dead[p] = 1;
+            }
+        }
+        for (int p = 0; p < P; ++p) if (dead[p]) { time_us[E(s, k, p)] = INVALID; ++counts[1]; }
+    }
+    if (mode == 1) {
+        // R3: island capacity share from the profiled atom throughput, slice demand = its length
+        std::vector<int64_t> C(K, 0); int64_t Ct = 0;
+        for (int k = 0; k < K; ++k) {
+            int64_t tau = 0; bool ok = true;
+            for (int l = 0; l < L && ok; ++l) {
+                int64_t best = INF;
+                for (int p = 0; p < P; ++p) { const int32_t t = time_us[E(sidx(L, l, l + 1), k, p)]; if (t != INVALID) best = std::min<int64_t>(best, t); }
+                if (best >= INF) ok = false; else tau += best;
+            }
+            if (ok) { C[k] = (int64_t(1) << 32) / std::max<int64_t>(tau, 1); Ct += C[k]; }
+        }
+        for (int a = 0; a < L; ++a) for (int b = a + 1; b <= L; ++b) for (int k = 0; k < K; ++k) {
+            if (C[k] == 0) continue;
+            const int64_t len = b - a;
+            const bool over = len * Ct * 1000 > threshold * C[k] * L;
+            const bool under = len * Ct * threshold < int64_t(1000) * C[k] * L;
+            if (!(over || under)) continue;
+            for (int p = 0; p < P; ++p) { const size_t e = E(sidx(L, a, b), k, p); if (time_us[e] != INVALID) { time_us[e] = INVALID; ++counts[2]; } }
+        }
+    }
+    if (mode == 2)
+        for (int s = 0; s < NS; ++s) for (int k = 0; k < K; ++k) for (int p = 0; p < P; ++p)
+            if (time_us[E(s, k, p)] != INVALID && int64_t(time_us[E(s, k, p)]) > threshold) { time_us[E(s, k, p)] = INVALID; ++counts[3]; }
+    return 0;
 }
 
 }  // extern "C"
