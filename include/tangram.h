@@ -102,7 +102,7 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
  * feasible iff mem_mb + q * actmem_mb <= cap_mb[k]; the stage cost becomes c_q = min over the plans feasible
  * at depth q, and the candidate thresholds are the distinct finite c_q of all depths.  Everything else
  * (sum, T, iter, tie-breaks) is unchanged; stage_plan[i] is the lowest p attaining c_q of that stage.
- * tg_reduce keeps reporting depth 1; tg_prune returns TG_ERR_RANGE for such instances.  Synchronises the
+ * tg_reduce keeps reporting depth 1; tg_prune then uses the three-axis rules stated there.  Synchronises the
  * legacy default stream. */
 tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb);
 
@@ -175,6 +175,10 @@ typedef enum {
  * Marks entries of the instance's time table dead (TG_INVALID), in place and monotone (never revives
  * an entry).  EXACT and BOTTLENECK are idempotent; IMBALANCE re-estimates the islands' atom profile
  * from the live table on every call, so a second call may kill more.
+ * On an instance with a footprint table (tg_instance_set_actmem) R1 is
+ * "infeasible at the shallowest depth", mem_mb + actmem_mb > cap_mb[k], and R2 dominance is on the three
+ * axes (time, mem_mb, actmem_mb): q kills p iff q is no larger on every axis and differs, or equals p with
+ * q < p; such a q is feasible at every depth where p is and no slower.  R3 and R4 read the times only.
  *   counts_out  HOST int64[4]: entries newly killed by R1..R4.  The call synchronises `cuda_stream`. */
 tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4],
                    void* cuda_stream);

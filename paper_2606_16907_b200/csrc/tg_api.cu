@@ -738,7 +738,6 @@ tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int
     if (mode == TG_PRUNE_IMBALANCE && (threshold < 1000 || threshold > 16384))
         return fail(TG_ERR_RANGE, "theta must be in [1000, 16384] permille");
     if (mode == TG_PRUNE_BOTTLENECK && threshold < 0) return fail(TG_ERR_RANGE, "bottleneck cap must be >= 0");
-    if (inst->actmem) return fail(TG_ERR_RANGE, "tg_prune is not defined for instances with an actmem table (dominance would need the third axis)");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const int cells = inst->NS * inst->K;
     char* ws = nullptr;
@@ -746,7 +745,7 @@ tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int
     unsigned long long* dCounts = reinterpret_cast<unsigned long long*>(ws);
     long long* dCap = reinterpret_cast<long long*>(ws + 32);
     TG_CUDA(cudaMemsetAsync(ws, 0, 32, st));
-    tgPruneCellKernel<<<(cells + 255) / 256, 256, 0, st>>>(inst->time_us, inst->mem_mb, inst->cap_mb, cells, inst->K,
+    tgPruneCellKernel<<<(cells + 255) / 256, 256, 0, st>>>(inst->time_us, inst->mem_mb, inst->actmem, inst->cap_mb, cells, inst->K,
                                                           inst->P, int(mode), threshold, dCounts);
     if (mode == TG_PRUNE_IMBALANCE) {
         tgPruneTauKernel<<<1, 256, 0, st>>>(inst->time_us, inst->L, inst->K, inst->P, dCap);

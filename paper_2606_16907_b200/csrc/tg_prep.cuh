@@ -445,6 +445,7 @@ __global__ void tgExportKernel(const TgInstDev* __restrict__ insts, int32_t* __r
 // ---------------------------------------------------------------------------------------------
 // R1 infeasible, R2 dominated inside one (slice, island) cell, optional R4 bottleneck cap.
 __global__ void __launch_bounds__(256) tgPruneCellKernel(int32_t* __restrict__ time_us, const int32_t* __restrict__ mem_mb,
+                                                         const int32_t* __restrict__ actmem_mb,   // nullptr: no footprint
                                                          const int32_t* __restrict__ cap, int nCells, int K, int P,
                                                          int mode, int64_t threshold, unsigned long long* counts) {
     const int cell = blockIdx.x * 256 + threadIdx.x;
@@ -452,20 +453,25 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(int32_t* __restrict__ t
     if (cell < nCells) {
         int32_t* t = time_us + size_t(cell) * P;
         const int32_t* mm = mem_mb + size_t(cell) * P;
+        const int32_t* am = actmem_mb ? actmem_mb + size_t(cell) * P : nullptr;
         const int32_t capk = cap[cell % K];
+        // R1: with a footprint the shallowest depth (one microbatch in flight) decides "never feasible"
         for (int p = 0; p < P; ++p)
-            if (t[p] != TG_INVALID && mm[p] > capk) { t[p] = TG_INVALID; ++c1; }
+            if (t[p] != TG_INVALID && int64_t(mm[p]) + (am ? am[p] : 0) > capk) { t[p] = TG_INVALID; ++c1; }
+        // R2: q kills p iff q <= p on every axis (time, memory and, if present, footprint) and differs, or ties with q < p
         uint32_t dead[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         for (int p = 0; p < P; ++p) {
             const int32_t tp = t[p];
             if (tp == TG_INVALID) continue;
-            const int32_t mp = mm[p];
+            const int32_t mp = mm[p], ap = am ? am[p] : 0;
             bool dd = false;
             for (int q = 0; q < P && !dd; ++q) {
                 const int32_t tq = t[q];
                 if (q == p || tq == TG_INVALID) continue;
-                const int32_t mq = mm[q];
-                dd = (tq < tp && mq <= mp) || (tq <= tp && mq < mp) || (tq == tp && mq == mp && q < p);
+                const int32_t mq = mm[q], aq = am ? am[q] : 0;
+                const bool le = tq <= tp && mq <= mp && aq <= ap;
+                const bool eq = tq == tp && mq == mp && aq == ap;
+                dd = le && (!eq || q < p);
             }
             if (dd) dead[p >> 5] |= 1u << (p & 31);
         }

@@ -66,9 +66,6 @@ def test_zero_footprint_and_removal(tg):
 def test_errors_with_actmem(tg):
     inst = gen.with_actmem(gen.config1(), 0)
     h = tg.instance_from_inputs(inst)
-    with pytest.raises(tg.TangramError) as e:
-        tg.tg_prune(h, 0, 0)
-    assert e.value.status == 3
     bad = inst.actmem_mb.copy(); bad[2, 1, 0] = -1
     with pytest.raises(tg.TangramError) as e:
         tg.tg_instance_set_actmem(h, bad)

@@ -47,6 +47,42 @@ def test_prune_table_and_counts(tg, mode, thr):
         h.destroy()
 
 
+def cases_with_footprint():
+    out = [gen.with_actmem(gen.random_small(s + 8500, Lmax=9, Kmax=6, Pmax=7, style=STYLES[s % 5]), s) for s in range(60)]
+    out += [gen.with_actmem(gen.random_small(s + 8600, Lmax=6, Kmax=3, Pmax=40, style=STYLES[s % 5]), s) for s in range(5)]
+    out += [gen.with_actmem(gen.config1(0, 10), 1, 0, 300), gen.with_actmem(gen.config2(), 4, 0, 2000),
+            gen.with_actmem(gen.config3(0, L=21, K=5), 1, 500, 6000), gen.with_actmem(gen.config4(0, L=18, K=6), 2, 2000, 20000)]
+    return out
+
+
+@pytest.mark.parametrize("mode,thr", [(0, 0), (1, 3000), (1, 1000), (2, 700), (2, 1 << 25)])
+def test_prune_with_footprint_table_and_counts(tg, mode, thr):
+    """R1 at depth 1 and 3-way R2 (oracle.prune_depth); the pruned instance solves like the
+    depth oracle on the oracle's pruned tables; removing the footprint afterwards leaves the core rules."""
+    killed3 = 0
+    for inst in cases_with_footprint():
+        h = tg.instance_from_inputs(inst)
+        counts = tg.tg_prune(h, mode, thr)
+        t = tg.tg_instance_read_time(h)
+        pr, ocounts = oracle.prune_depth(inst, mode, thr)
+        assert counts.tolist() == ocounts.tolist(), (inst.name, mode, thr)
+        assert np.array_equal(t, pr.time_us.reshape(t.shape)), (inst.name, mode, thr)
+        killed3 += int(ocounts[0] + ocounts[1])
+        same(oracle.solve_depth(pr), tg.tg_solve_batch([h])[0], inst.name)
+        again = tg.tg_prune(h, mode, thr)
+        pr2, ocounts2 = oracle.prune_depth(pr, mode, thr)
+        assert again.tolist() == ocounts2.tolist()
+        assert np.array_equal(tg.tg_instance_read_time(h), pr2.time_us.reshape(t.shape))
+        tg.tg_instance_set_actmem(h, None)                      # footprint removed: the two-axis rules apply again
+        core = pr2.copy(); core.actmem_mb = None
+        after = tg.tg_prune(h, 0, 0)
+        pr3, ocounts3 = oracle.prune(core, 0, 0)
+        assert after.tolist() == ocounts3.tolist()
+        assert np.array_equal(tg.tg_instance_read_time(h), pr3.time_us.reshape(t.shape))
+        h.destroy()
+    assert killed3 > 100
+
+
 def test_prune_errors(tg):
     h = tg.instance_from_inputs(gen.config1())
     for mode, thr in [(3, 0), (1, 999), (1, 16385), (2, -1)]:
