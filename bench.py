@@ -37,8 +37,10 @@ UNIT = "plans/s"
 NCU_TRAFFIC_BYTES = {("cfg4", False): 0.171e9}
 
 
-def make_workload(name: str, rank: int, n_inst: int):
-    """Seeded synthetic instances (DESIGN.md input recipe).  Rank r takes its own seeds (weak scaling)."""
+def make_workload(name: str, rank: int, n_inst: int, n_make: int = None):
+    """Seeded synthetic instances (DESIGN.md input recipe).  Rank r takes its own seeds (weak scaling).
+    n_make: build only the first n_make instances of the workload (the CPU arm's bounded sample); the
+    description stays that of the whole workload."""
     import tg_inputs as gen
     if name == "cfg4":
         return [gen.config4(rank)], "cfg4 MoE-like L=64 K=16 P=8 m=64 (BASELINE.json configs[3]), 1 instance/GPU"
@@ -60,7 +62,7 @@ def make_workload(name: str, rank: int, n_inst: int):
             "cfg3 70B-like L=80 K=12 P=8 m=32 + transfers as pipeline slots (NEXT-3(b)), 1 instance/GPU"
     if name == "cfg5":
         from paper_2606_16907_b200.shard import weak_seeds
-        return [gen.config5_one(sd) for sd in weak_seeds(n_inst, rank)], \
+        return [gen.config5_one(sd) for sd in weak_seeds(n_inst, rank)[:n_make]], \
             f"cfg5 throughput batch: {n_inst} instances L=48 K=10 P=4 m in {{4..64}} (configs[4]) per GPU"
     raise SystemExit(f"unknown workload {name}")
 
@@ -157,22 +159,40 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def oracle_sample(insts, workload: str, threads: int):
-    """Bounded sample of the workload on the CPU oracle, as it stands: `threads` concurrent single
-    DP(T) calls (oracle.dp_at releases the GIL inside the C++ library).  Returns (plans, seconds, text)."""
+def oracle_sample(insts, workload: str, threads: int, seconds: float = 10.0):
+    """Bounded sample of the workload on the CPU oracle, as it stands: `threads` host threads run single DP(T)
+    calls (oracle.dp_at releases the GIL inside the C++ library) over thresholds spread over the upper half of the
+    candidate lists (feasible region) of the first instances, until about `seconds` of wall time have passed
+    (every thread finishes the DP it is in; at least one DP per thread).  Returns (plans, seconds, text)."""
     import oracle
-    inst = insts[0]
-    _, _, _, cand = oracle.reduce(inst)
-    # thresholds spread over the upper half of the candidate list (feasible region)
-    picks = [int(cand[len(cand) // 2 + (i * (len(cand) // 2 - 1)) // max(1, threads - 1)]) for i in range(threads)]
+    sample_insts = insts[:min(len(insts), 4)]
+    work = []                                        # (instance, T) in a fixed order: thread i takes i, i+threads, ...
+    for inst in sample_insts:
+        _, _, _, cand = oracle.reduce(inst)
+        half = len(cand) // 2
+        work.append([(inst, int(cand[half + (i * (half - 1)) // max(1, threads - 1)])) for i in range(threads)])
+    done = [0.0] * threads
     t0 = time.perf_counter()
-    ths = [threading.Thread(target=oracle.dp_at, args=(inst, T, False)) for T in picks]
+
+    def worker(i):
+        r = 0
+        while True:
+            inst, T = work[r % len(work)][(i + r // len(work)) % threads]
+            oracle.dp_at(inst, T, False)
+            done[i] += dense_plans(inst)
+            r += 1
+            if time.perf_counter() - t0 >= seconds:
+                return
+
+    ths = [threading.Thread(target=worker, args=(i,)) for i in range(threads)]
     for t in ths:
         t.start()
     for t in ths:
         t.join()
     dt = time.perf_counter() - t0
-    return dense_plans(inst) * len(picks), dt, f"{len(picks)} single-threshold DPs (oracle.dp_at) of {inst.name}, one per thread"
+    n_dp = sum(round(d / dense_plans(sample_insts[0])) for d in done)
+    return sum(done), dt, (f"{n_dp} single-threshold DPs (oracle.dp_at) over {len(sample_insts)} instance(s) from {sample_insts[0].name}, "
+                           f"{threads} threads, {dt:.1f} s of wall time")
 
 
 def run_reference(args):
@@ -181,14 +201,15 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
-    insts, desc = make_workload(args.workload, 0, min(args.n_inst, 4))
+    insts, desc = make_workload(args.workload, 0, args.n_inst, 4)
     cores = max(1, min(oracle.hw_threads(), args.cpu_threads))
+    per_step = max(2.0, min(10.0, 100.0 / max(1, args.steps)))        # the whole run stays within a few minutes
     for _ in range(min(args.warmup, 1)):
-        oracle_sample(insts, args.workload, cores)
+        oracle_sample(insts, args.workload, cores, 1.0)
     plans = secs = 0.0
     sample = ""
     for _ in range(args.steps):
-        p, dt, sample = oracle_sample(insts, args.workload, cores)
+        p, dt, sample = oracle_sample(insts, args.workload, cores, per_step)
         plans += p
         secs += dt
     v = plans / secs
