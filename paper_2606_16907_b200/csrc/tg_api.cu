@@ -284,8 +284,22 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.rankOf = D->rankOf;
     c.specOut = reinterpret_cast<tg_result*>(W.base + oSpec);
 
-    const dim3 g((maxCells + 255) / 256, n);
-    tgLoadKernel<<<g, 256, 0, st>>>(W.inst);
+    // loader grid: 256 * U cells per CTA, U = TG_LOAD_U when that still gives every SM two CTAs, else 1; the
+    // batched-load path is compiled for P = 4 and P = 8 (picked from the first instance; instances of another
+    // shape take the kernel's cell-at-a-time path)
+    const int ctasU = (maxCells + 256 * TG_LOAD_U - 1) / (256 * TG_LOAD_U);
+    const bool wide = int64_t(ctasU) * n >= 2 * D->numSMs;
+    const dim3 g(wide ? ctasU : (maxCells + 255) / 256, n);
+    const int P0 = instances[0]->P;
+    if (wide) {
+        if (P0 == 4) tgLoadKernel<1, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);
+        else if (P0 == 8) tgLoadKernel<2, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);
+        else tgLoadKernel<0, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);
+    } else {
+        if (P0 == 4) tgLoadKernel<1, 1><<<g, 256, 0, st>>>(W.inst);
+        else if (P0 == 8) tgLoadKernel<2, 1><<<g, 256, 0, st>>>(W.inst);
+        else tgLoadKernel<0, 1><<<g, 256, 0, st>>>(W.inst);
+    }
     tgPrepareKernel<<<n, TG_PREP_NT, TG_SORT_SMEM_MAX * 4, st>>>(W.inst);
     TG_CUDA(cudaGetLastError());
     return TG_OK;

@@ -117,7 +117,7 @@ __global__ void tgValidateNonNegKernel(const int32_t* __restrict__ v, size_t n, 
 }
 
 // ---------------------------------------------------------------------------------------------
-// Step 1: cost-table loader.  One thread per (slice, island) cell, reduction over the P plans.
+// Step 1: cost-table loader.  One thread per (slice, island) cell at a time, reduction over the P plans.
 //   c = min_p { time : time != INVALID, mem <= cap_k }, ties -> lowest p
 // Output goes straight into the diagonal-major layout the DP stages from, plus a flat copy for
 // the candidate sort.  HBM-bound stream: 8*P bytes read per cell.
@@ -145,55 +145,118 @@ __device__ __forceinline__ void tgReduceCell(const int32_t* __restrict__ tp, con
     }
 }
 
+#define TG_LOAD_U 4   // cells per thread of the loader when the batch fills the GPU (1 otherwise)
+
+// outputs of one cell at depth q: the diagonal-major cost, its plan, the sort key
+__device__ __forceinline__ void tgLoadEmit(TgInstDev& I, int L, int K, int nCells, int cell, int a, int b, int k, int q,
+                                           uint32_t bq, int bp, uint32_t& prev, uint32_t& myMax) {
+    const int d = b - a;
+    uint32_t* row = I.cd + (size_t(q - 1) * K + k) * I.triG + tgGOff(L, d);
+    row[a] = bq;
+    if (b == L) {   // last element of the row: write the INF padding up to a multiple of 4
+        const int rl = (L - d + 1 + 3) & ~3;
+        for (int p = a + 1; p < rl; ++p) row[p] = TG_INFU;
+    }
+    I.argp[size_t(q - 1) * nCells + cell] = uint8_t(bp);
+    // candidate thresholds: every distinct finite cost of any depth (deeper costs repeat the shallower one
+    // until a plan stops fitting, so equal neighbours are dropped here already)
+    I.sortbuf[size_t(q - 1) * nCells + cell] = (q == I.nDepth || bq != prev) ? bq : TG_INFU;
+    prev = bq;
+    if (bq < TG_INFU) myMax = max(myMax, bq);
+}
+
+// One CTA per 256 * U consecutive cells of one instance; thread t takes cells t, t + 256, ... of the chunk.
+// PV > 0: instances with P = 4 * PV plans and no footprint table issue the 2 * PV * U 16-byte loads of their
+// cells first and reduce from registers (the stream is bound by the bytes in flight, not by the arithmetic); any
+// other instance of the batch takes the cell-at-a-time path.  The slice index is inverted once per thread
+// (tgSliceAB) and advanced incrementally: 256 cells further on are 256 / K slices and 256 % K islands further on.
+template <int PV, int U>
 __global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ insts) {
+    constexpr int PVA = PV > 0 ? PV : 1;
     TgInstDev& I = insts[blockIdx.y];
     const int L = I.L, K = I.K, P = I.P;
     const int nCells = I.NS * K;
+    const int cellFirst = int(blockIdx.x) * (256 * U) + int(threadIdx.x);
+    if (int(blockIdx.x) * (256 * U) >= nCells) return;
     __shared__ uint32_t sMin[TG_MAX_K];
+    __shared__ int32_t sCap[TG_MAX_K];
     __shared__ uint32_t sMax;
-    if (int(blockIdx.x) * 256 >= nCells) return;
-    if (threadIdx.x < TG_MAX_K) sMin[threadIdx.x] = TG_INFU;
+    const bool fast = PV > 0 && P == 4 * PV && I.actmem_mb == nullptr;
+    int4 tv[U][PVA], mv[U][PVA];
+    if (fast) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int cell = cellFirst + 256 * u;
+            if (cell < nCells) {
+                const int4* t4 = reinterpret_cast<const int4*>(I.time_us + size_t(cell) * P);
+                const int4* m4 = reinterpret_cast<const int4*>(I.mem_mb + size_t(cell) * P);
+#pragma unroll
+                for (int v = 0; v < PVA; ++v) { tv[u][v] = __ldg(t4 + v); mv[u][v] = __ldg(m4 + v); }
+            }
+        }
+    }
+    if (threadIdx.x < TG_MAX_K) {
+        sMin[threadIdx.x] = TG_INFU;
+        sCap[threadIdx.x] = int(threadIdx.x) < K ? __ldg(I.cap_mb + threadIdx.x) : 0;
+    }
     if (threadIdx.x == 0) sMax = 0;
     __syncthreads();
     uint32_t myMax = 0;
-    const int cell = blockIdx.x * 256 + threadIdx.x;
-    if (cell < nCells) {
-        const int s = cell / K, k = cell - s * K;
-        const int32_t capk = __ldg(I.cap_mb + k);
-        const size_t e = size_t(cell) * P;
-        int a, b;
-        tgSliceAB(L, s, a, b);
-        const int d = b - a;
-        const int rl = (L - d + 1 + 3) & ~3;
-        uint32_t best = TG_INFU, prev = TG_INFU;   // best ends up as the depth-1 cost (the least constrained)
-        for (int q = I.nDepth; q >= 1; --q) {
-            // depth q: the stage holds q microbatches in flight: feasible iff
-            // mem + q * actmem <= cap.  Without an actmem table there is the one static test.
-            uint32_t bq; int bp;
-            if (I.actmem_mb == nullptr) {
-                if ((P & 3) == 0) tgReduceCell<true>(I.time_us + e, I.mem_mb + e, P, capk, bq, bp);
-                else tgReduceCell<false>(I.time_us + e, I.mem_mb + e, P, capk, bq, bp);
-            } else {
-                bq = TG_INFU; bp = 0xff;
-                for (int p = 0; p < P; ++p) {
-                    const int32_t t = __ldg(I.time_us + e + p);
-                    const long long need = (long long)__ldg(I.mem_mb + e + p) + (long long)q * __ldg(I.actmem_mb + e + p);
-                    if (t != TG_INVALID && need <= (long long)capk && uint32_t(t) < bq) { bq = uint32_t(t); bp = p; }
+    if (cellFirst < nCells) {
+        const int s0 = cellFirst / K;
+        int k = cellFirst - s0 * K, a, b;
+        tgSliceAB(L, s0, a, b);
+        const int ds = 256 / K, dk = 256 - ds * K;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int cell = cellFirst + 256 * u;
+            if (cell < nCells) {
+                const int32_t capk = sCap[k];
+                uint32_t best, prev = TG_INFU;
+                if (fast) {
+                    uint32_t bq = TG_INFU; int bp = 0xff;
+#pragma unroll
+                    for (int v = 0; v < PVA; ++v) {
+                        const int32_t t4[4] = {tv[u][v].x, tv[u][v].y, tv[u][v].z, tv[u][v].w};
+                        const int32_t m4[4] = {mv[u][v].x, mv[u][v].y, mv[u][v].z, mv[u][v].w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (t4[e] != TG_INVALID && m4[e] <= capk && uint32_t(t4[e]) < bq) { bq = uint32_t(t4[e]); bp = 4 * v + e; }
+                    }
+                    tgLoadEmit(I, L, K, nCells, cell, a, b, k, 1, bq, bp, prev, myMax);
+                    best = bq;
+                } else {
+                    const size_t e = size_t(cell) * P;
+                    best = TG_INFU;
+                    for (int q = I.nDepth; q >= 1; --q) {
+                        // depth q: the stage holds q microbatches in flight: feasible iff
+                        // mem + q * actmem <= cap.  Without an actmem table there is the one static test.
+                        uint32_t bq; int bp;
+                        if (I.actmem_mb == nullptr) {
+                            if ((P & 3) == 0) tgReduceCell<true>(I.time_us + e, I.mem_mb + e, P, capk, bq, bp);
+                            else tgReduceCell<false>(I.time_us + e, I.mem_mb + e, P, capk, bq, bp);
+                        } else {
+                            bq = TG_INFU; bp = 0xff;
+                            for (int p = 0; p < P; ++p) {
+                                const int32_t t = __ldg(I.time_us + e + p);
+                                const long long need = (long long)__ldg(I.mem_mb + e + p) + (long long)q * __ldg(I.actmem_mb + e + p);
+                                if (t != TG_INVALID && need <= (long long)capk && uint32_t(t) < bq) { bq = uint32_t(t); bp = p; }
+                            }
+                        }
+                        tgLoadEmit(I, L, K, nCells, cell, a, b, k, q, bq, bp, prev, myMax);
+                        best = bq;   // ends up as the depth-1 cost (the least constrained)
+                    }
                 }
+                if (best < sMin[k]) atomicMin(&sMin[k], best);
+                // the thread's next cell: 256 cells = ds slices and dk islands further on
+                int adv = ds;
+                k += dk;
+                if (k >= K) { k -= K; ++adv; }
+                int pos = b - a - 1 + adv;
+                while (a < L && pos >= L - a) { pos -= L - a; ++a; }
+                b = a + 1 + pos;
             }
-            uint32_t* row = I.cd + (size_t(q - 1) * K + k) * I.triG + tgGOff(L, d);
-            row[a] = bq;
-            if (b == L)   // last element of the row: write the INF padding up to a multiple of 4
-                for (int p = a + 1; p < rl; ++p) row[p] = TG_INFU;
-            I.argp[size_t(q - 1) * nCells + cell] = uint8_t(bp);
-            // candidate thresholds: every distinct finite cost of any depth (deeper costs repeat the shallower one
-            // until a plan stops fitting, so equal neighbours are dropped here already)
-            I.sortbuf[size_t(q - 1) * nCells + cell] = (q == I.nDepth || bq != prev) ? bq : TG_INFU;
-            prev = bq;
-            best = bq;
-            if (bq < TG_INFU) myMax = max(myMax, bq);
         }
-        if (best < TG_INFU) atomicMin(&sMin[k], best);
     }
     myMax = __reduce_max_sync(0xffffffffu, myMax);
     if ((threadIdx.x & 31) == 0 && myMax) atomicMax(&sMax, myMax);

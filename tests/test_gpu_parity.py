@@ -220,3 +220,17 @@ def test_batch_sizes_around_the_scheduling_modes(tg, n):
     insts = [gen.random_small(s + 99_000 + 1000 * n, Lmax=8, Kmax=5, Pmax=3, style=STYLES[s % 5]) for s in range(n)]
     for inst, g in zip(insts, solve_all(tg, insts)):
         same(oracle.solve(inst), g, inst.name)
+
+
+def test_loader_paths_in_one_batch(tg):
+    """Cost-table loader: batches large enough for the many-cells-per-thread mode whose
+    instances take every path of the kernel -- batched loads for P = 4 and P = 8, the cell-at-a-time path for
+    another P, for a footprint table, and for an instance whose P differs from the first one's; chunk tails that
+    end inside a row of the slice triangle."""
+    p8 = [gen.config3(s, L=17 + s % 5, K=4 + s % 3) for s in range(150)]                      # P = 8 first
+    p4 = [gen.config5_one(s, L=14 + s % 7, K=5 + s % 2) for s in range(150)]                  # P = 4 first
+    odd = [gen.random_small(s + 12_000, Lmax=9, Kmax=6, Pmax=7, style=STYLES[s % 5]) for s in range(40)]
+    foot = [gen.with_actmem(gen.config3(s, L=15, K=4), s, 500, 6000) for s in range(10)]
+    for batch in (p8 + odd + p4[:20] + foot, p4 + odd + p8[:20] + foot, odd + p4 + p8):
+        for inst, g in zip(batch, solve_all(tg, batch)):
+            same(oracle.solve_depth(inst) if inst.actmem_mb is not None else oracle.solve(inst), g, inst.name)
