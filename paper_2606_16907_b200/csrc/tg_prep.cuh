@@ -171,7 +171,7 @@ __device__ __forceinline__ void tgLoadEmit(TgInstDev& I, int L, int K, int nCell
 // other instance of the batch takes the cell-at-a-time path.  The slice index is inverted once per thread
 // (tgSliceAB) and advanced incrementally: 256 cells further on are 256 / K slices and 256 % K islands further on.
 template <int PV, int U>
-__global__ void __launch_bounds__(256) tgLoadKernel(TgInstDev* __restrict__ insts) {
+__global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(TgInstDev* __restrict__ insts) {
     constexpr int PVA = PV > 0 ? PV : 1;
     TgInstDev& I = insts[blockIdx.y];
     const int L = I.L, K = I.K, P = I.P;
