@@ -33,8 +33,8 @@ UNIT = "plans/s"
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE tgSolveKernel launch from the committed ncu capture
-# (profiles/r1b_ncu_cfg4_solver.md); only valid for the default cfg4 windowed run
-NCU_TRAFFIC_BYTES = {("cfg4", False): 0.171e9}
+# (profiles/r1c_ncu_cfg4_solver.md); only valid for the default cfg4 windowed run
+NCU_TRAFFIC_BYTES = {("cfg4", False): 0.170e9}
 
 
 def make_workload(name: str, rank: int, n_inst: int, n_make: int = None):
@@ -320,7 +320,7 @@ def run_ours(args):
                 "gpu_launches": 3 * args.steps,   # tgLoadKernel + tgPrepareKernel + tgSolveKernel per tg_solve_batch
                 "roofline": {"bound": "hbm", "kernel": "tgSolveKernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                              "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.full_sweep)),
-                             "traffic_source": "profiles/r1b_ncu_cfg4_solver.md" if (args.workload, args.full_sweep) in NCU_TRAFFIC_BYTES else None,
+                             "traffic_source": "profiles/r1c_ncu_cfg4_solver.md" if (args.workload, args.full_sweep) in NCU_TRAFFIC_BYTES else None,
                              "peak_source": peak_src,
                              "kernel_ms": km, "step_ms": [round(x, 3) for x in step_ms],
                              "kernel_ms_steps": [round(x, 3) for x in kern_ms],
