@@ -33,8 +33,9 @@ UNIT = "plans/s"
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE tgSolveKernel launch from the committed ncu capture
-# (profiles/r1c_ncu_cfg4_solver.md); only valid for the default cfg4 windowed run
-NCU_TRAFFIC_BYTES = {("cfg4", False): 0.170e9}
+# (profiles/); only valid for the windowed run of the workload as captured (cfg5: 1024 instances)
+NCU_TRAFFIC_BYTES = {("cfg4", False): (0.170e9, "profiles/r1c_ncu_cfg4_solver.md"),
+                     ("cfg5", False): (1.341e9, "profiles/r1c_ncu_cfg5_solver.md")}
 
 
 def make_workload(name: str, rank: int, n_inst: int, n_make: int = None):
@@ -307,6 +308,9 @@ def run_ours(args):
         alg_bytes = states / args.steps * 8.0                          # live state: 4 B written + 4 B read
         achieved = alg_bytes / (km * 1e-3) / 1e9
         inst0 = insts[0]
+        ncu_traffic = NCU_TRAFFIC_BYTES.get((args.workload, args.full_sweep), (None, None))
+        if args.workload == "cfg5" and n != 1024:
+            ncu_traffic = (None, None)
         line = {"metric": METRIC, "value": plans_all / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms / args.steps,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
@@ -319,8 +323,7 @@ def run_ours(args):
                         "ms_per_step": e2e_s / e2e_steps * 1e3},
                 "gpu_launches": 3 * args.steps,   # tgLoadKernel + tgPrepareKernel + tgSolveKernel per tg_solve_batch
                 "roofline": {"bound": "hbm", "kernel": "tgSolveKernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                             "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.full_sweep)),
-                             "traffic_source": "profiles/r1c_ncu_cfg4_solver.md" if (args.workload, args.full_sweep) in NCU_TRAFFIC_BYTES else None,
+                             "frac": achieved / peak, "traffic": ncu_traffic[0], "traffic_source": ncu_traffic[1],
                              "peak_source": peak_src,
                              "kernel_ms": km, "step_ms": [round(x, 3) for x in step_ms],
                              "kernel_ms_steps": [round(x, 3) for x in kern_ms],
