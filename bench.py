@@ -255,7 +255,7 @@ def run_ours(args):
         tg.tg_solve_batch(handles, out=out, flags=flags, stats=st)
     barrier()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern_ms, plans, states, n_dp = [], 0, 0, 0
+    kern_ms, load_ms, plans, states, n_dp = [], [], 0, 0, 0
     cyc = [0] * 8
     relax = 0
     with clk:
@@ -266,6 +266,7 @@ def run_ours(args):
             ev[s][1].record(stream)
             torch.cuda.synchronize()
             kern_ms.append(tg.tg_last_solver_kernel_ms())
+            load_ms.append(tg.tg_last_loader_kernel_ms())
             plans += st.plans_dense
             states += st.states_live
             n_dp += st.n_dp
@@ -308,6 +309,7 @@ def run_ours(args):
         alg_bytes = states / args.steps * 8.0                          # live state: 4 B written + 4 B read
         achieved = alg_bytes / (km * 1e-3) / 1e9
         inst0 = insts[0]
+        load_bytes = sum(i.time_us.shape[0] * i.K * ((12 * i.P + 9 * i.K) if i.actmem_mb is not None else (8 * i.P + 9)) for i in insts)
         ncu_traffic = NCU_TRAFFIC_BYTES.get((args.workload, args.full_sweep), (None, None))
         if args.workload == "cfg5" and n != 1024:
             ncu_traffic = (None, None)
@@ -333,6 +335,12 @@ def run_ours(args):
                                      "achieved_Trelax_s": relax / args.steps / (km * 1e-3) / 1e12,
                                      "peak_Trelax_s": 148 * 64 * 1.965e9 / 1e12,
                                      "frac": relax / args.steps / (km * 1e-3) / (148 * 64 * 1.965e9)},
+                             # step 1 of the path (cost-table loader): 8*P bytes read and 9 bytes written per (slice, island) cell
+                             "loader": {"kernel": "tgLoadKernel", "kernel_ms": sum(load_ms) / len(load_ms),
+                                        "algorithmic_bytes_per_launch": float(load_bytes),
+                                        "achieved": load_bytes / (sum(load_ms) / len(load_ms) * 1e-3) / 1e9, "unit": "GB/s",
+                                        "frac": load_bytes / (sum(load_ms) / len(load_ms) * 1e-3) / 1e9 / peak,
+                                        "note": "a few MB: bound by launch latency, not by HBM" if load_bytes < (32 << 20) else "HBM stream"},
                              "cta_cycle_shares": dict(zip(["stage", "unused1", "unused2", "dp_levels", "level_barrier_wait",
                                                            "grid_wait", "scheduler", "backtrack"],
                                                           [round(c / max(1, sum(cyc)), 4) for c in cyc]))}}

@@ -205,6 +205,10 @@ tg_status tg_instance_read_time(tg_instance* inst, int32_t* time_out);
  * thread (CUDA events recorded on its stream around the launch; waits for it to finish).  HOST out. */
 tg_status tg_last_solver_kernel_ms(float* ms_out);
 
+/* The same for the cost-table loader kernel of the most recent tg_solve_batch, tg_reduce or
+ * tg_dp_at of this host thread.  HOST out. */
+tg_status tg_last_loader_kernel_ms(float* ms_out);
+
 const char* tg_last_error(void); /* thread-local, valid until the next tg_* call on the thread */
 int32_t tg_version(void);
 

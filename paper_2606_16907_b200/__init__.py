@@ -62,7 +62,7 @@ class TangramError(RuntimeError):
 
 _lib = None
 EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
-           "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_error", "tg_version"]
+           "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
 
 
 def lib():
@@ -90,6 +90,7 @@ def lib():
         L.tg_dp_at.argtypes = [vp, i64, vp, vp]
         L.tg_instance_read_time.argtypes = [vp, vp]
         L.tg_last_solver_kernel_ms.argtypes = [C.POINTER(C.c_float)]
+        L.tg_last_loader_kernel_ms.argtypes = [C.POINTER(C.c_float)]
         L.tg_last_error.restype = C.c_char_p
         L.tg_version.restype = i32
         for name in EXPORTS:
@@ -269,6 +270,12 @@ def tg_instance_read_time(inst: Instance) -> np.ndarray:
 def tg_last_solver_kernel_ms() -> float:
     ms = C.c_float(0)
     _check(lib().tg_last_solver_kernel_ms(C.byref(ms)))
+    return ms.value
+
+
+def tg_last_loader_kernel_ms() -> float:
+    ms = C.c_float(0)
+    _check(lib().tg_last_loader_kernel_ms(C.byref(ms)))
     return ms.value
 
 

@@ -147,6 +147,8 @@ struct Workspace {
 };
 
 // Lays out the per-call workspace, uploads the instance records and runs loader + prepare.
+thread_local cudaEvent_t g_evL0 = nullptr, g_evL1 = nullptr;  // bracket the last loader kernel of this thread
+
 tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStream_t st, Workspace& W) {
     if (!instances) return fail(TG_ERR_NULL, "instances is NULL");
     if (n < 1 || n > 65535) return fail(TG_ERR_SHAPE, "n must be in [1, 65535]");
@@ -291,6 +293,8 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const bool wide = int64_t(ctasU) * n >= 2 * D->numSMs;
     const dim3 g(wide ? ctasU : (maxCells + 255) / 256, n);
     const int P0 = instances[0]->P;
+    if (!g_evL0) { TG_CUDA(cudaEventCreate(&g_evL0)); TG_CUDA(cudaEventCreate(&g_evL1)); }
+    TG_CUDA(cudaEventRecord(g_evL0, st));
     if (wide) {
         if (P0 == 4) tgLoadKernel<1, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);
         else if (P0 == 8) tgLoadKernel<2, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);
@@ -300,6 +304,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         else if (P0 == 8) tgLoadKernel<2, 1><<<g, 256, 0, st>>>(W.inst);
         else tgLoadKernel<0, 1><<<g, 256, 0, st>>>(W.inst);
     }
+    TG_CUDA(cudaEventRecord(g_evL1, st));
     tgPrepareKernel<<<n, TG_PREP_NT, TG_SORT_SMEM_MAX * 4, st>>>(W.inst);
     TG_CUDA(cudaGetLastError());
     return TG_OK;
@@ -780,6 +785,14 @@ tg_status tg_last_solver_kernel_ms(float* ms_out) {
     if (!g_evA) return fail(TG_ERR_CUDA, "no solver kernel was launched on this thread");
     TG_CUDA(cudaEventSynchronize(g_evB));
     TG_CUDA(cudaEventElapsedTime(ms_out, g_evA, g_evB));
+    return TG_OK;
+}
+
+tg_status tg_last_loader_kernel_ms(float* ms_out) {
+    if (!ms_out) return fail(TG_ERR_NULL, "ms_out is NULL");
+    if (!g_evL0) return fail(TG_ERR_CUDA, "no loader kernel was launched on this thread");
+    TG_CUDA(cudaEventSynchronize(g_evL1));
+    TG_CUDA(cudaEventElapsedTime(ms_out, g_evL0, g_evL1));
     return TG_OK;
 }
 

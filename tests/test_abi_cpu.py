@@ -64,6 +64,7 @@ def test_argument_errors_need_no_device(tg):
     assert L.tg_dp_at(None, 0, None, None) == 1
     assert L.tg_reduce(None, None, None, None, None, None, None) == 1
     assert L.tg_last_solver_kernel_ms(None) == 1
+    assert L.tg_last_loader_kernel_ms(None) == 1
 
 
 def test_no_cpu_fallback_without_a_device(tg):
