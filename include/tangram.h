@@ -183,6 +183,14 @@ typedef enum {
 tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4],
                    void* cuda_stream);
 
+/* tg_prune_batch — tg_prune over n DISTINCT instances with one mode and threshold in one pass: one grid over every
+ * cell of the batch (the raw tables streamed once, 385 MB for the 1024-instance batch), one
+ * synchronisation.  counts_out: HOST int64 [n][4], row i = what tg_prune(instances[i], ...) would have returned;
+ * the tables end up exactly as after n single calls.  n == 0 is a no-op; n in [0, 65535]; an instance listed twice
+ * -> TG_ERR_RANGE; argument errors are reported before anything is modified. */
+tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode mode, int64_t threshold,
+                         int64_t* counts_out, void* cuda_stream);
+
 /* ---- step-level entry points (used by the parity tests to check single steps) ---------------- */
 
 /* Steps 1-3 alone: reduced tables and candidate thresholds.  All outputs HOST, any may be NULL.

@@ -61,7 +61,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune",
+EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
            "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -86,6 +86,7 @@ def lib():
         L.tg_solve_batch.argtypes = [C.POINTER(vp), i32, vp, vp]
         L.tg_solve_batch_ex.argtypes = [C.POINTER(vp), i32, vp, u32, vp, vp]
         L.tg_prune.argtypes = [vp, C.c_int, i64, C.POINTER(i64), vp]
+        L.tg_prune_batch.argtypes = [C.POINTER(vp), i32, C.c_int, i64, C.POINTER(i64), vp]
         L.tg_reduce.argtypes = [vp, vp, vp, vp, vp, C.POINTER(i32), vp]
         L.tg_dp_at.argtypes = [vp, i64, vp, vp]
         L.tg_instance_read_time.argtypes = [vp, vp]
@@ -259,6 +260,14 @@ def tg_prune(inst: Instance, mode: int = TG_PRUNE_EXACT, threshold: int = 0, str
     counts = (C.c_int64 * 4)()
     _check(lib().tg_prune(inst.handle, mode, threshold, counts, _stream_ptr(stream)))
     return np.array(list(counts), dtype=np.int64)
+
+
+def tg_prune_batch(instances, mode: int = TG_PRUNE_EXACT, threshold: int = 0, stream=None) -> np.ndarray:
+    """tg_prune over distinct instances in one pass; returns counts [n, 4]."""
+    n = len(instances)
+    counts = (C.c_int64 * (4 * max(n, 1)))()
+    _check(lib().tg_prune_batch(_handles(instances), n, mode, threshold, counts, _stream_ptr(stream)))
+    return np.array(list(counts), dtype=np.int64)[:4 * n].reshape(n, 4)
 
 
 def tg_instance_read_time(inst: Instance) -> np.ndarray:

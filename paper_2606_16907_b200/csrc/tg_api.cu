@@ -6,6 +6,7 @@
 #include <atomic>
 #include <mutex>
 #include <string>
+#include <algorithm>
 #include <vector>
 
 #include "tg_common.cuh"
@@ -750,34 +751,56 @@ tg_status tg_reduce(tg_instance* inst, int32_t* c_out, int32_t* argp_out, int32_
     return TG_OK;
 }
 
-tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4], void* cuda_stream) {
-    if (!inst || !counts_out) return fail(TG_ERR_NULL, "NULL argument");
+tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode mode, int64_t threshold, int64_t* counts_out,
+                         void* cuda_stream) {
+    if (n == 0) return TG_OK;
+    if (!instances || !counts_out) return fail(TG_ERR_NULL, "NULL argument");
+    if (n < 0 || n > 65535) return fail(TG_ERR_SHAPE, "n must be in [0, 65535]");
     if (mode != TG_PRUNE_EXACT && mode != TG_PRUNE_IMBALANCE && mode != TG_PRUNE_BOTTLENECK)
         return fail(TG_ERR_RANGE, "unknown prune mode");
     if (mode == TG_PRUNE_IMBALANCE && (threshold < 1000 || threshold > 16384))
         return fail(TG_ERR_RANGE, "theta must be in [1000, 16384] permille");
     if (mode == TG_PRUNE_BOTTLENECK && threshold < 0) return fail(TG_ERR_RANGE, "bottleneck cap must be >= 0");
+    std::vector<TgPruneDesc> h(n);
+    int maxCells = 0;
+    for (int i = 0; i < n; ++i) {
+        tg_instance* t = instances[i];
+        if (!t) return fail(TG_ERR_NULL, "instances[" + std::to_string(i) + "] is NULL");
+        h[i] = TgPruneDesc{t->time_us, t->mem_mb, t->actmem, t->cap_mb, t->L, t->K, t->P, t->NS * t->K};
+        maxCells = std::max(maxCells, h[i].nCells);
+    }
+    {   // an instance listed twice would be pruned by two grids at once
+        std::vector<const tg_instance*> seen(instances, instances + n);
+        std::sort(seen.begin(), seen.end());
+        if (std::adjacent_find(seen.begin(), seen.end()) != seen.end()) return fail(TG_ERR_RANGE, "an instance appears twice in the batch");
+    }
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    const int cells = inst->NS * inst->K;
+    const size_t oCounts = 0, oCap = size_t(n) * 32, oDesc = oCap + size_t(n) * (TG_MAX_K + 1) * 8;
     char* ws = nullptr;
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&ws), 4 * 8 + (TG_MAX_K + 1) * 8, st));
-    unsigned long long* dCounts = reinterpret_cast<unsigned long long*>(ws);
-    long long* dCap = reinterpret_cast<long long*>(ws + 32);
-    TG_CUDA(cudaMemsetAsync(ws, 0, 32, st));
-    tgPruneCellKernel<<<(cells + 255) / 256, 256, 0, st>>>(inst->time_us, inst->mem_mb, inst->actmem, inst->cap_mb, cells, inst->K,
-                                                          inst->P, int(mode), threshold, dCounts);
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&ws), oDesc + sizeof(TgPruneDesc) * size_t(n), st));
+    unsigned long long* dCounts = reinterpret_cast<unsigned long long*>(ws + oCounts);
+    long long* dCap = reinterpret_cast<long long*>(ws + oCap);
+    TgPruneDesc* dDesc = reinterpret_cast<TgPruneDesc*>(ws + oDesc);
+    TG_CUDA(cudaMemsetAsync(ws, 0, oCap, st));
+    TG_CUDA(cudaMemcpyAsync(dDesc, h.data(), sizeof(TgPruneDesc) * size_t(n), cudaMemcpyHostToDevice, st));
+    const dim3 g((maxCells + 255) / 256, n);
+    tgPruneCellKernel<<<g, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
     if (mode == TG_PRUNE_IMBALANCE) {
-        tgPruneTauKernel<<<1, 256, 0, st>>>(inst->time_us, inst->L, inst->K, inst->P, dCap);
-        tgPruneImbalanceKernel<<<(cells + 255) / 256, 256, 0, st>>>(inst->time_us, dCap, inst->L, inst->K, inst->P, cells,
-                                                                   threshold, dCounts);
+        tgPruneTauKernel<<<n, 256, 0, st>>>(dDesc, dCap);
+        tgPruneImbalanceKernel<<<g, 256, 0, st>>>(dDesc, dCap, threshold, dCounts);
     }
     TG_CUDA(cudaGetLastError());
-    unsigned long long hc[4];
-    TG_CUDA(cudaMemcpyAsync(hc, dCounts, 32, cudaMemcpyDeviceToHost, st));
-    TG_CUDA(cudaStreamSynchronize(st));
+    std::vector<unsigned long long> hc(size_t(n) * 4);
+    TG_CUDA(cudaMemcpyAsync(hc.data(), dCounts, size_t(n) * 32, cudaMemcpyDeviceToHost, st));
+    TG_CUDA(cudaStreamSynchronize(st));   // also keeps h alive until the descriptor upload has been read
     TG_CUDA(cudaFreeAsync(ws, st));
-    for (int i = 0; i < 4; ++i) counts_out[i] = int64_t(hc[i]);
+    for (size_t i = 0; i < size_t(n) * 4; ++i) counts_out[i] = int64_t(hc[i]);
     return TG_OK;
+}
+
+tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4], void* cuda_stream) {
+    if (!inst || !counts_out) return fail(TG_ERR_NULL, "NULL argument");
+    return tg_prune_batch(&inst, 1, mode, threshold, counts_out, cuda_stream);
 }
 
 tg_status tg_last_solver_kernel_ms(float* ms_out) {

@@ -507,10 +507,25 @@ __global__ void tgExportKernel(const TgInstDev* __restrict__ insts, int32_t* __r
 // Step 0: pruning pass (SURVEY.md §8(c) rules R1-R4)
 // ---------------------------------------------------------------------------------------------
 // R1 infeasible, R2 dominated inside one (slice, island) cell, optional R4 bottleneck cap.
-__global__ void __launch_bounds__(256) tgPruneCellKernel(int32_t* __restrict__ time_us, const int32_t* __restrict__ mem_mb,
-                                                         const int32_t* __restrict__ actmem_mb,   // nullptr: no footprint
-                                                         const int32_t* __restrict__ cap, int nCells, int K, int P,
-                                                         int mode, int64_t threshold, unsigned long long* counts) {
+// One instance of a pruning batch (tg_prune is a batch of one): grid.y = instance, counts[4 * y + rule].
+struct TgPruneDesc {
+    int32_t* time_us;
+    const int32_t* mem_mb;
+    const int32_t* actmem_mb;   // nullptr: no footprint
+    const int32_t* cap;
+    int L, K, P, nCells;
+};
+
+__global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __restrict__ descs, int mode, int64_t threshold,
+                                                         unsigned long long* counts) {
+    const TgPruneDesc D = descs[blockIdx.y];
+    int32_t* const time_us = D.time_us;
+    const int32_t* const mem_mb = D.mem_mb;
+    const int32_t* const actmem_mb = D.actmem_mb;
+    const int32_t* const cap = D.cap;
+    const int nCells = D.nCells, K = D.K, P = D.P;
+    counts += 4 * blockIdx.y;
+    if (int(blockIdx.x) * 256 >= nCells) return;
     const int cell = blockIdx.x * 256 + threadIdx.x;
     unsigned c1 = 0, c2 = 0, c4 = 0;
     if (cell < nCells) {
@@ -558,8 +573,12 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(int32_t* __restrict__ t
 }
 
 // R3 pre-pass: island capacity from profiled atom throughput.  capOut[k] = floor(2^32 / tau_k)
-// (0 = exempt), capOut[K] = sum.  One CTA.
-__global__ void tgPruneTauKernel(const int32_t* __restrict__ time_us, int L, int K, int P, long long* capOut) {
+// (0 = exempt), capOut[K] = sum.  One CTA per instance.
+__global__ void tgPruneTauKernel(const TgPruneDesc* __restrict__ descs, long long* capOut) {
+    const TgPruneDesc D = descs[blockIdx.x];
+    const int32_t* const time_us = D.time_us;
+    const int L = D.L, K = D.K, P = D.P;
+    capOut += (TG_MAX_K + 1) * blockIdx.x;
     __shared__ unsigned long long tau[TG_MAX_K];
     __shared__ int bad[TG_MAX_K];
     if (threadIdx.x < TG_MAX_K) { tau[threadIdx.x] = 0; bad[threadIdx.x] = 0; }
@@ -587,9 +606,14 @@ __global__ void tgPruneTauKernel(const int32_t* __restrict__ time_us, int L, int
 
 // R3 imbalance: kill every plan of a (slice, island) pair whose atom share mismatches the island's
 // capacity share by more than theta (permille).
-__global__ void __launch_bounds__(256) tgPruneImbalanceKernel(int32_t* __restrict__ time_us, const long long* __restrict__ capIn,
-                                                              int L, int K, int P, int nCells, int64_t theta,
-                                                              unsigned long long* counts) {
+__global__ void __launch_bounds__(256) tgPruneImbalanceKernel(const TgPruneDesc* __restrict__ descs, const long long* __restrict__ capIn,
+                                                              int64_t theta, unsigned long long* counts) {
+    const TgPruneDesc D = descs[blockIdx.y];
+    int32_t* const time_us = D.time_us;
+    const int L = D.L, K = D.K, P = D.P, nCells = D.nCells;
+    capIn += (TG_MAX_K + 1) * blockIdx.y;
+    counts += 4 * blockIdx.y;
+    if (int(blockIdx.x) * 256 >= nCells) return;
     const int cell = blockIdx.x * 256 + threadIdx.x;
     unsigned c3 = 0;
     if (cell < nCells) {

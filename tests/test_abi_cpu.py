@@ -61,6 +61,8 @@ def test_argument_errors_need_no_device(tg):
     assert L.tg_solve_batch(None, 0, None, None) == 0                                    # n == 0: no-op
     cnt = (C.c_int64 * 4)()
     assert L.tg_prune(None, 0, 0, cnt, None) == 1
+    assert L.tg_prune_batch(None, 3, 0, 0, cnt, None) == 1
+    assert L.tg_prune_batch(None, 0, 0, 0, cnt, None) == 0                               # n == 0: no-op
     assert L.tg_dp_at(None, 0, None, None) == 1
     assert L.tg_reduce(None, None, None, None, None, None, None) == 1
     assert L.tg_last_solver_kernel_ms(None) == 1

@@ -83,11 +83,42 @@ def test_prune_with_footprint_table_and_counts(tg, mode, thr):
     assert killed3 > 100
 
 
+@pytest.mark.parametrize("mode,thr", [(0, 0), (1, 3000), (1, 1000), (2, 700), (2, 1 << 25)])
+def test_prune_batch_equals_single_calls(tg, mode, thr):
+    """tg_prune_batch: instances of every shape, with and without a footprint table, in one pass; row i of the counts
+    and the tables as after tg_prune on instance i (oracle.prune / oracle.prune_depth); then the pruned batch solves
+    like the oracle on the oracle's pruned tables."""
+    insts = cases() + cases_with_footprint()
+    hs = [tg.instance_from_inputs(i) for i in insts]
+    counts = tg.tg_prune_batch(hs, mode, thr)
+    assert counts.shape == (len(insts), 4)
+    pruned = []
+    for inst, h, c in zip(insts, hs, counts):
+        pr, oc = (oracle.prune_depth if inst.actmem_mb is not None else oracle.prune)(inst, mode, thr)
+        assert c.tolist() == oc.tolist(), (inst.name, mode, thr)
+        t = tg.tg_instance_read_time(h)
+        assert np.array_equal(t, pr.time_us.reshape(t.shape)), (inst.name, mode, thr)
+        pruned.append(pr)
+    for pr, g in zip(pruned, tg.tg_solve_batch(hs)):
+        same(oracle.solve_depth(pr) if pr.actmem_mb is not None else oracle.solve(pr), g, pr.name)
+    if mode != 1:                                               # idempotent (R3 re-profiles: DESIGN.md R-r3)
+        assert not tg.tg_prune_batch(hs, mode, thr).any()
+    assert tg.tg_prune_batch([], mode, thr).shape == (0, 4)
+    with pytest.raises(tg.TangramError) as e:                   # the same instance twice
+        tg.tg_prune_batch([hs[0], hs[1], hs[0]], mode, thr)
+    assert e.value.status == 3
+    for h in hs:
+        h.destroy()
+
+
 def test_prune_errors(tg):
     h = tg.instance_from_inputs(gen.config1())
     for mode, thr in [(3, 0), (1, 999), (1, 16385), (2, -1)]:
         with pytest.raises(tg.TangramError) as e:
             tg.tg_prune(h, mode, thr)
+        assert e.value.status == 3
+        with pytest.raises(tg.TangramError) as e:
+            tg.tg_prune_batch([h], mode, thr)
         assert e.value.status == 3
     h.destroy()
 
