@@ -784,7 +784,26 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
     TG_CUDA(cudaMemsetAsync(ws, 0, oCap, st));
     TG_CUDA(cudaMemcpyAsync(dDesc, h.data(), sizeof(TgPruneDesc) * size_t(n), cudaMemcpyHostToDevice, st));
     const dim3 g((maxCells + 255) / 256, n);
-    tgPruneCellKernel<<<g, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+    {   // cell pass: the register path is compiled for P = 4 and P = 8 (picked from the first instance); two cells per
+        // thread once that still leaves every SM a few CTAs
+        DeviceState* DS = nullptr;
+        int dev = 0;
+        TG_CUDA(cudaGetDevice(&dev));
+        const tg_status sd = deviceInit(dev, &DS);
+        if (sd != TG_OK) { cudaFreeAsync(ws, st); return sd; }
+        const int P0 = instances[0]->P;
+        const dim3 g2((maxCells + 511) / 512, n);
+        const bool wide = int64_t(g2.x) * n >= 4 * DS->numSMs;
+        if (P0 == 4) {
+            if (wide) tgPruneCellKernel<1, 2><<<g2, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+            else tgPruneCellKernel<1, 1><<<g, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+        } else if (P0 == 8) {
+            if (wide) tgPruneCellKernel<2, 2><<<g2, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+            else tgPruneCellKernel<2, 1><<<g, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+        } else {
+            tgPruneCellKernel<0, 1><<<g, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+        }
+    }
     if (mode == TG_PRUNE_IMBALANCE) {
         tgPruneTauKernel<<<n, 256, 0, st>>>(dDesc, dCap);
         tgPruneImbalanceKernel<<<g, 256, 0, st>>>(dDesc, dCap, threshold, dCounts);

@@ -516,8 +516,13 @@ struct TgPruneDesc {
     int L, K, P, nCells;
 };
 
+// PV > 0: an instance with P = 4 * PV plans is pruned from registers -- the 16-byte loads of the thread's U cells are
+// issued first, the rules run on the register copy and a cell whose column changed is stored back as 16-byte words;
+// any other instance of the batch takes the entry-by-entry path.  grid = (cells / (256 U), instances).
+template <int PV, int U>
 __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __restrict__ descs, int mode, int64_t threshold,
                                                          unsigned long long* counts) {
+    constexpr int PVA = PV > 0 ? PV : 1, PP = 4 * PVA;
     const TgPruneDesc D = descs[blockIdx.y];
     int32_t* const time_us = D.time_us;
     const int32_t* const mem_mb = D.mem_mb;
@@ -525,39 +530,101 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
     const int32_t* const cap = D.cap;
     const int nCells = D.nCells, K = D.K, P = D.P;
     counts += 4 * blockIdx.y;
-    if (int(blockIdx.x) * 256 >= nCells) return;
-    const int cell = blockIdx.x * 256 + threadIdx.x;
+    if (int(blockIdx.x) * (256 * U) >= nCells) return;
+    const int cellFirst = blockIdx.x * (256 * U) + threadIdx.x;
     unsigned c1 = 0, c2 = 0, c4 = 0;
-    if (cell < nCells) {
-        int32_t* t = time_us + size_t(cell) * P;
-        const int32_t* mm = mem_mb + size_t(cell) * P;
-        const int32_t* am = actmem_mb ? actmem_mb + size_t(cell) * P : nullptr;
-        const int32_t capk = cap[cell % K];
-        // R1: with a footprint the shallowest depth (one microbatch in flight) decides "never feasible"
-        for (int p = 0; p < P; ++p)
-            if (t[p] != TG_INVALID && int64_t(mm[p]) + (am ? am[p] : 0) > capk) { t[p] = TG_INVALID; ++c1; }
-        // R2: q kills p iff q <= p on every axis (time, memory and, if present, footprint) and differs, or ties with q < p
-        uint32_t dead[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        for (int p = 0; p < P; ++p) {
-            const int32_t tp = t[p];
-            if (tp == TG_INVALID) continue;
-            const int32_t mp = mm[p], ap = am ? am[p] : 0;
-            bool dd = false;
-            for (int q = 0; q < P && !dd; ++q) {
-                const int32_t tq = t[q];
-                if (q == p || tq == TG_INVALID) continue;
-                const int32_t mq = mm[q], aq = am ? am[q] : 0;
-                const bool le = tq <= tp && mq <= mp && aq <= ap;
-                const bool eq = tq == tp && mq == mp && aq == ap;
-                dd = le && (!eq || q < p);
+    if (PV > 0 && P == PP) {
+        int4 tv[U][PVA], mv[U][PVA], av[U][PVA];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int cell = cellFirst + 256 * u;
+            if (cell < nCells) {
+#pragma unroll
+                for (int v = 0; v < PVA; ++v) {
+                    tv[u][v] = *(reinterpret_cast<const int4*>(time_us + size_t(cell) * PP) + v);
+                    mv[u][v] = __ldg(reinterpret_cast<const int4*>(mem_mb + size_t(cell) * PP) + v);
+                    av[u][v] = actmem_mb ? __ldg(reinterpret_cast<const int4*>(actmem_mb + size_t(cell) * PP) + v) : make_int4(0, 0, 0, 0);
+                }
             }
-            if (dd) dead[p >> 5] |= 1u << (p & 31);
         }
-        for (int p = 0; p < P; ++p)
-            if (dead[p >> 5] >> (p & 31) & 1u) { t[p] = TG_INVALID; ++c2; }
-        if (mode == TG_PRUNE_BOTTLENECK)
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int cell = cellFirst + 256 * u;
+            if (cell < nCells) {
+                int32_t t[PP], mm[PP], am[PP];
+#pragma unroll
+                for (int v = 0; v < PVA; ++v) {
+                    t[4 * v] = tv[u][v].x; t[4 * v + 1] = tv[u][v].y; t[4 * v + 2] = tv[u][v].z; t[4 * v + 3] = tv[u][v].w;
+                    mm[4 * v] = mv[u][v].x; mm[4 * v + 1] = mv[u][v].y; mm[4 * v + 2] = mv[u][v].z; mm[4 * v + 3] = mv[u][v].w;
+                    am[4 * v] = av[u][v].x; am[4 * v + 1] = av[u][v].y; am[4 * v + 2] = av[u][v].z; am[4 * v + 3] = av[u][v].w;
+                }
+                const int32_t capk = __ldg(cap + cell % K);
+                unsigned kill = 0;
+#pragma unroll
+                for (int p = 0; p < PP; ++p)   // R1
+                    if (t[p] != TG_INVALID && int64_t(mm[p]) + am[p] > capk) { t[p] = TG_INVALID; kill |= 1u << p; ++c1; }
+                unsigned dead = 0;
+#pragma unroll
+                for (int p = 0; p < PP; ++p) {   // R2, decided on the cell as R1 left it
+                    bool dd = false;
+#pragma unroll
+                    for (int q = 0; q < PP; ++q) {
+                        if (q == p) continue;
+                        const bool le = t[q] <= t[p] && mm[q] <= mm[p] && am[q] <= am[p];   // t[q] == INVALID is never <= a live t[p]
+                        const bool eq = t[q] == t[p] && mm[q] == mm[p] && am[q] == am[p];
+                        dd = dd || (le && (!eq || q < p));
+                    }
+                    if (t[p] != TG_INVALID && dd) dead |= 1u << p;
+                }
+#pragma unroll
+                for (int p = 0; p < PP; ++p)
+                    if (dead >> p & 1u) { t[p] = TG_INVALID; ++c2; }
+                kill |= dead;
+                if (mode == TG_PRUNE_BOTTLENECK) {
+#pragma unroll
+                    for (int p = 0; p < PP; ++p)
+                        if (t[p] != TG_INVALID && int64_t(t[p]) > threshold) { t[p] = TG_INVALID; kill |= 1u << p; ++c4; }
+                }
+#pragma unroll
+                for (int v = 0; v < PVA; ++v)
+                    if (kill >> (4 * v) & 0xfu)
+                        *(reinterpret_cast<int4*>(time_us + size_t(cell) * PP) + v) = make_int4(t[4 * v], t[4 * v + 1], t[4 * v + 2], t[4 * v + 3]);
+            }
+        }
+    } else {
+        for (int u = 0; u < U; ++u) {
+            const int cell = cellFirst + 256 * u;
+            if (cell >= nCells) break;
+            int32_t* t = time_us + size_t(cell) * P;
+            const int32_t* mm = mem_mb + size_t(cell) * P;
+            const int32_t* am = actmem_mb ? actmem_mb + size_t(cell) * P : nullptr;
+            const int32_t capk = cap[cell % K];
+            // R1: with a footprint the shallowest depth (one microbatch in flight) decides "never feasible"
             for (int p = 0; p < P; ++p)
-                if (t[p] != TG_INVALID && int64_t(t[p]) > threshold) { t[p] = TG_INVALID; ++c4; }
+                if (t[p] != TG_INVALID && int64_t(mm[p]) + (am ? am[p] : 0) > capk) { t[p] = TG_INVALID; ++c1; }
+            // R2: q kills p iff q <= p on every axis (time, memory and, if present, footprint) and differs, or ties with q < p
+            uint32_t dead[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            for (int p = 0; p < P; ++p) {
+                const int32_t tp = t[p];
+                if (tp == TG_INVALID) continue;
+                const int32_t mp = mm[p], ap = am ? am[p] : 0;
+                bool dd = false;
+                for (int q = 0; q < P && !dd; ++q) {
+                    const int32_t tq = t[q];
+                    if (q == p || tq == TG_INVALID) continue;
+                    const int32_t mq = mm[q], aq = am ? am[q] : 0;
+                    const bool le = tq <= tp && mq <= mp && aq <= ap;
+                    const bool eq = tq == tp && mq == mp && aq == ap;
+                    dd = le && (!eq || q < p);
+                }
+                if (dd) dead[p >> 5] |= 1u << (p & 31);
+            }
+            for (int p = 0; p < P; ++p)
+                if (dead[p >> 5] >> (p & 31) & 1u) { t[p] = TG_INVALID; ++c2; }
+            if (mode == TG_PRUNE_BOTTLENECK)
+                for (int p = 0; p < P; ++p)
+                    if (t[p] != TG_INVALID && int64_t(t[p]) > threshold) { t[p] = TG_INVALID; ++c4; }
+        }
     }
     // warp-aggregate the counters
     for (int o = 16; o > 0; o >>= 1) {
