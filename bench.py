@@ -300,6 +300,23 @@ def run_ours(args):
             h.destroy()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
+    prune_info = None
+    if args.with_prune:
+        # step 0 of the path, outside every timed region above: tg_prune_batch(EXACT) once on a fresh copy of the
+        # workload (the pass mutates its instances); wall clock of the call, which synchronises
+        hs = tg.tg_instance_create_batch([(i.L, i.K, i.P, i.m, *pp, i.act_mb) for i, pp in zip(insts, pinned)])
+        for h, pa in zip(hs, pinned_act):
+            if pa is not None:
+                tg.tg_instance_set_actmem(h, pa)
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        tp = time.perf_counter()
+        killed = tg.tg_prune_batch(hs, tg.TG_PRUNE_EXACT, 0)
+        prune_ms = (time.perf_counter() - tp) * 1e3
+        for h in hs:
+            h.destroy()
+        prune_info = {"call": "tg_prune_batch(EXACT)", "wall_ms": prune_ms, "killed_r1_r2": killed.sum(0)[:2].tolist(),
+                      "entries": int(sum(i.time_us.size for i in insts))}
     from paper_2606_16907_b200.shard import aggregate
     (plans_all, plans_e2e, ndp_all), (total_ms, e2e_s) = aggregate(
         [float(plans), float(plans) / args.steps * e2e_steps, float(n_dp)], [total_ms, e2e_s], device="cuda")
@@ -344,6 +361,8 @@ def run_ours(args):
                              "cta_cycle_shares": dict(zip(["stage", "unused1", "unused2", "dp_levels", "level_barrier_wait",
                                                            "grid_wait", "scheduler", "backtrack"],
                                                           [round(c / max(1, sum(cyc)), 4) for c in cyc]))}}
+        if prune_info is not None:
+            line["prune"] = prune_info
         if not args.no_cpu_baseline:
             import oracle
             cores = max(1, min(oracle.hw_threads(), args.cpu_threads))
@@ -368,6 +387,7 @@ def main():
     ap.add_argument("--full-sweep", action="store_true", help="run the DP at every candidate T")
     ap.add_argument("--cpu-threads", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--with-prune", action="store_true", help="also run tg_prune_batch once on a fresh copy of the workload (untimed legs unchanged)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":
