@@ -382,9 +382,24 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
         const int k = w / stride, d = w - k * stride;
         uint32_t mn = TG_INFU, mnAll = TG_INFU;
         if (d >= 1 && d <= L) {
-            const uint32_t* row = I.cd + size_t(k) * I.triG + tgGOff(L, d);
-            for (int a = 0; a <= L - 1 - d; ++a) mn = min(mn, row[a]);
-            mnAll = min(mn, row[L - d]);
+            // the row holds a = 0..L-d, padded with INF to a multiple of 4 words and 16-byte aligned: 16-byte loads,
+            // four in flight; the last element (b = L) only counts for the all-slices minimum
+            const uint4* row4 = reinterpret_cast<const uint4*>(I.cd + size_t(k) * I.triG + tgGOff(L, d));
+            const int n4 = (L - d + 4) >> 2, last = L - d;
+            for (int q0 = 0; q0 < n4; q0 += 4) {
+                uint4 v[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) v[e] = q0 + e < n4 ? __ldcg(row4 + q0 + e) : make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t w[4] = {v[e].x, v[e].y, v[e].z, v[e].w};
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        mnAll = min(mnAll, w[c]);
+                        if (4 * (q0 + e) + c != last) mn = min(mn, w[c]);
+                    }
+                }
+            }
         }
         sbuf[w] = mn;                 // (shared memory: the suffix scan below is a chain of dependent accesses)
         sbuf[K * stride + w] = mnAll;
