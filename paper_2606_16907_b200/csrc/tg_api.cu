@@ -55,6 +55,7 @@ struct DeviceState {
     uint64_t budget = 0;  // bytes the DP scratch may take (from cudaMemGetInfo; refreshed every 64 solves or after a failed allocation)
     int budgetAge = 0;
     uint16_t* rankOf = nullptr;
+    uint16_t* maskOf = nullptr;
 };
 std::mutex g_mu;
 int g_gallopMax = [] { const char* e = getenv("TG_GALLOP_MAX"); int v = e ? atoi(e) : 10; return v < 1 ? 1 : (v > 16 ? 16 : v); }();
@@ -85,27 +86,35 @@ tg_status deviceInit(int dev, DeviceState** out) {
             binom[n][0] = 1;
             for (int r = 1; r <= n; ++r) binom[n][r] = uint16_t(binom[n - 1][r - 1] + (r <= n - 1 ? binom[n - 1][r] : 0));
         }
-        uint32_t fill[17];
+        uint32_t fill[17], popOff[18];
         memset(fill, 0, sizeof(fill));
+        popOff[0] = 0;
+        for (int r = 0; r <= 16; ++r) popOff[r + 1] = popOff[r] + binom[16][r];
+        std::vector<uint16_t> maskOf(65536);   // masks ordered by (popcount, value): the inverse of rankOf
         for (uint32_t mk = 0; mk < 65536; ++mk) {
             const int r = __builtin_popcount(mk);
             rankOf[mk] = uint16_t(fill[r]);
+            maskOf[popOff[r] + fill[r]] = uint16_t(mk);
             ++fill[r];
         }
-        TG_CUDA(cudaMalloc(&D.rankOf, 65536 * sizeof(uint16_t)));
+        TG_CUDA(cudaMalloc(&D.rankOf, 2 * 65536 * sizeof(uint16_t)));
+        D.maskOf = D.rankOf + 65536;
         TG_CUDA(cudaMemcpy(D.rankOf, rankOf.data(), 65536 * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        TG_CUDA(cudaMemcpy(D.maskOf, maskOf.data(), 65536 * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        TG_CUDA(cudaMemcpyToSymbol(tgPopOff, popOff, sizeof(popOff)));
         TG_CUDA(cudaMemcpyToSymbol(tgBinom, binom, sizeof(binom)));
         TG_CUDA(cudaFuncSetAttribute(tgPrepareKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TG_SORT_SMEM_MAX * 4));
         cudaFuncAttributes fa;
         TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
-        int dyn = D.smemOptin - int(fa.sharedSizeBytes) - 1024;   // one CTA per SM
+        // TG_CTAS_PER_SM co-resident CTAs share the SM's shared memory (each CTA also pays 1 KB of system reserve)
+        int dyn = std::min(D.smemOptin, D.smemPerSM / TG_CTAS_PER_SM) - int(fa.sharedSizeBytes) - 1024;
         dyn &= ~1023;
-        if (dyn < 64 * 1024) return fail(TG_ERR_CUDA, "not enough shared memory per block for the solver");
+        if (dyn < 48 * 1024) return fail(TG_ERR_CUDA, "not enough shared memory per block for the solver");
         TG_CUDA(cudaFuncSetAttribute(tgSolveKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
         int occ = 0;
         TG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tgSolveKernel, TG_NT, size_t(dyn)));
-        if (occ < 1) return fail(TG_ERR_CUDA, "solver kernel does not fit on an SM");
-        D.ctasPerSM = 1;
+        if (occ < TG_CTAS_PER_SM) return fail(TG_ERR_CUDA, "solver kernel: fewer co-resident CTAs per SM than it was built for");
+        D.ctasPerSM = TG_CTAS_PER_SM;
         D.dynSmem = dyn;
         // keep stream-ordered scratch cached between calls
         cudaMemPool_t pool;
@@ -269,10 +278,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const int totalWords = W.dynSmem / 4;
     TgSolveCtx& c = W.ctx;
     memset(&c, 0, sizeof(c));
-    c.wbufWords = 2 * maxK * (maxLp + 16);
-    c.nActiveWarps = std::min(TG_NT / 32, (totalWords * 3 / 4) / c.wbufWords);
-    if (c.nActiveWarps < 1) return fail(TG_ERR_SHAPE, "shared memory too small for this instance shape");
-    c.csWords = (totalWords - c.nActiveWarps * c.wbufWords) & ~3;
+    c.dynWords = totalWords & ~3;
     c.inst = W.inst; c.nInst = n;
     c.items = reinterpret_cast<TgItem*>(W.base + oItems);
     c.keys = reinterpret_cast<unsigned long long*>(W.base + oKeys);
@@ -285,6 +291,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.wishFloor = g_wishFloor;
     c.ctrl = reinterpret_cast<TgCtrl*>(W.base + oCtrl);
     c.rankOf = D->rankOf;
+    c.maskOf = D->maskOf;
     c.specOut = reinterpret_cast<tg_result*>(W.base + oSpec);
 
     // loader grid: 256 * U cells per CTA, U = TG_LOAD_U when that still gives every SM two CTAs, else 1; the

@@ -8,7 +8,13 @@
 
 #define TG_INFU 0x40000000u   // saturating "no plan" (2^30); all DP values are uint32 <= 2^31
 #define TG_TINF 0x3fffffffu   // threshold standing for T = infinity: c <= TG_TINF  <=>  c finite
-#define TG_NT 512             // threads per CTA of the persistent solver (1 CTA per SM)
+#ifndef TG_NT
+#define TG_NT 256             // threads per CTA of the persistent solver
+#endif
+#ifndef TG_CTAS_PER_SM
+#define TG_CTAS_PER_SM 2      // co-resident solver CTAs per SM: each runs its own DP (or its own share of a team's DP), so one
+                              // CTA's barriers, copy latencies and level tails are filled by the other
+#endif
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
 #define TG_MAX_EVAL 1024      // evaluated thresholds remembered per instance
 #define TG_MAX_WISH 64        // DPs per instance and round, upper bound
@@ -96,7 +102,7 @@ struct TgItem {
     uint8_t Ke;          // islands with some admissible slice at T (written by the CTA that runs the item)
     uint8_t flags;       // bit0: keep every level (back-track follows)
     uint8_t isl[TG_MAX_K];  // compact label -> original island
-    uint8_t ctaBeg, ctaCnt;  // team of CTAs that runs the item (weighted team mode; written by the scheduler)
+    uint16_t ctaBeg, ctaCnt;  // team of CTAs that runs the item (weighted team mode; written by the scheduler)
 };
 
 struct TgCtrl {
@@ -108,7 +114,7 @@ struct TgCtrl {
     int32_t errFlag;
     int32_t nActive;      // instances not done after the previous round's planning (wide scheduling: bounds W)
     int32_t weighted[2];  // per round parity: team sizes follow the items' estimated cost (teamOf / ctaBeg / ctaCnt)
-    uint8_t teamOf[2][256];   // weighted team mode: item of each CTA
+    uint8_t teamOf[2][1024];  // weighted team mode: item of each CTA
     tg_solve_stats stats;
     // debugging aid (TG_DEBUG=1): start time and item count of the first rounds
     unsigned long long roundNs[256];
@@ -136,13 +142,15 @@ struct TgSolveCtx {
     tg_result* specOut;         // [TG_MAX_ITEMS] results of the current round's speculative back-tracks
     tg_result* out;
     const uint16_t* rankOf;     // [65536] rank of a mask inside its popcount class
+    const uint16_t* maskOf;     // [65536] the inverse: masks ordered by (popcount, value); class r starts at tgPopOff[r]
     uint32_t flags;             // TG_SOLVE_*
     int32_t mode;               // 0 = solve, 1 = single DP at dpT (tg_dp_at)
     uint32_t dpT;
-    int32_t csWords;            // words of shared memory available for staged cost tables
-    int32_t wbufWords;          // words of warp-private shared memory: 2*Kmax rows of up to Lp + 16
-    int32_t nActiveWarps;       // warps per CTA that stream masks (all of them unless L is huge)
+    int32_t dynWords;           // words of dynamic shared memory of a solver CTA
 };
 
 // binomials up to 16 choose r
 __constant__ uint16_t tgBinom[17][17];
+// start of popcount class r in maskOf: sum_{q<r} C(16, q).  The masks of class r with all bits below Ke are its first
+// C(Ke, r) entries (any mask with a higher bit is larger), so one table serves every Ke.
+__constant__ uint32_t tgPopOff[18];

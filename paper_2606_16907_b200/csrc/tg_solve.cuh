@@ -18,6 +18,8 @@
 #include "tg_prep.cuh"
 
 #define TG_NW (TG_NT / 32)     // warps per CTA
+#define TG_NB_MAX 256   // masks per batch, upper bound (row index inside a batch fits 16 bits: 256 * 16)
+#define TG_DESC_W 6     // words of a mask descriptor: R | cap(R) << 16, pad, non-members (16 nibbles), members (16 nibbles)
 
 struct TgShared {
     // staged item
@@ -26,8 +28,12 @@ struct TgShared {
     uint32_t sT;
     // row windows (see "Row windows" below): rows hold Wd starts, row of state (S, k) begins at start lo4(cap(S))
     int sWd, sSlack, sWindowed;
-    // split of the dynamic shared memory for this item: [cost rows | nWarps x wbufWords]
-    int nWarps, wbufWords, wbufOff;
+    // split of the dynamic shared memory for this item: [cost rows | batch buffers of the level (tgLevelBatched)]
+    int batchOff;
+    uint32_t lvMagic[3];            // division magics of nbw, lvNsg, r
+    int lvNB, lvNsl, lvNsg;         // level geometry: masks per batch, rows per phase-1 item, groups of them per mask
+    uint32_t lvDesc[2], lvList, lvH, lvSrc[2];   // word offsets of the batch buffers
+    int cnt[2][TG_MAX_K];           // rows filed in each island's list (per batch parity)
     int csUsed4;                    // 16-byte words of the staged cost rows of all islands (incl. the pads between them)
     uint32_t cdOff;                 // word offset of the reduced table of the depth currently staged
     uint8_t maxlenK[TG_MAX_K];      // longest admissible slice of island k at T, any position
@@ -38,9 +44,6 @@ struct TgShared {
     alignas(16) uint32_t xInf[TG_MAX_K];            // all-INF transfer row for a lane's unused k slot
     uint8_t isl[TG_MAX_K];
     uint16_t binom[17][17];
-    // per-warp streaming state
-    uint32_t rowOf[TG_NW][2 * TG_MAX_K];            // source row of each member of the mask being issued (per half warp)
-    uint8_t kl[TG_NW][2 * TG_MAX_K];                // islands not in the current mask, ascending (per half warp)
     // scheduler / queue
     uint32_t warpSums[33];
     float wgt[32];                  // estimated cost of the round's items (weighted team mode)
@@ -183,6 +186,9 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
 // words between consecutive rows of a warp's buffer: 4 (mod 8), so consecutive rows start in different 16-byte
 // bank groups (rows are read by several island groups at the same chunk offset)
 __device__ __forceinline__ int tgRowStride(int Wd) { return Wd + 12 + (((Wd + 12) & 7) == 0 ? 4 : 0); }
+// words between consecutive source rows in shared memory: a multiple of 4 with an odd number of 16-byte
+// units, so rows of neighbouring masks start in different bank groups
+__device__ __forceinline__ int tgSrcStride(int Wd) { return Wd + 4 + (((Wd + 4) & 7) == 0 ? 4 : 0); }
 
 // ---------------------------------------------------------------------------------------------
 // Staging of one item's thresholded cost tables into shared memory.
@@ -222,8 +228,8 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
             if (Ke) atomicAdd((unsigned long long*)&ctx.ctrl->stats.states_live, (unsigned long long)L * Ke << (Ke - 1));
         }
     }
-    if (tid < Ke * Ke) {
-        const int kc = tid / Ke, jc = tid - kc * Ke;
+    for (int w = tid; w < Ke * Ke; w += TG_NT) {
+        const int kc = w / Ke, jc = w - kc * Ke;
         const uint32_t xv = I.x[int(sm.isl[kc]) * TG_MAX_K + int(sm.isl[jc])];
         sm.xS[kc][jc] = (I.xbound && xv > T) ? TG_INFU : xv;   // transfer bound (NEXT-3(b)): a slower link is not admissible at T
     }
@@ -231,8 +237,7 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
     // every island: sufMin / sufMinAll are non-decreasing in d, so each is the number of lengths whose entry is
     // <= T.  One warp per island, lanes over the lengths: one round trip to L2 instead of a binary search's seven.
     {
-        const int w = tid >> 5;
-        if (w < Ke) {
+        for (int w = tid >> 5; w < Ke; w += TG_NW) {
             const uint32_t* sf = I.sufMin + size_t(sm.isl[w]) * (L + 2);
             const uint32_t* sa = I.sufMinAll + size_t(sm.isl[w]) * (L + 2);
             unsigned nd = 0, nl = 0;
@@ -257,18 +262,15 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         // + 4 words per island: tables of different islands start in different 16-byte bank groups, so the
         // island groups of a warp do not collide when they read the same diagonal
         for (int kc = 0; kc < Ke; ++kc) { sm.baseK[kc] = acc; acc += uint32_t((sm.dmaxK[kc] + 3) & ~3) * uint32_t(Lp) + 4u; }
-        // dynamic shared memory of this item: every warp gets room for one mask's rows at the widest level
-        // (2 Ke - 1 rows), the cost rows come next if they still fit, and what is left doubles the warps'
-        // buffers so that two masks run side by side (tgWarpLevel<16>)
-        const int total = ctx.csWords + ctx.nActiveWarps * ctx.wbufWords;
-        const int perMask = max(1, 2 * Ke - 1) * tgRowStride(sm.sWd);
-        const int nWp = max(1, min(TG_NW, total / perMask));
-        sm.useGlobalC = acc > uint32_t(total - nWp * perMask) ? 1 : 0;
-        const int csUsed = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
-        sm.nWarps = nWp;
+        // dynamic shared memory of this item: the cost rows if a batch of at least 8 masks still fits behind them
+        // at the level that needs the most rows per mask (else the L2 fallback), the rest for the batches
+        const int HS = tgRowStride(sm.sWd), SS = tgSrcStride(sm.sWd);
+        int perMask = 0;
+        for (int r = 1; r < Ke; ++r) perMask = max(perMask, (Ke - r) * HS + 2 * r * SS);
+        perMask += 2 * TG_DESC_W + 2 * Ke;
+        sm.useGlobalC = int64_t(acc) + 16 + 8ll * perMask > int64_t(ctx.dynWords) ? 1 : 0;
         sm.csUsed4 = int(acc >> 2);
-        sm.wbufOff = csUsed;
-        sm.wbufWords = min(2 * perMask, (total - csUsed) / nWp) & ~3;
+        sm.batchOff = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
     }
     __syncthreads();
@@ -305,16 +307,22 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
 }
 
 // ---------------------------------------------------------------------------------------------
-// Levels r >= 1: one WARP per mask R, streaming over a contiguous range of masks (colexicographic
-// order, successor by Gosper's hack).  Nothing but the item's staged tables is shared between the
-// warps of a CTA, so a level needs no CTA barrier at all.  Per mask R (|R| = r, nk = Ke - r):
-//   issue   16-byte cp.async copies of the r source rows G_{r-1}[R\{j}][j][.] into the warp's
-//           shared-memory buffer, one mask ahead of their use (double buffer, commit / wait_group)
-//   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[j][b]       lane = (4 consecutive b) x (k group)
-//   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]    lane = (4 consecutive a) x (k group)
-// Warp-private shared memory: rows of Wd + 12 (+4 against bank conflicts) words: [0, nk) the H rows (4 INF | H[b] at index
-// b - lo4(R) | 8 INF), then two source buffers of r rows each.
+// Levels r >= 1: the CTA walks its share of the level's masks in BATCHES of NB masks (colexicographic
+// rank order).  Per batch, all threads of the CTA:
+//   prepass  (one thread per mask, one batch ahead)  mask R from its rank (table maskOf), cap(R) and the
+//            nibble lists of its members / non-members -> a 6-word descriptor in shared memory
+//   copies   16-byte cp.async (LDGSTS) of the batch's r source rows G_{r-1}[R\{j}][j][.] per mask into shared
+//            memory, one batch ahead of their use (double buffer); source row = rankOf[R\{j}] (table)
+//   phase 1  H[R][k][b] = min_{j in R} x[k][j] + src[j][b]          item = (mask, 4 consecutive b, NSL rows k)
+//            and, per row (R, k), an 8-byte row record appended to the list of island k
+//   phase 2  G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]       item = (row, 4 consecutive a), rows taken
+//            ISLAND BY ISLAND from the lists: the lanes of a warp then share the cost table of one island and
+//            run (nearly) the same number of diagonal blocks.  (Round 1 gave one warp one mask: its rows
+//            belong to different islands whose admissible diagonals differ by up to 19:1, and the ncu source
+//            page showed 10-14 of 32 lanes active in the min-plus loop.)
+// Two CTA barriers per batch.  Shared memory of a batch: [descriptors x2 | lists | H rows | source rows x2].
 // ---------------------------------------------------------------------------------------------
+
 __device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
 __device__ __forceinline__ uint4 tgLds4(uint32_t addr) {
@@ -331,111 +339,111 @@ __device__ __forceinline__ void tgSts4(uint32_t addr, uint4 v) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-// colexicographic unrank: rank -> mask with r bits among Ke (masks of one popcount ordered by value)
-__device__ __forceinline__ uint32_t tgUnrank(const TgShared& sm, uint32_t rank, int r, int Ke) {
-    uint32_t R = 0;
-    int e = Ke - 1;
-    for (int i = r; i >= 1; --i) {
-        while (uint32_t(sm.binom[e][i]) > rank) --e;
-        rank -= sm.binom[e][i];
-        R |= 1u << e;
-        --e;
-    }
-    return R;
-}
-// next mask with the same popcount (Gosper)
-__device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
-    const uint32_t c = R & (0u - R), t = R + c;
-    return (((R ^ t) >> 2) >> (__ffs(c) - 1)) | t;
-}
+// division of small numbers by a CTA-uniform divisor d: q = t / d for t * d < 2^32 (magic = ceil(2^32 / d), 0 for d = 1)
+__device__ __forceinline__ uint32_t tgMagic(uint32_t d) { return d <= 1u ? 0u : 0xffffffffu / d + 1u; }
+__device__ __forceinline__ uint32_t tgDivM(uint32_t t, uint32_t magic) { return magic ? __umulhi(t, magic) : t; }
 
-// Issue the copies of the r source rows of mask R into the warp's buffer: 16-byte asynchronous copies
-// (cp.async, LDGSTS), one lane per (source, chunk of 4 starts), committed as one group.  Source row of
-// member j = state (R\{j}, first island j) of level r-1, whose mask rank is
-//   sum_{i<p} C(e_i, i+1) + sum_{i>p} C(e_i, i)   (p = position of j in R: the elements below keep their
-// position, those above move down by one) -- two warp scans over the member lanes.
-// (Bulk TMA copies, one per row, were measured slower here: with row windows a row is often 32-64 bytes
-// and the per-SM TMA issue rate, not bandwidth, became the bound -- DESIGN.md 7.4.)
-// SW = lanes per mask (32, or 16 when a warp runs two masks side by side); sl = lane within the sub-warp;
-// `valid` = this sub-warp has a mask to issue (the shuffles are executed by every lane regardless).
-template <int SW>
-__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, bool valid, int r, int nk, int Wd, int nbw, int cpShift,
-                                            uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
-    const int sl = lane & (SW - 1);
-    const bool member = valid && ((R >> sl) & 1u);   // R < 2^16: lanes 16..31 of a full warp are never members
-    const int p = __popc(R & ((1u << sl) - 1u));
-    // both sums stay below C(16,8) = 12870, so they share one register: low half "kept position", high half "moved down"
-    const uint32_t mine = member ? (uint32_t(sm.binom[sl & 15][p + 1]) | uint32_t(sm.binom[sl & 15][p]) << 16) : 0u;
-    uint32_t incl = mine;
-#pragma unroll
-    for (int o = 1; o < 16; o <<= 1) {
-        const uint32_t a = __shfl_up_sync(0xffffffffu, incl, o);
-        if ((lane & 15) >= o) incl += a;
-    }
-    const uint32_t total = __shfl_sync(0xffffffffu, incl, (lane & 16) | 15);
-    if (member)
-        rowOf[p] = (((incl - mine) & 0xffffu) + ((total - incl) >> 16)) * uint32_t(nk + 1) + uint32_t(sl - p);
-    __syncwarp();
-    if (valid) {
-        const int CP = 1 << cpShift;   // chunks per row, rounded up to a power of two
-        for (int w = sl; w < (r << cpShift); w += SW) {
-            const int ji = w >> cpShift, ch = w & (CP - 1);
-            if (ch < nbw) {
-                const uint32_t* src = Gprev + size_t(rowOf[ji]) * Wd + 4 * ch;
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(bufAddr + uint32_t(ji) * rowBytes + uint32_t(ch) * 16u), "l"(src) : "memory");
-            }
+// prepass of one mask: descriptor from the mask's rank inside level r
+__device__ __forceinline__ void tgPrepassMask(const TgSolveCtx& ctx, const TgShared& sm, uint32_t* desc, uint32_t rank, int r, int Ke) {
+    const uint32_t R = __ldg(ctx.maskOf + tgPopOff[r] + rank);
+    uint32_t cap = 0, klLo = 0, klHi = 0, mlLo = 0, mlHi = 0;
+    int nm = 0, nc = 0;
+    for (int e = 0; e < Ke; ++e) {
+        if (R >> e & 1u) {
+            cap += sm.maxlenK[e];
+            if (nm < 8) mlLo |= uint32_t(e) << (4 * nm); else mlHi |= uint32_t(e) << (4 * (nm - 8));
+            ++nm;
+        } else {
+            if (nc < 8) klLo |= uint32_t(e) << (4 * nc); else klHi |= uint32_t(e) << (4 * (nc - 8));
+            ++nc;
         }
     }
+    desc[0] = R | cap << 16;
+    desc[2] = klLo; desc[3] = klHi; desc[4] = mlLo; desc[5] = mlHi;
 }
 
-#define TG_SPL 8   // k slots per lane handled together in phase 1 (accumulators: TG_SPL x 4)
+__device__ __forceinline__ uint32_t tgNibble(uint32_t lo, uint32_t hi, int i) { return ((i < 8 ? lo : hi) >> (4 * (i & 7))) & 15u; }
 
-// phase 1 for the NSL k slots  slot0, slot0+NG, ...  of this lane's island group and its b chunks:
-//   H[R][k][b] = min_{j in R} x[k][j] + src[j][b],  written to the warp's H rows.
-// All slots but the last are valid for every lane; an invalid last slot reads an all-INF x row.
-template <int NSL>
-__device__ __forceinline__ void tgPhase1(const TgShared& sm, uint32_t R, int r, int nk, int nb4, int c0, int CH, int NG,
-                                         int slot0, uint32_t srcAddr, uint32_t rowBytes, uint32_t hAddr0, const uint8_t* kl,
-                                         uint32_t xsBase, uint32_t xInfAddr) {
-    uint32_t xrow[NSL];
-#pragma unroll
-    for (int i = 0; i < NSL; ++i) {
-        const int s = slot0 + NG * i;
-        xrow[i] = (i + 1 < NSL || s < nk) ? xsBase + uint32_t(kl[s]) * (TG_MAX_K * 4u) : xInfAddr;
+// copies of a batch's source rows: item = (mask i, member ji, chunk of 4 starts), chunk fastest (coalesced 16-byte
+// pieces).  Source row of member j of R = state (R\{j}, first island j) of level r-1: mask rank from the table,
+// slot of j among the non-members of R\{j} = j - (members of R below j) = j - ji.
+__device__ __forceinline__ void tgIssueBatch(const TgSolveCtx& ctx, const uint32_t* desc, uint32_t srcAddr, const uint32_t* Gprev,
+                                             int nb, int r, int nk, int Wd, int nbw, uint32_t mNbw, uint32_t mR, uint32_t SSB) {
+    const int nItems = nb * r * nbw;
+    for (int t = threadIdx.x; t < nItems; t += TG_NT) {
+        const uint32_t pr = tgDivM(uint32_t(t), mNbw), ch = uint32_t(t) - pr * uint32_t(nbw);
+        const uint32_t i = tgDivM(pr, mR), ji = pr - i * uint32_t(r);
+        const uint32_t* d = desc + i * TG_DESC_W;
+        const uint32_t R = d[0] & 0xffffu, j = tgNibble(d[4], d[5], int(ji));
+        const uint32_t row = uint32_t(__ldg(ctx.rankOf + (R ^ (1u << j)))) * uint32_t(nk + 1) + (j - ji);
+        const uint32_t* src = Gprev + size_t(row) * Wd + 4u * ch;
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(srcAddr + pr * SSB + ch * 16u), "l"(src) : "memory");
     }
-    const bool lastValid = slot0 + NG * (NSL - 1) < nk;
-    for (int c = c0; c < nb4; c += CH) {
+    asm volatile("cp.async.commit_group;" ::: "memory");
+}
+
+#define TG_SPL 8   // most k slots (rows) a phase-1 item handles together (accumulators: TG_SPL x 4)
+
+// phase 1 of a batch.  Item = (mask i, chunk ch of 4 consecutive b, group sg of NSL rows): the chunk of every
+// source row is read once (LDS.128) and serves NSL rows; slots past the mask's last row read an all-INF x row.
+// The item of chunk 0 also files its rows in the island lists phase 2 works from:
+//   record = { row-in-batch | lo4(S)/4 << 16 | (lo4(R) - lo4(S))/4 << 24 ,  S = R u {k} }
+template <int NSL>
+__device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* desc, uint32_t srcAddr, uint32_t hAddr, uint2* list, int* cnt,
+                                          int nb, int r, int nk, int nbw, int nsg, uint32_t mNbw, uint32_t mNsg, uint32_t SSB,
+                                          uint32_t HSB, int NB, uint32_t xsBase, uint32_t xInfAddr) {
+    const int nItems = nb * nbw * nsg;
+    const int Lw = sm.sWindowed ? sm.sL : 0;
+    const uint4 inf4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+    for (int t = threadIdx.x; t < nItems; t += TG_NT) {
+        const uint32_t u = tgDivM(uint32_t(t), mNbw), ch = uint32_t(t) - u * uint32_t(nbw);
+        const uint32_t i = tgDivM(u, mNsg), sg = u - i * uint32_t(nsg);
+        const uint32_t* d = desc + i * TG_DESC_W;
+        const uint32_t w0 = d[0], klLo = d[2], klHi = d[3];
+        const uint32_t R = w0 & 0xffffu;
+        const int s0 = int(sg) * NSL;
+        uint32_t xrow[NSL];
+#pragma unroll
+        for (int e = 0; e < NSL; ++e)
+            xrow[e] = (s0 + e < nk) ? xsBase + tgNibble(klLo, klHi, s0 + e) * (TG_MAX_K * 4u) : xInfAddr;
         uint32_t acc[NSL][4];
 #pragma unroll
-        for (int i = 0; i < NSL; ++i) { acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = TG_INFU; }
-        const bool hasNx = c + 1 < nb4;
-        uint32_t sA = srcAddr + uint32_t(c) * 16u;
+        for (int e = 0; e < NSL; ++e) { acc[e][0] = acc[e][1] = acc[e][2] = acc[e][3] = TG_INFU; }
+        uint32_t sA = srcAddr + i * uint32_t(r) * SSB + ch * 16u;
         uint32_t Rb = R;
 #pragma unroll 2
         for (int ji = 0; ji < r; ++ji) {
             const uint32_t j4 = uint32_t(__ffs(Rb) - 1) * 4u;
             Rb &= Rb - 1;
             const uint4 g4 = tgLds4(sA);
-            sA += rowBytes;
+            sA += SSB;
 #pragma unroll
-            for (int i = 0; i < NSL; ++i) {
-                const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
-                acc[i][0] = tgAddMin(xv, g4.x, acc[i][0]);
-                acc[i][1] = tgAddMin(xv, g4.y, acc[i][1]);
-                acc[i][2] = tgAddMin(xv, g4.z, acc[i][2]);
-                acc[i][3] = tgAddMin(xv, g4.w, acc[i][3]);
+            for (int e = 0; e < NSL; ++e) {
+                const uint32_t xv = tgLds1(xrow[e] + j4);   // x[k][j]: k sends to j
+                acc[e][0] = tgAddMin(xv, g4.x, acc[e][0]);
+                acc[e][1] = tgAddMin(xv, g4.y, acc[e][1]);
+                acc[e][2] = tgAddMin(xv, g4.z, acc[e][2]);
+                acc[e][3] = tgAddMin(xv, g4.w, acc[e][3]);
             }
         }
+        const bool first = ch == 0, last = int(ch) + 1 == nbw;
 #pragma unroll
-        for (int i = 0; i < NSL; ++i) {
-            if (i + 1 < NSL || lastValid) {
-                // H row = [4 x INF | Wd values, H[b] at index b - lo4R | 8 x INF]
-                const uint32_t hA = hAddr0 + uint32_t(slot0 + NG * i) * rowBytes + 16u + uint32_t(c) * 16u;
-                tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));
-                if (c == 0) tgSts4(hA - 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
-                if (!hasNx) {
-                    tgSts4(hA + 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
-                    tgSts4(hA + 32, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+        for (int e = 0; e < NSL; ++e) {
+            const int s = s0 + e;
+            if (s < nk) {
+                // H row = [4 x INF | Wd values, H[b] at index b - lo4(R) | 8 x INF]
+                const uint32_t hrow = i * uint32_t(nk) + uint32_t(s);
+                const uint32_t hA = hAddr + hrow * HSB + 16u + ch * 16u;
+                tgSts4(hA, make_uint4(acc[e][0], acc[e][1], acc[e][2], acc[e][3]));
+                if (last) { tgSts4(hA + 16, inf4); tgSts4(hA + 32, inf4); }
+                if (first) {
+                    tgSts4(hA - 16, inf4);
+                    const uint32_t k = tgNibble(klLo, klHi, s);
+                    const int cap = int(w0 >> 16);
+                    const int lo4R = max(0, Lw - cap) & ~3, lo4S = max(0, Lw - cap - int(sm.maxlenK[k])) & ~3;
+                    const int pos = atomicAdd(&cnt[k], 1);
+                    list[k * uint32_t(NB) + uint32_t(pos)] =
+                        make_uint2(hrow | uint32_t(lo4S >> 2) << 16 | uint32_t((lo4R - lo4S) >> 2) << 24, R | (1u << k));
                 }
             }
         }
@@ -473,148 +481,142 @@ __device__ __forceinline__ void tgPhase1(const TgShared& sm, uint32_t R, int r, 
         dq += 4;                                                                               \
     }
 
-// phase 2 for this lane's rows (slots g, g+NG, ...) and a chunks of mask R:
-//   G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]
-// Row of (R u {k}, k) starts at start lo4S = lo4(capR + maxlen_k); the H row starts at b = lo4R, so
+// phase 2 of a batch.  Item = (row record e of island k's list, chunk cw of 4 consecutive a); the items are numbered
+// island by island, chunk fastest.  Row (S, k) begins at start lo4S = lo4(cap(S)); its H row begins at b = lo4R, so
 // H[a + d] sits at stored index (a - lo4S) + d - delta, delta = lo4R - lo4S (a multiple of 4).
 template <bool GLOBALC>
-__device__ __forceinline__ void tgPhase2(const TgSolveCtx& ctx, const TgShared& sm, uint32_t R, int capR, int nk, int nbw, int c0,
-                                         int CH, int NG, int g, uint32_t hAddr0, uint32_t rowBytes, uint32_t csBase,
-                                         uint32_t cStride, const uint8_t* kl, uint32_t* gRow, unsigned long long& bestKey) {
+__device__ __forceinline__ void tgPhase2B(const TgSolveCtx& ctx, const TgShared& sm, const uint2* list, const int* cnt, uint32_t hAddr,
+                                          uint32_t csBase, uint32_t* gBatch, int Ke, int nbw, uint32_t mNbw, uint32_t HSB,
+                                          uint32_t cStride, int NB, unsigned long long& bestKey) {
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int L = sm.sL, Lp = sm.sLp, Wd = sm.sWd;
     const uint32_t T = sm.sT;
-    const int Lw = sm.sWindowed ? L : 0;              // lo4(cap) = floor4(max(0, Lw - cap)): 0 when rows are not windowed
-    const int lo4R = max(0, Lw - capR) & ~3;
-    for (int s = g; s < nk; s += NG) {
-        const int k = kl[s];
-        const int lo4S = max(0, Lw - capR - int(sm.maxlenK[k])) & ~3, dq4 = (lo4R - lo4S) >> 2;
-        const uint32_t* cdk = GLOBALC ? I.cd + sm.cdOff + size_t(sm.isl[k]) * I.triG : nullptr;
-        const uint32_t cBase = csBase + (sm.baseK[k] + uint32_t(lo4S)) * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes + 16u;
-        uint32_t* const gOut = gRow + size_t(s) * Wd;
-        for (int cw = c0; cw < nbw; cw += CH) {
-            const int a0 = lo4S + 4 * cw, c = a0 >> 2;   // c = absolute tile of 4 starts
-            uint32_t out[4] = {TG_INFU, TG_INFU, TG_INFU, TG_INFU};
-            if (a0 < Lp) {
-                // blocks of 4 diagonals: from the first that reaches the H row to the last admissible one
-                // (never past the end of the H row: such entries lie right of this row's window)
-                const int dm = sm.dmaxTile[k][c], q0 = max(0, dq4 - 1 - cw);
-                const int nq = min((dm + 3) >> 2, nbw - cw + dq4 + 1);
-                if (q0 < nq) {
-                    uint32_t hA = hRow + uint32_t(4 * (cw + q0 - dq4)) * 4u;
-                    uint32_t cA = cBase + uint32_t(cw) * 16u + uint32_t(4 * q0) * cStride;
-                    int dq = 4 * q0;
-                    uint32_t Wa[4], Wb[4];
-                    {
-                        const uint4 h = tgLds4(hA);
-                        hA += 16;
-                        Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
-                    }
+    int k = 0, off = 0, end = cnt[0] * nbw;   // items of island k: [off, end)
+    for (int t = threadIdx.x;; t += TG_NT) {
+        while (t >= end) {
+            if (++k >= Ke) return;
+            off = end;
+            end += cnt[k] * nbw;
+        }
+        const uint32_t u = uint32_t(t - off), e = tgDivM(u, mNbw);
+        const int cw = int(u - e * uint32_t(nbw));
+        const uint2 info = list[uint32_t(k) * uint32_t(NB) + e];
+        const uint32_t hrow = info.x & 0xffffu;
+        const int lo4S = int(info.x >> 16 & 0xffu) << 2, dq4 = int(info.x >> 24);
+        const int a0 = lo4S + 4 * cw, c = a0 >> 2;   // c = absolute tile of 4 starts
+        uint32_t out[4] = {TG_INFU, TG_INFU, TG_INFU, TG_INFU};
+        if (a0 < Lp) {
+            // blocks of 4 diagonals: from the first that reaches the H row to the last admissible one
+            // (never past the end of the H row: such entries lie right of this row's window)
+            const int dm = sm.dmaxTile[k][c], q0 = max(0, dq4 - 1 - cw);
+            const int nq = min((dm + 3) >> 2, nbw - cw + dq4 + 1);
+            if (q0 < nq) {
+                const uint32_t* cdk = GLOBALC ? I.cd + sm.cdOff + size_t(sm.isl[k]) * I.triG : nullptr;
+                uint32_t hA = hAddr + hrow * HSB + 16u + uint32_t(4 * (cw + q0 - dq4)) * 4u;
+                uint32_t cA = csBase + (sm.baseK[k] + uint32_t(a0)) * 4u + uint32_t(4 * q0) * cStride;
+                int dq = 4 * q0;
+                uint32_t Wa[4], Wb[4];
+                {
+                    const uint4 h = tgLds4(hA);
+                    hA += 16;
+                    Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
+                }
 #pragma unroll 1
-                    for (int q = q0; q < nq; q += 2) {
-                        TG_P2_STEP(Wa, Wb)
-                        if (q + 1 >= nq) break;
-                        TG_P2_STEP(Wb, Wa)
-                    }
+                for (int q = q0; q < nq; q += 2) {
+                    TG_P2_STEP(Wa, Wb)
+                    if (q + 1 >= nq) break;
+                    TG_P2_STEP(Wb, Wa)
                 }
             }
-            *reinterpret_cast<uint4*>(gOut + 4 * cw) = make_uint4(out[0], out[1], out[2], out[3]);
-            if (a0 == 0 && out[0] < TG_INFU) {
-                const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)(R | (1u << k)) << 8 | (unsigned long long)k;
-                bestKey = kk < bestKey ? kk : bestKey;
-            }
+        }
+        *reinterpret_cast<uint4*>(gBatch + size_t(hrow) * Wd + 4 * cw) = make_uint4(out[0], out[1], out[2], out[3]);
+        if (a0 == 0 && out[0] < TG_INFU) {
+            const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)info.y << 8 | (unsigned long long)k;
+            bestKey = kk < bestKey ? kk : bestKey;
         }
     }
 }
 
-// One wavefront level for this warp's share of the masks.  SW = 32: one mask at a time on the whole warp.
-// SW = 16: two masks side by side, one per half warp (narrow row windows leave most of a full warp idle and
-// the per-mask bookkeeping -- successor, ranks, copies, windows -- then costs more than the relaxations;
-// two masks share every one of those instructions).  Each sub-warp owns a contiguous run of masks and its
-// own H rows and source buffers inside the warp's buffer.
-template <int SW>
-__device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
-                            uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW) {
-    constexpr int M = 32 / SW, SWSH = SW == 32 ? 5 : 4;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int sub = lane >> SWSH, sl = lane & (SW - 1);
+// One wavefront level for this CTA's share [lo, hi) of the level's masks (member `member` of a team of `teamSize`).
+// Pipeline per batch n (two CTA barriers):   wait copies(n) | barrier | issue copies(n+1) ; phase 1(n) | barrier |
+// phase 2(n) ; prepass(n+2).  Descriptors and source rows are double buffered; lists and H rows are single.
+__device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, const uint32_t* Gprev, uint32_t* Gcur,
+                               unsigned long long* key, int Ke, int r, int member, int teamSize) {
+    const int tid = threadIdx.x;
     const int Lp = sm.sLp, Wd = sm.sWd, nbw = Wd >> 2, nk = Ke - r;
-    const int HS = tgRowStride(Wd);
     const int nMasks = sm.binom[Ke][r];
-    const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
+    const int lo = int((int64_t(nMasks) * member) / teamSize), hi = int((int64_t(nMasks) * (member + 1)) / teamSize);
     if (lo >= hi) return;
-    const int per = (hi - lo + M - 1) / M;                       // masks per sub-warp
-    const int myLo = lo + sub * per, myHi = min(hi, myLo + per);
-    // sub-lane = (chunk of 4 starts) x (island group): CH chunk lanes, NG = SW / CH groups
-    const int cpShift = nbw <= 2 ? 1 : (nbw <= 4 ? 2 : (nbw <= 8 ? 3 : (nbw <= 16 ? 4 : (nbw <= 32 ? 5 : 6))));
-    const int chShift = min(cpShift, SWSH);
-    const int CH = 1 << chShift, NG = SW >> chShift;
-    const int c0 = sl & (CH - 1), g = sl >> chShift;
-    const uint32_t rowBytes = uint32_t(HS) * 4u, cStride = uint32_t(Lp) * 4u;
-    const uint32_t hAddr0 = tgSmemAddr(wbuf) + uint32_t(sub) * uint32_t(nk + 2 * r) * rowBytes;
-    const uint32_t csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
-    const uint32_t xInfAddr = tgSmemAddr(&sm.xInf[0]);
-    const uint32_t bufAddr[2] = {hAddr0 + uint32_t(nk) * rowBytes, hAddr0 + uint32_t(nk + r) * rowBytes};
-    uint32_t* rowOf = &sm.rowOf[warp][sub * TG_MAX_K];
-    uint8_t* kl = &sm.kl[warp][sub * TG_MAX_K];
-    const uint32_t keMask = (1u << Ke) - 1u;
-    const bool globalC = sm.useGlobalC != 0;
-    const int myLen = sl < Ke ? int(sm.maxlenK[sl & 15]) : 0;
-    unsigned long long bestKey = TG_KEY_NONE;
-
-    uint32_t R = myLo < myHi ? tgUnrank(sm, uint32_t(myLo), r, Ke) : 0u;
-    tgIssueMask<SW>(sm, R, myLo < myHi, r, nk, Wd, nbw, cpShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
-    asm volatile("cp.async.commit_group;" ::: "memory");
-    int b = 0;
-    for (int it = 0; it < per; ++it, b ^= 1) {
-        const int idx = myLo + it;
-        const bool valid = idx < myHi, more = idx + 1 < myHi;
-        const uint32_t Rn = more ? tgNextMask(R) : 0u;
-        tgIssueMask<SW>(sm, Rn, more, r, nk, Wd, nbw, cpShift, bufAddr[b ^ 1], rowBytes, Gprev, rowOf, lane);
-        asm volatile("cp.async.commit_group;" ::: "memory");   // possibly empty: keeps the group count uniform
-        const uint32_t comp = ~R & keMask;
-        if (valid && sl < Ke && (comp >> sl & 1u)) kl[__popc(comp & ((1u << sl) - 1u))] = uint8_t(sl);
-        int capR;                                               // cap(R) = sum of the members' longest slices
-        if (SW == 32) {
-            capR = int(__reduce_add_sync(0xffffffffu, (R >> sl & 1u) ? unsigned(myLen) : 0u));
-        } else {
-            capR = (R >> sl & 1u) ? myLen : 0;
-#pragma unroll
-            for (int o = SW / 2; o > 0; o >>= 1) capR += __shfl_xor_sync(0xffffffffu, capR, o);
+    const int HS = tgRowStride(Wd), SS = tgSrcStride(Wd);
+    if (tid == 0) {
+        // split of the shared memory behind the cost rows for this level
+        const int avail = ctx.dynWords - sm.batchOff;
+        const int perMask = nk * HS + 2 * r * SS + 2 * TG_DESC_W + 2 * Ke;
+        int NB = min(min(TG_NB_MAX, hi - lo), max(1, (avail - 16) / perMask));
+        // phase-1 items take NSL rows each: fewest CTA passes x instructions per item
+        int best = 1, bestCost = 0x7fffffff;
+        const int nbFull = min(NB, hi - lo);
+        for (int nsl = 1; nsl <= TG_SPL; nsl <<= 1) {
+            const int items = nbFull * nbw * ((nk + nsl - 1) / nsl);
+            const int cost = ((items + TG_NT - 1) / TG_NT) * (3 + 5 * nsl);
+            if (cost < bestCost) { bestCost = cost; best = nsl; }
         }
-        asm volatile("cp.async.wait_group 1;" ::: "memory");   // this mask's rows have landed (the next mask's may be in flight)
-        __syncwarp();
-
-        // ---- phase 1: transfer pre-minimum, H rows into the sub-warp's shared memory -----------
-        if (valid) {
-            for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
-                const int nsl = min(TG_SPL, (nk - s0 + NG - 1) >> (SWSH - chShift));   // slots of the widest island group
-#define TG_P1_CASE(N) case N: tgPhase1<N>(sm, R, r, nk, nbw, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
-                switch (nsl) {
-                    TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
-                    TG_P1_CASE(5) TG_P1_CASE(6) TG_P1_CASE(7) TG_P1_CASE(8)
-                }
-#undef TG_P1_CASE
-            }
-        }
-        __syncwarp();
-
-        // ---- phase 2: min-plus product with the thresholded cost rows ----------------------------
-        if (valid) {
-            uint32_t* const gRow = Gcur + size_t(idx) * nk * Wd;
-            if (globalC) tgPhase2<true>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
-            else tgPhase2<false>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
-        }
-        __syncwarp();
-        R = Rn;
+        sm.lvNB = NB; sm.lvNsl = best; sm.lvNsg = (nk + best - 1) / best;
+        sm.lvMagic[0] = tgMagic(uint32_t(nbw)); sm.lvMagic[1] = tgMagic(uint32_t(sm.lvNsg)); sm.lvMagic[2] = tgMagic(uint32_t(r));
+        uint32_t o = uint32_t(sm.batchOff);
+        sm.lvDesc[0] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3);
+        sm.lvDesc[1] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3);
+        sm.lvList = o; o += uint32_t((2 * Ke * NB + 3) & ~3);
+        sm.lvH = o; o += uint32_t(NB * nk * HS);
+        sm.lvSrc[0] = o; o += uint32_t(NB * r * SS);
+        sm.lvSrc[1] = o;
     }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (tid < 2 * TG_MAX_K) (&sm.cnt[0][0])[tid] = 0;
+    __syncthreads();
+    const int NB = sm.lvNB, nsl = sm.lvNsl, nsg = sm.lvNsg;
+    const uint32_t mNbw = sm.lvMagic[0], mNsg = sm.lvMagic[1], mR = sm.lvMagic[2];
+    uint32_t* const descB[2] = {dyn + sm.lvDesc[0], dyn + sm.lvDesc[1]};
+    uint2* const list = reinterpret_cast<uint2*>(dyn + sm.lvList);
+    const uint32_t hAddr = tgSmemAddr(dyn + sm.lvH);
+    const uint32_t srcAddr[2] = {tgSmemAddr(dyn + sm.lvSrc[0]), tgSmemAddr(dyn + sm.lvSrc[1])};
+    const uint32_t HSB = uint32_t(HS) * 4u, SSB = uint32_t(SS) * 4u, cStride = uint32_t(Lp) * 4u;
+    const uint32_t csBase = tgSmemAddr(dyn), xsBase = tgSmemAddr(&sm.xS[0][0]), xInfAddr = tgSmemAddr(&sm.xInf[0]);
+    const bool globalC = sm.useGlobalC != 0;
+    const int nBatches = (hi - lo + NB - 1) / NB;
+    unsigned long long bestKey = TG_KEY_NONE;
+    // the prepass runs on the threads that get the fewest phase-2 items (the last ones)
+    const int pi = TG_NT - 1 - tid;
+    for (int b = 0; b < 2 && b < nBatches; ++b) {
+        const int m0 = lo + b * NB;
+        if (pi < min(NB, hi - m0)) tgPrepassMask(ctx, sm, descB[b] + pi * TG_DESC_W, uint32_t(m0 + pi), r, Ke);
+    }
+    __syncthreads();
+    tgIssueBatch(ctx, descB[0], srcAddr[0], Gprev, min(NB, hi - lo), r, nk, Wd, nbw, mNbw, mR, SSB);
+    for (int n = 0; n < nBatches; ++n) {
+        const int m0 = lo + n * NB, nb = min(NB, hi - m0), par = n & 1;
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        __syncthreads();   // copies(n) have landed; descriptors(n+1) are visible; phase 2 of batch n-1 is over
+        if (n + 1 < nBatches)
+            tgIssueBatch(ctx, descB[par ^ 1], srcAddr[par ^ 1], Gprev, min(NB, hi - m0 - NB), r, nk, Wd, nbw, mNbw, mR, SSB);
+#define TG_P1_CASE(N) case N: tgPhase1B<N>(sm, descB[par], srcAddr[par], hAddr, list, sm.cnt[par], nb, r, nk, nbw, nsg, mNbw, mNsg, SSB, HSB, NB, xsBase, xInfAddr); break;
+        switch (nsl) { TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(4) TG_P1_CASE(8) }
+#undef TG_P1_CASE
+        __syncthreads();   // H rows and island lists of batch n are complete
+        uint32_t* const gBatch = Gcur + size_t(m0) * nk * Wd;
+        if (globalC) tgPhase2B<true>(ctx, sm, list, sm.cnt[par], hAddr, csBase, gBatch, Ke, nbw, mNbw, HSB, cStride, NB, bestKey);
+        else tgPhase2B<false>(ctx, sm, list, sm.cnt[par], hAddr, csBase, gBatch, Ke, nbw, mNbw, HSB, cStride, NB, bestKey);
+        if (n + 2 < nBatches) {
+            const int m2 = m0 + 2 * NB;
+            if (pi < min(NB, hi - m2)) tgPrepassMask(ctx, sm, descB[par] + pi * TG_DESC_W, uint32_t(m2 + pi), r, Ke);
+        }
+        if (tid < TG_MAX_K) sm.cnt[par ^ 1][tid] = 0;   // (used by batch n-1, needed empty by batch n+1)
+    }
     if (__any_sync(0xffffffffu, bestKey != TG_KEY_NONE)) {
         for (int o = 16; o > 0; o >>= 1) {
             const unsigned long long ot = __shfl_xor_sync(0xffffffffu, bestKey, o);
             bestKey = ot < bestKey ? ot : bestKey;
         }
-        if (lane == 0) atomicMin(key, bestKey);
+        if ((tid & 31) == 0) atomicMin(key, bestKey);
     }
 }
 
@@ -725,7 +727,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     tgMark(sm, 0);
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int Ke = sm.sSlack >= 0 ? sm.sKe : 0;   // the islands' longest slices cannot cover L layers: infeasible at T
-    const int Wd = sm.sWd, nW = sm.nWarps, warp = threadIdx.x >> 5;
+    const int Wd = sm.sWd;
     uint64_t bufWords = 0;   // words of one ping-pong half; 0 = keep every level (a back-track follows)
     if (Ke > 0 && !(__ldcg(&itp->flags) & 1)) {
         uint32_t mx = 1;
@@ -734,7 +736,6 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     }
     uint32_t* slot = ctx.scratch + uint64_t(slotIdx) * ctx.slotWords;
     uint32_t* bar = ctx.slotBar + slotIdx;
-    uint32_t* wbuf = wbufAll + sm.wbufOff + size_t(warp) * sm.wbufWords;   // (wbufAll = start of the dynamic shared memory)
     uint32_t arrivals = 0;
     if (Ke > 0) {
         tgLevel0(ctx, sm, slot, key, member == 0);
@@ -743,12 +744,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Wd, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Wd, r);
             if (I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
-            if (warp < nW) {
-                // two masks per warp when the windows are narrow and both masks' rows fit the warp's buffer
-                const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= sm.wbufWords;
-                if (pair) tgWarpLevel<16>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
-                else tgWarpLevel<32>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
-            }
+            tgLevelBatched(ctx, sm, wbufAll, Gprev, Gcur, key, Ke, r, member, teamSize);
             tgMark(sm, 3);
             if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();
@@ -768,7 +764,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
 // measured best at 8 (cfg4, K = 16) to 10-12 (cfg3, K = 12) probes a round.
 __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
     const int widest = tgBinom[K][K >> 1];
-    const int team = max(1, widest / (8 * ctx.nActiveWarps));
+    const int team = max(1, widest / (8 * TG_NW));
     return min(max(int(gridDim.x) / team, ctx.wishFloor), ctx.wishCap);
 }
 
@@ -1044,7 +1040,7 @@ __device__ void tgFoldPlanAll(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn
     P.items = itemsPrev; P.keys = keysPrev; P.keyS = nullptr; P.tidxS = nullptr; P.candS = nullptr; P.flagS = nullptr; P.nStage = 0;
     if (!wide) {   // stage keys, candidate indices, their thresholds and flags of the previous items in the (idle) dynamic shared memory
         const int nPrev = round > 0 ? ctrl->nItems[prv] : 0;
-        const int room = int((size_t(ctx.csWords) + size_t(ctx.nActiveWarps) * ctx.wbufWords) * 4 / 20);   // 17 bytes an item, padded
+        const int room = int(size_t(ctx.dynWords) * 4 / 20);   // 17 bytes an item, padded
         const int nStage = min(nPrev, room) & ~1;   // even: keeps the arrays behind the keys 8-byte aligned
         unsigned long long* keyS = reinterpret_cast<unsigned long long*>(dyn);
         int32_t* tidxS = reinterpret_cast<int32_t*>(keyS + nStage);
@@ -1072,7 +1068,7 @@ __device__ void tgFoldPlanAll(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn
     // back.  In global memory every field access of that single thread is a dependent L1/L2 access, and a store
     // invalidates the line the next load wants (the merge of the evaluated list paid one L2 trip per entry).
     constexpr int INST_W = int(sizeof(TgInstDev) / 4);
-    const size_t dynWords = size_t(ctx.csWords) + size_t(ctx.nActiveWarps) * ctx.wbufWords;
+    const size_t dynWords = size_t(ctx.dynWords);
     const bool local = !wide && ctx.nInst <= TG_SCHED_SMEM_INST &&
                        ((5 * size_t(P.nStage) + 3) & ~size_t(3)) + size_t(ctx.nInst) * (INST_W + 2 * TG_MAX_EVAL + TG_CAND_WIN) <= dynWords;
     uint32_t* sInst = dyn + ((5 * size_t(P.nStage) + 3) & ~size_t(3));   // behind the staged previous items (17 bytes each)
@@ -1198,7 +1194,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
     // ---- C: team sizes.  A few items share the grid as teams of CTAs; a DP's cost varies a lot with its
     // threshold (row-window width, islands alive) and with the instance shape, so the CTAs are dealt out in
     // proportion to an estimate of it:  masks x rows x (per-row bookkeeping + lanes a row's chunks occupy).
-    const bool weighted = nIt > 1 && nIt <= 32 && nIt < ctx.nSlots && gridDim.x <= 255;
+    const bool weighted = nIt > 1 && nIt <= 32 && nIt < ctx.nSlots && gridDim.x <= 1024;
     if (weighted) {
         const int lane = tid & 31, warp = tid >> 5;
         for (int t = warp; t < nIt; t += TG_NW) {
@@ -1260,8 +1256,8 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
             }
             beg -= n;
             if (tid < nIt) {
-                items[tid].ctaBeg = uint8_t(beg);
-                items[tid].ctaCnt = uint8_t(n);
+                items[tid].ctaBeg = uint16_t(beg);
+                items[tid].ctaCnt = uint16_t(n);
                 for (int c = beg; c < beg + n; ++c) ctrl->teamOf[par][c] = uint8_t(tid);
             }
         }
@@ -1289,7 +1285,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
 // ---------------------------------------------------------------------------------------------
 extern __shared__ uint4 tgDynSmem[];
 
-__global__ void __launch_bounds__(TG_NT, 1) tgSolveKernel(const TgSolveCtx ctx) {
+__global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgSolveCtx ctx) {
     __shared__ TgShared sm;
     uint32_t* dyn = reinterpret_cast<uint32_t*>(tgDynSmem);
     uint32_t* Cs = dyn;
