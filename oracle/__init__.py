@@ -172,12 +172,17 @@ def _args_variant(inst):
     return (keep, am), a[:6] + (amp,) + a[6:] + (C.c_int(1 if getattr(inst, "transfer_bound", False) else 0),)
 
 
-def solve_variant(inst) -> Result:
+def solve_variant(inst, n_threads: int = 0) -> Result:
     """Variants of SURVEY §8(f): NEXT-1 depth-aware memory (inst.actmem_mb) and NEXT-3(b) transfers bounded by
-    T (inst.transfer_bound), alone or together; with neither this is the core definition."""
+    T (inst.transfer_bound), alone or together; with neither this is the core definition.
+    n_threads > 0: the same arithmetic with the schedule of the core oracle's solve (bisection for the lowest feasible
+    threshold, blocks of n_threads DPs) -- for the K = 16 configs."""
     keep, a = _args_variant(inst)
     r = _Res()
-    lib().orc_variant_solve(*a, C.byref(r))
+    if n_threads > 0:
+        lib().orc_variant_solve_mt(*a, C.c_int(n_threads), C.byref(r))
+    else:
+        lib().orc_variant_solve(*a, C.byref(r))
     return _conv(r)
 
 

@@ -226,6 +226,72 @@ int orc_variant_solve(int L, int K, int P, int m, const int32_t* time_us, const 
     return 0;
 }
 
+// The same search with the schedule of the core oracle's orc_solve, for the K = 16 configs whose plain ascending sweep
+// from the lowest candidate would take hours: bisection for the lowest feasible candidate (feasibility is monotone in
+// T: every plan admissible at T stays admissible at T' > T, also with the footprint and the transfer bound, which only
+// restrict the set of plans per T), then the ascending sweep with the stop rule A7, evaluated in blocks of n_threads
+// independent DP(T) calls that are folded in ascending order with the sequential rules.  The arithmetic (reduce_tables,
+// candidates, run_dp, back-track) is that of orc_variant_solve; tests/test_oracle_depth.py pins the two against each
+// other (value, plan and the number of candidates) and both against the literal enumeration.
+int orc_variant_solve_mt(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                         const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, int xbound, int n_threads, orc_result* out) {
+    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, xbound};
+    Reduced R = reduce_tables(I);
+    std::vector<int64_t> cand = candidates(R, xbound != 0);
+    set_infeasible(out);
+    out->n_candidates = int(cand.size());
+    DP D0;
+    const Top tinf = run_dp(I, R, INF, D0, false);
+    if (tinf.best >= INF) return 0;
+    const int n = int(cand.size());
+    if (n_threads < 1) n_threads = 1;
+    int n_dp = 0;
+    int l = 0, r = n - 1;                    // cand[n-1] is feasible because f_inf is finite
+    while (l < r) {
+        const int mid = (l + r) / 2;
+        DP D; ++n_dp;
+        if (run_dp(I, R, cand[mid], D, false).best < INF) r = mid; else l = mid + 1;
+    }
+    bool have = false; int64_t best_iter = 0, best_T = 0;
+    std::vector<Top> res;
+    for (int i0 = l; i0 < n; i0 += n_threads) {
+        const int cnt = std::min(n_threads, n - i0);
+        if (have && tinf.best + int64_t(m - 1) * cand[i0] >= best_iter) break;            // A7
+        res.assign(cnt, Top{INF, 0, 0});
+        std::vector<std::thread> th;
+        for (int t = 0; t < cnt; ++t)
+            th.emplace_back([&, t] { DP D; res[t] = run_dp(I, R, cand[i0 + t], D, false); });
+        for (auto& x : th) x.join();
+        bool stop = false;
+        for (int t = 0; t < cnt; ++t) {
+            const int64_t T = cand[i0 + t];
+            if (have && tinf.best + int64_t(m - 1) * T >= best_iter) { stop = true; break; }
+            ++n_dp;
+            if (res[t].best >= INF) continue;
+            const int64_t it = res[t].best + int64_t(m - 1) * T;
+            if (!have || it < best_iter) { have = true; best_iter = it; best_T = T; }    // ties keep the lower T
+        }
+        if (stop) break;
+    }
+    DP D;
+    const Top t = run_dp(I, R, best_T, D, true);
+    out->iter_time_us = best_iter; out->sum_us = t.best; out->bottleneck_us = best_T;
+    out->island_mask = t.S; out->n_dp_run = n_dp;
+    int a = 0, k = t.k, ns = 0; uint32_t S = t.S;
+    while (true) {
+        const int b = D.gb[D.at(a, S, k)];
+        out->stage_begin[ns] = a; out->stage_island[ns] = k;
+        out->stage_plan[ns] = R.A(__builtin_popcount(S), sidx(L, a, b), k);
+        ++ns;
+        if (b == L) break;
+        const uint32_t Rm = S ^ (1u << k);
+        const int j = D.hj[D.at(b, Rm, k)];
+        a = b; S = Rm; k = j;
+    }
+    out->n_stages = ns;
+    return 0;
+}
+
 int orc_depth_solve(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
                     const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
     return orc_variant_solve(L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, 0, out);

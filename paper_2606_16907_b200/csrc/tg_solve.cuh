@@ -30,10 +30,14 @@ struct TgShared {
     int sWd, sSlack, sWindowed;
     // split of the dynamic shared memory for this item: [cost rows | batch buffers of the level (tgLevelBatched)]
     int batchOff;
-    uint32_t lvMagic[3];            // division magics of nbw, lvNsg, r
+    int nWarps, wbufWords, wbufOff;   // team mode: [cost rows | nWarps x wbufWords of warp-private row buffers]
+    uint32_t rowOf[TG_NW][2 * TG_MAX_K];   // team mode: source row of each member of the mask being issued (per half warp)
+    uint8_t kl[TG_NW][2 * TG_MAX_K];       // team mode: islands not in the current mask, ascending (per half warp)
+    uint32_t lvMagic[2];            // division magics of nbw, lvNsg
     int lvNB, lvNsl, lvNsg;         // level geometry: masks per batch, rows per phase-1 item, groups of them per mask
-    uint32_t lvDesc[2], lvList, lvH, lvSrc[2];   // word offsets of the batch buffers
-    int cnt[2][TG_MAX_K];           // rows filed in each island's list (per batch parity)
+    uint32_t lvDesc[2], lvSrcRow[2], lvList, lvH, lvSrc[2];   // word offsets of the batch buffers
+    int cntP[2][TG_MAX_K];          // rows of each island in a batch, counted by its prepass (per batch parity)
+    int cur[2][TG_MAX_K];           // next free list position of each island (starts at the prefix of the counts)
     int csUsed4;                    // 16-byte words of the staged cost rows of all islands (incl. the pads between them)
     uint32_t cdOff;                 // word offset of the reduced table of the depth currently staged
     uint8_t maxlenK[TG_MAX_K];      // longest admissible slice of island k at T, any position
@@ -197,7 +201,7 @@ __device__ __forceinline__ int tgSrcStride(int Wd) { return Wd + 4 + (((Wd + 4) 
 // multiple of 4 so that the min-plus loop needs no row predicate; uniform row stride Lp.
 // dmaxTile[k][t] = widest admissible diagonal of starts a = 4t..4t+3: bounds the phase-2 loop.
 // ---------------------------------------------------------------------------------------------
-__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t*, const TgItem* itp, bool count) {
+__device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t*, const TgItem* itp, bool count, bool team) {
     __syncthreads();
     unsigned nAdm = 0;   // admissible (a, b, k) cost entries with b <= L-1 seen by this thread
     const int tid = threadIdx.x, lane = tid & 31;
@@ -267,10 +271,22 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         const int HS = tgRowStride(sm.sWd), SS = tgSrcStride(sm.sWd);
         int perMask = 0;
         for (int r = 1; r < Ke; ++r) perMask = max(perMask, (Ke - r) * HS + 2 * r * SS);
-        perMask += 2 * TG_DESC_W + 2 * Ke;
+        perMask += 2 * TG_DESC_W + 4 * Ke;
         sm.useGlobalC = int64_t(acc) + 16 + 8ll * perMask > int64_t(ctx.dynWords) ? 1 : 0;
         sm.csUsed4 = int(acc >> 2);
         sm.batchOff = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
+        if (team) {
+            // team mode: every warp gets room for one mask's rows at the widest level (2 Ke - 1 rows), the cost rows come
+            // next if they still fit, and what is left doubles the warps' buffers so that two masks run side by side
+            const int total = ctx.dynWords;
+            const int perMaskW = max(1, 2 * Ke - 1) * HS;
+            const int nWp = max(1, min(TG_NW, total / perMaskW));
+            sm.useGlobalC = acc > uint32_t(total - nWp * perMaskW) ? 1 : 0;
+            const int csUsed = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
+            sm.nWarps = nWp;
+            sm.wbufOff = csUsed;
+            sm.wbufWords = min(2 * perMaskW, (total - csUsed) / nWp) & ~3;
+        }
         if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
     }
     __syncthreads();
@@ -343,40 +359,41 @@ __device__ __forceinline__ void tgSts4(uint32_t addr, uint4 v) {
 __device__ __forceinline__ uint32_t tgMagic(uint32_t d) { return d <= 1u ? 0u : 0xffffffffu / d + 1u; }
 __device__ __forceinline__ uint32_t tgDivM(uint32_t t, uint32_t magic) { return magic ? __umulhi(t, magic) : t; }
 
-// prepass of one mask: descriptor from the mask's rank inside level r
-__device__ __forceinline__ void tgPrepassMask(const TgSolveCtx& ctx, const TgShared& sm, uint32_t* desc, uint32_t rank, int r, int Ke) {
+// prepass of one mask: descriptor from the mask's rank inside level r, the rows of its r sources in level r-1 and one
+// count per non-member island (the island lists of phase 2 are laid out from these counts).
+// Source row of member j of R = state (R\{j}, first island j): mask rank from the table, slot of j among the
+// non-members of R\{j} = j - (members of R below j).
+__device__ __forceinline__ void tgPrepassMask(const TgSolveCtx& ctx, const TgShared& sm, uint32_t* desc, uint32_t* srcRow, int* cntP,
+                                              uint32_t rank, int r, int Ke) {
     const uint32_t R = __ldg(ctx.maskOf + tgPopOff[r] + rank);
-    uint32_t cap = 0, klLo = 0, klHi = 0, mlLo = 0, mlHi = 0;
+    uint32_t cap = 0, klLo = 0, klHi = 0;
     int nm = 0, nc = 0;
+    const int nk = Ke - r;
     for (int e = 0; e < Ke; ++e) {
         if (R >> e & 1u) {
             cap += sm.maxlenK[e];
-            if (nm < 8) mlLo |= uint32_t(e) << (4 * nm); else mlHi |= uint32_t(e) << (4 * (nm - 8));
+            srcRow[nm] = uint32_t(__ldg(ctx.rankOf + (R ^ (1u << e)))) * uint32_t(nk + 1) + uint32_t(e - nm);
             ++nm;
         } else {
             if (nc < 8) klLo |= uint32_t(e) << (4 * nc); else klHi |= uint32_t(e) << (4 * (nc - 8));
             ++nc;
+            atomicAdd(&cntP[e], 1);
         }
     }
     desc[0] = R | cap << 16;
-    desc[2] = klLo; desc[3] = klHi; desc[4] = mlLo; desc[5] = mlHi;
+    desc[2] = klLo; desc[3] = klHi;
 }
 
 __device__ __forceinline__ uint32_t tgNibble(uint32_t lo, uint32_t hi, int i) { return ((i < 8 ? lo : hi) >> (4 * (i & 7))) & 15u; }
 
-// copies of a batch's source rows: item = (mask i, member ji, chunk of 4 starts), chunk fastest (coalesced 16-byte
-// pieces).  Source row of member j of R = state (R\{j}, first island j) of level r-1: mask rank from the table,
-// slot of j among the non-members of R\{j} = j - (members of R below j) = j - ji.
-__device__ __forceinline__ void tgIssueBatch(const TgSolveCtx& ctx, const uint32_t* desc, uint32_t srcAddr, const uint32_t* Gprev,
-                                             int nb, int r, int nk, int Wd, int nbw, uint32_t mNbw, uint32_t mR, uint32_t SSB) {
+// copies of a batch's source rows: item = (source row pr = i * r + ji of the batch, chunk of 4 starts), chunk fastest
+// (coalesced 16-byte pieces); the row's index in level r-1 was looked up by the prepass.
+__device__ __forceinline__ void tgIssueBatch(const uint32_t* srcRow, uint32_t srcAddr, const uint32_t* Gprev, int nb, int r, int Wd,
+                                             int nbw, uint32_t mNbw, uint32_t SSB) {
     const int nItems = nb * r * nbw;
     for (int t = threadIdx.x; t < nItems; t += TG_NT) {
         const uint32_t pr = tgDivM(uint32_t(t), mNbw), ch = uint32_t(t) - pr * uint32_t(nbw);
-        const uint32_t i = tgDivM(pr, mR), ji = pr - i * uint32_t(r);
-        const uint32_t* d = desc + i * TG_DESC_W;
-        const uint32_t R = d[0] & 0xffffu, j = tgNibble(d[4], d[5], int(ji));
-        const uint32_t row = uint32_t(__ldg(ctx.rankOf + (R ^ (1u << j)))) * uint32_t(nk + 1) + (j - ji);
-        const uint32_t* src = Gprev + size_t(row) * Wd + 4u * ch;
+        const uint32_t* src = Gprev + size_t(srcRow[pr]) * Wd + 4u * ch;
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(srcAddr + pr * SSB + ch * 16u), "l"(src) : "memory");
     }
     asm volatile("cp.async.commit_group;" ::: "memory");
@@ -387,11 +404,11 @@ __device__ __forceinline__ void tgIssueBatch(const TgSolveCtx& ctx, const uint32
 // phase 1 of a batch.  Item = (mask i, chunk ch of 4 consecutive b, group sg of NSL rows): the chunk of every
 // source row is read once (LDS.128) and serves NSL rows; slots past the mask's last row read an all-INF x row.
 // The item of chunk 0 also files its rows in the island lists phase 2 works from:
-//   record = { row-in-batch | lo4(S)/4 << 16 | (lo4(R) - lo4(S))/4 << 24 ,  S = R u {k} }
+//   record = { row-in-batch | lo4(S)/4 << 16 | (lo4(R) - lo4(S))/4 << 24 ,  S = R u {k} | k << 16 }
 template <int NSL>
-__device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* desc, uint32_t srcAddr, uint32_t hAddr, uint2* list, int* cnt,
+__device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* desc, uint32_t srcAddr, uint32_t hAddr, uint2* list, int* cur,
                                           int nb, int r, int nk, int nbw, int nsg, uint32_t mNbw, uint32_t mNsg, uint32_t SSB,
-                                          uint32_t HSB, int NB, uint32_t xsBase, uint32_t xInfAddr) {
+                                          uint32_t HSB, uint32_t xsBase, uint32_t xInfAddr) {
     const int nItems = nb * nbw * nsg;
     const int Lw = sm.sWindowed ? sm.sL : 0;
     const uint4 inf4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
@@ -441,9 +458,8 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
                     const uint32_t k = tgNibble(klLo, klHi, s);
                     const int cap = int(w0 >> 16);
                     const int lo4R = max(0, Lw - cap) & ~3, lo4S = max(0, Lw - cap - int(sm.maxlenK[k])) & ~3;
-                    const int pos = atomicAdd(&cnt[k], 1);
-                    list[k * uint32_t(NB) + uint32_t(pos)] =
-                        make_uint2(hrow | uint32_t(lo4S >> 2) << 16 | uint32_t((lo4R - lo4S) >> 2) << 24, R | (1u << k));
+                    const int pos = atomicAdd(&cur[k], 1);   // island k's stretch of the list starts at its prefix count
+                    list[pos] = make_uint2(hrow | uint32_t(lo4S >> 2) << 16 | uint32_t((lo4R - lo4S) >> 2) << 24, R | (1u << k) | k << 16);
                 }
             }
         }
@@ -481,26 +497,21 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
         dq += 4;                                                                               \
     }
 
-// phase 2 of a batch.  Item = (row record e of island k's list, chunk cw of 4 consecutive a); the items are numbered
-// island by island, chunk fastest.  Row (S, k) begins at start lo4S = lo4(cap(S)); its H row begins at b = lo4R, so
-// H[a + d] sits at stored index (a - lo4S) + d - delta, delta = lo4R - lo4S (a multiple of 4).
+// phase 2 of a batch.  Item = (row record e, chunk cw of 4 consecutive a), chunk fastest; the records are sorted by
+// island (each island's stretch of the list was sized by the prepass).  Row (S, k) begins at start lo4S = lo4(cap(S));
+// its H row begins at b = lo4R, so H[a + d] sits at stored index (a - lo4S) + d - delta, delta = lo4R - lo4S (a multiple of 4).
 template <bool GLOBALC>
-__device__ __forceinline__ void tgPhase2B(const TgSolveCtx& ctx, const TgShared& sm, const uint2* list, const int* cnt, uint32_t hAddr,
-                                          uint32_t csBase, uint32_t* gBatch, int Ke, int nbw, uint32_t mNbw, uint32_t HSB,
-                                          uint32_t cStride, int NB, unsigned long long& bestKey) {
+__device__ __forceinline__ void tgPhase2B(const TgSolveCtx& ctx, const TgShared& sm, const uint2* list, int nItems, uint32_t hAddr,
+                                          uint32_t csBase, uint32_t* gBatch, int nbw, uint32_t mNbw, uint32_t HSB,
+                                          uint32_t cStride, unsigned long long& bestKey) {
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int L = sm.sL, Lp = sm.sLp, Wd = sm.sWd;
     const uint32_t T = sm.sT;
-    int k = 0, off = 0, end = cnt[0] * nbw;   // items of island k: [off, end)
-    for (int t = threadIdx.x;; t += TG_NT) {
-        while (t >= end) {
-            if (++k >= Ke) return;
-            off = end;
-            end += cnt[k] * nbw;
-        }
-        const uint32_t u = uint32_t(t - off), e = tgDivM(u, mNbw);
-        const int cw = int(u - e * uint32_t(nbw));
-        const uint2 info = list[uint32_t(k) * uint32_t(NB) + e];
+    for (int t = threadIdx.x; t < nItems; t += TG_NT) {
+        const uint32_t e = tgDivM(uint32_t(t), mNbw);
+        const int cw = int(uint32_t(t) - e * uint32_t(nbw));
+        const uint2 info = list[e];
+        const int k = int(info.y >> 16);
         const uint32_t hrow = info.x & 0xffffu;
         const int lo4S = int(info.x >> 16 & 0xffu) << 2, dq4 = int(info.x >> 24);
         const int a0 = lo4S + 4 * cw, c = a0 >> 2;   // c = absolute tile of 4 starts
@@ -531,15 +542,17 @@ __device__ __forceinline__ void tgPhase2B(const TgSolveCtx& ctx, const TgShared&
         }
         *reinterpret_cast<uint4*>(gBatch + size_t(hrow) * Wd + 4 * cw) = make_uint4(out[0], out[1], out[2], out[3]);
         if (a0 == 0 && out[0] < TG_INFU) {
-            const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)info.y << 8 | (unsigned long long)k;
+            const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)(info.y & 0xffffu) << 8 | (unsigned long long)k;
             bestKey = kk < bestKey ? kk : bestKey;
         }
     }
 }
 
 // One wavefront level for this CTA's share [lo, hi) of the level's masks (member `member` of a team of `teamSize`).
-// Pipeline per batch n (two CTA barriers):   wait copies(n) | barrier | issue copies(n+1) ; phase 1(n) | barrier |
-// phase 2(n) ; prepass(n+2).  Descriptors and source rows are double buffered; lists and H rows are single.
+// Pipeline per batch n (two CTA barriers):
+//   wait copies(n) | barrier | issue copies(n+1) ; phase 1(n) ; list cursors(n+1) | barrier | phase 2(n) ; prepass(n+2)
+// Descriptors, source-row indices, island counts / cursors and source rows are double buffered; the list and the H rows
+// are single.
 __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, const uint32_t* Gprev, uint32_t* Gcur,
                                unsigned long long* key, int Ke, int r, int member, int teamSize) {
     const int tid = threadIdx.x;
@@ -551,31 +564,31 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
     if (tid == 0) {
         // split of the shared memory behind the cost rows for this level
         const int avail = ctx.dynWords - sm.batchOff;
-        const int perMask = nk * HS + 2 * r * SS + 2 * TG_DESC_W + 2 * Ke;
-        int NB = min(min(TG_NB_MAX, hi - lo), max(1, (avail - 16) / perMask));
+        const int perMask = nk * HS + 2 * r * SS + 2 * TG_DESC_W + 2 * r + 2 * nk;
+        const int NB = min(min(TG_NB_MAX, hi - lo), max(1, (avail - 32) / perMask));
         // phase-1 items take NSL rows each: fewest CTA passes x instructions per item
         int best = 1, bestCost = 0x7fffffff;
-        const int nbFull = min(NB, hi - lo);
         for (int nsl = 1; nsl <= TG_SPL; nsl <<= 1) {
-            const int items = nbFull * nbw * ((nk + nsl - 1) / nsl);
+            const int items = NB * nbw * ((nk + nsl - 1) / nsl);
             const int cost = ((items + TG_NT - 1) / TG_NT) * (3 + 5 * nsl);
             if (cost < bestCost) { bestCost = cost; best = nsl; }
         }
         sm.lvNB = NB; sm.lvNsl = best; sm.lvNsg = (nk + best - 1) / best;
-        sm.lvMagic[0] = tgMagic(uint32_t(nbw)); sm.lvMagic[1] = tgMagic(uint32_t(sm.lvNsg)); sm.lvMagic[2] = tgMagic(uint32_t(r));
+        sm.lvMagic[0] = tgMagic(uint32_t(nbw)); sm.lvMagic[1] = tgMagic(uint32_t(sm.lvNsg));
         uint32_t o = uint32_t(sm.batchOff);
-        sm.lvDesc[0] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3);
-        sm.lvDesc[1] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3);
-        sm.lvList = o; o += uint32_t((2 * Ke * NB + 3) & ~3);
+        for (int b = 0; b < 2; ++b) { sm.lvDesc[b] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3); }
+        for (int b = 0; b < 2; ++b) { sm.lvSrcRow[b] = o; o += uint32_t((NB * r + 3) & ~3); }
+        sm.lvList = o; o += uint32_t((2 * nk * NB + 3) & ~3);
         sm.lvH = o; o += uint32_t(NB * nk * HS);
         sm.lvSrc[0] = o; o += uint32_t(NB * r * SS);
         sm.lvSrc[1] = o;
     }
-    if (tid < 2 * TG_MAX_K) (&sm.cnt[0][0])[tid] = 0;
+    if (tid < 2 * TG_MAX_K) (&sm.cntP[0][0])[tid] = 0;
     __syncthreads();
     const int NB = sm.lvNB, nsl = sm.lvNsl, nsg = sm.lvNsg;
-    const uint32_t mNbw = sm.lvMagic[0], mNsg = sm.lvMagic[1], mR = sm.lvMagic[2];
+    const uint32_t mNbw = sm.lvMagic[0], mNsg = sm.lvMagic[1];
     uint32_t* const descB[2] = {dyn + sm.lvDesc[0], dyn + sm.lvDesc[1]};
+    uint32_t* const srcRowB[2] = {dyn + sm.lvSrcRow[0], dyn + sm.lvSrcRow[1]};
     uint2* const list = reinterpret_cast<uint2*>(dyn + sm.lvList);
     const uint32_t hAddr = tgSmemAddr(dyn + sm.lvH);
     const uint32_t srcAddr[2] = {tgSmemAddr(dyn + sm.lvSrc[0]), tgSmemAddr(dyn + sm.lvSrc[1])};
@@ -586,30 +599,48 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
     unsigned long long bestKey = TG_KEY_NONE;
     // the prepass runs on the threads that get the fewest phase-2 items (the last ones)
     const int pi = TG_NT - 1 - tid;
-    for (int b = 0; b < 2 && b < nBatches; ++b) {
-        const int m0 = lo + b * NB;
-        if (pi < min(NB, hi - m0)) tgPrepassMask(ctx, sm, descB[b] + pi * TG_DESC_W, uint32_t(m0 + pi), r, Ke);
-    }
+    // list cursors of a batch = exclusive prefix of its island counts (lanes 0..15 of warp 0); the counts are cleared for
+    // the prepass that reuses the buffer two batches later
+    auto cursors = [&](int par) {
+        if (tid < 32) {
+            const int c = tid < Ke ? sm.cntP[par][tid] : 0;
+            int inc = c;
+#pragma unroll
+            for (int o = 1; o < 16; o <<= 1) {
+                const int a = __shfl_up_sync(0xffffffffu, inc, o);
+                if ((tid & 15) >= o) inc += a;
+            }
+            if (tid < TG_MAX_K) { sm.cur[par][tid] = inc - c; sm.cntP[par][tid] = 0; }
+        }
+    };
+    for (int pass = 0; pass <= (NB - 1) / TG_NT; ++pass)   // (NB <= TG_NT unless the CTA is built with fewer than 256 threads)
+        for (int b = 0; b < 2 && b < nBatches; ++b) {
+            const int m0 = lo + b * NB, i = pi + pass * TG_NT;
+            if (i < min(NB, hi - m0)) tgPrepassMask(ctx, sm, descB[b] + i * TG_DESC_W, srcRowB[b] + i * r, sm.cntP[b], uint32_t(m0 + i), r, Ke);
+        }
     __syncthreads();
-    tgIssueBatch(ctx, descB[0], srcAddr[0], Gprev, min(NB, hi - lo), r, nk, Wd, nbw, mNbw, mR, SSB);
+    cursors(0);
+    tgIssueBatch(srcRowB[0], srcAddr[0], Gprev, min(NB, hi - lo), r, Wd, nbw, mNbw, SSB);
     for (int n = 0; n < nBatches; ++n) {
         const int m0 = lo + n * NB, nb = min(NB, hi - m0), par = n & 1;
         asm volatile("cp.async.wait_all;" ::: "memory");
-        __syncthreads();   // copies(n) have landed; descriptors(n+1) are visible; phase 2 of batch n-1 is over
-        if (n + 1 < nBatches)
-            tgIssueBatch(ctx, descB[par ^ 1], srcAddr[par ^ 1], Gprev, min(NB, hi - m0 - NB), r, nk, Wd, nbw, mNbw, mR, SSB);
-#define TG_P1_CASE(N) case N: tgPhase1B<N>(sm, descB[par], srcAddr[par], hAddr, list, sm.cnt[par], nb, r, nk, nbw, nsg, mNbw, mNsg, SSB, HSB, NB, xsBase, xInfAddr); break;
+        __syncthreads();   // copies(n) have landed; descriptors / cursors of this batch are visible; phase 2 of batch n-1 is over
+        if (n + 1 < nBatches) {
+            tgIssueBatch(srcRowB[par ^ 1], srcAddr[par ^ 1], Gprev, min(NB, hi - m0 - NB), r, Wd, nbw, mNbw, SSB);
+            cursors(par ^ 1);
+        }
+#define TG_P1_CASE(N) case N: tgPhase1B<N>(sm, descB[par], srcAddr[par], hAddr, list, sm.cur[par], nb, r, nk, nbw, nsg, mNbw, mNsg, SSB, HSB, xsBase, xInfAddr); break;
         switch (nsl) { TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(4) TG_P1_CASE(8) }
 #undef TG_P1_CASE
-        __syncthreads();   // H rows and island lists of batch n are complete
+        __syncthreads();   // H rows and the island-sorted list of batch n are complete
         uint32_t* const gBatch = Gcur + size_t(m0) * nk * Wd;
-        if (globalC) tgPhase2B<true>(ctx, sm, list, sm.cnt[par], hAddr, csBase, gBatch, Ke, nbw, mNbw, HSB, cStride, NB, bestKey);
-        else tgPhase2B<false>(ctx, sm, list, sm.cnt[par], hAddr, csBase, gBatch, Ke, nbw, mNbw, HSB, cStride, NB, bestKey);
+        if (globalC) tgPhase2B<true>(ctx, sm, list, nb * nk * nbw, hAddr, csBase, gBatch, nbw, mNbw, HSB, cStride, bestKey);
+        else tgPhase2B<false>(ctx, sm, list, nb * nk * nbw, hAddr, csBase, gBatch, nbw, mNbw, HSB, cStride, bestKey);
         if (n + 2 < nBatches) {
             const int m2 = m0 + 2 * NB;
-            if (pi < min(NB, hi - m2)) tgPrepassMask(ctx, sm, descB[par] + pi * TG_DESC_W, uint32_t(m2 + pi), r, Ke);
+            for (int i = pi; i < min(NB, hi - m2); i += TG_NT)
+                tgPrepassMask(ctx, sm, descB[par] + i * TG_DESC_W, srcRowB[par] + i * r, sm.cntP[par], uint32_t(m2 + i), r, Ke);
         }
-        if (tid < TG_MAX_K) sm.cnt[par ^ 1][tid] = 0;   // (used by batch n-1, needed empty by batch n+1)
     }
     if (__any_sync(0xffffffffu, bestKey != TG_KEY_NONE)) {
         for (int o = 16; o > 0; o >>= 1) {
@@ -617,6 +648,271 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
             bestKey = ot < bestKey ? ot : bestKey;
         }
         if ((tid & 31) == 0) atomicMin(key, bestKey);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Levels r >= 1 of a DP that a TEAM of CTAs shares (few instances: cfg3 / cfg4): one WARP per mask, streaming over a
+// contiguous range of masks (colexicographic order, successor by Gosper's hack); nothing but the item's staged tables is
+// shared between the warps of a CTA, so a level needs no CTA barrier at all.  Per mask R (|R| = r, nk = Ke - r):
+//   issue   16-byte cp.async copies of the r source rows G_{r-1}[R\{j}][j][.] into the warp's
+//           shared-memory buffer, one mask ahead of their use (double buffer, commit / wait_group)
+//   phase 1 H[R][k][b] = min_{j in R} x[k][j] + src[j][b]       lane = (4 consecutive b) x (k group)
+//   phase 2 G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]    lane = (4 consecutive a) x (k group)
+// A team's share of a level is dozens of small batches per CTA; measured at cfg4 the CTA-wide batches above (1.60 ms),
+// the same batches per warp (2.04 ms) and this streaming form (1.40 ms), so the team keeps it.
+// ---------------------------------------------------------------------------------------------
+// colexicographic unrank: rank -> mask with r bits among Ke (masks of one popcount ordered by value)
+__device__ __forceinline__ uint32_t tgUnrank(const TgShared& sm, uint32_t rank, int r, int Ke) {
+    uint32_t R = 0;
+    int e = Ke - 1;
+    for (int i = r; i >= 1; --i) {
+        while (uint32_t(sm.binom[e][i]) > rank) --e;
+        rank -= sm.binom[e][i];
+        R |= 1u << e;
+        --e;
+    }
+    return R;
+}
+// next mask with the same popcount (Gosper)
+__device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
+    const uint32_t c = R & (0u - R), t = R + c;
+    return (((R ^ t) >> 2) >> (__ffs(c) - 1)) | t;
+}
+
+// Issue the copies of the r source rows of mask R into the warp's buffer: 16-byte asynchronous copies
+// (cp.async, LDGSTS), one lane per (source, chunk of 4 starts), committed as one group.  Source row of
+// member j = state (R\{j}, first island j) of level r-1, whose mask rank is
+//   sum_{i<p} C(e_i, i+1) + sum_{i>p} C(e_i, i)   (p = position of j in R: the elements below keep their
+// position, those above move down by one) -- two warp scans over the member lanes.
+// (Bulk TMA copies, one per row, were measured slower here: with row windows a row is often 32-64 bytes
+// and the per-SM TMA issue rate, not bandwidth, became the bound -- DESIGN.md 7.4.)
+// SW = lanes per mask (32, or 16 when a warp runs two masks side by side); sl = lane within the sub-warp;
+// `valid` = this sub-warp has a mask to issue (the shuffles are executed by every lane regardless).
+template <int SW>
+__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, bool valid, int r, int nk, int Wd, int nbw, int cpShift,
+                                            uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
+    const int sl = lane & (SW - 1);
+    const bool member = valid && ((R >> sl) & 1u);   // R < 2^16: lanes 16..31 of a full warp are never members
+    const int p = __popc(R & ((1u << sl) - 1u));
+    // both sums stay below C(16,8) = 12870, so they share one register: low half "kept position", high half "moved down"
+    const uint32_t mine = member ? (uint32_t(sm.binom[sl & 15][p + 1]) | uint32_t(sm.binom[sl & 15][p]) << 16) : 0u;
+    uint32_t incl = mine;
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        const uint32_t a = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((lane & 15) >= o) incl += a;
+    }
+    const uint32_t total = __shfl_sync(0xffffffffu, incl, (lane & 16) | 15);
+    if (member)
+        rowOf[p] = (((incl - mine) & 0xffffu) + ((total - incl) >> 16)) * uint32_t(nk + 1) + uint32_t(sl - p);
+    __syncwarp();
+    if (valid) {
+        const int CP = 1 << cpShift;   // chunks per row, rounded up to a power of two
+        for (int w = sl; w < (r << cpShift); w += SW) {
+            const int ji = w >> cpShift, ch = w & (CP - 1);
+            if (ch < nbw) {
+                const uint32_t* src = Gprev + size_t(rowOf[ji]) * Wd + 4 * ch;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(bufAddr + uint32_t(ji) * rowBytes + uint32_t(ch) * 16u), "l"(src) : "memory");
+            }
+        }
+    }
+}
+
+// phase 1 for the NSL k slots  slot0, slot0+NG, ...  of this lane's island group and its b chunks:
+//   H[R][k][b] = min_{j in R} x[k][j] + src[j][b],  written to the warp's H rows.
+// All slots but the last are valid for every lane; an invalid last slot reads an all-INF x row.
+template <int NSL>
+__device__ __forceinline__ void tgPhase1W(const TgShared& sm, uint32_t R, int r, int nk, int nb4, int c0, int CH, int NG,
+                                         int slot0, uint32_t srcAddr, uint32_t rowBytes, uint32_t hAddr0, const uint8_t* kl,
+                                         uint32_t xsBase, uint32_t xInfAddr) {
+    uint32_t xrow[NSL];
+#pragma unroll
+    for (int i = 0; i < NSL; ++i) {
+        const int s = slot0 + NG * i;
+        xrow[i] = (i + 1 < NSL || s < nk) ? xsBase + uint32_t(kl[s]) * (TG_MAX_K * 4u) : xInfAddr;
+    }
+    const bool lastValid = slot0 + NG * (NSL - 1) < nk;
+    for (int c = c0; c < nb4; c += CH) {
+        uint32_t acc[NSL][4];
+#pragma unroll
+        for (int i = 0; i < NSL; ++i) { acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = TG_INFU; }
+        const bool hasNx = c + 1 < nb4;
+        uint32_t sA = srcAddr + uint32_t(c) * 16u;
+        uint32_t Rb = R;
+#pragma unroll 2
+        for (int ji = 0; ji < r; ++ji) {
+            const uint32_t j4 = uint32_t(__ffs(Rb) - 1) * 4u;
+            Rb &= Rb - 1;
+            const uint4 g4 = tgLds4(sA);
+            sA += rowBytes;
+#pragma unroll
+            for (int i = 0; i < NSL; ++i) {
+                const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
+                acc[i][0] = tgAddMin(xv, g4.x, acc[i][0]);
+                acc[i][1] = tgAddMin(xv, g4.y, acc[i][1]);
+                acc[i][2] = tgAddMin(xv, g4.z, acc[i][2]);
+                acc[i][3] = tgAddMin(xv, g4.w, acc[i][3]);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NSL; ++i) {
+            if (i + 1 < NSL || lastValid) {
+                // H row = [4 x INF | Wd values, H[b] at index b - lo4R | 8 x INF]
+                const uint32_t hA = hAddr0 + uint32_t(slot0 + NG * i) * rowBytes + 16u + uint32_t(c) * 16u;
+                tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));
+                if (c == 0) tgSts4(hA - 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+                if (!hasNx) {
+                    tgSts4(hA + 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+                    tgSts4(hA + 32, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
+                }
+            }
+        }
+    }
+}
+
+// phase 2 for this lane's rows (slots g, g+NG, ...) and a chunks of mask R:
+//   G_r[R][k][a] = min_{b>a} Cs_k[a][b] + H[R][k][b]
+// Row of (R u {k}, k) starts at start lo4S = lo4(capR + maxlen_k); the H row starts at b = lo4R, so
+// H[a + d] sits at stored index (a - lo4S) + d - delta, delta = lo4R - lo4S (a multiple of 4).
+template <bool GLOBALC>
+__device__ __forceinline__ void tgPhase2W(const TgSolveCtx& ctx, const TgShared& sm, uint32_t R, int capR, int nk, int nbw, int c0,
+                                         int CH, int NG, int g, uint32_t hAddr0, uint32_t rowBytes, uint32_t csBase,
+                                         uint32_t cStride, const uint8_t* kl, uint32_t* gRow, unsigned long long& bestKey) {
+    const TgInstDev& I = ctx.inst[sm.sInst];
+    const int L = sm.sL, Lp = sm.sLp, Wd = sm.sWd;
+    const uint32_t T = sm.sT;
+    const int Lw = sm.sWindowed ? L : 0;              // lo4(cap) = floor4(max(0, Lw - cap)): 0 when rows are not windowed
+    const int lo4R = max(0, Lw - capR) & ~3;
+    for (int s = g; s < nk; s += NG) {
+        const int k = kl[s];
+        const int lo4S = max(0, Lw - capR - int(sm.maxlenK[k])) & ~3, dq4 = (lo4R - lo4S) >> 2;
+        const uint32_t* cdk = GLOBALC ? I.cd + sm.cdOff + size_t(sm.isl[k]) * I.triG : nullptr;
+        const uint32_t cBase = csBase + (sm.baseK[k] + uint32_t(lo4S)) * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes + 16u;
+        uint32_t* const gOut = gRow + size_t(s) * Wd;
+        for (int cw = c0; cw < nbw; cw += CH) {
+            const int a0 = lo4S + 4 * cw, c = a0 >> 2;   // c = absolute tile of 4 starts
+            uint32_t out[4] = {TG_INFU, TG_INFU, TG_INFU, TG_INFU};
+            if (a0 < Lp) {
+                // blocks of 4 diagonals: from the first that reaches the H row to the last admissible one
+                // (never past the end of the H row: such entries lie right of this row's window)
+                const int dm = sm.dmaxTile[k][c], q0 = max(0, dq4 - 1 - cw);
+                const int nq = min((dm + 3) >> 2, nbw - cw + dq4 + 1);
+                if (q0 < nq) {
+                    uint32_t hA = hRow + uint32_t(4 * (cw + q0 - dq4)) * 4u;
+                    uint32_t cA = cBase + uint32_t(cw) * 16u + uint32_t(4 * q0) * cStride;
+                    int dq = 4 * q0;
+                    uint32_t Wa[4], Wb[4];
+                    {
+                        const uint4 h = tgLds4(hA);
+                        hA += 16;
+                        Wa[0] = h.x; Wa[1] = h.y; Wa[2] = h.z; Wa[3] = h.w;
+                    }
+#pragma unroll 1
+                    for (int q = q0; q < nq; q += 2) {
+                        TG_P2_STEP(Wa, Wb)
+                        if (q + 1 >= nq) break;
+                        TG_P2_STEP(Wb, Wa)
+                    }
+                }
+            }
+            *reinterpret_cast<uint4*>(gOut + 4 * cw) = make_uint4(out[0], out[1], out[2], out[3]);
+            if (a0 == 0 && out[0] < TG_INFU) {
+                const unsigned long long kk = (unsigned long long)out[0] << 32 | (unsigned long long)(R | (1u << k)) << 8 | (unsigned long long)k;
+                bestKey = kk < bestKey ? kk : bestKey;
+            }
+        }
+    }
+}
+
+// One wavefront level for this warp's share of the masks.  SW = 32: one mask at a time on the whole warp.
+// SW = 16: two masks side by side, one per half warp (narrow row windows leave most of a full warp idle and
+// the per-mask bookkeeping -- successor, ranks, copies, windows -- then costs more than the relaxations;
+// two masks share every one of those instructions).  Each sub-warp owns a contiguous run of masks and its
+// own H rows and source buffers inside the warp's buffer.
+template <int SW>
+__device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
+                            uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW) {
+    constexpr int M = 32 / SW, SWSH = SW == 32 ? 5 : 4;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int sub = lane >> SWSH, sl = lane & (SW - 1);
+    const int Lp = sm.sLp, Wd = sm.sWd, nbw = Wd >> 2, nk = Ke - r;
+    const int HS = tgRowStride(Wd);
+    const int nMasks = sm.binom[Ke][r];
+    const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
+    if (lo >= hi) return;
+    const int per = (hi - lo + M - 1) / M;                       // masks per sub-warp
+    const int myLo = lo + sub * per, myHi = min(hi, myLo + per);
+    // sub-lane = (chunk of 4 starts) x (island group): CH chunk lanes, NG = SW / CH groups
+    const int cpShift = nbw <= 2 ? 1 : (nbw <= 4 ? 2 : (nbw <= 8 ? 3 : (nbw <= 16 ? 4 : (nbw <= 32 ? 5 : 6))));
+    const int chShift = min(cpShift, SWSH);
+    const int CH = 1 << chShift, NG = SW >> chShift;
+    const int c0 = sl & (CH - 1), g = sl >> chShift;
+    const uint32_t rowBytes = uint32_t(HS) * 4u, cStride = uint32_t(Lp) * 4u;
+    const uint32_t hAddr0 = tgSmemAddr(wbuf) + uint32_t(sub) * uint32_t(nk + 2 * r) * rowBytes;
+    const uint32_t csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
+    const uint32_t xInfAddr = tgSmemAddr(&sm.xInf[0]);
+    const uint32_t bufAddr[2] = {hAddr0 + uint32_t(nk) * rowBytes, hAddr0 + uint32_t(nk + r) * rowBytes};
+    uint32_t* rowOf = &sm.rowOf[warp][sub * TG_MAX_K];
+    uint8_t* kl = &sm.kl[warp][sub * TG_MAX_K];
+    const uint32_t keMask = (1u << Ke) - 1u;
+    const bool globalC = sm.useGlobalC != 0;
+    const int myLen = sl < Ke ? int(sm.maxlenK[sl & 15]) : 0;
+    unsigned long long bestKey = TG_KEY_NONE;
+
+    uint32_t R = myLo < myHi ? tgUnrank(sm, uint32_t(myLo), r, Ke) : 0u;
+    tgIssueMask<SW>(sm, R, myLo < myHi, r, nk, Wd, nbw, cpShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    int b = 0;
+    for (int it = 0; it < per; ++it, b ^= 1) {
+        const int idx = myLo + it;
+        const bool valid = idx < myHi, more = idx + 1 < myHi;
+        const uint32_t Rn = more ? tgNextMask(R) : 0u;
+        tgIssueMask<SW>(sm, Rn, more, r, nk, Wd, nbw, cpShift, bufAddr[b ^ 1], rowBytes, Gprev, rowOf, lane);
+        asm volatile("cp.async.commit_group;" ::: "memory");   // possibly empty: keeps the group count uniform
+        const uint32_t comp = ~R & keMask;
+        if (valid && sl < Ke && (comp >> sl & 1u)) kl[__popc(comp & ((1u << sl) - 1u))] = uint8_t(sl);
+        int capR;                                               // cap(R) = sum of the members' longest slices
+        if (SW == 32) {
+            capR = int(__reduce_add_sync(0xffffffffu, (R >> sl & 1u) ? unsigned(myLen) : 0u));
+        } else {
+            capR = (R >> sl & 1u) ? myLen : 0;
+#pragma unroll
+            for (int o = SW / 2; o > 0; o >>= 1) capR += __shfl_xor_sync(0xffffffffu, capR, o);
+        }
+        asm volatile("cp.async.wait_group 1;" ::: "memory");   // this mask's rows have landed (the next mask's may be in flight)
+        __syncwarp();
+
+        // ---- phase 1: transfer pre-minimum, H rows into the sub-warp's shared memory -----------
+        if (valid) {
+            for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
+                const int nsl = min(TG_SPL, (nk - s0 + NG - 1) >> (SWSH - chShift));   // slots of the widest island group
+#define TG_P1_CASE(N) case N: tgPhase1W<N>(sm, R, r, nk, nbw, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
+                switch (nsl) {
+                    TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
+                    TG_P1_CASE(5) TG_P1_CASE(6) TG_P1_CASE(7) TG_P1_CASE(8)
+                }
+#undef TG_P1_CASE
+            }
+        }
+        __syncwarp();
+
+        // ---- phase 2: min-plus product with the thresholded cost rows ----------------------------
+        if (valid) {
+            uint32_t* const gRow = Gcur + size_t(idx) * nk * Wd;
+            if (globalC) tgPhase2W<true>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+            else tgPhase2W<false>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
+        }
+        __syncwarp();
+        R = Rn;
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (__any_sync(0xffffffffu, bestKey != TG_KEY_NONE)) {
+        for (int o = 16; o > 0; o >>= 1) {
+            const unsigned long long ot = __shfl_xor_sync(0xffffffffu, bestKey, o);
+            bestKey = ot < bestKey ? ot : bestKey;
+        }
+        if (lane == 0) atomicMin(key, bestKey);
     }
 }
 
@@ -723,7 +1019,7 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
 // ---------------------------------------------------------------------------------------------
 __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uint32_t* wbufAll, const TgItem* itp,
                           unsigned long long* key, int member, int teamSize, int slotIdx, int itemIdx) {
-    tgStageItem(ctx, sm, Cs, wbufAll, itp, member == 0);
+    tgStageItem(ctx, sm, Cs, wbufAll, itp, member == 0, teamSize > 1);
     tgMark(sm, 0);
     const TgInstDev& I = ctx.inst[sm.sInst];
     const int Ke = sm.sSlack >= 0 ? sm.sKe : 0;   // the islands' longest slices cannot cover L layers: infeasible at T
@@ -744,7 +1040,18 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Wd, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Wd, r);
             if (I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
-            tgLevelBatched(ctx, sm, wbufAll, Gprev, Gcur, key, Ke, r, member, teamSize);
+            if (teamSize > 1) {
+                const int warp = threadIdx.x >> 5, nW = sm.nWarps;
+                if (warp < nW) {
+                    uint32_t* wbuf = wbufAll + sm.wbufOff + size_t(warp) * sm.wbufWords;
+                    // two masks per warp when the windows are narrow and both masks' rows fit the warp's buffer
+                    const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= sm.wbufWords;
+                    if (pair) tgWarpLevel<16>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
+                    else tgWarpLevel<32>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
+                }
+            } else {
+                tgLevelBatched(ctx, sm, wbufAll, Gprev, Gcur, key, Ke, r, member, teamSize);
+            }
             tgMark(sm, 3);
             if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();

@@ -118,3 +118,23 @@ def test_hand_worked_transfer_bound():
     core, xb = oracle.solve(b), oracle.solve_variant(gen.with_transfer_bound(b))
     assert (core.iter_time_us, core.bottleneck_us, core.sum_us) == (145, 10, 55)
     assert (xb.iter_time_us, xb.bottleneck_us, xb.sum_us, xb.island_mask, xb.stages) == (300, 30, 30, 1, [(0, 0, 0)])
+
+
+@pytest.mark.parametrize("style", ["mixed", "ties", "tightmem", "asym", "sparse"])
+def test_threaded_variant_solve_equals_sequential_and_bruteforce(style):
+    """orc_variant_solve_mt (bisection + blocks of threads, used for the K = 16 goldens) against the plain ascending
+    sweep and against the literal enumeration: value, plan and candidate count, with and without either variant."""
+    for s in range(60):
+        inst = gen.random_small(4000 + s, Lmax=7, Kmax=5, Pmax=3, style=style)
+        if s % 2:
+            inst = gen.with_actmem(inst, s, 0, 40)
+        if s % 3 == 0:
+            inst = gen.with_transfer_bound(inst)
+        seq = oracle.solve_variant(inst)
+        for nt in (1, 3):
+            mt = oracle.solve_variant(inst, nt)
+            assert mt.plan_key() == seq.plan_key() and mt.n_candidates == seq.n_candidates, inst.name
+        if inst.actmem_mb is None:
+            inst.actmem_mb = np.zeros_like(inst.time_us)
+        bf = oracle.bruteforce_variant(inst)
+        assert bf.plan_key() == seq.plan_key(), inst.name
