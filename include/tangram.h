@@ -143,9 +143,14 @@ typedef struct { /* optional diagnostics of one tg_solve_batch_ex call, written 
     uint64_t n_items_global_c; /* DPs whose cost tables did not fit in shared memory           */
     uint64_t error_flag;     /* internal consistency flag of the solver, 0 = none                */
     uint64_t relax_admissible; /* admissible relaxations executed: stage (c <= T) + transfer, summed over DPs */
-    uint64_t cyc[8];         /* SM cycles summed over CTAs (thread 0 of each): 0 cost-table staging, 3 DP levels
-                                (streaming over masks), 4 wait at the level barrier (team or CTA), 5 wait at the
-                                grid barrier between rounds, 6 scheduler, 7 back-track; 1, 2 unused         */
+    uint64_t states_windowed;  /* DP states the kernel actually wrote: sum over DPs of Ke*2^(Ke-1) rows x the row window */
+    /* SM cycles summed over the solver's CTAs (thread 0 of each): */
+    uint64_t cyc_stage;         /* staging the thresholded cost rows of an item                         */
+    uint64_t cyc_levels;        /* DP levels (streaming over the masks)                                 */
+    uint64_t cyc_level_barrier; /* wait at the barrier between two levels (team or CTA)                 */
+    uint64_t cyc_grid_wait;     /* wait at the grid barriers between scheduler rounds                   */
+    uint64_t cyc_scheduler;     /* folding results, planning the next thresholds, laying out the items  */
+    uint64_t cyc_backtrack;     /* plan back-tracker                                                    */
 } tg_solve_stats;
 
 /* tg_solve_batch — north_star "tg_solve_batch(instances, stream) -> best iteration time and plan".
@@ -157,7 +162,13 @@ typedef struct { /* optional diagnostics of one tg_solve_batch_ex call, written 
  *               stream is synchronised.  HOST: the call copies the results back and synchronises.
  *   cuda_stream a cudaStream_t (NULL = legacy default stream)
  * Never mutates the instances.  An infeasible instance is not an error (iter_time_us = INT64_MAX,
- * n_stages = 0).  n == 0 is a no-op.  Scratch memory is taken from the stream-ordered pool. */
+ * n_stages = 0).  n == 0 is a no-op.  Scratch memory comes from a stream-ordered pool of the library's own (the device's
+ * default pool is not touched).  Freed workspaces stay cached in that pool -- up to 14 GB, the DP scratch of the largest
+ * shapes; the environment variable TG_POOL_KEEP_MB lowers it -- until tg_release_cached_memory() is called.
+ * Internal errors of the solver (they have never been observed; the checks exist because the search keeps bounded
+ * lists): a call with a HOST buffer or HOST statistics returns TG_ERR_CUDA; in the fully asynchronous form (DEVICE
+ * results, no statistics) every result of the call is instead written with n_stages = -1 and
+ * iter_time_us = INT64_MAX, so a plan of a failed search can never be mistaken for the optimum. */
 tg_status tg_solve_batch(tg_instance* const* instances, int32_t n, tg_result* out, void* cuda_stream);
 
 /* Same, with flags and optional statistics (stats: EITHER or NULL; HOST forces a synchronise). */
@@ -195,11 +206,23 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
 
 /* Steps 1-3 alone: reduced tables and candidate thresholds.  All outputs HOST, any may be NULL.
  *   c_out    [NS][K] int32, TG_INF where no feasible plan      argp_out [NS][K] int32, -1 if none
+ *            (on an instance with a footprint table: the tables of depth 1, the least restrictive)
  *   x_out    [K][K] int32 (0 on the diagonal, TG_INF if > TG_TIME_MAX)
- *   cand_out capacity NS*K int32, ascending distinct finite c; *n_cand_out receives the count.
+ *   cand_out capacity NS*K int32: ascending distinct candidate thresholds; *n_cand_out receives their count.
+ * On a core instance the count is at most NS*K.  With tg_instance_set_actmem the thresholds are the distinct finite
+ * costs of ALL K depths and with tg_instance_set_transfer_bound the finite transfer times join them, so the count can
+ * reach NS*K*K + K*K: tg_reduce then writes only the first NS*K of them (it never writes past the documented
+ * capacity) while *n_cand_out still reports the full count; tg_candidates returns the whole list.
  * Synchronises `cuda_stream`. */
 tg_status tg_reduce(tg_instance* inst, int32_t* c_out, int32_t* argp_out, int32_t* x_out,
                     int32_t* cand_out, int32_t* n_cand_out, void* cuda_stream);
+
+/* Step 3 alone with an explicit capacity (PAPER.md:250 (1) "ranks the slowest stages"): the
+ * ascending distinct candidate thresholds of the instance as the solver sees them (all depths, plus the transfer times
+ * under the transfer bound).  cand_out: HOST, `capacity` int32 (may be NULL with capacity 0 to query the count);
+ * at most `capacity` entries are written, *n_cand_out (HOST, required) receives the full count.  capacity < 0 ->
+ * TG_ERR_RANGE.  Synchronises `cuda_stream`. */
+tg_status tg_candidates(tg_instance* inst, int32_t* cand_out, int64_t capacity, int32_t* n_cand_out, void* cuda_stream);
 
 /* Step 5 + 7 at ONE threshold: DP at T (T < 0 means infinity), top reduction and back-track.
  * out (EITHER): iter_time_us = f_T + (m-1)*T with T = 2^30 for infinity, bottleneck_us = that T,
@@ -208,6 +231,10 @@ tg_status tg_dp_at(tg_instance* inst, int64_t T, tg_result* out, void* cuda_stre
 
 /* Copies the instance's current time table (after pruning) to HOST time_out [NS][K][P]. */
 tg_status tg_instance_read_time(tg_instance* inst, int32_t* time_out);
+
+/* Returns the workspaces cached by the library's memory pool on the current device to the driver (an embedding
+ * framework with an allocator of its own may need the memory back).  Synchronises the device.  No-op before the first call. */
+tg_status tg_release_cached_memory(void);
 
 /* Device time in milliseconds of the persistent solver kernel most recently launched by this host
  * thread (CUDA events recorded on its stream around the launch; waits for it to finish).  HOST out. */

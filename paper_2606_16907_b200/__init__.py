@@ -44,7 +44,11 @@ class TgResult(C.Structure):
 class TgSolveStats(C.Structure):
     _fields_ = [("n_dp", C.c_uint64), ("plans_dense", C.c_uint64), ("states_live", C.c_uint64),
                 ("n_rounds", C.c_uint64), ("n_barriers", C.c_uint64), ("n_items_global_c", C.c_uint64),
-                ("error_flag", C.c_uint64), ("relax_admissible", C.c_uint64), ("cyc", C.c_uint64 * 8)]
+                ("error_flag", C.c_uint64), ("relax_admissible", C.c_uint64), ("states_windowed", C.c_uint64),
+                ("cyc_stage", C.c_uint64), ("cyc_levels", C.c_uint64), ("cyc_level_barrier", C.c_uint64),
+                ("cyc_grid_wait", C.c_uint64), ("cyc_scheduler", C.c_uint64), ("cyc_backtrack", C.c_uint64)]
+
+    CYC = ("cyc_stage", "cyc_levels", "cyc_level_barrier", "cyc_grid_wait", "cyc_scheduler", "cyc_backtrack")
 
 
 RESULT_BYTES = C.sizeof(TgResult)
@@ -62,7 +66,7 @@ class TangramError(RuntimeError):
 
 _lib = None
 EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
-           "tg_reduce", "tg_dp_at", "tg_instance_read_time", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
+           "tg_reduce", "tg_candidates", "tg_dp_at", "tg_instance_read_time", "tg_release_cached_memory", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
 
 
 def lib():
@@ -88,6 +92,7 @@ def lib():
         L.tg_prune.argtypes = [vp, C.c_int, i64, C.POINTER(i64), vp]
         L.tg_prune_batch.argtypes = [C.POINTER(vp), i32, C.c_int, i64, C.POINTER(i64), vp]
         L.tg_reduce.argtypes = [vp, vp, vp, vp, vp, C.POINTER(i32), vp]
+        L.tg_candidates.argtypes = [vp, vp, i64, C.POINTER(i32), vp]
         L.tg_dp_at.argtypes = [vp, i64, vp, vp]
         L.tg_instance_read_time.argtypes = [vp, vp]
         L.tg_last_solver_kernel_ms.argtypes = [C.POINTER(C.c_float)]
@@ -253,7 +258,16 @@ def tg_reduce(inst: Instance, stream=None):
     n = C.c_int32(0)
     _check(lib().tg_reduce(inst.handle, c.ctypes.data, argp.ctypes.data, x.ctypes.data, cand.ctypes.data,
                            C.byref(n), _stream_ptr(stream)))
-    return c, argp, x, cand[:n.value].copy()
+    return c, argp, x, cand[:min(n.value, cand.size)].copy()
+
+
+def tg_candidates(inst: Instance, stream=None) -> np.ndarray:
+    """The instance's candidate thresholds as the solver sees them (all depths, transfer times under the bound)."""
+    n = C.c_int32(0)
+    _check(lib().tg_candidates(inst.handle, None, 0, C.byref(n), _stream_ptr(stream)))
+    cand = np.empty(max(n.value, 1), dtype=np.int32)
+    _check(lib().tg_candidates(inst.handle, cand.ctypes.data, cand.size, C.byref(n), _stream_ptr(stream)))
+    return cand[:n.value].copy()
 
 
 def tg_prune(inst: Instance, mode: int = TG_PRUNE_EXACT, threshold: int = 0, stream=None) -> np.ndarray:
@@ -268,6 +282,10 @@ def tg_prune_batch(instances, mode: int = TG_PRUNE_EXACT, threshold: int = 0, st
     counts = (C.c_int64 * (4 * max(n, 1)))()
     _check(lib().tg_prune_batch(_handles(instances), n, mode, threshold, counts, _stream_ptr(stream)))
     return np.array(list(counts), dtype=np.int64)[:4 * n].reshape(n, 4)
+
+
+def tg_release_cached_memory():
+    _check(lib().tg_release_cached_memory())
 
 
 def tg_instance_read_time(inst: Instance) -> np.ndarray:

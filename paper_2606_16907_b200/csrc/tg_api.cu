@@ -56,6 +56,9 @@ struct DeviceState {
     int budgetAge = 0;
     uint16_t* rankOf = nullptr;
     uint16_t* maskOf = nullptr;
+    cudaMemPool_t pool = nullptr;   // the library's own stream-ordered pool for per-call workspaces
+    cudaStream_t up[4] = {nullptr, nullptr, nullptr, nullptr};   // upload streams of tg_instance_create_batch
+    cudaEvent_t upEv[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
 };
 std::mutex g_mu;
 int g_gallopMax = [] { const char* e = getenv("TG_GALLOP_MAX"); int v = e ? atoi(e) : 10; return v < 1 ? 1 : (v > 16 ? 16 : v); }();
@@ -116,12 +119,25 @@ tg_status deviceInit(int dev, DeviceState** out) {
         if (occ < TG_CTAS_PER_SM) return fail(TG_ERR_CUDA, "solver kernel: fewer co-resident CTAs per SM than it was built for");
         D.ctasPerSM = TG_CTAS_PER_SM;
         D.dynSmem = dyn;
-        // keep stream-ordered scratch cached between calls
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            uint64_t thr = UINT64_MAX;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        // Per-call workspaces come from a pool of the library's own (the device's default pool, which the embedding
+        // framework may share, is left as it is).  Freed workspaces stay cached up to the release threshold, so
+        // back-to-back solves do not go to the driver; anything above it returns to the device at the next synchronisation.
+        {
+            cudaMemPoolProps props;
+            memset(&props, 0, sizeof(props));
+            props.allocType = cudaMemAllocationTypePinned;
+            props.handleTypes = cudaMemHandleTypeNone;
+            props.location.type = cudaMemLocationTypeDevice;
+            props.location.id = dev;
+            TG_CUDA(cudaMemPoolCreate(&D.pool, &props));
+            // (the largest workspace is the DP scratch, capped at 12 GB in prepare(): a lower threshold would hand it back
+            // to the driver at every synchronisation and map it again on the next call -- measured 125 ms a call)
+            uint64_t thr = 14ull << 30;
+            if (const char* e = getenv("TG_POOL_KEEP_MB")) thr = uint64_t(std::max(0ll, atoll(e))) << 20;
+            TG_CUDA(cudaMemPoolSetAttribute(D.pool, cudaMemPoolAttrReleaseThreshold, &thr));
         }
+        for (int q = 0; q < 4; ++q) TG_CUDA(cudaStreamCreateWithFlags(&D.up[q], cudaStreamNonBlocking));
+        for (int q = 0; q < 5; ++q) TG_CUDA(cudaEventCreateWithFlags(&D.upEv[q], cudaEventDisableTiming));
         D.ready = true;
     }
     *out = &D;
@@ -147,7 +163,9 @@ bool isDevicePtr(const void* p) {
 }
 
 struct Workspace {
-    char* base = nullptr;
+    char* base = nullptr;           // freed (stream-ordered) when the workspace goes out of scope, on every path
+    cudaStream_t stream = nullptr;
+    ~Workspace() { if (base) cudaFreeAsync(base, stream); }
     size_t bytes = 0;
     TgInstDev* inst = nullptr;
     TgSolveCtx ctx;
@@ -235,22 +253,28 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const uint64_t slotWords = alignUp(size_t(maxFull) + 1024, 1024);
     int nSlots = 0;
     if (needSolve) {
-        if (D->budget == 0 || ++D->budgetAge >= 64) {   // (the query costs tens of microseconds: not on every solve)
-            size_t freeB = 0, totalB = 0;
-            TG_CUDA(cudaMemGetInfo(&freeB, &totalB));
-            D->budget = std::min<uint64_t>(uint64_t(freeB) * 6 / 10, 12ull << 30);   // bytes
-            D->budgetAge = 0;
+        uint64_t budget;
+        {
+            std::lock_guard<std::mutex> lk(g_mu);   // (solves may come from several host threads)
+            if (D->budget == 0 || ++D->budgetAge >= 64) {   // (the query costs tens of microseconds: not on every solve)
+                size_t freeB = 0, totalB = 0;
+                TG_CUDA(cudaMemGetInfo(&freeB, &totalB));
+                D->budget = std::min<uint64_t>(uint64_t(freeB) * 6 / 10, 12ull << 30);   // bytes
+                D->budgetAge = 0;
+            }
+            budget = D->budget;
         }
-        nSlots = int(std::min<uint64_t>(uint64_t(numCtas), D->budget / (slotWords * 4)));
+        nSlots = int(std::min<uint64_t>(uint64_t(numCtas), budget / (slotWords * 4)));
         if (nSlots < 1) nSlots = 1;   // let the allocation decide
     }
     const size_t oBar = cv.take(sizeof(uint32_t) * size_t(std::max(nSlots, 1)));
     const size_t oScratch = cv.take(size_t(slotWords) * 4 * size_t(nSlots), 4096);
     W.bytes = cv.off + 4096;
     {
-        const cudaError_t ea = cudaMallocAsync(reinterpret_cast<void**>(&W.base), W.bytes, st);
+        W.stream = st;
+        const cudaError_t ea = cudaMallocFromPoolAsync(reinterpret_cast<void**>(&W.base), W.bytes, D->pool, st);
         if (ea != cudaSuccess) {
-            D->budget = 0;   // measure again on the next call
+            { std::lock_guard<std::mutex> lk(g_mu); D->budget = 0; }   // measure again on the next call
             cudaGetLastError();
             return fail(ea == cudaErrorMemoryAllocation ? TG_ERR_OOM : TG_ERR_CUDA, std::string("workspace allocation: ") + cudaGetErrorString(ea));
         }
@@ -333,6 +357,7 @@ tg_status launchSolve(Workspace& W, cudaStream_t st) {
 tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cudaStream_t st) {
     const bool outDev = isDevicePtr(out);
     bool sync = !outDev;
+    tgPoisonOnErrorKernel<<<std::max(1, std::min((n + 255) / 256, 64)), 256, 0, st>>>(W.ctx.ctrl, W.outDev, n);
     TG_CUDA(cudaMemcpyAsync(out, W.outDev, sizeof(tg_result) * n, cudaMemcpyDefault, st));
     if (stats) {
         if (!isDevicePtr(stats)) sync = true;
@@ -584,6 +609,12 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
         return fail(e == cudaErrorMemoryAllocation ? TG_ERR_OOM : TG_ERR_CUDA, std::string("batch allocation: ") + cudaGetErrorString(e));
     }
     char* base = blk->base;
+    {   // the upload streams start behind the allocation (stream-ordered on the legacy default stream)
+        std::lock_guard<std::mutex> lk(g_mu);   // one batch at a time uses the upload streams and their events
+        e = cudaEventRecord(D->upEv[4], 0);
+        for (int q = 0; q < 4 && e == cudaSuccess; ++q) e = cudaStreamWaitEvent(D->up[q], D->upEv[4], 0);
+    }
+    if (e != cudaSuccess) { cudaFreeAsync(blk->base, 0); delete blk; cudaGetLastError(); return fail(TG_ERR_CUDA, "batch upload: stream setup"); }
     int32_t* dSmall = reinterpret_cast<int32_t*>(base + oSmall);
     std::vector<int32_t> hSmall(smallInts);
     std::vector<TgValidateDesc> hDesc(nn);
@@ -607,8 +638,10 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
         t->cap_mb = t->gpus + Ki;
         t->bw = t->cap_mb + Ki;
         out[i] = t;
-        e = cudaMemcpyAsync(t->time_us, time_us[i], nE * 4, cudaMemcpyDefault, 0);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(t->mem_mb, mem_mb[i], nE * 4, cudaMemcpyDefault, 0);
+        // the table uploads are dealt to four streams: a single stream moved 188 KB tables at a third of the link's
+        // rate (every copy waits for the previous one's completion before it starts)
+        e = cudaMemcpyAsync(t->time_us, time_us[i], nE * 4, cudaMemcpyDefault, D->up[(2 * i) & 3]);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(t->mem_mb, mem_mb[i], nE * 4, cudaMemcpyDefault, D->up[(2 * i + 1) & 3]);
         const int32_t* srcs[3] = {island_gpus[i], island_cap_mb[i], bw_gbps[i]};
         int32_t* dsts[3] = {t->gpus, t->cap_mb, t->bw};
         const size_t lens[3] = {size_t(Ki), size_t(Ki), size_t(Ki) * Ki};
@@ -621,6 +654,11 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
     }
     int* dErr = reinterpret_cast<int*>(base + oErr);
     std::vector<int> herr(nn, 0);
+    for (int q = 0; q < 4; ++q) {   // the validation (default stream) runs behind every upload, also on the error paths
+        cudaError_t e2 = cudaEventRecord(D->upEv[q], D->up[q]);
+        if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(0, D->upEv[q], 0);
+        if (e == cudaSuccess) e = e2;
+    }
     if (e == cudaSuccess) e = cudaMemcpyAsync(dSmall, hSmall.data(), smallInts * 4, cudaMemcpyHostToDevice, 0);
     for (size_t q = 0; q < late.size() && e == cudaSuccess; ++q)
         e = cudaMemcpyAsync(late[q].dst, late[q].src, late[q].ints * 4, cudaMemcpyDeviceToDevice, 0);
@@ -705,10 +743,10 @@ tg_status tg_solve_batch_ex(tg_instance* const* instances, int32_t n, tg_result*
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     Workspace W;
     tg_status s = prepare(instances, n, true, st, W);
-    if (s != TG_OK) { if (W.base) cudaFreeAsync(W.base, st); return s; }
+    if (s != TG_OK) return s;
     W.ctx.out = W.outDev; W.ctx.flags = flags; W.ctx.mode = 0;
     s = launchSolve(W, st);
-    if (s != TG_OK) { cudaFreeAsync(W.base, st); return s; }
+    if (s != TG_OK) return s;
     return finish(W, n, out, stats, st);
 }
 
@@ -723,39 +761,55 @@ tg_status tg_dp_at(tg_instance* inst, int64_t T, tg_result* out, void* cuda_stre
     Workspace W;
     tg_instance* arr[1] = {inst};
     tg_status s = prepare(arr, 1, true, st, W);
-    if (s != TG_OK) { if (W.base) cudaFreeAsync(W.base, st); return s; }
+    if (s != TG_OK) return s;
     W.ctx.out = W.outDev; W.ctx.flags = 0; W.ctx.mode = 1;
     W.ctx.dpT = T < 0 ? TG_TINF : uint32_t(T);
     s = launchSolve(W, st);
-    if (s != TG_OK) { cudaFreeAsync(W.base, st); return s; }
+    if (s != TG_OK) return s;
     return finish(W, 1, out, nullptr, st);
 }
 
-tg_status tg_reduce(tg_instance* inst, int32_t* c_out, int32_t* argp_out, int32_t* x_out, int32_t* cand_out,
-                    int32_t* n_cand_out, void* cuda_stream) {
+// steps 1-3 for one instance; cand_out receives at most cand_capacity thresholds, *n_cand_out the full count
+static tg_status reduceImpl(tg_instance* inst, int32_t* c_out, int32_t* argp_out, int32_t* x_out, int32_t* cand_out,
+                            int64_t cand_capacity, int32_t* n_cand_out, void* cuda_stream) {
     if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     Workspace W;
     tg_instance* arr[1] = {inst};
     tg_status s = prepare(arr, 1, false, st, W);
-    if (s != TG_OK) { if (W.base) cudaFreeAsync(W.base, st); return s; }
+    if (s != TG_OK) return s;
     const int cells = inst->NS * inst->K, K = inst->K;
     int32_t *dc = nullptr, *da = nullptr, *dx = nullptr;
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&dc), size_t(cells) * 4 * 2 + K * K * 4, st));
-    da = dc + cells; dx = da + cells;
-    tgExportKernel<<<std::max(1, std::min((cells + 255) / 256, 1024)), 256, 0, st>>>(W.inst, dc, da, dx);
+    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&dc), size_t(cells) * 4 * 2 + K * K * 4, st);
     TgInstDev hI;
-    TG_CUDA(cudaMemcpyAsync(&hI, W.inst, sizeof(TgInstDev), cudaMemcpyDeviceToHost, st));
-    TG_CUDA(cudaStreamSynchronize(st));
-    if (c_out) TG_CUDA(cudaMemcpyAsync(c_out, dc, size_t(cells) * 4, cudaMemcpyDeviceToHost, st));
-    if (argp_out) TG_CUDA(cudaMemcpyAsync(argp_out, da, size_t(cells) * 4, cudaMemcpyDeviceToHost, st));
-    if (x_out) TG_CUDA(cudaMemcpyAsync(x_out, dx, size_t(K) * K * 4, cudaMemcpyDeviceToHost, st));
-    if (cand_out && hI.ncand > 0) TG_CUDA(cudaMemcpyAsync(cand_out, hI.cand, size_t(hI.ncand) * 4, cudaMemcpyDeviceToHost, st));
+    if (e == cudaSuccess) {
+        da = dc + cells; dx = da + cells;
+        tgExportKernel<<<std::max(1, std::min((cells + 255) / 256, 1024)), 256, 0, st>>>(W.inst, dc, da, dx);
+        e = cudaMemcpyAsync(&hI, W.inst, sizeof(TgInstDev), cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess && c_out) e = cudaMemcpyAsync(c_out, dc, size_t(cells) * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && argp_out) e = cudaMemcpyAsync(argp_out, da, size_t(cells) * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && x_out) e = cudaMemcpyAsync(x_out, dx, size_t(K) * K * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && cand_out && hI.ncand > 0 && cand_capacity > 0)
+        e = cudaMemcpyAsync(cand_out, hI.cand, size_t(std::min<int64_t>(hI.ncand, cand_capacity)) * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (dc) cudaFreeAsync(dc, st);
+    if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? TG_ERR_OOM : TG_ERR_CUDA, std::string("tg_reduce: ") + cudaGetErrorString(e));
     if (n_cand_out) *n_cand_out = hI.ncand;
-    TG_CUDA(cudaStreamSynchronize(st));
-    TG_CUDA(cudaFreeAsync(dc, st));
-    TG_CUDA(cudaFreeAsync(W.base, st));
     return TG_OK;
+}
+
+tg_status tg_reduce(tg_instance* inst, int32_t* c_out, int32_t* argp_out, int32_t* x_out, int32_t* cand_out,
+                    int32_t* n_cand_out, void* cuda_stream) {
+    if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
+    return reduceImpl(inst, c_out, argp_out, x_out, cand_out, int64_t(inst->NS) * inst->K, n_cand_out, cuda_stream);
+}
+
+tg_status tg_candidates(tg_instance* inst, int32_t* cand_out, int64_t capacity, int32_t* n_cand_out, void* cuda_stream) {
+    if (!inst || !n_cand_out) return fail(TG_ERR_NULL, "NULL argument");
+    if (capacity < 0 || (capacity > 0 && !cand_out)) return fail(TG_ERR_RANGE, "capacity < 0, or capacity > 0 without a buffer");
+    return reduceImpl(inst, nullptr, nullptr, nullptr, cand_out, capacity, n_cand_out, cuda_stream);
 }
 
 tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode mode, int64_t threshold, int64_t* counts_out,
@@ -827,6 +881,17 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
 tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4], void* cuda_stream) {
     if (!inst || !counts_out) return fail(TG_ERR_NULL, "NULL argument");
     return tg_prune_batch(&inst, 1, mode, threshold, counts_out, cuda_stream);
+}
+
+tg_status tg_release_cached_memory(void) {
+    int dev = 0;
+    TG_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (dev >= 0 && dev < 64 && g_dev[dev].ready && g_dev[dev].pool) {
+        TG_CUDA(cudaDeviceSynchronize());
+        TG_CUDA(cudaMemPoolTrimTo(g_dev[dev].pool, 0));
+    }
+    return TG_OK;
 }
 
 tg_status tg_last_solver_kernel_ms(float* ms_out) {

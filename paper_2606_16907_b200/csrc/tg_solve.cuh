@@ -287,7 +287,10 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
             sm.wbufOff = csUsed;
             sm.wbufWords = min(2 * perMaskW, (total - csUsed) / nWp) & ~3;
         }
-        if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
+        if (count) {
+            if (sm.useGlobalC) atomicAdd((unsigned long long*)&ctx.ctrl->stats.n_items_global_c, 1ull);
+            if (Ke && sm.sSlack >= 0) atomicAdd((unsigned long long*)&ctx.ctrl->stats.states_windowed, (unsigned long long)sm.sWd * Ke << (Ke - 1));
+        }
     }
     __syncthreads();
     nAdm = tgStageCosts(ctx, sm, Cs, 1, count);
@@ -1657,7 +1660,26 @@ __global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgS
         tgGridBarrier(ctrl, epoch);
         tgMark(sm, 5);
     }
-    if (threadIdx.x == 0)
-        for (int i = 0; i < 8; ++i) atomicAdd((unsigned long long*)&ctrl->stats.cyc[i], sm.cyc[i]);
+    if (threadIdx.x == 0) {
+        tg_solve_stats& S = ctrl->stats;
+        atomicAdd((unsigned long long*)&S.cyc_stage, sm.cyc[0]);
+        atomicAdd((unsigned long long*)&S.cyc_levels, sm.cyc[3]);
+        atomicAdd((unsigned long long*)&S.cyc_level_barrier, sm.cyc[4]);
+        atomicAdd((unsigned long long*)&S.cyc_grid_wait, sm.cyc[5]);
+        atomicAdd((unsigned long long*)&S.cyc_scheduler, sm.cyc[6]);
+        atomicAdd((unsigned long long*)&S.cyc_backtrack, sm.cyc[7]);
+    }
     if (b == 0 && threadIdx.x == 0) ctrl->stats.n_barriers = epoch;
+}
+
+// Runs behind the solver on the same stream: if the solver raised its internal error flag (a back-track without a
+// predecessor, an overflowing list of evaluated thresholds) every result of the call is marked unusable
+// (n_stages = -1, iter_time_us = INT64_MAX), so that a caller who never synchronises on a status -- DEVICE results, no
+// statistics -- cannot take a plan from a failed search for the optimum.
+__global__ void tgPoisonOnErrorKernel(const TgCtrl* __restrict__ ctrl, tg_result* __restrict__ out, int n) {
+    if (ctrl->errFlag == 0) return;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        out[i].n_stages = -1;
+        out[i].iter_time_us = INT64_MAX;
+    }
 }

@@ -41,7 +41,7 @@ def test_result_struct_layout(tg):
     assert C.sizeof(tg.TgResult) == 224 and tg.RESULT_DTYPE.itemsize == 224
     for name, _ in tg.TgResult._fields_:
         assert getattr(tg.TgResult, name).offset == tg.RESULT_DTYPE.fields[name][1]
-    assert C.sizeof(tg.TgSolveStats) == 128
+    assert C.sizeof(tg.TgSolveStats) == 120
     assert tg.tg_version() >= 100
 
 

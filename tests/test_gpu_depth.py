@@ -89,3 +89,23 @@ def test_full_size_cfg3_with_actmem(tg):
     assert s["iter_time_us"] >= e["core"]["iter_time_us"]
     st = [tuple(x) for x in got[4]]
     assert rescore_depth(inst, st) == (got[1], got[2], got[0], got[3])
+
+
+def test_full_size_cfg4_with_actmem(tg):
+    """The K = 16 depth-aware workload bench.py times as `cfg4d` (full-size MoE-like config with a footprint, the loader
+    restaging its cost rows at each of 16 levels); stored result of the variant oracle
+    (tests/golden/make_expected.py cfg4d) and of the core oracle for the same tables without the footprint."""
+    import json, os
+    here = os.path.dirname(os.path.abspath(__file__))
+    e = json.load(open(os.path.join(here, "golden", "expected_cfg4d.json")))["records"][0]
+    core = json.load(open(os.path.join(here, "golden", "expected_cfg4.json")))["records"][0]
+    inst = gen.with_actmem(gen.config4(), 11, 300, 3000)
+    g = solve_all(tg, [inst])[0]
+    n = int(g["n_stages"])
+    got = [int(g["iter_time_us"]), int(g["sum_us"]), int(g["bottleneck_us"]), int(g["island_mask"]),
+           [[int(g["stage_begin"][i]), int(g["stage_island"][i]), int(g["stage_plan"][i])] for i in range(n)]]
+    s = e["solve"]
+    assert got == [s["iter_time_us"], s["sum_us"], s["bottleneck_us"], s["island_mask"], s["stages"]]
+    assert s["iter_time_us"] >= core["solve"]["iter_time_us"]          # a footprint never improves the optimum
+    st = [tuple(x) for x in got[4]]
+    assert rescore_depth(inst, st) == (got[1], got[2], got[0], got[3])

@@ -83,9 +83,10 @@ def test_full_sweep_matches_on_cfg3(tg):
 
 
 def test_cfg5_batch_1024(tg):
-    """The whole throughput batch in ONE tg_solve_batch call; sampled seeds against stored oracle
-    results, every instance against the re-scorer."""
+    """The whole throughput batch in ONE tg_solve_batch call; EVERY instance against its stored oracle result (value
+    and plan, tests/golden/make_expected.py cfg5: all 1024 seeds) and against the re-scorer."""
     exp = {r["seed"]: r for r in expected("cfg5")}
+    assert sorted(exp) == list(range(1024))
     insts = gen.config5(1024)
     hs = [tg.instance_from_inputs(i) for i in insts]
     res = tg.tg_solve_batch(hs)

@@ -93,3 +93,55 @@ def test_full_size_cfg3_with_transfer_bound(tg):
     assert got == [s["iter_time_us"], s["sum_us"], s["bottleneck_us"], s["island_mask"], s["stages"]]
     assert s["iter_time_us"] >= e["core"]["iter_time_us"]
     assert rescore_xbound(inst, stages_of(g)) == (got[1], got[2], got[0], got[3])
+
+
+def test_full_size_cfg4_with_transfer_bound(tg):
+    """The K = 16 workload bench.py times as `cfg4xb`; stored result of the variant oracle
+    (tests/golden/make_expected.py cfg4xb) and of the core oracle for the same tables without the bound."""
+    here = os.path.dirname(os.path.abspath(__file__))
+    e = json.load(open(os.path.join(here, "golden", "expected_cfg4xb.json")))["records"][0]
+    core = json.load(open(os.path.join(here, "golden", "expected_cfg4.json")))["records"][0]
+    inst = gen.with_transfer_bound(gen.config4())
+    g = solve_all(tg, [inst])[0]
+    got = [int(g["iter_time_us"]), int(g["sum_us"]), int(g["bottleneck_us"]), int(g["island_mask"]), [list(t) for t in stages_of(g)]]
+    s = e["solve"]
+    assert got == [s["iter_time_us"], s["sum_us"], s["bottleneck_us"], s["island_mask"], s["stages"]]
+    assert s["iter_time_us"] >= core["solve"]["iter_time_us"]          # bounding the transfers never improves the optimum
+    assert rescore_xbound(inst, stages_of(g)) == (got[1], got[2], got[0], got[3])
+
+
+def test_reduce_and_candidates_on_variant_instances(tg):
+    """tg_reduce never writes past its documented capacity NS*K although a variant instance has more thresholds (all
+    depths / the transfer times); tg_candidates returns the whole list.  Expected lists: the transfer-bound list is the
+    union of the oracle's finite depth-1 costs and finite off-diagonal transfers; with a footprint the count is the
+    variant oracle's n_candidates and the list is sorted, distinct and contains every depth-1 cost."""
+    for seed in range(12):
+        base = gen.random_small(700 + seed, Lmax=3, Kmax=5, Pmax=3, style=STYLES[seed % 5])
+        NS = base.L * (base.L + 1) // 2
+        oc, _, ox, ocand = oracle.reduce(base)
+        for variant in ("xb", "act", "both"):
+            inst = base
+            if variant in ("act", "both"):
+                inst = gen.with_actmem(inst, seed, 0, 40)
+            if variant in ("xb", "both"):
+                inst = gen.with_transfer_bound(inst)
+            h = tg.instance_from_inputs(inst)
+            guard = np.full(NS * base.K + 64, -7, dtype=np.int32)            # room behind the documented capacity
+            n = np.zeros(1, dtype=np.int32)
+            import ctypes as C
+            st = tg.lib().tg_reduce(h.handle, None, None, None, guard.ctypes.data, n.ctypes.data_as(C.POINTER(C.c_int32)), None)
+            assert st == 0 and (guard[NS * base.K:] == -7).all(), "tg_reduce wrote past NS*K"
+            c, argp, x, cand_r = tg.tg_reduce(h)
+            cand = tg.tg_candidates(h).astype(np.int64)
+            assert int(n[0]) == cand.size and np.array_equal(cand[:cand_r.size], cand_r.astype(np.int64))
+            assert cand_r.size == min(cand.size, NS * base.K)
+            assert (np.diff(cand) > 0).all()
+            assert cand.size == oracle.solve_variant(inst).n_candidates
+            assert np.array_equal(x.astype(np.int64), ox)
+            if variant == "xb":                                               # depth-1 tables are the core tables
+                assert np.array_equal(c.astype(np.int64), oc)
+                fx = ox[(ox < (1 << 30)) & ~np.eye(base.K, dtype=bool)]
+                assert np.array_equal(cand, np.union1d(ocand, fx))
+            else:                                                             # depth 1 of the footprint: a subset of the list
+                assert np.isin(c[c < (1 << 30)].astype(np.int64), cand).all()
+            h.destroy()
