@@ -15,6 +15,8 @@ import numpy as np
 _DIR = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_DIR, "tangram_oracle.cpp")
 _SRC_DEPTH = os.path.join(_DIR, "tangram_oracle_depth.cpp")   # NEXT-1 variant, separate translation unit
+_SRC_STAGES = os.path.join(_DIR, "tangram_oracle_stages.cpp")  # NEXT-2 variant, separate translation unit
+_SRC_ISLANDS = os.path.join(_DIR, "tangram_oracle_islands.cpp")  # NEXT-4 front end, separate translation unit
 _SO = os.path.join(_DIR, "libtangram_oracle.so")
 MAXK = 16
 INF = 1 << 30
@@ -22,9 +24,11 @@ INT64_MAX = (1 << 63) - 1
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_DEPTH)):
+    srcs = [f for f in (_SRC, _SRC_DEPTH, _SRC_STAGES, _SRC_ISLANDS) if os.path.exists(f)]
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < max(os.path.getmtime(f) for f in srcs):
         tmp = _SO + f".tmp{os.getpid()}"
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-o", tmp, _SRC, _SRC_DEPTH])
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread"] + os.environ.get("TG_ORACLE_CXXFLAGS", "").split() +
+                              ["-o", tmp] + srcs)
         os.replace(tmp, _SO)
     return _SO
 
@@ -205,6 +209,33 @@ def prune_depth(inst, mode: int = 0, threshold: int = 0):
                           C.c_int(mode), C.c_int64(threshold), counts.ctypes.data_as(_I64P))
     out.time_us = t
     return out, counts
+
+
+def _args_stages(inst):
+    keep, a = _args(inst)
+    sl = np.ascontiguousarray(inst.slow_us, dtype=np.int32)
+    qs = None if getattr(inst, "q_stages", None) is None else np.ascontiguousarray(inst.q_stages, dtype=np.int32)
+    qp = C.cast(None, _I32P) if qs is None else _p32(qs)
+    return (keep, sl, qs), a[:6] + (_p32(sl), qp) + a[6:]
+
+
+def solve_stages(inst):
+    """NEXT-2: multi-stage partial plans (inst.slow_us [NS,K,P] slowest internal stage, inst.q_stages [NS,K,P] or None).
+    Returns (Result, total pipeline stages of the plan)."""
+    keep, a = _args_stages(inst)
+    r = _Res()
+    tot = C.c_int32(0)
+    lib().orc_stages_solve(*a, C.byref(r), C.byref(tot))
+    return _conv(r), tot.value
+
+
+def bruteforce_stages(inst):
+    keep, a = _args_stages(inst)
+    r = _Res()
+    tot = C.c_int32(0)
+    n = C.c_int64(0)
+    lib().orc_stages_bruteforce(*a, C.byref(r), C.byref(tot), C.byref(n))
+    return _conv(r), tot.value, n.value
 
 
 def hw_threads() -> int:

@@ -80,12 +80,16 @@ class Instance:
     meta: dict = field(default_factory=dict)
     actmem_mb: np.ndarray = None   # [NS, K, P] int32 or None: MB per in-flight microbatch (NEXT-1, depth-aware memory)
     transfer_bound: bool = False   # NEXT-3(b): transfers count toward the bottleneck (x <= T as well)
+    slow_us: np.ndarray = None     # [NS, K, P] int32 or None: slowest internal stage of the partial plan (NEXT-2)
+    q_stages: np.ndarray = None    # [NS, K, P] int32 or None: its number of internal pipeline stages (NEXT-2)
 
     def copy(self) -> "Instance":
         return Instance(self.name, self.L, self.K, self.P, self.m, self.time_us.copy(),
                         self.mem_mb.copy(), self.island_gpus.copy(), self.island_cap_mb.copy(),
                         self.bw_gbps.copy(), self.act_mb, dict(self.meta),
-                        None if self.actmem_mb is None else self.actmem_mb.copy(), self.transfer_bound)
+                        None if self.actmem_mb is None else self.actmem_mb.copy(), self.transfer_bound,
+                        None if self.slow_us is None else self.slow_us.copy(),
+                        None if self.q_stages is None else self.q_stages.copy())
 
 
 def _cdiv(a, b):
@@ -295,6 +299,26 @@ def with_transfer_bound(inst: Instance) -> Instance:
     o = inst.copy()
     o.transfer_bound = True
     o.name = inst.name + "_xb"
+    return o
+
+
+def with_stages(inst: Instance, seed: int, qmax: int = 4) -> Instance:
+    """NEXT-2: every entry becomes a partial plan of q = u(1, min(qmax, slice length)) internal pipeline stages whose
+    slowest stage is between an even split and 1.6 x it: slow = min(time, ceil(time / q * u(1000, 1600) / 1000)); q = 1 keeps
+    slow = time.  The paper prints no figures for the internal stages of a parallelizer's plan."""
+    o = inst.copy()
+    NS, K, P = inst.time_us.shape
+    a, b = slice_bounds(inst.L)
+    idx = np.arange(NS * K * P).reshape(NS, K, P)
+    q = 1 + (urand(seed, S_MISC + 40, idx, 0, qmax - 1) % np.minimum(qmax, (b - a))[:, None, None])
+    t = inst.time_us.astype(np.int64)
+    even = -(-t // q)
+    slow = np.minimum(t, -(-(even * urand(seed, S_MISC + 41, idx, 1000, 1600)) // 1000))
+    slow = np.where(q == 1, t, slow)
+    slow = np.where(inst.time_us == TG_INVALID, 0, slow)
+    o.slow_us = slow.astype(np.int32)
+    o.q_stages = q.astype(np.int32)
+    o.name = inst.name + "_st"
     return o
 
 
