@@ -114,6 +114,23 @@ tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb);
  * on == 0 restores the core definition.  Combines with tg_instance_set_actmem.  No device work. */
 tg_status tg_instance_set_transfer_bound(tg_instance* inst, int32_t on);
 
+/* tg_instance_set_stages — SURVEY.md §8(f) NEXT-2, multi-stage partial plans ("a model-slice/island plan
+ * can include multiple pipeline stages", :248, :250 (1) "ranks the slowest stages in all model-slice/island plans").
+ *   slow_us   EITHER [NS][K][P] int32: slowest internal pipeline stage of the partial plan, 0 <= slow_us <= time_us on
+ *             every valid entry (time_us is then the partial plan's whole time for one microbatch, the sum of its
+ *             internal stages); copied; NULL removes the tables
+ *   n_stages  EITHER [NS][K][P] int32 in [1, 255]: its number of internal stages, or NULL (all ones); copied
+ * With the tables set an entry is admissible at threshold T iff slow_us <= T; a plan's bottleneck is T = max slow_us of
+ * its partial plans, sum still adds the time_us (and transfers), iter = sum + (m-1)*T, and the candidate thresholds are
+ * the distinct slow_us at which some cell's cost changes.  The plan choice is part of the optimum: stage_plan[i] =
+ * lowest p with the least time_us among the entries of its cell that are admissible at T*.  slow_us == time_us is the
+ * core definition bit for bit.  n_stages does not enter the optimum; tg_plan_pipeline_stages adds it up for a result.
+ * Not combinable with tg_instance_set_actmem (the depth of a partial plan would count the internal stages behind it,
+ * which needs a stage counter in the DP state): either call on an instance that has the other table -> TG_ERR_SHAPE;
+ * tg_prune on such an instance -> TG_ERR_SHAPE.  Combines with tg_instance_set_transfer_bound.  Values out of range ->
+ * TG_ERR_RANGE.  Synchronises the legacy default stream. */
+tg_status tg_instance_set_stages(tg_instance* inst, const int32_t* slow_us, const int32_t* n_stages);
+
 /* NULL is a no-op.  The instance must not be in use by an unsynchronised tg_solve_batch. */
 tg_status tg_instance_destroy(tg_instance* inst);
 
@@ -174,6 +191,10 @@ tg_status tg_solve_batch(tg_instance* const* instances, int32_t n, tg_result* ou
 /* Same, with flags and optional statistics (stats: EITHER or NULL; HOST forces a synchronise). */
 tg_status tg_solve_batch_ex(tg_instance* const* instances, int32_t n, tg_result* out, uint32_t flags,
                             tg_solve_stats* stats, void* cuda_stream);
+
+/* Total number of pipeline stages of a returned plan: the sum of n_stages over its partial plans (n_stages of plain
+ * instances is 1, so this is result->n_stages for them).  result: HOST; n_out: HOST.  Synchronous. */
+tg_status tg_plan_pipeline_stages(tg_instance* inst, const tg_result* result, int32_t* n_out);
 
 typedef enum {
     TG_PRUNE_EXACT = 0,     /* R1 infeasible + R2 dominated; threshold ignored                  */

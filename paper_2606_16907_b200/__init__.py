@@ -65,7 +65,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
+EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_set_stages", "tg_plan_pipeline_stages", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
            "tg_reduce", "tg_candidates", "tg_dp_at", "tg_instance_read_time", "tg_release_cached_memory", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -85,6 +85,8 @@ def lib():
         L.tg_instance_create_classes.argtypes = [i32, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, i32, C.POINTER(vp)]
         L.tg_instance_create_batch.argtypes = [i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.tg_instance_set_transfer_bound.argtypes = [vp, i32]
+        L.tg_instance_set_stages.argtypes = [vp, vp, vp]
+        L.tg_plan_pipeline_stages.argtypes = [vp, vp, C.POINTER(i32)]
         L.tg_instance_destroy.argtypes = [vp]
         L.tg_instance_set_actmem.argtypes = [vp, vp]
         L.tg_solve_batch.argtypes = [C.POINTER(vp), i32, vp, vp]
@@ -207,6 +209,24 @@ def tg_instance_set_actmem(inst: Instance, actmem_mb):
     _check(lib().tg_instance_set_actmem(inst.handle, _ptr(a)))
 
 
+def tg_instance_set_stages(inst: Instance, slow_us, n_stages=None):
+    """NEXT-2: slowest internal stage and internal stage count per entry ([NS,K,P] int32); slow_us None removes them."""
+    a = np.ascontiguousarray(slow_us, dtype=np.int32) if isinstance(slow_us, np.ndarray) else slow_us
+    q = np.ascontiguousarray(n_stages, dtype=np.int32) if isinstance(n_stages, np.ndarray) else n_stages
+    _check(lib().tg_instance_set_stages(inst.handle, _ptr(a), _ptr(q)))
+
+
+def tg_plan_pipeline_stages(inst: Instance, result) -> int:
+    """Total pipeline stages of a plan: `result` is a TgResult or one record of the RESULT_DTYPE array."""
+    if isinstance(result, TgResult):
+        r = result
+    else:
+        r = TgResult.from_buffer_copy(np.asarray(result).tobytes())
+    n = C.c_int32(0)
+    _check(lib().tg_plan_pipeline_stages(inst.handle, C.addressof(r), C.byref(n)))
+    return n.value
+
+
 def tg_instance_set_transfer_bound(inst: Instance, on: bool):
     """NEXT-3(b): transfers count toward the bottleneck (x <= T as well)."""
     _check(lib().tg_instance_set_transfer_bound(inst.handle, C.c_int32(1 if on else 0)))
@@ -325,4 +345,6 @@ def instance_from_inputs(inst, device_tables: bool = False) -> Instance:
         tg_instance_set_actmem(h, inst.actmem_mb)
     if getattr(inst, "transfer_bound", False):
         tg_instance_set_transfer_bound(h, True)
+    if getattr(inst, "slow_us", None) is not None:
+        tg_instance_set_stages(h, inst.slow_us, getattr(inst, "q_stages", None))
     return h

@@ -25,6 +25,8 @@ struct tg_instance {
     int device;
     int32_t *time_us, *mem_mb, *gpus, *cap_mb, *bw;  // device
     int32_t* actmem;                                 // device, or nullptr (tg_instance_set_actmem)
+    int32_t* slow = nullptr;                         // device, or nullptr (tg_instance_set_stages): slowest internal stage [NS][K][P]
+    int32_t* qst = nullptr;                          // device, behind slow: internal stage counts [NS][K][P]
     int32_t xbound;                                  // tg_instance_set_transfer_bound
 };
 
@@ -193,7 +195,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     Carver cv;
     const size_t oInst = cv.take(sizeof(TgInstDev) * n);
     std::vector<TgInstDev> h(n);
-    std::vector<size_t> oCd(n), oArgp(n), oCand(n), oSort(n), oSort2(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
+    std::vector<size_t> oCd(n), oThr(n), oArgp(n), oCand(n), oSort(n), oSort2(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
     int maxCells = 0, maxLp = 4, maxK = 1;
     uint64_t maxFull = 0;
     size_t denseCs = 0;
@@ -204,6 +206,9 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         I.time_us = t.time_us; I.mem_mb = t.mem_mb; I.cap_mb = t.cap_mb; I.bw_gbps = t.bw;
         I.actmem_mb = t.actmem;
         I.nDepth = t.actmem ? t.K : 1;
+        I.slow_us = t.slow;
+        I.nLayers = t.slow ? t.P : 0;
+        I.nTables = std::max(std::max(I.nDepth, I.nLayers), 1);
         I.xbound = t.xbound;
         I.L = t.L; I.K = t.K; I.P = t.P; I.m = t.m; I.act_mb = t.act_mb; I.NS = t.NS;
         I.Lp = (t.L + 3) & ~3;
@@ -230,8 +235,9 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         maxCells = std::max(maxCells, cells);
         maxLp = std::max(maxLp, int(I.Lp));
         maxK = std::max(maxK, int(t.K));
-        const size_t nd = size_t(I.nDepth);
+        const size_t nd = size_t(I.nTables);
         oCd[i] = cv.take(nd * size_t(t.K) * I.triG * 4);
+        oThr[i] = I.nLayers ? cv.take(nd * size_t(t.K) * I.triG * 4) : 0;
         oArgp[i] = cv.take(nd * size_t(cells));
         const size_t nKeys = nd * size_t(cells) + size_t(t.K) * t.K;   // every reduced cost + (transfer bound) every transfer time
         oCand[i] = cv.take(nKeys * 4);
@@ -281,6 +287,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     }
     for (int i = 0; i < n; ++i) {
         h[i].cd = reinterpret_cast<uint32_t*>(W.base + oCd[i]);
+        h[i].thr = h[i].nLayers ? reinterpret_cast<uint32_t*>(W.base + oThr[i]) : nullptr;
         h[i].argp = reinterpret_cast<uint8_t*>(W.base + oArgp[i]);
         h[i].cand = reinterpret_cast<uint32_t*>(W.base + oCand[i]);
         h[i].sortbuf = reinterpret_cast<uint32_t*>(W.base + oSort[i]);
@@ -695,6 +702,7 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
 tg_status tg_instance_destroy(tg_instance* inst) {
     if (!inst) return TG_OK;
     if (inst->actmem) cudaFreeAsync(inst->actmem, 0);
+    if (inst->slow) cudaFreeAsync(inst->slow, 0);
     if (inst->block) {   // created by tg_instance_create_batch: the allocation goes with the last instance of the batch
         TgBatchBlock* blk = inst->block;
         if (blk->refs.fetch_sub(1) == 1) { cudaFreeAsync(blk->base, 0); delete blk; }
@@ -709,6 +717,7 @@ tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb) {
     if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
     if (inst->actmem) { cudaFreeAsync(inst->actmem, 0); inst->actmem = nullptr; }
     if (!actmem_mb) return TG_OK;
+    if (inst->slow) return fail(TG_ERR_SHAPE, "the instance has multi-stage partial plans (tg_instance_set_stages): the combination with a footprint table is not built");
     const size_t nE = size_t(inst->NS) * inst->K * inst->P;
     int32_t* d = nullptr;
     TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), nE * 4 + 4, 0));
@@ -727,6 +736,52 @@ tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb) {
         return fail(TG_ERR_RANGE, "actmem_mb must be in [0, 2^20]");
     }
     inst->actmem = d;
+    return TG_OK;
+}
+
+tg_status tg_instance_set_stages(tg_instance* inst, const int32_t* slow_us, const int32_t* n_stages) {
+    if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
+    if (inst->slow) { cudaFreeAsync(inst->slow, 0); inst->slow = nullptr; inst->qst = nullptr; }
+    if (!slow_us) return TG_OK;
+    if (inst->actmem) return fail(TG_ERR_SHAPE, "the instance has a footprint table (tg_instance_set_actmem): the combination with multi-stage partial plans is not built");
+    const size_t nE = size_t(inst->NS) * inst->K * inst->P;
+    int32_t* d = nullptr;
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), 2 * nE * 4 + 4, 0));
+    int32_t* dq = d + nE;
+    int* dErr = reinterpret_cast<int*>(d + 2 * nE);
+    cudaError_t e = cudaMemcpyAsync(d, slow_us, nE * 4, cudaMemcpyDefault, 0);
+    if (e == cudaSuccess) e = n_stages ? cudaMemcpyAsync(dq, n_stages, nE * 4, cudaMemcpyDefault, 0) : cudaSuccess;
+    if (e == cudaSuccess) e = cudaMemsetAsync(dErr, 0, 4, 0);
+    int herr = 0;
+    if (e == cudaSuccess) {
+        const int blocks = int(std::min<size_t>((nE + 255) / 256, 4096));
+        tgValidateStagesKernel<<<std::max(blocks, 1), 256>>>(inst->time_us, d, dq, n_stages != nullptr, nE, dErr);
+        e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);
+    }
+    if (e != cudaSuccess || herr) {
+        cudaFreeAsync(d, 0);
+        if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("stage tables upload: ") + cudaGetErrorString(e));
+        return fail(TG_ERR_RANGE, "slow_us must be in [0, time_us] on every valid entry and n_stages in [1, 255]");
+    }
+    inst->slow = d;
+    inst->qst = dq;
+    return TG_OK;
+}
+
+tg_status tg_plan_pipeline_stages(tg_instance* inst, const tg_result* result, int32_t* n_out) {
+    if (!inst || !result || !n_out) return fail(TG_ERR_NULL, "NULL argument");
+    const int n = result->n_stages;
+    if (n < 0 || n > TG_MAX_K) return fail(TG_ERR_RANGE, "result.n_stages outside [0, TG_MAX_K]");
+    int total = 0;
+    for (int i = 0; i < n; ++i) {
+        const int a = result->stage_begin[i], b = i + 1 < n ? result->stage_begin[i + 1] : inst->L;
+        const int k = result->stage_island[i], p = result->stage_plan[i];
+        if (a < 0 || b <= a || b > inst->L || k < 0 || k >= inst->K || p < 0 || p >= inst->P) return fail(TG_ERR_RANGE, "result does not describe a plan of this instance");
+        int q = 1;
+        if (inst->qst) TG_CUDA(cudaMemcpy(&q, inst->qst + (size_t(tgSliceIdx(inst->L, a, b)) * inst->K + k) * inst->P + p, 4, cudaMemcpyDeviceToHost));
+        total += q;
+    }
+    *n_out = total;
     return TG_OK;
 }
 
@@ -827,6 +882,7 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
     for (int i = 0; i < n; ++i) {
         tg_instance* t = instances[i];
         if (!t) return fail(TG_ERR_NULL, "instances[" + std::to_string(i) + "] is NULL");
+        if (t->slow) return fail(TG_ERR_SHAPE, "instances[" + std::to_string(i) + "] has multi-stage partial plans: tg_prune is not built for them");
         h[i] = TgPruneDesc{t->time_us, t->mem_mb, t->actmem, t->cap_mb, t->L, t->K, t->P, t->NS * t->K};
         maxCells = std::max(maxCells, h[i].nCells);
     }

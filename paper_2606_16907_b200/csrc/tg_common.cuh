@@ -55,6 +55,8 @@ struct TgInstDev {
     const int32_t* time_us;  // [NS][K][P] (instance-owned)
     const int32_t* mem_mb;   // [NS][K][P]
     const int32_t* actmem_mb;  // [NS][K][P] MB per in-flight microbatch, or nullptr (NEXT-1: depth-aware memory)
+    const int32_t* slow_us;    // [NS][K][P] slowest internal stage of the partial plan, or nullptr (NEXT-2: multi-stage partial plans)
+    uint32_t* thr;             // NEXT-2: [nLayers][K][triG] thresholds of the cells' cost steps (diagonal-major like cd), TG_INFU = no such step
     const int32_t* cap_mb;   // [K]
     const int32_t* bw_gbps;  // [K][K]
     uint32_t* cd;            // [nDepth][K][triG] diagonal-major reduced costs, TG_INFU = none; table q-1 holds the costs
@@ -69,6 +71,9 @@ struct TgInstDev {
     uint32_t* eF;            // [TG_MAX_EVAL] their f_T
     int32_t L, K, P, m, act_mb, NS, Lp, triG;
     int32_t nDepth;          // 1, or K when actmem_mb is set
+    int32_t nLayers;         // 0, or P when slow_us is set: the cost of a cell is then a step function of T -- step j becomes
+                             // admissible at thr[j] (ascending in j) and costs cd[j], plan argp[j]; cd / argp hold nLayers tables
+    int32_t nTables;         // tables of cd / argp and key sets of the candidate sort: max(nDepth, nLayers, 1)
     int32_t sortCap, ncand;
     uint32_t cminAll[TG_MAX_K];       // min over all slices of c[.][.][k]
     uint32_t maxKey;                  // largest finite reduced cost of any depth (bounds the radix sort's passes)
@@ -148,6 +153,45 @@ struct TgSolveCtx {
     uint32_t dpT;
     int32_t dynWords;           // words of dynamic shared memory of a solver CTA
 };
+
+// Cost of one cell at threshold T (TG_INFU = no admissible plan); `off` = word offset of the cell inside a [K][triG] table
+// (island * triG + row offset + start).  Core / depth tables: the one cost if it is <= T.  NEXT-2 (nLayers > 0): the cost
+// of the last step whose threshold is <= T (the thresholds ascend with the step index).  *layer = the step taken.
+__device__ __forceinline__ uint32_t tgCostAt(const TgInstDev& I, size_t tableOff, size_t off, uint32_t T, int* layer) {
+    if (I.nLayers == 0) {
+        if (layer) *layer = 0;
+        const uint32_t c = I.cd[tableOff + off];
+        return c <= T ? c : TG_INFU;
+    }
+    const size_t stride = size_t(I.K) * I.triG;
+    uint32_t c = TG_INFU;
+    for (int j = 0; j < I.nLayers; ++j) {
+        if (I.thr[j * stride + off] > T) break;
+        c = I.cd[j * stride + off];
+        if (layer) *layer = j;
+    }
+    return c;
+}
+
+// The same for 4 consecutive starts of one row (16-byte aligned offset).
+__device__ __forceinline__ uint4 tgCostAt4(const TgInstDev& I, size_t tableOff, size_t off, uint32_t T) {
+    if (I.nLayers == 0) {
+        uint4 v = __ldg(reinterpret_cast<const uint4*>(I.cd + tableOff + off));
+        v.x = v.x <= T ? v.x : TG_INFU; v.y = v.y <= T ? v.y : TG_INFU;
+        v.z = v.z <= T ? v.z : TG_INFU; v.w = v.w <= T ? v.w : TG_INFU;
+        return v;
+    }
+    const size_t stride = size_t(I.K) * I.triG;
+    uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+    for (int j = 0; j < I.nLayers; ++j) {
+        const uint4 t = __ldg(reinterpret_cast<const uint4*>(I.thr + j * stride + off));
+        if (min(min(t.x, t.y), min(t.z, t.w)) > T) break;
+        const uint4 cj = __ldg(reinterpret_cast<const uint4*>(I.cd + j * stride + off));
+        v.x = t.x <= T ? cj.x : v.x; v.y = t.y <= T ? cj.y : v.y;
+        v.z = t.z <= T ? cj.z : v.z; v.w = t.w <= T ? cj.w : v.w;
+    }
+    return v;
+}
 
 // binomials up to 16 choose r
 __constant__ uint16_t tgBinom[17][17];

@@ -109,6 +109,19 @@ __global__ void tgExpandClassesKernel(const int32_t* __restrict__ classOf, const
     if (bad) atomicOr(err, bad);
 }
 
+// tg_instance_set_stages: 0 <= slow <= time on every valid entry, stage counts in [1, 255] (absent: all ones)
+__global__ void tgValidateStagesKernel(const int32_t* __restrict__ time_us, const int32_t* __restrict__ slow, int32_t* __restrict__ q,
+                                       bool haveQ, size_t n, int* err) {
+    int bad = 0;
+    for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += size_t(gridDim.x) * blockDim.x) {
+        const int32_t t = time_us[i];
+        if (t != TG_INVALID && (slow[i] < 0 || slow[i] > t)) bad = 1;
+        if (!haveQ) q[i] = 1;
+        else if (q[i] < 1 || q[i] > 255) bad = 1;
+    }
+    if (bad) atomicOr(err, 1);
+}
+
 __global__ void tgValidateNonNegKernel(const int32_t* __restrict__ v, size_t n, int* err) {
     int bad = 0;
     for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < n; i += size_t(gridDim.x) * blockDim.x)
@@ -181,7 +194,7 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
     __shared__ uint32_t sMin[TG_MAX_K];
     __shared__ int32_t sCap[TG_MAX_K];
     __shared__ uint32_t sMax;
-    const bool fast = PV > 0 && P == 4 * PV && I.actmem_mb == nullptr;
+    const bool fast = PV > 0 && P == 4 * PV && I.actmem_mb == nullptr && I.slow_us == nullptr;
     int4 tv[U][PVA], mv[U][PVA];
     if (fast) {
 #pragma unroll
@@ -225,6 +238,54 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
                     }
                     tgLoadEmit(I, L, K, nCells, cell, a, b, k, 1, bq, bp, prev, myMax);
                     best = bq;
+                } else if (I.slow_us != nullptr) {
+                    // NEXT-2 (multi-stage partial plans): the cell's cost steps.  The feasible plans are visited in the order of
+                    // (slowest internal stage, time, p); a plan opens a step if it lowers the cost or ties it with a lower p.
+                    const size_t e = size_t(cell) * P;
+                    const int d = b - a;
+                    const size_t off = size_t(k) * I.triG + tgGOff(L, d) + a, stride = size_t(K) * I.triG;
+                    unsigned long long prevKey = 0;      // keys are biased by +1: 0 = none visited yet
+                    uint32_t bestT = TG_INFU;
+                    int bestP = 0xff, nsteps = 0;
+                    best = TG_INFU;
+                    while (true) {
+                        unsigned long long next = ~0ull;
+                        for (int p = 0; p < P; ++p) {
+                            const int32_t t = __ldg(I.time_us + e + p);
+                            if (t == TG_INVALID || __ldg(I.mem_mb + e + p) > capk) continue;
+                            const unsigned long long key = ((unsigned long long)uint32_t(__ldg(I.slow_us + e + p)) << 34 | (unsigned long long)uint32_t(t) << 8 | (unsigned long long)p) + 1ull;
+                            if (key > prevKey && key < next) next = key;
+                        }
+                        if (next == ~0ull) break;
+                        prevKey = next;
+                        const unsigned long long kk = next - 1ull;
+                        const uint32_t sl = uint32_t(kk >> 34), t = uint32_t(kk >> 8) & 0x3ffffffu;
+                        const int p = int(kk & 0xffu);
+                        if (t < bestT || (t == bestT && p < bestP)) {
+                            bestT = t; bestP = p;
+                            I.thr[nsteps * stride + off] = sl;
+                            I.cd[nsteps * stride + off] = t;
+                            I.argp[size_t(nsteps) * nCells + cell] = uint8_t(p);
+                            I.sortbuf[size_t(nsteps) * nCells + cell] = sl;
+                            if (nsteps == 0) best = sl;            // the cell becomes admissible at its first step
+                            myMax = max(myMax, sl);
+                            ++nsteps;
+                        }
+                    }
+                    for (int j = nsteps; j < I.nLayers; ++j) {
+                        I.thr[j * stride + off] = TG_INFU;
+                        I.cd[j * stride + off] = TG_INFU;
+                        I.argp[size_t(j) * nCells + cell] = 0xff;
+                        I.sortbuf[size_t(j) * nCells + cell] = TG_INFU;
+                    }
+                    if (b == L) {   // last element of the row: INF padding up to a multiple of 4, in every layer
+                        const int rl = (L - d + 1 + 3) & ~3;
+                        for (int j = 0; j < I.nLayers; ++j)
+                            for (int pp = a + 1; pp < rl; ++pp) {
+                                I.thr[j * stride + off + (pp - a)] = TG_INFU;
+                                I.cd[j * stride + off + (pp - a)] = TG_INFU;
+                            }
+                    }
                 } else {
                     const size_t e = size_t(cell) * P;
                     best = TG_INFU;
@@ -370,7 +431,7 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
         // transfer bound (NEXT-3(b)): the finite transfer times are candidate thresholds too
         if (I.xbound) {
             const bool fin = j != k && v < TG_INFU;
-            I.sortbuf[size_t(I.NS) * K * I.nDepth + tid] = fin ? v : TG_INFU;
+            I.sortbuf[size_t(I.NS) * K * I.nTables + tid] = fin ? v : TG_INFU;
             if (fin) atomicMax(&sMaxX, v);
         }
     }
@@ -384,7 +445,8 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
         if (d >= 1 && d <= L) {
             // the row holds a = 0..L-d, padded with INF to a multiple of 4 words and 16-byte aligned: 16-byte loads,
             // four in flight; the last element (b = L) only counts for the all-slices minimum
-            const uint4* row4 = reinterpret_cast<const uint4*>(I.cd + size_t(k) * I.triG + tgGOff(L, d));
+            // (NEXT-2: a slice is admissible from the threshold of its first cost step on)
+            const uint4* row4 = reinterpret_cast<const uint4*>((I.nLayers ? I.thr : I.cd) + size_t(k) * I.triG + tgGOff(L, d));
             const int n4 = (L - d + 4) >> 2, last = L - d;
             for (int q0 = 0; q0 < n4; q0 += 4) {
                 uint4 v[4];
@@ -419,7 +481,7 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     // bitmap with shared-memory atomics and read the set bits back in order -- O(n + maxKey/32) instead of a sort.
     // Larger keys: stable LSD radix sort (8- or 9-bit digits, per-warp histograms, ping-pong between two global
     // buffers) followed by a unique pass.
-    const int n = I.NS * K * I.nDepth + (I.xbound ? K * K : 0);
+    const int n = I.NS * K * I.nTables + (I.xbound ? K * K : 0);
     const uint32_t maxKey = max(I.maxKey, sMaxX);
     const uint32_t nWords = (maxKey >> 5) + 1u;
     uint32_t base = 0;
@@ -510,8 +572,9 @@ __global__ void tgExportKernel(const TgInstDev* __restrict__ insts, int32_t* __r
         const int s = cell / K, k = cell - s * K;
         int a, b;
         tgSliceAB(L, s, a, b);
-        c_out[cell] = int32_t(I.cd[size_t(k) * I.triG + tgGOff(L, b - a) + a]);
-        const uint8_t p = I.argp[cell];
+        int layer = 0;
+        c_out[cell] = int32_t(tgCostAt(I, 0, size_t(k) * I.triG + tgGOff(L, b - a) + a, TG_TINF, &layer));
+        const uint8_t p = I.argp[size_t(layer) * nCells + cell];
         argp_out[cell] = p == 0xff ? -1 : int32_t(p);
     }
     if (blockIdx.x == 0 && threadIdx.x < K * K)

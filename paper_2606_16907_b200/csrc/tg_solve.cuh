@@ -146,16 +146,15 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
             const int w = f - int(sm.baseK[kc] >> 2);
             const int dk = sm.dmaxK[kc], Dk = (dk + 3) & ~3;
             if (w >= Dk * nb4) continue;   // the pad between two islands' tables
-            const uint32_t* cdk = I.cd + sm.cdOff + size_t(sm.isl[kc]) * I.triG;
             const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
             uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
             if (d <= dk && a4 < ((L - d + 3) >> 2)) {
-                v = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + a4);
+                v = tgCostAt4(I, sm.cdOff, size_t(sm.isl[kc]) * I.triG + tgGOff(L, d) + 4 * a4, T);
                 const int a = a4 * 4, amax = L - 1 - d;
-                v.x = (a + 0 <= amax && v.x <= T) ? v.x : TG_INFU;
-                v.y = (a + 1 <= amax && v.y <= T) ? v.y : TG_INFU;
-                v.z = (a + 2 <= amax && v.z <= T) ? v.z : TG_INFU;
-                v.w = (a + 3 <= amax && v.w <= T) ? v.w : TG_INFU;
+                v.x = (a + 0 <= amax) ? v.x : TG_INFU;
+                v.y = (a + 1 <= amax) ? v.y : TG_INFU;
+                v.z = (a + 2 <= amax) ? v.z : TG_INFU;
+                v.w = (a + 3 <= amax) ? v.w : TG_INFU;
                 nAdm += (v.x < TG_INFU) + (v.y < TG_INFU) + (v.z < TG_INFU) + (v.w < TG_INFU);
             }
             reinterpret_cast<uint4*>(Cs + sm.baseK[kc])[w] = v;
@@ -178,7 +177,7 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
         }
         if (count)
             for (int kc = 0; kc < Ke; ++kc) {
-                const uint32_t* cdk = I.cd + sm.cdOff + size_t(sm.isl[kc]) * I.triG;
+                const uint32_t* cdk = (I.nLayers ? I.thr : I.cd + sm.cdOff) + size_t(sm.isl[kc]) * I.triG;   // (NEXT-2: admissible from the first step on)
                 for (int d = 1; d <= sm.dmaxK[kc]; ++d)
                     for (int a = tid; a <= L - 1 - d; a += TG_NT) nAdm += cdk[tgGOff(L, d) + a] <= T ? 1u : 0u;
             }
@@ -316,8 +315,7 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
         const int kc = w / Wd, a = tgLo4(sm, sm.maxlenK[kc]) + (w - kc * Wd);
         uint32_t v = TG_INFU;
         if (a < L) {
-            v = I.cd[size_t(sm.isl[kc]) * I.triG + tgGOff(L, L - a) + a];
-            if (v > T) v = TG_INFU;
+            v = tgCostAt(I, 0, size_t(sm.isl[kc]) * I.triG + tgGOff(L, L - a) + a, T, nullptr);
         }
         G[w] = v;
         if (post && a == 0 && v < TG_INFU)
@@ -482,12 +480,12 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
                 const int d = dq + 1 + e;                                                      \
                 c4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);                           \
                 if (d <= dm && c < ((L - d + 3) >> 2)) {                                       \
-                    c4 = __ldg(reinterpret_cast<const uint4*>(cdk + tgGOff(L, d)) + c);        \
+                    c4 = tgCostAt4(I, sm.cdOff, cdkOff + tgGOff(L, d) + 4 * c, T);             \
                     const int amax = L - 1 - d;                                                \
-                    c4.x = (a0 + 0 <= amax && c4.x <= T) ? c4.x : TG_INFU;                     \
-                    c4.y = (a0 + 1 <= amax && c4.y <= T) ? c4.y : TG_INFU;                     \
-                    c4.z = (a0 + 2 <= amax && c4.z <= T) ? c4.z : TG_INFU;                     \
-                    c4.w = (a0 + 3 <= amax && c4.w <= T) ? c4.w : TG_INFU;                     \
+                    c4.x = (a0 + 0 <= amax) ? c4.x : TG_INFU;                                  \
+                    c4.y = (a0 + 1 <= amax) ? c4.y : TG_INFU;                                  \
+                    c4.z = (a0 + 2 <= amax) ? c4.z : TG_INFU;                                  \
+                    c4.w = (a0 + 3 <= amax) ? c4.w : TG_INFU;                                  \
                 }                                                                              \
             } else {                                                                           \
                 c4 = tgLds4(cA + e * cStride);                                                 \
@@ -525,7 +523,7 @@ __device__ __forceinline__ void tgPhase2B(const TgSolveCtx& ctx, const TgShared&
             const int dm = sm.dmaxTile[k][c], q0 = max(0, dq4 - 1 - cw);
             const int nq = min((dm + 3) >> 2, nbw - cw + dq4 + 1);
             if (q0 < nq) {
-                const uint32_t* cdk = GLOBALC ? I.cd + sm.cdOff + size_t(sm.isl[k]) * I.triG : nullptr;
+                const size_t cdkOff = size_t(sm.isl[k]) * I.triG;   // island k's table (L2 fallback of the cost rows)
                 uint32_t hA = hAddr + hrow * HSB + 16u + uint32_t(4 * (cw + q0 - dq4)) * 4u;
                 uint32_t cA = csBase + (sm.baseK[k] + uint32_t(a0)) * 4u + uint32_t(4 * q0) * cStride;
                 int dq = 4 * q0;
@@ -790,7 +788,7 @@ __device__ __forceinline__ void tgPhase2W(const TgSolveCtx& ctx, const TgShared&
     for (int s = g; s < nk; s += NG) {
         const int k = kl[s];
         const int lo4S = max(0, Lw - capR - int(sm.maxlenK[k])) & ~3, dq4 = (lo4R - lo4S) >> 2;
-        const uint32_t* cdk = GLOBALC ? I.cd + sm.cdOff + size_t(sm.isl[k]) * I.triG : nullptr;
+        const size_t cdkOff = size_t(sm.isl[k]) * I.triG;   // island k's table (L2 fallback of the cost rows)
         const uint32_t cBase = csBase + (sm.baseK[k] + uint32_t(lo4S)) * 4u, hRow = hAddr0 + uint32_t(s) * rowBytes + 16u;
         uint32_t* const gOut = gRow + size_t(s) * Wd;
         for (int cw = c0; cw < nbw; cw += CH) {
@@ -962,17 +960,18 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
             const uint32_t* Gl = slot + tgLevelOff(0, Ke, Wd, r - 1);
             // this stage is followed by r later ones: its cost and plan come from the table of depth r + 1
             const size_t dq = I.nDepth > 1 ? size_t(r) : 0;
-            const uint32_t* cdk = I.cd + (dq * K + ko) * I.triG;
             int capR = 0;   // every source row (R\{j}, j) starts at start lo4(cap(R))
             for (int j = 0; j < Ke; ++j) if (R >> j & 1u) capR += sm.maxlenK[j];
             const int lo4R = tgLo4(sm, capR);
             unsigned long long best = TG_KEY_NONE;
+            int bestLayer = 0;   // NEXT-2: the cost step the winning slice took (selects its plan)
             // lanes over (member j, boundary b) pairs, b inside the source rows' window: every load is independent
             const int bLo = max(a + 1, lo4R), nb = min(L - 1, lo4R + Wd - 1) - bLo + 1;
             for (int p = lane; p < nb * r; p += 32) {
                 const int ji = p / nb, bb = bLo + (p - ji * nb);
-                const uint32_t c = cdk[tgGOff(L, bb - a) + a];
-                if (c > T) continue;
+                int layer = 0;
+                const uint32_t c = tgCostAt(I, dq * K * I.triG, size_t(ko) * I.triG + tgGOff(L, bb - a) + a, T, &layer);
+                if (c >= TG_INFU) continue;
                 const int j = int(__fns(R, 0, ji + 1));
                 const uint32_t Rp = R ^ (1u << j);
                 const size_t row = size_t(ctx.rankOf[Rp]) * (Ke - r + 1) + (j - __popc(R & ((1u << j) - 1u)));
@@ -982,21 +981,25 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
                 if (v >= TG_INFU) continue;
                 // lowest value, then lowest b, then lowest j
                 const unsigned long long kk = (unsigned long long)v << 32 | (unsigned long long)bb << 8 | (unsigned long long)j;
-                best = kk < best ? kk : best;
+                if (kk < best) { best = kk; bestLayer = layer; }
             }
             for (int o = 16; o > 0; o >>= 1) {
                 const unsigned long long ot = __shfl_xor_sync(0xffffffffu, best, o);
-                best = ot < best ? ot : best;
+                const int ol = __shfl_xor_sync(0xffffffffu, bestLayer, o);
+                if (ot < best) { best = ot; bestLayer = ol; }
             }
             if (best == TG_KEY_NONE) { bad = true; break; }
             b = int(best >> 8) & 0xffffff;
             const int j = int(best & 0xffu);
-            sb[n] = a; si[n] = ko; sp[n] = I.argp[dq * size_t(I.NS) * K + size_t(tgSliceIdx(L, a, b)) * K + ko];
+            const size_t tbl = I.nLayers ? size_t(bestLayer) : dq;   // (the layer depends on (a, b, k) only: every lane with the winning b agrees)
+            sb[n] = a; si[n] = ko; sp[n] = I.argp[tbl * size_t(I.NS) * K + size_t(tgSliceIdx(L, a, b)) * K + ko];
             ++n;
             a = b; k = j; R ^= 1u << j;
             continue;
         }
-        sb[n] = a; si[n] = ko; sp[n] = I.argp[size_t(tgSliceIdx(L, a, b)) * K + ko];
+        int lastLayer = 0;
+        tgCostAt(I, 0, size_t(ko) * I.triG + tgGOff(L, b - a) + a, T, &lastLayer);
+        sb[n] = a; si[n] = ko; sp[n] = I.argp[size_t(lastLayer) * I.NS * K + size_t(tgSliceIdx(L, a, b)) * K + ko];
         ++n;
         break;
     }

@@ -3,7 +3,7 @@
 configs of BASELINE.json, which take the oracle minutes and so cannot be recomputed inside the test run.
 Calls ONLY oracle/ and the seeded input generator; never the CUDA path.
 
-    python tests/golden/make_expected.py cfg3 cfg4 cfg5 cfg3x cfg4x cfg3d cfg3xb cfg4d cfg4xb   (cfg5 = all 1024 seeds, about 35 min on 8 cores)
+    python tests/golden/make_expected.py cfg3 cfg4 cfg5 cfg3x cfg4x cfg3d cfg3xb cfg3st cfg4d cfg4xb   (cfg5 = all 1024 seeds, about 35 min on 8 cores)
 
 Also stores oracle.dp_at results at fixed quantile thresholds (single-DP parity for tg_dp_at)."""
 import json
@@ -62,6 +62,12 @@ def main():
             data = [{"name": inst.name, "L": inst.L, "K": inst.K, "P": inst.P, "m": inst.m,
                      "solve": rec(oracle.solve_variant(inst)), "core": rec(oracle.solve(inst, n_threads=threads)),
                      "oracle_seconds": round(time.time() - t0, 1)}]
+        elif name == "cfg3st":     # NEXT-2: the 70B-like config with multi-stage partial plans (stages oracle)
+            inst = gen.with_stages(gen.config3(), 3)
+            t0 = time.time()
+            r, tq = oracle.solve_stages(inst)
+            data = [{"name": inst.name, "L": inst.L, "K": inst.K, "P": inst.P, "m": inst.m, "solve": rec(r),
+                     "pipeline_stages": tq, "oracle_seconds": round(time.time() - t0, 1)}]
         elif name in ("cfg4d", "cfg4xb"):   # the K = 16 variant workloads bench.py times: threaded variant oracle (same arithmetic)
             inst = gen.with_actmem(gen.config4(), 11, 300, 3000) if name == "cfg4d" else gen.with_transfer_bound(gen.config4())
             t0 = time.time()
