@@ -238,5 +238,20 @@ def bruteforce_stages(inst):
     return _conv(r), tot.value, n.value
 
 
+def islands(gpus, comp, mem_mb, intra, inter, eps_c: int, eps_m: int, eps_i: int):
+    """NEXT-4: island construction from per-node profiles (tolerances in permille).
+    Returns (island_of_node [N], island_gpus [K], island_cap_mb [K], bw [K,K])."""
+    g, c, mm, b = (np.ascontiguousarray(a, dtype=np.int32) for a in (gpus, comp, mem_mb, intra))
+    e = np.ascontiguousarray(inter, dtype=np.int32)
+    N = g.size
+    of = np.zeros(N, dtype=np.int32)
+    ig, ic, bw = np.zeros(N, dtype=np.int32), np.zeros(N, dtype=np.int32), np.zeros(N * N, dtype=np.int32)
+    K = C.c_int32(0)
+    lib().orc_islands(C.c_int(N), _p32(g), _p32(c), _p32(mm), _p32(b), _p32(e), C.c_int(eps_c), C.c_int(eps_m), C.c_int(eps_i),
+                      _p32(of), C.byref(K), _p32(ig), _p32(ic), _p32(bw))
+    k = K.value
+    return of, ig[:k].copy(), ic[:k].copy(), bw[:k * k].reshape(k, k).copy()
+
+
 def hw_threads() -> int:
     return lib().orc_hw_threads()

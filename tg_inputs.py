@@ -322,5 +322,44 @@ def with_stages(inst: Instance, seed: int, qmax: int = 4) -> Instance:
     return o
 
 
+# ---- NEXT-4: cluster profiles for the island construction (PAPER.md:177 per-GPU attributes, given per node) -------------
+# GPU types of Tab. 3: (relative compute, memory MB, intra-node link GB/s: PCIe 32, NVLink 300/600/900).
+# The paper prints no bandwidth figures: nodes bought together share a dedicated interconnect, modelled as
+# 100 GB/s between nodes of one type and 25 GB/s across types.
+GPU_TYPES = {"T4": (65, 16000, 32), "V100-16": (125, 16000, 32), "V100-32": (125, 32000, 300),
+             "A100-80": (312, 80000, 600), "H100NVL": (835, 94000, 900)}
+CLUSTERS = {"C1": [("T4", 4, 4), ("V100-16", 4, 4)],                                   # (type, nodes, GPUs per node)
+            "C2": [("A100-80", 2, 4), ("H100NVL", 4, 2)],
+            "C3": [("T4", 1, 4), ("V100-16", 1, 4), ("V100-32", 1, 8), ("A100-80", 1, 4)]}
+
+
+def cluster_profile(name: str, same: int = 100, cross: int = 25):
+    """(gpus, comp, mem_mb, intra, inter [N,N]) of an evaluation cluster of PAPER.md Tab. 3."""
+    gp, cp, mm, ib, ty = [], [], [], [], []
+    for t, nodes, g in CLUSTERS[name]:
+        c, m, b = GPU_TYPES[t]
+        for _ in range(nodes):
+            gp.append(g); cp.append(c); mm.append(m); ib.append(b); ty.append(t)
+    n = len(gp)
+    inter = np.array([[0 if i == j else (same if ty[i] == ty[j] else cross) for j in range(n)] for i in range(n)], dtype=np.int32)
+    return (np.array(gp, np.int32), np.array(cp, np.int32), np.array(mm, np.int32), np.array(ib, np.int32), inter)
+
+
+def random_cluster(seed: int, nmax: int = 12):
+    """A random cluster: 2-nmax nodes drawn from a few GPU types with a few percent of spread, asymmetric links."""
+    n = int(urand(seed, S_MISC + 50, 0, 2, nmax))
+    idx = np.arange(n)
+    types = list(GPU_TYPES.values())
+    t = urand(seed, S_MISC + 51, idx, 0, len(types) - 1)
+    gp = 1 << urand(seed, S_MISC + 52, t, 1, 3)                                       # GPUs per node follow the type
+    comp = np.array([types[i][0] for i in t]) * urand(seed, S_MISC + 53, idx, 97, 103) // 100
+    mem = np.array([types[i][1] for i in t]) * urand(seed, S_MISC + 54, idx, 99, 101) // 100
+    intra = np.array([types[i][2] for i in t])
+    pair = idx[:, None] * n + idx[None, :]
+    inter = np.where(t[:, None] == t[None, :], urand(seed, S_MISC + 55, pair, 80, 120), urand(seed, S_MISC + 56, pair, 10, 90))
+    np.fill_diagonal(inter, 0)
+    return (gp.astype(np.int32), comp.astype(np.int32), mem.astype(np.int32), intra.astype(np.int32), inter.astype(np.int32))
+
+
 def by_name(name: str, seed: int = 0):
     return {"cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4}[name](seed)
