@@ -47,6 +47,7 @@ enum {
     TG_MAX_P = 255,
     TG_MAX_M = 1 << 20,
     TG_TIME_MAX = 1 << 25,
+    TG_MAX_NODES = 64,       /* nodes of a cluster profile (tg_islands_build)     */
     TG_INVALID = 0x7fffffff, /* "no such intra-slice plan" marker in time_us */
     TG_INF = 1 << 30         /* saturating "no plan" value of the DP        */
 };
@@ -252,6 +253,24 @@ tg_status tg_dp_at(tg_instance* inst, int64_t T, tg_result* out, void* cuda_stre
 
 /* Copies the instance's current time table (after pruning) to HOST time_out [NS][K][P]. */
 tg_status tg_instance_read_time(tg_instance* inst, int32_t* time_out);
+
+/* tg_islands_build — SURVEY.md §8(f) NEXT-4: GPU island construction as a front end that produces the
+ * island arguments of tg_instance_create from per-node profiles.  All pointers HOST.
+ *   node_gpus / node_compute / node_mem_mb / node_intra_bw  [n_nodes]: GPUs of the node and, per GPU, compute capacity
+ *             (any unit), memory in MB and intra-node interconnect bandwidth (the GPUs of a node are identical)
+ *   inter_bw  [n_nodes][n_nodes] sender-major network bandwidth between nodes (directional), diagonal ignored
+ *   eps_c / eps_m / eps_i  tolerances of Eq. 1-2 in permille (100 = 10 %)
+ * Islands satisfy PAPER.md Eq. 1-3 (same GPU count, compute / memory / intra-node bandwidth ratios within 1 + eps, every
+ * link inside an island at least as fast as every link leaving it) and are built by the three steps of PAPER.md:193 as
+ * DESIGN.md reading N4 fixes them (run-cutting by compute, memory and intra-node bandwidth, then greedy agglomerative
+ * clustering on the inter-node bandwidth).  Outputs: island_of_node [n_nodes]; *k_out = K; island_gpus [K], island_cap_mb
+ * [K] (smallest memory of the island), bw_gbps [K][K] (slowest link from a node of j to a node of k; diagonal: slowest
+ * inner link, or the intra-node bandwidth of a single-node island) -- buffers of n_nodes (n_nodes^2) entries suffice.
+ * 1 <= n_nodes <= TG_MAX_NODES else TG_ERR_SHAPE; values < 1 (memory < 0) or above 2^20 -> TG_ERR_RANGE.  K may exceed
+ * TG_MAX_K: tg_instance_create then rejects it.  Runs one small kernel; synchronises the legacy default stream. */
+tg_status tg_islands_build(int32_t n_nodes, const int32_t* node_gpus, const int32_t* node_compute, const int32_t* node_mem_mb,
+                           const int32_t* node_intra_bw, const int32_t* inter_bw, int32_t eps_c, int32_t eps_m, int32_t eps_i,
+                           int32_t* island_of_node, int32_t* k_out, int32_t* island_gpus, int32_t* island_cap_mb, int32_t* bw_gbps);
 
 /* Returns the workspaces cached by the library's memory pool on the current device to the driver (an embedding
  * framework with an allocator of its own may need the memory back).  Synchronises the device.  No-op before the first call. */

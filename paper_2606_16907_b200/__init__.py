@@ -66,7 +66,7 @@ class TangramError(RuntimeError):
 
 _lib = None
 EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_set_stages", "tg_plan_pipeline_stages", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
-           "tg_reduce", "tg_candidates", "tg_dp_at", "tg_instance_read_time", "tg_release_cached_memory", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
+           "tg_reduce", "tg_candidates", "tg_dp_at", "tg_instance_read_time", "tg_islands_build", "tg_release_cached_memory", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
 
 
 def lib():
@@ -97,6 +97,7 @@ def lib():
         L.tg_candidates.argtypes = [vp, vp, i64, C.POINTER(i32), vp]
         L.tg_dp_at.argtypes = [vp, i64, vp, vp]
         L.tg_instance_read_time.argtypes = [vp, vp]
+        L.tg_islands_build.argtypes = [i32, vp, vp, vp, vp, vp, i32, i32, i32, vp, C.POINTER(i32), vp, vp, vp]
         L.tg_last_solver_kernel_ms.argtypes = [C.POINTER(C.c_float)]
         L.tg_last_loader_kernel_ms.argtypes = [C.POINTER(C.c_float)]
         L.tg_last_error.restype = C.c_char_p
@@ -302,6 +303,18 @@ def tg_prune_batch(instances, mode: int = TG_PRUNE_EXACT, threshold: int = 0, st
     counts = (C.c_int64 * (4 * max(n, 1)))()
     _check(lib().tg_prune_batch(_handles(instances), n, mode, threshold, counts, _stream_ptr(stream)))
     return np.array(list(counts), dtype=np.int64)[:4 * n].reshape(n, 4)
+
+
+def tg_islands_build(node_gpus, node_compute, node_mem_mb, node_intra_bw, inter_bw, eps_c: int, eps_m: int, eps_i: int):
+    """NEXT-4: islands from per-node profiles.  Returns (island_of_node [N], island_gpus [K], island_cap_mb [K], bw [K,K])."""
+    g, c, mm, ib = (np.ascontiguousarray(a, dtype=np.int32) for a in (node_gpus, node_compute, node_mem_mb, node_intra_bw))
+    e = np.ascontiguousarray(inter_bw, dtype=np.int32)
+    n = g.size
+    of, ig, ic, bw = (np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n * n, np.int32))
+    k = C.c_int32(0)
+    _check(lib().tg_islands_build(n, g.ctypes.data, c.ctypes.data, mm.ctypes.data, ib.ctypes.data, e.ctypes.data, eps_c, eps_m, eps_i,
+                                  of.ctypes.data, C.byref(k), ig.ctypes.data, ic.ctypes.data, bw.ctypes.data))
+    return of, ig[:k.value].copy(), ic[:k.value].copy(), bw[:k.value * k.value].reshape(k.value, k.value).copy()
 
 
 def tg_release_cached_memory():

@@ -9,7 +9,7 @@ _DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_DIR, "csrc")
 LIB = os.path.join(_DIR, "libtangram.so")
 SOURCES = ["tg_api.cu"]
-HEADERS = ["tg_common.cuh", "tg_prep.cuh", "tg_solve.cuh", os.path.join("..", "..", "include", "tangram.h")]
+HEADERS = ["tg_common.cuh", "tg_prep.cuh", "tg_solve.cuh", "tg_islands.cuh", os.path.join("..", "..", "include", "tangram.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

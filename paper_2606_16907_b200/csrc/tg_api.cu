@@ -12,6 +12,7 @@
 #include "tg_common.cuh"
 #include "tg_prep.cuh"
 #include "tg_solve.cuh"
+#include "tg_islands.cuh"
 
 // One device allocation shared by the instances of a tg_instance_create_batch call; freed with the last of them.
 struct TgBatchBlock {
@@ -937,6 +938,59 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
 tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int64_t counts_out[4], void* cuda_stream) {
     if (!inst || !counts_out) return fail(TG_ERR_NULL, "NULL argument");
     return tg_prune_batch(&inst, 1, mode, threshold, counts_out, cuda_stream);
+}
+
+tg_status tg_islands_build(int32_t n_nodes, const int32_t* node_gpus, const int32_t* node_compute, const int32_t* node_mem_mb,
+                           const int32_t* node_intra_bw, const int32_t* inter_bw, int32_t eps_c, int32_t eps_m, int32_t eps_i,
+                           int32_t* island_of_node, int32_t* k_out, int32_t* island_gpus, int32_t* island_cap_mb, int32_t* bw_gbps) {
+    if (!node_gpus || !node_compute || !node_mem_mb || !node_intra_bw || !inter_bw || !island_of_node || !k_out || !island_gpus ||
+        !island_cap_mb || !bw_gbps)
+        return fail(TG_ERR_NULL, "NULL argument");
+    if (n_nodes < 1 || n_nodes > TG_MAX_NODES) return fail(TG_ERR_SHAPE, "n_nodes outside [1, TG_MAX_NODES]");
+    if (eps_c < 0 || eps_m < 0 || eps_i < 0 || eps_c > 1000000 || eps_m > 1000000 || eps_i > 1000000)
+        return fail(TG_ERR_RANGE, "tolerances must be in [0, 10^6] permille");
+    const int N = n_nodes;
+    for (int n = 0; n < N; ++n) {
+        if (node_gpus[n] < 1 || node_compute[n] < 1 || node_mem_mb[n] < 0 || node_intra_bw[n] < 1)
+            return fail(TG_ERR_RANGE, "node " + std::to_string(n) + ": gpus, compute and intra-node bandwidth must be >= 1, memory >= 0");
+        if (node_gpus[n] > (1 << 20) || node_compute[n] > (1 << 20) || node_intra_bw[n] > (1 << 20))
+            return fail(TG_ERR_RANGE, "node " + std::to_string(n) + ": value above 2^20");
+        for (int m = 0; m < N; ++m)
+            if (m != n && (inter_bw[size_t(n) * N + m] < 1 || inter_bw[size_t(n) * N + m] > (1 << 20)))
+                return fail(TG_ERR_RANGE, "inter_bw must be in [1, 2^20] off the diagonal");
+    }
+    int dev = 0;
+    TG_CUDA(cudaGetDevice(&dev));
+    DeviceState* D;
+    tg_status st = deviceInit(dev, &D);
+    if (st != TG_OK) return st;
+    // one device buffer: [gpus | comp | mem | intra | inter | islandOf | K | islandGpus | islandCap | bw]
+    const size_t nIn = size_t(4) * N + size_t(N) * N, nOut = size_t(N) + 1 + 2 * size_t(N) + size_t(N) * N;
+    std::vector<int32_t> h(nIn + nOut, 0);
+    memcpy(h.data(), node_gpus, N * 4); memcpy(h.data() + N, node_compute, N * 4); memcpy(h.data() + 2 * N, node_mem_mb, N * 4);
+    memcpy(h.data() + 3 * N, node_intra_bw, N * 4); memcpy(h.data() + 4 * N, inter_bw, size_t(N) * N * 4);
+    int32_t* d = nullptr;
+    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), h.size() * 4, 0));
+    cudaError_t e = cudaMemcpyAsync(d, h.data(), nIn * 4, cudaMemcpyHostToDevice, 0);
+    if (e == cudaSuccess) {
+        TgIslandsArgs A;
+        A.N = N; A.gpus = d; A.comp = d + N; A.mem = d + 2 * N; A.intra = d + 3 * N; A.inter = d + 4 * N;
+        A.epsC = eps_c; A.epsM = eps_m; A.epsI = eps_i;
+        A.islandOf = d + nIn; A.K = A.islandOf + N; A.islandGpus = A.K + 1; A.islandCap = A.islandGpus + N; A.bw = A.islandCap + N;
+        tgIslandsKernel<<<1, TG_ISL_NT>>>(A);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(h.data() + nIn, d + nIn, nOut * 4, cudaMemcpyDeviceToHost);
+    cudaFreeAsync(d, 0);
+    if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("tg_islands_build: ") + cudaGetErrorString(e));
+    const int32_t* o = h.data() + nIn;
+    const int K = o[N];
+    memcpy(island_of_node, o, N * 4);
+    *k_out = K;
+    memcpy(island_gpus, o + N + 1, K * 4);
+    memcpy(island_cap_mb, o + 2 * N + 1, K * 4);
+    memcpy(bw_gbps, o + 3 * N + 1, size_t(K) * K * 4);
+    return TG_OK;
 }
 
 tg_status tg_release_cached_memory(void) {
