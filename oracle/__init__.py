@@ -17,7 +17,10 @@ _SRC = os.path.join(_DIR, "tangram_oracle.cpp")
 _SRC_DEPTH = os.path.join(_DIR, "tangram_oracle_depth.cpp")   # NEXT-1 variant, separate translation unit
 _SRC_STAGES = os.path.join(_DIR, "tangram_oracle_stages.cpp")  # NEXT-2 variant, separate translation unit
 _SRC_ISLANDS = os.path.join(_DIR, "tangram_oracle_islands.cpp")  # NEXT-4 front end, separate translation unit
-_SO = os.path.join(_DIR, "libtangram_oracle.so")
+# TG_ORACLE_LIB / TG_ORACLE_CXXFLAGS: an instrumented build beside the plain one (the CPU suite under
+# AddressSanitizer + UBSan:  TG_ORACLE_LIB=oracle/libtangram_oracle_asan.so TG_ORACLE_CXXFLAGS="-fsanitize=address,undefined
+# -fno-sanitize-recover=all -g" LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 pytest -m "not gpu")
+_SO = os.path.abspath(os.environ.get("TG_ORACLE_LIB", os.path.join(_DIR, "libtangram_oracle.so")))
 MAXK = 16
 INF = 1 << 30
 INT64_MAX = (1 << 63) - 1

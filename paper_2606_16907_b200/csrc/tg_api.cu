@@ -335,7 +335,23 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const int P0 = instances[0]->P;
     if (!g_evL0) { TG_CUDA(cudaEventCreate(&g_evL0)); TG_CUDA(cudaEventCreate(&g_evL1)); }
     TG_CUDA(cudaEventRecord(g_evL0, st));
-    if (wide) {
+    // a batch of plain instances with P = 4 or 8 that fills the GPU takes the row-group loader (reduced costs transposed
+    // through shared memory, 32-byte runs into the diagonal-major tables)
+    bool rows = wide && (P0 == 4 || P0 == 8) && size_t(maxK) * (maxLp) * TG_LOAD_RG * 4 <= size_t(96) * 1024;
+    for (int i = 0; i < n && rows; ++i) rows = instances[i]->P == P0 && !instances[i]->actmem && !instances[i]->slow;
+    if (rows) {
+        int maxL = 1;
+        for (int i = 0; i < n; ++i) maxL = std::max(maxL, int(instances[i]->L));
+        const dim3 gr((maxL + TG_LOAD_RG - 1) / TG_LOAD_RG, n);
+        const size_t sh = size_t(maxK) * maxL * TG_LOAD_RG * 4;
+        if (P0 == 4) {
+            TG_CUDA(cudaFuncSetAttribute(tgLoadRowsKernel<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+            tgLoadRowsKernel<1, 4><<<gr, 256, sh, st>>>(W.inst);
+        } else {
+            TG_CUDA(cudaFuncSetAttribute(tgLoadRowsKernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
+            tgLoadRowsKernel<2, 2><<<gr, 256, sh, st>>>(W.inst);
+        }
+    } else if (wide) {
         if (P0 == 4) tgLoadKernel<1, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);
         else if (P0 == 8) tgLoadKernel<2, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);
         else tgLoadKernel<0, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);

@@ -326,6 +326,97 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
     if (threadIdx.x == 0 && sMax) atomicMax(&I.maxKey, sMax);
 }
 
+// Step 1 for batches of plain instances (P = 4 * PV plans, no footprint / stage tables), the HBM-bound stream of the path
+// (385 MB at the 1024-instance batch).  A CTA takes TG_LOAD_RG consecutive start rows a0 .. a0+7 of one instance -- a
+// contiguous stretch of the raw tables -- reduces its cells from registers (16-byte loads, U cells of a thread in flight)
+// and collects the reduced costs in a shared-memory tile [island][diagonal][8 starts]; the tile is then written to the
+// diagonal-major tables as 32-byte runs (two 16-byte stores of neighbouring lanes = one full sector).  The cell-order
+// kernel above writes one 4-byte word per sector there (12 sectors per store request, profiles/r1c_ncu_cfg5_loader.md).
+#define TG_LOAD_RG 8
+template <int PV, int U>
+__global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ insts) {
+    extern __shared__ uint32_t tile[];   // [K][L][TG_LOAD_RG]
+    TgInstDev& I = insts[blockIdx.y];
+    const int L = I.L, K = I.K;
+    const int a0 = int(blockIdx.x) * TG_LOAD_RG;
+    if (a0 >= L) return;
+    const int a1 = min(L, a0 + TG_LOAD_RG);
+    const int nCells = I.NS * K;
+    const int cellBeg = tgSliceIdx(L, a0, a0 + 1) * K, cellEnd = a1 < L ? tgSliceIdx(L, a1, a1 + 1) * K : nCells;
+    __shared__ uint32_t sMin[TG_MAX_K];
+    __shared__ int32_t sCap[TG_MAX_K];
+    __shared__ uint32_t sMax;
+    const int tid = threadIdx.x;
+    for (int w = tid; w < K * L * TG_LOAD_RG; w += 256) tile[w] = TG_INFU;
+    if (tid < TG_MAX_K) { sMin[tid] = TG_INFU; sCap[tid] = tid < K ? __ldg(I.cap_mb + tid) : 0; }
+    if (tid == 0) sMax = 0;
+    __syncthreads();
+    uint32_t myMax = 0;
+    const int ds = 256 / K, dk = 256 - ds * K;
+    for (int base = cellBeg; base < cellEnd; base += 256 * U) {
+        int4 tv[U][PV], mv[U][PV];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int cell = base + 256 * u + tid;
+            if (cell < cellEnd) {
+                const int4* t4 = reinterpret_cast<const int4*>(I.time_us + size_t(cell) * (4 * PV));
+                const int4* m4 = reinterpret_cast<const int4*>(I.mem_mb + size_t(cell) * (4 * PV));
+#pragma unroll
+                for (int v = 0; v < PV; ++v) { tv[u][v] = __ldg(t4 + v); mv[u][v] = __ldg(m4 + v); }
+            }
+        }
+        const int cellFirst = base + tid;
+        if (cellFirst < cellEnd) {
+            const int s0 = cellFirst / K;
+            int k = cellFirst - s0 * K, a, b;
+            tgSliceAB(L, s0, a, b);
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int cell = cellFirst + 256 * u;
+                if (cell < cellEnd) {
+                    const int32_t capk = sCap[k];
+                    uint32_t bq = TG_INFU; int bp = 0xff;
+#pragma unroll
+                    for (int v = 0; v < PV; ++v) {
+                        const int32_t t4[4] = {tv[u][v].x, tv[u][v].y, tv[u][v].z, tv[u][v].w};
+                        const int32_t m4[4] = {mv[u][v].x, mv[u][v].y, mv[u][v].z, mv[u][v].w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            if (t4[e] != TG_INVALID && m4[e] <= capk && uint32_t(t4[e]) < bq) { bq = uint32_t(t4[e]); bp = 4 * v + e; }
+                    }
+                    tile[(k * L + (b - a - 1)) * TG_LOAD_RG + (a - a0)] = bq;
+                    I.argp[cell] = uint8_t(bp);
+                    I.sortbuf[cell] = bq;
+                    if (bq < TG_INFU) myMax = max(myMax, bq);
+                    if (bq < sMin[k]) atomicMin(&sMin[k], bq);
+                    // the thread's next cell: 256 cells = ds slices and dk islands further on
+                    int adv = ds;
+                    k += dk;
+                    if (k >= K) { k -= K; ++adv; }
+                    int pos = b - a - 1 + adv;
+                    while (a < L && pos >= L - a) { pos -= L - a; ++a; }
+                    b = a + 1 + pos;
+                }
+            }
+        }
+    }
+    myMax = __reduce_max_sync(0xffffffffu, myMax);
+    if ((tid & 31) == 0 && myMax) atomicMax(&sMax, myMax);
+    __syncthreads();
+    // tile -> diagonal-major rows: row d of island k holds a = 0 .. L-d, padded with INF to a multiple of 4 words; this
+    // CTA owns the starts a0 .. a0+7 of every row that reaches them
+    const int nd = L - a0;                                   // diagonals with an entry at start a0
+    for (int w = tid; w < K * nd * 2; w += 256) {
+        const int q = w & 1, r = w >> 1, k = r / nd, d = 1 + (r - k * nd);
+        const int a = a0 + 4 * q, rl = (L - d + 1 + 3) & ~3;  // padded row length
+        if (a < rl)
+            *reinterpret_cast<uint4*>(I.cd + size_t(k) * I.triG + tgGOff(L, d) + a) =
+                *reinterpret_cast<const uint4*>(tile + (k * L + (d - 1)) * TG_LOAD_RG + 4 * q);
+    }
+    if (tid < K && sMin[tid] < TG_INFU) atomicMin(&I.cminAll[tid], sMin[tid]);
+    if (tid == 0 && sMax) atomicMax(&I.maxKey, sMax);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Steps 2-3 and per-instance DP metadata.  One CTA per instance.
 //   x[j][k] = ceil(act_mb*1000 / bw[j][k])

@@ -18,6 +18,9 @@
 #include "tg_prep.cuh"
 
 #define TG_NW (TG_NT / 32)     // warps per CTA
+#ifndef TG_STAGE_TMA
+#define TG_STAGE_TMA 0          // 1: stage the cost rows with TMA bulk copies (A/B variant, see tgStageCosts)
+#endif
 #define TG_NB_MAX 256   // masks per batch, upper bound (row index inside a batch fits 16 bits: 256 * 16)
 #define TG_DESC_W 6     // words of a mask descriptor: R | cap(R) << 16, pad, non-members (16 nibbles), members (16 nibbles)
 
@@ -54,9 +57,15 @@ struct TgShared {
     int iTmp[8];
     unsigned long long llTmp[2];
     int curItem;
+#if TG_STAGE_TMA
+    alignas(8) unsigned long long mbar;   // completion barrier of the bulk copies of the cost rows
+    uint32_t mbarPhase;
+#endif
     long long tmark;                // phase timer of thread 0
     unsigned long long cyc[8];      // per-CTA cycle counters, flushed to the statistics at exit
 };
+
+__device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
 // Phase timer: thread 0 charges the cycles since its previous mark to counter `which`.
 __device__ __forceinline__ void tgMark(TgShared& sm, int which) {
@@ -140,6 +149,38 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
         // baseK[k] / 4): all loads of a thread are independent, one trip to L2 for the whole table instead of one
         // per island
         const int tot4 = sm.csUsed4;
+#if TG_STAGE_TMA
+        // A/B variant (profiles/r2_sass_summary.md): the raw cost rows come in as TMA bulk copies (cp.async.bulk, one per
+        // island and diagonal, completion on an mbarrier) and are thresholded in place; core tables only.
+        const bool bulk = I.nLayers == 0;
+        if (bulk) {
+            const uint32_t mbar = tgSmemAddr(&sm.mbar);
+            const uint32_t phase = sm.mbarPhase;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // earlier generic-proxy writes of this memory are ordered first
+            uint32_t bytes = 0;
+            int rows = 0;
+            for (int kc = 0; kc < Ke; ++kc) rows += sm.dmaxK[kc];
+            for (int rw = tid; rw < rows; rw += TG_NT) {
+                int kc = 0, d = rw;
+                while (d >= sm.dmaxK[kc]) { d -= sm.dmaxK[kc]; ++kc; }
+                ++d;
+                const uint32_t words = uint32_t(min(Lp, (L - d + 1 + 3) & ~3));
+                const uint32_t* src = I.cd + sm.cdOff + size_t(sm.isl[kc]) * I.triG + tgGOff(L, d);
+                const uint32_t dst = tgSmemAddr(Cs + sm.baseK[kc] + (d - 1) * Lp);
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             ::"r"(dst), "l"(src), "r"(words * 4u), "r"(mbar) : "memory");
+                bytes += words * 4u;
+            }
+            if (bytes) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+            else asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar) : "memory");
+            uint32_t done = 0;
+            while (!done)
+                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                             : "=r"(done) : "r"(mbar), "r"(phase) : "memory");
+        }
+#else
+        const bool bulk = false;
+#endif
         for (int f = tid; f < tot4; f += TG_NT) {
             int kc = 0;
             while (kc + 1 < Ke && int(sm.baseK[kc + 1] >> 2) <= f) ++kc;
@@ -149,6 +190,11 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
             const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
             uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
             if (d <= dk && a4 < ((L - d + 3) >> 2)) {
+                if (bulk) {
+                    v = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc])[w];
+                    v.x = v.x <= T ? v.x : TG_INFU; v.y = v.y <= T ? v.y : TG_INFU;
+                    v.z = v.z <= T ? v.z : TG_INFU; v.w = v.w <= T ? v.w : TG_INFU;
+                } else
                 v = tgCostAt4(I, sm.cdOff, size_t(sm.isl[kc]) * I.triG + tgGOff(L, d) + 4 * a4, T);
                 const int a = a4 * 4, amax = L - 1 - d;
                 v.x = (a + 0 <= amax) ? v.x : TG_INFU;
@@ -160,6 +206,9 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
             reinterpret_cast<uint4*>(Cs + sm.baseK[kc])[w] = v;
         }
         __syncthreads();
+#if TG_STAGE_TMA
+        if (bulk && tid == 0) sm.mbarPhase ^= 1u;
+#endif
         for (int w = tid; w < Ke * nb4; w += TG_NT) {   // widest admissible diagonal per 4 starts
             const int kc = w / nb4, a4 = w - kc * nb4;
             const uint4* col = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc]) + a4;
@@ -340,7 +389,6 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
 // Two CTA barriers per batch.  Shared memory of a batch: [descriptors x2 | lists | H rows | source rows x2].
 // ---------------------------------------------------------------------------------------------
 
-__device__ __forceinline__ uint32_t tgSmemAddr(const void* p) { return uint32_t(__cvta_generic_to_shared(p)); }
 
 __device__ __forceinline__ uint4 tgLds4(uint32_t addr) {
     uint4 v;
@@ -1612,6 +1660,13 @@ __global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgS
     }
     for (int w = threadIdx.x; w < 17 * 17; w += TG_NT) sm.binom[w / 17][w % 17] = tgBinom[w / 17][w % 17];
     if (threadIdx.x < TG_MAX_K) sm.xInf[threadIdx.x] = TG_INFU;
+#if TG_STAGE_TMA
+    if (threadIdx.x == 0) {
+        sm.mbarPhase = 0;
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tgSmemAddr(&sm.mbar)), "r"(TG_NT) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+#endif
     __syncthreads();
     const bool wide = ctx.nInst >= TG_WIDE_MIN_INST;
     for (int round = 0;; ++round) {
