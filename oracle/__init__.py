@@ -193,6 +193,28 @@ def solve_variant(inst, n_threads: int = 0) -> Result:
     return _conv(r)
 
 
+def _args_variant_b(inst):
+    keep, a = _args_variant(inst)                      # (..., act_mb, xbound)
+    ab = None if getattr(inst, "act_mb_b", None) is None else np.ascontiguousarray(inst.act_mb_b, dtype=np.int32)
+    abp = C.cast(None, _I32P) if ab is None else _p32(ab)
+    return (keep, ab), a[:-1] + (abp, a[-1])
+
+
+def solve_variant_b(inst) -> Result:
+    """Variant oracle with per-boundary activation sizes (inst.act_mb_b [L+1] or None), NEXT-3(b) second half."""
+    keep, a = _args_variant_b(inst)
+    r = _Res()
+    lib().orc_variant_solve_b(*a, C.byref(r))
+    return _conv(r)
+
+
+def bruteforce_variant_b(inst) -> Result:
+    keep, a = _args_variant_b(inst)
+    r = _Res()
+    lib().orc_variant_bruteforce_b(*a, C.byref(r))
+    return _conv(r)
+
+
 def bruteforce_variant(inst) -> Result:
     keep, a = _args_variant(inst)
     r = _Res()

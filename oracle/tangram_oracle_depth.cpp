@@ -51,6 +51,7 @@ struct Inst {
     const int32_t *time_us, *mem_mb, *actmem_mb, *cap_mb, *bw_gbps;   // actmem_mb may be null (= zeros)
     int act_mb;
     int xbound = 0;   // NEXT-3(b): transfers are bounded by T as well
+    const int32_t* act_b = nullptr;   // NEXT-3(b), second half: activation MB crossing boundary b (entries 1..L-1), or null
     int NS() const { return L * (L + 1) / 2; }
 };
 
@@ -94,6 +95,19 @@ Reduced reduce_tables(const Inst& I) {
     return R;
 }
 
+// Transfer time across boundary b from the stage on island j to the stage on island k.  With per-boundary activation sizes
+// (PAPER.md:240 (1) "only transferring stage inputs and outputs": what crosses a boundary is the output of the layer in
+// front of it, whose size may differ from layer to layer, e.g. between attention and MoE blocks) it is
+//     x_b[j][k] = ceil(act_b[b] * 1000 / bw[j][k])  microseconds,  unusable (INF) above TIME_MAX,
+// else the one table of the core path.
+inline int64_t xfer(const Inst& I, const Reduced& R, int b, int j, int k) {
+    if (!I.act_b) return R.x[size_t(j) * I.K + k];
+    if (j == k) return 0;
+    const int64_t num = int64_t(I.act_b[b]) * 1000, den = I.bw_gbps[j * I.K + k];
+    const int64_t v = (num + den - 1) / den;
+    return v > TIME_MAX ? INF : v;
+}
+
 std::vector<int64_t> candidates(const Reduced& R, bool xbound) {
     std::vector<int64_t> v;
     for (int64_t c : R.c) if (c < INF) v.push_back(c);
@@ -101,6 +115,20 @@ std::vector<int64_t> candidates(const Reduced& R, bool xbound) {
         for (int j = 0; j < R.K; ++j)
             for (int k = 0; k < R.K; ++k)
                 if (j != k && R.x[size_t(j) * R.K + k] < INF) v.push_back(R.x[size_t(j) * R.K + k]);
+    std::sort(v.begin(), v.end());
+    v.erase(std::unique(v.begin(), v.end()), v.end());
+    return v;
+}
+
+// the same with per-boundary activation sizes: under the transfer bound every boundary's finite transfer times are candidates
+std::vector<int64_t> candidates(const Inst& I, const Reduced& R) {
+    if (!I.act_b || !I.xbound) return candidates(R, I.xbound != 0);
+    std::vector<int64_t> v;
+    for (int64_t c : R.c) if (c < INF) v.push_back(c);
+    for (int b = 1; b < I.L; ++b)
+        for (int j = 0; j < I.K; ++j)
+            for (int k = 0; k < I.K; ++k)
+                if (j != k && xfer(I, R, b, j, k) < INF) v.push_back(xfer(I, R, b, j, k));
     std::sort(v.begin(), v.end());
     v.erase(std::unique(v.begin(), v.end()), v.end());
     return v;
@@ -135,8 +163,8 @@ Top run_dp(const Inst& I, const Reduced& R, int64_t T, DP& D, bool keep) {
                         int64_t best = INF; int bj = 0;
                         for (int j = 0; j < K; ++j) {
                             if (!(Rm >> j & 1)) continue;
-                            if (I.xbound && R.x[size_t(k) * K + j] > T) continue;   // NEXT-3(b): the transfer is a pipeline slot
-                            const int64_t v = sat(R.x[size_t(k) * K + j] + D.g[D.at(b, Rm, j)]);
+                            if (I.xbound && xfer(I, R, b, k, j) > T) continue;   // NEXT-3(b): the transfer is a pipeline slot
+                            const int64_t v = sat(xfer(I, R, b, k, j) + D.g[D.at(b, Rm, j)]);
                             if (v < best) { best = v; bj = j; }
                         }
                         D.h[D.at(b, Rm, k)] = int32_t(best);
@@ -292,6 +320,48 @@ int orc_variant_solve_mt(int L, int K, int P, int m, const int32_t* time_us, con
     return 0;
 }
 
+// Per-boundary activation sizes (second half; PAPER.md:240 (1), :350): act_b[b] MB cross boundary
+// b (1 <= b <= L-1; entries 0 and L are ignored).  Same search as orc_variant_solve_mt / literal enumeration as
+// orc_variant_bruteforce with the transfer of a boundary taken from xfer().  act_b == null is the scalar act_mb.
+int orc_variant_solve_b(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                        const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, const int32_t* act_b, int xbound, orc_result* out) {
+    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, xbound};
+    I.act_b = act_b;
+    Reduced R = reduce_tables(I);
+    std::vector<int64_t> cand = candidates(I, R);
+    set_infeasible(out);
+    out->n_candidates = int(cand.size());
+    DP D0;
+    const Top tinf = run_dp(I, R, INF, D0, false);
+    if (tinf.best >= INF) return 0;
+    bool have = false; int64_t best_iter = 0, best_T = 0; int n_dp = 0;
+    for (int64_t T : cand) {
+        if (have && tinf.best + int64_t(m - 1) * T >= best_iter) break;
+        DP D; ++n_dp;
+        const Top t = run_dp(I, R, T, D, false);
+        if (t.best >= INF) continue;
+        const int64_t it = t.best + int64_t(m - 1) * T;
+        if (!have || it < best_iter) { have = true; best_iter = it; best_T = T; }
+    }
+    DP D;
+    const Top t = run_dp(I, R, best_T, D, true);
+    out->iter_time_us = best_iter; out->sum_us = t.best; out->bottleneck_us = best_T;
+    out->island_mask = t.S; out->n_dp_run = n_dp;
+    int a = 0, k = t.k, n = 0; uint32_t S = t.S;
+    while (true) {
+        const int b = D.gb[D.at(a, S, k)];
+        out->stage_begin[n] = a; out->stage_island[n] = k;
+        out->stage_plan[n] = R.A(__builtin_popcount(S), sidx(L, a, b), k);
+        ++n;
+        if (b == L) break;
+        const uint32_t Rm = S ^ (1u << k);
+        const int j = D.hj[D.at(b, Rm, k)];
+        a = b; S = Rm; k = j;
+    }
+    out->n_stages = n;
+    return 0;
+}
+
 int orc_depth_solve(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
                     const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, orc_result* out) {
     return orc_variant_solve(L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, 0, out);
@@ -314,7 +384,7 @@ struct BF {
             if (cv >= INF) return;
             sum += cv; T = std::max(T, cv); mask |= 1u << ks[i];
             if (i + 1 < n) {
-                const int64_t xs = R->x[size_t(ks[i]) * I->K + ks[i + 1]];
+                const int64_t xs = xfer(*I, *R, bs[i], ks[i], ks[i + 1]);
                 if (xs >= INF) return;
                 sum += xs;
                 if (I->xbound) T = std::max(T, xs);
@@ -343,6 +413,30 @@ struct BF {
 int orc_variant_bruteforce(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
                            const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, int xbound, orc_result* out) {
     Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, xbound};
+    Reduced R = reduce_tables(I);
+    BF bf; bf.I = &I; bf.R = &R;
+    bf.rec(0, 0);
+    set_infeasible(out);
+    if (!bf.have) return 0;
+    out->iter_time_us = bf.bestkey[0]; out->bottleneck_us = bf.bestkey[1];
+    out->island_mask = uint32_t(bf.bestkey[2]);
+    out->sum_us = bf.bestkey[0] - int64_t(m - 1) * bf.bestkey[1];
+    const int n = int(bf.bestkey.size() - 3) / 2;
+    out->n_stages = n;
+    int a = 0;
+    for (int i = 0; i < n; ++i) {
+        const int k = int(bf.bestkey[3 + 2 * i]), b = int(bf.bestkey[4 + 2 * i]);
+        out->stage_begin[i] = a; out->stage_island[i] = k;
+        out->stage_plan[i] = R.A(n - i, sidx(L, a, b), k);
+        a = b;
+    }
+    return 0;
+}
+
+int orc_variant_bruteforce_b(int L, int K, int P, int m, const int32_t* time_us, const int32_t* mem_mb, const int32_t* actmem_mb,
+                             const int32_t* cap_mb, const int32_t* bw_gbps, int act_mb, const int32_t* act_b, int xbound, orc_result* out) {
+    Inst I{L, K, P, m, time_us, mem_mb, actmem_mb, cap_mb, bw_gbps, act_mb, xbound};
+    I.act_b = act_b;
     Reduced R = reduce_tables(I);
     BF bf; bf.I = &I; bf.R = &R;
     bf.rec(0, 0);

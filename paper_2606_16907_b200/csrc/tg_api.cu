@@ -926,10 +926,11 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
         const tg_status sd = deviceInit(dev, &DS);
         if (sd != TG_OK) { cudaFreeAsync(ws, st); return sd; }
         const int P0 = instances[0]->P;
-        const dim3 g2((maxCells + 511) / 512, n);
-        const bool wide = int64_t(g2.x) * n >= 4 * DS->numSMs;
+        const dim3 g2((maxCells + 511) / 512, n), g4((maxCells + 1023) / 1024, n);
+        const bool wide = int64_t(g2.x) * n >= 4 * DS->numSMs, wide4 = int64_t(g4.x) * n >= 8 * DS->numSMs;
         if (P0 == 4) {
-            if (wide) tgPruneCellKernel<1, 2><<<g2, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+            if (wide4) tgPruneCellKernel<1, 4><<<g4, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
+            else if (wide) tgPruneCellKernel<1, 2><<<g2, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
             else tgPruneCellKernel<1, 1><<<g, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);
         } else if (P0 == 8) {
             if (wide) tgPruneCellKernel<2, 2><<<g2, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts);

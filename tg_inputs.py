@@ -80,6 +80,7 @@ class Instance:
     meta: dict = field(default_factory=dict)
     actmem_mb: np.ndarray = None   # [NS, K, P] int32 or None: MB per in-flight microbatch (NEXT-1, depth-aware memory)
     transfer_bound: bool = False   # NEXT-3(b): transfers count toward the bottleneck (x <= T as well)
+    act_mb_b: np.ndarray = None    # [L+1] int32 or None: activation MB crossing boundary b = 1..L-1 (NEXT-3(b), per-boundary sizes)
     slow_us: np.ndarray = None     # [NS, K, P] int32 or None: slowest internal stage of the partial plan (NEXT-2)
     q_stages: np.ndarray = None    # [NS, K, P] int32 or None: its number of internal pipeline stages (NEXT-2)
 
@@ -88,6 +89,7 @@ class Instance:
                         self.mem_mb.copy(), self.island_gpus.copy(), self.island_cap_mb.copy(),
                         self.bw_gbps.copy(), self.act_mb, dict(self.meta),
                         None if self.actmem_mb is None else self.actmem_mb.copy(), self.transfer_bound,
+                        None if self.act_mb_b is None else self.act_mb_b.copy(),
                         None if self.slow_us is None else self.slow_us.copy(),
                         None if self.q_stages is None else self.q_stages.copy())
 
@@ -299,6 +301,16 @@ def with_transfer_bound(inst: Instance) -> Instance:
     o = inst.copy()
     o.transfer_bound = True
     o.name = inst.name + "_xb"
+    return o
+
+
+def with_boundary_act(inst: Instance, seed: int, sizes=(16, 64, 256)) -> Instance:
+    """NEXT-3(b): the activation crossing boundary b has one of a few sizes (MB), e.g. narrow after an attention block,
+    wide after an MoE block or the embedding (the paper prints no activation sizes)."""
+    o = inst.copy()
+    b = np.arange(inst.L + 1)
+    o.act_mb_b = np.asarray(sizes, dtype=np.int64)[urand(seed, S_MISC + 60, b, 0, len(sizes) - 1)].astype(np.int32)
+    o.name = inst.name + "_ab"
     return o
 
 
