@@ -67,17 +67,16 @@ def test_constant_size_is_the_scalar_definition():
 
 
 def test_hand_worked_cut_moves_to_the_cheap_boundary():
-    """Three layers, two islands, one plan, m = 1 (iter = sum).  Island 0 runs a layer in 10 us, island 1 in 10 us; each
-    island alone would need 100 us per layer on the other's share... concretely: slice times on island 0: 1 layer 10, 2 layers 20,
-    3 layers 200; on island 1: 1 layer 10, 2 layers 20, 3 layers 200 -> two stages are needed.  bw = 1 GB/s: x = act * 1000 us.
-    Boundary 1 carries 5 MB (5000 us), boundary 2 carries 1 MB (1000 us).
-    Cut at 1: 10 + 5000 + 20 = 5030.   Cut at 2: 20 + 1000 + 10 = 1030  <- optimum, first stage on island 0 (lowest mask / k_0).
-    With the sizes swapped the cut moves to boundary 1: 10 + 1000 + 20 = 1030."""
+    """Three layers, two islands, one plan, m = 1 (iter = sum).  On either island a slice of 1 / 2 / 3 layers takes
+    10 / 20 / 9000 us, so the model is split in two.  bw = 1 GB/s: x = act * 1000 us.  Boundary 1 carries 5 MB (5000 us),
+    boundary 2 carries 1 MB (1000 us).
+    Cut at 1: 10 + 5000 + 20 = 5030.   Cut at 2: 20 + 1000 + 10 = 1030  <- optimum (one stage: 9000); first stage on island 0
+    (lowest k_0).  With the sizes swapped the cut moves to boundary 1: 10 + 1000 + 20 = 1030."""
     L, K = 3, 2
     t = np.zeros((6, K, 1), dtype=np.int32)
     for a in range(L):
         for b in range(a + 1, L + 1):
-            t[gen.slice_index(L, a, b), :, 0] = {1: 10, 2: 20, 3: 200}[b - a]
+            t[gen.slice_index(L, a, b), :, 0] = {1: 10, 2: 20, 3: 9000}[b - a]
     inst = gen.Instance("handb", L, K, 1, 1, t, np.zeros_like(t), np.ones(K, np.int32), np.full(K, 10, np.int32),
                         np.ones((K, K), np.int32), 3)
     inst.act_mb_b = np.array([0, 5, 1, 0], dtype=np.int32)
