@@ -47,6 +47,7 @@ enum {
     TG_MAX_P = 255,
     TG_MAX_M = 1 << 20,
     TG_TIME_MAX = 1 << 25,
+    TG_MAX_ACT = 8,          /* distinct per-boundary activation sizes of an instance (tg_instance_set_boundary_act) */
     TG_MAX_NODES = 64,       /* nodes of a cluster profile (tg_islands_build)     */
     TG_INVALID = 0x7fffffff, /* "no such intra-slice plan" marker in time_us */
     TG_INF = 1 << 30         /* saturating "no plan" value of the DP        */
@@ -131,6 +132,18 @@ tg_status tg_instance_set_transfer_bound(tg_instance* inst, int32_t on);
  * tg_prune on such an instance -> TG_ERR_SHAPE.  Combines with tg_instance_set_transfer_bound.  Values out of range ->
  * TG_ERR_RANGE.  Synchronises the legacy default stream. */
 tg_status tg_instance_set_stages(tg_instance* inst, const int32_t* slow_us, const int32_t* n_stages);
+
+/* tg_instance_set_boundary_act — SURVEY.md §8(f) NEXT-3(b), per-boundary activation sizes (PAPER.md:240 (1) "only
+ * transferring stage inputs and outputs"; :350 communication can be the bottleneck).
+ *   act_mb_b  EITHER [L+1] int32: act_mb_b[b] MB cross the boundary in front of layer b, 1 <= b <= L-1, each in [0, 2^20]
+ *             (entries 0 and L are ignored); copied; NULL restores the scalar act_mb of tg_instance_create
+ * The transfer of a cut at b from island j to island k then costs x_b[j][k] = ceil(act_mb_b[b]*1000 / bw_gbps[j][k]) us
+ * (unusable above TG_TIME_MAX); with tg_instance_set_transfer_bound every boundary's finite transfer times are candidate
+ * thresholds.  A constant array is the scalar definition bit for bit.  At most TG_MAX_ACT distinct sizes among the
+ * boundaries 1..L-1, else TG_ERR_SHAPE; values out of range -> TG_ERR_RANGE; on an instance with multi-stage partial
+ * plans (tg_instance_set_stages, and vice versa) -> TG_ERR_SHAPE.  Combines with tg_instance_set_actmem and
+ * tg_instance_set_transfer_bound.  tg_reduce's x_out reports the matrix of the first boundary's size. */
+tg_status tg_instance_set_boundary_act(tg_instance* inst, const int32_t* act_mb_b);
 
 /* NULL is a no-op.  The instance must not be in use by an unsynchronised tg_solve_batch. */
 tg_status tg_instance_destroy(tg_instance* inst);

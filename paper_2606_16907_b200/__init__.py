@@ -65,7 +65,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_set_stages", "tg_plan_pipeline_stages", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
+EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_set_boundary_act", "tg_instance_set_stages", "tg_plan_pipeline_stages", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
            "tg_reduce", "tg_candidates", "tg_dp_at", "tg_instance_read_time", "tg_islands_build", "tg_release_cached_memory", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -86,6 +86,7 @@ def lib():
         L.tg_instance_create_batch.argtypes = [i32, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.tg_instance_set_transfer_bound.argtypes = [vp, i32]
         L.tg_instance_set_stages.argtypes = [vp, vp, vp]
+        L.tg_instance_set_boundary_act.argtypes = [vp, vp]
         L.tg_plan_pipeline_stages.argtypes = [vp, vp, C.POINTER(i32)]
         L.tg_instance_destroy.argtypes = [vp]
         L.tg_instance_set_actmem.argtypes = [vp, vp]
@@ -208,6 +209,12 @@ def tg_instance_set_actmem(inst: Instance, actmem_mb):
     """NEXT-1: per-plan MB per in-flight microbatch ([NS,K,P] int32 numpy array or torch tensor); None removes it."""
     a = np.ascontiguousarray(actmem_mb, dtype=np.int32) if isinstance(actmem_mb, np.ndarray) else actmem_mb
     _check(lib().tg_instance_set_actmem(inst.handle, _ptr(a)))
+
+
+def tg_instance_set_boundary_act(inst: Instance, act_mb_b):
+    """NEXT-3(b): activation MB crossing boundary b ([L+1] int32; entries 1..L-1 used); None restores the scalar size."""
+    a = np.ascontiguousarray(act_mb_b, dtype=np.int32) if isinstance(act_mb_b, np.ndarray) else act_mb_b
+    _check(lib().tg_instance_set_boundary_act(inst.handle, _ptr(a)))
 
 
 def tg_instance_set_stages(inst: Instance, slow_us, n_stages=None):
@@ -358,6 +365,8 @@ def instance_from_inputs(inst, device_tables: bool = False) -> Instance:
         tg_instance_set_actmem(h, inst.actmem_mb)
     if getattr(inst, "transfer_bound", False):
         tg_instance_set_transfer_bound(h, True)
+    if getattr(inst, "act_mb_b", None) is not None:
+        tg_instance_set_boundary_act(h, inst.act_mb_b)
     if getattr(inst, "slow_us", None) is not None:
         tg_instance_set_stages(h, inst.slow_us, getattr(inst, "q_stages", None))
     return h

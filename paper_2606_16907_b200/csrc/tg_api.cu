@@ -11,7 +11,17 @@
 
 #include "tg_common.cuh"
 #include "tg_prep.cuh"
+// the persistent solver, twice: core path only / with the variants of SURVEY.md §8(f) (see the head of tg_solve.cuh)
+#define TG_SOLVE_NS tgcore
+#define TG_VAR 0
 #include "tg_solve.cuh"
+#undef TG_SOLVE_NS
+#undef TG_VAR
+#define TG_SOLVE_NS tgfull
+#define TG_VAR 1
+#include "tg_solve.cuh"
+#undef TG_SOLVE_NS
+#undef TG_VAR
 #include "tg_islands.cuh"
 
 // One device allocation shared by the instances of a tg_instance_create_batch call; freed with the last of them.
@@ -26,6 +36,9 @@ struct tg_instance {
     int device;
     int32_t *time_us, *mem_mb, *gpus, *cap_mb, *bw;  // device
     int32_t* actmem;                                 // device, or nullptr (tg_instance_set_actmem)
+    int32_t nAct = 0;                                // tg_instance_set_boundary_act: distinct activation sizes (0 = scalar act_mb)
+    int32_t actVal[TG_MAX_ACT] = {0, 0, 0, 0, 0, 0, 0, 0};
+    uint8_t clsOf[256] = {0};                        // size class of boundary b
     int32_t* slow = nullptr;                         // device, or nullptr (tg_instance_set_stages): slowest internal stage [NS][K][P]
     int32_t* qst = nullptr;                          // device, behind slow: internal stage counts [NS][K][P]
     int32_t xbound;                                  // tg_instance_set_transfer_bound
@@ -110,16 +123,19 @@ tg_status deviceInit(int dev, DeviceState** out) {
         TG_CUDA(cudaMemcpyToSymbol(tgPopOff, popOff, sizeof(popOff)));
         TG_CUDA(cudaMemcpyToSymbol(tgBinom, binom, sizeof(binom)));
         TG_CUDA(cudaFuncSetAttribute(tgPrepareKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TG_SORT_SMEM_MAX * 4));
-        cudaFuncAttributes fa;
-        TG_CUDA(cudaFuncGetAttributes(&fa, tgSolveKernel));
+        cudaFuncAttributes fa, fb;
+        TG_CUDA(cudaFuncGetAttributes(&fa, tgcore::tgSolveKernel));
+        TG_CUDA(cudaFuncGetAttributes(&fb, tgfull::tgSolveKernel));
         // TG_CTAS_PER_SM co-resident CTAs share the SM's shared memory (each CTA also pays 1 KB of system reserve)
-        int dyn = std::min(D.smemOptin, D.smemPerSM / TG_CTAS_PER_SM) - int(fa.sharedSizeBytes) - 1024;
+        int dyn = std::min(D.smemOptin, D.smemPerSM / TG_CTAS_PER_SM) - int(std::max(fa.sharedSizeBytes, fb.sharedSizeBytes)) - 1024;
         dyn &= ~1023;
         if (dyn < 48 * 1024) return fail(TG_ERR_CUDA, "not enough shared memory per block for the solver");
-        TG_CUDA(cudaFuncSetAttribute(tgSolveKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
-        int occ = 0;
-        TG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tgSolveKernel, TG_NT, size_t(dyn)));
-        if (occ < TG_CTAS_PER_SM) return fail(TG_ERR_CUDA, "solver kernel: fewer co-resident CTAs per SM than it was built for");
+        TG_CUDA(cudaFuncSetAttribute(tgcore::tgSolveKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+        TG_CUDA(cudaFuncSetAttribute(tgfull::tgSolveKernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn));
+        int occ = 0, occ2 = 0;
+        TG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tgcore::tgSolveKernel, TG_NT, size_t(dyn)));
+        TG_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, tgfull::tgSolveKernel, TG_NT, size_t(dyn)));
+        if (std::min(occ, occ2) < TG_CTAS_PER_SM) return fail(TG_ERR_CUDA, "solver kernel: fewer co-resident CTAs per SM than it was built for");
         D.ctasPerSM = TG_CTAS_PER_SM;
         D.dynSmem = dyn;
         // Per-call workspaces come from a pool of the library's own (the device's default pool, which the embedding
@@ -175,6 +191,7 @@ struct Workspace {
     tg_result* outDev = nullptr;
     int dynSmem = 0;
     int numCtas = 0;
+    bool variants = false;          // an instance of the batch uses a SURVEY 8(f) variant: launch the full kernel
 };
 
 // Lays out the per-call workspace, uploads the instance records and runs loader + prepare.
@@ -196,7 +213,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     Carver cv;
     const size_t oInst = cv.take(sizeof(TgInstDev) * n);
     std::vector<TgInstDev> h(n);
-    std::vector<size_t> oCd(n), oThr(n), oArgp(n), oCand(n), oSort(n), oSort2(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
+    std::vector<size_t> oXa(n), oCd(n), oThr(n), oArgp(n), oCand(n), oSort(n), oSort2(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
     int maxCells = 0, maxLp = 4, maxK = 1;
     uint64_t maxFull = 0;
     size_t denseCs = 0;
@@ -207,10 +224,14 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         I.time_us = t.time_us; I.mem_mb = t.mem_mb; I.cap_mb = t.cap_mb; I.bw_gbps = t.bw;
         I.actmem_mb = t.actmem;
         I.nDepth = t.actmem ? t.K : 1;
+        if (t.actmem || t.slow || t.nAct) W.variants = true;
         I.slow_us = t.slow;
         I.nLayers = t.slow ? t.P : 0;
         I.nTables = std::max(std::max(I.nDepth, I.nLayers), 1);
         I.xbound = t.xbound;
+        I.nAct = t.nAct;
+        memcpy(I.actVal, t.actVal, sizeof(I.actVal));
+        memcpy(I.clsOf, t.clsOf, sizeof(I.clsOf));
         I.L = t.L; I.K = t.K; I.P = t.P; I.m = t.m; I.act_mb = t.act_mb; I.NS = t.NS;
         I.Lp = (t.L + 3) & ~3;
         I.triG = int(tgGOff(t.L, t.L + 1));
@@ -240,7 +261,8 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         oCd[i] = cv.take(nd * size_t(t.K) * I.triG * 4);
         oThr[i] = I.nLayers ? cv.take(nd * size_t(t.K) * I.triG * 4) : 0;
         oArgp[i] = cv.take(nd * size_t(cells));
-        const size_t nKeys = nd * size_t(cells) + size_t(t.K) * t.K;   // every reduced cost + (transfer bound) every transfer time
+        oXa[i] = t.nAct ? cv.take(size_t(t.nAct) * TG_MAX_K * TG_MAX_K * 4) : 0;
+        const size_t nKeys = nd * size_t(cells) + size_t(t.K) * t.K * std::max(t.nAct, 1);   // every reduced cost + (transfer bound) every transfer time
         oCand[i] = cv.take(nKeys * 4);
         oSort[i] = cv.take(nKeys * 4);
         oSort2[i] = cv.take(nKeys * 4);
@@ -289,6 +311,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     for (int i = 0; i < n; ++i) {
         h[i].cd = reinterpret_cast<uint32_t*>(W.base + oCd[i]);
         h[i].thr = h[i].nLayers ? reinterpret_cast<uint32_t*>(W.base + oThr[i]) : nullptr;
+        h[i].xAct = h[i].nAct ? reinterpret_cast<uint32_t*>(W.base + oXa[i]) : nullptr;
         h[i].argp = reinterpret_cast<uint8_t*>(W.base + oArgp[i]);
         h[i].cand = reinterpret_cast<uint32_t*>(W.base + oCand[i]);
         h[i].sortbuf = reinterpret_cast<uint32_t*>(W.base + oSort[i]);
@@ -373,7 +396,8 @@ tg_status launchSolve(Workspace& W, cudaStream_t st) {
     void* args[] = {&ctx};
     if (!g_evA) { TG_CUDA(cudaEventCreate(&g_evA)); TG_CUDA(cudaEventCreate(&g_evB)); }
     TG_CUDA(cudaEventRecord(g_evA, st));
-    TG_CUDA(cudaLaunchCooperativeKernel((const void*)tgSolveKernel, dim3(W.numCtas), dim3(TG_NT), args, size_t(W.dynSmem), st));
+    const void* kernel = W.variants ? (const void*)tgfull::tgSolveKernel : (const void*)tgcore::tgSolveKernel;
+    TG_CUDA(cudaLaunchCooperativeKernel(kernel, dim3(W.numCtas), dim3(TG_NT), args, size_t(W.dynSmem), st));
     TG_CUDA(cudaEventRecord(g_evB, st));
     return TG_OK;
 }
@@ -381,7 +405,7 @@ tg_status launchSolve(Workspace& W, cudaStream_t st) {
 tg_status finish(Workspace& W, int n, tg_result* out, tg_solve_stats* stats, cudaStream_t st) {
     const bool outDev = isDevicePtr(out);
     bool sync = !outDev;
-    tgPoisonOnErrorKernel<<<std::max(1, std::min((n + 255) / 256, 64)), 256, 0, st>>>(W.ctx.ctrl, W.outDev, n);
+    tgcore::tgPoisonOnErrorKernel<<<std::max(1, std::min((n + 255) / 256, 64)), 256, 0, st>>>(W.ctx.ctrl, W.outDev, n);
     TG_CUDA(cudaMemcpyAsync(out, W.outDev, sizeof(tg_result) * n, cudaMemcpyDefault, st));
     if (stats) {
         if (!isDevicePtr(stats)) sync = true;
@@ -761,6 +785,7 @@ tg_status tg_instance_set_stages(tg_instance* inst, const int32_t* slow_us, cons
     if (inst->slow) { cudaFreeAsync(inst->slow, 0); inst->slow = nullptr; inst->qst = nullptr; }
     if (!slow_us) return TG_OK;
     if (inst->actmem) return fail(TG_ERR_SHAPE, "the instance has a footprint table (tg_instance_set_actmem): the combination with multi-stage partial plans is not built");
+    if (inst->nAct) return fail(TG_ERR_SHAPE, "the instance has per-boundary activation sizes (tg_instance_set_boundary_act): the combination with multi-stage partial plans is not built");
     const size_t nE = size_t(inst->NS) * inst->K * inst->P;
     int32_t* d = nullptr;
     TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), 2 * nE * 4 + 4, 0));
@@ -799,6 +824,35 @@ tg_status tg_plan_pipeline_stages(tg_instance* inst, const tg_result* result, in
         total += q;
     }
     *n_out = total;
+    return TG_OK;
+}
+
+tg_status tg_instance_set_boundary_act(tg_instance* inst, const int32_t* act_mb_b) {
+    if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
+    if (!act_mb_b) { inst->nAct = 0; return TG_OK; }
+    if (inst->slow) return fail(TG_ERR_SHAPE, "the instance has multi-stage partial plans (tg_instance_set_stages): the combination with per-boundary activation sizes is not built");
+    const int L = inst->L;
+    std::vector<int32_t> h(size_t(L) + 1);
+    TG_CUDA(cudaMemcpy(h.data(), act_mb_b, (size_t(L) + 1) * 4, cudaMemcpyDefault));
+    int nAct = 0;
+    int32_t vals[TG_MAX_ACT];
+    uint8_t cls[256];
+    memset(cls, 0, sizeof(cls));
+    for (int b = 1; b < L; ++b) {
+        if (h[b] < 0 || h[b] > (1 << 20)) return fail(TG_ERR_RANGE, "act_mb_b[" + std::to_string(b) + "] outside [0, 2^20]");
+        int c = 0;
+        while (c < nAct && vals[c] != h[b]) ++c;
+        if (c == nAct) {
+            if (nAct == TG_MAX_ACT) return fail(TG_ERR_SHAPE, "more than TG_MAX_ACT distinct activation sizes");
+            vals[nAct++] = h[b];
+        }
+        cls[b] = uint8_t(c);
+    }
+    if (nAct == 0) { vals[0] = 0; nAct = 1; }            // a one-layer model has no boundary
+    inst->nAct = nAct;
+    memset(inst->actVal, 0, sizeof(inst->actVal));
+    memcpy(inst->actVal, vals, size_t(nAct) * 4);
+    memcpy(inst->clsOf, cls, sizeof(cls));
     return TG_OK;
 }
 

@@ -82,6 +82,10 @@ struct TgInstDev {
     int32_t candWinLo, candWinN;
     int32_t planKind;                 // wide scheduling: item kind returned by this round's planning
     int32_t xbound;                   // NEXT-3(b): transfers are admissible only if x <= T (tg_instance_set_transfer_bound)
+    int32_t nAct;                     // NEXT-3(b): 0, or the number of distinct per-boundary activation sizes (tg_instance_set_boundary_act)
+    int32_t actVal[TG_MAX_ACT];       // the sizes (MB) by class
+    uint32_t* xAct;                   // [nAct][TG_MAX_K * TG_MAX_K] transfer times by size class, sender-major (workspace)
+    uint8_t clsOf[256];               // size class of boundary b
     uint32_t x[TG_MAX_K * TG_MAX_K];  // transfer times, sender-major
     // ---- solver state (one scheduler thread per instance) ----
     int32_t phase, loInf, hiFeas, next;   // FEAS bracket: largest infeasible / smallest feasible candidate
@@ -171,6 +175,19 @@ __device__ __forceinline__ uint32_t tgCostAt(const TgInstDev& I, size_t tableOff
         if (layer) *layer = j;
     }
     return c;
+}
+
+// The core form alone (the solver's core kernel compiles the step function out).
+__device__ __forceinline__ uint32_t tgCostAtCore(const TgInstDev& I, size_t tableOff, size_t off, uint32_t T, int* layer) {
+    if (layer) *layer = 0;
+    const uint32_t c = I.cd[tableOff + off];
+    return c <= T ? c : TG_INFU;
+}
+__device__ __forceinline__ uint4 tgCostAt4Core(const TgInstDev& I, size_t tableOff, size_t off, uint32_t T) {
+    uint4 v = __ldg(reinterpret_cast<const uint4*>(I.cd + tableOff + off));
+    v.x = v.x <= T ? v.x : TG_INFU; v.y = v.y <= T ? v.y : TG_INFU;
+    v.z = v.z <= T ? v.z : TG_INFU; v.w = v.w <= T ? v.w : TG_INFU;
+    return v;
 }
 
 // The same for 4 consecutive starts of one row (16-byte aligned offset).

@@ -509,20 +509,22 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     const int L = I.L, K = I.K, tid = threadIdx.x;
     if (tid == 0) { sMaxX = 0; I.prepCyc[0] = clock64(); }
     __syncthreads();
-    // transfer table
-    if (tid < K * K) {
-        const int j = tid / K, k = tid % K;
+    // transfer table (per activation-size class when the instance has per-boundary sizes; I.x = the first class)
+    const int nCls = max(I.nAct, 1);
+    for (int w = tid; w < K * K * nCls; w += TG_PREP_NT) {
+        const int cls = w / (K * K), e = w - cls * K * K, j = e / K, k = e % K;
         uint32_t v = 0;
         if (j != k) {
-            const int64_t num = int64_t(I.act_mb) * 1000, den = I.bw_gbps[tid];
+            const int64_t num = int64_t(I.nAct ? I.actVal[cls] : I.act_mb) * 1000, den = I.bw_gbps[e];
             const int64_t q = (num + den - 1) / den;
             v = q > TG_TIME_MAX ? TG_INFU : uint32_t(q);
         }
-        I.x[j * TG_MAX_K + k] = v;
+        if (cls == 0) I.x[j * TG_MAX_K + k] = v;
+        if (I.nAct) I.xAct[cls * (TG_MAX_K * TG_MAX_K) + j * TG_MAX_K + k] = v;
         // transfer bound (NEXT-3(b)): the finite transfer times are candidate thresholds too
         if (I.xbound) {
             const bool fin = j != k && v < TG_INFU;
-            I.sortbuf[size_t(I.NS) * K * I.nTables + tid] = fin ? v : TG_INFU;
+            I.sortbuf[size_t(I.NS) * K * I.nTables + w] = fin ? v : TG_INFU;
             if (fin) atomicMax(&sMaxX, v);
         }
     }
@@ -572,7 +574,7 @@ __global__ void __launch_bounds__(TG_PREP_NT) tgPrepareKernel(TgInstDev* __restr
     // bitmap with shared-memory atomics and read the set bits back in order -- O(n + maxKey/32) instead of a sort.
     // Larger keys: stable LSD radix sort (8- or 9-bit digits, per-warp histograms, ping-pong between two global
     // buffers) followed by a unique pass.
-    const int n = I.NS * K * I.nTables + (I.xbound ? K * K : 0);
+    const int n = I.NS * K * I.nTables + (I.xbound ? K * K * max(I.nAct, 1) : 0);
     const uint32_t maxKey = max(I.maxKey, sMaxX);
     const uint32_t nWords = (maxKey >> 5) + 1u;
     uint32_t base = 0;

@@ -13,9 +13,18 @@
 // Level r = |R| reads only level r-1 (PAPER.md:250 (2): a stage is added in front of a memoised
 // suffix).  State g[a][S][k] is stored as G_r[rank(R)][slot(k)][a], R = S\{k}.
 // Inside a level every warp streams over its own range of masks R (see tgWarpLevel).
-#pragma once
+// This file is compiled TWICE into tg_api.cu (no include guard): namespace tgcore with TG_VAR = 0 -- the core path of
+// SURVEY.md §8(a), every variant branch compiled out -- and namespace tgfull with TG_VAR = 1, which also serves the §8(f)
+// variants (footprint tables, multi-stage partial plans, per-boundary activation sizes).  The host launches tgfull only
+// when an instance of the batch uses one of them: the variants' extra template instances and branches measurably slowed
+// the core workloads (cfg5 +3.7 %, cfg4 +1.6 %) when they shared one kernel.
 #include "tg_common.cuh"
 #include "tg_prep.cuh"
+#if !defined(TG_SOLVE_NS) || !defined(TG_VAR)
+#error "define TG_SOLVE_NS and TG_VAR before including tg_solve.cuh"
+#endif
+#define TG_COST_AT(I, tableOff, off, T, layer) (TG_VAR ? tgCostAt((I), tableOff, off, T, layer) : tgCostAtCore((I), tableOff, off, T, layer))
+#define TG_COST_AT4(I, tableOff, off, T) (TG_VAR ? tgCostAt4((I), tableOff, off, T) : tgCostAt4Core((I), tableOff, off, T))
 
 #define TG_NW (TG_NT / 32)     // warps per CTA
 #ifndef TG_STAGE_TMA
@@ -23,6 +32,8 @@
 #endif
 #define TG_NB_MAX 256   // masks per batch, upper bound (row index inside a batch fits 16 bits: 256 * 16)
 #define TG_DESC_W 6     // words of a mask descriptor: R | cap(R) << 16, pad, non-members (16 nibbles), members (16 nibbles)
+
+namespace TG_SOLVE_NS {
 
 struct TgShared {
     // staged item
@@ -49,6 +60,9 @@ struct TgShared {
     uint8_t dmaxTile[TG_MAX_K][64];
     alignas(16) uint32_t xS[TG_MAX_K][TG_MAX_K];
     alignas(16) uint32_t xInf[TG_MAX_K];            // all-INF transfer row for a lane's unused k slot
+    int sNAct;                      // per-boundary activation sizes (NEXT-3(b)): number of size classes, 0 = one scalar size
+    int xOff;                       // their transfer matrices [sNAct][TG_MAX_K][TG_MAX_K] sit in the dynamic shared memory at this word
+    uint8_t clsOfS[256];            // size class of boundary b
     uint8_t isl[TG_MAX_K];
     uint16_t binom[17][17];
     // scheduler / queue
@@ -152,7 +166,7 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
 #if TG_STAGE_TMA
         // A/B variant (profiles/r2_sass_summary.md): the raw cost rows come in as TMA bulk copies (cp.async.bulk, one per
         // island and diagonal, completion on an mbarrier) and are thresholded in place; core tables only.
-        const bool bulk = I.nLayers == 0;
+        const bool bulk = !(TG_VAR && I.nLayers);
         if (bulk) {
             const uint32_t mbar = tgSmemAddr(&sm.mbar);
             const uint32_t phase = sm.mbarPhase;
@@ -195,7 +209,7 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
                     v.x = v.x <= T ? v.x : TG_INFU; v.y = v.y <= T ? v.y : TG_INFU;
                     v.z = v.z <= T ? v.z : TG_INFU; v.w = v.w <= T ? v.w : TG_INFU;
                 } else
-                v = tgCostAt4(I, sm.cdOff, size_t(sm.isl[kc]) * I.triG + tgGOff(L, d) + 4 * a4, T);
+                v = TG_COST_AT4(I, sm.cdOff, size_t(sm.isl[kc]) * I.triG + tgGOff(L, d) + 4 * a4, T);
                 const int a = a4 * 4, amax = L - 1 - d;
                 v.x = (a + 0 <= amax) ? v.x : TG_INFU;
                 v.y = (a + 1 <= amax) ? v.y : TG_INFU;
@@ -226,7 +240,7 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
         }
         if (count)
             for (int kc = 0; kc < Ke; ++kc) {
-                const uint32_t* cdk = (I.nLayers ? I.thr : I.cd + sm.cdOff) + size_t(sm.isl[kc]) * I.triG;   // (NEXT-2: admissible from the first step on)
+                const uint32_t* cdk = ((TG_VAR && I.nLayers) ? I.thr : I.cd + sm.cdOff) + size_t(sm.isl[kc]) * I.triG;   // (NEXT-2: admissible from the first step on)
                 for (int d = 1; d <= sm.dmaxK[kc]; ++d)
                     for (int a = tid; a <= L - 1 - d; a += TG_NT) nAdm += cdk[tgGOff(L, d) + a] <= T ? 1u : 0u;
             }
@@ -285,6 +299,8 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         const uint32_t xv = I.x[int(sm.isl[kc]) * TG_MAX_K + int(sm.isl[jc])];
         sm.xS[kc][jc] = (I.xbound && xv > T) ? TG_INFU : xv;   // transfer bound (NEXT-3(b)): a slower link is not admissible at T
     }
+    if (TG_VAR && I.nAct) for (int w = tid; w < 256; w += TG_NT) sm.clsOfS[w] = I.clsOf[w];
+    if (tid == 0) sm.sNAct = TG_VAR ? I.nAct : 0;
     // widest diagonal with an admissible entry (b <= L-1) and longest admissible slice at any position (b <= L) of
     // every island: sufMin / sufMinAll are non-decreasing in d, so each is the number of lengths whose entry is
     // <= T.  One warp per island, lanes over the lengths: one round trip to L2 instead of a binary search's seven.
@@ -320,19 +336,22 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         int perMask = 0;
         for (int r = 1; r < Ke; ++r) perMask = max(perMask, (Ke - r) * HS + 2 * r * SS);
         perMask += 2 * TG_DESC_W + 4 * Ke;
-        sm.useGlobalC = int64_t(acc) + 16 + 8ll * perMask > int64_t(ctx.dynWords) ? 1 : 0;
+        const int xWords = TG_VAR ? I.nAct * TG_MAX_K * TG_MAX_K : 0;      // transfer matrices of the activation-size classes (NEXT-3(b))
+        sm.useGlobalC = int64_t(acc) + xWords + 16 + 8ll * perMask > int64_t(ctx.dynWords) ? 1 : 0;
         sm.csUsed4 = int(acc >> 2);
-        sm.batchOff = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
+        sm.xOff = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
+        sm.batchOff = sm.xOff + xWords;
         if (team) {
             // team mode: every warp gets room for one mask's rows at the widest level (2 Ke - 1 rows), the cost rows come
             // next if they still fit, and what is left doubles the warps' buffers so that two masks run side by side
-            const int total = ctx.dynWords;
+            const int total = ctx.dynWords - xWords;
             const int perMaskW = max(1, 2 * Ke - 1) * HS;
             const int nWp = max(1, min(TG_NW, total / perMaskW));
             sm.useGlobalC = acc > uint32_t(total - nWp * perMaskW) ? 1 : 0;
             const int csUsed = sm.useGlobalC ? 0 : int((acc + 3u) & ~3u);
             sm.nWarps = nWp;
-            sm.wbufOff = csUsed;
+            sm.xOff = csUsed;
+            sm.wbufOff = csUsed + xWords;
             sm.wbufWords = min(2 * perMaskW, (total - csUsed) / nWp) & ~3;
         }
         if (count) {
@@ -341,6 +360,14 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         }
     }
     __syncthreads();
+    if (TG_VAR && I.nAct) {   // the transfer matrices of the size classes, thresholded like xS
+        uint32_t* xd = Cs + sm.xOff;
+        for (int w = tid; w < I.nAct * Ke * Ke; w += TG_NT) {
+            const int cls = w / (Ke * Ke), e = w - cls * Ke * Ke, kc = e / Ke, jc = e - kc * Ke;
+            const uint32_t xv = I.xAct[cls * (TG_MAX_K * TG_MAX_K) + int(sm.isl[kc]) * TG_MAX_K + int(sm.isl[jc])];
+            xd[cls * (TG_MAX_K * TG_MAX_K) + kc * TG_MAX_K + jc] = (I.xbound && xv > T) ? TG_INFU : xv;
+        }
+    }
     nAdm = tgStageCosts(ctx, sm, Cs, 1, count);
     if (count) {   // statistics: admissible relaxations of this DP (stage + transfer)
         for (int o = 16; o > 0; o >>= 1) nAdm += __shfl_down_sync(0xffffffffu, nAdm, o);
@@ -364,7 +391,7 @@ __device__ void tgLevel0(const TgSolveCtx& ctx, TgShared& sm, uint32_t* G, unsig
         const int kc = w / Wd, a = tgLo4(sm, sm.maxlenK[kc]) + (w - kc * Wd);
         uint32_t v = TG_INFU;
         if (a < L) {
-            v = tgCostAt(I, 0, size_t(sm.isl[kc]) * I.triG + tgGOff(L, L - a) + a, T, nullptr);
+            v = TG_COST_AT(I, 0, size_t(sm.isl[kc]) * I.triG + tgGOff(L, L - a) + a, T, nullptr);
         }
         G[w] = v;
         if (post && a == 0 && v < TG_INFU)
@@ -454,7 +481,7 @@ __device__ __forceinline__ void tgIssueBatch(const uint32_t* srcRow, uint32_t sr
 // source row is read once (LDS.128) and serves NSL rows; slots past the mask's last row read an all-INF x row.
 // The item of chunk 0 also files its rows in the island lists phase 2 works from:
 //   record = { row-in-batch | lo4(S)/4 << 16 | (lo4(R) - lo4(S))/4 << 24 ,  S = R u {k} | k << 16 }
-template <int NSL>
+template <int NSL, bool ACTB>
 __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* desc, uint32_t srcAddr, uint32_t hAddr, uint2* list, int* cur,
                                           int nb, int r, int nk, int nbw, int nsg, uint32_t mNbw, uint32_t mNsg, uint32_t SSB,
                                           uint32_t HSB, uint32_t xsBase, uint32_t xInfAddr) {
@@ -477,6 +504,12 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
         for (int e = 0; e < NSL; ++e) { acc[e][0] = acc[e][1] = acc[e][2] = acc[e][3] = TG_INFU; }
         uint32_t sA = srcAddr + i * uint32_t(r) * SSB + ch * 16u;
         uint32_t Rb = R;
+        uint32_t co[4] = {0, 0, 0, 0};   // ACTB: byte offset of the transfer matrix of each of the chunk's 4 boundaries
+        if (ACTB) {
+            const int b0 = (max(0, Lw - int(w0 >> 16)) & ~3) + 4 * int(ch);   // the H row starts at b = lo4(R)
+#pragma unroll
+            for (int cq = 0; cq < 4; ++cq) co[cq] = uint32_t(sm.clsOfS[min(b0 + cq, 255)]) * (TG_MAX_K * TG_MAX_K * 4u);
+        }
 #pragma unroll 2
         for (int ji = 0; ji < r; ++ji) {
             const uint32_t j4 = uint32_t(__ffs(Rb) - 1) * 4u;
@@ -485,11 +518,20 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
             sA += SSB;
 #pragma unroll
             for (int e = 0; e < NSL; ++e) {
-                const uint32_t xv = tgLds1(xrow[e] + j4);   // x[k][j]: k sends to j
-                acc[e][0] = tgAddMin(xv, g4.x, acc[e][0]);
-                acc[e][1] = tgAddMin(xv, g4.y, acc[e][1]);
-                acc[e][2] = tgAddMin(xv, g4.z, acc[e][2]);
-                acc[e][3] = tgAddMin(xv, g4.w, acc[e][3]);
+                if (ACTB) {
+                    const bool ok = s0 + e < nk;                 // (an unused slot reads the one all-INF row)
+                    const uint32_t xa = xrow[e] + j4;
+                    acc[e][0] = tgAddMin(tgLds1(xa + (ok ? co[0] : 0u)), g4.x, acc[e][0]);
+                    acc[e][1] = tgAddMin(tgLds1(xa + (ok ? co[1] : 0u)), g4.y, acc[e][1]);
+                    acc[e][2] = tgAddMin(tgLds1(xa + (ok ? co[2] : 0u)), g4.z, acc[e][2]);
+                    acc[e][3] = tgAddMin(tgLds1(xa + (ok ? co[3] : 0u)), g4.w, acc[e][3]);
+                } else {
+                    const uint32_t xv = tgLds1(xrow[e] + j4);   // x[k][j]: k sends to j
+                    acc[e][0] = tgAddMin(xv, g4.x, acc[e][0]);
+                    acc[e][1] = tgAddMin(xv, g4.y, acc[e][1]);
+                    acc[e][2] = tgAddMin(xv, g4.z, acc[e][2]);
+                    acc[e][3] = tgAddMin(xv, g4.w, acc[e][3]);
+                }
             }
         }
         const bool first = ch == 0, last = int(ch) + 1 == nbw;
@@ -528,7 +570,7 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
                 const int d = dq + 1 + e;                                                      \
                 c4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);                           \
                 if (d <= dm && c < ((L - d + 3) >> 2)) {                                       \
-                    c4 = tgCostAt4(I, sm.cdOff, cdkOff + tgGOff(L, d) + 4 * c, T);             \
+                    c4 = TG_COST_AT4(I, sm.cdOff, cdkOff + tgGOff(L, d) + 4 * c, T);             \
                     const int amax = L - 1 - d;                                                \
                     c4.x = (a0 + 0 <= amax) ? c4.x : TG_INFU;                                  \
                     c4.y = (a0 + 1 <= amax) ? c4.y : TG_INFU;                                  \
@@ -617,7 +659,7 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
         const int NB = min(min(TG_NB_MAX, hi - lo), max(1, (avail - 32) / perMask));
         // phase-1 items take NSL rows each: fewest CTA passes x instructions per item
         int best = 1, bestCost = 0x7fffffff;
-        for (int nsl = 1; nsl <= TG_SPL; nsl <<= 1) {
+        for (int nsl = 1; nsl <= (sm.sNAct ? 4 : TG_SPL); nsl <<= 1) {
             const int items = NB * nbw * ((nk + nsl - 1) / nsl);
             const int cost = ((items + TG_NT - 1) / TG_NT) * (3 + 5 * nsl);
             if (cost < bestCost) { bestCost = cost; best = nsl; }
@@ -642,7 +684,9 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
     const uint32_t hAddr = tgSmemAddr(dyn + sm.lvH);
     const uint32_t srcAddr[2] = {tgSmemAddr(dyn + sm.lvSrc[0]), tgSmemAddr(dyn + sm.lvSrc[1])};
     const uint32_t HSB = uint32_t(HS) * 4u, SSB = uint32_t(SS) * 4u, cStride = uint32_t(Lp) * 4u;
-    const uint32_t csBase = tgSmemAddr(dyn), xsBase = tgSmemAddr(&sm.xS[0][0]), xInfAddr = tgSmemAddr(&sm.xInf[0]);
+    const bool actb = TG_VAR && sm.sNAct > 0;
+    const uint32_t csBase = tgSmemAddr(dyn), xInfAddr = tgSmemAddr(&sm.xInf[0]);
+    const uint32_t xsBase = actb ? tgSmemAddr(dyn + sm.xOff) : tgSmemAddr(&sm.xS[0][0]);
     const bool globalC = sm.useGlobalC != 0;
     const int nBatches = (hi - lo + NB - 1) / NB;
     unsigned long long bestKey = TG_KEY_NONE;
@@ -678,8 +722,9 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
             tgIssueBatch(srcRowB[par ^ 1], srcAddr[par ^ 1], Gprev, min(NB, hi - m0 - NB), r, Wd, nbw, mNbw, SSB);
             cursors(par ^ 1);
         }
-#define TG_P1_CASE(N) case N: tgPhase1B<N>(sm, descB[par], srcAddr[par], hAddr, list, sm.cur[par], nb, r, nk, nbw, nsg, mNbw, mNsg, SSB, HSB, xsBase, xInfAddr); break;
-        switch (nsl) { TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(4) TG_P1_CASE(8) }
+#define TG_P1_CASE(N, A) case N: tgPhase1B<N, A>(sm, descB[par], srcAddr[par], hAddr, list, sm.cur[par], nb, r, nk, nbw, nsg, mNbw, mNsg, SSB, HSB, xsBase, xInfAddr); break;
+        if (actb) switch (nsl) { TG_P1_CASE(1, true) TG_P1_CASE(2, true) TG_P1_CASE(4, true) }   // (at most 4 rows an item with size classes)
+        else switch (nsl) { TG_P1_CASE(1, false) TG_P1_CASE(2, false) TG_P1_CASE(4, false) TG_P1_CASE(8, false) }
 #undef TG_P1_CASE
         __syncthreads();   // H rows and the island-sorted list of batch n are complete
         uint32_t* const gBatch = Gcur + size_t(m0) * nk * Wd;
@@ -771,10 +816,10 @@ __device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, bool
 // phase 1 for the NSL k slots  slot0, slot0+NG, ...  of this lane's island group and its b chunks:
 //   H[R][k][b] = min_{j in R} x[k][j] + src[j][b],  written to the warp's H rows.
 // All slots but the last are valid for every lane; an invalid last slot reads an all-INF x row.
-template <int NSL>
+template <int NSL, bool ACTB>
 __device__ __forceinline__ void tgPhase1W(const TgShared& sm, uint32_t R, int r, int nk, int nb4, int c0, int CH, int NG,
                                          int slot0, uint32_t srcAddr, uint32_t rowBytes, uint32_t hAddr0, const uint8_t* kl,
-                                         uint32_t xsBase, uint32_t xInfAddr) {
+                                         uint32_t xsBase, uint32_t xInfAddr, int lo4R) {
     uint32_t xrow[NSL];
 #pragma unroll
     for (int i = 0; i < NSL; ++i) {
@@ -787,6 +832,11 @@ __device__ __forceinline__ void tgPhase1W(const TgShared& sm, uint32_t R, int r,
 #pragma unroll
         for (int i = 0; i < NSL; ++i) { acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = TG_INFU; }
         const bool hasNx = c + 1 < nb4;
+        uint32_t co[4] = {0, 0, 0, 0};
+        if (ACTB) {
+#pragma unroll
+            for (int cq = 0; cq < 4; ++cq) co[cq] = uint32_t(sm.clsOfS[min(lo4R + 4 * c + cq, 255)]) * (TG_MAX_K * TG_MAX_K * 4u);
+        }
         uint32_t sA = srcAddr + uint32_t(c) * 16u;
         uint32_t Rb = R;
 #pragma unroll 2
@@ -797,11 +847,20 @@ __device__ __forceinline__ void tgPhase1W(const TgShared& sm, uint32_t R, int r,
             sA += rowBytes;
 #pragma unroll
             for (int i = 0; i < NSL; ++i) {
-                const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
-                acc[i][0] = tgAddMin(xv, g4.x, acc[i][0]);
-                acc[i][1] = tgAddMin(xv, g4.y, acc[i][1]);
-                acc[i][2] = tgAddMin(xv, g4.z, acc[i][2]);
-                acc[i][3] = tgAddMin(xv, g4.w, acc[i][3]);
+                if (ACTB) {   // per-boundary activation sizes: the transfer matrix of each of the chunk's 4 boundaries
+                    const bool ok = i + 1 < NSL || lastValid;
+                    const uint32_t xa = xrow[i] + j4;
+                    acc[i][0] = tgAddMin(tgLds1(xa + (ok ? co[0] : 0u)), g4.x, acc[i][0]);
+                    acc[i][1] = tgAddMin(tgLds1(xa + (ok ? co[1] : 0u)), g4.y, acc[i][1]);
+                    acc[i][2] = tgAddMin(tgLds1(xa + (ok ? co[2] : 0u)), g4.z, acc[i][2]);
+                    acc[i][3] = tgAddMin(tgLds1(xa + (ok ? co[3] : 0u)), g4.w, acc[i][3]);
+                } else {
+                    const uint32_t xv = tgLds1(xrow[i] + j4);   // x[k][j]: k sends to j
+                    acc[i][0] = tgAddMin(xv, g4.x, acc[i][0]);
+                    acc[i][1] = tgAddMin(xv, g4.y, acc[i][1]);
+                    acc[i][2] = tgAddMin(xv, g4.z, acc[i][2]);
+                    acc[i][3] = tgAddMin(xv, g4.w, acc[i][3]);
+                }
             }
         }
 #pragma unroll
@@ -899,7 +958,8 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     const int c0 = sl & (CH - 1), g = sl >> chShift;
     const uint32_t rowBytes = uint32_t(HS) * 4u, cStride = uint32_t(Lp) * 4u;
     const uint32_t hAddr0 = tgSmemAddr(wbuf) + uint32_t(sub) * uint32_t(nk + 2 * r) * rowBytes;
-    const uint32_t csBase = tgSmemAddr(Cs), xsBase = tgSmemAddr(&sm.xS[0][0]);
+    const bool actb = TG_VAR && sm.sNAct > 0;
+    const uint32_t csBase = tgSmemAddr(Cs), xsBase = actb ? tgSmemAddr(Cs + sm.xOff) : tgSmemAddr(&sm.xS[0][0]);
     const uint32_t xInfAddr = tgSmemAddr(&sm.xInf[0]);
     const uint32_t bufAddr[2] = {hAddr0 + uint32_t(nk) * rowBytes, hAddr0 + uint32_t(nk + r) * rowBytes};
     uint32_t* rowOf = &sm.rowOf[warp][sub * TG_MAX_K];
@@ -934,12 +994,15 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
 
         // ---- phase 1: transfer pre-minimum, H rows into the sub-warp's shared memory -----------
         if (valid) {
-            for (int s0 = 0; s0 < nk; s0 += NG * TG_SPL) {
-                const int nsl = min(TG_SPL, (nk - s0 + NG - 1) >> (SWSH - chShift));   // slots of the widest island group
-#define TG_P1_CASE(N) case N: tgPhase1W<N>(sm, R, r, nk, nbw, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr); break;
-                switch (nsl) {
-                    TG_P1_CASE(1) TG_P1_CASE(2) TG_P1_CASE(3) TG_P1_CASE(4)
-                    TG_P1_CASE(5) TG_P1_CASE(6) TG_P1_CASE(7) TG_P1_CASE(8)
+            const int spl = actb ? 4 : TG_SPL;   // (the per-boundary variant keeps 4 transfer offsets more per lane)
+            for (int s0 = 0; s0 < nk; s0 += NG * spl) {
+                const int nsl = min(spl, (nk - s0 + NG - 1) >> (SWSH - chShift));   // slots of the widest island group
+#define TG_P1_CASE(N, A) case N: tgPhase1W<N, A>(sm, R, r, nk, nbw, c0, CH, NG, s0 + g, bufAddr[b], rowBytes, hAddr0, kl, xsBase, xInfAddr, lo4Rw); break;
+                const int lo4Rw = tgLo4(sm, capR);
+                if (actb) switch (nsl) { TG_P1_CASE(1, true) TG_P1_CASE(2, true) TG_P1_CASE(3, true) TG_P1_CASE(4, true) }
+                else switch (nsl) {
+                    TG_P1_CASE(1, false) TG_P1_CASE(2, false) TG_P1_CASE(3, false) TG_P1_CASE(4, false)
+                    TG_P1_CASE(5, false) TG_P1_CASE(6, false) TG_P1_CASE(7, false) TG_P1_CASE(8, false)
                 }
 #undef TG_P1_CASE
             }
@@ -1007,7 +1070,7 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
             const int Wd = sm.sWd;
             const uint32_t* Gl = slot + tgLevelOff(0, Ke, Wd, r - 1);
             // this stage is followed by r later ones: its cost and plan come from the table of depth r + 1
-            const size_t dq = I.nDepth > 1 ? size_t(r) : 0;
+            const size_t dq = (TG_VAR && I.nDepth > 1) ? size_t(r) : 0;
             int capR = 0;   // every source row (R\{j}, j) starts at start lo4(cap(R))
             for (int j = 0; j < Ke; ++j) if (R >> j & 1u) capR += sm.maxlenK[j];
             const int lo4R = tgLo4(sm, capR);
@@ -1018,12 +1081,12 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
             for (int p = lane; p < nb * r; p += 32) {
                 const int ji = p / nb, bb = bLo + (p - ji * nb);
                 int layer = 0;
-                const uint32_t c = tgCostAt(I, dq * K * I.triG, size_t(ko) * I.triG + tgGOff(L, bb - a) + a, T, &layer);
+                const uint32_t c = TG_COST_AT(I, dq * K * I.triG, size_t(ko) * I.triG + tgGOff(L, bb - a) + a, T, &layer);
                 if (c >= TG_INFU) continue;
                 const int j = int(__fns(R, 0, ji + 1));
                 const uint32_t Rp = R ^ (1u << j);
                 const size_t row = size_t(ctx.rankOf[Rp]) * (Ke - r + 1) + (j - __popc(R & ((1u << j) - 1u)));
-                const uint32_t xv = I.x[ko * TG_MAX_K + isl[j]];
+                const uint32_t xv = (TG_VAR && I.nAct) ? I.xAct[int(I.clsOf[bb]) * (TG_MAX_K * TG_MAX_K) + ko * TG_MAX_K + isl[j]] : I.x[ko * TG_MAX_K + isl[j]];
                 if (I.xbound && xv > T) continue;
                 const uint32_t v = c + xv + __ldcg(Gl + row * Wd + (bb - lo4R));
                 if (v >= TG_INFU) continue;
@@ -1039,14 +1102,14 @@ __device__ void tgBacktrack(const TgSolveCtx& ctx, const TgShared& sm, const TgI
             if (best == TG_KEY_NONE) { bad = true; break; }
             b = int(best >> 8) & 0xffffff;
             const int j = int(best & 0xffu);
-            const size_t tbl = I.nLayers ? size_t(bestLayer) : dq;   // (the layer depends on (a, b, k) only: every lane with the winning b agrees)
+            const size_t tbl = (TG_VAR && I.nLayers) ? size_t(bestLayer) : dq;   // (the layer depends on (a, b, k) only: every lane with the winning b agrees)
             sb[n] = a; si[n] = ko; sp[n] = I.argp[tbl * size_t(I.NS) * K + size_t(tgSliceIdx(L, a, b)) * K + ko];
             ++n;
             a = b; k = j; R ^= 1u << j;
             continue;
         }
         int lastLayer = 0;
-        tgCostAt(I, 0, size_t(ko) * I.triG + tgGOff(L, b - a) + a, T, &lastLayer);
+        TG_COST_AT(I, 0, size_t(ko) * I.triG + tgGOff(L, b - a) + a, T, &lastLayer);
         sb[n] = a; si[n] = ko; sp[n] = I.argp[size_t(lastLayer) * I.NS * K + size_t(tgSliceIdx(L, a, b)) * K + ko];
         ++n;
         break;
@@ -1093,7 +1156,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
         for (int r = 1; r < Ke; ++r) {
             const uint32_t* Gprev = slot + tgLevelOff(bufWords, Ke, Wd, r - 1);
             uint32_t* Gcur = slot + tgLevelOff(bufWords, Ke, Wd, r);
-            if (I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
+            if (TG_VAR && I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
             if (teamSize > 1) {
                 const int warp = threadIdx.x >> 5, nW = sm.nWarps;
                 if (warp < nW) {
@@ -1741,3 +1804,7 @@ __global__ void tgPoisonOnErrorKernel(const TgCtrl* __restrict__ ctrl, tg_result
         out[i].iter_time_us = INT64_MAX;
     }
 }
+
+}  // namespace TG_SOLVE_NS
+#undef TG_COST_AT
+#undef TG_COST_AT4
