@@ -76,8 +76,12 @@ tg_status tg_instance_create(int32_t L, int32_t K, int32_t P, int32_t m, const i
  *   class_time_us   EITHER [n_classes][K][P], class_mem_mb likewise (same value rules as tg_instance_create)
  * and the instance is by definition the one whose time_us[s][k][p] = class_time_us[class_of_slice[s]][k][p] (same
  * for mem_mb); 1 <= n_classes <= NS.  Only the class tables cross the host-device link (for identical layers
- * n_classes = L: NS/L = (L+1)/2 times fewer bytes); they are expanded on the device.  Everything else as
- * tg_instance_create; a class index out of range -> TG_ERR_RANGE. */
+ * n_classes = L: NS/L = (L+1)/2 times fewer bytes).  The instance keeps them: tg_solve_batch's cost-table loader reads the
+ * class rows (n_classes*K*P entries, L2 resident) instead of the NS*K*P expanded entries, and when the class of a slice
+ * depends on its length only (identical layers; detected at creation) a staged cost row is one value per diagonal,
+ * broadcast instead of read per start.  The expanded tables are also materialised on the device (tg_instance_read_time,
+ * tg_prune and the variant tables work on them; after tg_prune, tg_instance_set_actmem or tg_instance_set_stages they
+ * alone define the instance).  Everything else as tg_instance_create; a class index out of range -> TG_ERR_RANGE. */
 tg_status tg_instance_create_classes(int32_t L, int32_t K, int32_t P, int32_t m, int32_t n_classes,
                                      const int32_t* class_of_slice, const int32_t* class_time_us,
                                      const int32_t* class_mem_mb, const int32_t* island_gpus,

@@ -36,6 +36,9 @@ struct tg_instance {
     int device;
     int32_t *time_us, *mem_mb, *gpus, *cap_mb, *bw;  // device
     int32_t* actmem;                                 // device, or nullptr (tg_instance_set_actmem)
+    int32_t* cls = nullptr;                          // device block [classOf NS | class time NC*K*P | class mem NC*K*P], or nullptr
+    int32_t nClasses = 0;                            //   (tg_instance_create_classes; dropped when the instance is pruned or gets
+    bool toeplitz = false;                           //   footprint / stage tables: they work on the expanded tables)
     int32_t nAct = 0;                                // tg_instance_set_boundary_act: distinct activation sizes (0 = scalar act_mb)
     int32_t actVal[TG_MAX_ACT] = {0, 0, 0, 0, 0, 0, 0, 0};
     uint8_t clsOf[256] = {0};                        // size class of boundary b
@@ -213,7 +216,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     Carver cv;
     const size_t oInst = cv.take(sizeof(TgInstDev) * n);
     std::vector<TgInstDev> h(n);
-    std::vector<size_t> oXa(n), oCd(n), oThr(n), oArgp(n), oCand(n), oSort(n), oSort2(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
+    std::vector<size_t> oCdT(n), oXa(n), oCd(n), oThr(n), oArgp(n), oCand(n), oSort(n), oSort2(n), oSuf(n), oSufA(n), oEI(n), oEF(n);
     int maxCells = 0, maxLp = 4, maxK = 1;
     uint64_t maxFull = 0;
     size_t denseCs = 0;
@@ -225,6 +228,13 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         I.actmem_mb = t.actmem;
         I.nDepth = t.actmem ? t.K : 1;
         if (t.actmem || t.slow || t.nAct) W.variants = true;
+        if (t.cls) {
+            const size_t nC4 = size_t(t.nClasses) * t.K * t.P * 4;
+            I.classOf = t.cls;
+            I.ctime = reinterpret_cast<const int32_t*>(reinterpret_cast<const char*>(t.cls) + alignUp(size_t(t.NS) * 4, 256));
+            I.cmem = reinterpret_cast<const int32_t*>(reinterpret_cast<const char*>(I.ctime) + alignUp(nC4, 256));
+            I.toeplitz = t.toeplitz ? 1 : 0;
+        }
         I.slow_us = t.slow;
         I.nLayers = t.slow ? t.P : 0;
         I.nTables = std::max(std::max(I.nDepth, I.nLayers), 1);
@@ -261,6 +271,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         oCd[i] = cv.take(nd * size_t(t.K) * I.triG * 4);
         oThr[i] = I.nLayers ? cv.take(nd * size_t(t.K) * I.triG * 4) : 0;
         oArgp[i] = cv.take(nd * size_t(cells));
+        oCdT[i] = (t.cls && t.toeplitz) ? cv.take(size_t(t.K) * (t.L + 2) * 4) : 0;
         oXa[i] = t.nAct ? cv.take(size_t(t.nAct) * TG_MAX_K * TG_MAX_K * 4) : 0;
         const size_t nKeys = nd * size_t(cells) + size_t(t.K) * t.K * std::max(t.nAct, 1);   // every reduced cost + (transfer bound) every transfer time
         oCand[i] = cv.take(nKeys * 4);
@@ -311,6 +322,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     for (int i = 0; i < n; ++i) {
         h[i].cd = reinterpret_cast<uint32_t*>(W.base + oCd[i]);
         h[i].thr = h[i].nLayers ? reinterpret_cast<uint32_t*>(W.base + oThr[i]) : nullptr;
+        h[i].cdT = (h[i].classOf && h[i].toeplitz) ? reinterpret_cast<uint32_t*>(W.base + oCdT[i]) : nullptr;
         h[i].xAct = h[i].nAct ? reinterpret_cast<uint32_t*>(W.base + oXa[i]) : nullptr;
         h[i].argp = reinterpret_cast<uint8_t*>(W.base + oArgp[i]);
         h[i].cand = reinterpret_cast<uint32_t*>(W.base + oCand[i]);
@@ -570,6 +582,7 @@ tg_status tg_instance_create_classes(int32_t L, int32_t K, int32_t P, int32_t m,
     char *base = nullptr, *tmp = nullptr;
     Carver cv, ct;
     const size_t oT = cv.take(nE * 4), oM = cv.take(nE * 4), oG = cv.take(K * 4), oC = cv.take(K * 4), oB = cv.take(K * K * 4), oE = cv.take(4);
+    // one block, kept by the instance: [classOf | class time | class mem], each 256-byte aligned (16-byte loads)
     const size_t oCls = ct.take(size_t(NS) * 4), oCt = ct.take(nC * 4), oCm = ct.take(nC * 4);
     TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&base), cv.off, 0));
     cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&tmp), ct.off, 0);
@@ -596,16 +609,21 @@ tg_status tg_instance_create_classes(int32_t L, int32_t K, int32_t P, int32_t m,
     int herr = 0;
     if (e == cudaSuccess) {
         const int blocks = std::max(1, int(std::min<size_t>((nE + 255) / 256, 4096)));
-        tgExpandClassesKernel<<<blocks, 256>>>(dCls, dCt, dCm, n_classes, int(KP), nE, t->time_us, t->mem_mb, dErr);
+        tgExpandClassesKernel<<<blocks, 256>>>(dCls, dCt, dCm, n_classes, L, int(KP), nE, t->time_us, t->mem_mb, dErr);
         tgValidateKernel<<<blocks, 256>>>(t->time_us, t->mem_mb, t->gpus, t->cap_mb, t->bw, K, nE, dErr);
         e = cudaMemcpy(&herr, dErr, 4, cudaMemcpyDeviceToHost);   // the one synchronisation of the call
     }
-    cudaFreeAsync(tmp, 0);
+    const bool toeplitz = !(herr & 64);   // bit 64 is not an error: the class of some slice depends on more than its length
+    herr &= ~64;
     if (e != cudaSuccess || herr) {
+        cudaFreeAsync(tmp, 0);
         tg_instance_destroy(t);
         if (e != cudaSuccess) return fail(TG_ERR_CUDA, std::string("instance upload: ") + cudaGetErrorString(e));
         return fail(TG_ERR_RANGE, "value out of range (bits: 1 time, 2 mem, 4 bw, 8 gpus, 16 cap, 32 class index): " + std::to_string(herr));
     }
+    t->cls = reinterpret_cast<int32_t*>(tmp);
+    t->nClasses = n_classes;
+    t->toeplitz = toeplitz;
     *out = t;
     return TG_OK;
 }
@@ -744,6 +762,7 @@ tg_status tg_instance_destroy(tg_instance* inst) {
     if (!inst) return TG_OK;
     if (inst->actmem) cudaFreeAsync(inst->actmem, 0);
     if (inst->slow) cudaFreeAsync(inst->slow, 0);
+    if (inst->cls) cudaFreeAsync(inst->cls, 0);
     if (inst->block) {   // created by tg_instance_create_batch: the allocation goes with the last instance of the batch
         TgBatchBlock* blk = inst->block;
         if (blk->refs.fetch_sub(1) == 1) { cudaFreeAsync(blk->base, 0); delete blk; }
@@ -758,6 +777,7 @@ tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb) {
     if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
     if (inst->actmem) { cudaFreeAsync(inst->actmem, 0); inst->actmem = nullptr; }
     if (!actmem_mb) return TG_OK;
+    if (inst->cls) { cudaFreeAsync(inst->cls, 0); inst->cls = nullptr; }   // (from here on the expanded tables are the instance)
     if (inst->slow) return fail(TG_ERR_SHAPE, "the instance has multi-stage partial plans (tg_instance_set_stages): the combination with a footprint table is not built");
     const size_t nE = size_t(inst->NS) * inst->K * inst->P;
     int32_t* d = nullptr;
@@ -784,6 +804,7 @@ tg_status tg_instance_set_stages(tg_instance* inst, const int32_t* slow_us, cons
     if (!inst) return fail(TG_ERR_NULL, "inst is NULL");
     if (inst->slow) { cudaFreeAsync(inst->slow, 0); inst->slow = nullptr; inst->qst = nullptr; }
     if (!slow_us) return TG_OK;
+    if (inst->cls) { cudaFreeAsync(inst->cls, 0); inst->cls = nullptr; }   // (from here on the expanded tables are the instance)
     if (inst->actmem) return fail(TG_ERR_SHAPE, "the instance has a footprint table (tg_instance_set_actmem): the combination with multi-stage partial plans is not built");
     if (inst->nAct) return fail(TG_ERR_SHAPE, "the instance has per-boundary activation sizes (tg_instance_set_boundary_act): the combination with multi-stage partial plans is not built");
     const size_t nE = size_t(inst->NS) * inst->K * inst->P;
@@ -954,6 +975,7 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
         tg_instance* t = instances[i];
         if (!t) return fail(TG_ERR_NULL, "instances[" + std::to_string(i) + "] is NULL");
         if (t->slow) return fail(TG_ERR_SHAPE, "instances[" + std::to_string(i) + "] has multi-stage partial plans: tg_prune is not built for them");
+        if (t->cls) { cudaFreeAsync(t->cls, 0); t->cls = nullptr; }   // pruning edits the expanded tables: they are the instance from now on
         h[i] = TgPruneDesc{t->time_us, t->mem_mb, t->actmem, t->cap_mb, t->L, t->K, t->P, t->NS * t->K};
         maxCells = std::max(maxCells, h[i].nCells);
     }

@@ -55,6 +55,14 @@ struct TgInstDev {
     const int32_t* time_us;  // [NS][K][P] (instance-owned)
     const int32_t* mem_mb;   // [NS][K][P]
     const int32_t* actmem_mb;  // [NS][K][P] MB per in-flight microbatch, or nullptr (NEXT-1: depth-aware memory)
+    // NEXT-3(a), tables per signature class (tg_instance_create_classes): the loader reads the class tables
+    // (nClasses * K * P entries) instead of the expanded ones; toeplitz = the class of a slice depends on its length only
+    // (identical layers): a cost row is then one value per diagonal, kept in cdT and broadcast when the rows are staged
+    const int32_t* classOf;    // [NS] class of slice s, or nullptr
+    const int32_t* ctime;      // [nClasses][K][P]
+    const int32_t* cmem;       // [nClasses][K][P]
+    uint32_t* cdT;             // [K][L+2] toeplitz: reduced cost of island k at slice length d (workspace), else nullptr
+    int32_t toeplitz;
     const int32_t* slow_us;    // [NS][K][P] slowest internal stage of the partial plan, or nullptr (NEXT-2: multi-stage partial plans)
     uint32_t* thr;             // NEXT-2: [nLayers][K][triG] thresholds of the cells' cost steps (diagonal-major like cd), TG_INFU = no such step
     const int32_t* cap_mb;   // [K]

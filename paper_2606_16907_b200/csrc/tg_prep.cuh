@@ -96,13 +96,18 @@ __global__ void tgValidateBatchKernel(const TgValidateDesc* __restrict__ desc, i
 
 // tg_instance_create_classes: time/mem[s][k][p] = class table[class_of[s]][k][p]; err bit 32 = class index out of range
 __global__ void tgExpandClassesKernel(const int32_t* __restrict__ classOf, const int32_t* __restrict__ ctime,
-                                      const int32_t* __restrict__ cmem, int nClasses, int KP, size_t nEntries,
+                                      const int32_t* __restrict__ cmem, int nClasses, int L, int KP, size_t nEntries,
                                       int32_t* __restrict__ time_us, int32_t* __restrict__ mem_mb, int* err) {
     int bad = 0;
     for (size_t i = size_t(blockIdx.x) * blockDim.x + threadIdx.x; i < nEntries; i += size_t(gridDim.x) * blockDim.x) {
         const size_t s = i / size_t(KP), r = i - s * size_t(KP);
         const int c = classOf[s];
         if (c < 0 || c >= nClasses) { bad = 32; time_us[i] = TG_INVALID; mem_mb[i] = 0; continue; }
+        if (r == 0) {   // class map of identical layers: the class depends on the slice length only (bit 64 = it does not)
+            int a, b;
+            tgSliceAB(L, int(s), a, b);
+            if (a > 0 && classOf[b - a - 1] != c) bad |= 64;
+        }
         time_us[i] = ctime[size_t(c) * KP + r];
         mem_mb[i] = cmem[size_t(c) * KP + r];
     }
@@ -194,7 +199,7 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
     __shared__ uint32_t sMin[TG_MAX_K];
     __shared__ int32_t sCap[TG_MAX_K];
     __shared__ uint32_t sMax;
-    const bool fast = PV > 0 && P == 4 * PV && I.actmem_mb == nullptr && I.slow_us == nullptr;
+    const bool fast = PV > 0 && P == 4 * PV && I.actmem_mb == nullptr && I.slow_us == nullptr && I.classOf == nullptr;
     int4 tv[U][PVA], mv[U][PVA];
     if (fast) {
 #pragma unroll
@@ -286,6 +291,16 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
                                 I.cd[j * stride + off + (pp - a)] = TG_INFU;
                             }
                     }
+                } else if (I.classOf != nullptr) {
+                    // NEXT-3(a): the cell's plans are those of its slice's signature class -- nClasses * K * P entries are
+                    // read (and stay in L2) instead of NS * K * P
+                    const size_t e = (size_t(__ldg(I.classOf + cell / K)) * K + k) * P;
+                    uint32_t bq; int bp;
+                    if ((P & 3) == 0) tgReduceCell<true>(I.ctime + e, I.cmem + e, P, capk, bq, bp);
+                    else tgReduceCell<false>(I.ctime + e, I.cmem + e, P, capk, bq, bp);
+                    tgLoadEmit(I, L, K, nCells, cell, a, b, k, 1, bq, bp, prev, myMax);
+                    if (I.cdT && a == 0) I.cdT[k * (L + 2) + (b - a)] = bq;
+                    best = bq;
                 } else {
                     const size_t e = size_t(cell) * P;
                     best = TG_INFU;
@@ -359,8 +374,10 @@ __global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ 
         for (int u = 0; u < U; ++u) {
             const int cell = base + 256 * u + tid;
             if (cell < cellEnd) {
-                const int4* t4 = reinterpret_cast<const int4*>(I.time_us + size_t(cell) * (4 * PV));
-                const int4* m4 = reinterpret_cast<const int4*>(I.mem_mb + size_t(cell) * (4 * PV));
+                // (NEXT-3(a): a class instance reads the rows of its slice's signature class)
+                const size_t src = I.classOf ? size_t(__ldg(I.classOf + cell / K)) * K + size_t(cell % K) : size_t(cell);
+                const int4* t4 = reinterpret_cast<const int4*>((I.classOf ? I.ctime : I.time_us) + src * (4 * PV));
+                const int4* m4 = reinterpret_cast<const int4*>((I.classOf ? I.cmem : I.mem_mb) + src * (4 * PV));
 #pragma unroll
                 for (int v = 0; v < PV; ++v) { tv[u][v] = __ldg(t4 + v); mv[u][v] = __ldg(m4 + v); }
             }
@@ -385,6 +402,7 @@ __global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ 
                             if (t4[e] != TG_INVALID && m4[e] <= capk && uint32_t(t4[e]) < bq) { bq = uint32_t(t4[e]); bp = 4 * v + e; }
                     }
                     tile[(k * L + (b - a - 1)) * TG_LOAD_RG + (a - a0)] = bq;
+                    if (I.cdT && a == 0) I.cdT[k * (L + 2) + (b - a)] = bq;
                     I.argp[cell] = uint8_t(bp);
                     I.sortbuf[cell] = bq;
                     if (bq < TG_INFU) myMax = max(myMax, bq);

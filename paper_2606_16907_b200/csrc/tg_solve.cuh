@@ -208,6 +208,10 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
                     v = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc])[w];
                     v.x = v.x <= T ? v.x : TG_INFU; v.y = v.y <= T ? v.y : TG_INFU;
                     v.z = v.z <= T ? v.z : TG_INFU; v.w = v.w <= T ? v.w : TG_INFU;
+                } else if (I.cdT) {
+                    // identical layers (NEXT-3(a)): the row is one value, read once per diagonal instead of once per start
+                    const uint32_t cv = __ldg(I.cdT + int(sm.isl[kc]) * (L + 2) + d);
+                    v = cv <= T ? make_uint4(cv, cv, cv, cv) : make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
                 } else
                 v = TG_COST_AT4(I, sm.cdOff, size_t(sm.isl[kc]) * I.triG + tgGOff(L, d) + 4 * a4, T);
                 const int a = a4 * 4, amax = L - 1 - d;

@@ -85,3 +85,30 @@ def test_class_errors(tg):
         big = np.zeros((NS + 1, b.K, b.P), np.int32)
         create(tg, b, class_of, big, big)
     assert e.value.status == 2
+
+
+def test_class_instances_after_prune_and_variant_tables(tg):
+    """The loader of a class instance reads the class tables; pruning or attaching footprint / stage tables makes the
+    expanded tables the instance (the class tables would be stale): results must follow the expanded definition."""
+    for seed in range(12):
+        b = gen.random_small(seed + 99_000, Lmax=8, Kmax=5, Pmax=3, style=STYLES[seed % 5])
+        class_of, ct, cm, e = gen.length_classes(b)
+        h = create(tg, b, class_of, ct, cm)
+        same(oracle.solve(e), tg.tg_solve_batch([h])[0], "class tables")
+        tg.tg_prune(h, tg.TG_PRUNE_BOTTLENECK, int(np.median(e.time_us[e.time_us != 0x7FFFFFFF])))
+        pr, _ = oracle.prune(e, 2, int(np.median(e.time_us[e.time_us != 0x7FFFFFFF])))
+        g = tg.tg_solve_batch([h])[0]
+        o = oracle.solve(pr)
+        assert o.feasible == (int(g["iter_time_us"]) != (1 << 63) - 1)
+        if o.feasible:
+            assert (o.iter_time_us, o.bottleneck_us, o.island_mask) == (int(g["iter_time_us"]), int(g["bottleneck_us"]), int(g["island_mask"]))
+        h.destroy()
+        h = create(tg, b, class_of, ct, cm)
+        ea = gen.with_actmem(e, seed, 0, 40)
+        tg.tg_instance_set_actmem(h, ea.actmem_mb)
+        od = oracle.solve_depth(ea)
+        g = tg.tg_solve_batch([h])[0]
+        assert od.feasible == (int(g["iter_time_us"]) != (1 << 63) - 1)
+        if od.feasible:
+            assert (od.iter_time_us, od.bottleneck_us, od.island_mask) == (int(g["iter_time_us"]), int(g["bottleneck_us"]), int(g["island_mask"]))
+        h.destroy()
