@@ -39,14 +39,14 @@ UNIT = "plans/s"
 
 
 def kernel_sources_sha() -> str:
-    """Fingerprint of the CUDA sources: an ncu figure is quoted only while the kernels are the ones that were profiled."""
+    """Fingerprint of the solver kernel's sources (tg_solve.cuh, tg_common.cuh): an ncu figure of that kernel is quoted only
+    while they are the ones that were profiled."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2606_16907_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
-            with open(os.path.join(d, f), "rb") as fh:
-                h.update(f.encode() + b"\0" + fh.read())
+    for f in ("tg_common.cuh", "tg_solve.cuh"):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read())
     return h.hexdigest()[:16]
 
 

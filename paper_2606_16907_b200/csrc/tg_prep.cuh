@@ -708,14 +708,16 @@ struct TgPruneDesc {
 // PV > 0: an instance with P = 4 * PV plans is pruned from registers -- the 16-byte loads of the thread's U cells are
 // issued first, the rules run on the register copy and a cell whose column changed is stored back as 16-byte words;
 // any other instance of the batch takes the entry-by-entry path.  grid = (cells / (256 U), instances).
-template <int PV, int U>
+// ACT = false: no instance of the batch has a footprint table -- the third dominance axis is compiled out (the pass is bound by
+// its comparisons, not by HBM: ncu showed the integer pipe at 72 %).
+template <int PV, int U, bool ACT>
 __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __restrict__ descs, int mode, int64_t threshold,
                                                          unsigned long long* counts) {
     constexpr int PVA = PV > 0 ? PV : 1, PP = 4 * PVA;
     const TgPruneDesc D = descs[blockIdx.y];
     int32_t* const time_us = D.time_us;
     const int32_t* const mem_mb = D.mem_mb;
-    const int32_t* const actmem_mb = D.actmem_mb;
+    const int32_t* const actmem_mb = ACT ? D.actmem_mb : nullptr;
     const int32_t* const cap = D.cap;
     const int nCells = D.nCells, K = D.K, P = D.P;
     counts += 4 * blockIdx.y;
@@ -732,7 +734,7 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
                 for (int v = 0; v < PVA; ++v) {
                     tv[u][v] = *(reinterpret_cast<const int4*>(time_us + size_t(cell) * PP) + v);
                     mv[u][v] = __ldg(reinterpret_cast<const int4*>(mem_mb + size_t(cell) * PP) + v);
-                    av[u][v] = actmem_mb ? __ldg(reinterpret_cast<const int4*>(actmem_mb + size_t(cell) * PP) + v) : make_int4(0, 0, 0, 0);
+                    av[u][v] = (ACT && actmem_mb) ? __ldg(reinterpret_cast<const int4*>(actmem_mb + size_t(cell) * PP) + v) : make_int4(0, 0, 0, 0);
                 }
             }
         }
@@ -751,7 +753,7 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
                 unsigned kill = 0;
 #pragma unroll
                 for (int p = 0; p < PP; ++p)   // R1
-                    if (t[p] != TG_INVALID && int64_t(mm[p]) + am[p] > capk) { t[p] = TG_INVALID; kill |= 1u << p; ++c1; }
+                    if (t[p] != TG_INVALID && (ACT ? int64_t(mm[p]) + am[p] > capk : mm[p] > capk)) { t[p] = TG_INVALID; kill |= 1u << p; ++c1; }
                 unsigned dead = 0;
 #pragma unroll
                 for (int p = 0; p < PP; ++p) {   // R2, decided on the cell as R1 left it
@@ -759,8 +761,8 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
 #pragma unroll
                     for (int q = 0; q < PP; ++q) {
                         if (q == p) continue;
-                        const bool le = t[q] <= t[p] && mm[q] <= mm[p] && am[q] <= am[p];   // t[q] == INVALID is never <= a live t[p]
-                        const bool eq = t[q] == t[p] && mm[q] == mm[p] && am[q] == am[p];
+                        const bool le = t[q] <= t[p] && mm[q] <= mm[p] && (!ACT || am[q] <= am[p]);   // t[q] == INVALID is never <= a live t[p]
+                        const bool eq = t[q] == t[p] && mm[q] == mm[p] && (!ACT || am[q] == am[p]);
                         dd = dd || (le && (!eq || q < p));
                     }
                     if (t[p] != TG_INVALID && dd) dead |= 1u << p;
