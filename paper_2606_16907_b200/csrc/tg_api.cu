@@ -84,6 +84,7 @@ int g_gallopMax = [] { const char* e = getenv("TG_GALLOP_MAX"); int v = e ? atoi
 // DPs per instance and scheduler round (speculation width of the threshold search / sweep)
 int g_wishFloor = [] { const char* e = getenv("TG_WISH_FLOOR"); int v = e ? atoi(e) : 8; return v < 1 ? 1 : (v > 12 ? 12 : v); }();
 int g_wishCap = [] { const char* e = getenv("TG_WISH_CAP"); int v = e ? atoi(e) : 12; return v < 8 ? 8 : (v > TG_MAX_WISH ? TG_MAX_WISH : v); }();
+int g_queueWish = [] { const char* e = getenv("TG_QUEUE_WISH"); int v = e ? atoi(e) : 6; return v < 1 ? 1 : (v > 12 ? 12 : v); }();
 int g_wishMax = [] { const char* e = getenv("TG_WISH_MAX"); int v = e ? atoi(e) : 64; return v < 1 ? 1 : (v > TG_MAX_WISH ? TG_MAX_WISH : v); }();
 DeviceState g_dev[64];
 
@@ -286,7 +287,8 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     const size_t oKeys = cv.take(sizeof(unsigned long long) * 2 * TG_MAX_ITEMS);
     const size_t oCtrl = cv.take(sizeof(TgCtrl));
     const size_t oOut = cv.take(sizeof(tg_result) * n);
-    const size_t oSpec = cv.take(sizeof(tg_result) * TG_MAX_ITEMS);
+    const size_t oSpec = cv.take(sizeof(tg_result) * TG_QCAP);
+    const size_t oSeq = cv.take(sizeof(uint32_t) * TG_QCAP);
     // DP scratch: nSlots slots, each able to hold every level of the largest instance.  A slot
     // belongs to one team (team mode) or one CTA (solo mode) for the duration of a DP.
     const int numCtas = D->numSMs * D->ctasPerSM;
@@ -338,6 +340,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     W.numCtas = numCtas;
     TG_CUDA(cudaMemcpyAsync(W.inst, h.data(), sizeof(TgInstDev) * n, cudaMemcpyHostToDevice, st));
     TG_CUDA(cudaMemsetAsync(W.base + oCtrl, 0, sizeof(TgCtrl), st));
+    TG_CUDA(cudaMemsetAsync(W.base + oSeq, 0, sizeof(uint32_t) * TG_QCAP, st));
 
     // shared-memory split of the solver: warp-private row buffers (H rows + two source buffers =
     // 2*Kmax rows of Lp+8 words per warp) vs staged cost tables (at least a quarter of the total)
@@ -353,6 +356,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.slotWords = slotWords; c.nSlots = nSlots;
     c.slotBar = reinterpret_cast<uint32_t*>(W.base + oBar);
     c.wishMax = g_wishMax;
+    c.queueWish = g_queueWish;
     c.gallopMax = g_gallopMax;
     c.wishCap = g_wishCap;
     c.wishFloor = g_wishFloor;
@@ -360,6 +364,7 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     c.rankOf = D->rankOf;
     c.maskOf = D->maskOf;
     c.specOut = reinterpret_cast<tg_result*>(W.base + oSpec);
+    c.itemSeq = reinterpret_cast<uint32_t*>(W.base + oSeq);
 
     // loader grid: 256 * U cells per CTA, U = TG_LOAD_U when that still gives every SM two CTAs, else 1; the
     // batched-load path is compiled for P = 4 and P = 8 (picked from the first instance; instances of another

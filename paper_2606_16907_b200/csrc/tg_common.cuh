@@ -16,6 +16,8 @@
                               // CTA's barriers, copy latencies and level tails are filled by the other
 #endif
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
+#define TG_QCAP (2 * TG_MAX_ITEMS)   // queue mode: ring slots (the two per-round item arrays back to back)
+#define TG_QUEUE_MAX_INST 1024       // queue mode: at most this many instances (each has <= 12 items in flight: 12 288 < TG_QCAP)
 #define TG_MAX_EVAL 1024      // evaluated thresholds remembered per instance
 #define TG_MAX_WISH 64        // DPs per instance and round, upper bound
 #define TG_PROBE_FINAL 0x40000000   // flag in probe[]: speculative final DP at the incumbent (S* only; keep every level, back-track)
@@ -98,6 +100,7 @@ struct TgInstDev {
     // ---- solver state (one scheduler thread per instance) ----
     int32_t phase, loInf, hiFeas, next;   // FEAS bracket: largest infeasible / smallest feasible candidate
     int32_t itemBeg, itemCnt, gstep, nrun;
+    int32_t pending;                      // queue mode: items of the current round still running (the CTA that takes it to 0 folds and plans)
     int32_t lbIdx;                        // first candidate passing the necessary condition sum_k maxlen_k(T) >= L
     int32_t incIdx;                       // incumbent = lexicographic min of (iter, candidate index); -1 = none
     int64_t incIter;
@@ -130,6 +133,11 @@ struct TgCtrl {
     uint32_t barrier;     // monotone arrival counter of the grid barrier
     int32_t errFlag;
     int32_t nActive;      // instances not done after the previous round's planning (wide scheduling: bounds W)
+    // queue mode (a batch of 64..TG_QUEUE_MAX_INST instances): no rounds, the items form one growing queue in a ring
+    uint32_t qHead;       // next item sequence number to hand out
+    uint32_t qTail;       // next sequence number to reserve for new items
+    int32_t nDoneInst;    // instances finished
+    int32_t allDone;      // every instance finished: CTAs waiting for an item leave
     int32_t weighted[2];  // per round parity: team sizes follow the items' estimated cost (teamOf / ctaBeg / ctaCnt)
     uint8_t teamOf[2][1024];  // weighted team mode: item of each CTA
     tg_solve_stats stats;
@@ -153,10 +161,12 @@ struct TgSolveCtx {
     int32_t wishMax;            // DPs per instance and round, upper bound
     int32_t gallopMax;          // probes of one galloping round
     int32_t wishFloor;          // lower end of the same
+    int32_t queueWish;          // queue mode: most probes an instance plans at a time (rounds are cheap there: less speculation pays)
     int32_t wishCap;            // upper end of the per-round probe count chosen from the instance shape (tgWish)
     uint32_t* slotBar;          // [nSlots] arrival counters of the team barriers, zeroed every round
     TgCtrl* ctrl;
-    tg_result* specOut;         // [TG_MAX_ITEMS] results of the current round's speculative back-tracks
+    tg_result* specOut;         // [2 * TG_MAX_ITEMS] results of speculative back-tracks, by item slot
+    uint32_t* itemSeq;          // [2 * TG_MAX_ITEMS] queue mode: sequence number + 1 of the item published in each ring slot
     tg_result* out;
     const uint16_t* rankOf;     // [65536] rank of a mask inside its popcount class
     const uint16_t* maskOf;     // [65536] the inverse: masks ordered by (popcount, value); class r starts at tgPopOff[r]

@@ -1257,9 +1257,11 @@ struct TgPrev {
     const uint32_t* candS;   // cand[tidx] of the item's instance
     const uint8_t* flagS;
     int nStage;
-    __device__ __forceinline__ unsigned long long key(int i) const { return i < nStage ? keyS[i] : __ldcg(keys + i); }
-    __device__ __forceinline__ int tidx(int i) const { return i < nStage ? tidxS[i] : __ldcg(&items[i].tidx); }
-    __device__ __forceinline__ int flags(int i) const { return i < nStage ? int(flagS[i]) : int(__ldcg(&items[i].flags)); }
+    uint32_t mask;           // item index -> slot: all ones (round mode: indices of one round's array) or TG_QCAP - 1 (queue mode: ring)
+    __device__ __forceinline__ int slot(int i) const { return int(uint32_t(i) & mask); }
+    __device__ __forceinline__ unsigned long long key(int i) const { return i < nStage ? keyS[i] : __ldcg(keys + slot(i)); }
+    __device__ __forceinline__ int tidx(int i) const { return i < nStage ? tidxS[i] : __ldcg(&items[slot(i)].tidx); }
+    __device__ __forceinline__ int flags(int i) const { return i < nStage ? int(flagS[i]) : int(__ldcg(&items[slot(i)].flags)); }
     __device__ __forceinline__ uint32_t cand(const TgInstDev& I, int i, int tx) const { return i < nStage ? candS[i] : I.cand[tx]; }
 };
 
@@ -1294,7 +1296,7 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev
         I.incIter = incIter; I.incIdx = incIdx;
         const uint32_t Sc = uint32_t(incKey >> 8) & 0xffffu;   // compact labels of that item
         uint32_t So = 0;
-        for (int e = 0; e < TG_MAX_K; ++e) if (Sc >> e & 1u) So |= 1u << __ldcg(&itemsPrev[beg + incQ].isl[e]);
+        for (int e = 0; e < TG_MAX_K; ++e) if (Sc >> e & 1u) So |= 1u << __ldcg(&itemsPrev[P.slot(beg + incQ)].isl[e]);
         I.incMask = So;
     }
     I.nrun += cnt;
@@ -1438,7 +1440,7 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
     }
     if (I.phase == TG_PH_FINAL) {
         if (ctx.mode == 0 && specItem >= 0) {   // already back-tracked (speculatively) in the round just folded
-            const unsigned long long* src = reinterpret_cast<const unsigned long long*>(ctx.specOut + specItem);
+            const unsigned long long* src = reinterpret_cast<const unsigned long long*>(ctx.specOut + (specItem & (TG_QCAP - 1)));
             unsigned long long* dst = reinterpret_cast<unsigned long long*>(ctx.out + i);
             for (int w = 0; w < int(sizeof(tg_result) / 8); ++w) dst[w] = __ldcg(src + w);
             ctx.out[i].n_thresholds_run = uint32_t(I.nrun);
@@ -1466,6 +1468,7 @@ __device__ void tgFoldPlanAll(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn
     if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->schedCyc[round][0] = clock64();
     TgPrev P;
     P.items = itemsPrev; P.keys = keysPrev; P.keyS = nullptr; P.tidxS = nullptr; P.candS = nullptr; P.flagS = nullptr; P.nStage = 0;
+    P.mask = 0xffffffffu;
     if (!wide) {   // stage keys, candidate indices, their thresholds and flags of the previous items in the (idle) dynamic shared memory
         const int nPrev = round > 0 ? ctrl->nItems[prv] : 0;
         const int room = int(size_t(ctx.dynWords) * 4 / 20);   // 17 bytes an item, padded
@@ -1557,6 +1560,98 @@ __device__ void tgFoldPlanAll(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn
         __syncthreads();
     }
     if (tid == 0 && round < 8 && blockIdx.x == 0) ctrl->schedCyc[round][1] = clock64();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Queue mode (a batch of TG_WIDE_MIN_INST .. TG_QUEUE_MAX_INST instances, default search).  The scheduler rounds cost
+// such a batch a grid barrier per round with the whole grid waiting for the round's last DP, the slowest instance's fold
+// and plan and the item layout (12 rounds: 13.5 % of the CTA cycles at cfg5, 18 % of the warp samples at the barrier).  But
+// an instance's next probes depend only on its OWN results.  So after the first round is laid out the items form one
+// queue in a ring of TG_QCAP slots: a CTA takes the next sequence number, waits until that item is published, runs the
+// DP, and decrements its instance's count of running items; the CTA that takes it to zero folds and plans THAT instance
+// right away (state machine of tgFoldInstance / tgPlanInstance, unchanged, on a shared-memory copy of the instance's
+// search state) and appends its new items to the queue.  No grid barrier after the first round; CTAs leave when every
+// instance is done.  An instance plans few probes at a time (TG_QUEUE_WISH, default 6) while the queue is long and the full
+// width once CTAs would otherwise wait, so the NUMBER of DPs an instance runs (n_thresholds_run, a diagnostic) depends on
+// the timing; the result does not -- every schedule of the exact search returns the same optimum and plan.
+// Measured at cfg5: 27.8 -> 23.8 ms, 47 588 -> ~44 600 DPs, grid-wait share of the CTA cycles 13.5 -> 4 %.
+// ---------------------------------------------------------------------------------------------
+__device__ void tgQueueFoldPlan(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn, int i) {
+    const int tid = threadIdx.x;
+    TgCtrl* ctrl = ctx.ctrl;
+    constexpr int INST_W = int(sizeof(TgInstDev) / 4);
+    uint32_t* sInst = dyn;                                  // [INST_W] copy of the instance record
+    uint32_t* sEval = sInst + ((INST_W + 3) & ~3);          // [2][TG_MAX_EVAL] evaluated thresholds
+    uint32_t* sCand = sEval + 2 * TG_MAX_EVAL;              // [TG_CAND_WIN] window of the candidate list
+    __threadfence();                                        // the keys the other CTAs posted for this instance's items
+    {
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(ctx.inst + i);
+        for (int w = tid; w < INST_W; w += TG_NT) sInst[w] = __ldcg(src + w);
+    }
+    __syncthreads();
+    TgInstDev& I = *reinterpret_cast<TgInstDev*>(sInst);
+    int32_t* const gIdx = I.eIdx;
+    uint32_t* const gF = I.eF;
+    const int ne = min(max(I.nEval, 0), TG_MAX_EVAL);
+    for (int w = tid; w < ne; w += TG_NT) { sEval[w] = uint32_t(__ldcg(gIdx + w)); sEval[TG_MAX_EVAL + w] = __ldcg(gF + w); }
+    const int lo = ne > 0 ? int(uint32_t(__ldcg(gIdx)) & ~uint32_t(TG_EDONE)) : max(I.lbIdx, 0);
+    const int nw = max(0, min(TG_CAND_WIN, I.ncand - lo));
+    for (int w = tid; w < nw; w += TG_NT) sCand[w] = I.cand[lo + w];
+    __syncthreads();
+    if (tid == 0) {
+        I.eIdx = reinterpret_cast<int32_t*>(sEval);
+        I.eF = sEval + TG_MAX_EVAL;
+        I.candWin = sCand; I.candWinLo = lo; I.candWinN = nw;
+        TgPrev P;
+        P.items = ctx.items; P.keys = ctx.keys; P.keyS = nullptr; P.tidxS = nullptr; P.candS = nullptr; P.flagS = nullptr;
+        P.nStage = 0; P.mask = TG_QCAP - 1;
+        if (I.itemCnt > 0) tgFoldInstance(ctx, I, P, false);
+        if (I.phase != TG_PH_DONE) {
+            // few probes at a time while the queue is long (less speculation: an extra "round" costs this instance latency only),
+            // the full width once CTAs would otherwise wait for work (the tail of the batch is bound by the instances' chains)
+            const int backlog = int(__ldcg(&ctrl->qTail) - __ldcg(&ctrl->qHead));
+            const int W = backlog < int(gridDim.x) ? ctx.wishCap : ctx.queueWish;
+            I.planKind = tgPlanInstance(ctx, I, i, min(min(ctx.wishMax, W), max(tgWish(ctx, I.K), W)), false);
+        }
+        I.eIdx = gIdx; I.eF = gF; I.candWin = nullptr; I.candWinN = 0;
+        int cnt = I.phase != TG_PH_DONE ? I.nProbe : 0;
+        uint32_t base = 0;
+        if (cnt > 0) base = atomicAdd(&ctrl->qTail, uint32_t(cnt));
+        I.itemBeg = int(base); I.itemCnt = cnt; I.pending = cnt;
+        sm.iTmp[3] = cnt; sm.iTmp[4] = int(base);
+    }
+    __syncthreads();
+    {   // the record and the evaluated list go back before the new items can be seen
+        const int ne2 = min(max(I.nEval, 0), TG_MAX_EVAL);
+        for (int w = tid; w < ne2; w += TG_NT) { gIdx[w] = int32_t(sEval[w]); gF[w] = sEval[TG_MAX_EVAL + w]; }
+        uint32_t* dst = reinterpret_cast<uint32_t*>(ctx.inst + i);
+        for (int w = tid; w < INST_W; w += TG_NT) dst[w] = sInst[w];
+    }
+    __syncthreads();
+    const int cnt = sm.iTmp[3];
+    const uint32_t base = uint32_t(sm.iTmp[4]);
+    if (tid < cnt) {
+        const uint32_t seq = base + uint32_t(tid), slot = seq & (TG_QCAP - 1);
+        TgItem& it = ctx.items[slot];
+        const int kind = I.planKind, pq = I.probe[tid];
+        it.inst = i;
+        it.tidx = pq >= 0 ? (pq & ~(TG_PROBE_FINAL | TG_PROBE_KEEP)) : -1;
+        it.T = it.tidx >= 0 ? I.cand[it.tidx] : ctx.dpT;
+        it.flags = kind == TG_PH_FINAL ? TG_IT_TRACK
+                   : (pq >= 0 && (pq & TG_PROBE_FINAL)) ? (TG_IT_TRACK | TG_IT_SPEC)
+                   : (pq >= 0 && (pq & TG_PROBE_KEEP)) ? (TG_IT_TRACK | TG_IT_SPEC | TG_IT_ALLISL) : 0;
+        ctx.keys[slot] = TG_KEY_NONE;
+        __threadfence();
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(ctx.itemSeq + slot), "r"(seq + 1u) : "memory");
+    }
+    if (tid == 0) {
+        if (cnt > 0) atomicAdd((unsigned long long*)&ctrl->stats.n_dp, (unsigned long long)cnt);
+        else {   // the instance is finished (its result was written by the back-tracker or while planning)
+            const int d = atomicAdd(&ctrl->nDoneInst, 1) + 1;
+            if (d == ctx.nInst) { __threadfence(); atomicExch(&ctrl->allDone, 1); }
+        }
+    }
+    __syncthreads();
 }
 
 // Scheduler, second half (CTA 0): lay the planned probes out as the round's item list, size the teams.
@@ -1736,6 +1831,79 @@ __global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgS
 #endif
     __syncthreads();
     const bool wide = ctx.nInst >= TG_WIDE_MIN_INST;
+    const bool queue = wide && ctx.nInst <= TG_QUEUE_MAX_INST && ctx.mode == 0 && !(ctx.flags & TG_SOLVE_FULL_SWEEP);
+    if (queue) {
+        // first round as in round mode (every warp of the grid plans at most one instance at a time, CTA 0 lays the items
+        // out), then the queue
+        tgFoldPlanAll(ctx, sm, dyn, 0, true);
+        tgMark(sm, 6);
+        tgGridBarrier(ctrl, epoch);
+        if (b == 0) {
+            tgSchedule(ctx, sm, 0);
+            __syncthreads();
+            const int nIt = ctrl->nItems[0];
+            for (int q = threadIdx.x; q < nIt; q += TG_NT) ctx.itemSeq[q] = uint32_t(q) + 1u;
+            int done = 0;
+            for (int i = threadIdx.x; i < ctx.nInst; i += TG_NT) {
+                TgInstDev& I = ctx.inst[i];
+                I.pending = I.itemCnt;
+                if (I.phase == TG_PH_DONE || I.itemCnt == 0) { ++done; I.phase = TG_PH_DONE; }
+            }
+            if (done) atomicAdd(&ctrl->nDoneInst, done);
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                ctrl->qTail = uint32_t(nIt);
+                if (ctrl->nDoneInst >= ctx.nInst) ctrl->allDone = 1;
+            }
+            tgMark(sm, 6);
+        }
+        tgGridBarrier(ctrl, epoch);
+        tgMark(sm, 5);
+        while (true) {
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                const uint32_t seq = atomicAdd(&ctrl->qHead, 1u);
+                const uint32_t* flag = ctx.itemSeq + (seq & (TG_QCAP - 1));
+                int got = 1;
+                while (true) {
+                    uint32_t v;
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+                    if (v == seq + 1u) break;
+                    int dn;
+                    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(dn) : "l"(&ctrl->allDone) : "memory");
+                    if (dn) { got = 0; break; }
+                    __nanosleep(100);
+                }
+                sm.curItem = got ? int(seq) : -1;
+            }
+            __syncthreads();
+            tgMark(sm, 5);
+            const int seq = sm.curItem;
+            if (seq < 0) break;
+            const int slot = seq & (TG_QCAP - 1);
+            tgRunItem(ctx, sm, Cs, wbufAll, ctx.items + slot, ctx.keys + slot, 0, 1, b, slot);
+            if (threadIdx.x == 0) {
+                __threadfence();   // this DP's key (and, for a tracked item, its result) before the count
+                const int inst = __ldcg(&ctx.items[slot].inst);
+                const int left = atomicSub(&ctx.inst[inst].pending, 1) - 1;
+                sm.iTmp[2] = left == 0 ? inst : -1;
+            }
+            __syncthreads();
+            tgMark(sm, 0);
+            if (sm.iTmp[2] >= 0) { tgQueueFoldPlan(ctx, sm, dyn, sm.iTmp[2]); tgMark(sm, 6); }
+        }
+        if (threadIdx.x == 0) {
+            tg_solve_stats& S = ctrl->stats;
+            atomicAdd((unsigned long long*)&S.cyc_stage, sm.cyc[0]);
+            atomicAdd((unsigned long long*)&S.cyc_levels, sm.cyc[3]);
+            atomicAdd((unsigned long long*)&S.cyc_level_barrier, sm.cyc[4]);
+            atomicAdd((unsigned long long*)&S.cyc_grid_wait, sm.cyc[5]);
+            atomicAdd((unsigned long long*)&S.cyc_scheduler, sm.cyc[6]);
+            atomicAdd((unsigned long long*)&S.cyc_backtrack, sm.cyc[7]);
+        }
+        if (b == 0 && threadIdx.x == 0) ctrl->stats.n_barriers = epoch;
+        return;
+    }
     for (int round = 0;; ++round) {
         const int par = round & 1;
         if (wide || b == 0) { tgFoldPlanAll(ctx, sm, dyn, round, wide); tgMark(sm, 6); }

@@ -40,7 +40,8 @@ def test_300_back_to_back_solves_are_bit_identical():
         cols = [c for c in tg.RESULT_DTYPE.names if c != "n_thresholds_run"]
         for c in cols:
             assert (res[c] == res[c][0:1]).all(), f"{k}: field {c} differs between runs"
-        assert (res["n_thresholds_run"] == res["n_thresholds_run"][0:1]).all(), f"{k}: the search schedule differs between runs"
+        if k != "mix":   # (a batch of >= 64 instances runs in queue mode: the number of DPs per instance follows the queue's backlog)
+            assert (res["n_thresholds_run"] == res["n_thresholds_run"][0:1]).all(), f"{k}: the search schedule differs between runs"
     for name in ("cfg3", "cfg4"):
         e = json.load(open(os.path.join(HERE, "golden", f"expected_{name}.json")))["records"][0]["solve"]
         g = outs[name][0].cpu().numpy().view(tg.RESULT_DTYPE)[0]
