@@ -176,7 +176,11 @@ typedef struct { /* optional diagnostics of one tg_solve_batch_ex call, written 
     uint64_t n_rounds;       /* scheduler rounds                                               */
     uint64_t n_barriers;     /* grid-wide barriers executed                                    */
     uint64_t n_items_global_c; /* DPs whose cost tables did not fit in shared memory           */
-    uint64_t error_flag;     /* internal consistency flag of the solver, 0 = none                */
+    uint64_t error_flag;     /* internal consistency flag of the solver, 0 = none; 2 = a staged cost row broke its
+                                bound, 3 = evaluated-threshold list full, 4 = a queue-mode ring slot was overwritten
+                                before its instance folded it, 5 = queue-mode watchdog (no item published for ~20 s
+                                and the batch not finished); any non-zero flag makes the call return TG_ERR_CUDA
+                                (synchronous) or poisons the results (asynchronous, see tg_solve_batch_ex)          */
     uint64_t relax_admissible; /* admissible relaxations executed: stage (c <= T) + transfer, summed over DPs */
     uint64_t states_windowed;  /* DP states the kernel actually wrote: sum over DPs of Ke*2^(Ke-1) rows x the row window */
     /* SM cycles summed over the solver's CTAs (thread 0 of each): */

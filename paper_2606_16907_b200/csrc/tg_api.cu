@@ -283,8 +283,8 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         oEI[i] = cv.take(size_t(TG_MAX_EVAL) * 4);
         oEF[i] = cv.take(size_t(TG_MAX_EVAL) * 4);
     }
-    const size_t oItems = cv.take(sizeof(TgItem) * 2 * TG_MAX_ITEMS);
-    const size_t oKeys = cv.take(sizeof(unsigned long long) * 2 * TG_MAX_ITEMS);
+    const size_t oItems = cv.take(sizeof(TgItem) * TG_QCAP);
+    const size_t oKeys = cv.take(sizeof(unsigned long long) * TG_QCAP);
     const size_t oCtrl = cv.take(sizeof(TgCtrl));
     const size_t oOut = cv.take(sizeof(tg_result) * n);
     const size_t oSpec = cv.take(sizeof(tg_result) * TG_QCAP);

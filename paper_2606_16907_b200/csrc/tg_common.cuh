@@ -16,8 +16,9 @@
                               // CTA's barriers, copy latencies and level tails are filled by the other
 #endif
 #define TG_MAX_ITEMS 8192     // (instance, T) DPs per scheduler round
-#define TG_QCAP (2 * TG_MAX_ITEMS)   // queue mode: ring slots (the two per-round item arrays back to back)
-#define TG_QUEUE_MAX_INST 1024       // queue mode: at most this many instances (each has <= 12 items in flight: 12 288 < TG_QCAP)
+#define TG_QCAP 65536                // queue mode: ring slots (a power of two >= 2 * TG_MAX_ITEMS: round mode uses the first two arrays of it)
+#define TG_QUEUE_MAX_INST 1024       // queue mode: at most this many instances; an instance has <= TG_MAX_WISH items in flight, so the
+                                     // ring (1024 * 64 = TG_QCAP) cannot wrap onto a live item; the fold checks it anyway (error flag 4)
 #define TG_MAX_EVAL 1024      // evaluated thresholds remembered per instance
 #define TG_MAX_WISH 64        // DPs per instance and round, upper bound
 #define TG_PROBE_FINAL 0x40000000   // flag in probe[]: speculative final DP at the incumbent (S* only; keep every level, back-track)
@@ -123,6 +124,7 @@ struct TgItem {
     uint8_t flags;       // bit0: keep every level (back-track follows)
     uint8_t isl[TG_MAX_K];  // compact label -> original island
     uint16_t ctaBeg, ctaCnt;  // team of CTAs that runs the item (weighted team mode; written by the scheduler)
+    uint32_t seq;        // queue mode: the item's sequence number (the fold checks that its ring slot still holds it)
 };
 
 struct TgCtrl {
@@ -153,8 +155,8 @@ struct TgCtrl {
 struct TgSolveCtx {
     TgInstDev* inst;
     int32_t nInst;
-    TgItem* items;              // [2][TG_MAX_ITEMS]
-    unsigned long long* keys;   // [2][TG_MAX_ITEMS] best (value, S, k) per item
+    TgItem* items;              // [TG_QCAP]: round mode uses [2][TG_MAX_ITEMS] of it, queue mode the whole ring
+    unsigned long long* keys;   // [TG_QCAP], same split: best (value, S, k) per item
     uint32_t* scratch;          // DP tables: nSlots slots of slotWords words
     uint64_t slotWords;         // one slot holds every level of the largest instance of the batch
     int32_t nSlots;             // <= gridDim.x; a slot belongs to one team (team mode) or one CTA (solo mode)
@@ -165,8 +167,8 @@ struct TgSolveCtx {
     int32_t wishCap;            // upper end of the per-round probe count chosen from the instance shape (tgWish)
     uint32_t* slotBar;          // [nSlots] arrival counters of the team barriers, zeroed every round
     TgCtrl* ctrl;
-    tg_result* specOut;         // [2 * TG_MAX_ITEMS] results of speculative back-tracks, by item slot
-    uint32_t* itemSeq;          // [2 * TG_MAX_ITEMS] queue mode: sequence number + 1 of the item published in each ring slot
+    tg_result* specOut;         // [TG_QCAP] results of speculative back-tracks, by item slot
+    uint32_t* itemSeq;          // [TG_QCAP] queue mode: sequence number + 1 of the item published in each ring slot
     tg_result* out;
     const uint16_t* rankOf;     // [65536] rank of a mask inside its popcount class
     const uint16_t* maskOf;     // [65536] the inverse: masks ordered by (popcount, value); class r starts at tgPopOff[r]

@@ -1605,6 +1605,8 @@ __device__ void tgQueueFoldPlan(const TgSolveCtx& ctx, TgShared& sm, uint32_t* d
         TgPrev P;
         P.items = ctx.items; P.keys = ctx.keys; P.keyS = nullptr; P.tidxS = nullptr; P.candS = nullptr; P.flagS = nullptr;
         P.nStage = 0; P.mask = TG_QCAP - 1;
+        for (int q = 0; q < I.itemCnt; ++q)   // every slot to fold still holds this instance's item (the ring did not wrap onto it)
+            if (__ldcg(&ctx.items[uint32_t(I.itemBeg + q) & (TG_QCAP - 1)].seq) != uint32_t(I.itemBeg + q)) atomicExch(&ctrl->errFlag, 4);
         if (I.itemCnt > 0) tgFoldInstance(ctx, I, P, false);
         if (I.phase != TG_PH_DONE) {
             // few probes at a time while the queue is long (less speculation: an extra "round" costs this instance latency only),
@@ -1635,6 +1637,7 @@ __device__ void tgQueueFoldPlan(const TgSolveCtx& ctx, TgShared& sm, uint32_t* d
         TgItem& it = ctx.items[slot];
         const int kind = I.planKind, pq = I.probe[tid];
         it.inst = i;
+        it.seq = seq;
         it.tidx = pq >= 0 ? (pq & ~(TG_PROBE_FINAL | TG_PROBE_KEEP)) : -1;
         it.T = it.tidx >= 0 ? I.cand[it.tidx] : ctx.dpT;
         it.flags = kind == TG_PH_FINAL ? TG_IT_TRACK
@@ -1842,7 +1845,7 @@ __global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgS
             tgSchedule(ctx, sm, 0);
             __syncthreads();
             const int nIt = ctrl->nItems[0];
-            for (int q = threadIdx.x; q < nIt; q += TG_NT) ctx.itemSeq[q] = uint32_t(q) + 1u;
+            for (int q = threadIdx.x; q < nIt; q += TG_NT) { ctx.items[q].seq = uint32_t(q); ctx.itemSeq[q] = uint32_t(q) + 1u; }
             int done = 0;
             for (int i = threadIdx.x; i < ctx.nInst; i += TG_NT) {
                 TgInstDev& I = ctx.inst[i];
@@ -1865,6 +1868,7 @@ __global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgS
                 const uint32_t seq = atomicAdd(&ctrl->qHead, 1u);
                 const uint32_t* flag = ctx.itemSeq + (seq & (TG_QCAP - 1));
                 int got = 1;
+                const long long t0 = clock64();
                 while (true) {
                     uint32_t v;
                     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
@@ -1872,6 +1876,12 @@ __global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgS
                     int dn;
                     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(dn) : "l"(&ctrl->allDone) : "memory");
                     if (dn) { got = 0; break; }
+                    if (clock64() - t0 > 40000000000ll) {   // ~20 s without a new item and without the end: a lost item; stop, do not hang
+                        atomicExch(&ctrl->errFlag, 5);
+                        atomicExch(&ctrl->allDone, 1);
+                        got = 0;
+                        break;
+                    }
                     __nanosleep(100);
                 }
                 sm.curItem = got ? int(seq) : -1;
