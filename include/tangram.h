@@ -245,6 +245,23 @@ tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int
 tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode mode, int64_t threshold,
                          int64_t* counts_out, void* cuda_stream);
 
+/* tg_prune_batch_static — tg_prune_batch for callers that cannot allocate device memory (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): same kernels, same results, but the pass's scratch
+ * (per-rule counters, R3 caps, instance descriptors) lives in one file-scope device array of the library, 216 KB, that
+ * every GPU which loads the library holds until exit.  The call allocates and frees nothing on the device -- no
+ * cudaMalloc / cudaMallocAsync / cudaFree, no pool -- and does not need the library's per-device set-up.
+ *   n           in [0, TG_PRUNE_STATIC_MAX_N]; more -> TG_ERR_SHAPE (the message names the limit; use tg_prune_batch)
+ *   instances   as tg_prune_batch, but an instance that still keeps class tables (tg_instance_create_classes, never
+ *               pruned or given a variant table) -> TG_ERR_SHAPE: pruning it would have to free those tables
+ *   counts_out  HOST int64 [n][4]; the call synchronises `cuda_stream`
+ * Every call shares the one array, which keeps the previous call's contents; the call clears what must start at zero.
+ * Calls from threads of one process are serialised inside the library; two calls that overlap on the GPU some other
+ * way (two processes cannot: each has its own copy) would race on it.  Argument errors are reported before anything
+ * is modified. */
+#define TG_PRUNE_STATIC_MAX_N 1024
+tg_status tg_prune_batch_static(tg_instance* const* instances, int32_t n, tg_prune_mode mode, int64_t threshold,
+                                int64_t* counts_out, void* cuda_stream);
+
 /* ---- step-level entry points (used by the parity tests to check single steps) ---------------- */
 
 /* Steps 1-3 alone: reduced tables and candidate thresholds.  All outputs HOST, any may be NULL.

@@ -65,7 +65,7 @@ class TangramError(RuntimeError):
 
 
 _lib = None
-EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_set_boundary_act", "tg_instance_set_stages", "tg_plan_pipeline_stages", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch",
+EXPORTS = ["tg_instance_create", "tg_instance_create_classes", "tg_instance_create_batch", "tg_instance_set_actmem", "tg_instance_set_transfer_bound", "tg_instance_set_boundary_act", "tg_instance_set_stages", "tg_plan_pipeline_stages", "tg_instance_destroy", "tg_solve_batch", "tg_solve_batch_ex", "tg_prune", "tg_prune_batch", "tg_prune_batch_static",
            "tg_reduce", "tg_candidates", "tg_dp_at", "tg_instance_read_time", "tg_islands_build", "tg_release_cached_memory", "tg_last_solver_kernel_ms", "tg_last_loader_kernel_ms", "tg_last_error", "tg_version"]
 
 
@@ -94,6 +94,7 @@ def lib():
         L.tg_solve_batch_ex.argtypes = [C.POINTER(vp), i32, vp, u32, vp, vp]
         L.tg_prune.argtypes = [vp, C.c_int, i64, C.POINTER(i64), vp]
         L.tg_prune_batch.argtypes = [C.POINTER(vp), i32, C.c_int, i64, C.POINTER(i64), vp]
+        L.tg_prune_batch_static.argtypes = [C.POINTER(vp), i32, C.c_int, i64, C.POINTER(i64), vp]
         L.tg_reduce.argtypes = [vp, vp, vp, vp, vp, C.POINTER(i32), vp]
         L.tg_candidates.argtypes = [vp, vp, i64, C.POINTER(i32), vp]
         L.tg_dp_at.argtypes = [vp, i64, vp, vp]
@@ -309,6 +310,18 @@ def tg_prune_batch(instances, mode: int = TG_PRUNE_EXACT, threshold: int = 0, st
     n = len(instances)
     counts = (C.c_int64 * (4 * max(n, 1)))()
     _check(lib().tg_prune_batch(_handles(instances), n, mode, threshold, counts, _stream_ptr(stream)))
+    return np.array(list(counts), dtype=np.int64)[:4 * n].reshape(n, 4)
+
+
+TG_PRUNE_STATIC_MAX_N = 1024
+
+
+def tg_prune_batch_static(instances, mode: int = TG_PRUNE_EXACT, threshold: int = 0, stream=None) -> np.ndarray:
+    """tg_prune_batch without any device allocation: scratch in the library's file-scope device array; at most
+    TG_PRUNE_STATIC_MAX_N instances.  Returns counts [n, 4]."""
+    n = len(instances)
+    counts = (C.c_int64 * (4 * max(n, 1)))()
+    _check(lib().tg_prune_batch_static(_handles(instances), n, mode, threshold, counts, _stream_ptr(stream)))
     return np.array(list(counts), dtype=np.int64)[:4 * n].reshape(n, 4)
 
 

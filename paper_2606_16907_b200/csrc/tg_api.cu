@@ -1041,6 +1041,102 @@ tg_status tg_prune(tg_instance* inst, tg_prune_mode mode, int64_t threshold, int
     return tg_prune_batch(&inst, 1, mode, threshold, counts_out, cuda_stream);
 }
 
+// ---------------------------------------------------------------------------------------------
+// tg_prune_batch_static: tg_prune_batch for callers that must not allocate device memory (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid cudaMalloc).  The pass's scratch -- the per-rule counters, the R3 caps and
+// the instance descriptors the kernels read -- lives in ONE file-scope device array of fixed size; every GPU that loads
+// the library holds it until exit.  The kernels are the ones tg_prune_batch launches, unchanged.
+// ---------------------------------------------------------------------------------------------
+constexpr size_t TG_PS_COUNTS = size_t(TG_PRUNE_STATIC_MAX_N) * 32;                       // [n][4] unsigned long long
+constexpr size_t TG_PS_CAP = size_t(TG_PRUNE_STATIC_MAX_N) * (TG_MAX_K + 1) * 8;          // [n][TG_MAX_K + 1] long long (R3)
+constexpr size_t TG_PS_DESC = size_t(TG_PRUNE_STATIC_MAX_N) * sizeof(TgPruneDesc);
+constexpr size_t TG_PS_BYTES = TG_PS_COUNTS + TG_PS_CAP + TG_PS_DESC;                     // 221 184 bytes
+static_assert(TG_PS_COUNTS % 256 == 0 && TG_PS_CAP % 256 == 0, "parts of the static scratch keep the 256-byte alignment");
+static_assert(TG_PS_BYTES <= (256u << 10), "static prune scratch: stated maximum is 256 KB");
+static __device__ __align__(256) unsigned char tgPruneStaticScratch[TG_PS_BYTES];
+
+struct StaticPruneState {
+    bool ready = false;
+    unsigned char* scratch = nullptr;   // DEVICE address of tgPruneStaticScratch on this device (the symbol itself is a host-side stand-in)
+    int numSMs = 0;
+};
+StaticPruneState g_staticPrune[64];
+std::mutex g_staticPruneMu;   // set-up, and the host-side descriptor staging below
+
+tg_status tg_prune_batch_static(tg_instance* const* instances, int32_t n, tg_prune_mode mode, int64_t threshold, int64_t* counts_out,
+                                void* cuda_stream) {
+    if (n == 0) return TG_OK;
+    if (!instances || !counts_out) return fail(TG_ERR_NULL, "NULL argument");
+    if (n < 0 || n > TG_PRUNE_STATIC_MAX_N)
+        return fail(TG_ERR_SHAPE, "tg_prune_batch_static: n = " + std::to_string(n) + " outside [0, TG_PRUNE_STATIC_MAX_N = " +
+                                      std::to_string(TG_PRUNE_STATIC_MAX_N) + "]: the static scratch holds no more; use tg_prune_batch");
+    if (mode != TG_PRUNE_EXACT && mode != TG_PRUNE_IMBALANCE && mode != TG_PRUNE_BOTTLENECK)
+        return fail(TG_ERR_RANGE, "unknown prune mode");
+    if (mode == TG_PRUNE_IMBALANCE && (threshold < 1000 || threshold > 16384))
+        return fail(TG_ERR_RANGE, "theta must be in [1000, 16384] permille");
+    if (mode == TG_PRUNE_BOTTLENECK && threshold < 0) return fail(TG_ERR_RANGE, "bottleneck cap must be >= 0");
+    int dev = 0;
+    TG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return fail(TG_ERR_CUDA, "device ordinal out of range");
+    std::lock_guard<std::mutex> lk(g_staticPruneMu);
+    static TgPruneDesc h[TG_PRUNE_STATIC_MAX_N];            // host staging, fixed size (under the mutex)
+    static const tg_instance* seen[TG_PRUNE_STATIC_MAX_N];
+    int maxCells = 0;
+    bool act = false;
+    for (int i = 0; i < n; ++i) {
+        tg_instance* t = instances[i];
+        if (!t) return fail(TG_ERR_NULL, "instances[" + std::to_string(i) + "] is NULL");
+        if (t->device != dev) return fail(TG_ERR_CUDA, "instance was created on another device");
+        if (t->slow) return fail(TG_ERR_SHAPE, "instances[" + std::to_string(i) + "] has multi-stage partial plans: tg_prune is not built for them");
+        if (t->cls) return fail(TG_ERR_SHAPE, "instances[" + std::to_string(i) + "] keeps class tables: pruning would have to free them; use tg_prune_batch");
+        h[i] = TgPruneDesc{t->time_us, t->mem_mb, t->actmem, t->cap_mb, t->L, t->K, t->P, t->NS * t->K};
+        maxCells = std::max(maxCells, h[i].nCells);
+        act = act || t->actmem != nullptr;
+        seen[i] = t;
+    }
+    std::sort(seen, seen + n);
+    if (std::adjacent_find(seen, seen + n) != seen + n) return fail(TG_ERR_RANGE, "an instance appears twice in the batch");
+    StaticPruneState& S = g_staticPrune[dev];
+    if (!S.ready) {   // once per device, with that device current: the array's device address; nothing is allocated
+        void* ptr = nullptr;
+        TG_CUDA(cudaGetSymbolAddress(&ptr, tgPruneStaticScratch));
+        if (!ptr) return fail(TG_ERR_CUDA, "cudaGetSymbolAddress returned NULL for the static scratch");
+        TG_CUDA(cudaDeviceGetAttribute(&S.numSMs, cudaDevAttrMultiProcessorCount, dev));
+        S.scratch = static_cast<unsigned char*>(ptr);
+        S.ready = true;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned long long* dCounts = reinterpret_cast<unsigned long long*>(S.scratch);
+    long long* dCap = reinterpret_cast<long long*>(S.scratch + TG_PS_COUNTS);
+    TgPruneDesc* dDesc = reinterpret_cast<TgPruneDesc*>(S.scratch + TG_PS_COUNTS + TG_PS_CAP);
+    // the array keeps the last call's contents: counters and caps start at zero, the descriptors are overwritten
+    TG_CUDA(cudaMemsetAsync(S.scratch, 0, TG_PS_COUNTS + TG_PS_CAP, st));
+    TG_CUDA(cudaMemcpyAsync(dDesc, h, sizeof(TgPruneDesc) * size_t(n), cudaMemcpyHostToDevice, st));
+    const dim3 g((maxCells + 255) / 256, n), g2((maxCells + 511) / 512, n);
+    const bool wide = int64_t(g2.x) * n >= 4 * S.numSMs;
+    const int P0 = instances[0]->P;
+#define TG_PRUNE_LAUNCH(PV, U, G) \
+    do { if (act) tgPruneCellKernel<PV, U, true><<<G, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts); \
+         else tgPruneCellKernel<PV, U, false><<<G, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts); } while (0)
+    if (P0 == 4) {
+        if (wide) TG_PRUNE_LAUNCH(1, 2, g2); else TG_PRUNE_LAUNCH(1, 1, g);
+    } else if (P0 == 8) {
+        if (wide) TG_PRUNE_LAUNCH(2, 2, g2); else TG_PRUNE_LAUNCH(2, 1, g);
+    } else {
+        TG_PRUNE_LAUNCH(0, 1, g);
+    }
+#undef TG_PRUNE_LAUNCH
+    if (mode == TG_PRUNE_IMBALANCE) {
+        tgPruneTauKernel<<<n, 256, 0, st>>>(dDesc, dCap);
+        tgPruneImbalanceKernel<<<g, 256, 0, st>>>(dDesc, dCap, threshold, dCounts);
+    }
+    TG_CUDA(cudaGetLastError());
+    static_assert(sizeof(unsigned long long) == sizeof(int64_t), "counts are copied as they are");
+    TG_CUDA(cudaMemcpyAsync(counts_out, dCounts, size_t(n) * 32, cudaMemcpyDeviceToHost, st));
+    TG_CUDA(cudaStreamSynchronize(st));   // counts_out is valid; the host staging and the scratch are free for the next call
+    return TG_OK;
+}
+
 tg_status tg_islands_build(int32_t n_nodes, const int32_t* node_gpus, const int32_t* node_compute, const int32_t* node_mem_mb,
                            const int32_t* node_intra_bw, const int32_t* inter_bw, int32_t eps_c, int32_t eps_m, int32_t eps_i,
                            int32_t* island_of_node, int32_t* k_out, int32_t* island_gpus, int32_t* island_cap_mb, int32_t* bw_gbps) {
