@@ -656,37 +656,37 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
     const int lo = int((int64_t(nMasks) * member) / teamSize), hi = int((int64_t(nMasks) * (member + 1)) / teamSize);
     if (lo >= hi) return;
     const int HS = tgRowStride(Wd), SS = tgSrcStride(Wd);
-    if (tid == 0) {
-        // split of the shared memory behind the cost rows for this level
+    // split of the shared memory behind the cost rows for this level: computed by every thread (a few dozen instructions)
+    // rather than by one thread and a CTA barrier; the island counts are zero on entry (cleared at the start of the item
+    // and by cursors() for every batch that was counted)
+    int NB, nsl, nsg;
+    uint32_t oDesc[2], oSrcRow[2], oList, oH, oSrc[2];
+    {
         const int avail = ctx.dynWords - sm.batchOff;
         const int perMask = nk * HS + 2 * r * SS + 2 * TG_DESC_W + 2 * r + 2 * nk;
-        const int NB = min(min(TG_NB_MAX, hi - lo), max(1, (avail - 32) / perMask));
+        NB = min(min(TG_NB_MAX, hi - lo), max(1, (avail - 32) / perMask));
         // phase-1 items take NSL rows each: fewest CTA passes x instructions per item
         int best = 1, bestCost = 0x7fffffff;
-        for (int nsl = 1; nsl <= (sm.sNAct ? 4 : TG_SPL); nsl <<= 1) {
-            const int items = NB * nbw * ((nk + nsl - 1) / nsl);
-            const int cost = ((items + TG_NT - 1) / TG_NT) * (3 + 5 * nsl);
-            if (cost < bestCost) { bestCost = cost; best = nsl; }
+        for (int q = 1; q <= (sm.sNAct ? 4 : TG_SPL); q <<= 1) {
+            const int items = NB * nbw * ((nk + q - 1) / q);
+            const int cost = ((items + TG_NT - 1) / TG_NT) * (3 + 5 * q);
+            if (cost < bestCost) { bestCost = cost; best = q; }
         }
-        sm.lvNB = NB; sm.lvNsl = best; sm.lvNsg = (nk + best - 1) / best;
-        sm.lvMagic[0] = tgMagic(uint32_t(nbw)); sm.lvMagic[1] = tgMagic(uint32_t(sm.lvNsg));
+        nsl = best; nsg = (nk + best - 1) / best;
         uint32_t o = uint32_t(sm.batchOff);
-        for (int b = 0; b < 2; ++b) { sm.lvDesc[b] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3); }
-        for (int b = 0; b < 2; ++b) { sm.lvSrcRow[b] = o; o += uint32_t((NB * r + 3) & ~3); }
-        sm.lvList = o; o += uint32_t((2 * nk * NB + 3) & ~3);
-        sm.lvH = o; o += uint32_t(NB * nk * HS);
-        sm.lvSrc[0] = o; o += uint32_t(NB * r * SS);
-        sm.lvSrc[1] = o;
+        for (int b = 0; b < 2; ++b) { oDesc[b] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3); }
+        for (int b = 0; b < 2; ++b) { oSrcRow[b] = o; o += uint32_t((NB * r + 3) & ~3); }
+        oList = o; o += uint32_t((2 * nk * NB + 3) & ~3);
+        oH = o; o += uint32_t(NB * nk * HS);
+        oSrc[0] = o; o += uint32_t(NB * r * SS);
+        oSrc[1] = o;
     }
-    if (tid < 2 * TG_MAX_K) (&sm.cntP[0][0])[tid] = 0;
-    __syncthreads();
-    const int NB = sm.lvNB, nsl = sm.lvNsl, nsg = sm.lvNsg;
-    const uint32_t mNbw = sm.lvMagic[0], mNsg = sm.lvMagic[1];
-    uint32_t* const descB[2] = {dyn + sm.lvDesc[0], dyn + sm.lvDesc[1]};
-    uint32_t* const srcRowB[2] = {dyn + sm.lvSrcRow[0], dyn + sm.lvSrcRow[1]};
-    uint2* const list = reinterpret_cast<uint2*>(dyn + sm.lvList);
-    const uint32_t hAddr = tgSmemAddr(dyn + sm.lvH);
-    const uint32_t srcAddr[2] = {tgSmemAddr(dyn + sm.lvSrc[0]), tgSmemAddr(dyn + sm.lvSrc[1])};
+    const uint32_t mNbw = tgMagic(uint32_t(nbw)), mNsg = tgMagic(uint32_t(nsg));
+    uint32_t* const descB[2] = {dyn + oDesc[0], dyn + oDesc[1]};
+    uint32_t* const srcRowB[2] = {dyn + oSrcRow[0], dyn + oSrcRow[1]};
+    uint2* const list = reinterpret_cast<uint2*>(dyn + oList);
+    const uint32_t hAddr = tgSmemAddr(dyn + oH);
+    const uint32_t srcAddr[2] = {tgSmemAddr(dyn + oSrc[0]), tgSmemAddr(dyn + oSrc[1])};
     const uint32_t HSB = uint32_t(HS) * 4u, SSB = uint32_t(SS) * 4u, cStride = uint32_t(Lp) * 4u;
     const bool actb = TG_VAR && sm.sNAct > 0;
     const uint32_t csBase = tgSmemAddr(dyn), xInfAddr = tgSmemAddr(&sm.xInf[0]);
@@ -710,11 +710,10 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
             if (tid < TG_MAX_K) { sm.cur[par][tid] = inc - c; sm.cntP[par][tid] = 0; }
         }
     };
-    for (int pass = 0; pass <= (NB - 1) / TG_NT; ++pass)   // (NB <= TG_NT unless the CTA is built with fewer than 256 threads)
-        for (int b = 0; b < 2 && b < nBatches; ++b) {
-            const int m0 = lo + b * NB, i = pi + pass * TG_NT;
-            if (i < min(NB, hi - m0)) tgPrepassMask(ctx, sm, descB[b] + i * TG_DESC_W, srcRowB[b] + i * r, sm.cntP[b], uint32_t(m0 + i), r, Ke);
-        }
+    for (int j = pi; j < 2 * NB; j += TG_NT) {   // the first two batches side by side: one mask a thread
+        const int b = j >= NB ? 1 : 0, i = j - b * NB, m0 = lo + b * NB;
+        if (i < hi - m0) tgPrepassMask(ctx, sm, descB[b] + i * TG_DESC_W, srcRowB[b] + i * r, sm.cntP[b], uint32_t(m0 + i), r, Ke);
+    }
     __syncthreads();
     cursors(0);
     tgIssueBatch(srcRowB[0], srcAddr[0], Gprev, min(NB, hi - lo), r, Wd, nbw, mNbw, SSB);
@@ -1155,6 +1154,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     uint32_t* bar = ctx.slotBar + slotIdx;
     uint32_t arrivals = 0;
     if (Ke > 0) {
+        if (threadIdx.x < 2 * TG_MAX_K) (&sm.cntP[0][0])[threadIdx.x] = 0;   // island counts of the batched levels: zero at every level's entry
         tgLevel0(ctx, sm, slot, key, member == 0);
         __syncthreads();
         for (int r = 1; r < Ke; ++r) {
