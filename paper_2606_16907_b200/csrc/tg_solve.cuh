@@ -436,7 +436,10 @@ __device__ __forceinline__ void tgSts4(uint32_t addr, uint4 v) {
 }
 
 // division of small numbers by a CTA-uniform divisor d: q = t / d for t * d < 2^32 (magic = ceil(2^32 / d), 0 for d = 1)
-__device__ __forceinline__ uint32_t tgMagic(uint32_t d) { return d <= 1u ? 0u : 0xffffffffu / d + 1u; }
+// (divisors up to 32 -- chunks of a row window, row groups of a mask -- come from a constant table: a 32-bit division is a
+// dependent chain of ~70 instructions, and the level geometry below sits on every level's critical path)
+__constant__ uint32_t tgMagicTab[33] = {0u, 0u, 2147483648u, 1431655766u, 1073741824u, 858993460u, 715827883u, 613566757u, 536870912u, 477218589u, 429496730u, 390451573u, 357913942u, 330382100u, 306783379u, 286331154u, 268435456u, 252645136u, 238609295u, 226050911u, 214748365u, 204522253u, 195225787u, 186737709u, 178956971u, 171798692u, 165191050u, 159072863u, 153391690u, 148102321u, 143165577u, 138547333u, 134217728u};
+__device__ __forceinline__ uint32_t tgMagic(uint32_t d) { return d <= 32u ? tgMagicTab[d] : 0xffffffffu / d + 1u; }
 __device__ __forceinline__ uint32_t tgDivM(uint32_t t, uint32_t magic) { return magic ? __umulhi(t, magic) : t; }
 
 // prepass of one mask: descriptor from the mask's rank inside level r, the rows of its r sources in level r-1 and one
@@ -664,15 +667,21 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
     {
         const int avail = ctx.dynWords - sm.batchOff;
         const int perMask = nk * HS + 2 * r * SS + 2 * TG_DESC_W + 2 * r + 2 * nk;
-        NB = min(min(TG_NB_MAX, hi - lo), max(1, (avail - 32) / perMask));
+        // (floor of the quotient through a float reciprocal rounded down, then corrected: no integer division)
+        int fit = int(float(max(avail - 32, 0)) * __frcp_rd(float(perMask)));
+        if ((fit + 1) * perMask <= avail - 32) ++fit;
+        if (fit * perMask > avail - 32) --fit;
+        NB = min(min(TG_NB_MAX, hi - lo), max(1, fit));
         // phase-1 items take NSL rows each: fewest CTA passes x instructions per item
-        int best = 1, bestCost = 0x7fffffff;
-        for (int q = 1; q <= (sm.sNAct ? 4 : TG_SPL); q <<= 1) {
-            const int items = NB * nbw * ((nk + q - 1) / q);
-            const int cost = ((items + TG_NT - 1) / TG_NT) * (3 + 5 * q);
-            if (cost < bestCost) { bestCost = cost; best = q; }
+        int best = 0, bestCost = 0x7fffffff;
+#pragma unroll
+        for (int lq = 0; lq <= 3; ++lq) {   // NSL = 1, 2, 4, 8 (TG_SPL)
+            if ((1 << lq) > (sm.sNAct ? 4 : TG_SPL)) break;
+            const int items = NB * nbw * ((nk + (1 << lq) - 1) >> lq);
+            const int cost = ((items + TG_NT - 1) / TG_NT) * (3 + 5 * (1 << lq));
+            if (cost < bestCost) { bestCost = cost; best = lq; }
         }
-        nsl = best; nsg = (nk + best - 1) / best;
+        nsl = 1 << best; nsg = (nk + nsl - 1) >> best;
         uint32_t o = uint32_t(sm.batchOff);
         for (int b = 0; b < 2; ++b) { oDesc[b] = o; o += uint32_t((NB * TG_DESC_W + 3) & ~3); }
         for (int b = 0; b < 2; ++b) { oSrcRow[b] = o; o += uint32_t((NB * r + 3) & ~3); }
