@@ -452,10 +452,17 @@ __device__ __forceinline__ void tgPrepassMask(const TgSolveCtx& ctx, const TgSha
     uint32_t cap = 0, klLo = 0, klHi = 0;
     int nm = 0, nc = 0;
     const int nk = Ke - r;
-    for (int e = 0; e < Ke; ++e) {
+    // the rank look-ups of all islands are issued together (a non-member's look-up is a valid, unused table entry): one
+    // load latency on the level's critical path instead of r
+    uint16_t rk[TG_MAX_K];
+#pragma unroll
+    for (int e = 0; e < TG_MAX_K; ++e) rk[e] = e < Ke ? __ldg(ctx.rankOf + (R ^ (1u << e))) : uint16_t(0);
+#pragma unroll
+    for (int e = 0; e < TG_MAX_K; ++e) {
+        if (e >= Ke) break;
         if (R >> e & 1u) {
             cap += sm.maxlenK[e];
-            srcRow[nm] = uint32_t(__ldg(ctx.rankOf + (R ^ (1u << e)))) * uint32_t(nk + 1) + uint32_t(e - nm);
+            srcRow[nm] = uint32_t(rk[e]) * uint32_t(nk + 1) + uint32_t(e - nm);
             ++nm;
         } else {
             if (nc < 8) klLo |= uint32_t(e) << (4 * nc); else klHi |= uint32_t(e) << (4 * (nc - 8));
