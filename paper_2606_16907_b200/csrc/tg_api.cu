@@ -340,7 +340,8 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
     W.numCtas = numCtas;
     TG_CUDA(cudaMemcpyAsync(W.inst, h.data(), sizeof(TgInstDev) * n, cudaMemcpyHostToDevice, st));
     TG_CUDA(cudaMemsetAsync(W.base + oCtrl, 0, sizeof(TgCtrl), st));
-    TG_CUDA(cudaMemsetAsync(W.base + oSeq, 0, sizeof(uint32_t) * TG_QCAP, st));
+    if (n >= TG_WIDE_MIN_INST && n <= TG_QUEUE_MAX_INST)   // the publication flags of queue mode (the only mode that reads them)
+        TG_CUDA(cudaMemsetAsync(W.base + oSeq, 0, sizeof(uint32_t) * TG_QCAP, st));
 
     // shared-memory split of the solver: warp-private row buffers (H rows + two source buffers =
     // 2*Kmax rows of Lp+8 words per warp) vs staged cost tables (at least a quarter of the total)

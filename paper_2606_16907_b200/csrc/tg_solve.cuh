@@ -47,9 +47,6 @@ struct TgShared {
     int nWarps, wbufWords, wbufOff;   // team mode: [cost rows | nWarps x wbufWords of warp-private row buffers]
     uint32_t rowOf[TG_NW][2 * TG_MAX_K];   // team mode: source row of each member of the mask being issued (per half warp)
     uint8_t kl[TG_NW][2 * TG_MAX_K];       // team mode: islands not in the current mask, ascending (per half warp)
-    uint32_t lvMagic[2];            // division magics of nbw, lvNsg
-    int lvNB, lvNsl, lvNsg;         // level geometry: masks per batch, rows per phase-1 item, groups of them per mask
-    uint32_t lvDesc[2], lvSrcRow[2], lvList, lvH, lvSrc[2];   // word offsets of the batch buffers
     int cntP[2][TG_MAX_K];          // rows of each island in a batch, counted by its prepass (per batch parity)
     int cur[2][TG_MAX_K];           // next free list position of each island (starts at the prefix of the counts)
     int csUsed4;                    // 16-byte words of the staged cost rows of all islands (incl. the pads between them)
