@@ -1227,6 +1227,18 @@ __device__ __forceinline__ int tgWish(const TgSolveCtx& ctx, int K) {
 // could candidate c, whose sum is at least lbF, still beat the incumbent?
 // (the incumbent and the candidate list, read once into registers: the scheduler is a single thread per
 // instance and every field of TgInstDev it touches is a memory access)
+// CTA-wide copy of n words of read-only global memory into shared memory, eight loads of a thread in flight (a plain
+// `dst[w] = src[w]` loop through generic pointers is compiled as load, store, load, ...: one L2 round trip per word)
+__device__ __forceinline__ void tgCopyToShared(uint32_t* dst, const uint32_t* src, int n) {
+    for (int w0 = threadIdx.x; w0 < n; w0 += 8 * TG_NT) {
+        uint32_t v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = w0 + u * TG_NT < n ? __ldg(src + w0 + u * TG_NT) : 0u;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) if (w0 + u * TG_NT < n) dst[w0 + u * TG_NT] = v[u];
+    }
+}
+
 struct TgInc {
     int64_t incIter, m1;
     int incIdx;
@@ -1249,6 +1261,14 @@ __device__ __forceinline__ int tgLastBeating(const TgInc& B, int64_t lbF, int lo
         if (tgBeats(B, lbF, mid)) lo = mid; else hi = mid - 1;
     }
     return lo;
+}
+
+// the same by galloping from lo: for a stretch whose answer lies close to its left end (the one above the last evaluated
+// threshold runs to the end of the candidate list) the probes stay inside the staged candidate window
+__device__ __forceinline__ int tgLastBeatingGallop(const TgInc& B, int64_t lbF, int lo, int hi) {
+    int step = 1;
+    while (lo + step <= hi && tgBeats(B, lbF, lo + step)) { lo += step; step <<= 1; }
+    return tgLastBeating(B, lbF, lo, min(hi, lo + step - 1));
 }
 
 __device__ void tgWriteInfeasible(const TgSolveCtx& ctx, TgInstDev& I, int i) {
@@ -1309,7 +1329,11 @@ __device__ void tgFoldInstance(const TgSolveCtx& ctx, TgInstDev& I, const TgPrev
         I.incIter = incIter; I.incIdx = incIdx;
         const uint32_t Sc = uint32_t(incKey >> 8) & 0xffffu;   // compact labels of that item
         uint32_t So = 0;
-        for (int e = 0; e < TG_MAX_K; ++e) if (Sc >> e & 1u) So |= 1u << __ldcg(&itemsPrev[P.slot(beg + incQ)].isl[e]);
+        uint8_t isl[TG_MAX_K];   // (all 16 labels loaded at once: one L2 round trip, not one per member of the mask)
+#pragma unroll
+        for (int e = 0; e < TG_MAX_K; ++e) isl[e] = __ldcg(&itemsPrev[P.slot(beg + incQ)].isl[e]);
+#pragma unroll
+        for (int e = 0; e < TG_MAX_K; ++e) if (Sc >> e & 1u) So |= 1u << isl[e];
         I.incMask = So;
     }
     I.nrun += cnt;
@@ -1410,7 +1434,7 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
         {   // above the last evaluated point only the trivial bound f >= 0 is known: probe just the right end of
             // that stretch; once it is evaluated the stretch gets a real bound and shrinks
             const int last = eIdx[nEval - 1] & ~TG_EDONE;
-            if (last < n - 1 && tgBeats(B, 0, last + 1)) topEnd = tgLastBeating(B, 0, last + 1, n - 1);
+            if (last < n - 1 && tgBeats(B, 0, last + 1)) topEnd = tgLastBeatingGallop(B, 0, last + 1, n - 1);
         }
         if (ns == 0 && topEnd < 0) I.phase = TG_PH_FINAL;
         else {
@@ -1419,10 +1443,12 @@ __device__ int tgPlanInstance(const TgSolveCtx& ctx, TgInstDev& I, int i, int W,
             int32_t* const probe = I.probe;
             int np = 0;
             for (int s = 0; s < ns && budget > 0; ++s) {
+                // (32-bit arithmetic: stretch sizes are counts of candidates, at most NS * K = 33 280, probes at most 64 -- a
+                // 64-bit division is a ~300-cycle chain and this code is on the critical path of every round)
                 const int size = sHi[s] - sLo[s];
-                int share = int(max(1ll, (long long)budget0 * size / max(total, 1ll)));
+                int share = int(max(1u, uint32_t(budget0) * uint32_t(size) / uint32_t(max(total, 1ll))));
                 share = min(min(share, size), budget);
-                for (int q = 1; q <= share; ++q) probe[np++] = sLo[s] + int(((long long)q * size + share - 1) / share);
+                for (int q = 1; q <= share; ++q) probe[np++] = sLo[s] + int((uint32_t(q) * uint32_t(size) + uint32_t(share - 1)) / uint32_t(share));
                 budget -= share;
             }
             if (topEnd >= 0) { probe[np++] = topEnd; total += W; }   // (total += W: not every candidate is probed)
@@ -1534,7 +1560,7 @@ __device__ void tgFoldPlanAll(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dyn
             const int lo = ne > 0 ? int(uint32_t(S.eIdx[0]) & ~uint32_t(TG_EDONE)) : max(S.lbIdx, 0);
             const int nw = max(0, min(TG_CAND_WIN, S.ncand - lo));
             uint32_t* sCand = sEval + size_t(ctx.nInst) * 2 * TG_MAX_EVAL + size_t(i) * TG_CAND_WIN;
-            for (int w = tid; w < nw; w += TG_NT) sCand[w] = S.cand[lo + w];
+            tgCopyToShared(sCand, S.cand + lo, nw);   // (cand is read-only during the solve)
             if (tid == 0) {
                 TgInstDev& Sw = *reinterpret_cast<TgInstDev*>(sInst + size_t(i) * INST_W);
                 Sw.candWin = sCand; Sw.candWinLo = lo; Sw.candWinN = nw;
@@ -1609,7 +1635,7 @@ __device__ void tgQueueFoldPlan(const TgSolveCtx& ctx, TgShared& sm, uint32_t* d
     for (int w = tid; w < ne; w += TG_NT) { sEval[w] = uint32_t(__ldcg(gIdx + w)); sEval[TG_MAX_EVAL + w] = __ldcg(gF + w); }
     const int lo = ne > 0 ? int(uint32_t(__ldcg(gIdx)) & ~uint32_t(TG_EDONE)) : max(I.lbIdx, 0);
     const int nw = max(0, min(TG_CAND_WIN, I.ncand - lo));
-    for (int w = tid; w < nw; w += TG_NT) sCand[w] = I.cand[lo + w];
+    tgCopyToShared(sCand, I.cand + lo, nw);   // (cand is read-only during the solve)
     __syncthreads();
     if (tid == 0) {
         I.eIdx = reinterpret_cast<int32_t*>(sEval);
@@ -1710,6 +1736,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
             if (pos + cnt > TG_MAX_ITEMS) { cnt = 0; I.specIdx = -1; }   // more active instances than items: wait a round
             I.itemBeg = int(pos); I.itemCnt = cnt;
             if (cnt > 0) atomicMax(&sm.iTmp[1], int(pos) + cnt);
+            if (nInst > TG_NW)   // many instances: one thread lays out its instance's probes (a handful: below)
             for (int q = 0; q < cnt; ++q) {
                 TgItem& it = items[pos + q];
                 it.inst = i;
@@ -1723,6 +1750,26 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
         }
     }
     __syncthreads();
+    if (nInst <= TG_NW) {
+        // a handful of instances (the latency-bound case): warp w lays out instance w's probes, one lane per probe -- the
+        // chain probe -> candidate threshold -> item is two dependent L2 round trips, paid once instead of once per probe
+        const int w = tid >> 5, lane = tid & 31;
+        if (w < nInst && ctx.inst[w].phase != TG_PH_DONE) {
+            TgInstDev& I = ctx.inst[w];
+            const int cnt = I.itemCnt, pos = I.itemBeg, kind = I.planKind;
+            for (int q = lane; q < cnt; q += 32) {
+                TgItem& it = items[pos + q];
+                it.inst = w;
+                const int pq = I.probe[q];
+                it.tidx = pq >= 0 ? (pq & ~(TG_PROBE_FINAL | TG_PROBE_KEEP)) : -1;
+                it.T = it.tidx >= 0 ? I.cand[it.tidx] : ctx.dpT;
+                it.flags = kind == TG_PH_FINAL ? TG_IT_TRACK
+                           : (pq >= 0 && (pq & TG_PROBE_FINAL)) ? (TG_IT_TRACK | TG_IT_SPEC)
+                           : (pq >= 0 && (pq & TG_PROBE_KEEP)) ? (TG_IT_TRACK | TG_IT_SPEC | TG_IT_ALLISL) : 0;
+            }
+        }
+        __syncthreads();
+    }
     const int nIt = sm.iTmp[1];
     if (tid == 0 && round < 8) ctrl->schedCyc[round][2] = clock64();
 
@@ -1748,7 +1795,7 @@ __device__ void tgSchedule(const TgSolveCtx& ctx, TgShared& sm, int round) {
             unsigned cnt = 0;
             if (k < K && (allow >> k & 1u)) {
                 const uint32_t* sf = I.sufMinAll + size_t(k) * (L + 2);
-#pragma unroll 8
+#pragma unroll 32
                 for (int d = 1 + half; d <= L; d += 2) cnt += (sf[d] <= T) ? 1u : 0u;
             }
             cnt += __shfl_xor_sync(0xffffffffu, cnt, 16);
