@@ -253,7 +253,9 @@ def _handles(instances):
 def tg_solve_batch(instances, out=None, stream=None, flags: int = TG_SOLVE_DEFAULT, stats=None):
     """Solves the batch.  `out`: a uint8 CUDA tensor of len(instances)*224 bytes (asynchronous on
     `stream`), or None for a host result array (synchronous).  Returns `out`, or a numpy structured
-    array of RESULT_DTYPE when out is None.  `stats`: optional TgSolveStats (host) filled on return."""
+    array of RESULT_DTYPE when out is None.  `stats`: optional TgSolveStats (host: filled on return, the call then
+    synchronises) or a uint8 CUDA tensor of at least sizeof(TgSolveStats) bytes (written asynchronously on `stream`; read it
+    with stats_from_tensor after synchronising)."""
     n = len(instances)
     h = _handles(instances)
     sp = _stream_ptr(stream)
@@ -263,9 +265,14 @@ def tg_solve_batch(instances, out=None, stream=None, flags: int = TG_SOLVE_DEFAU
         optr = host.ctypes.data
     else:
         optr = _ptr(out)
-    sptr = C.addressof(stats) if stats is not None else None
+    sptr = None if stats is None else (C.addressof(stats) if isinstance(stats, TgSolveStats) else _ptr(stats))
     _check(lib().tg_solve_batch_ex(h, n, optr, flags, sptr, sp))
     return host if out is None else out
+
+
+def stats_from_tensor(t) -> "TgSolveStats":
+    """TgSolveStats from the device buffer a tg_solve_batch(..., stats=<CUDA tensor>) call wrote (after synchronising)."""
+    return TgSolveStats.from_buffer_copy(bytes(t[:C.sizeof(TgSolveStats)].cpu().numpy().tobytes()))
 
 
 def tg_solve_batch_ex(instances, out, flags, stats, stream=None):
