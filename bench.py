@@ -448,7 +448,7 @@ def summarize(R, args, workload, world, peak, peak_src, agg):
         "dps_on_l2_cost_rows": R["global_c"] / steps,
         # step 1 of the path (cost-table loader): 8*P bytes read and 9 bytes written per (slice, island) cell -- the kernel
         # of the path that IS HBM-bound on the batched workload
-        "loader": {"bound": "hbm", "kernel": "tgLoadKernel", "kernel_ms": lm, "algorithmic_bytes_per_launch": float(R["load_bytes"]),
+        "loader": {"bound": "hbm", "kernel": "tgLoadRowsKernel" if R["load_bytes"] >= (32 << 20) else "tgLoadKernel", "kernel_ms": lm, "algorithmic_bytes_per_launch": float(R["load_bytes"]),
                    "achieved": R["load_bytes"] / (lm * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                    "frac": R["load_bytes"] / (lm * 1e-3) / 1e9 / peak,
                    "note": "a few MB: bound by launch latency, not by HBM" if R["load_bytes"] < (32 << 20) else "HBM stream"},
