@@ -213,10 +213,11 @@ def test_large_stage_times(tg):
         h.destroy()
 
 
-@pytest.mark.parametrize("n", [1, 2, 4, 5, 63, 64, 65, 147, 148, 149, 300])
+@pytest.mark.parametrize("n", [1, 2, 4, 5, 8, 9, 63, 64, 65, 147, 148, 149, 300, 1024, 1025])
 def test_batch_sizes_around_the_scheduling_modes(tg, n):
-    """1-4 instances: every probe of the last round back-tracks; < 64: one thread per instance on CTA 0; >= 64: wide
-    scheduling; items below / at / above the number of slots: team mode vs solo mode."""
+    """1-4 instances: every probe of the last round back-tracks; <= 8: a warp lays out an instance's probes; < 64: one thread
+    per instance on CTA 0; 64..1024: queue mode (no rounds after the first); above: wide scheduling in rounds; items below /
+    at / above the number of slots: team mode vs solo mode."""
     insts = [gen.random_small(s + 99_000 + 1000 * n, Lmax=8, Kmax=5, Pmax=3, style=STYLES[s % 5]) for s in range(n)]
     for inst, g in zip(insts, solve_all(tg, insts)):
         same(oracle.solve(inst), g, inst.name)
