@@ -762,8 +762,8 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
 }
 
 // ---------------------------------------------------------------------------------------------
-// Levels r >= 1 of a DP that a TEAM of CTAs shares (few instances: cfg3 / cfg4): one WARP per mask, streaming over a
-// contiguous range of masks (colexicographic order, successor by Gosper's hack); nothing but the item's staged tables is
+// Levels r >= 1 of a DP that a TEAM of CTAs shares (few instances: cfg3 / cfg4): one WARP (or half warp) per mask, streaming
+// over its strided share of the level's masks (colexicographic rank order); nothing but the item's staged tables is
 // shared between the warps of a CTA, so a level needs no CTA barrier at all.  Per mask R (|R| = r, nk = Ke - r):
 //   issue   16-byte cp.async copies of the r source rows G_{r-1}[R\{j}][j][.] into the warp's
 //           shared-memory buffer, one mask ahead of their use (double buffer, commit / wait_group)
@@ -772,63 +772,6 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
 // A team's share of a level is dozens of small batches per CTA; measured at cfg4 the CTA-wide batches above (1.60 ms),
 // the same batches per warp (2.04 ms) and this streaming form (1.40 ms), so the team keeps it.
 // ---------------------------------------------------------------------------------------------
-// colexicographic unrank: rank -> mask with r bits among Ke (masks of one popcount ordered by value)
-__device__ __forceinline__ uint32_t tgUnrank(const TgShared& sm, uint32_t rank, int r, int Ke) {
-    uint32_t R = 0;
-    int e = Ke - 1;
-    for (int i = r; i >= 1; --i) {
-        while (uint32_t(sm.binom[e][i]) > rank) --e;
-        rank -= sm.binom[e][i];
-        R |= 1u << e;
-        --e;
-    }
-    return R;
-}
-// next mask with the same popcount (Gosper)
-__device__ __forceinline__ uint32_t tgNextMask(uint32_t R) {
-    const uint32_t c = R & (0u - R), t = R + c;
-    return (((R ^ t) >> 2) >> (__ffs(c) - 1)) | t;
-}
-
-// Issue the copies of the r source rows of mask R into the warp's buffer: 16-byte asynchronous copies
-// (cp.async, LDGSTS), one lane per (source, chunk of 4 starts), committed as one group.  Source row of
-// member j = state (R\{j}, first island j) of level r-1, whose mask rank is
-//   sum_{i<p} C(e_i, i+1) + sum_{i>p} C(e_i, i)   (p = position of j in R: the elements below keep their
-// position, those above move down by one) -- two warp scans over the member lanes.
-// (Bulk TMA copies, one per row, were measured slower here: with row windows a row is often 32-64 bytes
-// and the per-SM TMA issue rate, not bandwidth, became the bound -- DESIGN.md 7.4.)
-// SW = lanes per mask (32, or 16 when a warp runs two masks side by side); sl = lane within the sub-warp;
-// `valid` = this sub-warp has a mask to issue (the shuffles are executed by every lane regardless).
-template <int SW>
-__device__ __forceinline__ void tgIssueMask(const TgShared& sm, uint32_t R, bool valid, int r, int nk, int Wd, int nbw, int cpShift,
-                                            uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
-    const int sl = lane & (SW - 1);
-    const bool member = valid && ((R >> sl) & 1u);   // R < 2^16: lanes 16..31 of a full warp are never members
-    const int p = __popc(R & ((1u << sl) - 1u));
-    // both sums stay below C(16,8) = 12870, so they share one register: low half "kept position", high half "moved down"
-    const uint32_t mine = member ? (uint32_t(sm.binom[sl & 15][p + 1]) | uint32_t(sm.binom[sl & 15][p]) << 16) : 0u;
-    uint32_t incl = mine;
-#pragma unroll
-    for (int o = 1; o < 16; o <<= 1) {
-        const uint32_t a = __shfl_up_sync(0xffffffffu, incl, o);
-        if ((lane & 15) >= o) incl += a;
-    }
-    const uint32_t total = __shfl_sync(0xffffffffu, incl, (lane & 16) | 15);
-    if (member)
-        rowOf[p] = (((incl - mine) & 0xffffu) + ((total - incl) >> 16)) * uint32_t(nk + 1) + uint32_t(sl - p);
-    __syncwarp();
-    if (valid) {
-        const int CP = 1 << cpShift;   // chunks per row, rounded up to a power of two
-        for (int w = sl; w < (r << cpShift); w += SW) {
-            const int ji = w >> cpShift, ch = w & (CP - 1);
-            if (ch < nbw) {
-                const uint32_t* src = Gprev + size_t(rowOf[ji]) * Wd + 4 * ch;
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(bufAddr + uint32_t(ji) * rowBytes + uint32_t(ch) * 16u), "l"(src) : "memory");
-            }
-        }
-    }
-}
-
 // phase 1 for the NSL k slots  slot0, slot0+NG, ...  of this lane's island group and its b chunks:
 //   H[R][k][b] = min_{j in R} x[k][j] + src[j][b],  written to the warp's H rows.
 // All slots but the last are valid for every lane; an invalid last slot reads an all-INF x row.
@@ -951,9 +894,37 @@ __device__ __forceinline__ void tgPhase2W(const TgSolveCtx& ctx, const TgShared&
 
 // One wavefront level for this warp's share of the masks.  SW = 32: one mask at a time on the whole warp.
 // SW = 16: two masks side by side, one per half warp (narrow row windows leave most of a full warp idle and
-// the per-mask bookkeeping -- successor, ranks, copies, windows -- then costs more than the relaxations;
-// two masks share every one of those instructions).  Each sub-warp owns a contiguous run of masks and its
-// own H rows and source buffers inside the warp's buffer.
+// the per-mask bookkeeping -- copies, windows, complement list -- then costs more than the relaxations;
+// two masks share every one of those instructions).  Each sub-warp has its own H rows and source buffers
+// inside the warp's buffer.
+// The masks are dealt out STRIDED and looked up in the rank tables: sub-warp q of Q takes the masks of rank
+// q, q+Q, q+2Q, ...  (Rounds 1 and 2 gave every warp a contiguous run of ranks, walked with Gosper's successor, the source
+// ranks from two 16-lane scans of binomials: 13.6 % of the kernel's instructions at cfg4.)
+// That arithmetic is replaced by the device tables (maskOf: rank -> mask, rankOf: mask -> rank), read three and two masks
+// ahead of their use so that their L2 latency is covered by the masks in between: iteration `it` computes mask it, issues
+// the copies of mask it+1, loads the source ranks of mask it+2 and the mask it+3.  A strided share also samples the level
+// evenly (a run of colexicographic ranks shares its high islands, whose admissible diagonals differ by up to 19:1).
+// Measured at cfg4: solver 1.393 -> 1.342 ms, the levels' share of the CTA cycles 69 -> 66 %.
+template <int SW>
+__device__ __forceinline__ void tgIssueMaskT(uint32_t R, uint32_t rk, bool valid, int r, int nk, int Wd, int nbw, int cpShift,
+                                             uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
+    const int sl = lane & (SW - 1);
+    const bool member = valid && sl < TG_MAX_K && ((R >> sl) & 1u);
+    const int p = __popc(R & ((1u << sl) - 1u));
+    if (member) rowOf[p] = rk * uint32_t(nk + 1) + uint32_t(sl - p);   // row of state (R\{sl}, first island sl) in level r-1
+    __syncwarp();
+    if (valid) {
+        const int CP = 1 << cpShift;   // chunks per row, rounded up to a power of two
+        for (int w = sl; w < (r << cpShift); w += SW) {
+            const int ji = w >> cpShift, ch = w & (CP - 1);
+            if (ch < nbw) {
+                const uint32_t* src = Gprev + size_t(rowOf[ji]) * Wd + 4 * ch;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(bufAddr + uint32_t(ji) * rowBytes + uint32_t(ch) * 16u), "l"(src) : "memory");
+            }
+        }
+    }
+}
+
 template <int SW>
 __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
                             uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW) {
@@ -963,10 +934,10 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     const int Lp = sm.sLp, Wd = sm.sWd, nbw = Wd >> 2, nk = Ke - r;
     const int HS = tgRowStride(Wd);
     const int nMasks = sm.binom[Ke][r];
-    const int lo = int((int64_t(nMasks) * gw) / GW), hi = int((int64_t(nMasks) * (gw + 1)) / GW);
-    if (lo >= hi) return;
-    const int per = (hi - lo + M - 1) / M;                       // masks per sub-warp
-    const int myLo = lo + sub * per, myHi = min(hi, myLo + per);
+    const int q = gw * M + sub, Q = GW * M;
+    if (gw * M >= nMasks) return;                                        // (sub-warp 0 of a warp has the most masks)
+    const int per = (nMasks - 1 - gw * M) / Q + 1;                       // masks of sub-warp 0 = trips of the warp
+    const int cnt = q < nMasks ? (nMasks - 1 - q) / Q + 1 : 0;           // masks of this sub-warp (per or per - 1)
     // sub-lane = (chunk of 4 starts) x (island group): CH chunk lanes, NG = SW / CH groups
     const int cpShift = nbw <= 2 ? 1 : (nbw <= 4 ? 2 : (nbw <= 8 ? 3 : (nbw <= 16 ? 4 : (nbw <= 32 ? 5 : 6))));
     const int chShift = min(cpShift, SWSH);
@@ -985,16 +956,23 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     const int myLen = sl < Ke ? int(sm.maxlenK[sl & 15]) : 0;
     unsigned long long bestKey = TG_KEY_NONE;
 
-    uint32_t R = myLo < myHi ? tgUnrank(sm, uint32_t(myLo), r, Ke) : 0u;
-    tgIssueMask<SW>(sm, R, myLo < myHi, r, nk, Wd, nbw, cpShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
+    const uint16_t* mtab = ctx.maskOf + tgPopOff[r];
+    const uint32_t myBit = sl < TG_MAX_K ? (1u << sl) : 0u;
+    uint32_t R = cnt > 0 ? uint32_t(__ldg(mtab + q)) : 0u;                 // mask of trip 0
+    uint32_t R1 = cnt > 1 ? uint32_t(__ldg(mtab + q + Q)) : 0u;            // trip 1
+    uint32_t R2 = cnt > 2 ? uint32_t(__ldg(mtab + q + 2 * Q)) : 0u;        // trip 2
+    uint32_t rk = (R & myBit) ? uint32_t(__ldg(ctx.rankOf + (R ^ myBit))) : 0u;      // lane sl in R: rank of R \ {sl}
+    uint32_t rk1 = (R1 & myBit) ? uint32_t(__ldg(ctx.rankOf + (R1 ^ myBit))) : 0u;
+    tgIssueMaskT<SW>(R, rk, cnt > 0, r, nk, Wd, nbw, cpShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
     asm volatile("cp.async.commit_group;" ::: "memory");
     int b = 0;
     for (int it = 0; it < per; ++it, b ^= 1) {
-        const int idx = myLo + it;
-        const bool valid = idx < myHi, more = idx + 1 < myHi;
-        const uint32_t Rn = more ? tgNextMask(R) : 0u;
-        tgIssueMask<SW>(sm, Rn, more, r, nk, Wd, nbw, cpShift, bufAddr[b ^ 1], rowBytes, Gprev, rowOf, lane);
+        const int idx = q + it * Q;
+        const bool valid = it < cnt, more = it + 1 < cnt;
+        tgIssueMaskT<SW>(R1, rk1, more, r, nk, Wd, nbw, cpShift, bufAddr[b ^ 1], rowBytes, Gprev, rowOf, lane);
         asm volatile("cp.async.commit_group;" ::: "memory");   // possibly empty: keeps the group count uniform
+        const uint32_t rk2 = (it + 2 < cnt && (R2 & myBit)) ? uint32_t(__ldg(ctx.rankOf + (R2 ^ myBit))) : 0u;
+        const uint32_t R3 = it + 3 < cnt ? uint32_t(__ldg(mtab + idx + 3 * Q)) : 0u;
         const uint32_t comp = ~R & keMask;
         if (valid && sl < Ke && (comp >> sl & 1u)) kl[__popc(comp & ((1u << sl) - 1u))] = uint8_t(sl);
         int capR;                                               // cap(R) = sum of the members' longest slices
@@ -1032,7 +1010,7 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
             else tgPhase2W<false>(ctx, sm, R, capR, nk, nbw, c0, CH, NG, g, hAddr0, rowBytes, csBase, cStride, kl, gRow, bestKey);
         }
         __syncwarp();
-        R = Rn;
+        R = R1; R1 = R2; R2 = R3; rk1 = rk2;
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     if (__any_sync(0xffffffffu, bestKey != TG_KEY_NONE)) {
@@ -1179,7 +1157,9 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
                 if (warp < nW) {
                     uint32_t* wbuf = wbufAll + sm.wbufOff + size_t(warp) * sm.wbufWords;
                     // two masks per warp when the windows are narrow and both masks' rows fit the warp's buffer
-                    const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= sm.wbufWords;
+                    // ... and the level has more masks than the team has warps (else a mask gets the whole warp: the small
+                    // levels at both ends of a DP are one trip of pure latency -- cfg3 0.506 -> 0.478 ms, cfg4 1.343 -> 1.327 ms)
+                    const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= sm.wbufWords && int(sm.binom[Ke][r]) > teamSize * nW;
                     if (pair) tgWarpLevel<16>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
                     else tgWarpLevel<32>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
                 }
