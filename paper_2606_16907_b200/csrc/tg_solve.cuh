@@ -143,6 +143,13 @@ __device__ __forceinline__ int tgLo4(const TgShared& sm, int cap) {
     return sm.sWindowed ? (max(0, sm.sL - cap) & ~3) : 0;
 }
 
+// division of small numbers by a CTA-uniform divisor d: q = t / d for t * d < 2^32 (magic = ceil(2^32 / d), 0 for d = 1)
+// (divisors up to 32 -- chunks of a row window, row groups of a mask -- come from a constant table: a 32-bit division is a
+// dependent chain of ~70 instructions, and the level geometry below sits on every level's critical path)
+__constant__ uint32_t tgMagicTab[33] = {0u, 0u, 2147483648u, 1431655766u, 1073741824u, 858993460u, 715827883u, 613566757u, 536870912u, 477218589u, 429496730u, 390451573u, 357913942u, 330382100u, 306783379u, 286331154u, 268435456u, 252645136u, 238609295u, 226050911u, 214748365u, 204522253u, 195225787u, 186737709u, 178956971u, 171798692u, 165191050u, 159072863u, 153391690u, 148102321u, 143165577u, 138547333u, 134217728u};
+__device__ __forceinline__ uint32_t tgMagic(uint32_t d) { return d <= 32u ? tgMagicTab[d] : 0xffffffffu / d + 1u; }
+__device__ __forceinline__ uint32_t tgDivM(uint32_t t, uint32_t magic) { return magic ? __umulhi(t, magic) : t; }
+
 // Fills the staged cost rows (and dmaxTile) from the reduced table of depth q (q = 1 unless the instance has
 // an actmem table: then level r of the DP, whose stages have r later stages, uses q = r + 1 -- SURVEY NEXT-1).
 // The layout (baseK, D_k) comes from depth 1, whose costs are the lowest, so it covers every depth.
@@ -192,48 +199,78 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
 #else
         const bool bulk = false;
 #endif
-        for (int f = tid; f < tot4; f += TG_NT) {
-            int kc = 0;
-            while (kc + 1 < Ke && int(sm.baseK[kc + 1] >> 2) <= f) ++kc;
-            const int w = f - int(sm.baseK[kc] >> 2);
-            const int dk = sm.dmaxK[kc], Dk = (dk + 3) & ~3;
-            if (w >= Dk * nb4) continue;   // the pad between two islands' tables
-            const int d = 1 + w / nb4, a4 = w - (d - 1) * nb4;
-            uint4 v = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
-            if (d <= dk && a4 < ((L - d + 3) >> 2)) {
-                if (bulk) {
-                    v = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc])[w];
-                    v.x = v.x <= T ? v.x : TG_INFU; v.y = v.y <= T ? v.y : TG_INFU;
-                    v.z = v.z <= T ? v.z : TG_INFU; v.w = v.w <= T ? v.w : TG_INFU;
-                } else if (I.cdT) {
-                    // identical layers (NEXT-3(a)): the row is one value, read once per diagonal instead of once per start
-                    const uint32_t cv = __ldg(I.cdT + int(sm.isl[kc]) * (L + 2) + d);
-                    v = cv <= T ? make_uint4(cv, cv, cv, cv) : make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
-                } else
-                v = TG_COST_AT4(I, sm.cdOff, size_t(sm.isl[kc]) * I.triG + tgGOff(L, d) + 4 * a4, T);
-                const int a = a4 * 4, amax = L - 1 - d;
-                v.x = (a + 0 <= amax) ? v.x : TG_INFU;
-                v.y = (a + 1 <= amax) ? v.y : TG_INFU;
-                v.z = (a + 2 <= amax) ? v.z : TG_INFU;
-                v.w = (a + 3 <= amax) ? v.w : TG_INFU;
-                nAdm += (v.x < TG_INFU) + (v.y < TG_INFU) + (v.z < TG_INFU) + (v.w < TG_INFU);
+        // A thread takes one column (island, 4 starts) -- or one of S interleaved shares of its diagonals when there are fewer
+        // columns than threads -- and walks down the diagonals: island, start and base addresses are worked out once per
+        // column, a step is a load, the threshold, the row-end mask and a store.  (The flat loop over the 16-byte words that
+        // was here spent ~125 instructions a word on finding its island and diagonal: 12-15k of an item's 22-26k staging
+        // cycles at cfg3 / cfg4 were instruction issue.)  Four loads of a thread are in flight.
+        const uint32_t mNb4 = tgMagic(uint32_t(nb4));
+        const uint32_t* const cdP = I.cd + sm.cdOff;
+        const uint32_t* const cdTP = I.cdT;
+        const size_t triG = size_t(I.triG);
+        const bool layered = TG_VAR && I.nLayers != 0;
+        const int nCols = Ke * nb4;
+        int sh = 0;
+        while (sh < 3 && (nCols << (sh + 1)) <= TG_NT) ++sh;   // S = 2^sh threads a column
+        const int S = 1 << sh;
+        for (int cs0 = 0; cs0 < (nCols << sh); cs0 += TG_NT) {   // (warp-uniform trips: the shares of a column meet in a shuffle below)
+            const int cs = cs0 + tid;
+            const bool active = cs < (nCols << sh);
+            const int col = active ? (cs >> sh) : 0, sub = cs & (S - 1);
+            const int kc = int(tgDivM(uint32_t(col), mNb4)), a4 = col - kc * nb4, a = 4 * a4;
+            const int dk = active ? sm.dmaxK[kc] : 0, Dk = (dk + 3) & ~3;
+            int dTop = 0;   // widest diagonal of this share with an admissible entry
+            uint4* const dst = reinterpret_cast<uint4*>(Cs + sm.baseK[kc]) + a4;
+            const size_t islOff = size_t(sm.isl[kc]) * triG + size_t(a);
+            const int islT = int(sm.isl[kc]) * (L + 2);
+            for (int d0 = 1 + sub; d0 <= Dk; d0 += 4 * S) {
+                uint4 v[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int d = d0 + u * S;
+                    v[u] = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+                    if (d <= dk && a4 < ((L - d + 3) >> 2)) {
+                        if (bulk) {
+                            v[u] = dst[(d - 1) * nb4];
+                        } else if (cdTP) {
+                            // identical layers (NEXT-3(a)): the row is one value, read once per diagonal instead of once per start
+                            const uint32_t cv = __ldg(cdTP + islT + d);
+                            v[u] = make_uint4(cv, cv, cv, cv);
+                        } else if (layered) {
+                            v[u] = TG_COST_AT4(I, sm.cdOff, islOff + tgGOff(L, d), T);
+                        } else {
+                            v[u] = __ldg(reinterpret_cast<const uint4*>(cdP + islOff + tgGOff(L, d)));
+                        }
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int d = d0 + u * S;
+                    if (d > Dk) continue;
+                    const int amax = L - 1 - d;
+                    uint4 x = v[u];
+                    // (multi-stage partial plans, NEXT-2: admissible by the slowest internal stage, already applied by
+                    // TG_COST_AT4 -- the cost itself, the whole time, may exceed T)
+                    const uint32_t Tc = layered ? TG_INFU - 1u : T;
+                    x.x = (x.x <= Tc && a + 0 <= amax) ? x.x : TG_INFU;
+                    x.y = (x.y <= Tc && a + 1 <= amax) ? x.y : TG_INFU;
+                    x.z = (x.z <= Tc && a + 2 <= amax) ? x.z : TG_INFU;
+                    x.w = (x.w <= Tc && a + 3 <= amax) ? x.w : TG_INFU;
+                    const unsigned fin = (x.x < TG_INFU) + (x.y < TG_INFU) + (x.z < TG_INFU) + (x.w < TG_INFU);
+                    nAdm += fin;
+                    if (fin) dTop = max(dTop, d);
+                    dst[(d - 1) * nb4] = x;
+                }
             }
-            reinterpret_cast<uint4*>(Cs + sm.baseK[kc])[w] = v;
+            // dmaxTile = widest admissible diagonal of the column's 4 starts (bounds the phase-2 loop): the column's S shares
+            // are neighbouring lanes
+            for (int o = 1; o < S; o <<= 1) dTop = max(dTop, __shfl_xor_sync(0xffffffffu, dTop, o));
+            if (active && sub == 0) sm.dmaxTile[kc][a4] = uint8_t(dTop);
         }
-        __syncthreads();
 #if TG_STAGE_TMA
+        __syncthreads();
         if (bulk && tid == 0) sm.mbarPhase ^= 1u;
 #endif
-        for (int w = tid; w < Ke * nb4; w += TG_NT) {   // widest admissible diagonal per 4 starts
-            const int kc = w / nb4, a4 = w - kc * nb4;
-            const uint4* col = reinterpret_cast<const uint4*>(Cs + sm.baseK[kc]) + a4;
-            int d = sm.dmaxK[kc];
-            for (; d >= 1; --d) {
-                const uint4 v = col[(d - 1) * nb4];
-                if (min(min(v.x, v.y), min(v.z, v.w)) < TG_INFU) break;
-            }
-            sm.dmaxTile[kc][a4] = uint8_t(d);
-        }
     } else {
         for (int w = tid; w < Ke * nb4; w += TG_NT) {
             const int kc = w / nb4, a4 = w - kc * nb4;
@@ -310,9 +347,12 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
             const uint32_t* sf = I.sufMin + size_t(sm.isl[w]) * (L + 2);
             const uint32_t* sa = I.sufMinAll + size_t(sm.isl[w]) * (L + 2);
             unsigned nd = 0, nl = 0;
-            for (int d = 1 + lane; d <= L; d += 32) {
-                nd += (d <= L - 1 && sf[d] <= T) ? 1u : 0u;
-                nl += (sa[d] <= T) ? 1u : 0u;
+            for (int d0 = 1 + lane; d0 <= L; d0 += 64) {   // two lengths a lane and trip, their four loads issued together
+                const int d1 = d0 + 32;
+                const uint32_t f0 = sf[d0], a0 = sa[d0];
+                const uint32_t f1 = d1 <= L ? sf[d1] : TG_INFU, a1 = d1 <= L ? sa[d1] : TG_INFU;
+                nd += ((d0 <= L - 1 && f0 <= T) ? 1u : 0u) + ((d1 <= L - 1 && f1 <= T) ? 1u : 0u);
+                nl += ((a0 <= T) ? 1u : 0u) + ((d1 <= L && a1 <= T) ? 1u : 0u);
             }
             nd = __reduce_add_sync(0xffffffffu, nd);
             nl = __reduce_add_sync(0xffffffffu, nl);
@@ -432,12 +472,6 @@ __device__ __forceinline__ void tgSts4(uint32_t addr, uint4 v) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 
-// division of small numbers by a CTA-uniform divisor d: q = t / d for t * d < 2^32 (magic = ceil(2^32 / d), 0 for d = 1)
-// (divisors up to 32 -- chunks of a row window, row groups of a mask -- come from a constant table: a 32-bit division is a
-// dependent chain of ~70 instructions, and the level geometry below sits on every level's critical path)
-__constant__ uint32_t tgMagicTab[33] = {0u, 0u, 2147483648u, 1431655766u, 1073741824u, 858993460u, 715827883u, 613566757u, 536870912u, 477218589u, 429496730u, 390451573u, 357913942u, 330382100u, 306783379u, 286331154u, 268435456u, 252645136u, 238609295u, 226050911u, 214748365u, 204522253u, 195225787u, 186737709u, 178956971u, 171798692u, 165191050u, 159072863u, 153391690u, 148102321u, 143165577u, 138547333u, 134217728u};
-__device__ __forceinline__ uint32_t tgMagic(uint32_t d) { return d <= 32u ? tgMagicTab[d] : 0xffffffffu / d + 1u; }
-__device__ __forceinline__ uint32_t tgDivM(uint32_t t, uint32_t magic) { return magic ? __umulhi(t, magic) : t; }
 
 // prepass of one mask: descriptor from the mask's rank inside level r, the rows of its r sources in level r-1 and one
 // count per non-member island (the island lists of phase 2 are laid out from these counts).
