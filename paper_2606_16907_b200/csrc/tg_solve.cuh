@@ -1936,10 +1936,17 @@ __global__ void __launch_bounds__(TG_NT, TG_CTAS_PER_SM) tgSolveKernel(const TgS
         }
         tgGridBarrier(ctrl, epoch);
         tgMark(sm, 5);
+        // (thread 0) the ticket after the current one is taken while the current item runs, as long as the queue is long: the
+        // two L2 round trips of a fetch (ticket, publication flag) then overlap the DP.  On a short queue an early ticket
+        // would hold an item back that an idle CTA could run, so there the ticket is taken when it is needed.
+        uint32_t nextSeq = 0;
+        bool haveNext = false;
         while (true) {
             __syncthreads();
             if (threadIdx.x == 0) {
-                const uint32_t seq = atomicAdd(&ctrl->qHead, 1u);
+                const uint32_t seq = haveNext ? nextSeq : atomicAdd(&ctrl->qHead, 1u);
+                haveNext = false;
+                if (int(__ldcg(&ctrl->qTail) - seq) > 2 * int(gridDim.x)) { nextSeq = atomicAdd(&ctrl->qHead, 1u); haveNext = true; }
                 const uint32_t* flag = ctx.itemSeq + (seq & (TG_QCAP - 1));
                 int got = 1;
                 const long long t0 = clock64();
