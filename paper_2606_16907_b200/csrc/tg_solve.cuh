@@ -166,7 +166,6 @@ __device__ unsigned tgStageCosts(const TgSolveCtx& ctx, TgShared& sm, uint32_t* 
         // one flat loop over the 16-byte words of every island's rows (island k occupies D_k * nb4 + 1 of them from
         // baseK[k] / 4): all loads of a thread are independent, one trip to L2 for the whole table instead of one
         // per island
-        const int tot4 = sm.csUsed4;
 #if TG_STAGE_TMA
         // A/B variant (profiles/r2_sass_summary.md): the raw cost rows come in as TMA bulk copies (cp.async.bulk, one per
         // island and diagonal, completion on an mbarrier) and are thresholded in place; core tables only.
@@ -524,10 +523,9 @@ __device__ __forceinline__ void tgIssueBatch(const uint32_t* srcRow, uint32_t sr
 
 // phase 1 of a batch.  Item = (mask i, chunk ch of 4 consecutive b, group sg of NSL rows): the chunk of every
 // source row is read once (LDS.128) and serves NSL rows; slots past the mask's last row read an all-INF x row.
-// The item of chunk 0 also files its rows in the island lists phase 2 works from:
-//   record = { row-in-batch | lo4(S)/4 << 16 | (lo4(R) - lo4(S))/4 << 24 ,  S = R u {k} | k << 16 }
+// (The island lists phase 2 works from are filed by tgBuildLists below, during the same phase.)
 template <int NSL, bool ACTB>
-__device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* desc, uint32_t srcAddr, uint32_t hAddr, uint2* list, int* cur,
+__device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* desc, uint32_t srcAddr, uint32_t hAddr,
                                           int nb, int r, int nk, int nbw, int nsg, uint32_t mNbw, uint32_t mNsg, uint32_t SSB,
                                           uint32_t HSB, uint32_t xsBase, uint32_t xInfAddr) {
     const int nItems = nb * nbw * nsg;
@@ -589,15 +587,30 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
                 const uint32_t hA = hAddr + hrow * HSB + 16u + ch * 16u;
                 tgSts4(hA, make_uint4(acc[e][0], acc[e][1], acc[e][2], acc[e][3]));
                 if (last) { tgSts4(hA + 16, inf4); tgSts4(hA + 32, inf4); }
-                if (first) {
-                    tgSts4(hA - 16, inf4);
-                    const uint32_t k = tgNibble(klLo, klHi, s);
-                    const int cap = int(w0 >> 16);
-                    const int lo4R = max(0, Lw - cap) & ~3, lo4S = max(0, Lw - cap - int(sm.maxlenK[k])) & ~3;
-                    const int pos = atomicAdd(&cur[k], 1);   // island k's stretch of the list starts at its prefix count
-                    list[pos] = make_uint2(hrow | uint32_t(lo4S >> 2) << 16 | uint32_t((lo4R - lo4S) >> 2) << 24, R | (1u << k) | k << 16);
-                }
+                if (first) tgSts4(hA - 16, inf4);
             }
+        }
+    }
+}
+
+// The island lists phase 2 works from, one thread per mask of the batch (the last threads of the CTA, during phase 1):
+//   record of row (R, k) = { row-in-batch | lo4(S)/4 << 16 | (lo4(R) - lo4(S))/4 << 24 ,  S = R u {k} | k << 16 }
+// filed at the next free position of island k's stretch (the stretches start at the prefix of the prepass counts).
+// (Until round 2's last day the phase-1 item of chunk 0 filed its rows itself: those lanes sit in EVERY warp of the CTA --
+// items are chunk-fastest --, so every warp paid the ~100 instructions and the shared-memory atomics of the filing on each pass.)
+__device__ __forceinline__ void tgBuildLists(const TgShared& sm, const uint32_t* desc, uint2* list, int* cur, int nb, int nk) {
+    const int Lw = sm.sWindowed ? sm.sL : 0;
+    for (int i = TG_NT - 1 - int(threadIdx.x); i < nb; i += TG_NT) {
+        const uint32_t* d = desc + i * TG_DESC_W;
+        const uint32_t w0 = d[0], klLo = d[2], klHi = d[3];
+        const uint32_t R = w0 & 0xffffu;
+        const int cap = int(w0 >> 16);
+        const int lo4R = max(0, Lw - cap) & ~3;
+        for (int s = 0; s < nk; ++s) {
+            const uint32_t k = tgNibble(klLo, klHi, s);
+            const int lo4S = max(0, Lw - cap - int(sm.maxlenK[k])) & ~3;
+            const int pos = atomicAdd(&cur[k], 1);
+            list[pos] = make_uint2(uint32_t(i * nk + s) | uint32_t(lo4S >> 2) << 16 | uint32_t((lo4R - lo4S) >> 2) << 24, R | (1u << k) | k << 16);
         }
     }
 }
@@ -772,10 +785,11 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
             tgIssueBatch(srcRowB[par ^ 1], srcAddr[par ^ 1], Gprev, min(NB, hi - m0 - NB), r, Wd, nbw, mNbw, SSB);
             cursors(par ^ 1);
         }
-#define TG_P1_CASE(N, A) case N: tgPhase1B<N, A>(sm, descB[par], srcAddr[par], hAddr, list, sm.cur[par], nb, r, nk, nbw, nsg, mNbw, mNsg, SSB, HSB, xsBase, xInfAddr); break;
+#define TG_P1_CASE(N, A) case N: tgPhase1B<N, A>(sm, descB[par], srcAddr[par], hAddr, nb, r, nk, nbw, nsg, mNbw, mNsg, SSB, HSB, xsBase, xInfAddr); break;
         if (actb) switch (nsl) { TG_P1_CASE(1, true) TG_P1_CASE(2, true) TG_P1_CASE(4, true) }   // (at most 4 rows an item with size classes)
         else switch (nsl) { TG_P1_CASE(1, false) TG_P1_CASE(2, false) TG_P1_CASE(4, false) TG_P1_CASE(8, false) }
 #undef TG_P1_CASE
+        tgBuildLists(sm, descB[par], list, sm.cur[par], nb, nk);
         __syncthreads();   // H rows and the island-sorted list of batch n are complete
         uint32_t* const gBatch = Gcur + size_t(m0) * nk * Wd;
         if (globalC) tgPhase2B<true>(ctx, sm, list, nb * nk * nbw, hAddr, csBase, gBatch, nbw, mNbw, HSB, cStride, bestKey);
