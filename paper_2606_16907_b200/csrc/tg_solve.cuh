@@ -530,7 +530,6 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
                                           uint32_t HSB, uint32_t xsBase, uint32_t xInfAddr) {
     const int nItems = nb * nbw * nsg;
     const int Lw = sm.sWindowed ? sm.sL : 0;
-    const uint4 inf4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
     for (int t = threadIdx.x; t < nItems; t += TG_NT) {
         const uint32_t u = tgDivM(uint32_t(t), mNbw), ch = uint32_t(t) - u * uint32_t(nbw);
         const uint32_t i = tgDivM(u, mNsg), sg = u - i * uint32_t(nsg);
@@ -577,7 +576,6 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
                 }
             }
         }
-        const bool first = ch == 0, last = int(ch) + 1 == nbw;
 #pragma unroll
         for (int e = 0; e < NSL; ++e) {
             const int s = s0 + e;
@@ -585,9 +583,7 @@ __device__ __forceinline__ void tgPhase1B(const TgShared& sm, const uint32_t* de
                 // H row = [4 x INF | Wd values, H[b] at index b - lo4(R) | 8 x INF]
                 const uint32_t hrow = i * uint32_t(nk) + uint32_t(s);
                 const uint32_t hA = hAddr + hrow * HSB + 16u + ch * 16u;
-                tgSts4(hA, make_uint4(acc[e][0], acc[e][1], acc[e][2], acc[e][3]));
-                if (last) { tgSts4(hA + 16, inf4); tgSts4(hA + 32, inf4); }
-                if (first) tgSts4(hA - 16, inf4);
+                tgSts4(hA, make_uint4(acc[e][0], acc[e][1], acc[e][2], acc[e][3]));   // (the INF pads of the row: once per level, tgLevelBatched)
             }
         }
     }
@@ -770,6 +766,15 @@ __device__ void tgLevelBatched(const TgSolveCtx& ctx, TgShared& sm, uint32_t* dy
             if (tid < TG_MAX_K) { sm.cur[par][tid] = inc - c; sm.cntP[par][tid] = 0; }
         }
     };
+    {   // H row = [4 x INF | Wd values, H[b] at index b - lo4(R) | 8 x INF]: the pads are the same for every batch of the level
+        const uint4 inf4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+        for (int w = tid; w < NB * nk; w += TG_NT) {
+            const uint32_t rowA = hAddr + uint32_t(w) * HSB;
+            tgSts4(rowA, inf4);
+            tgSts4(rowA + 16u + uint32_t(nbw) * 16u, inf4);
+            tgSts4(rowA + 32u + uint32_t(nbw) * 16u, inf4);
+        }
+    }
     for (int j = pi; j < 2 * NB; j += TG_NT) {   // the first two batches side by side: one mask a thread
         const int b = j >= NB ? 1 : 0, i = j - b * NB, m0 = lo + b * NB;
         if (i < hi - m0) tgPrepassMask(ctx, sm, descB[b] + i * TG_DESC_W, srcRowB[b] + i * r, sm.cntP[b], uint32_t(m0 + i), r, Ke);
@@ -838,7 +843,6 @@ __device__ __forceinline__ void tgPhase1W(const TgShared& sm, uint32_t R, int r,
         uint32_t acc[NSL][4];
 #pragma unroll
         for (int i = 0; i < NSL; ++i) { acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = TG_INFU; }
-        const bool hasNx = c + 1 < nb4;
         uint32_t co[4] = {0, 0, 0, 0};
         if (ACTB) {
 #pragma unroll
@@ -875,12 +879,7 @@ __device__ __forceinline__ void tgPhase1W(const TgShared& sm, uint32_t R, int r,
             if (i + 1 < NSL || lastValid) {
                 // H row = [4 x INF | Wd values, H[b] at index b - lo4R | 8 x INF]
                 const uint32_t hA = hAddr0 + uint32_t(slot0 + NG * i) * rowBytes + 16u + uint32_t(c) * 16u;
-                tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));
-                if (c == 0) tgSts4(hA - 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
-                if (!hasNx) {
-                    tgSts4(hA + 16, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
-                    tgSts4(hA + 32, make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU));
-                }
+                tgSts4(hA, make_uint4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]));   // (the INF pads: once per level, tgWarpLevel)
             }
         }
     }
@@ -1004,6 +1003,16 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     const int myLen = sl < Ke ? int(sm.maxlenK[sl & 15]) : 0;
     unsigned long long bestKey = TG_KEY_NONE;
 
+    {   // the INF pads of the sub-warp's H rows (4 words before, 8 behind the Wd values): the same for every mask of the level
+        const uint4 inf4 = make_uint4(TG_INFU, TG_INFU, TG_INFU, TG_INFU);
+        for (int s = sl; s < nk; s += SW) {
+            const uint32_t rowA = hAddr0 + uint32_t(s) * rowBytes;
+            tgSts4(rowA, inf4);
+            tgSts4(rowA + 16u + uint32_t(nbw) * 16u, inf4);
+            tgSts4(rowA + 32u + uint32_t(nbw) * 16u, inf4);
+        }
+        __syncwarp();
+    }
     const uint16_t* mtab = ctx.maskOf + tgPopOff[r];
     const uint32_t myBit = sl < TG_MAX_K ? (1u << sl) : 0u;
     uint32_t R = cnt > 0 ? uint32_t(__ldg(mtab + q)) : 0u;                 // mask of trip 0
