@@ -52,6 +52,7 @@ struct TgShared {
     int csUsed4;                    // 16-byte words of the staged cost rows of all islands (incl. the pads between them)
     uint32_t cdOff;                 // word offset of the reduced table of the depth currently staged
     uint8_t maxlenK[TG_MAX_K];      // longest admissible slice of island k at T, any position
+    uint16_t capLo[256], capHi[256];   // cap(R) = capLo[R & 255] + capHi[R >> 8]: sums of maxlenK over the low / high islands of a mask
     uint32_t baseK[TG_MAX_K];
     int dmaxK[TG_MAX_K];
     uint8_t dmaxTile[TG_MAX_K][64];
@@ -359,6 +360,15 @@ __device__ void tgStageItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, u
         }
     }
     __syncthreads();
+    for (int t = tid; t < 256; t += TG_NT) {   // cap(R) by two look-ups instead of a reduction over the members of every mask
+        int lo = 0, hi = 0;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            if ((t >> e & 1) && e < Ke) lo += sm.maxlenK[e];
+            if ((t >> e & 1) && 8 + e < Ke) hi += sm.maxlenK[8 + e];
+        }
+        sm.capLo[t] = uint16_t(lo); sm.capHi[t] = uint16_t(hi);
+    }
     if (tid == 0) {
         int ctot = 0;
         for (int kc = 0; kc < Ke; ++kc) ctot += sm.maxlenK[kc];
@@ -479,7 +489,7 @@ __device__ __forceinline__ void tgSts4(uint32_t addr, uint4 v) {
 __device__ __forceinline__ void tgPrepassMask(const TgSolveCtx& ctx, const TgShared& sm, uint32_t* desc, uint32_t* srcRow, int* cntP,
                                               uint32_t rank, int r, int Ke) {
     const uint32_t R = __ldg(ctx.maskOf + tgPopOff[r] + rank);
-    uint32_t cap = 0, klLo = 0, klHi = 0;
+    uint32_t klLo = 0, klHi = 0;
     int nm = 0, nc = 0;
     const int nk = Ke - r;
     // the rank look-ups of all islands are issued together (a non-member's look-up is a valid, unused table entry): one
@@ -491,7 +501,6 @@ __device__ __forceinline__ void tgPrepassMask(const TgSolveCtx& ctx, const TgSha
     for (int e = 0; e < TG_MAX_K; ++e) {
         if (e >= Ke) break;
         if (R >> e & 1u) {
-            cap += sm.maxlenK[e];
             srcRow[nm] = uint32_t(rk[e]) * uint32_t(nk + 1) + uint32_t(e - nm);
             ++nm;
         } else {
@@ -500,7 +509,7 @@ __device__ __forceinline__ void tgPrepassMask(const TgSolveCtx& ctx, const TgSha
             atomicAdd(&cntP[e], 1);
         }
     }
-    desc[0] = R | cap << 16;
+    desc[0] = R | (uint32_t(sm.capLo[R & 255u]) + uint32_t(sm.capHi[R >> 8])) << 16;
     desc[2] = klLo; desc[3] = klHi;
 }
 
@@ -1000,7 +1009,6 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     uint8_t* kl = &sm.kl[warp][sub * TG_MAX_K];
     const uint32_t keMask = (1u << Ke) - 1u;
     const bool globalC = sm.useGlobalC != 0;
-    const int myLen = sl < Ke ? int(sm.maxlenK[sl & 15]) : 0;
     unsigned long long bestKey = TG_KEY_NONE;
 
     {   // the INF pads of the sub-warp's H rows (4 words before, 8 behind the Wd values): the same for every mask of the level
@@ -1032,14 +1040,7 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
         const uint32_t R3 = it + 3 < cnt ? uint32_t(__ldg(mtab + idx + 3 * Q)) : 0u;
         const uint32_t comp = ~R & keMask;
         if (valid && sl < Ke && (comp >> sl & 1u)) kl[__popc(comp & ((1u << sl) - 1u))] = uint8_t(sl);
-        int capR;                                               // cap(R) = sum of the members' longest slices
-        if (SW == 32) {
-            capR = int(__reduce_add_sync(0xffffffffu, (R >> sl & 1u) ? unsigned(myLen) : 0u));
-        } else {
-            capR = (R >> sl & 1u) ? myLen : 0;
-#pragma unroll
-            for (int o = SW / 2; o > 0; o >>= 1) capR += __shfl_xor_sync(0xffffffffu, capR, o);
-        }
+        const int capR = int(sm.capLo[R & 255u]) + int(sm.capHi[R >> 8]);   // cap(R) = sum of the members' longest slices
         asm volatile("cp.async.wait_group 1;" ::: "memory");   // this mask's rows have landed (the next mask's may be in flight)
         __syncwarp();
 
