@@ -202,8 +202,9 @@ typedef struct { /* optional diagnostics of one tg_solve_batch_ex call, written 
  *   cuda_stream a cudaStream_t (NULL = legacy default stream)
  * Never mutates the instances.  An infeasible instance is not an error (iter_time_us = INT64_MAX,
  * n_stages = 0).  n == 0 is a no-op.  Scratch memory comes from a stream-ordered pool of the library's own (the device's
- * default pool is not touched).  Freed workspaces stay cached in that pool -- up to 14 GB, the DP scratch of the largest
- * shapes; the environment variable TG_POOL_KEEP_MB lowers it -- until tg_release_cached_memory() is called.
+ * default pool is not touched; the tables of the instances come from the same pool).  Freed workspaces and tables stay
+ * cached in that pool -- up to 14 GB, the DP scratch of the largest shapes; the environment variable TG_POOL_KEEP_MB
+ * lowers it -- until tg_release_cached_memory() is called.
  * Internal errors of the solver (they have never been observed; the checks exist because the search keeps bounded
  * lists): a call with a HOST buffer or HOST statistics returns TG_ERR_CUDA; in the fully asynchronous form (DEVICE
  * results, no statistics) every result of the call is instead written with n_stages = -1 and

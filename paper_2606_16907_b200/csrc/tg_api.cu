@@ -169,6 +169,19 @@ tg_status deviceInit(int dev, DeviceState** out) {
 
 inline size_t alignUp(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Stream-ordered device memory from the library's own pool (instance tables as well as per-call workspaces: memory freed
+// into the device's DEFAULT pool goes back to the driver at the next synchronisation and is mapped again on the next
+// allocation -- an end-to-end loop that creates and destroys 385 MB of tables per step then stalls for up to a second now
+// and then).
+cudaError_t poolAlloc(void** p, size_t bytes, cudaStream_t st) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    DeviceState* D = nullptr;
+    if (deviceInit(dev, &D) != TG_OK) return cudaErrorInitializationError;
+    return cudaMallocFromPoolAsync(p, bytes, D->pool, st);
+}
+
 struct Carver {
     size_t off = 0;
     size_t take(size_t bytes, size_t align = 256) {
@@ -509,7 +522,7 @@ tg_status createAsync(int32_t L, int32_t K, int32_t P, int32_t m, const int32_t*
     Carver cv;
     const size_t oT = cv.take(nE * 4), oM = cv.take(nE * 4), oG = cv.take(K * 4), oC = cv.take(K * 4), oB = cv.take(K * K * 4), oE = cv.take(4);
     // stream-ordered allocation on the legacy default stream (pool-cached: no device synchronisation)
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&base), cv.off, 0));
+    TG_CUDA(poolAlloc(reinterpret_cast<void**>(&base), cv.off, 0));
     tg_instance* t = new (std::nothrow) tg_instance();
     if (!t) { cudaFreeAsync(base, 0); return fail(TG_ERR_OOM, "host allocation failed"); }
     t->L = L; t->K = K; t->P = P; t->m = m; t->act_mb = act_mb; t->NS = NS; t->device = dev;
@@ -590,8 +603,8 @@ tg_status tg_instance_create_classes(int32_t L, int32_t K, int32_t P, int32_t m,
     const size_t oT = cv.take(nE * 4), oM = cv.take(nE * 4), oG = cv.take(K * 4), oC = cv.take(K * 4), oB = cv.take(K * K * 4), oE = cv.take(4);
     // one block, kept by the instance: [classOf | class time | class mem], each 256-byte aligned (16-byte loads)
     const size_t oCls = ct.take(size_t(NS) * 4), oCt = ct.take(nC * 4), oCm = ct.take(nC * 4);
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&base), cv.off, 0));
-    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&tmp), ct.off, 0);
+    TG_CUDA(poolAlloc(reinterpret_cast<void**>(&base), cv.off, 0));
+    cudaError_t e = poolAlloc(reinterpret_cast<void**>(&tmp), ct.off, 0);
     if (e != cudaSuccess) { cudaFreeAsync(base, 0); return fail(TG_ERR_OOM, std::string("class tables: ") + cudaGetErrorString(e)); }
     tg_instance* t = new (std::nothrow) tg_instance();
     if (!t) { cudaFreeAsync(base, 0); cudaFreeAsync(tmp, 0); return fail(TG_ERR_OOM, "host allocation failed"); }
@@ -674,7 +687,7 @@ tg_status tg_instance_create_batch(int32_t n, const int32_t* L, const int32_t* K
     const size_t oSmall = cv.take(smallInts * 4), oDesc = cv.take(sizeof(TgValidateDesc) * size_t(n)), oErr = cv.take(size_t(n) * 4);
     TgBatchBlock* blk = new (std::nothrow) TgBatchBlock();
     if (!blk) return fail(TG_ERR_OOM, "host allocation failed");
-    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&blk->base), cv.off, 0);
+    cudaError_t e = poolAlloc(reinterpret_cast<void**>(&blk->base), cv.off, 0);
     if (e != cudaSuccess) {
         delete blk;
         cudaGetLastError();
@@ -787,7 +800,7 @@ tg_status tg_instance_set_actmem(tg_instance* inst, const int32_t* actmem_mb) {
     if (inst->slow) return fail(TG_ERR_SHAPE, "the instance has multi-stage partial plans (tg_instance_set_stages): the combination with a footprint table is not built");
     const size_t nE = size_t(inst->NS) * inst->K * inst->P;
     int32_t* d = nullptr;
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), nE * 4 + 4, 0));
+    TG_CUDA(poolAlloc(reinterpret_cast<void**>(&d), nE * 4 + 4, 0));
     int* dErr = reinterpret_cast<int*>(d + nE);
     cudaError_t e = cudaMemcpyAsync(d, actmem_mb, nE * 4, cudaMemcpyDefault, 0);
     if (e == cudaSuccess) e = cudaMemsetAsync(dErr, 0, 4, 0);
@@ -815,7 +828,7 @@ tg_status tg_instance_set_stages(tg_instance* inst, const int32_t* slow_us, cons
     if (inst->nAct) return fail(TG_ERR_SHAPE, "the instance has per-boundary activation sizes (tg_instance_set_boundary_act): the combination with multi-stage partial plans is not built");
     const size_t nE = size_t(inst->NS) * inst->K * inst->P;
     int32_t* d = nullptr;
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), 2 * nE * 4 + 4, 0));
+    TG_CUDA(poolAlloc(reinterpret_cast<void**>(&d), 2 * nE * 4 + 4, 0));
     int32_t* dq = d + nE;
     int* dErr = reinterpret_cast<int*>(d + 2 * nE);
     cudaError_t e = cudaMemcpyAsync(d, slow_us, nE * 4, cudaMemcpyDefault, 0);
@@ -933,7 +946,7 @@ static tg_status reduceImpl(tg_instance* inst, int32_t* c_out, int32_t* argp_out
     if (s != TG_OK) return s;
     const int cells = inst->NS * inst->K, K = inst->K;
     int32_t *dc = nullptr, *da = nullptr, *dx = nullptr;
-    cudaError_t e = cudaMallocAsync(reinterpret_cast<void**>(&dc), size_t(cells) * 4 * 2 + K * K * 4, st);
+    cudaError_t e = poolAlloc(reinterpret_cast<void**>(&dc), size_t(cells) * 4 * 2 + K * K * 4, st);
     TgInstDev hI;
     if (e == cudaSuccess) {
         da = dc + cells; dx = da + cells;
@@ -993,7 +1006,7 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t oCounts = 0, oCap = size_t(n) * 32, oDesc = oCap + size_t(n) * (TG_MAX_K + 1) * 8;
     char* ws = nullptr;
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&ws), oDesc + sizeof(TgPruneDesc) * size_t(n), st));
+    TG_CUDA(poolAlloc(reinterpret_cast<void**>(&ws), oDesc + sizeof(TgPruneDesc) * size_t(n), st));
     unsigned long long* dCounts = reinterpret_cast<unsigned long long*>(ws + oCounts);
     long long* dCap = reinterpret_cast<long long*>(ws + oCap);
     TgPruneDesc* dDesc = reinterpret_cast<TgPruneDesc*>(ws + oDesc);
@@ -1168,7 +1181,7 @@ tg_status tg_islands_build(int32_t n_nodes, const int32_t* node_gpus, const int3
     memcpy(h.data(), node_gpus, N * 4); memcpy(h.data() + N, node_compute, N * 4); memcpy(h.data() + 2 * N, node_mem_mb, N * 4);
     memcpy(h.data() + 3 * N, node_intra_bw, N * 4); memcpy(h.data() + 4 * N, inter_bw, size_t(N) * N * 4);
     int32_t* d = nullptr;
-    TG_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&d), h.size() * 4, 0));
+    TG_CUDA(poolAlloc(reinterpret_cast<void**>(&d), h.size() * 4, 0));
     cudaError_t e = cudaMemcpyAsync(d, h.data(), nIn * 4, cudaMemcpyHostToDevice, 0);
     if (e == cudaSuccess) {
         TgIslandsArgs A;
