@@ -1225,7 +1225,9 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
                 tgLevelBatched(ctx, sm, wbufAll, Gprev, Gcur, key, Ke, r, member, teamSize);
             }
             tgMark(sm, 3);
-            if (teamSize > 1) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
+            // (after the last level of a DP that is not back-tracked nothing reads the team's rows: the round's grid barrier
+            // is the next thing every member does, so the team barrier is left out)
+            if (teamSize > 1 && (r + 1 < Ke || bufWords == 0)) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();
             tgMark(sm, 4);
         }
