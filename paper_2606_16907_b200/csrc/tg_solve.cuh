@@ -122,6 +122,22 @@ __device__ __forceinline__ void tgTeamBarrier(uint32_t* bar, uint32_t target) {
     __syncthreads();
 }
 
+// The same barrier in two halves: arrive when the level is done, wait at the start of the next level -- behind the table
+// look-ups of that level's first masks, which need nothing the other members write (tgRunItem).
+__device__ __forceinline__ void tgTeamArrive(uint32_t* bar) {
+    __syncthreads();
+    if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
+}
+__device__ __forceinline__ void tgTeamWait(uint32_t* bar, uint32_t target) {
+    if (threadIdx.x == 0) {
+        uint32_t v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while (v < target);
+    }
+    __syncthreads();
+}
+
 // rows (R,k) of wavefront level r with Ke islands alive
 __device__ __forceinline__ uint32_t tgLevelRows(int Ke, int r) { return uint32_t(tgBinom[Ke][r]) * uint32_t(Ke - r); }
 
@@ -961,6 +977,26 @@ __device__ __forceinline__ void tgPhase2W(const TgSolveCtx& ctx, const TgShared&
 // the copies of mask it+1, loads the source ranks of mask it+2 and the mask it+3.  A strided share also samples the level
 // evenly (a run of colexicographic ranks shares its high islands, whose admissible diagonals differ by up to 19:1).
 // Measured at cfg4: solver 1.393 -> 1.342 ms, the levels' share of the CTA cycles 69 -> 66 %.
+// The first trips of a (sub-)warp in a level: masks of trips 0..2 and the source ranks of trips 0..1 (sw = lanes per mask of
+// that level, 16 or 32).  Looked up BEFORE the wait for the previous level's team barrier: the two dependent table
+// look-ups (mask, then ranks) overlap the wait instead of following it.
+struct TgPre { uint32_t R0, R1, R2, rk0, rk1; };
+__device__ __forceinline__ TgPre tgPreLookup(const TgSolveCtx& ctx, const TgShared& sm, int Ke, int r, int gw, int GW, int sw) {
+    const int lane = threadIdx.x & 31;
+    const int M = 32 / sw, sub = sw == 32 ? 0 : (lane >> 4), sl = lane & (sw - 1);
+    const int nMasks = sm.binom[Ke][r];
+    const int q = gw * M + sub, Q = GW * M;
+    const uint16_t* mtab = ctx.maskOf + tgPopOff[r];
+    const uint32_t myBit = sl < TG_MAX_K ? (1u << sl) : 0u;
+    TgPre P;
+    P.R0 = q < nMasks ? uint32_t(__ldg(mtab + q)) : 0u;
+    P.R1 = q + Q < nMasks ? uint32_t(__ldg(mtab + q + Q)) : 0u;
+    P.R2 = q + 2 * Q < nMasks ? uint32_t(__ldg(mtab + q + 2 * Q)) : 0u;
+    P.rk0 = (P.R0 & myBit) ? uint32_t(__ldg(ctx.rankOf + (P.R0 ^ myBit))) : 0u;   // lane sl in R: rank of R \ {sl}
+    P.rk1 = (P.R1 & myBit) ? uint32_t(__ldg(ctx.rankOf + (P.R1 ^ myBit))) : 0u;
+    return P;
+}
+
 template <int SW>
 __device__ __forceinline__ void tgIssueMaskT(uint32_t R, uint32_t rk, bool valid, int r, int nk, int Wd, int nbw, int cpShift,
                                              uint32_t bufAddr, uint32_t rowBytes, const uint32_t* Gprev, uint32_t* rowOf, int lane) {
@@ -983,7 +1019,7 @@ __device__ __forceinline__ void tgIssueMaskT(uint32_t R, uint32_t rk, bool valid
 
 template <int SW>
 __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t* Cs, uint32_t* wbuf, const uint32_t* Gprev,
-                            uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW) {
+                            uint32_t* Gcur, unsigned long long* key, int Ke, int r, int gw, int GW, const TgPre pre) {
     constexpr int M = 32 / SW, SWSH = SW == 32 ? 5 : 4;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int sub = lane >> SWSH, sl = lane & (SW - 1);
@@ -1023,11 +1059,8 @@ __device__ void tgWarpLevel(const TgSolveCtx& ctx, TgShared& sm, const uint32_t*
     }
     const uint16_t* mtab = ctx.maskOf + tgPopOff[r];
     const uint32_t myBit = sl < TG_MAX_K ? (1u << sl) : 0u;
-    uint32_t R = cnt > 0 ? uint32_t(__ldg(mtab + q)) : 0u;                 // mask of trip 0
-    uint32_t R1 = cnt > 1 ? uint32_t(__ldg(mtab + q + Q)) : 0u;            // trip 1
-    uint32_t R2 = cnt > 2 ? uint32_t(__ldg(mtab + q + 2 * Q)) : 0u;        // trip 2
-    uint32_t rk = (R & myBit) ? uint32_t(__ldg(ctx.rankOf + (R ^ myBit))) : 0u;      // lane sl in R: rank of R \ {sl}
-    uint32_t rk1 = (R1 & myBit) ? uint32_t(__ldg(ctx.rankOf + (R1 ^ myBit))) : 0u;
+    uint32_t R = pre.R0, R1 = pre.R1, R2 = pre.R2;   // masks of trips 0..2 (0 = none), looked up by the caller (tgPreLookup)
+    uint32_t rk = pre.rk0, rk1 = pre.rk1;            // lane sl in R: rank of R \ {sl}
     tgIssueMaskT<SW>(R, rk, cnt > 0, r, nk, Wd, nbw, cpShift, bufAddr[0], rowBytes, Gprev, rowOf, lane);
     asm volatile("cp.async.commit_group;" ::: "memory");
     int b = 0;
@@ -1202,6 +1235,7 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
     uint32_t* slot = ctx.scratch + uint64_t(slotIdx) * ctx.slotWords;
     uint32_t* bar = ctx.slotBar + slotIdx;
     uint32_t arrivals = 0;
+    bool pendingBar = false;
     if (Ke > 0) {
         if (threadIdx.x < 2 * TG_MAX_K) (&sm.cntP[0][0])[threadIdx.x] = 0;   // island counts of the batched levels: zero at every level's entry
         tgLevel0(ctx, sm, slot, key, member == 0);
@@ -1212,14 +1246,18 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
             if (TG_VAR && I.nDepth > 1) tgStageCosts(ctx, sm, Cs, r + 1, false);   // stages of this level hold r + 1 microbatches
             if (teamSize > 1) {
                 const int warp = threadIdx.x >> 5, nW = sm.nWarps;
+                TgPre pre = {0u, 0u, 0u, 0u, 0u};
+                const bool pairL = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= sm.wbufWords && int(sm.binom[Ke][r]) > teamSize * nW;
+                if (warp < nW) pre = tgPreLookup(ctx, sm, Ke, r, member * nW + warp, teamSize * nW, pairL ? 16 : 32);
+                if (pendingBar) { tgTeamWait(bar, arrivals); pendingBar = false; tgMark(sm, 4); }   // level r-1 is complete on every member
                 if (warp < nW) {
                     uint32_t* wbuf = wbufAll + sm.wbufOff + size_t(warp) * sm.wbufWords;
                     // two masks per warp when the windows are narrow and both masks' rows fit the warp's buffer
                     // ... and the level has more masks than the team has warps (else a mask gets the whole warp: the small
                     // levels at both ends of a DP are one trip of pure latency -- cfg3 0.506 -> 0.478 ms, cfg4 1.343 -> 1.327 ms)
                     const bool pair = (Wd >> 2) <= 16 && 2 * (Ke + r) * tgRowStride(Wd) <= sm.wbufWords && int(sm.binom[Ke][r]) > teamSize * nW;
-                    if (pair) tgWarpLevel<16>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
-                    else tgWarpLevel<32>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW);
+                    if (pair) tgWarpLevel<16>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, pre);
+                    else tgWarpLevel<32>(ctx, sm, Cs, wbuf, Gprev, Gcur, key, Ke, r, member * nW + warp, teamSize * nW, pre);
                 }
             } else {
                 tgLevelBatched(ctx, sm, wbufAll, Gprev, Gcur, key, Ke, r, member, teamSize);
@@ -1227,7 +1265,9 @@ __device__ void tgRunItem(const TgSolveCtx& ctx, TgShared& sm, uint32_t* Cs, uin
             tgMark(sm, 3);
             // (after the last level of a DP that is not back-tracked nothing reads the team's rows: the round's grid barrier
             // is the next thing every member does, so the team barrier is left out)
-            if (teamSize > 1 && (r + 1 < Ke || bufWords == 0)) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
+            // Between two levels the barrier is split: arrive here, wait at the start of the next level behind its look-ups.
+            if (teamSize > 1 && r + 1 < Ke) { arrivals += uint32_t(teamSize); tgTeamArrive(bar); pendingBar = true; }
+            else if (teamSize > 1 && bufWords == 0) { arrivals += uint32_t(teamSize); tgTeamBarrier(bar, arrivals); }
             else __syncthreads();
             tgMark(sm, 4);
         }
