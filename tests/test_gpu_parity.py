@@ -235,3 +235,27 @@ def test_loader_paths_in_one_batch(tg):
     for batch in (p8 + odd + p4[:20] + foot, p4 + odd + p8[:20] + foot, odd + p4 + p8):
         for inst, g in zip(batch, solve_all(tg, batch)):
             same(oracle.solve_depth(inst) if inst.actmem_mb is not None else oracle.solve(inst), g, inst.name)
+
+
+def test_statistics_on_the_device_match_the_host_form(tg):
+    """tg_solve_stats written to a DEVICE buffer (the call stays asynchronous; bench.py times it that way) against the HOST
+    form of the same solve: a few instances run in rounds, so every count is deterministic."""
+    import torch
+    insts = [gen.config2(), gen.config3(0, L=20, K=5), gen.random_small(77, Lmax=9, Kmax=5, Pmax=3, style="ties")]
+    hs = [tg.instance_from_inputs(i) for i in insts]
+    host = tg.TgSolveStats()
+    want = tg.tg_solve_batch(hs, stats=host)
+    out = torch.empty(len(hs) * tg.RESULT_BYTES, dtype=torch.uint8, device="cuda")
+    dev = torch.zeros(256, dtype=torch.uint8, device="cuda")
+    tg.tg_solve_batch(hs, out=out, stats=dev)
+    torch.cuda.synchronize()
+    got = tg.stats_from_tensor(dev)
+    for f in ("n_dp", "plans_dense", "states_live", "n_rounds", "error_flag", "relax_admissible", "states_windowed"):
+        assert getattr(got, f) == getattr(host, f), f
+    assert host.n_dp > 0 and host.error_flag == 0
+    res = tg.results_from_tensor(out, len(hs))
+    for inst, a, b in zip(insts, want, res):
+        assert int(a["iter_time_us"]) == int(b["iter_time_us"]) and int(a["island_mask"]) == int(b["island_mask"])
+        same(oracle.solve(inst), b, inst.name)
+    for h in hs:
+        h.destroy()
