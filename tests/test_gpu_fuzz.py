@@ -2,7 +2,10 @@
 instances: every probe of the last round back-tracks; <= 8: a warp lays out an instance's probes; < 64: rounds on CTA 0;
 64-1024: queue mode; team vs solo by the item count), random shapes (L, K, P) and table styles, the core path and the four
 variants of SURVEY.md §8(f) -- every instance against its oracle, value and plan, bit-exact through the C ABI.
-(The same loop ran for seven minutes on the final kernels of round 2: 4 608 batches, 478 886 instances, no difference.)"""
+(The same loop ran for seven minutes on the final kernels of round 2: 4 608 batches, 478 886 instances, no difference.)
+The second test does the same with mid-size instances of the paper's workload shapes (K = 10-13 islands): team mode with
+wide levels (two masks per warp, the split team barrier), the strided rank tables beyond K = 9, a K >= 10 batch on the
+round scheduler.  (Its loop with random shapes ran for 13 minutes on the same kernels: 77 batches, 1 198 instances.)"""
 import random
 
 import pytest
@@ -60,3 +63,23 @@ def test_random_batches_shapes_and_variants(tg, seed):
             h.destroy()
         n_inst += n
     assert n_inst > 1000
+
+
+# (instances, shape, L, K, kind): about 25 s of oracle time in all
+MID = [(1, "config3", 12, 13, "core"), (2, "config4", 16, 12, "core"), (3, "config3", 20, 12, "core"),
+       (4, "config4", 16, 13, "core"), (9, "config3", 12, 11, "core"), (2, "config5_one", 24, 10, "core"),
+       (1, "config5_one", 12, 10, "act"), (3, "config3", 12, 12, "xb"), (20, "config5_one", 12, 10, "core"),
+       (5, "config3", 20, 10, "act")]
+
+
+def test_mid_size_paper_shapes(tg):
+    rng = random.Random(21)
+    for n, shape, L, K, kind in MID:
+        seed0 = rng.randrange(1 << 20)
+        insts = [variant(kind, getattr(gen, shape)(seed0 + s, L=L, K=K), s) for s in range(n)]
+        hs = [tg.instance_from_inputs(i) for i in insts]
+        res = tg.tg_solve_batch(hs)
+        for inst, g in zip(insts, res):
+            same(ORACLE[kind](inst), g, f"{kind} n={n} {shape} L={L} K={K} seed0={seed0} {inst.name}")
+        for h in hs:
+            h.destroy()
