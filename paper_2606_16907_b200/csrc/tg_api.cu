@@ -400,10 +400,10 @@ tg_status prepare(tg_instance* const* instances, int n, bool needSolve, cudaStre
         const size_t sh = size_t(maxK) * maxL * TG_LOAD_RG * 4;
         if (P0 == 4) {
             TG_CUDA(cudaFuncSetAttribute(tgLoadRowsKernel<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-            tgLoadRowsKernel<1, 4><<<gr, 256, sh, st>>>(W.inst);
+            tgLoadRowsKernel<1, 4><<<gr, TG_LR_NT, sh, st>>>(W.inst);
         } else {
             TG_CUDA(cudaFuncSetAttribute(tgLoadRowsKernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024));
-            tgLoadRowsKernel<2, 2><<<gr, 256, sh, st>>>(W.inst);
+            tgLoadRowsKernel<2, 2><<<gr, TG_LR_NT, sh, st>>>(W.inst);
         }
     } else if (wide) {
         if (P0 == 4) tgLoadKernel<1, TG_LOAD_U><<<g, 256, 0, st>>>(W.inst);

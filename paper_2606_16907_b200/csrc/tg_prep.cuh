@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
                     }
                 }
                 if (best < sMin[k]) atomicMin(&sMin[k], best);
-                // the thread's next cell: 256 cells = ds slices and dk islands further on
+                // the thread's next cell: TG_LR_NT cells = ds slices and dk islands further on
                 int adv = ds;
                 k += dk;
                 if (k >= K) { k -= K; ++adv; }
@@ -348,8 +348,14 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
 // diagonal-major tables as 32-byte runs (two 16-byte stores of neighbouring lanes = one full sector).  The cell-order
 // kernel above writes one 4-byte word per sector there (12 sectors per store request, profiles/r1c_ncu_cfg5_loader.md).
 #define TG_LOAD_RG 8
+// CTAs of 128 threads: eight of them share an SM instead of four of 256, so the phases of a CTA that move no data (tile
+// initialisation, the barriers, the tail of the cell loop) are covered by more neighbours -- 0.109 -> 0.102 ms on the
+// 1024-instance batch (64 threads: 0.148 ms, 96: 0.109, 8 cells a thread in flight: 0.127 at 109 registers)
+#ifndef TG_LR_NT
+#define TG_LR_NT 128
+#endif
 template <int PV, int U>
-__global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ insts) {
+__global__ void __launch_bounds__(TG_LR_NT) tgLoadRowsKernel(TgInstDev* __restrict__ insts) {
     extern __shared__ uint32_t tile[];   // [K][L][TG_LOAD_RG]
     TgInstDev& I = insts[blockIdx.y];
     const int L = I.L, K = I.K;
@@ -362,17 +368,17 @@ __global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ 
     __shared__ int32_t sCap[TG_MAX_K];
     __shared__ uint32_t sMax;
     const int tid = threadIdx.x;
-    for (int w = tid; w < K * L * TG_LOAD_RG; w += 256) tile[w] = TG_INFU;
+    for (int w = tid; w < K * L * TG_LOAD_RG; w += TG_LR_NT) tile[w] = TG_INFU;
     if (tid < TG_MAX_K) { sMin[tid] = TG_INFU; sCap[tid] = tid < K ? __ldg(I.cap_mb + tid) : 0; }
     if (tid == 0) sMax = 0;
     __syncthreads();
     uint32_t myMax = 0;
-    const int ds = 256 / K, dk = 256 - ds * K;
-    for (int base = cellBeg; base < cellEnd; base += 256 * U) {
+    const int ds = TG_LR_NT / K, dk = TG_LR_NT - ds * K;
+    for (int base = cellBeg; base < cellEnd; base += TG_LR_NT * U) {
         int4 tv[U][PV], mv[U][PV];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int cell = base + 256 * u + tid;
+            const int cell = base + TG_LR_NT * u + tid;
             if (cell < cellEnd) {
                 // (NEXT-3(a): a class instance reads the rows of its slice's signature class)
                 const size_t src = I.classOf ? size_t(__ldg(I.classOf + cell / K)) * K + size_t(cell % K) : size_t(cell);
@@ -389,7 +395,7 @@ __global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ 
             tgSliceAB(L, s0, a, b);
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int cell = cellFirst + 256 * u;
+                const int cell = cellFirst + TG_LR_NT * u;
                 if (cell < cellEnd) {
                     const int32_t capk = sCap[k];
                     uint32_t bq = TG_INFU; int bp = 0xff;
@@ -407,7 +413,7 @@ __global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ 
                     I.sortbuf[cell] = bq;
                     if (bq < TG_INFU) myMax = max(myMax, bq);
                     if (bq < sMin[k]) atomicMin(&sMin[k], bq);
-                    // the thread's next cell: 256 cells = ds slices and dk islands further on
+                    // the thread's next cell: TG_LR_NT cells = ds slices and dk islands further on
                     int adv = ds;
                     k += dk;
                     if (k >= K) { k -= K; ++adv; }
@@ -424,7 +430,7 @@ __global__ void __launch_bounds__(256) tgLoadRowsKernel(TgInstDev* __restrict__ 
     // tile -> diagonal-major rows: row d of island k holds a = 0 .. L-d, padded with INF to a multiple of 4 words; this
     // CTA owns the starts a0 .. a0+7 of every row that reaches them
     const int nd = L - a0;                                   // diagonals with an entry at start a0
-    for (int w = tid; w < K * nd * 2; w += 256) {
+    for (int w = tid; w < K * nd * 2; w += TG_LR_NT) {
         const int q = w & 1, r = w >> 1, k = r / nd, d = 1 + (r - k * nd);
         const int a = a0 + 4 * q, rl = (L - d + 1 + 3) & ~3;  // padded row length
         if (a < rl)
