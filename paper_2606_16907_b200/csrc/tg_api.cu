@@ -1012,28 +1012,29 @@ tg_status tg_prune_batch(tg_instance* const* instances, int32_t n, tg_prune_mode
     TgPruneDesc* dDesc = reinterpret_cast<TgPruneDesc*>(ws + oDesc);
     TG_CUDA(cudaMemsetAsync(ws, 0, oCap, st));
     TG_CUDA(cudaMemcpyAsync(dDesc, h.data(), sizeof(TgPruneDesc) * size_t(n), cudaMemcpyHostToDevice, st));
-    const dim3 g((maxCells + 255) / 256, n);
-    {   // cell pass: the register path is compiled for P = 4 and P = 8 (picked from the first instance); two cells per
-        // thread once that still leaves every SM a few CTAs
+    const dim3 g((maxCells + 255) / 256, n), g1((maxCells + TG_PR_NT - 1) / TG_PR_NT, n);
+    {   // cell pass: the register path is compiled for P = 4 and P = 8 (picked from the first instance); TG_PR_U cells per
+        // thread (two of P = 8) once that still leaves every SM a few CTAs
         DeviceState* DS = nullptr;
         int dev = 0;
         TG_CUDA(cudaGetDevice(&dev));
         const tg_status sd = deviceInit(dev, &DS);
         if (sd != TG_OK) { cudaFreeAsync(ws, st); return sd; }
         const int P0 = instances[0]->P;
-        const dim3 g2((maxCells + 511) / 512, n);
-        const bool wide = int64_t(g2.x) * n >= 4 * DS->numSMs;   // (4 cells a thread measured slower: 143 vs 134 us on the 1024-instance batch)
+        const dim3 g2((maxCells + 2 * TG_PR_NT - 1) / (2 * TG_PR_NT), n);
+        const dim3 gU((maxCells + TG_PR_U * TG_PR_NT - 1) / (TG_PR_U * TG_PR_NT), n);
+        const bool wide = int64_t(g2.x) * n >= 4 * DS->numSMs;   // (several cells a thread once that still leaves every SM a few CTAs)
         bool act = false;
         for (int i = 0; i < n; ++i) act = act || instances[i]->actmem != nullptr;
 #define TG_PRUNE_LAUNCH(PV, U, G) \
-        do { if (act) tgPruneCellKernel<PV, U, true><<<G, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts); \
-             else tgPruneCellKernel<PV, U, false><<<G, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts); } while (0)
+        do { if (act) tgPruneCellKernel<PV, U, true><<<G, TG_PR_NT, 0, st>>>(dDesc, int(mode), threshold, dCounts); \
+             else tgPruneCellKernel<PV, U, false><<<G, TG_PR_NT, 0, st>>>(dDesc, int(mode), threshold, dCounts); } while (0)
         if (P0 == 4) {
-            if (wide) TG_PRUNE_LAUNCH(1, 2, g2); else TG_PRUNE_LAUNCH(1, 1, g);
+            if (wide) TG_PRUNE_LAUNCH(1, TG_PR_U, gU); else TG_PRUNE_LAUNCH(1, 1, g1);
         } else if (P0 == 8) {
-            if (wide) TG_PRUNE_LAUNCH(2, 2, g2); else TG_PRUNE_LAUNCH(2, 1, g);
+            if (wide) TG_PRUNE_LAUNCH(2, 2, g2); else TG_PRUNE_LAUNCH(2, 1, g1);
         } else {
-            TG_PRUNE_LAUNCH(0, 1, g);
+            TG_PRUNE_LAUNCH(0, 1, g1);
         }
 #undef TG_PRUNE_LAUNCH
     }
@@ -1126,18 +1127,19 @@ tg_status tg_prune_batch_static(tg_instance* const* instances, int32_t n, tg_pru
     // the array keeps the last call's contents: counters and caps start at zero, the descriptors are overwritten
     TG_CUDA(cudaMemsetAsync(S.scratch, 0, TG_PS_COUNTS + TG_PS_CAP, st));
     TG_CUDA(cudaMemcpyAsync(dDesc, h, sizeof(TgPruneDesc) * size_t(n), cudaMemcpyHostToDevice, st));
-    const dim3 g((maxCells + 255) / 256, n), g2((maxCells + 511) / 512, n);
+    const dim3 g((maxCells + 255) / 256, n), g1((maxCells + TG_PR_NT - 1) / TG_PR_NT, n), g2((maxCells + 2 * TG_PR_NT - 1) / (2 * TG_PR_NT), n),
+               gU((maxCells + TG_PR_U * TG_PR_NT - 1) / (TG_PR_U * TG_PR_NT), n);
     const bool wide = int64_t(g2.x) * n >= 4 * S.numSMs;
     const int P0 = instances[0]->P;
 #define TG_PRUNE_LAUNCH(PV, U, G) \
-    do { if (act) tgPruneCellKernel<PV, U, true><<<G, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts); \
-         else tgPruneCellKernel<PV, U, false><<<G, 256, 0, st>>>(dDesc, int(mode), threshold, dCounts); } while (0)
+    do { if (act) tgPruneCellKernel<PV, U, true><<<G, TG_PR_NT, 0, st>>>(dDesc, int(mode), threshold, dCounts); \
+         else tgPruneCellKernel<PV, U, false><<<G, TG_PR_NT, 0, st>>>(dDesc, int(mode), threshold, dCounts); } while (0)
     if (P0 == 4) {
-        if (wide) TG_PRUNE_LAUNCH(1, 2, g2); else TG_PRUNE_LAUNCH(1, 1, g);
+        if (wide) TG_PRUNE_LAUNCH(1, TG_PR_U, gU); else TG_PRUNE_LAUNCH(1, 1, g1);
     } else if (P0 == 8) {
-        if (wide) TG_PRUNE_LAUNCH(2, 2, g2); else TG_PRUNE_LAUNCH(2, 1, g);
+        if (wide) TG_PRUNE_LAUNCH(2, 2, g2); else TG_PRUNE_LAUNCH(2, 1, g1);
     } else {
-        TG_PRUNE_LAUNCH(0, 1, g);
+        TG_PRUNE_LAUNCH(0, 1, g1);
     }
 #undef TG_PRUNE_LAUNCH
     if (mode == TG_PRUNE_IMBALANCE) {

@@ -713,11 +713,21 @@ struct TgPruneDesc {
 
 // PV > 0: an instance with P = 4 * PV plans is pruned from registers -- the 16-byte loads of the thread's U cells are
 // issued first, the rules run on the register copy and a cell whose column changed is stored back as 16-byte words;
-// any other instance of the batch takes the entry-by-entry path.  grid = (cells / (256 U), instances).
+// any other instance of the batch takes the entry-by-entry path.  grid = (cells / (TG_PR_NT U), instances).
 // ACT = false: no instance of the batch has a footprint table -- the third dominance axis is compiled out (the pass is bound by
 // its comparisons, not by HBM: ncu showed the integer pipe at 72 %).
+// CTAs of TG_PR_NT = 128 threads, TG_PR_U = 4 cells of a P = 4 instance per thread (the 1024-instance batch under ncu: 256 x 2:
+// 101.6-102.9 us, 256 x 4: 94.5, 256 x 6: 92.7, 256 x 8: 106.6, 128 x 3: 93.0, 128 x 4: 90.2, 128 x 6: 88.7, 128 x 8: 93.3, 64 x 6: 88.0,
+// 64 x 8: 99.8): a CTA lives for two dependent memory trips (its descriptor, then its cells) and little else, so what counts
+// is the bytes each resident CTA has in flight and how many CTAs an SM holds.
+#ifndef TG_PR_NT
+#define TG_PR_NT 128
+#endif
+#ifndef TG_PR_U
+#define TG_PR_U 4
+#endif
 template <int PV, int U, bool ACT>
-__global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __restrict__ descs, int mode, int64_t threshold,
+__global__ void __launch_bounds__(TG_PR_NT) tgPruneCellKernel(const TgPruneDesc* __restrict__ descs, int mode, int64_t threshold,
                                                          unsigned long long* counts) {
     constexpr int PVA = PV > 0 ? PV : 1, PP = 4 * PVA;
     const TgPruneDesc D = descs[blockIdx.y];
@@ -727,14 +737,14 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
     const int32_t* const cap = D.cap;
     const int nCells = D.nCells, K = D.K, P = D.P;
     counts += 4 * blockIdx.y;
-    if (int(blockIdx.x) * (256 * U) >= nCells) return;
-    const int cellFirst = blockIdx.x * (256 * U) + threadIdx.x;
+    if (int(blockIdx.x) * (TG_PR_NT * U) >= nCells) return;
+    const int cellFirst = blockIdx.x * (TG_PR_NT * U) + threadIdx.x;
     unsigned c1 = 0, c2 = 0, c4 = 0;
     if (PV > 0 && P == PP) {
         int4 tv[U][PVA], mv[U][PVA], av[U][PVA];
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int cell = cellFirst + 256 * u;
+            const int cell = cellFirst + TG_PR_NT * u;
             if (cell < nCells) {
 #pragma unroll
                 for (int v = 0; v < PVA; ++v) {
@@ -746,7 +756,7 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
         }
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int cell = cellFirst + 256 * u;
+            const int cell = cellFirst + TG_PR_NT * u;
             if (cell < nCells) {
                 int32_t t[PP], mm[PP], am[PP];
 #pragma unroll
@@ -760,19 +770,22 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
 #pragma unroll
                 for (int p = 0; p < PP; ++p)   // R1
                     if (t[p] != TG_INVALID && (ACT ? int64_t(mm[p]) + am[p] > capk : mm[p] > capk)) { t[p] = TG_INVALID; kill |= 1u << p; ++c1; }
-                unsigned dead = 0;
+                // R2, decided on the cell as R1 left it, one pass over the unordered pairs p < q: q kills p iff q <= p on
+                // every axis and they differ (a tie goes to the lower index, p); p kills q iff p <= q, tie included.  (The
+                // ordered form -- le and eq of (q, p) for every q != p -- spent twice the comparisons: the pass is bound by them.)
+                unsigned dead = 0, live = 0;
 #pragma unroll
-                for (int p = 0; p < PP; ++p) {   // R2, decided on the cell as R1 left it
-                    bool dd = false;
+                for (int p = 0; p < PP; ++p) {
+                    if (t[p] != TG_INVALID) live |= 1u << p;
 #pragma unroll
-                    for (int q = 0; q < PP; ++q) {
-                        if (q == p) continue;
-                        const bool le = t[q] <= t[p] && mm[q] <= mm[p] && (!ACT || am[q] <= am[p]);   // t[q] == INVALID is never <= a live t[p]
-                        const bool eq = t[q] == t[p] && mm[q] == mm[p] && (!ACT || am[q] == am[p]);
-                        dd = dd || (le && (!eq || q < p));
+                    for (int q = p + 1; q < PP; ++q) {
+                        const bool leqp = t[q] <= t[p] && mm[q] <= mm[p] && (!ACT || am[q] <= am[p]);   // an INVALID t[q] is never <= a live t[p]
+                        const bool lepq = t[p] <= t[q] && mm[p] <= mm[q] && (!ACT || am[p] <= am[q]);
+                        if (leqp && !lepq) dead |= 1u << p;
+                        if (lepq) dead |= 1u << q;
                     }
-                    if (t[p] != TG_INVALID && dd) dead |= 1u << p;
                 }
+                dead &= live;
 #pragma unroll
                 for (int p = 0; p < PP; ++p)
                     if (dead >> p & 1u) { t[p] = TG_INVALID; ++c2; }
@@ -790,7 +803,7 @@ __global__ void __launch_bounds__(256) tgPruneCellKernel(const TgPruneDesc* __re
         }
     } else {
         for (int u = 0; u < U; ++u) {
-            const int cell = cellFirst + 256 * u;
+            const int cell = cellFirst + TG_PR_NT * u;
             if (cell >= nCells) break;
             int32_t* t = time_us + size_t(cell) * P;
             const int32_t* mm = mem_mb + size_t(cell) * P;
