@@ -237,6 +237,18 @@ def test_loader_paths_in_one_batch(tg):
             same(oracle.solve_depth(inst) if inst.actmem_mb is not None else oracle.solve(inst), g, inst.name)
 
 
+@pytest.mark.parametrize("shape,P", [("config4", 8), ("config5_one", 4)])
+def test_row_group_loader_on_uniform_batches(tg, shape, P):
+    """Cost-table loader, the row-group form (tgLoadRowsKernel: a CTA reduces 8 start rows and writes the diagonal-major
+    tables through a shared-memory tile): taken by a batch of plain instances of one P in {4, 8} that fills the GPU -- what
+    the 1024-instance batch runs with P = 4.  Here 320 instances each of P = 8 and P = 4 with L = 11 ... 16, so the last row
+    group of an instance is partial and instances of different L share one grid."""
+    insts = [getattr(gen, shape)(s + 300, L=11 + s % 6, K=5 + s % 4) for s in range(320)]
+    assert all(x.P == P for x in insts)
+    for inst, g in zip(insts, solve_all(tg, insts)):
+        same(oracle.solve(inst), g, inst.name)
+
+
 def test_statistics_on_the_device_match_the_host_form(tg):
     """tg_solve_stats written to a DEVICE buffer (the call stays asynchronous; bench.py times it that way) against the HOST
     form of the same solve: a few instances run in rounds, so every count is deterministic."""

@@ -160,3 +160,29 @@ def test_device_resident_tables_and_async_out(tg):
         same(oracle.solve(inst), g, inst.name)
     for h in hs:
         h.destroy()
+
+
+@pytest.mark.parametrize("shape,L,K,n,footprint", [("config5_one", 12, 10, 200, False), ("config4", 12, 8, 220, False),
+                                                     ("config5_one", 12, 10, 200, True), ("config4", 12, 8, 220, True)])
+def test_prune_batch_that_fills_the_gpu(tg, shape, L, K, n, footprint):
+    """The launch the 1024-instance batch takes: a batch with at least 4 CTAs per SM (here 200 x 4 and 220 x 3 CTAs of 4 and 2
+    cells a thread on 148 SMs) is pruned from registers, several cells of a thread in flight (P = 4 and P = 8, with and
+    without the footprint axis); the smaller batches above take one cell per thread.  Tables and counts against the oracle."""
+    insts = [getattr(gen, shape)(5000 + s, L=L, K=K) for s in range(n)]
+    if footprint:
+        insts = [gen.with_actmem(x, s) for s, x in enumerate(insts)]
+    assert insts[0].P == (4 if shape == "config5_one" else 8)
+    orc = oracle.prune_depth if footprint else oracle.prune
+    killed = 0
+    for mode, thr in [(0, 0), (1, 3000)]:
+        hs = [tg.instance_from_inputs(i) for i in insts]
+        counts = tg.tg_prune_batch(hs, mode, thr)
+        for inst, h, c in zip(insts, hs, counts):
+            pr, oc = orc(inst, mode, thr)
+            assert c.tolist() == oc.tolist(), (inst.name, mode, thr)
+            t = tg.tg_instance_read_time(h)
+            assert np.array_equal(t, pr.time_us.reshape(t.shape)), (inst.name, mode, thr)
+            killed += int(oc[0] + oc[1])
+        for h in hs:
+            h.destroy()
+    assert killed > 1000
