@@ -48,6 +48,21 @@ def test_length_classes_equal_the_expanded_instance(tg):
         h.destroy()
 
 
+def test_class_instances_in_a_batch_that_fills_the_gpu(tg):
+    """320 class instances of one P: the batch takes the row-group loader, which reads a cell's row through the class map
+    (the mixed batch above takes the cell-order loader)."""
+    bases = [gen.config5_one(s + 40, L=11 + s % 6, K=5 + s % 3) for s in range(320)]
+    hs, exp = [], []
+    for b in bases:
+        class_of, ct, cm, e = gen.length_classes(b)
+        hs.append(create(tg, b, class_of, ct, cm))
+        exp.append(e)
+    for e, g in zip(exp, tg.tg_solve_batch(hs)):
+        same(oracle.solve(e), g, e.name)
+    for h in hs:
+        h.destroy()
+
+
 def test_arbitrary_classes(tg):
     """Classes need not be slice lengths: random class maps with as few as one class and as many as NS."""
     for seed in range(40):
