@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(256, (PV == 1 && U > 1) ? 4 : 1) tgLoadKernel(
                     }
                 }
                 if (best < sMin[k]) atomicMin(&sMin[k], best);
-                // the thread's next cell: TG_LR_NT cells = ds slices and dk islands further on
+                // the thread's next cell: 256 cells = ds slices and dk islands further on
                 int adv = ds;
                 k += dk;
                 if (k >= K) { k -= K; ++adv; }
@@ -714,8 +714,8 @@ struct TgPruneDesc {
 // PV > 0: an instance with P = 4 * PV plans is pruned from registers -- the 16-byte loads of the thread's U cells are
 // issued first, the rules run on the register copy and a cell whose column changed is stored back as 16-byte words;
 // any other instance of the batch takes the entry-by-entry path.  grid = (cells / (TG_PR_NT U), instances).
-// ACT = false: no instance of the batch has a footprint table -- the third dominance axis is compiled out (the pass is bound by
-// its comparisons, not by HBM: ncu showed the integer pipe at 72 %).
+// ACT = false: no instance of the batch has a footprint table -- the third dominance axis is compiled out (ncu showed the integer
+// pipe at 72 % with it).
 // CTAs of TG_PR_NT = 128 threads, TG_PR_U = 4 cells of a P = 4 instance per thread (the 1024-instance batch under ncu: 256 x 2:
 // 101.6-102.9 us, 256 x 4: 94.5, 256 x 6: 92.7, 256 x 8: 106.6, 128 x 3: 93.0, 128 x 4: 90.2, 128 x 6: 88.7, 128 x 8: 93.3, 64 x 6: 88.0,
 // 64 x 8: 99.8): a CTA lives for two dependent memory trips (its descriptor, then its cells) and little else, so what counts
